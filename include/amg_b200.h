@@ -1,0 +1,202 @@
+/* amg_b200 — C ABI of the B200-native AMG-preconditioned Krylov solve with adjoint gradients.
+ *
+ * What it computes (arxiv/paper_2606_09001, "JAX-AMG"; citations are PAPER.md lines):
+ *   - the solve  A x = b  of a sparse PDE system in CSR by a Krylov method with an
+ *     aggregation-AMG preconditioner (§2.1 "jaxamg.solve", default BiCGSTAB + AMG;
+ *     :277 CG), returning iteration count, final residual and convergence status (:125);
+ *   - the adjoint solve  A^T lambda = dL/dx  (:87 Eq. 1) on the SAME cached hierarchy;
+ *   - the gradients  dL/dA = -lambda x^T  restricted to the stored entries and  dL/db = lambda
+ *     (:93 Eq. 2; :186 "gradients with respect to the matrix entries");
+ *   - the cached setup: one handle = one cache entry of the paper's solver cache (:103, :121),
+ *     reused for any number of right-hand sides (:116, :287 reuse_setup).
+ * The paper delegates the numerical algorithm to NVIDIA AmgX and states none of it; the
+ * algorithm implemented here is the reading fixed in SURVEY.md §8(c) and DESIGN.md:
+ * deterministic pairwise aggregation (handshake matching with a 3-bucket + hash key), Galerkin
+ * coarse operators with piecewise-constant prolongation, V(nu1,nu2) cycles with L1-/damped-
+ * Jacobi smoothing from a zero guess on every level, dense LU on the coarsest level, PCG or
+ * right-preconditioned BiCGSTAB with x0 = 0, stop on the recurrence residual
+ * ||r||_2 <= rtol * ||b||_2.
+ *
+ * Everything is fp64 values / int32 indices, single GPU (sm_100a).  No torch types cross this
+ * boundary: plain pointers and sizes.
+ *
+ * POINTERS.  Arguments prefixed d_ are DEVICE pointers, h_ are HOST pointers; `opt`, `info`,
+ * `out` scalars are host pointers.  The caller owns every buffer it passes; the library never
+ * frees or reallocates them and copies what it needs during amg_setup (the CSR arrays may be
+ * released after amg_setup returns).  Library-owned memory (hierarchy, work vectors) comes
+ * from cudaMalloc, or from the allocator hook if one is installed, and is released by
+ * amg_destroy.
+ *
+ * STREAMS.  Every call enqueues its work on `cuda_stream` (a cudaStream_t passed as void*;
+ * NULL = the legacy default stream) and returns after that work has completed (one
+ * synchronisation at the end of a solve; none inside the Krylov loop, whose scalars and
+ * convergence test live on the device).
+ *
+ * ERRORS.  Every function returns amg_status; no exception crosses the ABI.  On a failed
+ * amg_setup *out is NULL and amg_last_error(NULL) holds a message (thread-local).
+ * Non-convergence is NOT an error: it is reported in amg_info.status.
+ *
+ * NUMBERING.  Internally every level is stored in an aggregate-contiguous order (DESIGN.md
+ * §layout); vectors are permuted at this boundary.  All arrays crossing the ABI — b, x, g,
+ * lambda, gA, aggregates, level CSR — are in the caller's (natural) numbering.
+ *
+ * THREADS.  Distinct handles may be used concurrently from distinct host threads on distinct
+ * streams; one handle runs one call at a time.
+ */
+#ifndef AMG_B200_H
+#define AMG_B200_H
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define AMG_API __attribute__((visibility("default")))
+#else
+#define AMG_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct amg_handle_s* amg_handle;
+
+typedef enum {
+  AMG_OK = 0,
+  AMG_ERR_INVALID_ARG = 1,
+  AMG_ERR_BAD_CSR = 2,          /* rowptr not monotone / col out of range or unsorted / no positive diagonal */
+  AMG_ERR_CUDA = 3,
+  AMG_ERR_OOM = 4,
+  AMG_ERR_COARSE_SINGULAR = 5,  /* dense LU of the coarsest operator found a zero pivot */
+  AMG_ERR_COARSEN_STALL = 6,    /* coarsening stalled above 4096 rows */
+  AMG_ERR_UNSUPPORTED = 7
+} amg_status;
+
+typedef enum { AMG_CONVERGED = 0, AMG_MAXIT = 1, AMG_BREAKDOWN = 2, AMG_NONFINITE = 3 } amg_conv;
+
+/* Filled by amg_options_default(); struct_size guards ABI growth. */
+typedef struct {
+  int32_t struct_size;
+  int32_t krylov;           /* 0 = PCG, 1 = right-preconditioned BiCGSTAB (paper default)   */
+  int32_t symmetric;        /* 1 = caller asserts A == A^T (no transposition for the adjoint, :95, :114);
+                               0 = not symmetric (amg_solve_transpose -> AMG_ERR_UNSUPPORTED for now);
+                              -1 = check on the device at setup (bitwise a_ij == a_ji)                   */
+  int32_t pre_sweeps;       /* nu1, default 2                                                            */
+  int32_t post_sweeps;      /* nu2, default 2                                                            */
+  int32_t smoother;         /* 0 = L1-Jacobi (d_i = sum_j |a_ij|), 1 = damped Jacobi (omega / a_ii)      */
+  int32_t coarse_max_rows;  /* stop coarsening at n_l <= this (default 64); dense LU there               */
+  int32_t max_levels;       /* default 32                                                                */
+  int32_t max_match_rounds; /* 0 = handshake rounds until the fix-point                                  */
+  int32_t force_generic;    /* 1 = use the row-vector fallback kernels on every level (tests)            */
+  int32_t use_graph;        /* 1 = replay one Krylov iteration as a CUDA graph (default), 0 = plain launches */
+  int32_t reserved0;
+  double omega;             /* damped Jacobi weight, default 2/3                                         */
+  double strong_beta;       /* strength threshold beta, default 0.25                                     */
+  double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */
+  uint64_t hash_seed;       /* tie-break salt of the matching; level l uses hash_seed + l                */
+} amg_options;
+
+typedef struct {
+  int32_t iterations;   /* passes of the Krylov loop                                                     */
+  int32_t status;       /* amg_conv                                                                      */
+  double rel_residual;  /* recurrence ||r||_2 / ||b||_2 at exit                                          */
+  double b_norm;        /* ||b||_2                                                                       */
+} amg_info;
+
+/* Timings of the last amg_setup, for the report ("timed separately", BASELINE.json). */
+typedef struct {
+  double total_ms;      /* host wall clock of amg_setup                                                  */
+  double aggregate_ms;  /* U1-U3 over all levels                                                         */
+  double galerkin_ms;   /* U4 over all levels                                                            */
+  double reorder_ms;    /* aggregate-contiguous renumbering of the hierarchy                             */
+  double lu_ms;         /* U6                                                                            */
+  int32_t match_rounds_max;
+  int32_t reserved;
+} amg_setup_stats;
+
+AMG_API amg_status amg_options_default(amg_options* opt);
+
+/* Optional: route library-owned device memory through the caller's allocator (e.g. torch's
+ * caching allocator).  Process-wide; call before amg_setup.  Pass NULLs to restore cudaMalloc. */
+AMG_API amg_status amg_set_allocator(void* (*alloc_fn)(size_t bytes, void* cuda_stream, void* user),
+                             void (*free_fn)(void* ptr, void* user), void* user);
+
+/* U1-U7: validate the CSR (ascending unique columns, positive diagonal in every row), build
+ * and cache the hierarchy.  d_rowptr int32[n+1], d_col int32[nnz], d_val double[nnz]. */
+AMG_API amg_status amg_setup(amg_handle* out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
+                     const int32_t* d_col, const double* d_val, const amg_options* opt,
+                     void* cuda_stream);
+
+/* Test hook: same, but levels 0..nagg-1 use the given aggregate arrays (h_d_aggs is a HOST
+ * array of nagg DEVICE pointers; aggs[l] has rows(l) int32 ids in [0, nc_l), every id used)
+ * instead of the built-in matching; coarsening stops after nagg levels. */
+AMG_API amg_status amg_setup_with_aggregates(amg_handle* out, int64_t n, int64_t nnz,
+                                     const int32_t* d_rowptr, const int32_t* d_col,
+                                     const double* d_val, const amg_options* opt, int32_t nagg,
+                                     const int32_t* const* h_d_aggs, void* cuda_stream);
+
+AMG_API amg_status amg_destroy(amg_handle h);
+
+/* S1-S9: solve A x = b from x0 = 0 with the Krylov method of the options; x is output only.
+ * ||b|| = 0 gives x = 0, 0 iterations, converged.  info may be NULL. */
+AMG_API amg_status amg_solve(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit,
+                     amg_info* info, void* cuda_stream);
+/* Same with an explicit Krylov method (0 PCG, 1 BiCGSTAB) and preconditioner switch
+ * (1 = AMG V-cycle, 0 = identity: plain CG / BiCGSTAB as in PAPER.md:277). */
+AMG_API amg_status amg_solve_ex(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit,
+                        int32_t krylov, int32_t precond, amg_info* info, void* cuda_stream);
+/* G1: A^T lambda = g on the same hierarchy (Eq. 1).  symmetric = 1: the transposition is
+ * skipped and this is amg_solve on A. */
+AMG_API amg_status amg_solve_transpose(amg_handle h, const double* d_g, double* d_lambda, double rtol,
+                               int32_t maxit, amg_info* info, void* cuda_stream);
+/* S10: nrhs independent solves on one hierarchy; column s of B / X starts at s * ld.
+ * transpose = 1 solves the adjoint systems.  infos: host array of nrhs entries or NULL. */
+AMG_API amg_status amg_solve_batched(amg_handle h, int32_t transpose, const double* d_B, double* d_X,
+                             int32_t nrhs, int64_t ld, double rtol, int32_t maxit, amg_info* infos,
+                             void* cuda_stream);
+/* End-to-end variant with HOST buffers: copies b to the device, solves, copies x back. */
+AMG_API amg_status amg_solve_host(amg_handle h, const double* h_b, double* h_x, double rtol,
+                          int32_t maxit, amg_info* info, void* cuda_stream);
+
+/* G2: gA[k] (+)= - sum_{s < nrhs} lambda_s[i] * x_s[col[k]]  for rowptr[i] <= k < rowptr[i+1]
+ * on the pattern given to amg_setup (Eq. 2; each stored entry is its own parameter).
+ * Column s of Lambda / X starts at s * ld.  accumulate = 0 overwrites gA.
+ * G3: dL/db = lambda is the caller's lambda itself (no call). */
+AMG_API amg_status amg_grad_values(amg_handle h, const double* d_lambda, const double* d_x, int32_t nrhs,
+                           int64_t ld, double* d_gA, int32_t accumulate, void* cuda_stream);
+
+/* z = B r: one V-cycle from a zero guess (the preconditioner; also the V-cycle timing hook). */
+AMG_API amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, double* d_z,
+                                    void* cuda_stream);
+
+/* ---- introspection / parity hooks (natural numbering) ---- */
+AMG_API amg_status amg_get_num_levels(amg_handle h, int32_t* num_levels);
+AMG_API amg_status amg_get_level_info(amg_handle h, int32_t level, int64_t* rows, int64_t* nnz);
+AMG_API amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out);
+AMG_API amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int32_t* d_col,
+                             double* d_val, void* cuda_stream);
+AMG_API amg_status amg_get_setup_stats(amg_handle h, amg_setup_stats* stats);
+/* 1 if `level` runs the row-block streaming kernels, 0 if the row-vector fallback. */
+AMG_API amg_status amg_get_level_path(amg_handle h, int32_t level, int32_t* fast_path);
+/* Algorithmic bytes of: which = 0 one level-0 SpMV, 1 one V-cycle,
+ * 2 one PCG iteration (SpMV + vector ops + V-cycle), 3 one BiCGSTAB iteration,
+ * 4 one level-0 smoother sweep. */
+AMG_API amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes);
+
+/* Per-kernel hooks on one level, vectors in that level's natural numbering:
+ *   op 0: y = A_l x                               (d_in0 = x,           d_out rows(l))
+ *   op 1: xout = x + dinv o (b - A_l x)           (d_in0 = x, d_in1 = b, d_out rows(l))
+ *   op 2: rc = R (b - A_l x)                      (d_in0 = x, d_in1 = b, d_out rows(l+1))
+ *   op 3: xout = x + gamma * P e_c                (d_in0 = x, d_in1 = e_c rows(l+1), d_out rows(l))
+ *   op 4: two fused sweeps from zero: x2 of b     (d_in1 = b,           d_out rows(l))
+ *   op 5: V-cycle started at level l              (d_in1 = b,           d_out rows(l))
+ * `reps` > 1 repeats the kernel back to back (timing); results are those of one application. */
+AMG_API amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0,
+                        const double* d_in1, double* d_out, int32_t reps, void* cuda_stream);
+
+/* Message of the last error on this handle; NULL handle: last failed setup on this thread. */
+AMG_API const char* amg_last_error(amg_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

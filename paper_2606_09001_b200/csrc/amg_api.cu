@@ -1,0 +1,335 @@
+// extern "C" entry points of amg_b200 (include/amg_b200.h): argument checks, handle lifetime,
+// allocator hook.  All numerical work is in amg_setup.cu / amg_solve.cu.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+
+#include "amg_internal.cuh"
+
+namespace {
+
+thread_local std::string g_thread_error;
+
+void* (*g_alloc_fn)(size_t, void*, void*) = nullptr;
+void (*g_free_fn)(void*, void*) = nullptr;
+void* g_alloc_user = nullptr;
+
+}  // namespace
+
+void amg_set_thread_error(const std::string& s) { g_thread_error = s; }
+
+void* amg_dev_alloc(amg_handle_s* H, size_t bytes, cudaStream_t st) {
+  if (bytes == 0) bytes = 16;
+  void* p = nullptr;
+  if (g_alloc_fn) {
+    p = g_alloc_fn(bytes, (void*)st, g_alloc_user);
+  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    p = nullptr;
+  }
+  if (p) H->allocs.push_back(p);
+  return p;
+}
+
+static void raw_free(void* p) {
+  if (g_free_fn)
+    g_free_fn(p, g_alloc_user);
+  else
+    cudaFree(p);
+}
+
+void amg_dev_free(amg_handle_s* H, void* p) {
+  if (!p) return;
+  auto it = std::find(H->allocs.rbegin(), H->allocs.rend(), p);
+  if (it == H->allocs.rend()) return;  // not ours (e.g. the caller's val array)
+  H->allocs.erase(std::next(it).base());
+  raw_free(p);
+}
+
+void amg_free_all(amg_handle_s* H) {
+  for (void* p : H->allocs) raw_free(p);
+  H->allocs.clear();
+}
+
+namespace {
+
+amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t* d_rowptr, const int32_t* d_col,
+                         const double* d_val, const amg_options* opt, int32_t nagg, const int32_t* const* h_d_aggs,
+                         void* cuda_stream) {
+  if (!out) return AMG_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (n <= 0 || nnz <= 0 || !d_rowptr || !d_col || !d_val) {
+    amg_set_thread_error("amg_setup: null pointer or empty matrix");
+    return AMG_ERR_INVALID_ARG;
+  }
+  if (n >= (int64_t)1 << 31 || nnz >= (int64_t)1 << 31) {
+    amg_set_thread_error("amg_setup: n and nnz must be below 2^31 (int32 indices)");
+    return AMG_ERR_UNSUPPORTED;
+  }
+  amg_options o;
+  amg_options_default(&o);
+  if (opt) {
+    if (opt->struct_size <= 0 || opt->struct_size > (int32_t)sizeof(amg_options)) {
+      amg_set_thread_error("amg_setup: bad amg_options.struct_size");
+      return AMG_ERR_INVALID_ARG;
+    }
+    memcpy(&o, opt, (size_t)opt->struct_size);
+    o.struct_size = (int32_t)sizeof(amg_options);
+  }
+  if (o.pre_sweeps < 0 || o.post_sweeps < 0 || o.max_levels < 1 || o.coarse_max_rows < 1 ||
+      (o.smoother != 0 && o.smoother != 1) || (o.krylov != 0 && o.krylov != 1) || !(o.strong_beta >= 0.0) ||
+      o.symmetric < -1 || o.symmetric > 1 || nagg < 0) {
+    amg_set_thread_error("amg_setup: option out of range");
+    return AMG_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  amg_handle_s* H = new amg_handle_s;
+  H->opt = o;
+  H->n = n;
+  H->nnz = nnz;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    amg_set_thread_error(std::string("amg_setup: no CUDA device: ") + cudaGetErrorString(cudaGetLastError()));
+    delete H;
+    return AMG_ERR_CUDA;
+  }
+  H->sm_count = prop.multiProcessorCount;
+  H->l2_bytes = (size_t)prop.l2CacheSize;
+
+  auto fail = [&](amg_status s) {
+    amg_set_thread_error(H->err.empty() ? "amg_setup failed" : H->err);
+    cudaStreamSynchronize(st);
+    amg_destroy_graphs(H);
+    for (auto& e : H->ev)
+      if (e) cudaEventDestroy(e);
+    if (H->h_ctl) cudaFreeHost(H->h_ctl);
+    amg_free_all(H);
+    delete H;
+    cudaGetLastError();
+    return s;
+  };
+
+  amg_status s = amg_build_hierarchy(H, d_rowptr, d_col, d_val, nagg, h_d_aggs, st);
+  if (s != AMG_OK) return fail(s);
+
+  // Krylov workspace
+  auto setup_ws = [&]() -> amg_status {
+    const int n0 = H->lv[0].n;
+    for (int i = 0; i < 9; ++i) AMG_ALLOC(H, H->kv[i], double, n0, st);
+    AMG_ALLOC(H, H->io_tmp, double, n0, st);
+    AMG_ALLOC(H, H->io_tmp2, double, n0, st);
+    AMG_ALLOC(H, H->io_tmp3, double, n0, st);
+    AMG_ALLOC(H, H->ctl, KrylovCtl, 1, st);
+    int cap = H->sm_count * 8;
+    for (const Level& L : H->lv) cap = std::max(cap, L.nblk);
+    cap = std::max(cap, 4096);
+    H->partials_cap = cap;
+    AMG_ALLOC(H, H->partials, double, 2 * (size_t)cap, st);
+    AMG_ALLOC(H, H->counter, unsigned, 1, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(H->counter, 0, sizeof(unsigned), st));
+    AMG_CUDA_TRY(H, cudaMemsetAsync(H->ctl, 0, sizeof(KrylovCtl), st));
+    AMG_CUDA_TRY(H, cudaMallocHost((void**)&H->h_ctl, sizeof(KrylovCtl) * 8));
+    for (auto& e : H->ev) AMG_CUDA_TRY(H, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    return AMG_OK;
+  };
+  s = setup_ws();
+  if (s != AMG_OK) return fail(s);
+  *out = H;
+  return AMG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+amg_status amg_options_default(amg_options* o) {
+  if (!o) return AMG_ERR_INVALID_ARG;
+  memset(o, 0, sizeof(*o));
+  o->struct_size = (int32_t)sizeof(amg_options);
+  o->krylov = 0;
+  o->symmetric = 1;
+  o->pre_sweeps = 2;
+  o->post_sweeps = 2;
+  o->smoother = 0;
+  o->coarse_max_rows = 64;
+  o->max_levels = 32;
+  o->max_match_rounds = 0;
+  o->force_generic = 0;
+  o->use_graph = 1;
+  o->omega = 2.0 / 3.0;
+  o->strong_beta = 0.25;
+  o->coarse_scale = 1.0;
+  o->hash_seed = 0;
+  return AMG_OK;
+}
+
+amg_status amg_set_allocator(void* (*alloc_fn)(size_t, void*, void*), void (*free_fn)(void*, void*), void* user) {
+  if ((alloc_fn == nullptr) != (free_fn == nullptr)) return AMG_ERR_INVALID_ARG;
+  g_alloc_fn = alloc_fn;
+  g_free_fn = free_fn;
+  g_alloc_user = user;
+  return AMG_OK;
+}
+
+amg_status amg_setup(amg_handle* out, int64_t n, int64_t nnz, const int32_t* d_rowptr, const int32_t* d_col,
+                     const double* d_val, const amg_options* opt, void* cuda_stream) {
+  return create_handle(out, n, nnz, d_rowptr, d_col, d_val, opt, 0, nullptr, cuda_stream);
+}
+
+amg_status amg_setup_with_aggregates(amg_handle* out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
+                                     const int32_t* d_col, const double* d_val, const amg_options* opt,
+                                     int32_t nagg, const int32_t* const* h_d_aggs, void* cuda_stream) {
+  static const int32_t* const none[1] = {nullptr};
+  if (nagg < 0 || (nagg > 0 && !h_d_aggs)) {
+    if (out) *out = nullptr;
+    amg_set_thread_error("amg_setup_with_aggregates: bad aggregate list");
+    return AMG_ERR_INVALID_ARG;
+  }
+  return create_handle(out, n, nnz, d_rowptr, d_col, d_val, opt, nagg, nagg > 0 ? h_d_aggs : none, cuda_stream);
+}
+
+amg_status amg_destroy(amg_handle h) {
+  if (!h) return AMG_OK;
+  cudaDeviceSynchronize();
+  amg_destroy_graphs(h);
+  for (auto& e : h->ev)
+    if (e) cudaEventDestroy(e);
+  if (h->h_ctl) cudaFreeHost(h->h_ctl);
+  amg_free_all(h);
+  delete h;
+  return AMG_OK;
+}
+
+amg_status amg_solve_ex(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit, int32_t krylov,
+                        int32_t precond, amg_info* info, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!d_b || !d_x || maxit < 0 || !(rtol >= 0.0) || (krylov != 0 && krylov != 1)) {
+    h->err = "amg_solve: bad argument";
+    return AMG_ERR_INVALID_ARG;
+  }
+  return amg_krylov_solve(h, d_b, d_x, rtol, maxit, krylov, precond ? 1 : 0, info, (cudaStream_t)cuda_stream);
+}
+
+amg_status amg_solve(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit, amg_info* info,
+                     void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  return amg_solve_ex(h, d_b, d_x, rtol, maxit, h->opt.krylov, 1, info, cuda_stream);
+}
+
+amg_status amg_solve_transpose(amg_handle h, const double* d_g, double* d_lambda, double rtol, int32_t maxit,
+                               amg_info* info, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!h->symmetric) {
+    h->err = "amg_solve_transpose: nonsymmetric matrices are not supported yet";
+    return AMG_ERR_UNSUPPORTED;
+  }
+  // symmetric: the transposition is skipped, A lambda = g is solved on the same hierarchy
+  return amg_solve(h, d_g, d_lambda, rtol, maxit, info, cuda_stream);
+}
+
+amg_status amg_solve_batched(amg_handle h, int32_t transpose, const double* d_B, double* d_X, int32_t nrhs,
+                             int64_t ld, double rtol, int32_t maxit, amg_info* infos, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (nrhs < 0 || ld < h->n || !d_B || !d_X) {
+    h->err = "amg_solve_batched: bad argument";
+    return AMG_ERR_INVALID_ARG;
+  }
+  for (int32_t s = 0; s < nrhs; ++s) {
+    amg_info* inf = infos ? infos + s : nullptr;
+    amg_status st = transpose ? amg_solve_transpose(h, d_B + (size_t)s * ld, d_X + (size_t)s * ld, rtol, maxit, inf,
+                                                    cuda_stream)
+                              : amg_solve(h, d_B + (size_t)s * ld, d_X + (size_t)s * ld, rtol, maxit, inf,
+                                          cuda_stream);
+    if (st != AMG_OK) return st;
+  }
+  return AMG_OK;
+}
+
+amg_status amg_solve_host(amg_handle h, const double* h_b, double* h_x, double rtol, int32_t maxit, amg_info* info,
+                          void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!h_b || !h_x) {
+    h->err = "amg_solve_host: null pointer";
+    return AMG_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t bytes = sizeof(double) * (size_t)h->n;
+  AMG_CUDA_TRY(h, cudaMemcpyAsync(h->io_tmp, h_b, bytes, cudaMemcpyHostToDevice, st));
+  AMG_TRY(amg_solve(h, h->io_tmp, h->io_tmp2, rtol, maxit, info, cuda_stream));
+  AMG_CUDA_TRY(h, cudaMemcpyAsync(h_x, h->io_tmp2, bytes, cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(h, cudaStreamSynchronize(st));
+  return AMG_OK;
+}
+
+amg_status amg_grad_values(amg_handle h, const double* d_lambda, const double* d_x, int32_t nrhs, int64_t ld,
+                           double* d_gA, int32_t accumulate, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!d_lambda || !d_x || !d_gA || nrhs < 0 || (nrhs > 1 && ld < h->n)) {
+    h->err = "amg_grad_values: bad argument";
+    return AMG_ERR_INVALID_ARG;
+  }
+  return amg_grad_values_impl(h, d_lambda, d_x, nrhs, ld, d_gA, accumulate, (cudaStream_t)cuda_stream);
+}
+
+amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, double* d_z, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!d_r || !d_z) return AMG_ERR_INVALID_ARG;
+  return amg_level_op_impl(h, 0, 5, nullptr, d_r, d_z, 1, (cudaStream_t)cuda_stream);
+}
+
+amg_status amg_get_num_levels(amg_handle h, int32_t* num_levels) {
+  if (!h || !num_levels) return AMG_ERR_INVALID_ARG;
+  *num_levels = (int32_t)h->lv.size();
+  return AMG_OK;
+}
+
+amg_status amg_get_level_info(amg_handle h, int32_t level, int64_t* rows, int64_t* nnz) {
+  if (!h || level < 0 || level >= (int32_t)h->lv.size()) return AMG_ERR_INVALID_ARG;
+  if (rows) *rows = h->lv[level].n;
+  if (nnz) *nnz = h->lv[level].nnz;
+  return AMG_OK;
+}
+
+amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out) {
+  if (!h || level < 0 || level >= (int32_t)h->lv.size() - 1 || !d_agg_out) return AMG_ERR_INVALID_ARG;
+  AMG_CUDA_TRY(h, cudaMemcpy(d_agg_out, h->lv[level].nat_agg, sizeof(int) * (size_t)h->lv[level].n,
+                             cudaMemcpyDeviceToDevice));
+  return AMG_OK;
+}
+
+amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int32_t* d_col, double* d_val,
+                             void* cuda_stream) {
+  if (!h || level < 0 || level >= (int32_t)h->lv.size() || !d_rowptr || !d_col || !d_val)
+    return AMG_ERR_INVALID_ARG;
+  return amg_natural_level_csr(h, level, d_rowptr, d_col, d_val, (cudaStream_t)cuda_stream);
+}
+
+amg_status amg_get_setup_stats(amg_handle h, amg_setup_stats* stats) {
+  if (!h || !stats) return AMG_ERR_INVALID_ARG;
+  *stats = h->stats;
+  return AMG_OK;
+}
+
+amg_status amg_get_level_path(amg_handle h, int32_t level, int32_t* fast_path) {
+  if (!h || level < 0 || level >= (int32_t)h->lv.size() || !fast_path) return AMG_ERR_INVALID_ARG;
+  *fast_path = h->lv[level].fast;
+  return AMG_OK;
+}
+
+amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes) {
+  if (!h || !bytes || which < 0 || which > 4) return AMG_ERR_INVALID_ARG;
+  *bytes = amg_algorithmic_bytes(h, which);
+  return AMG_OK;
+}
+
+amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0, const double* d_in1,
+                        double* d_out, int32_t reps, void* cuda_stream) {
+  if (!h || level < 0 || level >= (int32_t)h->lv.size() || !d_out) return AMG_ERR_INVALID_ARG;
+  return amg_level_op_impl(h, level, op, d_in0, d_in1, d_out, reps, (cudaStream_t)cuda_stream);
+}
+
+const char* amg_last_error(amg_handle h) { return h ? h->err.c_str() : g_thread_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,163 @@
+// Internal definitions of the amg_b200 library (sm_100a).  Not part of the C ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "amg_b200.h"
+
+// ------------------------------------------------------------------------------------------
+// tuning constants of the row-block streaming kernels
+// ------------------------------------------------------------------------------------------
+constexpr int RB_THREADS = 256;   // threads per CTA
+constexpr int RB_TARGET = 3072;   // target nonzeros per row block
+constexpr int RB_CAP = 4096;      // products staged in shared memory per row block (incl. alignment slop)
+constexpr int RB_MAXROWS = 1024;  // rows per row block (shared rowptr / residual staging)
+constexpr int RED_THREADS = 256;  // BLAS-1 kernels
+constexpr int MAX_DENSE = 4096;   // largest coarsest level accepted
+
+// ------------------------------------------------------------------------------------------
+// device-resident Krylov scalars and loop control (S7-S9: no host round trip inside the loop)
+// ------------------------------------------------------------------------------------------
+struct KrylovCtl {
+  double rho, rho_new, sigma, alpha, beta, omega;
+  double rr, ss, ts, tt, rv;
+  double bnorm2, rtol;
+  int iter, status, done, maxit;
+  int first, halfstep, pad0, pad1;
+};
+
+enum FinalizeId {
+  FIN_NONE = 0,
+  FIN_INIT_PCG,    // sum0 = ||b||^2
+  FIN_INIT_BICG,   // sum0 = ||b||^2
+  FIN_RZ,          // sum0 = r.z          -> beta, rho
+  FIN_PQ,          // sum0 = p.q          -> alpha (or breakdown)
+  FIN_RR,          // sum0 = ||r||^2      -> iter++, convergence
+  FIN_RV,          // sum0 = rhat.v       -> alpha (or breakdown)
+  FIN_SS,          // sum0 = ||s||^2      -> iter++, half-step convergence
+  FIN_TS_TT,       // sum0 = t.s, sum1 = t.t -> omega
+  FIN_RR_RHO,      // sum0 = ||r||^2, sum1 = rhat.r -> convergence, beta, rho
+};
+
+// ------------------------------------------------------------------------------------------
+// one level of the hierarchy, stored in aggregate-contiguous ("permuted") numbering
+// ------------------------------------------------------------------------------------------
+struct Level {
+  int n = 0;        // rows
+  int nc = 0;       // rows of the next level (0 on the coarsest)
+  int nnz = 0;
+  int nnz_alloc = 0;  // padded to a multiple of 4 (+4) for 128-bit loads
+  // operator A_l
+  int* rowptr = nullptr;
+  int* col = nullptr;
+  double* val = nullptr;
+  double* dinv = nullptr;   // smoother diagonal (null on the coarsest)
+  int* agg = nullptr;       // [n]  coarse id of every row, non-decreasing
+  int* agg_ptr = nullptr;   // [nc+1] first row of every aggregate
+  // row-block partition (boundaries aligned to aggregate starts)
+  int* blk_ptr = nullptr;   // [nblk+1]
+  int nblk = 0;
+  int fast = 0;             // 1: row-block streaming kernels; 0: row-vector fallback
+  int lpr = 8;              // lanes per row of the fallback kernels
+  int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
+  // natural numbering (the caller's / oracle's): hooks and the ABI boundary
+  int* nat_agg = nullptr;   // [n] aggregate ids in natural numbering of levels l, l+1
+  int* pos = nullptr;       // [n] natural index -> permuted position
+  int* inv = nullptr;       // [n] permuted position -> natural index
+  // work vectors (permuted numbering)
+  double* b = nullptr;      // right-hand side of this level (levels > 0)
+  double* x = nullptr;      // iterate / ping
+  double* x2 = nullptr;     // pong
+  double* rtmp = nullptr;   // fine residual (fallback path only)
+  int match_rounds = 0;
+};
+
+struct amg_handle_s {
+  amg_options opt;
+  int64_t n = 0, nnz = 0;
+  std::vector<Level> lv;
+  // natural level-0 pattern for amg_grad_values
+  int* nat_rowptr = nullptr;
+  int* nat_col = nullptr;
+  // coarsest dense LU
+  int nL = 0;
+  double* lu = nullptr;
+  int* piv = nullptr;
+  // Krylov work vectors (level-0 size, permuted numbering)
+  double* kv[10] = {nullptr};
+  double* io_tmp = nullptr;  // staging for amg_solve_host / hooks
+  double* io_tmp2 = nullptr;
+  double* io_tmp3 = nullptr;
+  KrylovCtl* ctl = nullptr;       // device
+  KrylovCtl* h_ctl = nullptr;     // pinned host mirror
+  double* partials = nullptr;     // [2 * partials_cap]
+  int partials_cap = 0;
+  unsigned* counter = nullptr;
+  // CUDA graph of one Krylov iteration (keyed by krylov/precond)
+  cudaGraphExec_t graph_exec[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaStream_t cap_stream = nullptr;  // graphs are captured here (the legacy stream cannot capture)
+  int sm_count = 148;
+  size_t l2_bytes = 0;
+  int symmetric = 1;
+  amg_setup_stats stats{};
+  std::vector<void*> allocs;
+  std::string err;
+};
+
+// ------------------------------------------------------------------------------------------
+// host helpers
+// ------------------------------------------------------------------------------------------
+void amg_set_thread_error(const std::string& s);
+void* amg_dev_alloc(amg_handle_s* H, size_t bytes, cudaStream_t st);  // tracked; nullptr on failure
+void amg_dev_free(amg_handle_s* H, void* p);                           // early release of a tracked block
+void amg_free_all(amg_handle_s* H);
+
+#define AMG_CUDA_TRY(H, expr)                                                              \
+  do {                                                                                     \
+    cudaError_t _e = (expr);                                                               \
+    if (_e != cudaSuccess) {                                                               \
+      (H)->err = std::string(#expr) + ": " + cudaGetErrorString(_e);                        \
+      return AMG_ERR_CUDA;                                                                 \
+    }                                                                                      \
+  } while (0)
+
+#define AMG_TRY(expr)                    \
+  do {                                   \
+    amg_status _s = (expr);              \
+    if (_s != AMG_OK) return _s;         \
+  } while (0)
+
+#define AMG_ALLOC(H, ptr, type, count, st)                                         \
+  do {                                                                             \
+    (ptr) = (type*)amg_dev_alloc((H), sizeof(type) * (size_t)(count), (st));        \
+    if (!(ptr)) {                                                                  \
+      (H)->err = "device allocation failed: " #ptr;                                \
+      return AMG_ERR_OOM;                                                          \
+    }                                                                              \
+  } while (0)
+
+static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// setup.cu
+amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const int32_t* d_col,
+                               const double* d_val, int32_t nagg, const int32_t* const* h_d_aggs,
+                               cudaStream_t st);
+amg_status amg_natural_level_csr(amg_handle_s* H, int level, int32_t* d_rowptr, int32_t* d_col,
+                                 double* d_val, cudaStream_t st);
+amg_status amg_exclusive_scan(amg_handle_s* H, const int* d_in, int* d_out, int n, cudaStream_t st);
+
+// solve.cu
+amg_status amg_vcycle(amg_handle_s* H, int level, const double* b, double** x_out, KrylovCtl* ctl,
+                      bool fuse_rz, cudaStream_t st);
+amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, double rtol, int maxit,
+                            int krylov, int precond, amg_info* info, cudaStream_t st);
+amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d_in0,
+                             const double* d_in1, double* d_out, int reps, cudaStream_t st);
+amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const double* d_x, int nrhs,
+                                int64_t ld, double* d_gA, int accumulate, cudaStream_t st);
+double amg_algorithmic_bytes(amg_handle_s* H, int which);
+void amg_destroy_graphs(amg_handle_s* H);

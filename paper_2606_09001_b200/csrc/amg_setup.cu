@@ -1,0 +1,986 @@
+// Setup phase on the device: strength / row maxima, handshake matching,
+// singleton merge + numbering, Galerkin product, smoother diagonal, dense LU of the coarsest
+// operator, and the aggregate-contiguous renumbering of the whole hierarchy.
+//
+// The matching is the deterministic definition of DESIGN.md §readings (O-2): the result is a
+// pure function of the matrix and the salt, independent of the thread schedule, so a sequential
+// program following the same definition produces the same integers.
+#include <chrono>
+#include <cstdio>
+
+#include "amg_internal.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+
+inline double now_ms() {
+  using namespace std::chrono;
+  return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
+}
+
+// ------------------------------------------------------------------------------------------
+// exclusive scan of int32 (n inputs -> n+1 outputs, out[n] = total)
+// ------------------------------------------------------------------------------------------
+constexpr int SCAN_T = 512;
+constexpr int SCAN_ITEMS = 4;
+constexpr int SCAN_BLOCK = SCAN_T * SCAN_ITEMS;
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_block(const int* __restrict__ in, int* __restrict__ out,
+                                                       int n, int* __restrict__ bsum) {
+  __shared__ int wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int64_t base = (int64_t)blockIdx.x * SCAN_BLOCK + tid * SCAN_ITEMS;
+  int v[SCAN_ITEMS];
+  int tsum = 0;
+#pragma unroll
+  for (int j = 0; j < SCAN_ITEMS; ++j) {
+    int64_t idx = base + j;
+    v[j] = idx < n ? in[idx] : 0;
+    tsum += v[j];
+  }
+  int inc = tsum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) wsum[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int s = lane < SCAN_T / 32 ? wsum[lane] : 0;
+    int inc2 = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, inc2, o);
+      if (lane >= o) inc2 += t;
+    }
+    wsum[lane] = inc2 - s;
+  }
+  __syncthreads();
+  int excl = wsum[w] + inc - tsum;
+#pragma unroll
+  for (int j = 0; j < SCAN_ITEMS; ++j) {
+    int64_t idx = base + j;
+    if (idx <= n) out[idx] = excl;
+    excl += v[j];
+  }
+  if (tid == SCAN_T - 1 && bsum) bsum[blockIdx.x] = excl;
+}
+
+__global__ void k_scan_add(int* __restrict__ out, int n1, const int* __restrict__ boff) {
+  int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n1) out[idx] += boff[idx / SCAN_BLOCK];
+}
+
+}  // namespace
+
+amg_status amg_exclusive_scan(amg_handle_s* H, const int* d_in, int* d_out, int n, cudaStream_t st) {
+  const int n1 = n + 1;
+  const int nb = div_up(n1, SCAN_BLOCK);
+  if (nb == 1) {
+    k_scan_block<<<1, SCAN_T, 0, st>>>(d_in, d_out, n, nullptr);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    return AMG_OK;
+  }
+  int* bsum;
+  AMG_ALLOC(H, bsum, int, nb + 1, st);
+  k_scan_block<<<nb, SCAN_T, 0, st>>>(d_in, d_out, n, bsum);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, bsum, bsum, nb, st));  // in place: every block reads before it writes
+  k_scan_add<<<div_up(n1, TPB), TPB, 0, st>>>(d_out, n1, bsum);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, bsum);
+  return AMG_OK;
+}
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// validation
+// ------------------------------------------------------------------------------------------
+__global__ void k_validate_csr(int n, int nnz, const int* __restrict__ rowptr, const int* __restrict__ col,
+                               const double* __restrict__ val, int* __restrict__ bad) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int s = rowptr[i], e = rowptr[i + 1];
+  if (s < 0 || e < s || e > nnz) {
+    *bad = 1;
+    return;
+  }
+  bool diag = false;
+  int prev = -1;
+  for (int k = s; k < e; ++k) {
+    int c = col[k];
+    if (c < 0 || c >= n || c <= prev) {
+      *bad = 1;
+      return;
+    }
+    prev = c;
+    if (c == i) diag = val[k] > 0.0;
+  }
+  if (!diag) *bad = 1;
+}
+
+// bitwise symmetry check: a_ij == a_ji for every stored entry (options.symmetric = -1)
+__global__ void k_check_symmetric(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                                  const double* __restrict__ val, int* __restrict__ nonsym) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+    int j = col[k];
+    int lo = rowptr[j], hi = rowptr[j + 1] - 1;
+    bool found = false;
+    while (lo <= hi) {
+      int mid = (lo + hi) >> 1;
+      int c = col[mid];
+      if (c == i) {
+        found = (val[mid] == val[k]);
+        break;
+      }
+      if (c < i)
+        lo = mid + 1;
+      else
+        hi = mid - 1;
+    }
+    if (!found) {
+      *nonsym = 1;
+      return;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// U1-U3: strength, handshake matching, singleton merge, numbering
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {
+  z ^= z >> 30;
+  z *= 0xBF58476D1CE4E5B9ULL;
+  z ^= z >> 27;
+  z *= 0x94D049BB133111EBULL;
+  z ^= z >> 31;
+  return z;
+}
+
+struct EdgeKey {  // (-q, h, -lo, -hi): larger is better
+  int q;
+  uint64_t h;
+  int lo, hi;
+};
+
+__device__ __forceinline__ bool key_better(const EdgeKey& a, const EdgeKey& b) {
+  if (a.q != b.q) return a.q < b.q;
+  if (a.h != b.h) return a.h > b.h;
+  if (a.lo != b.lo) return a.lo < b.lo;
+  return a.hi < b.hi;
+}
+
+// candidate test and key of the entry (i, j, a_ij); m = row maxima of w = -a
+__device__ __forceinline__ bool edge_candidate(int i, int j, double aij, const double* __restrict__ m,
+                                               double mi, double beta, uint64_t salt, EdgeKey& key) {
+  if (j == i) return false;
+  double w = -aij;
+  if (!(w > 0.0)) return false;
+  double mj = m[j];
+  if (!(w >= beta * fmin(mi, mj))) return false;
+  double M = fmax(mi, mj);
+  key.q = (2.0 * w > M) ? 0 : ((4.0 * w > M) ? 1 : 2);
+  int lo = min(i, j), hi = max(i, j);
+  key.h = mix64((uint64_t)lo * 0x9E3779B97F4A7C15ULL + (uint64_t)hi * 0xBF58476D1CE4E5B9ULL + salt);
+  key.lo = lo;
+  key.hi = hi;
+  return true;
+}
+
+__global__ void k_row_max(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                          const double* __restrict__ val, double* __restrict__ m) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double mi = 0.0;
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k)
+    if (col[k] != i) mi = fmax(mi, fmax(-val[k], 0.0));
+  m[i] = mi;
+}
+
+// every unmatched vertex points to its best unmatched candidate neighbour (state = match[])
+__global__ void k_propose(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                          const double* __restrict__ val, const double* __restrict__ m, double beta,
+                          uint64_t salt, const int* __restrict__ match, int* __restrict__ ptr) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int best_j = -1;
+  if (match[i] < 0) {
+    EdgeKey best{};
+    double mi = m[i];
+    for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+      int j = col[k];
+      EdgeKey key;
+      if (!edge_candidate(i, j, val[k], m, mi, beta, salt, key)) continue;
+      if (match[j] >= 0) continue;
+      if (best_j < 0 || key_better(key, best)) {
+        best = key;
+        best_j = j;
+      }
+    }
+  }
+  ptr[i] = best_j;
+}
+
+__global__ void k_handshake(int n, const int* __restrict__ ptr, int* __restrict__ match,
+                            int* __restrict__ added) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int j = ptr[i];
+  if (j >= 0 && ptr[j] == i) {
+    match[i] = j;
+    if (i < j) atomicAdd(added, 1);
+  }
+}
+
+// root of every vertex after the singleton merge (one simultaneous step) + root flags
+__global__ void k_roots(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                        const double* __restrict__ val, const double* __restrict__ m, double beta,
+                        uint64_t salt, const int* __restrict__ match, int* __restrict__ root,
+                        int* __restrict__ isroot) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int mi_ = match[i];
+  int r;
+  if (mi_ >= 0) {
+    r = min(i, mi_);
+  } else {
+    r = i;
+    int best_j = -1;
+    EdgeKey best{};
+    double mi = m[i];
+    for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+      int j = col[k];
+      EdgeKey key;
+      if (!edge_candidate(i, j, val[k], m, mi, beta, salt, key)) continue;
+      if (match[j] < 0) continue;  // only matched neighbours
+      if (best_j < 0 || key_better(key, best)) {
+        best = key;
+        best_j = j;
+      }
+    }
+    if (best_j >= 0) r = min(best_j, match[best_j]);
+  }
+  root[i] = r;
+  isroot[i] = (r == i) ? 1 : 0;
+}
+
+__global__ void k_assign_agg(int n, const int* __restrict__ root, const int* __restrict__ id,
+                             int* __restrict__ agg) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) agg[i] = id[root[i]];
+}
+
+__global__ void k_fill_int(int n, int* __restrict__ a, int v) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) a[i] = v;
+}
+
+__global__ void k_iota(int n, int* __restrict__ a) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) a[i] = i;
+}
+
+__global__ void k_max_int(int n, const int* __restrict__ a, int* __restrict__ out, int* __restrict__ neg) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int v = a[i];
+  if (v < 0) *neg = 1;
+  atomicMax(out, v);
+}
+
+// member lists of the aggregates, ascending fine index inside each aggregate
+__global__ void k_count_members(int n, const int* __restrict__ agg, int* __restrict__ cnt,
+                                int* __restrict__ slot) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) slot[i] = atomicAdd(&cnt[agg[i]], 1);
+}
+__global__ void k_fill_members(int n, const int* __restrict__ agg, const int* __restrict__ mptr,
+                               const int* __restrict__ slot, int* __restrict__ mem) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) mem[mptr[agg[i]] + slot[i]] = i;
+}
+__global__ void k_sort_members(int nc, const int* __restrict__ mptr, int* __restrict__ mem) {
+  int I = blockIdx.x * blockDim.x + threadIdx.x;
+  if (I >= nc) return;
+  int s = mptr[I], e = mptr[I + 1];
+  for (int a = s + 1; a < e; ++a) {
+    int v = mem[a];
+    int b = a - 1;
+    while (b >= s && mem[b] > v) {
+      mem[b + 1] = mem[b];
+      --b;
+    }
+    mem[b + 1] = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// U4: Galerkin product with piecewise-constant P:  A_c[I,J] = sum_{i in I} sum_{j in J} a_ij
+// one thread per coarse row keeps a sorted list of (J, sum) in a scratch segment; the sum of
+// every (I,J) runs over ascending fine row, then ascending position (fixed order).
+// ------------------------------------------------------------------------------------------
+__global__ void k_rap_len(int nc, const int* __restrict__ mptr, const int* __restrict__ mem,
+                          const int* __restrict__ rowptr, int* __restrict__ len) {
+  int I = blockIdx.x * blockDim.x + threadIdx.x;
+  if (I >= nc) return;
+  int s = 0;
+  for (int t = mptr[I]; t < mptr[I + 1]; ++t) {
+    int i = mem[t];
+    s += rowptr[i + 1] - rowptr[i];
+  }
+  len[I] = s;
+}
+
+__global__ void k_rap_rows(int nc, const int* __restrict__ mptr, const int* __restrict__ mem,
+                           const int* __restrict__ rowptr, const int* __restrict__ col,
+                           const double* __restrict__ val, const int* __restrict__ agg,
+                           const int* __restrict__ segptr, int* __restrict__ skey,
+                           double* __restrict__ sval, int* __restrict__ cnt) {
+  int I = blockIdx.x * blockDim.x + threadIdx.x;
+  if (I >= nc) return;
+  int* key = skey + segptr[I];
+  double* acc = sval + segptr[I];
+  int m = 0;  // entries in the sorted list
+  for (int t = mptr[I]; t < mptr[I + 1]; ++t) {
+    int i = mem[t];
+    for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+      int J = agg[col[k]];
+      double a = val[k];
+      int p = m;  // find the slot from the back (columns arrive almost sorted)
+      while (p > 0 && key[p - 1] > J) --p;
+      if (p > 0 && key[p - 1] == J) {
+        acc[p - 1] += a;
+      } else {
+        for (int q = m; q > p; --q) {
+          key[q] = key[q - 1];
+          acc[q] = acc[q - 1];
+        }
+        key[p] = J;
+        acc[p] = a;
+        ++m;
+      }
+    }
+  }
+  cnt[I] = m;
+}
+
+__global__ void k_rap_compact(int nc, const int* __restrict__ segptr, const int* __restrict__ skey,
+                              const double* __restrict__ sval, const int* __restrict__ crowptr,
+                              int* __restrict__ ccol, double* __restrict__ cval) {
+  int I = blockIdx.x * blockDim.x + threadIdx.x;
+  if (I >= nc) return;
+  int s = segptr[I], d = crowptr[I], m = crowptr[I + 1] - d;
+  for (int t = 0; t < m; ++t) {
+    ccol[d + t] = skey[s + t];
+    cval[d + t] = sval[s + t];
+  }
+}
+
+// U5: smoother diagonal
+__global__ void k_dinv(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                       const double* __restrict__ val, int smoother, double omega, double* __restrict__ dinv) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double l1 = 0.0, aii = 0.0;
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+    l1 += fabs(val[k]);
+    if (col[k] == i) aii = val[k];
+  }
+  dinv[i] = smoother == 0 ? 1.0 / l1 : omega / aii;
+}
+
+// ------------------------------------------------------------------------------------------
+// U6: dense LU with partial pivoting of the coarsest operator (one CTA)
+// ------------------------------------------------------------------------------------------
+__global__ void k_csr_to_dense(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                               const double* __restrict__ val, double* __restrict__ a) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) a[(size_t)i * n + col[k]] = val[k];
+}
+
+__global__ void __launch_bounds__(1024) k_dense_lu(int n, double* __restrict__ a, int* __restrict__ piv,
+                                                   int* __restrict__ info) {
+  __shared__ double s_val[32];
+  __shared__ int s_idx[32];
+  __shared__ double s_amax;
+  __shared__ int s_p;
+  const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, w = tid >> 5;
+  // amax = max |a_ij|
+  double mx = 0.0;
+  for (size_t t = tid; t < (size_t)n * n; t += T) mx = fmax(mx, fabs(a[t]));
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if (lane == 0) s_val[w] = mx;
+  __syncthreads();
+  if (tid == 0) {
+    double v = 0.0;
+    for (int q = 0; q < (T + 31) / 32; ++q) v = fmax(v, s_val[q]);
+    s_amax = v;
+  }
+  __syncthreads();
+  const double amax = s_amax;
+  for (int k = 0; k < n; ++k) {
+    // pivot: first row i >= k with the largest |a_ik|
+    double bv = -1.0;
+    int bi = n;
+    for (int i = k + tid; i < n; i += T) {
+      double v = fabs(a[(size_t)i * n + k]);
+      if (v > bv) {
+        bv = v;
+        bi = i;
+      }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+      int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ov > bv || (ov == bv && oi < bi)) {
+        bv = ov;
+        bi = oi;
+      }
+    }
+    if (lane == 0) {
+      s_val[w] = bv;
+      s_idx[w] = bi;
+    }
+    __syncthreads();
+    if (tid == 0) {
+      double v = -1.0;
+      int p = n;
+      for (int q = 0; q < (T + 31) / 32; ++q)
+        if (s_val[q] > v || (s_val[q] == v && s_idx[q] < p)) {
+          v = s_val[q];
+          p = s_idx[q];
+        }
+      if (!(v > 1e-300 * amax) || !(amax > 0.0)) {
+        *info = 1;
+        p = k;
+      }
+      piv[k] = p;
+      s_p = p;
+    }
+    __syncthreads();
+    const int p = s_p;
+    if (p != k)
+      for (int j = tid; j < n; j += T) {
+        double t = a[(size_t)k * n + j];
+        a[(size_t)k * n + j] = a[(size_t)p * n + j];
+        a[(size_t)p * n + j] = t;
+      }
+    __syncthreads();
+    const double akk = a[(size_t)k * n + k];
+    for (int i = k + 1 + tid; i < n; i += T) a[(size_t)i * n + k] = a[(size_t)i * n + k] / akk;
+    __syncthreads();
+    const int mrem = n - k - 1;
+    for (int64_t t = tid; t < (int64_t)mrem * mrem; t += T) {
+      int i = k + 1 + (int)(t / mrem), j = k + 1 + (int)(t % mrem);
+      a[(size_t)i * n + j] -= a[(size_t)i * n + k] * a[(size_t)k * n + j];
+    }
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// aggregate-contiguous renumbering
+// ------------------------------------------------------------------------------------------
+__global__ void k_perm_sizes(int nc, const int* __restrict__ mptr, const int* __restrict__ pos_next,
+                             int* __restrict__ sizep) {
+  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a < nc) sizep[pos_next[a]] = mptr[a + 1] - mptr[a];
+}
+
+__global__ void k_perm_pos(int nc, const int* __restrict__ mptr, const int* __restrict__ mem,
+                           const int* __restrict__ pos_next, const int* __restrict__ startp,
+                           int* __restrict__ pos, int* __restrict__ inv, int* __restrict__ aggp) {
+  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= nc) return;
+  int ap = pos_next[a];
+  int base = startp[ap];
+  for (int t = mptr[a]; t < mptr[a + 1]; ++t) {
+    int i = mem[t];
+    int p = base + (t - mptr[a]);
+    pos[i] = p;
+    inv[p] = i;
+    aggp[p] = ap;
+  }
+}
+
+__global__ void k_perm_rowlen(int n, const int* __restrict__ rowptr, const int* __restrict__ src_row,
+                              int* __restrict__ len) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  int i = src_row[p];
+  len[p] = rowptr[i + 1] - rowptr[i];
+}
+
+// row p of the output is row src_row[p] of the input with columns relabelled by col_map and
+// re-sorted ascending
+__global__ void k_perm_fill(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                            const double* __restrict__ val, const int* __restrict__ src_row,
+                            const int* __restrict__ col_map, const int* __restrict__ rowptr_out,
+                            int* __restrict__ col_out, double* __restrict__ val_out) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  int i = src_row[p];
+  int s = rowptr[i], e = rowptr[i + 1], d = rowptr_out[p];
+  int m = 0;
+  for (int k = s; k < e; ++k) {
+    int c = col_map[col[k]];
+    double v = val[k];
+    int q = m;
+    while (q > 0 && col_out[d + q - 1] > c) {
+      col_out[d + q] = col_out[d + q - 1];
+      val_out[d + q] = val_out[d + q - 1];
+      --q;
+    }
+    col_out[d + q] = c;
+    val_out[d + q] = v;
+    ++m;
+  }
+}
+
+__global__ void k_gather_double(int n, const double* __restrict__ src, const int* __restrict__ idx,
+                                double* __restrict__ dst) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < n) dst[p] = src[idx[p]];
+}
+
+// row-block partition: block k starts at the first unit (aggregate, or row if unit_ptr == null)
+// whose first nonzero is at or beyond k * target
+__global__ void k_blk_partition(int nblk, int target, int nunits, const int* __restrict__ unit_ptr,
+                                const int* __restrict__ rowptr, int n, int* __restrict__ blk_ptr) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k > nblk) return;
+  if (k == nblk) {
+    blk_ptr[k] = n;
+    return;
+  }
+  int64_t want = (int64_t)k * target;
+  int lo = 0, hi = nunits;  // smallest u in [0, nunits] with rowptr[start(u)] >= want
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    int r = unit_ptr ? unit_ptr[mid] : mid;
+    if (rowptr[r] >= want)
+      hi = mid;
+    else
+      lo = mid + 1;
+  }
+  blk_ptr[k] = lo == nunits ? n : (unit_ptr ? unit_ptr[lo] : lo);
+}
+
+__global__ void k_blk_stats(int nblk, const int* __restrict__ blk_ptr, const int* __restrict__ rowptr,
+                            int* __restrict__ stats) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nblk) return;
+  int r0 = blk_ptr[k], r1 = blk_ptr[k + 1];
+  int k0 = rowptr[r0], k1 = rowptr[r1];
+  atomicMax(&stats[0], r1 - r0);
+  atomicMax(&stats[1], k1 - (k0 & ~3));
+}
+
+__global__ void k_pad_tail(int nnz, int nnz_alloc, int* __restrict__ col, double* __restrict__ val) {
+  int k = nnz + blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < nnz_alloc) {
+    col[k] = 0;
+    val[k] = 0.0;
+  }
+}
+
+// natural-numbering CSR of one level while the hierarchy is being built
+struct NatCsr {
+  int n = 0, nnz = 0;
+  int* rowptr = nullptr;
+  int* col = nullptr;
+  double* val = nullptr;
+  int* agg = nullptr;   // natural aggregates (kept in Level::nat_agg)
+  int* mptr = nullptr;  // member lists
+  int* mem = nullptr;
+  double* dinv = nullptr;
+  int nc = 0;
+};
+
+inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
+
+amg_status read_int(amg_handle_s* H, const int* d, int* h, cudaStream_t st) {
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(h, d, sizeof(int), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  return AMG_OK;
+}
+
+// U1-U3 on one level: fills N.agg / N.nc
+amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* rounds_out, cudaStream_t st) {
+  const int n = N.n;
+  const amg_options& o = H->opt;
+  double* m;
+  int *match, *ptr, *root, *isroot, *id, *added;
+  AMG_ALLOC(H, m, double, n, st);
+  AMG_ALLOC(H, match, int, n, st);
+  AMG_ALLOC(H, ptr, int, n, st);
+  AMG_ALLOC(H, root, int, n, st);
+  AMG_ALLOC(H, isroot, int, n, st);
+  AMG_ALLOC(H, id, int, n + 1, st);
+  AMG_ALLOC(H, added, int, 1, st);
+  const int g = grid_for(n);
+  k_row_max<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m);
+  k_fill_int<<<g, TPB, 0, st>>>(n, match, -1);
+  int rounds = 0;
+  for (;;) {
+    if (o.max_match_rounds > 0 && rounds >= o.max_match_rounds) break;
+    AMG_CUDA_TRY(H, cudaMemsetAsync(added, 0, sizeof(int), st));
+    k_propose<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m, o.strong_beta, salt, match, ptr);
+    k_handshake<<<g, TPB, 0, st>>>(n, ptr, match, added);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    int h_added = 0;
+    AMG_TRY(read_int(H, added, &h_added, st));
+    ++rounds;
+    if (h_added == 0) break;
+  }
+  *rounds_out = rounds;
+  k_roots<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m, o.strong_beta, salt, match, root, isroot);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, isroot, id, n, st));
+  AMG_TRY(read_int(H, id + n, &N.nc, st));
+  AMG_ALLOC(H, N.agg, int, n, st);
+  k_assign_agg<<<g, TPB, 0, st>>>(n, root, id, N.agg);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, m);
+  amg_dev_free(H, match);
+  amg_dev_free(H, ptr);
+  amg_dev_free(H, root);
+  amg_dev_free(H, isroot);
+  amg_dev_free(H, id);
+  amg_dev_free(H, added);
+  return AMG_OK;
+}
+
+amg_status build_members(amg_handle_s* H, NatCsr& N, cudaStream_t st) {
+  const int n = N.n, nc = N.nc;
+  int *cnt, *slot;
+  AMG_ALLOC(H, cnt, int, nc + 1, st);
+  AMG_ALLOC(H, slot, int, n, st);
+  AMG_ALLOC(H, N.mptr, int, nc + 1, st);
+  AMG_ALLOC(H, N.mem, int, n, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(cnt, 0, sizeof(int) * (nc + 1), st));
+  k_count_members<<<grid_for(n), TPB, 0, st>>>(n, N.agg, cnt, slot);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, cnt, N.mptr, nc, st));
+  k_fill_members<<<grid_for(n), TPB, 0, st>>>(n, N.agg, N.mptr, slot, N.mem);
+  k_sort_members<<<grid_for(nc), TPB, 0, st>>>(nc, N.mptr, N.mem);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, cnt);
+  amg_dev_free(H, slot);
+  return AMG_OK;
+}
+
+// U4: C = Galerkin(N)
+amg_status galerkin_level(amg_handle_s* H, const NatCsr& N, NatCsr& C, cudaStream_t st) {
+  const int nc = N.nc;
+  int *len, *segptr, *skey, *cnt;
+  double* sval;
+  AMG_ALLOC(H, len, int, nc, st);
+  AMG_ALLOC(H, segptr, int, nc + 1, st);
+  AMG_ALLOC(H, cnt, int, nc, st);
+  AMG_ALLOC(H, skey, int, N.nnz, st);
+  AMG_ALLOC(H, sval, double, N.nnz, st);
+  k_rap_len<<<grid_for(nc), TPB, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, len);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, len, segptr, nc, st));
+  k_rap_rows<<<div_up(nc, 128), 128, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, N.col, N.val, N.agg, segptr, skey,
+                                          sval, cnt);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  C.n = nc;
+  AMG_ALLOC(H, C.rowptr, int, nc + 1, st);
+  AMG_TRY(amg_exclusive_scan(H, cnt, C.rowptr, nc, st));
+  AMG_TRY(read_int(H, C.rowptr + nc, &C.nnz, st));
+  AMG_ALLOC(H, C.col, int, C.nnz, st);
+  AMG_ALLOC(H, C.val, double, C.nnz, st);
+  k_rap_compact<<<grid_for(nc), TPB, 0, st>>>(nc, segptr, skey, sval, C.rowptr, C.col, C.val);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, len);
+  amg_dev_free(H, segptr);
+  amg_dev_free(H, cnt);
+  amg_dev_free(H, skey);
+  amg_dev_free(H, sval);
+  return AMG_OK;
+}
+
+// permuted copy of a natural CSR: output row p = input row src_row[p], columns mapped by col_map
+amg_status permute_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
+                       const int* src_row, const int* col_map, int* rowptr_out, int* col_out,
+                       double* val_out, cudaStream_t st) {
+  int* len;
+  AMG_ALLOC(H, len, int, n, st);
+  k_perm_rowlen<<<grid_for(n), TPB, 0, st>>>(n, rowptr, src_row, len);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, len, rowptr_out, n, st));
+  k_perm_fill<<<div_up(n, 128), 128, 0, st>>>(n, rowptr, col, val, src_row, col_map, rowptr_out, col_out,
+                                          val_out);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, len);
+  (void)nnz;
+  return AMG_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// U7: the whole setup
+// ------------------------------------------------------------------------------------------
+amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const int32_t* d_col,
+                               const double* d_val, int32_t nagg, const int32_t* const* h_d_aggs,
+                               cudaStream_t st) {
+  const double t_start = now_ms();
+  const amg_options& o = H->opt;
+  const int n0 = (int)H->n, nnz0 = (int)H->nnz;
+  const bool imported = h_d_aggs != nullptr;
+
+  // ---- validation ----
+  {
+    int h_ends[2] = {-1, -1};
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(&h_ends[0], d_rowptr, sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(&h_ends[1], d_rowptr + n0, sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    if (h_ends[0] != 0 || h_ends[1] != nnz0) {
+      H->err = "bad CSR: rowptr[0] != 0 or rowptr[n] != nnz";
+      return AMG_ERR_BAD_CSR;
+    }
+    int* bad;
+    AMG_ALLOC(H, bad, int, 2, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(bad, 0, 2 * sizeof(int), st));
+    k_validate_csr<<<grid_for(n0), TPB, 0, st>>>(n0, nnz0, d_rowptr, d_col, d_val, bad);
+    if (o.symmetric < 0) k_check_symmetric<<<grid_for(n0), TPB, 0, st>>>(n0, d_rowptr, d_col, d_val, bad + 1);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    int h_bad[2] = {0, 0};
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_bad, bad, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, bad);
+    if (h_bad[0]) {
+      H->err = "bad CSR: rows must have ascending unique in-range columns and a positive diagonal";
+      return AMG_ERR_BAD_CSR;
+    }
+    H->symmetric = o.symmetric < 0 ? (h_bad[1] ? 0 : 1) : o.symmetric;
+  }
+
+  // ---- natural-numbering hierarchy ----
+  std::vector<NatCsr> nat(1);
+  nat[0].n = n0;
+  nat[0].nnz = nnz0;
+  AMG_ALLOC(H, H->nat_rowptr, int, n0 + 1, st);
+  AMG_ALLOC(H, H->nat_col, int, nnz0, st);
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(H->nat_rowptr, d_rowptr, sizeof(int) * (n0 + 1), cudaMemcpyDeviceToDevice, st));
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(H->nat_col, d_col, sizeof(int) * (size_t)nnz0, cudaMemcpyDeviceToDevice, st));
+  nat[0].rowptr = H->nat_rowptr;
+  nat[0].col = H->nat_col;
+  nat[0].val = const_cast<double*>(d_val);  // read only during setup
+
+  double t_agg = 0.0, t_rap = 0.0;
+  int rounds_max = 0;
+  std::vector<int> rounds_per_level;
+  int l = 0;
+  for (;;) {
+    NatCsr& cur = nat[l];
+    if (imported) {
+      if (l >= nagg) break;
+      // import: copy ids, nc = max + 1
+      AMG_ALLOC(H, cur.agg, int, cur.n, st);
+      AMG_CUDA_TRY(H, cudaMemcpyAsync(cur.agg, h_d_aggs[l], sizeof(int) * cur.n, cudaMemcpyDeviceToDevice, st));
+      int* mx;
+      AMG_ALLOC(H, mx, int, 2, st);
+      AMG_CUDA_TRY(H, cudaMemsetAsync(mx, 0, 2 * sizeof(int), st));
+      k_max_int<<<grid_for(cur.n), TPB, 0, st>>>(cur.n, cur.agg, mx, mx + 1);
+      int h_mx[2];
+      AMG_CUDA_TRY(H, cudaMemcpyAsync(h_mx, mx, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+      amg_dev_free(H, mx);
+      if (h_mx[1]) {
+        H->err = "imported aggregates contain a negative id";
+        return AMG_ERR_INVALID_ARG;
+      }
+      cur.nc = h_mx[0] + 1;
+      rounds_per_level.push_back(0);
+    } else {
+      if (cur.n <= o.coarse_max_rows || l == o.max_levels - 1) break;
+      double t0 = now_ms();
+      int rounds = 0;
+      AMG_TRY(aggregate_level(H, cur, o.hash_seed + (uint64_t)l, &rounds, st));
+      t_agg += now_ms() - t0;
+      if ((double)cur.nc > 0.8 * (double)cur.n) {  // stall: this level is the coarsest
+        amg_dev_free(H, cur.agg);
+        cur.agg = nullptr;
+        cur.nc = 0;
+        break;
+      }
+      rounds_max = rounds > rounds_max ? rounds : rounds_max;
+      rounds_per_level.push_back(rounds);
+    }
+    double t0 = now_ms();
+    AMG_TRY(build_members(H, cur, st));
+    {  // every id must be used (imported aggregates): no empty aggregate
+      // checked implicitly by the Galerkin product: an empty aggregate gives an empty coarse row,
+      // which fails the diagonal check below
+    }
+    AMG_ALLOC(H, cur.dinv, double, cur.n, st);
+    k_dinv<<<grid_for(cur.n), TPB, 0, st>>>(cur.n, cur.rowptr, cur.col, cur.val, o.smoother, o.omega, cur.dinv);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    nat.emplace_back();
+    AMG_TRY(galerkin_level(H, nat[l], nat[l + 1], st));
+    t_rap += now_ms() - t0;
+    ++l;
+  }
+  const int Lc = l;  // index of the coarsest level
+  if (nat[Lc].n > MAX_DENSE) {
+    H->err = "coarsening stalled above 4096 rows";
+    return AMG_ERR_COARSEN_STALL;
+  }
+  if (imported) {  // imported aggregates with an unused id give a coarse row without diagonal
+    int* bad;
+    AMG_ALLOC(H, bad, int, 1, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(bad, 0, sizeof(int), st));
+    for (int q = 1; q <= Lc; ++q)
+      k_validate_csr<<<grid_for(nat[q].n), TPB, 0, st>>>(nat[q].n, nat[q].nnz, nat[q].rowptr, nat[q].col,
+                                                        nat[q].val, bad);
+    int h_bad = 0;
+    AMG_TRY(read_int(H, bad, &h_bad, st));
+    amg_dev_free(H, bad);
+    if (h_bad) {
+      H->err = "imported aggregates: every id in [0, nc) must be used and coarse diagonals must be positive";
+      return AMG_ERR_INVALID_ARG;
+    }
+  }
+
+  // ---- aggregate-contiguous renumbering, bottom-up ----
+  const double t_reorder0 = now_ms();
+  H->lv.assign(Lc + 1, Level());
+  for (int q = 0; q <= Lc; ++q) {
+    Level& L = H->lv[q];
+    L.n = nat[q].n;
+    L.nnz = nat[q].nnz;
+    L.nc = q < Lc ? nat[q].nc : 0;
+    L.nat_agg = nat[q].agg;
+    L.match_rounds = q < (int)rounds_per_level.size() ? rounds_per_level[q] : 0;
+    AMG_ALLOC(H, L.pos, int, L.n, st);
+    AMG_ALLOC(H, L.inv, int, L.n, st);
+  }
+  {
+    Level& L = H->lv[Lc];
+    k_iota<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.pos);
+    k_iota<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.inv);
+  }
+  for (int q = Lc - 1; q >= 0; --q) {
+    Level& L = H->lv[q];
+    const NatCsr& N = nat[q];
+    int* sizep;
+    AMG_ALLOC(H, sizep, int, L.nc, st);
+    AMG_ALLOC(H, L.agg_ptr, int, L.nc + 1, st);
+    AMG_ALLOC(H, L.agg, int, L.n, st);
+    k_perm_sizes<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, N.mptr, H->lv[q + 1].pos, sizep);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_TRY(amg_exclusive_scan(H, sizep, L.agg_ptr, L.nc, st));
+    k_perm_pos<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, N.mptr, N.mem, H->lv[q + 1].pos, L.agg_ptr, L.pos, L.inv,
+                                              L.agg);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, sizep);
+  }
+  for (int q = 0; q <= Lc; ++q) {
+    Level& L = H->lv[q];
+    const NatCsr& N = nat[q];
+    L.nnz_alloc = ((L.nnz + 3) & ~3) + 4;
+    AMG_ALLOC(H, L.rowptr, int, L.n + 1, st);
+    AMG_ALLOC(H, L.col, int, L.nnz_alloc, st);
+    AMG_ALLOC(H, L.val, double, L.nnz_alloc, st);
+    AMG_TRY(permute_csr(H, L.n, L.nnz, N.rowptr, N.col, N.val, L.inv, L.pos, L.rowptr, L.col, L.val, st));
+    k_pad_tail<<<1, 32, 0, st>>>(L.nnz, L.nnz_alloc, L.col, L.val);
+    if (q < Lc) {
+      AMG_ALLOC(H, L.dinv, double, L.n, st);
+      k_gather_double<<<grid_for(L.n), TPB, 0, st>>>(L.n, N.dinv, L.inv, L.dinv);
+    }
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    // row-block partition
+    L.nblk = L.nnz > 0 ? div_up(L.nnz, RB_TARGET) : 1;
+    AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
+    k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, RB_TARGET, q < Lc ? L.nc : L.n,
+                                                         q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
+    int* stats;
+    AMG_ALLOC(H, stats, int, 2, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(stats, 0, 2 * sizeof(int), st));
+    k_blk_stats<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, stats);
+    int h_stats[2];
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_stats, stats, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, stats);
+    L.fast = (!o.force_generic && h_stats[0] <= RB_MAXROWS && h_stats[1] + 4 <= RB_CAP) ? 1 : 0;
+    double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
+    L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));
+    size_t mat_bytes = (size_t)L.nnz * 12 + (size_t)L.n * 4;
+    L.stream_hint = (H->l2_bytes > 0 && mat_bytes > H->l2_bytes / 2) ? 1 : 0;
+    // work vectors
+    AMG_ALLOC(H, L.x, double, L.n, st);
+    AMG_ALLOC(H, L.x2, double, L.n, st);
+    if (q > 0) AMG_ALLOC(H, L.b, double, L.n, st);
+    if (!L.fast && q < Lc) AMG_ALLOC(H, L.rtmp, double, L.n, st);
+  }
+  H->stats.reorder_ms = now_ms() - t_reorder0;
+
+  // ---- coarsest dense LU ----
+  const double t_lu0 = now_ms();
+  {
+    Level& L = H->lv[Lc];
+    H->nL = L.n;
+    AMG_ALLOC(H, H->lu, double, (size_t)L.n * L.n, st);
+    AMG_ALLOC(H, H->piv, int, L.n, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(H->lu, 0, sizeof(double) * (size_t)L.n * L.n, st));
+    k_csr_to_dense<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, H->lu);
+    int* info;
+    AMG_ALLOC(H, info, int, 1, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, sizeof(int), st));
+    int T = L.n <= 64 ? 256 : 1024;
+    k_dense_lu<<<1, T, 0, st>>>(L.n, H->lu, H->piv, info);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    int h_info = 0;
+    AMG_TRY(read_int(H, info, &h_info, st));
+    amg_dev_free(H, info);
+    if (h_info) {
+      H->err = "coarsest operator is singular";
+      return AMG_ERR_COARSE_SINGULAR;
+    }
+  }
+  H->stats.lu_ms = now_ms() - t_lu0;
+
+  // ---- release the natural-numbering scratch ----
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  for (int q = 0; q <= Lc; ++q) {
+    NatCsr& N = nat[q];
+    if (q > 0) {
+      amg_dev_free(H, N.rowptr);
+      amg_dev_free(H, N.col);
+      amg_dev_free(H, N.val);
+    }
+    amg_dev_free(H, N.mptr);
+    amg_dev_free(H, N.mem);
+    amg_dev_free(H, N.dinv);
+  }
+
+  H->stats.aggregate_ms = t_agg;
+  H->stats.galerkin_ms = t_rap;
+  H->stats.match_rounds_max = rounds_max;
+  H->stats.total_ms = now_ms() - t_start;
+  return AMG_OK;
+}
+
+// natural-numbering CSR of a level, rebuilt from the permuted storage (parity hook)
+amg_status amg_natural_level_csr(amg_handle_s* H, int level, int32_t* d_rowptr, int32_t* d_col,
+                                 double* d_val, cudaStream_t st) {
+  Level& L = H->lv[level];
+  // natural row i = permuted row pos[i]; permuted column c -> natural inv[c]
+  return permute_csr(H, L.n, L.nnz, L.rowptr, L.col, L.val, L.pos, L.inv, d_rowptr, d_col, d_val, st);
+}

@@ -1,0 +1,486 @@
+// Solve-phase host drivers: kernel dispatch, V-cycle (S6), PCG / BiCGSTAB (S7-S9) with the
+// iteration replayed as a CUDA graph and the convergence test on the device, per-level hooks,
+// gradient (G2), algorithmic byte counts.
+#include <cstdio>
+#include <cstring>
+
+#include "amg_kernels.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
+
+inline int red_grid(const amg_handle_s* H, int n) {
+  int g = div_up(n, RED_THREADS * 4);
+  int cap = H->sm_count * 8;
+  if (g > cap) g = cap;
+  if (g > H->partials_cap) g = H->partials_cap;
+  return g < 1 ? 1 : g;
+}
+
+// ---- dispatch of the row kernels ---------------------------------------------------------
+template <int OP, int NDOT>
+void launch_row(const Level& L, const RowArgs& a, cudaStream_t st) {
+  if (L.fast) {
+    if (L.stream_hint)
+      k_rowblock<OP, NDOT, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+    else
+      k_rowblock<OP, NDOT, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+  } else {
+    const int64_t threads = (int64_t)L.n * L.lpr;
+    int g = div_up(threads, RB_THREADS);
+    if (NDOT > 0 && g > 4096) g = 4096;  // bounded partials; the kernel strides over rows
+    if (g < 1) g = 1;
+    switch (L.lpr) {
+      case 4: k_rowvec<OP, NDOT, 4><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 8: k_rowvec<OP, NDOT, 8><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 16: k_rowvec<OP, NDOT, 16><<<g, RB_THREADS, 0, st>>>(a); break;
+      default: k_rowvec<OP, NDOT, 32><<<g, RB_THREADS, 0, st>>>(a); break;
+    }
+  }
+}
+
+RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
+  RowArgs a;
+  memset(&a, 0, sizeof(a));
+  a.n = L.n;
+  a.rowptr = L.rowptr;
+  a.col = L.col;
+  a.val = L.val;
+  a.blk_ptr = L.blk_ptr;
+  a.dinv = L.dinv;
+  a.agg = L.agg;
+  a.agg_ptr = L.agg_ptr;
+  a.gamma = H->opt.coarse_scale;
+  a.partials = H->partials;
+  a.counter = H->counter;
+  a.ctl = ctl;
+  a.fin = FIN_NONE;
+  return a;
+}
+
+// y = A x  [+ dots]
+void op_spmv(amg_handle_s* H, const Level& L, const double* x, double* y, int ndot, const double* d0, int fin,
+             KrylovCtl* ctl, cudaStream_t st) {
+  RowArgs a = base_args(H, L, ctl);
+  a.x = x;
+  a.out = y;
+  a.d0 = d0;
+  a.fin = fin;
+  if (ndot == 0)
+    launch_row<OP_SPMV, 0>(L, a, st);
+  else if (ndot == 1)
+    launch_row<OP_SPMV, 1>(L, a, st);
+  else
+    launch_row<OP_SPMV, 2>(L, a, st);
+}
+
+void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x, double* out, bool dot,
+               KrylovCtl* ctl, cudaStream_t st) {
+  RowArgs a = base_args(H, L, ctl);
+  a.x = x;
+  a.b = b;
+  a.out = out;
+  a.fin = FIN_RZ;
+  if (dot)
+    launch_row<OP_JACOBI, 1>(L, a, st);
+  else
+    launch_row<OP_JACOBI, 0>(L, a, st);
+}
+
+void op_jacobi0(amg_handle_s* H, const Level& L, const double* b, double* out, KrylovCtl* ctl, cudaStream_t st) {
+  RowArgs a = base_args(H, L, ctl);
+  a.b = b;
+  a.out = out;
+  launch_row<OP_JACOBI0, 0>(L, a, st);
+}
+
+void op_jacobi_prolong(amg_handle_s* H, const Level& L, const double* b, const double* x, const double* ec,
+                       double* out, bool dot, KrylovCtl* ctl, cudaStream_t st) {
+  RowArgs a = base_args(H, L, ctl);
+  a.x = x;
+  a.b = b;
+  a.ec = ec;
+  a.out = out;
+  a.fin = FIN_RZ;
+  if (dot)
+    launch_row<OP_JACOBI_PROLONG, 1>(L, a, st);
+  else
+    launch_row<OP_JACOBI_PROLONG, 0>(L, a, st);
+}
+
+void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, const double* x, double* rc,
+                          KrylovCtl* ctl, cudaStream_t st) {
+  RowArgs a = base_args(H, L, ctl);
+  a.x = x;
+  a.b = b;
+  if (L.fast) {
+    a.out = rc;
+    if (L.stream_hint)
+      k_rowblock<OP_RESTRICT, 0, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+    else
+      k_rowblock<OP_RESTRICT, 0, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+  } else {
+    a.out = L.rtmp;
+    launch_row<OP_RESID, 0>(L, a, st);
+    k_restrict_rows<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
+  }
+}
+
+void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl, cudaStream_t st) {
+  const int n = H->nL;
+  int T = n <= 32 ? 32 : (n <= 64 ? 64 : (n <= 256 ? 256 : 1024));
+  k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// S6: V-cycle from a zero guess.  *x_out points at the level's result buffer.
+// fuse_rz: the last smoother sweep of level 0 also produces r.z (FIN_RZ).
+// ------------------------------------------------------------------------------------------
+amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, KrylovCtl* ctl, bool fuse_rz,
+                      cudaStream_t st) {
+  const int Lc = (int)H->lv.size() - 1;
+  Level& L = H->lv[l];
+  if (l == Lc) {
+    op_coarse_solve(H, b, L.x, ctl, st);
+    *x_out = L.x;
+    if (fuse_rz && l == 0)
+      k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    return AMG_OK;
+  }
+  const int nu1 = H->opt.pre_sweeps, nu2 = H->opt.post_sweeps;
+  double* cur = L.x;
+  double* oth = L.x2;
+  int done_sweeps = 0;
+  if (nu1 >= 2) {
+    op_jacobi0(H, L, b, cur, ctl, st);
+    done_sweeps = 2;
+  } else if (nu1 == 1) {
+    k_scale_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.dinv, b, cur, ctl);
+    done_sweeps = 1;
+  } else {
+    k_zero<<<grid_for(L.n), TPB, 0, st>>>(L.n, cur, ctl);
+  }
+  for (int s = done_sweeps; s < nu1; ++s) {
+    op_jacobi(H, L, b, cur, oth, false, ctl, st);
+    std::swap(cur, oth);
+  }
+  Level& C = H->lv[l + 1];
+  op_residual_restrict(H, L, b, cur, C.b, ctl, st);
+  double* ec = nullptr;
+  AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st));
+  const bool want_dot = fuse_rz && l == 0;
+  if (nu2 >= 1) {
+    op_jacobi_prolong(H, L, b, cur, ec, oth, want_dot && nu2 == 1, ctl, st);
+    std::swap(cur, oth);
+    for (int s = 1; s < nu2; ++s) {
+      op_jacobi(H, L, b, cur, oth, want_dot && s == nu2 - 1, ctl, st);
+      std::swap(cur, oth);
+    }
+  } else {
+    k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
+    std::swap(cur, oth);
+    if (want_dot) k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
+  }
+  *x_out = cur;
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Krylov drivers.  Work vectors: kv[0]=x kv[1]=r kv[2]=p kv[3]=q/v kv[4]=rhat kv[5]=s kv[6]=t
+// kv[7]=phat (copy when the V-cycle result buffer is reused) kv[8]=shat
+// ------------------------------------------------------------------------------------------
+namespace {
+
+struct IterPlan {
+  int krylov, precond;
+};
+
+// one PCG iteration: q = A p, sigma; x,r update; z = B r, rho; p = z + beta p
+amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) {
+  Level& L0 = H->lv[0];
+  const int n = L0.n;
+  double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *q = H->kv[3];
+  op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
+  k_pcg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, p, q, x, r, H->partials, H->counter, H->ctl);
+  double* z = r;
+  if (precond) {
+    AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
+  } else {
+    k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+  }
+  k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
+
+amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st) {
+  Level& L0 = H->lv[0];
+  const int n = L0.n;
+  double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4], *s = H->kv[5],
+         *t = H->kv[6], *ph = H->kv[7];
+  k_bicg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, p, H->ctl);
+  double* phat = p;
+  if (precond) {
+    double* zz = nullptr;
+    AMG_TRY(amg_vcycle(H, 0, p, &zz, H->ctl, false, st));
+    // the second V-cycle of this iteration overwrites the level-0 buffers: keep phat
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(ph, zz, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    phat = ph;
+  }
+  op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
+  k_bicg_s<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, s, H->partials, H->counter, H->ctl);
+  double* shat = s;
+  if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st));
+  op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
+  k_bicg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
+                                                   H->ctl);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
+
+amg_status enqueue_iteration(amg_handle_s* H, int krylov, int precond, cudaStream_t st) {
+  return krylov == 0 ? enqueue_pcg_iteration(H, precond, st) : enqueue_bicg_iteration(H, precond, st);
+}
+
+amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStream_t st, cudaGraphExec_t* out) {
+  const int slot = krylov * 2 + precond;
+  if (H->graph_exec[slot]) {
+    *out = H->graph_exec[slot];
+    return AMG_OK;
+  }
+  cudaGraph_t g = nullptr;
+  (void)st;
+  if (!H->cap_stream) AMG_CUDA_TRY(H, cudaStreamCreateWithFlags(&H->cap_stream, cudaStreamNonBlocking));
+  AMG_CUDA_TRY(H, cudaStreamBeginCapture(H->cap_stream, cudaStreamCaptureModeThreadLocal));
+  amg_status s = enqueue_iteration(H, krylov, precond, H->cap_stream);
+  cudaError_t e = cudaStreamEndCapture(H->cap_stream, &g);
+  if (s != AMG_OK) {
+    if (g) cudaGraphDestroy(g);
+    return s;
+  }
+  AMG_CUDA_TRY(H, e);
+  cudaGraphExec_t ex = nullptr;
+  e = cudaGraphInstantiate(&ex, g, 0);
+  cudaGraphDestroy(g);
+  AMG_CUDA_TRY(H, e);
+  H->graph_exec[slot] = ex;
+  *out = ex;
+  return AMG_OK;
+}
+
+}  // namespace
+
+void amg_destroy_graphs(amg_handle_s* H) {
+  for (auto& g : H->graph_exec)
+    if (g) {
+      cudaGraphExecDestroy(g);
+      g = nullptr;
+    }
+  if (H->cap_stream) {
+    cudaStreamDestroy(H->cap_stream);
+    H->cap_stream = nullptr;
+  }
+}
+
+amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, double rtol, int maxit, int krylov,
+                            int precond, amg_info* info, cudaStream_t st) {
+  Level& L0 = H->lv[0];
+  const int n = L0.n;
+  double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4];
+  // loop control: rtol / maxit go to the device once
+  KrylovCtl init;
+  memset(&init, 0, sizeof(init));
+  init.rtol = rtol;
+  init.maxit = maxit;
+  init.status = AMG_MAXIT;
+  H->h_ctl[5] = init;
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
+  if (krylov == 0) {
+    k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
+                                                         H->counter, H->ctl, FIN_INIT_PCG);
+    double* z = r;
+    if (precond) {
+      AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
+    } else {
+      k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+    }
+    k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+  } else {
+    k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
+                                                         H->ctl, FIN_INIT_BICG);
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+
+  cudaGraphExec_t gexec = nullptr;
+  if (H->opt.use_graph && maxit > 0) AMG_TRY(get_iteration_graph(H, krylov, precond, st, &gexec));
+
+  // The host runs at most LAG iterations ahead of the device's convergence flag; iterations
+  // enqueued after convergence return at their first instruction.
+  constexpr int NSLOT = 4, LAG = 2;
+  for (int it = 0; it < maxit; ++it) {
+    if (gexec)
+      AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
+    else
+      AMG_TRY(enqueue_iteration(H, krylov, precond, st));
+    const int slot = it % NSLOT;
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[slot], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaEventRecord(H->ev[slot], st));
+    if (it >= LAG) {
+      const int old = (it - LAG) % NSLOT;
+      AMG_CUDA_TRY(H, cudaEventSynchronize(H->ev[old]));
+      if (H->h_ctl[old].done) break;
+    }
+  }
+  const bool half = (krylov == 1);
+  const double* phat = half ? (precond ? H->kv[7] : p) : nullptr;
+  k_krylov_output<<<grid_for(n), TPB, 0, st>>>(n, x, phat, L0.inv, d_x, H->ctl);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  if (info) {
+    const KrylovCtl& c = H->h_ctl[4];
+    info->iterations = c.iter;
+    info->status = c.status;
+    info->b_norm = sqrt(c.bnorm2);
+    info->rel_residual = c.bnorm2 > 0.0 ? sqrt(c.rr) / sqrt(c.bnorm2) : 0.0;
+    if (c.status == AMG_MAXIT && c.iter == 0) info->rel_residual = c.bnorm2 > 0.0 ? 1.0 : 0.0;
+  }
+  return AMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// per-level hooks (natural numbering at the boundary)
+// ------------------------------------------------------------------------------------------
+amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d_in0, const double* d_in1,
+                             double* d_out, int reps, cudaStream_t st) {
+  const int Lc = (int)H->lv.size() - 1;
+  Level& L = H->lv[level];
+  if (reps < 1) reps = 1;
+  double *t0 = H->io_tmp, *t1 = H->io_tmp2, *t2 = H->io_tmp3;
+  const bool needs_coarse = (op >= 1 && op <= 4);
+  if (needs_coarse && level >= Lc) {
+    H->err = "level op needs a level below the coarsest";
+    return AMG_ERR_INVALID_ARG;
+  }
+  auto perm_in = [&](const Level& Lv, const double* nat, double* out) {
+    k_permute_in<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, nat, Lv.inv, out);
+  };
+  auto perm_out = [&](const Level& Lv, const double* in, double* nat) {
+    k_permute_out<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, in, Lv.inv, nat);
+  };
+  switch (op) {
+    case 0:
+      if (!d_in0) return AMG_ERR_INVALID_ARG;
+      perm_in(L, d_in0, t0);
+      for (int r = 0; r < reps; ++r) op_spmv(H, L, t0, t2, 0, nullptr, FIN_NONE, nullptr, st);
+      perm_out(L, t2, d_out);
+      break;
+    case 1:
+      if (!d_in0 || !d_in1) return AMG_ERR_INVALID_ARG;
+      perm_in(L, d_in0, t0);
+      perm_in(L, d_in1, t1);
+      for (int r = 0; r < reps; ++r) op_jacobi(H, L, t1, t0, t2, false, nullptr, st);
+      perm_out(L, t2, d_out);
+      break;
+    case 2: {
+      if (!d_in0 || !d_in1) return AMG_ERR_INVALID_ARG;
+      Level& C = H->lv[level + 1];
+      perm_in(L, d_in0, t0);
+      perm_in(L, d_in1, t1);
+      for (int r = 0; r < reps; ++r) op_residual_restrict(H, L, t1, t0, t2, nullptr, st);
+      perm_out(C, t2, d_out);
+    } break;
+    case 3: {
+      if (!d_in0 || !d_in1) return AMG_ERR_INVALID_ARG;
+      Level& C = H->lv[level + 1];
+      perm_in(L, d_in0, t0);
+      perm_in(C, d_in1, t1);
+      for (int r = 0; r < reps; ++r)
+        k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
+      perm_out(L, t2, d_out);
+    } break;
+    case 4:
+      if (!d_in1) return AMG_ERR_INVALID_ARG;
+      perm_in(L, d_in1, t1);
+      for (int r = 0; r < reps; ++r) op_jacobi0(H, L, t1, t2, nullptr, st);
+      perm_out(L, t2, d_out);
+      break;
+    case 5: {
+      if (!d_in1) return AMG_ERR_INVALID_ARG;
+      perm_in(L, d_in1, t1);
+      double* z = nullptr;
+      for (int r = 0; r < reps; ++r) AMG_TRY(amg_vcycle(H, level, t1, &z, nullptr, false, st));
+      perm_out(L, z, d_out);
+    } break;
+    default:
+      H->err = "unknown level op";
+      return AMG_ERR_INVALID_ARG;
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  return AMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// G2
+// ------------------------------------------------------------------------------------------
+amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const double* d_x, int nrhs, int64_t ld,
+                                double* d_gA, int accumulate, cudaStream_t st) {
+  const int n = (int)H->n;
+  const double mean = n > 0 ? (double)H->nnz / n : 1.0;
+  if (mean <= 12.0) {
+    const int64_t threads = (int64_t)n * 8;
+    k_grad_values<8><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+                                                          d_gA, accumulate);
+  } else {
+    const int64_t threads = (int64_t)n * 32;
+    k_grad_values<32><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+                                                           d_gA, accumulate);
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  return AMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// algorithmic bytes
+// ------------------------------------------------------------------------------------------
+double amg_algorithmic_bytes(amg_handle_s* H, int which) {
+  const int Lc = (int)H->lv.size() - 1;
+  auto M = [&](int l) { return 12.0 * H->lv[l].nnz + 4.0 * (H->lv[l].n + 1); };
+  auto V = [&](int l) { return 8.0 * H->lv[l].n; };
+  auto vcycle = [&]() {
+    // per level l < L with V(2,2): 4 matrix passes + 13 vector passes + 2 index passes + 2 coarse vectors
+    const int nu1 = H->opt.pre_sweeps, nu2 = H->opt.post_sweeps;
+    double tot = 0.0;
+    for (int l = 0; l < Lc; ++l) {
+      const double Ml = M(l), Vl = V(l), Cl = 4.0 * H->lv[l].n, Vc = V(l + 1);
+      double b = 0.0;
+      if (nu1 >= 2) b += Ml + 3 * Vl;                       // fused first two sweeps: b, dinv -> x
+      else if (nu1 == 1) b += 3 * Vl;
+      else b += Vl;
+      for (int s = 2; s < nu1; ++s) b += Ml + 4 * Vl;       // x, b, dinv -> x'
+      b += Ml + 2 * Vl + Cl + Vc;                           // residual + restriction: x, b, agg_ptr -> r_c
+      if (nu2 >= 1) b += Ml + 4 * Vl + Cl + Vc;             // prolongation fused into the first post sweep
+      else b += 2 * Vl + Cl + Vc;
+      for (int s = 1; s < nu2; ++s) b += Ml + 4 * Vl;
+      tot += b;
+    }
+    tot += 8.0 * H->nL * H->nL + 16.0 * H->nL;
+    return tot;
+  };
+  switch (which) {
+    case 0: return M(0) + 2 * V(0);
+    case 1: return vcycle();
+    case 2: return (M(0) + 2 * V(0)) + 6 * V(0) + 3 * V(0) + vcycle();
+    case 3: return 2 * (M(0) + 2 * V(0)) + 2 * vcycle() + (4 + 3 + 8) * V(0) + 2 * V(0);
+    case 4: return M(0) + 4 * V(0);
+    default: return 0.0;
+  }
+}
