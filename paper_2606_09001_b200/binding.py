@@ -275,6 +275,9 @@ class AmgSolver:
     def level_info(self, level):
         return amg_get_level_info(self.h, level)
 
+    def level_path(self, level):
+        return amg_get_level_path(self.h, level)
+
     def aggregates(self, level):
         out = torch.empty(self.level_info(level)[0], dtype=torch.int32, device=self.device)
         amg_get_aggregates(self.h, level, out)

@@ -1,0 +1,446 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Sizes: small enough for the oracle to finish in
+seconds, large enough to span many row blocks and a ragged tail; plus the full-size headline
+configuration (cfg 3, 128^3) in the launch configuration bench.py times.
+
+Tolerances (BASELINE.json north_star):
+  host fp64 ||b - A x|| / ||b||  <= 1e-8
+  ||x - x_oracle|| / ||x_oracle|| <= 1e-6   (both sides at rtol_check = 1e-11 / 1e-13, reading A12)
+  gradient relative L2 error      <= 1e-5
+  iterations within +-2 of the oracle on the identical hierarchy (aggregates bit-equal, A13)
+  integer results (aggregates, coarse patterns, level counts): bit-exact
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from paper_2606_09001_b200 import inputs  # noqa: E402
+
+CASES = {
+    "cfg1_64": (1, 64),      # BASELINE configs[0] at full size
+    "cfg2_96": (2, 96),      # 2D manufactured solution
+    "cfg3_40": (3, 40),      # 3D Poisson, 64000 rows: ~150 row blocks on level 0, ragged tail
+    "cfg4_28": (4, 28),      # variable coefficients, random permutation
+}
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / max(np.linalg.norm(np.asarray(b)), 1e-300))
+
+
+class Case:
+    def __init__(self, name, oracle_mod, B, **gpu_opts):
+        cfg, edge = CASES[name]
+        self.cfg = cfg
+        self.A = inputs.config_matrix(cfg, edge)
+        self.Asp = self.A.to_scipy()
+        v = inputs.config_rhs(cfg, self.A.n)
+        self.x_true = v if cfg == 2 else None
+        self.b = self.Asp @ v if cfg == 2 else v
+        self.o = oracle_mod.Oracle(self.A.rowptr, self.A.col, self.A.val)
+        self.s = B.AmgSolver(self.A.rowptr, self.A.col, self.A.val, **gpu_opts)
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_09001_b200 import binding
+
+    assert torch.cuda.is_available()
+    binding.load_library()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def cases(oracle_mod, B):
+    cache = {}
+
+    def get(name, **opts):
+        key = (name, tuple(sorted(opts.items())))
+        if key not in cache:
+            cache[key] = Case(name, oracle_mod, B, **opts)
+        return cache[key]
+
+    yield get
+    for c in cache.values():
+        c.s.close()
+        c.o.close()
+
+
+# ------------------------------------------------------------------------------------------
+# setup phase U1-U7: identical hierarchy (integers bit-exact, coarse values to rounding)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", list(CASES))
+def test_hierarchy_is_identical(cases, name):
+    c = cases(name)
+    assert c.s.num_levels == c.o.num_levels
+    for l in range(c.s.num_levels):
+        assert c.s.level_info(l) == c.o.level_info(l)
+        if l < c.s.num_levels - 1:
+            assert np.array_equal(c.s.aggregates(l).cpu().numpy(), c.o.aggregates(l)), f"level {l}"
+        rp, cl, vl = [t.cpu().numpy() for t in c.s.level_csr(l)]
+        orp, ocl, ovl = c.o.level_csr(l)
+        assert np.array_equal(rp, orp) and np.array_equal(cl, ocl), f"pattern of level {l}"
+        # same summation order (ascending fine row, then position): equal to rounding
+        assert np.max(np.abs(vl - ovl)) <= 1e-13 * np.max(np.abs(ovl)), f"values of level {l}"
+
+
+# ------------------------------------------------------------------------------------------
+# solve-phase kernels S1-S5, one level at a time, both kernel families
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("generic", [0, 1])
+@pytest.mark.parametrize("name", list(CASES))
+def test_level_kernels(cases, name, generic):
+    c = cases(name, force_generic=generic)
+    rng = np.random.default_rng(7)
+    nlev = c.s.num_levels
+    if generic:
+        assert all(c.s.level_path(l) == 0 for l in range(nlev))
+    else:
+        assert c.s.level_path(0) == 1
+    for l in range(nlev - 1):
+        n, _ = c.s.level_info(l)
+        nc, _ = c.s.level_info(l + 1)
+        x, b, ec = rng.standard_normal(n), rng.standard_normal(n), rng.standard_normal(nc)
+        rp, cl, vl = c.o.level_csr(l)
+        scale = np.abs(vl).max() * 8  # row sums of |a_ij||x_j|, x ~ N(0,1)
+        agg = c.o.aggregates(l)
+        y = c.s.level_op(l, 0, x, None, n).cpu().numpy()
+        assert np.max(np.abs(y - c.o.spmv(l, x))) <= 1e-14 * scale * 8
+        y = c.s.level_op(l, 1, x, b, n).cpu().numpy()
+        assert np.max(np.abs(y - c.o.smooth(l, b, x))) <= 1e-13
+        y = c.s.level_op(l, 2, x, b, nc).cpu().numpy()
+        assert np.max(np.abs(y - c.o.residual_restrict(l, b, x))) <= 1e-13 * scale
+        y = c.s.level_op(l, 3, x, ec, n).cpu().numpy()
+        assert np.array_equal(y, x + 1.0 * ec[agg])
+        y = c.s.level_op(l, 4, None, b, n).cpu().numpy()
+        x1 = c.o.smooth(l, b, np.zeros(n))
+        assert np.max(np.abs(y - c.o.smooth(l, b, x1))) <= 1e-13
+        y = c.s.level_op(l, 5, None, b, n).cpu().numpy()
+        z = c.o.vcycle(b, l)
+        assert rel(y, z) <= 1e-12
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_apply_preconditioner(cases, name):
+    c = cases(name)
+    r = np.random.default_rng(11).standard_normal(c.A.n)
+    z = c.s.apply_preconditioner(r).cpu().numpy()
+    assert rel(z, c.o.vcycle(r, 0)) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------
+# S6-S9: whole solves
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("graph", [1, 0])
+@pytest.mark.parametrize("krylov", [0, 1])
+@pytest.mark.parametrize("name", list(CASES))
+def test_solve_parity(cases, name, krylov, graph):
+    c = cases(name, use_graph=graph)
+    bn = np.linalg.norm(c.b)
+    # timed tolerance: residual and iteration count
+    xg, ig = c.s.solve(c.b, 1e-8, 1000, krylov)
+    xo, io = c.o.solve(c.b, 1e-8, 1000, krylov, 1)
+    xg = xg.cpu().numpy()
+    assert ig.status == 0 and io.status == 0
+    assert np.linalg.norm(c.b - c.Asp @ xg) / bn <= 1e-8
+    assert abs(ig.iterations - io.iterations) <= 2
+    assert abs(ig.b_norm - bn) <= 1e-12 * bn
+    assert ig.rel_residual <= 1e-8
+    # parity tolerance (A12)
+    xg, ig = c.s.solve(c.b, 1e-11, 1000, krylov)
+    xo, io = c.o.solve(c.b, 1e-13, 1000, krylov, 1)
+    assert ig.status == 0 and io.status == 0
+    assert rel(xg.cpu().numpy(), xo) <= 1e-6
+    if c.x_true is not None:  # P9
+        assert rel(xg.cpu().numpy(), c.x_true) <= 1e-6
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_unpreconditioned_krylov(cases, krylov):
+    c = cases("cfg1_64")
+    xg, ig = c.s.solve(c.b, 1e-8, 2000, krylov, precond=0)
+    xo, io = c.o.solve(c.b, 1e-8, 2000, krylov, 0)
+    assert ig.status == 0
+    # unpreconditioned BiCGSTAB is sensitive to rounding order: a wider window than +-2 there
+    assert abs(ig.iterations - io.iterations) <= (2 if krylov == 0 else 12)
+    assert np.linalg.norm(c.b - c.Asp @ xg.cpu().numpy()) / np.linalg.norm(c.b) <= 1e-8
+
+
+def test_determinism_bitwise(cases, B):
+    c = cases("cfg3_40")
+    x1, i1 = c.s.solve(c.b, 1e-8, 500, 0)
+    x2, i2 = c.s.solve(c.b, 1e-8, 500, 0)
+    assert i1.iterations == i2.iterations and torch.equal(x1, x2)
+    s2 = B.AmgSolver(c.A.rowptr, c.A.col, c.A.val)
+    x3, i3 = s2.solve(c.b, 1e-8, 500, 0)
+    assert i3.iterations == i1.iterations and torch.equal(x1, x3)
+    for l in range(s2.num_levels - 1):
+        assert torch.equal(s2.aggregates(l), c.s.aggregates(l))
+    s2.close()
+
+
+def test_solve_host_and_batched(cases, B):
+    c = cases("cfg3_40")
+    n = c.A.n
+    xd, _ = c.s.solve(c.b, 1e-8, 500)
+    hb = torch.as_tensor(c.b).pin_memory()
+    hx = torch.empty(n, dtype=torch.float64).pin_memory()
+    info = B.amg_solve_host(c.s.h, hb, hx, 1e-8, 500)
+    assert info.status == 0 and torch.equal(hx, xd.cpu())
+    nrhs = 3
+    Bm = torch.stack([torch.as_tensor(inputs.config_rhs(5, n, k)) for k in range(nrhs)]).cuda().contiguous()
+    X = torch.empty_like(Bm)
+    infos = B.amg_solve_batched(c.s.h, 0, Bm, X, nrhs, n, 1e-8, 500)
+    for k in range(nrhs):
+        xo, io = c.o.solve(Bm[k].cpu().numpy(), 1e-8, 500, 0, 1)
+        assert infos[k].status == 0 and abs(infos[k].iterations - io.iterations) <= 2
+        bk = Bm[k].cpu().numpy()
+        assert np.linalg.norm(bk - c.Asp @ X[k].cpu().numpy()) / np.linalg.norm(bk) <= 1e-8
+    XT = torch.empty_like(Bm)
+    B.amg_solve_batched(c.s.h, 1, Bm, XT, nrhs, n, 1e-8, 500)
+    assert torch.equal(X, XT)  # symmetric: the transposed solve is the solve
+
+
+# ------------------------------------------------------------------------------------------
+# G1-G3: adjoint solve and gradients
+# ------------------------------------------------------------------------------------------
+def test_transpose_solve_is_solve_bitwise_when_symmetric(cases):
+    c = cases("cfg4_28")
+    g = np.random.default_rng(5).standard_normal(c.A.n)
+    x, i1 = c.s.solve(g, 1e-8, 500)
+    lam, i2 = c.s.solve_transpose(g, 1e-8, 500)
+    assert i1.iterations == i2.iterations and torch.equal(x, lam)
+
+
+@pytest.mark.parametrize("name", ["cfg3_40", "cfg4_28"])
+def test_adjoint_gradients(cases, name):
+    c = cases(name)
+    n = c.A.n
+    nrhs = 3
+    Bs = [inputs.config_rhs(5, n, k) for k in range(nrhs)]
+    Ts = [inputs.config_target(n, k) for k in range(nrhs)]
+    Xg, Lg, Xo, Lo = [], [], [], []
+    for b, t in zip(Bs, Ts):
+        x, _ = c.s.solve(b, 1e-11, 1000)
+        lam, _ = c.s.solve_transpose(x - torch.as_tensor(t).cuda(), 1e-11, 1000)
+        Xg.append(x)
+        Lg.append(lam)
+        xo, _ = c.o.solve(b, 1e-13, 1000, 0, 1)
+        lo, _ = c.o.solve_transpose(xo - t, 1e-13, 1000, 0, 1, 1)
+        Xo.append(xo)
+        Lo.append(lo)
+        assert rel(lam.cpu().numpy(), lo) <= 1e-5  # dL/db = lambda
+        # adjoint identity g.x = lambda.b (P10 iii)
+        g = (x - torch.as_tensor(t).cuda()).cpu().numpy()
+        assert abs(g @ x.cpu().numpy() - lam.cpu().numpy() @ b) <= 1e-8 * np.linalg.norm(g) * np.linalg.norm(x.cpu().numpy())
+    Xg, Lg = torch.stack(Xg).contiguous(), torch.stack(Lg).contiguous()
+    gO = c.o.grad_values(np.stack(Lo), np.stack(Xo))
+    gA = c.s.grad_values(Lg, Xg)
+    assert rel(gA.cpu().numpy(), gO) <= 1e-5
+    # same inputs on both sides: the gradient kernel itself to rounding
+    gO2 = c.o.grad_values(Lg.cpu().numpy(), Xg.cpu().numpy())
+    assert np.max(np.abs(gA.cpu().numpy() - gO2)) <= 1e-14 * np.max(np.abs(gO2)) * nrhs
+    # accumulate: one right-hand side at a time
+    acc = torch.zeros_like(gA)
+    for k in range(nrhs):
+        c.s.grad_values(Lg[k], Xg[k], accumulate_into=acc)
+    assert rel(acc.cpu().numpy(), gO2) <= 1e-14
+
+
+# ------------------------------------------------------------------------------------------
+# options, imported aggregates, edge cases
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("opts", [
+    dict(smoother=1), dict(pre_sweeps=1, post_sweeps=1), dict(pre_sweeps=3, post_sweeps=3),
+    dict(pre_sweeps=0, post_sweeps=0), dict(pre_sweeps=2, post_sweeps=1), dict(coarse_scale=1.3),
+    dict(coarse_max_rows=500), dict(hash_seed=12345), dict(strong_beta=0.5), dict(max_match_rounds=2),
+    dict(max_levels=3, coarse_max_rows=8),
+])
+def test_options(oracle_mod, B, opts):
+    A = inputs.config_matrix(3, 16)
+    b = inputs.config_rhs(3, A.n)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, **opts)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, **opts)
+    assert s.num_levels == o.num_levels
+    for l in range(s.num_levels - 1):
+        assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l))
+    r = np.random.default_rng(3).standard_normal(A.n)
+    assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+    if opts.get("pre_sweeps") == 0 and opts.get("post_sweeps") == 0:
+        s.close()  # V(0,0) is the rank-deficient coarse correction alone: not a preconditioner
+        o.close()
+        return
+    # unequal sweeps give a nonsymmetric B: BiCGSTAB for those
+    krylov = 1 if opts.get("pre_sweeps", 2) != opts.get("post_sweeps", 2) else 0
+    xg, ig = s.solve(b, 1e-8, 1000, krylov)
+    xo, io = o.solve(b, 1e-8, 1000, krylov, 1)
+    assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+    assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) / np.linalg.norm(b) <= 1e-8
+    s.close()
+    o.close()
+
+
+def test_imported_aggregates_1d_closed_form(oracle_mod, B):
+    # P5(i): pairs {2I, 2I+1} of tridiag(-1,2,-1) give exactly tridiag(-1,2,-1) of half the size
+    n = 4096
+    A = inputs.poisson_csr(n)
+    aggs, m = [], n
+    for _ in range(3):
+        aggs.append((np.arange(m) // 2).astype(np.int32))
+        m //= 2
+    s = B.AmgSolver(A.rowptr, A.col, A.val, aggregates=aggs)
+    assert s.num_levels == 4
+    for l in range(1, 4):
+        T = inputs.poisson_csr(n >> l)
+        rp, cl, vl = [t.cpu().numpy() for t in s.level_csr(l)]
+        assert np.array_equal(rp, T.rowptr) and np.array_equal(cl, T.col) and np.array_equal(vl, T.val)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, aggregates=aggs)
+    r = np.random.default_rng(2).standard_normal(n)
+    assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+    s.close()
+    o.close()
+
+
+def test_edge_cases(oracle_mod, B):
+    # tiny system: a single level, dense LU is the exact preconditioner -> 1 iteration (P4)
+    A = inputs.poisson_csr((6, 5))
+    b = inputs.rhs_uniform(A.n, 9)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    assert s.num_levels == 1
+    for krylov in (0, 1):
+        x, info = s.solve(b, 1e-10, 50, krylov)
+        assert info.status == 0 and info.iterations == 1
+        assert rel(x.cpu().numpy(), np.linalg.solve(A.to_dense(), b)) <= 1e-12
+    # zero right-hand side: x = 0, 0 iterations, converged
+    x, info = s.solve(np.zeros(A.n), 1e-8, 50)
+    assert info.status == 0 and info.iterations == 0 and float(x.abs().max()) == 0.0
+    s.close()
+    # 1x1 system
+    one = B.AmgSolver(np.array([0, 1]), np.array([0]), np.array([2.5]))
+    x, info = one.solve(np.array([5.0]), 1e-12, 5)
+    assert info.status == 0 and abs(float(x[0]) - 2.0) < 1e-15
+    one.close()
+    # maxit reached: status MAXIT, iterations == maxit; maxit = 0: x = 0
+    A = inputs.config_matrix(3, 16)
+    b = inputs.config_rhs(3, A.n)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    for krylov in (0, 1):
+        x, info = s.solve(b, 1e-8, 3, krylov)
+        xo, io = o.solve(b, 1e-8, 3, krylov, 1)
+        assert info.status == B.AMG_MAXIT == io.status and info.iterations == 3
+        assert rel(x.cpu().numpy(), xo) <= 1e-10
+        assert abs(info.rel_residual - io.rel_residual) <= 1e-9 * io.rel_residual + 1e-18
+    x, info = s.solve(b, 1e-8, 0)
+    assert info.iterations == 0 and float(x.abs().max()) == 0.0
+    # NaN in b: reported, not hung
+    bn = b.copy()
+    bn[5] = np.nan
+    x, info = s.solve(bn, 1e-8, 10)
+    assert info.status == B.AMG_NONFINITE
+    # the handle still works afterwards
+    x, info = s.solve(b, 1e-8, 100)
+    assert info.status == 0
+    s.close()
+    o.close()
+
+
+def test_error_returns(B):
+    A = inputs.poisson_csr((8, 8))
+    # unsorted columns
+    col = A.col.copy()
+    col[[0, 1]] = col[[1, 0]]
+    with pytest.raises(B.AmgError) as e:
+        B.AmgSolver(A.rowptr, col, A.val)
+    assert e.value.status == 2
+    # missing / non-positive diagonal
+    val = A.val.copy()
+    val[A.col == np.repeat(np.arange(A.n), np.diff(A.rowptr))] = -4.0
+    with pytest.raises(B.AmgError) as e:
+        B.AmgSolver(A.rowptr, A.col, val)
+    assert e.value.status == 2
+    # column out of range
+    col = A.col.copy()
+    col[-1] = A.n
+    with pytest.raises(B.AmgError):
+        B.AmgSolver(A.rowptr, col, A.val)
+    # singular coarsest operator: pure Neumann 1D Laplacian on <= 64 rows
+    n = 32
+    T = inputs.poisson_csr(n)
+    v = T.val.copy()
+    v[0] = 1.0
+    v[-1] = 1.0
+    with pytest.raises(B.AmgError) as e:
+        B.AmgSolver(T.rowptr, T.col, v)
+    assert e.value.status == 5
+    # nonsymmetric matrix: detected on the device, transpose solve refused (NEXT-2)
+    v = A.val.copy()
+    v[1] = -0.5
+    s = B.AmgSolver(A.rowptr, A.col, v, symmetric=-1)
+    with pytest.raises(B.AmgError) as e:
+        s.solve_transpose(np.ones(A.n))
+    assert e.value.status == 7
+    s.close()
+    with pytest.raises(AttributeError):
+        B.amg_options_default(no_such_option=1)
+
+
+# ------------------------------------------------------------------------------------------
+# full-size headline configuration, as bench.py launches it (cfg 3: 128^3, default options)
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def full3(oracle_mod, B):
+    A = inputs.config_matrix(3)
+    b = inputs.config_rhs(3, A.n)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    yield A, b, s
+    s.close()
+
+
+def test_full_size_cfg3_against_oracle(full3, oracle_mod):
+    import os
+
+    A, b, s = full3
+    oracle_mod.set_threads(os.cpu_count() or 1)
+    try:
+        o = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+        assert s.num_levels == o.num_levels
+        for l in range(s.num_levels):
+            assert s.level_info(l) == o.level_info(l)
+            if l < s.num_levels - 1:
+                assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l))
+        Asp = A.to_scipy()
+        for krylov in (0, 1):
+            xg, ig = s.solve(b, 1e-8, 500, krylov)
+            xo, io = o.solve(b, 1e-8, 500, krylov, 1)
+            xg = xg.cpu().numpy()
+            assert ig.status == 0 and abs(ig.iterations - io.iterations) <= 2
+            assert np.linalg.norm(b - Asp @ xg) / np.linalg.norm(b) <= 1e-8
+            # same algorithm, same hierarchy, same iteration: the iterates agree far below 1e-6
+            if ig.iterations == io.iterations:
+                assert rel(xg, xo) <= 1e-9
+        r = np.random.default_rng(1).standard_normal(A.n)
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+        o.close()
+    finally:
+        oracle_mod.set_threads(1)
+
+
+def test_full_size_cfg3_properties(full3):
+    A, b, s = full3
+    rng = np.random.default_rng(4)
+    # the preconditioner is symmetric: <B u, v> = <u, B v>  (P6 at full size)
+    u, v = rng.standard_normal(A.n), rng.standard_normal(A.n)
+    Bu, Bv = s.apply_preconditioner(u).cpu().numpy(), s.apply_preconditioner(v).cpu().numpy()
+    assert abs(Bu @ v - u @ Bv) <= 1e-12 * np.linalg.norm(Bu) * np.linalg.norm(v)
+    assert Bu @ u > 0
+    # sampled gradient entries, recomputed one by one from the definition (Eq. 2)
+    x, _ = s.solve(b, 1e-8, 500)
+    lam, _ = s.solve_transpose(x - 1.0, 1e-8, 500)
+    gA = s.grad_values(lam, x).cpu().numpy()
+    xs, ls = x.cpu().numpy(), lam.cpu().numpy()
+    ks = rng.integers(0, A.nnz, 2000)
+    rows = np.searchsorted(A.rowptr, ks, side="right") - 1
+    assert np.array_equal(gA[ks], -(ls[rows] * xs[A.col[ks]]))
