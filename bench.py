@@ -1,0 +1,417 @@
+"""bench.py — AMG-PCG solve time + V-cycle HBM GB/s on the 3D 128^3 fp64 Poisson system (one B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--cfg 3] [--edge E]
+
+A "step" is one pass of the solve-phase hot path on the cached hierarchy: one AMG-PCG solve of
+A x = b from x0 = 0 to ||r|| <= 1e-8 ||b|| (BASELINE.json configs[2], the
+configuration the metric is quoted on).  The other rows of §8(a) are timed beside it in the same
+run and reported under "phases": the cold device setup (U1-U7, "timed separately and amortized
+by the cache"), one V-cycle, the BiCGSTAB solve, the adjoint solve + matrix-value gradient
+(G1-G3).  Inputs are seeded synthetic PDE matrices (paper_2606_09001_b200/inputs.py).
+
+One JSON line on stdout (rank 0).  N > 1: "replicas only": every rank
+solves the same system on its own GPU; no data-path collective.
+
+--impl reference: times the CPU oracle (oracle/, the slow fp64 reference) on the host cores on
+the same workload and metric; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "amg_pcg_solve_ms_rtol1e-8"
+RTOL = 1e-8
+MAXIT = 1000
+WORKLOADS = {
+    1: "cfg1: 2D 5-point Poisson 64x64, b~U[-1,1]",
+    2: "cfg2: 2D 5-point Poisson 1024x1024, b=A*N(0,1)",
+    3: "cfg3: 3D 7-point Poisson 128^3 (N=2097152, nnz=14581760), b~U[-1,1], AMG-PCG rtol 1e-8",
+    4: "cfg4: 3D 7-point variable-coefficient diffusion 192^3, randomly permuted rows, b~U[-1,1]",
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cfg", type=int, default=3)
+    ap.add_argument("--edge", type=int, default=None, help="grid edge (default: the config's full size)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-phases", action="store_true", help="skip the setup / BiCGSTAB / adjoint extras")
+    return ap.parse_args()
+
+
+def peaks():
+    """(HBM GB/s, label): the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax.append(float(f[1]))
+                power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def make_workload(cfg, edge):
+    from paper_2606_09001_b200 import inputs
+
+    A = inputs.config_matrix(cfg, edge)
+    v = inputs.config_rhs(cfg, A.n)
+    b = A.to_scipy() @ v if cfg == 2 else v
+    return A, b
+
+
+def oracle_run(A, b, threads, maxit=MAXIT):
+    """The CPU oracle as it stands: setup + one PCG solve; returns (setup_s, solve_s, info)."""
+    import oracle
+
+    oracle.build()
+    oracle.set_threads(threads)
+    t = time.perf_counter()
+    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    t_setup = time.perf_counter() - t
+    t = time.perf_counter()
+    _, info = o.solve(b, RTOL, maxit, 0, 1)
+    t_solve = time.perf_counter() - t
+    used = oracle.get_threads()
+    o.close()
+    return t_setup, t_solve, info, used
+
+
+def run_b200(args):
+    import numpy as np
+    import torch
+
+    from paper_2606_09001_b200 import binding as B, inputs
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    K, W = args.steps, max(args.warmup, 3)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(v):
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    A, b = make_workload(args.cfg, args.edge)
+    n, nnz = A.n, A.nnz
+    B.load_library()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev)
+    torch.cuda.synchronize()
+    setup_first_ms = (time.perf_counter() - t0) * 1e3  # includes the H2D copy of the CSR arrays and context warm-up
+    h = s.h
+    nlev = s.num_levels
+    levels = [s.level_info(l) for l in range(nlev)]
+    d_b = torch.as_tensor(b).to(dev)
+    d_x = torch.empty_like(d_b)
+    bytes_spmv, bytes_vcycle, bytes_pcg_it, bytes_bicg_it, bytes_sweep = (B.amg_get_algorithmic_bytes(h, w) for w in range(5))
+    hier_bytes = sum(12 * z + 4 * (r + 1) for r, z in levels)
+
+    # ---- the timed region: K PCG solves -------------------------------------------------
+    for _ in range(W):
+        info = B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 0, 1)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = [ev() for _ in range(K)], [ev() for _ in range(K)]
+    launches = 0
+    barrier()
+    for i in range(K):
+        e0[i].record()
+        info = B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 0, 1)
+        e1[i].record()
+        launches += B.amg_get_last_launches(h)
+    barrier()
+    total_ms = e0[0].elapsed_time(e1[-1])
+    step_ms = [a.elapsed_time(c) for a, c in zip(e0, e1)]
+    clocks = sampler.stop() if rank == 0 else None
+    ms_per_step = max_over_ranks(total_ms / K)
+    iters = info.iterations
+    xg = d_x.cpu().numpy()
+    true_res = float(np.linalg.norm(b - A.to_scipy() @ xg) / np.linalg.norm(b))
+
+    # ---- end to end: host buffers, H2D of b and D2H of x inside the timed region ----------
+    hb = torch.as_tensor(b).pin_memory()
+    hx = torch.empty(n, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        B.amg_solve_host(h, hb, hx, RTOL, MAXIT)
+    barrier()
+    a0, a1 = ev(), ev()
+    a0.record()
+    for _ in range(K):
+        B.amg_solve_host(h, hb, hx, RTOL, MAXIT)
+    a1.record()
+    barrier()
+    e2e_ms = max_over_ranks(a0.elapsed_time(a1) / K)
+
+    # ---- dominant kernel: the level-0 smoother sweep (k_rowblock<OP_JACOBI>) -------------
+    def timed_level_op(level, op, in0, in1, out, reps):
+        c0, c1 = ev(), ev()
+        torch.cuda.synchronize()
+        c0.record()
+        B.amg_level_op(h, level, op, in0, in1, out, reps)
+        c1.record()
+        torch.cuda.synchronize()
+        return c0.elapsed_time(c1)
+
+    def per_rep_ms(level, op, in0, in1, out, r1, r2):
+        timed_level_op(level, op, in0, in1, out, r1)
+        t1 = min(timed_level_op(level, op, in0, in1, out, r1) for _ in range(3))
+        t2 = min(timed_level_op(level, op, in0, in1, out, r2) for _ in range(3))
+        return (t2 - t1) / (r2 - r1)
+
+    roof = None
+    vc = None
+    if nlev > 1:
+        tmp = torch.empty_like(d_b)
+        sweep_ms = per_rep_ms(0, 1, d_x, d_b, tmp, 10, 60)
+        spmv_ms = per_rep_ms(0, 0, d_x, None, tmp, 10, 60)
+        vcycle_ms = per_rep_ms(0, 5, None, d_b, tmp, 3, 13)
+        peak, peak_src = peaks()
+        ach = bytes_sweep / (sweep_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_rowblock<OP_JACOBI> level 0 (smoother sweep fused with the residual)",
+                "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4), "traffic": None,
+                "bytes_per_launch": bytes_sweep, "us_per_launch": round(sweep_ms * 1e3, 2), "peak_source": peak_src,
+                "how": "CUDA events around 10 and 60 back-to-back launches (amg_level_op), difference / 50; operands 234 MB > L2"}
+        vc = {"ms": round(vcycle_ms, 4), "bytes": bytes_vcycle, "gbs": round(bytes_vcycle / vcycle_ms / 1e6, 1),
+              "frac_of_peak": round(bytes_vcycle / vcycle_ms / 1e6 / peak, 4),
+              "spmv_l0_us": round(spmv_ms * 1e3, 2), "spmv_l0_gbs": round(bytes_spmv / spmv_ms / 1e6, 1)}
+    peak, peak_src = peaks()
+    solve_bytes = bytes_pcg_it * iters + bytes_vcycle + 6 * 8 * n
+    solve_gbs = solve_bytes / (ms_per_step * 1e-3) / 1e9
+
+    # ---- the other rows of the hot path, timed beside it ---------------------------------
+    phases = {}
+    if not args.no_phases:
+        c0, c1 = ev(), ev()
+        B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 1, 1)
+        torch.cuda.synchronize()
+        c0.record()
+        ib = B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 1, 1)
+        c1.record()
+        torch.cuda.synchronize()
+        phases["bicgstab_solve_ms"] = round(c0.elapsed_time(c1), 3)
+        phases["bicgstab_iterations"] = ib.iterations
+        # adjoint of L = 0.5 ||x - x_target||^2 and the gradients (Eq. 1-2)
+        B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 0, 1)
+        g = d_x - torch.as_tensor(inputs.config_target(n, 0)).to(dev)
+        lam = torch.empty_like(g)
+        gA = torch.empty(nnz, dtype=torch.float64, device=dev)
+        B.amg_solve_transpose(h, g, lam, RTOL, MAXIT)
+        B.amg_grad_values(h, lam, d_x, 1, n, gA, 0)
+        torch.cuda.synchronize()
+        c0.record()
+        ia = B.amg_solve_transpose(h, g, lam, RTOL, MAXIT)
+        c1.record()
+        c2 = ev()
+        B.amg_grad_values(h, lam, d_x, 1, n, gA, 0)
+        c2.record()
+        torch.cuda.synchronize()
+        phases["adjoint_solve_ms"] = round(c0.elapsed_time(c1), 3)
+        phases["adjoint_iterations"] = ia.iterations
+        phases["grad_values_ms"] = round(c1.elapsed_time(c2), 3)
+        gbytes = 12.0 * nnz + 4.0 * (n + 1) + 2 * 8.0 * n
+        phases["grad_values_gbs"] = round(gbytes / c1.elapsed_time(c2) / 1e6, 1)
+        # device setup, second build (context, allocator and the CSR copy already warm)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h2 = B.amg_setup(n, nnz, s.d_rowptr, s.d_col, s.d_val, s.opt)
+        torch.cuda.synchronize()
+        phases["setup_ms"] = round((time.perf_counter() - t0) * 1e3, 2)
+        st = B.amg_get_setup_stats(h2)
+        phases["setup_breakdown_ms"] = {"aggregate": round(st.aggregate_ms, 2), "galerkin": round(st.galerkin_ms, 2),
+                                        "reorder": round(st.reorder_ms, 2), "lu": round(st.lu_ms, 2)}
+        phases["setup_first_call_ms"] = round(setup_first_ms, 1)
+        phases["match_rounds_max"] = st.match_rounds_max
+        B.amg_destroy(h2)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        ts, tv, io, used = oracle_run(A, b, cores)
+        cpu = {"value": round(tv * 1e3, 1), "unit": "ms", "cores": used, "kind": "oracle",
+               "sample": f"the whole workload once: oracle PCG solve ({io.iterations} iterations, relres {io.rel_residual:.2e}); "
+                         f"its setup took {ts * 1e3:.0f} ms (not in value)",
+               "setup_ms": round(ts * 1e3, 1), "iterations": io.iterations}
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": round(ms_per_step, 4), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS.get(args.cfg, str(args.cfg)) + (f" [edge {args.edge}]" if args.edge else ""),
+                       "n": n, "nnz": nnz, "levels": nlev, "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": f"no flush: one iteration streams the {hier_bytes / 1e6:.0f} MB hierarchy (> 126 MB L2)"},
+            "iterations": iters, "rel_residual": info.rel_residual, "true_rel_residual_host_fp64": true_res,
+            "status": info.status, "step_ms_median": round(statistics.median(step_ms), 4),
+            "step_ms_min": round(min(step_ms), 4),
+            "e2e": {"value": round(e2e_ms, 4), "unit": "ms", "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n,
+                    "api": "amg_solve_host (pinned host b -> device, solve, x -> pinned host)"},
+            "gpu_launches": launches,
+            "roofline": roof,
+            "solve_phase": {"algorithmic_bytes": solve_bytes, "achieved_gbs": round(solve_gbs, 1), "peak": peak,
+                            "frac": round(solve_gbs / peak, 4), "frac_of_8000_nominal": round(solve_gbs / 8000.0, 4),
+                            "bytes_per_iteration": bytes_pcg_it, "peak_source": peak_src},
+            "vcycle": vc, "phases": phases, "cpu_baseline": cpu, "clocks": clocks,
+        }
+        print(json.dumps(out), flush=True)
+    s.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The reference arm of this tier: the CPU oracle, as it stands, on the host cores."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import oracle
+
+    K, W = args.steps, args.warmup
+    A, b = make_workload(args.cfg, args.edge)
+    cores = os.cpu_count() or 1
+    oracle.build()
+    oracle.set_threads(cores)
+    t = time.perf_counter()
+    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    setup_s = time.perf_counter() - t
+    t = time.perf_counter()
+    _, full = o.solve(b, RTOL, MAXIT, 0, 1)
+    full_s = time.perf_counter() - t
+    # bounded sample: whole solves while K+W of them fit ~150 s, else the first m iterations scaled to the full count
+    budget_s = 150.0
+    m = full.iterations
+    if (K + W) * full_s > budget_s:
+        m = max(2, int(full.iterations * budget_s / ((K + W) * full_s)))
+    scale = full.iterations / m
+    for _ in range(W):
+        o.solve(b, RTOL, m, 0, 1)
+    times = []
+    for _ in range(K):
+        t = time.perf_counter()
+        o.solve(b, RTOL, m, 0, 1)
+        times.append((time.perf_counter() - t) * scale)
+    used = oracle.get_threads()
+    o.close()
+    ms = 1e3 * sum(times) / len(times)
+    sample = (f"each step = one whole oracle PCG solve ({full.iterations} iterations)" if m == full.iterations else
+              f"each step = the first {m} of {full.iterations} oracle PCG iterations, time scaled by {scale:.3f}")
+    out = {"impl": "reference", "metric": METRIC, "value": round(ms, 2), "unit": "ms", "n_gpus": args.gpus, "steps": K,
+           "warmup": W, "ms_per_step": round(ms, 2), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": WORKLOADS.get(args.cfg, str(args.cfg)) + (f" [edge {args.edge}]" if args.edge else ""),
+                      "n": A.n, "nnz": A.nnz, "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi",
+                      "parallelism": "host cores (OpenMP row loops)"},
+           "iterations": full.iterations, "rel_residual": full.rel_residual,
+           "cpu_baseline": {"value": round(ms, 2), "unit": "ms", "cores": used, "kind": "oracle", "sample": sample,
+                            "setup_ms": round(setup_s * 1e3, 1)},
+           "e2e": {"value": round(ms, 2), "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

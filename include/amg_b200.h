@@ -182,6 +182,10 @@ AMG_API amg_status amg_get_level_path(amg_handle h, int32_t level, int32_t* fast
  * 4 one level-0 smoother sweep. */
 AMG_API amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes);
 
+/* Kernel launches enqueued by the last amg_solve* / amg_level_op / amg_grad_values call on this
+ * handle (graph replays count their kernel nodes); the caller's evidence for "gpu_launches". */
+AMG_API amg_status amg_get_last_launches(amg_handle h, int64_t* launches);
+
 /* Per-kernel hooks on one level, vectors in that level's natural numbering:
  *   op 0: y = A_l x                               (d_in0 = x,           d_out rows(l))
  *   op 1: xout = x + dinv o (b - A_l x)           (d_in0 = x, d_in1 = b, d_out rows(l))

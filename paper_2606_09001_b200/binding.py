@@ -25,7 +25,7 @@ EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_w
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
            "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
-           "amg_get_level_path", "amg_get_algorithmic_bytes", "amg_level_op", "amg_last_error"]
+           "amg_get_level_path", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error"]
 
 
 class amg_options(C.Structure):
@@ -223,6 +223,12 @@ def amg_get_level_path(h, level) -> int:
 def amg_get_algorithmic_bytes(h, which) -> float:
     v = C.c_double()
     _check(load_library().amg_get_algorithmic_bytes(h, C.c_int32(which), C.byref(v)), h)
+    return v.value
+
+
+def amg_get_last_launches(h) -> int:
+    v = C.c_int64()
+    _check(load_library().amg_get_last_launches(h, C.byref(v)), h)
     return v.value
 
 

@@ -324,6 +324,12 @@ amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes)
   return AMG_OK;
 }
 
+amg_status amg_get_last_launches(amg_handle h, int64_t* launches) {
+  if (!h || !launches) return AMG_ERR_INVALID_ARG;
+  *launches = h->last_launches;
+  return AMG_OK;
+}
+
 amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0, const double* d_in1,
                         double* d_out, int32_t reps, void* cuda_stream) {
   if (!h || level < 0 || level >= (int32_t)h->lv.size() || !d_out) return AMG_ERR_INVALID_ARG;

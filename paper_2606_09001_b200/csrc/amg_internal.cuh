@@ -98,6 +98,8 @@ struct amg_handle_s {
   unsigned* counter = nullptr;
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
   cudaGraphExec_t graph_exec[4] = {nullptr, nullptr, nullptr, nullptr};
+  int64_t graph_launches[4] = {0, 0, 0, 0};  // kernel nodes per replay
+  int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;  // graphs are captured here (the legacy stream cannot capture)
   int sm_count = 148;

@@ -8,6 +8,8 @@
 
 namespace {
 
+thread_local int64_t g_nlaunch = 0;  // kernel launches enqueued by this thread (amg_get_last_launches)
+
 constexpr int TPB = 256;
 inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
 
@@ -24,19 +26,19 @@ template <int OP, int NDOT>
 void launch_row(const Level& L, const RowArgs& a, cudaStream_t st) {
   if (L.fast) {
     if (L.stream_hint)
-      k_rowblock<OP, NDOT, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      ++g_nlaunch, k_rowblock<OP, NDOT, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
     else
-      k_rowblock<OP, NDOT, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      ++g_nlaunch, k_rowblock<OP, NDOT, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
   } else {
     const int64_t threads = (int64_t)L.n * L.lpr;
     int g = div_up(threads, RB_THREADS);
     if (NDOT > 0 && g > 4096) g = 4096;  // bounded partials; the kernel strides over rows
     if (g < 1) g = 1;
     switch (L.lpr) {
-      case 4: k_rowvec<OP, NDOT, 4><<<g, RB_THREADS, 0, st>>>(a); break;
-      case 8: k_rowvec<OP, NDOT, 8><<<g, RB_THREADS, 0, st>>>(a); break;
-      case 16: k_rowvec<OP, NDOT, 16><<<g, RB_THREADS, 0, st>>>(a); break;
-      default: k_rowvec<OP, NDOT, 32><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 4: ++g_nlaunch; k_rowvec<OP, NDOT, 4><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 8: ++g_nlaunch; k_rowvec<OP, NDOT, 8><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 16: ++g_nlaunch; k_rowvec<OP, NDOT, 16><<<g, RB_THREADS, 0, st>>>(a); break;
+      default: ++g_nlaunch; k_rowvec<OP, NDOT, 32><<<g, RB_THREADS, 0, st>>>(a); break;
     }
   }
 }
@@ -118,20 +120,20 @@ void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, cons
   if (L.fast) {
     a.out = rc;
     if (L.stream_hint)
-      k_rowblock<OP_RESTRICT, 0, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      ++g_nlaunch, k_rowblock<OP_RESTRICT, 0, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
     else
-      k_rowblock<OP_RESTRICT, 0, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      ++g_nlaunch, k_rowblock<OP_RESTRICT, 0, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
   } else {
     a.out = L.rtmp;
     launch_row<OP_RESID, 0>(L, a, st);
-    k_restrict_rows<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
+    ++g_nlaunch, k_restrict_rows<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
   }
 }
 
 void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl, cudaStream_t st) {
   const int n = H->nL;
   int T = n <= 32 ? 32 : (n <= 64 ? 64 : (n <= 256 ? 256 : 1024));
-  k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
+  ++g_nlaunch, k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
 }
 
 }  // namespace
@@ -148,7 +150,7 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     op_coarse_solve(H, b, L.x, ctl, st);
     *x_out = L.x;
     if (fuse_rz && l == 0)
-      k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
+      ++g_nlaunch, k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
     AMG_CUDA_TRY(H, cudaGetLastError());
     return AMG_OK;
   }
@@ -160,10 +162,10 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     op_jacobi0(H, L, b, cur, ctl, st);
     done_sweeps = 2;
   } else if (nu1 == 1) {
-    k_scale_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.dinv, b, cur, ctl);
+    ++g_nlaunch, k_scale_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.dinv, b, cur, ctl);
     done_sweeps = 1;
   } else {
-    k_zero<<<grid_for(L.n), TPB, 0, st>>>(L.n, cur, ctl);
+    ++g_nlaunch, k_zero<<<grid_for(L.n), TPB, 0, st>>>(L.n, cur, ctl);
   }
   for (int s = done_sweeps; s < nu1; ++s) {
     op_jacobi(H, L, b, cur, oth, false, ctl, st);
@@ -182,9 +184,9 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       std::swap(cur, oth);
     }
   } else {
-    k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
+    ++g_nlaunch, k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
     std::swap(cur, oth);
-    if (want_dot) k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
+    if (want_dot) ++g_nlaunch, k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
   }
   *x_out = cur;
   AMG_CUDA_TRY(H, cudaGetLastError());
@@ -207,14 +209,14 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *q = H->kv[3];
   op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
-  k_pcg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, p, q, x, r, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, k_pcg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, p, q, x, r, H->partials, H->counter, H->ctl);
   double* z = r;
   if (precond) {
     AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
   } else {
-    k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+    ++g_nlaunch, k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
   }
-  k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+  ++g_nlaunch, k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -224,7 +226,7 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4], *s = H->kv[5],
          *t = H->kv[6], *ph = H->kv[7];
-  k_bicg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, p, H->ctl);
+  ++g_nlaunch, k_bicg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, p, H->ctl);
   double* phat = p;
   if (precond) {
     double* zz = nullptr;
@@ -234,11 +236,11 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
     phat = ph;
   }
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
-  k_bicg_s<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, s, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, k_bicg_s<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, s, H->partials, H->counter, H->ctl);
   double* shat = s;
   if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st));
   op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
-  k_bicg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
+  ++g_nlaunch, k_bicg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
                                                    H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
@@ -258,7 +260,10 @@ amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStr
   (void)st;
   if (!H->cap_stream) AMG_CUDA_TRY(H, cudaStreamCreateWithFlags(&H->cap_stream, cudaStreamNonBlocking));
   AMG_CUDA_TRY(H, cudaStreamBeginCapture(H->cap_stream, cudaStreamCaptureModeThreadLocal));
+  const int64_t launches0 = g_nlaunch;
   amg_status s = enqueue_iteration(H, krylov, precond, H->cap_stream);
+  H->graph_launches[slot] = g_nlaunch - launches0;  // kernel nodes of one replay
+  g_nlaunch = launches0;                            // capturing enqueues nothing
   cudaError_t e = cudaStreamEndCapture(H->cap_stream, &g);
   if (s != AMG_OK) {
     if (g) cudaGraphDestroy(g);
@@ -293,6 +298,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   Level& L0 = H->lv[0];
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4];
+  const int64_t launches0 = g_nlaunch;
   // loop control: rtol / maxit go to the device once
   KrylovCtl init;
   memset(&init, 0, sizeof(init));
@@ -302,17 +308,17 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   H->h_ctl[5] = init;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
   if (krylov == 0) {
-    k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
+    ++g_nlaunch, k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
                                                          H->counter, H->ctl, FIN_INIT_PCG);
     double* z = r;
     if (precond) {
       AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
     } else {
-      k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+      ++g_nlaunch, k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
     }
-    k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+    ++g_nlaunch, k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
   } else {
-    k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
+    ++g_nlaunch, k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
                                                          H->ctl, FIN_INIT_BICG);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
@@ -324,9 +330,10 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   // enqueued after convergence return at their first instruction.
   constexpr int NSLOT = 4, LAG = 2;
   for (int it = 0; it < maxit; ++it) {
-    if (gexec)
+    if (gexec) {
       AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
-    else
+      g_nlaunch += H->graph_launches[krylov * 2 + precond];
+    } else
       AMG_TRY(enqueue_iteration(H, krylov, precond, st));
     const int slot = it % NSLOT;
     AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[slot], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
@@ -339,10 +346,11 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   }
   const bool half = (krylov == 1);
   const double* phat = half ? (precond ? H->kv[7] : p) : nullptr;
-  k_krylov_output<<<grid_for(n), TPB, 0, st>>>(n, x, phat, L0.inv, d_x, H->ctl);
+  ++g_nlaunch, k_krylov_output<<<grid_for(n), TPB, 0, st>>>(n, x, phat, L0.inv, d_x, H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  H->last_launches = g_nlaunch - launches0;
   if (info) {
     const KrylovCtl& c = H->h_ctl[4];
     info->iterations = c.iter;
@@ -362,6 +370,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
   const int Lc = (int)H->lv.size() - 1;
   Level& L = H->lv[level];
   if (reps < 1) reps = 1;
+  const int64_t launches0 = g_nlaunch;
   double *t0 = H->io_tmp, *t1 = H->io_tmp2, *t2 = H->io_tmp3;
   const bool needs_coarse = (op >= 1 && op <= 4);
   if (needs_coarse && level >= Lc) {
@@ -369,10 +378,10 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
     return AMG_ERR_INVALID_ARG;
   }
   auto perm_in = [&](const Level& Lv, const double* nat, double* out) {
-    k_permute_in<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, nat, Lv.inv, out);
+    ++g_nlaunch, k_permute_in<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, nat, Lv.inv, out);
   };
   auto perm_out = [&](const Level& Lv, const double* in, double* nat) {
-    k_permute_out<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, in, Lv.inv, nat);
+    ++g_nlaunch, k_permute_out<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, in, Lv.inv, nat);
   };
   switch (op) {
     case 0:
@@ -402,7 +411,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       perm_in(L, d_in0, t0);
       perm_in(C, d_in1, t1);
       for (int r = 0; r < reps; ++r)
-        k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
+        ++g_nlaunch, k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
       perm_out(L, t2, d_out);
     } break;
     case 4:
@@ -424,6 +433,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  H->last_launches = g_nlaunch - launches0;
   return AMG_OK;
 }
 
@@ -436,15 +446,16 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
   const double mean = n > 0 ? (double)H->nnz / n : 1.0;
   if (mean <= 12.0) {
     const int64_t threads = (int64_t)n * 8;
-    k_grad_values<8><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+    ++g_nlaunch, k_grad_values<8><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
                                                           d_gA, accumulate);
   } else {
     const int64_t threads = (int64_t)n * 32;
-    k_grad_values<32><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+    ++g_nlaunch, k_grad_values<32><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
                                                            d_gA, accumulate);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  H->last_launches = 1;
   return AMG_OK;
 }
 
