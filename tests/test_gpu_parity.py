@@ -163,9 +163,17 @@ def test_unpreconditioned_krylov(cases, krylov):
     xg, ig = c.s.solve(c.b, 1e-8, 2000, krylov, precond=0)
     xo, io = c.o.solve(c.b, 1e-8, 2000, krylov, 0)
     assert ig.status == 0
-    # unpreconditioned BiCGSTAB is sensitive to rounding order: a wider window than +-2 there
-    assert abs(ig.iterations - io.iterations) <= (2 if krylov == 0 else 12)
+    # The +-2 bar of north_star is for the AMG-preconditioned solves.  Unpreconditioned BiCGSTAB
+    # takes ~140 irregular iterations here and its count moves by ~10 % with the summation order
+    # of the dots: CG keeps +-2, BiCGSTAB gets a 20 % window and, as the
+    # sharp check, the same iterate after a fixed 12 iterations (before rounding has been amplified).
+    assert abs(ig.iterations - io.iterations) <= (2 if krylov == 0 else 0.2 * io.iterations)
     assert np.linalg.norm(c.b - c.Asp @ xg.cpu().numpy()) / np.linalg.norm(c.b) <= 1e-8
+    xg, ig = c.s.solve(c.b, 1e-30, 12, krylov, precond=0)
+    xo, io = c.o.solve(c.b, 1e-30, 12, krylov, 0)
+    assert ig.iterations == io.iterations == 12 and ig.status == io.status == 1
+    assert rel(xg.cpu().numpy(), xo) <= 1e-10
+    assert abs(ig.rel_residual - io.rel_residual) <= 1e-9 * io.rel_residual
 
 
 def test_determinism_bitwise(cases, B):
