@@ -426,9 +426,16 @@ def test_full_size_cfg3_against_oracle(full3, oracle_mod):
             xg = xg.cpu().numpy()
             assert ig.status == 0 and abs(ig.iterations - io.iterations) <= 2
             assert np.linalg.norm(b - Asp @ xg) / np.linalg.norm(b) <= 1e-8
-            # same algorithm, same hierarchy, same iteration: the iterates agree far below 1e-6
+            # same algorithm, same hierarchy, same iteration count: the two iterates differ only by
+            # rounding order (FMA, reduction trees), amplified by the recurrences over ~40 iterations
+            # (BiCGSTAB: 9e-9 measured at 128^3); far below the 1e-6 of north_star
             if ig.iterations == io.iterations:
-                assert rel(xg, xo) <= 1e-9
+                assert rel(xg, xo) <= 1e-7
+        # north_star: relative L2 error <= 1e-6 against the oracle's converged solution (A12: GPU at
+        # rtol_check 1e-11, oracle converged to 1e-13)
+        xg, ig = s.solve(b, 1e-11, 500, 0)
+        xo, io = o.solve(b, 1e-13, 500, 0, 1)
+        assert ig.status == 0 and rel(xg.cpu().numpy(), xo) <= 1e-6
         r = np.random.default_rng(1).standard_normal(A.n)
         assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
         o.close()
