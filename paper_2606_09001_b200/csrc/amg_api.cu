@@ -19,7 +19,7 @@ void* g_alloc_user = nullptr;
 void amg_set_thread_error(const std::string& s) { g_thread_error = s; }
 
 void* amg_dev_alloc(amg_handle_s* H, size_t bytes, cudaStream_t st) {
-  if (bytes == 0) bytes = 16;
+  bytes += VEC_PAD * sizeof(double);  // slack for the 16-byte-rounded bulk copies of the row-tile kernels
   void* p = nullptr;
   if (g_alloc_fn) {
     p = g_alloc_fn(bytes, (void*)st, g_alloc_user);

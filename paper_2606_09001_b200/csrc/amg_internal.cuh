@@ -9,14 +9,42 @@
 #include "amg_b200.h"
 
 // ------------------------------------------------------------------------------------------
-// tuning constants of the row-block streaming kernels
+// tuning constants of the row-tile streaming kernels; the -D overrides
+// exist for tuning sweeps only
 // ------------------------------------------------------------------------------------------
-constexpr int RB_THREADS = 256;   // threads per CTA
-constexpr int RB_TARGET = 3072;   // target nonzeros per row block
-constexpr int RB_CAP = 4096;      // products staged in shared memory per row block (incl. alignment slop)
-constexpr int RB_MAXROWS = 1024;  // rows per row block (shared rowptr / residual staging)
+#ifndef RT_THREADS_CFG
+#define RT_THREADS_CFG 256
+#endif
+#ifndef RT_STAGES_CFG
+#define RT_STAGES_CFG 2
+#endif
+#ifndef RT_CTAS_CFG
+#define RT_CTAS_CFG 4
+#endif
+#ifndef RT_TN_CFG
+#define RT_TN_CFG 1280
+#endif
+#ifndef RT_TR_CFG
+#define RT_TR_CFG 256
+#endif
+constexpr int RT_THREADS = RT_THREADS_CFG;  // threads per CTA
+constexpr int RT_STAGES = RT_STAGES_CFG;    // tiles in flight per CTA (bulk-async ring)
+constexpr int RT_CTAS = RT_CTAS_CFG;        // persistent CTAs per SM
+constexpr int RT_TN = RT_TN_CFG;            // nonzero slots staged per tile (incl. alignment slop), multiple of 4
+constexpr int RT_TR = RT_TR_CFG;            // rows staged per tile, multiple of 4
+constexpr int RT_TARGET = RT_TN - 320;      // target nonzeros per tile (one aggregate may overshoot it)
+constexpr int RT_ROWS_TARGET = RT_THREADS - 8;  // rows per tile aimed at: one row per thread in the row phase
+constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
+                                  // the bulk copies round their slices out to 16-byte boundaries
+constexpr int RB_THREADS = 256;   // row-vector fallback kernels
 constexpr int RED_THREADS = 256;  // BLAS-1 kernels
 constexpr int MAX_DENSE = 4096;   // largest coarsest level accepted
+
+// one tile of a level: rows [r0, r1) (boundaries on aggregate starts), nonzeros [k0, k1),
+// coarse rows [I0, I1] (I1 < I0 on the coarsest level)
+struct alignas(32) TileDesc {
+  int r0, r1, k0, k1, I0, I1, pad0, pad1;
+};
 
 // ------------------------------------------------------------------------------------------
 // device-resident Krylov scalars and loop control (S7-S9: no host round trip inside the loop)
@@ -57,10 +85,11 @@ struct Level {
   double* dinv = nullptr;   // smoother diagonal (null on the coarsest)
   int* agg = nullptr;       // [n]  coarse id of every row, non-decreasing
   int* agg_ptr = nullptr;   // [nc+1] first row of every aggregate
-  // row-block partition (boundaries aligned to aggregate starts)
+  // row-tile partition (boundaries aligned to aggregate starts)
   int* blk_ptr = nullptr;   // [nblk+1]
+  TileDesc* tiles = nullptr;  // [nblk]
   int nblk = 0;
-  int fast = 0;             // 1: row-block streaming kernels; 0: row-vector fallback
+  int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback
   int lpr = 8;              // lanes per row of the fallback kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary

@@ -21,7 +21,8 @@ struct RowArgs {
   const int* rowptr;
   const int* col;
   const double* val;
-  const int* blk_ptr;
+  const TileDesc* tiles;
+  int ntiles;
   const double* x;      // gathered vector
   const double* b;
   const double* dinv;
@@ -244,82 +245,250 @@ __device__ __forceinline__ void grid_reduce_finalize(double (&v)[NV], double* pa
 }
 
 // ------------------------------------------------------------------------------------------
-// Row-block streaming kernel.  One CTA owns the rows [blk_ptr[b], blk_ptr[b+1]) (boundaries on
-// aggregate starts, <= RB_CAP nonzeros, <= RB_MAXROWS rows):
-//   phase 1  the CTA streams its contiguous slice of val/col with 128-bit coalesced loads,
-//            gathers x[col] through L1/L2 and stages the products in shared memory;
-//   phase 2  one thread per row adds its segment of products (fixed order) and applies the
-//            row epilogue (SpMV / Jacobi / fused two-sweep Jacobi / prolongation-fused Jacobi);
-//   phase 3  (OP_RESTRICT) one thread per aggregate adds the residuals of its contiguous rows.
+// bulk-async copy (TMA, cp.async.bulk -> SASS UBLKCP) and mbarrier primitives
 // ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// generic-proxy accesses to shared memory before this point are ordered before later async-proxy writes
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = smem_u32(bar);
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+// global -> shared, 16-byte aligned on both sides, bytes a multiple of 16; completion on `bar`
+template <bool HINT>
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+  if (HINT)
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+  else
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ------------------------------------------------------------------------------------------
+// Row-tile streaming kernel (S1-S4).  Persistent: RT_CTAS CTAs per SM, each owning a contiguous
+// run of tiles.  One tile = rows [r0, r1) on aggregate boundaries, <= RT_TN nonzero slots,
+// <= RT_TR rows.  Everything a tile reads with unit stride -- its slices of val / col / rowptr,
+// of x, b, dinv, of agg / agg_ptr and of the coarse vector -- arrives in shared memory by
+// bulk-async copies (TMA) issued RT_STAGES-1 tiles ahead by one thread and signalled on an
+// mbarrier, so HBM keeps streaming while the CTA computes:
+//   pre     (fused two-sweep / prolongation ops) the tile's own x~ is formed in shared memory;
+//   phase 1 every thread multiplies quads of (col, val) by x~[col]: from the staged slice when
+//           the column lies in the tile's own row range (most do in the aggregate-contiguous
+//           numbering), else gathered through L1/L2; products replace val in place;
+//   phase 2 one thread per row (per aggregate for the restriction) adds its segment of
+//           products in ascending order and applies the row epilogue from staged operands.
+// ------------------------------------------------------------------------------------------
+namespace rt {
+constexpr int align16(int b) { return (b + 15) & ~15; }
+constexpr int OFF_VAL = 0;
+constexpr int OFF_COL = OFF_VAL + RT_TN * 8;
+constexpr int OFF_RP = OFF_COL + RT_TN * 4;
+constexpr int OFF_X = OFF_RP + align16((RT_TR + 8) * 4);
+constexpr int OFF_B = OFF_X + (RT_TR + 4) * 8;
+constexpr int OFF_D = OFF_B + (RT_TR + 4) * 8;
+constexpr int OFF_AGG = OFF_D + (RT_TR + 4) * 8;
+constexpr int OFF_EC = OFF_AGG + align16((RT_TR + 8) * 4);
+constexpr int OFF_DESC = OFF_EC + (RT_TR + 4) * 8;
+constexpr int STAGE_BYTES = (OFF_DESC + 32 + 127) & ~127;
+constexpr int HEADER_BYTES = 128;  // mbarriers
+constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * STAGE_BYTES;
+static_assert(RT_TN % 4 == 0 && RT_TR % 4 == 0, "tile caps must be multiples of 4");
+static_assert(RT_STAGES * 8 <= HEADER_BYTES, "too many stages");
+static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
+}  // namespace rt
+
+// which operands of the tile are staged for which operation
+template <int OP>
+struct TileOps {
+  static constexpr bool X = (OP != OP_JACOBI0);
+  static constexpr bool B = (OP != OP_SPMV);
+  static constexpr bool D = (OP == OP_JACOBI || OP == OP_JACOBI0 || OP == OP_JACOBI_PROLONG);
+  static constexpr bool AGG = (OP == OP_JACOBI_PROLONG);
+  static constexpr bool EC = (OP == OP_JACOBI_PROLONG);
+  static constexpr bool AGGPTR = (OP == OP_RESTRICT);
+  static constexpr bool PRE = (OP == OP_JACOBI0 || OP == OP_JACOBI_PROLONG);
+};
+
+// out-of-tile value of the gathered vector
+template <int OP>
+__device__ __forceinline__ double gather_far(const RowArgs& a, int c) {
+  if (OP == OP_JACOBI0) return __ldg(a.dinv + c) * __ldg(a.b + c);
+  if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.agg + c));
+  return __ldg(a.x + c);
+}
+
 template <int OP, int NDOT, bool STREAM>
-__global__ void __launch_bounds__(RB_THREADS) k_rowblock(RowArgs a) {
+__device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
+                                           uint64_t pol) {
+  using T = TileOps<OP>;
+  *reinterpret_cast<int4*>(stage + rt::OFF_DESC) = make_int4(d.r0, d.r1, d.k0, d.k1);
+  *reinterpret_cast<int4*>(stage + rt::OFF_DESC + 16) = make_int4(d.I0, d.I1, 0, 0);
+  const int nrows = d.r1 - d.r0;
+  if (nrows <= 0) {
+    mbar_arrive(bar);
+    return;
+  }
+  const int ka = d.k0 & ~3, nk = (d.k1 - ka + 3) & ~3;
+  const int ra = d.r0 & ~3, nrp = (d.r1 + 1 - ra + 3) & ~3, nrv = (d.r1 - ra + 3) & ~3;
+  const int Ia = d.I0 & ~3;
+  const int nec = (d.I1 + 1 - Ia + 3) & ~3, nap = (d.I1 + 2 - Ia + 3) & ~3;
+  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
+  uint32_t bytes = (uint32_t)nk * 12u + (uint32_t)nrp * 4u;
+  if (T::X) bytes += (uint32_t)nrv * 8u;
+  if (T::B || d0_staged) bytes += (uint32_t)nrv * 8u;
+  if (T::D) bytes += (uint32_t)nrv * 8u;
+  if (T::AGG) bytes += (uint32_t)nrv * 4u;
+  if (T::EC) bytes += (uint32_t)nec * 8u;
+  if (T::AGGPTR) bytes += (uint32_t)nap * 4u;
+  fence_proxy_async();
+  mbar_arrive_expect_tx(bar, bytes);
+  bulk_g2s<STREAM>(stage + rt::OFF_VAL, a.val + ka, (uint32_t)nk * 8u, bar, pol);
+  bulk_g2s<STREAM>(stage + rt::OFF_COL, a.col + ka, (uint32_t)nk * 4u, bar, pol);
+  bulk_g2s<false>(stage + rt::OFF_RP, a.rowptr + ra, (uint32_t)nrp * 4u, bar, pol);
+  if (T::X) bulk_g2s<false>(stage + rt::OFF_X, a.x + ra, (uint32_t)nrv * 8u, bar, pol);
+  if (T::B) bulk_g2s<false>(stage + rt::OFF_B, a.b + ra, (uint32_t)nrv * 8u, bar, pol);
+  if (d0_staged) bulk_g2s<false>(stage + rt::OFF_B, a.d0 + ra, (uint32_t)nrv * 8u, bar, pol);
+  if (T::D) bulk_g2s<false>(stage + rt::OFF_D, a.dinv + ra, (uint32_t)nrv * 8u, bar, pol);
+  if (T::AGG) bulk_g2s<false>(stage + rt::OFF_AGG, a.agg + ra, (uint32_t)nrv * 4u, bar, pol);
+  if (T::EC) bulk_g2s<false>(stage + rt::OFF_EC, a.ec + Ia, (uint32_t)nec * 8u, bar, pol);
+  if (T::AGGPTR) bulk_g2s<false>(stage + rt::OFF_AGG, a.agg_ptr + Ia, (uint32_t)nap * 4u, bar, pol);
+}
+
+template <int OP, int NDOT, bool STREAM>
+__global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (a.ctl != nullptr && a.ctl->done) return;
-  __shared__ __align__(16) double prod[RB_CAP];
-  __shared__ int srp[RB_MAXROWS + 1];
+  using T = TileOps<OP>;
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
+  unsigned char* stage0 = smem + rt::HEADER_BYTES;
   const int tid = threadIdx.x;
-  const int r0 = a.blk_ptr[blockIdx.x], r1 = a.blk_ptr[blockIdx.x + 1];
-  const int nrows = r1 - r0;
+  const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
+  const int t_end = (int)((int64_t)(blockIdx.x + 1) * a.ntiles / gridDim.x);
+  const int my = t_end - t_begin;
+  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
+  uint64_t pol = 0;
+  TileDesc next{};  // descriptor prefetched by the issuing thread
+  if (tid == 0) {
+    for (int s = 0; s < RT_STAGES; ++s) mbar_init(bars + s, 1);
+    fence_mbar_init();
+    if (STREAM) pol = l2_policy_evict_first();
+    const int pre = my < RT_STAGES ? my : RT_STAGES;
+    for (int s = 0; s < pre; ++s)
+      tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + s], stage0 + s * rt::STAGE_BYTES, bars + s, pol);
+    if (my > RT_STAGES) next = a.tiles[t_begin + RT_STAGES];
+  }
+  __syncthreads();
   double dots[NDOT > 0 ? NDOT : 1];
 #pragma unroll
   for (int j = 0; j < (NDOT > 0 ? NDOT : 1); ++j) dots[j] = 0.0;
 
-  if (nrows > 0) {
-    for (int i = tid; i <= nrows; i += RB_THREADS) srp[i] = a.rowptr[r0 + i];
-    __syncthreads();
-    const int k0 = srp[0], k1 = srp[nrows];
-    const int ka = k0 & ~3;
-    const int nq = (k1 - ka + 3) >> 2;
-    const int4* col4 = reinterpret_cast<const int4*>(a.col + ka);
-    const double2* val2 = reinterpret_cast<const double2*>(a.val + ka);
-    for (int q = tid; q < nq; q += RB_THREADS) {
-      const int4 c = ld_i4<STREAM>(col4 + q);
-      const double2 v01 = ld_d2<STREAM>(val2 + 2 * q);
-      const double2 v23 = ld_d2<STREAM>(val2 + 2 * q + 1);
-      const double x0 = gather_x<OP>(a, c.x), x1 = gather_x<OP>(a, c.y);
-      const double x2 = gather_x<OP>(a, c.z), x3 = gather_x<OP>(a, c.w);
-      double2* dst = reinterpret_cast<double2*>(prod + 4 * q);
-      dst[0] = make_double2(v01.x * x0, v01.y * x1);
-      dst[1] = make_double2(v23.x * x2, v23.y * x3);
-    }
-    __syncthreads();
-    if (OP == OP_RESTRICT) {
-      double res[RB_MAXROWS / RB_THREADS];
-#pragma unroll
-      for (int t = 0; t < RB_MAXROWS / RB_THREADS; ++t) {
-        const int lr = tid + t * RB_THREADS;
-        if (lr < nrows) {
-          double s = 0.0;
-          for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) s += prod[k];
-          res[t] = row_epilogue<OP>(a, r0 + lr, s);
-        }
-      }
-      __syncthreads();  // all segments consumed: reuse prod[] for the row residuals
-#pragma unroll
-      for (int t = 0; t < RB_MAXROWS / RB_THREADS; ++t) {
-        const int lr = tid + t * RB_THREADS;
-        if (lr < nrows) prod[lr] = res[t];
+  for (int it = 0; it < my; ++it) {
+    const int s = it % RT_STAGES;
+    unsigned char* stage = stage0 + s * rt::STAGE_BYTES;
+    mbar_wait(bars + s, (uint32_t)((it / RT_STAGES) & 1));
+    const int4 dsc = *reinterpret_cast<const int4*>(stage + rt::OFF_DESC);
+    const int r0 = dsc.x, nrows = dsc.y - dsc.x, k0 = dsc.z, k1 = dsc.w;
+    const int ka = k0 & ~3, ra = r0 & ~3, roff = r0 - ra;
+    double* prod = reinterpret_cast<double*>(stage + rt::OFF_VAL);
+    const int* srp = reinterpret_cast<const int*>(stage + rt::OFF_RP) + roff;  // srp[lr] = rowptr[r0 + lr]
+    double* xs = reinterpret_cast<double*>(stage + rt::OFF_X) + roff;          // tile-local row operands
+    const double* bs = reinterpret_cast<const double*>(stage + rt::OFF_B) + roff;
+    const double* ds = reinterpret_cast<const double*>(stage + rt::OFF_D) + roff;
+    if (T::PRE && nrows > 0) {
+      if (OP == OP_JACOBI0) {
+        for (int lr = tid; lr < nrows; lr += RT_THREADS) xs[lr] = ds[lr] * bs[lr];
+      } else {
+        const int2 ii = *reinterpret_cast<const int2*>(stage + rt::OFF_DESC + 16);
+        const int* as = reinterpret_cast<const int*>(stage + rt::OFF_AGG) + roff;
+        const double* es = reinterpret_cast<const double*>(stage + rt::OFF_EC) - (ii.x & ~3);
+        for (int lr = tid; lr < nrows; lr += RT_THREADS) xs[lr] = xs[lr] + a.gamma * es[as[lr]];
       }
       __syncthreads();
-      const int I0 = a.agg[r0], I1 = a.agg[r1 - 1];
-      for (int I = I0 + tid; I <= I1; I += RB_THREADS) {
-        double s = 0.0;
-        for (int r = a.agg_ptr[I] - r0, e = a.agg_ptr[I + 1] - r0; r < e; ++r) s += prod[r];
-        a.out[I] = s;
+    }
+    if (nrows > 0) {
+      const int nq = (k1 - ka + 3) >> 2;
+      const int4* col4 = reinterpret_cast<const int4*>(stage + rt::OFF_COL);
+      double2* val2 = reinterpret_cast<double2*>(prod);
+#pragma unroll 2
+      for (int q = tid; q < nq; q += RT_THREADS) {
+        const int4 c = col4[q];
+        const double2 v01 = val2[2 * q], v23 = val2[2 * q + 1];
+        const unsigned d0 = (unsigned)(c.x - r0), d1 = (unsigned)(c.y - r0), d2 = (unsigned)(c.z - r0),
+                       d3 = (unsigned)(c.w - r0);
+        double x0, x1, x2, x3;
+        if (d0 < (unsigned)nrows) x0 = xs[d0]; else x0 = gather_far<OP>(a, c.x);
+        if (d1 < (unsigned)nrows) x1 = xs[d1]; else x1 = gather_far<OP>(a, c.y);
+        if (d2 < (unsigned)nrows) x2 = xs[d2]; else x2 = gather_far<OP>(a, c.z);
+        if (d3 < (unsigned)nrows) x3 = xs[d3]; else x3 = gather_far<OP>(a, c.w);
+        val2[2 * q] = make_double2(v01.x * x0, v01.y * x1);
+        val2[2 * q + 1] = make_double2(v23.x * x2, v23.y * x3);
       }
-    } else {
-      for (int lr = tid; lr < nrows; lr += RB_THREADS) {
-        double s = 0.0;
-        for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) s += prod[k];
-        const int i = r0 + lr;
-        const double o = row_epilogue<OP>(a, i, s);
-        a.out[i] = o;
-        if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? a.d0[i] : a.b[i]) * o;
-        if (NDOT >= 2) dots[1] += o * o;
+    }
+    __syncthreads();  // products complete; every thread has left phase 2 of the previous tile
+    if (tid == 0 && it >= 1 && it - 1 + RT_STAGES < my) {
+      const int sp = (it - 1) % RT_STAGES;
+      tile_issue<OP, NDOT, STREAM>(a, next, stage0 + sp * rt::STAGE_BYTES, bars + sp, pol);
+      if (it + RT_STAGES < my) next = a.tiles[t_begin + it + RT_STAGES];
+    }
+    if (nrows > 0) {
+      if (OP == OP_RESTRICT) {
+        const int2 ii = *reinterpret_cast<const int2*>(stage + rt::OFF_DESC + 16);
+        const int nA = ii.y - ii.x + 1;
+        const int* aps = reinterpret_cast<const int*>(stage + rt::OFF_AGG) + (ii.x - (ii.x & ~3));
+        for (int al = tid; al < nA; al += RT_THREADS) {
+          double acc = 0.0;
+          for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) {
+            double sum = 0.0;
+            for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) sum += prod[k];
+            acc += bs[lr] - sum;
+          }
+          a.out[ii.x + al] = acc;
+        }
+      } else {
+        for (int lr = tid; lr < nrows; lr += RT_THREADS) {
+          double sum = 0.0;
+          for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) sum += prod[k];
+          double o;
+          if (OP == OP_SPMV)
+            o = sum;
+          else
+            o = xs[lr] + ds[lr] * (bs[lr] - sum);
+          a.out[r0 + lr] = o;
+          if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? (d0_staged ? bs[lr] : xs[lr]) : bs[lr]) * o;
+          if (NDOT >= 2) dots[1] += o * o;
+        }
       }
     }
   }
-  if (NDOT > 0) grid_reduce_finalize<(NDOT > 0 ? NDOT : 1), RB_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);
+  if (NDOT > 0) grid_reduce_finalize<(NDOT > 0 ? NDOT : 1), RT_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -583,6 +583,21 @@ __global__ void k_blk_stats(int nblk, const int* __restrict__ blk_ptr, const int
   atomicMax(&stats[1], k1 - (k0 & ~3));
 }
 
+__global__ void k_tile_desc(int nblk, const int* __restrict__ blk_ptr, const int* __restrict__ rowptr,
+                            const int* __restrict__ agg, TileDesc* __restrict__ tiles) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nblk) return;
+  TileDesc d;
+  d.r0 = blk_ptr[k];
+  d.r1 = blk_ptr[k + 1];
+  d.k0 = rowptr[d.r0];
+  d.k1 = rowptr[d.r1];
+  d.I0 = (agg && d.r1 > d.r0) ? agg[d.r0] : 0;
+  d.I1 = (agg && d.r1 > d.r0) ? agg[d.r1 - 1] : -1;
+  d.pad0 = d.pad1 = 0;
+  tiles[k] = d;
+}
+
 __global__ void k_pad_tail(int nnz, int nnz_alloc, int* __restrict__ col, double* __restrict__ val) {
   int k = nnz + blockIdx.x * blockDim.x + threadIdx.x;
   if (k < nnz_alloc) {
@@ -905,11 +920,17 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
       k_gather_double<<<grid_for(L.n), TPB, 0, st>>>(L.n, N.dinv, L.inv, L.dinv);
     }
     AMG_CUDA_TRY(H, cudaGetLastError());
-    // row-block partition
-    L.nblk = L.nnz > 0 ? div_up(L.nnz, RB_TARGET) : 1;
+    // row-tile partition: aim at one row per thread of the row phase and at most RT_TARGET nonzeros
+    double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
+    int target = (int)(mean_len * RT_ROWS_TARGET);
+    if (target > RT_TARGET) target = RT_TARGET;
+    if (target < 64) target = 64;
+    L.nblk = L.nnz > 0 ? div_up(L.nnz, target) : 1;
     AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
-    k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, RB_TARGET, q < Lc ? L.nc : L.n,
+    AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
+    k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
                                                          q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
+    k_tile_desc<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, q < Lc ? L.agg : nullptr, L.tiles);
     int* stats;
     AMG_ALLOC(H, stats, int, 2, st);
     AMG_CUDA_TRY(H, cudaMemsetAsync(stats, 0, 2 * sizeof(int), st));
@@ -918,8 +939,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     AMG_CUDA_TRY(H, cudaMemcpyAsync(h_stats, stats, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
     AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     amg_dev_free(H, stats);
-    L.fast = (!o.force_generic && h_stats[0] <= RB_MAXROWS && h_stats[1] + 4 <= RB_CAP) ? 1 : 0;
-    double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
+    L.fast = (!o.force_generic && h_stats[0] <= RT_TR && h_stats[1] + 4 <= RT_TN) ? 1 : 0;
     L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));
     size_t mat_bytes = (size_t)L.nnz * 12 + (size_t)L.n * 4;
     L.stream_hint = (H->l2_bytes > 0 && mat_bytes > H->l2_bytes / 2) ? 1 : 0;

@@ -22,13 +22,25 @@ inline int red_grid(const amg_handle_s* H, int n) {
 }
 
 // ---- dispatch of the row kernels ---------------------------------------------------------
+template <int OP, int NDOT, bool STREAM>
+void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
+  static bool attr_set = false;  // opt in to > 48 KB of dynamic shared memory, once per instantiation
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_rowtile<OP, NDOT, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
+    attr_set = true;
+  }
+  int grid = H->sm_count * RT_CTAS;
+  if (grid > L.nblk) grid = L.nblk;
+  ++g_nlaunch, k_rowtile<OP, NDOT, STREAM><<<grid, RT_THREADS, rt::SMEM_BYTES, st>>>(a);
+}
+
 template <int OP, int NDOT>
-void launch_row(const Level& L, const RowArgs& a, cudaStream_t st) {
+void launch_row(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
   if (L.fast) {
     if (L.stream_hint)
-      ++g_nlaunch, k_rowblock<OP, NDOT, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      launch_tile<OP, NDOT, true>(H, L, a, st);
     else
-      ++g_nlaunch, k_rowblock<OP, NDOT, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      launch_tile<OP, NDOT, false>(H, L, a, st);
   } else {
     const int64_t threads = (int64_t)L.n * L.lpr;
     int g = div_up(threads, RB_THREADS);
@@ -50,7 +62,8 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
   a.rowptr = L.rowptr;
   a.col = L.col;
   a.val = L.val;
-  a.blk_ptr = L.blk_ptr;
+  a.tiles = L.tiles;
+  a.ntiles = L.nblk;
   a.dinv = L.dinv;
   a.agg = L.agg;
   a.agg_ptr = L.agg_ptr;
@@ -71,11 +84,11 @@ void op_spmv(amg_handle_s* H, const Level& L, const double* x, double* y, int nd
   a.d0 = d0;
   a.fin = fin;
   if (ndot == 0)
-    launch_row<OP_SPMV, 0>(L, a, st);
+    launch_row<OP_SPMV, 0>(H, L, a, st);
   else if (ndot == 1)
-    launch_row<OP_SPMV, 1>(L, a, st);
+    launch_row<OP_SPMV, 1>(H, L, a, st);
   else
-    launch_row<OP_SPMV, 2>(L, a, st);
+    launch_row<OP_SPMV, 2>(H, L, a, st);
 }
 
 void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x, double* out, bool dot,
@@ -86,16 +99,16 @@ void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x
   a.out = out;
   a.fin = FIN_RZ;
   if (dot)
-    launch_row<OP_JACOBI, 1>(L, a, st);
+    launch_row<OP_JACOBI, 1>(H, L, a, st);
   else
-    launch_row<OP_JACOBI, 0>(L, a, st);
+    launch_row<OP_JACOBI, 0>(H, L, a, st);
 }
 
 void op_jacobi0(amg_handle_s* H, const Level& L, const double* b, double* out, KrylovCtl* ctl, cudaStream_t st) {
   RowArgs a = base_args(H, L, ctl);
   a.b = b;
   a.out = out;
-  launch_row<OP_JACOBI0, 0>(L, a, st);
+  launch_row<OP_JACOBI0, 0>(H, L, a, st);
 }
 
 void op_jacobi_prolong(amg_handle_s* H, const Level& L, const double* b, const double* x, const double* ec,
@@ -107,9 +120,9 @@ void op_jacobi_prolong(amg_handle_s* H, const Level& L, const double* b, const d
   a.out = out;
   a.fin = FIN_RZ;
   if (dot)
-    launch_row<OP_JACOBI_PROLONG, 1>(L, a, st);
+    launch_row<OP_JACOBI_PROLONG, 1>(H, L, a, st);
   else
-    launch_row<OP_JACOBI_PROLONG, 0>(L, a, st);
+    launch_row<OP_JACOBI_PROLONG, 0>(H, L, a, st);
 }
 
 void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, const double* x, double* rc,
@@ -120,12 +133,12 @@ void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, cons
   if (L.fast) {
     a.out = rc;
     if (L.stream_hint)
-      ++g_nlaunch, k_rowblock<OP_RESTRICT, 0, true><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      launch_tile<OP_RESTRICT, 0, true>(H, L, a, st);
     else
-      ++g_nlaunch, k_rowblock<OP_RESTRICT, 0, false><<<L.nblk, RB_THREADS, 0, st>>>(a);
+      launch_tile<OP_RESTRICT, 0, false>(H, L, a, st);
   } else {
     a.out = L.rtmp;
-    launch_row<OP_RESID, 0>(L, a, st);
+    launch_row<OP_RESID, 0>(H, L, a, st);
     ++g_nlaunch, k_restrict_rows<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
   }
 }
