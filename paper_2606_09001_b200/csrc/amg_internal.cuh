@@ -33,7 +33,7 @@ constexpr int RT_CTAS = RT_CTAS_CFG;        // persistent CTAs per SM
 constexpr int RT_TN = RT_TN_CFG;            // nonzero slots staged per tile (incl. alignment slop), multiple of 4
 constexpr int RT_TR = RT_TR_CFG;            // rows staged per tile, multiple of 4
 constexpr int RT_TARGET = RT_TN - 320;      // target nonzeros per tile (one aggregate may overshoot it)
-constexpr int RT_ROWS_TARGET = RT_THREADS - 8;  // rows per tile aimed at: one row per thread in the row phase
+constexpr int RT_ROWS_TARGET = (RT_THREADS < RT_TR ? RT_THREADS : RT_TR) - 8;  // rows per tile aimed at: one row per thread in the row phase
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
                                   // the bulk copies round their slices out to 16-byte boundaries
 constexpr int RB_THREADS = 256;   // row-vector fallback kernels

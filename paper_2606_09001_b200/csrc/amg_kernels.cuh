@@ -590,6 +590,55 @@ __global__ void k_lu_solve(int n, const double* __restrict__ lu, const int* __re
   for (int i = tid; i < n; i += T) x[i] = y[i];
 }
 
+// n <= LU_SMALL_MAX: the factors (row pitch n+1: conflict-free column reads) and y sit in shared
+// memory and ONE warp runs both substitutions, lane i owning rows i, i+32, ...: no block-wide
+// barrier inside the 2n dependent steps.  `sm` holds n*(n+1) + n doubles.
+constexpr int LU_SMALL_MAX = 72;  // 72*73*8 + 72*8 bytes < 48 KB
+__device__ __forceinline__ void lu_solve_small_cta(int n, const double* __restrict__ lu, const int* __restrict__ piv,
+                                                   const double* b, double* x, double* sm) {
+  const int tid = threadIdx.x, T = blockDim.x, P = n + 1;
+  double* y = sm + (size_t)n * P;
+  for (int t = tid; t < n * n; t += T) sm[(t / n) * P + (t % n)] = __ldg(lu + t);
+  for (int i = tid; i < n; i += T) y[i] = __ldcg(b + i);
+  __syncthreads();
+  if (tid < 32) {
+    const int lane = tid;
+    if (lane == 0)
+      for (int k = 0; k < n; ++k) {
+        const int p = __ldg(piv + k);
+        if (p != k) {
+          const double t = y[k];
+          y[k] = y[p];
+          y[p] = t;
+        }
+      }
+    __syncwarp();
+    for (int k = 0; k < n - 1; ++k) {  // forward substitution, unit lower triangle
+      const double yk = y[k];
+      for (int i = lane; i < n; i += 32)
+        if (i > k) y[i] -= sm[i * P + k] * yk;
+      __syncwarp();
+    }
+    for (int i = n - 1; i >= 0; --i) {  // backward substitution
+      const double yi = y[i] / sm[i * P + i];
+      __syncwarp();
+      if (lane == 0) y[i] = yi;
+      for (int j = lane; j < i; j += 32) y[j] -= sm[j * P + i] * yi;
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  for (int i = tid; i < n; i += T) x[i] = y[i];
+}
+
+__global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __restrict__ lu,
+                                                        const int* __restrict__ piv, const double* __restrict__ b,
+                                                        double* __restrict__ x, const KrylovCtl* ctl) {
+  if (ctl != nullptr && ctl->done) return;
+  extern __shared__ double lu_sm[];
+  lu_solve_small_cta(n, lu, piv, b, x, lu_sm);
+}
+
 // ------------------------------------------------------------------------------------------
 // S7/S8: fused Krylov vector kernels (grid-stride, one pass each, scalars read from KrylovCtl)
 // ------------------------------------------------------------------------------------------

@@ -145,6 +145,11 @@ void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, cons
 
 void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl, cudaStream_t st) {
   const int n = H->nL;
+  if (n <= LU_SMALL_MAX) {
+    const size_t sm = sizeof(double) * ((size_t)n * (n + 1) + n);
+    ++g_nlaunch, k_lu_solve_small<<<1, 256, sm, st>>>(n, H->lu, H->piv, b, x, ctl);
+    return;
+  }
   int T = n <= 32 ? 32 : (n <= 64 ? 64 : (n <= 256 ? 256 : 1024));
   ++g_nlaunch, k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
 }
