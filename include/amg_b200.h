@@ -88,7 +88,9 @@ typedef struct {
   int32_t max_match_rounds; /* 0 = handshake rounds until the fix-point                                  */
   int32_t force_generic;    /* 1 = use the row-vector fallback kernels on every level (tests)            */
   int32_t use_graph;        /* 1 = replay one Krylov iteration as a CUDA graph (default), 0 = plain launches */
-  int32_t reserved0;
+  int32_t tail_max_rows;    /* levels with at most this many rows (and everything below them) run inside ONE
+                               persistent kernel per V-cycle (grid barriers instead of launches); default
+                               65536, 0 = off                                                            */
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */

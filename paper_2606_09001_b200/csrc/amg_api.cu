@@ -128,6 +128,7 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
     AMG_ALLOC(H, H->partials, double, 2 * (size_t)cap, st);
     AMG_ALLOC(H, H->counter, unsigned, 1, st);
     AMG_CUDA_TRY(H, cudaMemsetAsync(H->counter, 0, sizeof(unsigned), st));
+    AMG_TRY(amg_setup_tail(H, st));
     AMG_CUDA_TRY(H, cudaMemsetAsync(H->ctl, 0, sizeof(KrylovCtl), st));
     AMG_CUDA_TRY(H, cudaMallocHost((void**)&H->h_ctl, sizeof(KrylovCtl) * 8));
     for (auto& e : H->ev) AMG_CUDA_TRY(H, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -158,6 +159,7 @@ amg_status amg_options_default(amg_options* o) {
   o->max_match_rounds = 0;
   o->force_generic = 0;
   o->use_graph = 1;
+  o->tail_max_rows = 65536;
   o->omega = 2.0 / 3.0;
   o->strong_beta = 0.25;
   o->coarse_scale = 1.0;

@@ -125,6 +125,11 @@ struct amg_handle_s {
   double* partials = nullptr;     // [2 * partials_cap]
   int partials_cap = 0;
   unsigned* counter = nullptr;
+  // coarse tail of the V-cycle: levels >= tail_first run inside one persistent kernel (amg_tail.cuh)
+  int tail_first = -1;               // -1: off
+  int tail_grid = 0;
+  void* d_tail = nullptr;            // TailLevel[levels] on the device
+  unsigned long long* tail_bar = nullptr;
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
   cudaGraphExec_t graph_exec[4] = {nullptr, nullptr, nullptr, nullptr};
   int64_t graph_launches[4] = {0, 0, 0, 0};  // kernel nodes per replay
@@ -192,3 +197,4 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
                                 int64_t ld, double* d_gA, int accumulate, cudaStream_t st);
 double amg_algorithmic_bytes(amg_handle_s* H, int which);
 void amg_destroy_graphs(amg_handle_s* H);
+amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st);

@@ -5,6 +5,7 @@
 #include <cstring>
 
 #include "amg_kernels.cuh"
+#include "amg_tail.cuh"
 
 namespace {
 
@@ -154,7 +155,70 @@ void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl
   ++g_nlaunch, k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
 }
 
+// levels l..coarsest in one persistent kernel (amg_tail.cuh); returns the result buffer of level l
+double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin, cudaStream_t st) {
+  const int Lc = (int)H->lv.size() - 1;
+  TailArgs a;
+  memset(&a, 0, sizeof(a));
+  a.lv = (const TailLevel*)H->d_tail;
+  a.first = l;
+  a.last = Lc;
+  a.b_first = b;
+  a.nu1 = H->opt.pre_sweeps;
+  a.nu2 = H->opt.post_sweeps;
+  a.gamma = H->opt.coarse_scale;
+  a.nL = H->nL;
+  a.lu = H->lu;
+  a.piv = H->piv;
+  a.bar = H->tail_bar;
+  a.partials = H->partials;
+  a.ctl = ctl;
+  a.fin = fin;
+  ++g_nlaunch, k_vcycle_tail<<<H->tail_grid, TAIL_THREADS, tail_smem_bytes(H->nL), st>>>(a);
+  Level& L = H->lv[l];
+  if (l == Lc) return L.x;
+  return tail_result_in_x2(a.nu1, a.nu2) ? L.x2 : L.x;
+}
+
 }  // namespace
+
+amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
+  H->tail_first = -1;
+  const int nlev = (int)H->lv.size();
+  if (H->opt.tail_max_rows <= 0 || H->opt.force_generic || nlev > TAIL_MAX_LEVELS) return AMG_OK;
+  int first = nlev;
+  while (first > 0 && H->lv[first - 1].n <= H->opt.tail_max_rows) --first;
+  if (first >= nlev) return AMG_OK;
+  std::vector<TailLevel> h(nlev);
+  for (int l = 0; l < nlev; ++l) {
+    const Level& L = H->lv[l];
+    TailLevel& T = h[l];
+    T.n = L.n;
+    T.nc = L.nc;
+    T.nnz = L.nnz;
+    const double mean = L.n > 0 ? (double)L.nnz / L.n : 1.0;
+    T.lpr = mean <= 6.0 ? 4 : (mean <= 24.0 ? 8 : 16);
+    T.rowptr = L.rowptr;
+    T.col = L.col;
+    T.val = L.val;
+    T.dinv = L.dinv;
+    T.agg = L.agg;
+    T.agg_ptr = L.agg_ptr;
+    T.b = L.b;
+    T.x = L.x;
+    T.x2 = L.x2;
+  }
+  TailLevel* d;
+  AMG_ALLOC(H, d, TailLevel, nlev, st);
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(d, h.data(), sizeof(TailLevel) * nlev, cudaMemcpyHostToDevice, st));
+  AMG_ALLOC(H, H->tail_bar, unsigned long long, 32, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(H->tail_bar, 0, sizeof(unsigned long long) * 32, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));  // h goes out of scope
+  H->d_tail = d;
+  H->tail_grid = H->sm_count;  // one resident CTA per SM: the grid barrier needs co-residency
+  H->tail_first = first;
+  return AMG_OK;
+}
 
 // ------------------------------------------------------------------------------------------
 // S6: V-cycle from a zero guess.  *x_out points at the level's result buffer.
@@ -164,6 +228,11 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
                       cudaStream_t st) {
   const int Lc = (int)H->lv.size() - 1;
   Level& L = H->lv[l];
+  if (H->tail_first >= 0 && l >= H->tail_first) {
+    *x_out = op_tail(H, l, b, ctl, (fuse_rz && l == 0) ? FIN_RZ : FIN_NONE, st);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    return AMG_OK;
+  }
   if (l == Lc) {
     op_coarse_solve(H, b, L.x, ctl, st);
     *x_out = L.x;

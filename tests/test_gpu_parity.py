@@ -122,22 +122,51 @@ def test_level_kernels(cases, name, generic):
         assert rel(y, z) <= 1e-12
 
 
+# tail_max_rows: the levels at or below this size run inside the persistent coarse-tail kernel
+# (default 65536: almost every level of these small cases); 0 = one kernel per pass on every
+# level; 600 = a mixed cycle
+@pytest.mark.parametrize("tail", [65536, 0, 600])
 @pytest.mark.parametrize("name", list(CASES))
-def test_apply_preconditioner(cases, name):
-    c = cases(name)
+def test_apply_preconditioner(cases, name, tail):
+    c = cases(name, tail_max_rows=tail)
     r = np.random.default_rng(11).standard_normal(c.A.n)
     z = c.s.apply_preconditioner(r).cpu().numpy()
     assert rel(z, c.o.vcycle(r, 0)) <= 1e-12
 
 
+@pytest.mark.parametrize("sweeps", [(1, 1), (3, 2), (0, 1), (2, 0), (1, 3)])
+@pytest.mark.parametrize("tail", [65536, 0, 600])
+def test_vcycle_sweep_counts(cases, oracle_mod, B, sweeps, tail):
+    """V(nu1, nu2) for sweep counts other than the default (2, 2), every kernel family."""
+    nu1, nu2 = sweeps
+    A = inputs.config_matrix(3, 20)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, pre_sweeps=nu1, post_sweeps=nu2)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, pre_sweeps=nu1, post_sweeps=nu2, tail_max_rows=tail)
+    try:
+        r = np.random.default_rng(13).standard_normal(A.n)
+        z = s.apply_preconditioner(r).cpu().numpy()
+        assert rel(z, o.vcycle(r, 0)) <= 1e-12
+        b = inputs.config_rhs(3, A.n)
+        if nu1 == nu2:  # symmetric cycle: PCG applies
+            xg, ig = s.solve(b, 1e-8, 500, 0)
+            xo, io = o.solve(b, 1e-8, 500, 0, 1)
+            assert ig.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        xg, ig = s.solve(b, 1e-8, 500, 1)
+        assert ig.status == 0
+        assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+    finally:
+        s.close()
+        o.close()
+
+
 # ------------------------------------------------------------------------------------------
 # S6-S9: whole solves
 # ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("graph", [1, 0])
+@pytest.mark.parametrize("graph,tail", [(1, 65536), (0, 65536), (1, 0), (1, 600)])
 @pytest.mark.parametrize("krylov", [0, 1])
 @pytest.mark.parametrize("name", list(CASES))
-def test_solve_parity(cases, name, krylov, graph):
-    c = cases(name, use_graph=graph)
+def test_solve_parity(cases, name, krylov, graph, tail):
+    c = cases(name, use_graph=graph, tail_max_rows=tail)
     bn = np.linalg.norm(c.b)
     # timed tolerance: residual and iteration count
     xg, ig = c.s.solve(c.b, 1e-8, 1000, krylov)
