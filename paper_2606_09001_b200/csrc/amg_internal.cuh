@@ -12,28 +12,22 @@
 // tuning constants of the row-tile streaming kernels; the -D overrides
 // exist for tuning sweeps only
 // ------------------------------------------------------------------------------------------
-#ifndef RT_THREADS_CFG
-#define RT_THREADS_CFG 256
-#endif
 #ifndef RT_STAGES_CFG
-#define RT_STAGES_CFG 2
+#define RT_STAGES_CFG 3
 #endif
 #ifndef RT_CTAS_CFG
 #define RT_CTAS_CFG 4
 #endif
-#ifndef RT_TN_CFG
-#define RT_TN_CFG 1280
+#ifndef RT_STAGE_BYTES_CFG
+#define RT_STAGE_BYTES_CFG 16384
 #endif
-#ifndef RT_TR_CFG
-#define RT_TR_CFG 256
-#endif
-constexpr int RT_THREADS = RT_THREADS_CFG;  // threads per CTA
-constexpr int RT_STAGES = RT_STAGES_CFG;    // tiles in flight per CTA (bulk-async ring)
-constexpr int RT_CTAS = RT_CTAS_CFG;        // persistent CTAs per SM
-constexpr int RT_TN = RT_TN_CFG;            // nonzero slots staged per tile (incl. alignment slop), multiple of 4
-constexpr int RT_TR = RT_TR_CFG;            // rows staged per tile, multiple of 4
-constexpr int RT_TARGET = RT_TN - 320;      // target nonzeros per tile (one aggregate may overshoot it)
-constexpr int RT_ROWS_TARGET = (RT_THREADS < RT_TR ? RT_THREADS : RT_TR) - 8;  // rows per tile aimed at: one row per thread in the row phase
+constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA: one quad of nonzeros each per tile
+constexpr int RT_THREADS = RT_CONSUMERS + 32;      // + one producer warp (issues the bulk copies)
+constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA
+constexpr int RT_CTAS = RT_CTAS_CFG;               // persistent CTAs per SM
+constexpr int RT_STAGE_BYTES = RT_STAGE_BYTES_CFG; // shared memory of one ring stage (descriptor + operands of one tile)
+constexpr int RT_DESC_BYTES = 64;                  // stage header written by the producer
+constexpr int RT_MAX_SLOTS = RT_CONSUMERS * 4;     // nonzero slots of a tile (incl. alignment slop)
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
                                   // the bulk copies round their slices out to 16-byte boundaries
 constexpr int RB_THREADS = 256;   // row-vector fallback kernels
@@ -45,6 +39,36 @@ constexpr int MAX_DENSE = 4096;   // largest coarsest level accepted (SURVEY.md 
 struct alignas(32) TileDesc {
   int r0, r1, k0, k1, I0, I1, pad0, pad1;
 };
+
+// Placement of a tile's operands inside its ring stage (after the RT_DESC_BYTES header).  Every
+// slice is rounded out to 16-byte boundaries of the source array (bulk copies need 16-byte
+// aligned addresses and sizes), so every section is a multiple of 16 bytes.
+struct TileLayout {
+  int ka, nk;        // first staged nonzero slot (multiple of 4), slots staged
+  int ra, nrp, nrv;  // first staged row (multiple of 4), rowptr entries, row-vector entries
+  int Ia, nec, nap;  // first staged coarse row, coarse-vector entries, agg_ptr entries
+  int o_col, o_rp, o_x, o_b, o_d, o_agg, o_ec, end;  // byte offsets (val at 0)
+};
+__host__ __device__ inline TileLayout tile_layout(int r0, int r1, int k0, int k1, int I0, int I1) {
+  TileLayout t;
+  t.ka = k0 & ~3;
+  t.nk = (k1 - t.ka + 3) & ~3;
+  t.ra = r0 & ~3;
+  t.nrp = (r1 + 1 - t.ra + 3) & ~3;
+  t.nrv = (r1 - t.ra + 3) & ~3;
+  t.Ia = I0 & ~3;
+  t.nec = I1 >= I0 ? ((I1 + 1 - t.Ia + 3) & ~3) : 0;
+  t.nap = I1 >= I0 ? ((I1 + 2 - t.Ia + 3) & ~3) : 0;
+  t.o_col = 8 * t.nk;
+  t.o_rp = t.o_col + 4 * t.nk;
+  t.o_x = t.o_rp + 4 * t.nrp;
+  t.o_b = t.o_x + 8 * t.nrv;
+  t.o_d = t.o_b + 8 * t.nrv;
+  t.o_agg = t.o_d + 8 * t.nrv;
+  t.o_ec = t.o_agg + 4 * (t.nrv > t.nap ? t.nrv : t.nap);
+  t.end = t.o_ec + 8 * t.nec;
+  return t;
+}
 
 // ------------------------------------------------------------------------------------------
 // device-resident Krylov scalars and loop control (S7-S9: no host round trip inside the loop)
@@ -91,6 +115,7 @@ struct Level {
   int nblk = 0;
   int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback
   int lpr = 8;              // lanes per row of the fallback kernels
+  int lpr2 = 1;             // lanes per row of the row phase of the row-tile kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary
   int* nat_agg = nullptr;   // [n] aggregate ids in natural numbering of levels l, l+1

@@ -29,6 +29,7 @@ struct RowArgs {
   double* out;
   const int* agg;       // prolongation / restriction
   const int* agg_ptr;
+  int lpr2;             // lanes per row of the row phase (row-tile kernels)
   const double* ec;
   double gamma;
   const double* d0;     // second operand of the fused dot (SpMV)
@@ -293,37 +294,39 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // ------------------------------------------------------------------------------------------
-// Row-tile streaming kernel (S1-S4).  Persistent: RT_CTAS CTAs per SM, each owning a contiguous
-// run of tiles.  One tile = rows [r0, r1) on aggregate boundaries, <= RT_TN nonzero slots,
-// <= RT_TR rows.  Everything a tile reads with unit stride -- its slices of val / col / rowptr,
-// of x, b, dinv, of agg / agg_ptr and of the coarse vector -- arrives in shared memory by
-// bulk-async copies (TMA) issued RT_STAGES-1 tiles ahead by one thread and signalled on an
-// mbarrier, so HBM keeps streaming while the CTA computes:
-//   pre     (fused two-sweep / prolongation ops) the tile's own x~ is formed in shared memory;
-//   phase 1 every thread multiplies quads of (col, val) by x~[col]: from the staged slice when
-//           the column lies in the tile's own row range (most do in the aggregate-contiguous
-//           numbering), else gathered through L1/L2; products replace val in place;
-//   phase 2 one thread per row (per aggregate for the restriction) adds its segment of
-//           products in ascending order and applies the row epilogue from staged operands.
+// Row-tile streaming kernel (S1-S4).  Persistent and warp-specialised: RT_CTAS CTAs per SM, each
+// owning a contiguous run of tiles; 8 consumer warps + 1 producer warp per CTA.
+//
+// One tile = rows [r0, r1) on aggregate boundaries, at most RT_MAX_SLOTS nonzero slots and
+// RT_STAGE_BYTES of operands.  Everything a tile reads with unit stride -- its slices of val /
+// col / rowptr, of x, b, dinv, of agg / agg_ptr and of the coarse vector -- arrives in shared
+// memory by bulk-async copies (TMA) that the producer warp issues up to RT_STAGES tiles ahead,
+// throttled only by the consumers' "stage empty" mbarriers: HBM keeps streaming whatever the
+// consumers are doing.  The consumers read the stage and never write it: LPR2 lanes per row
+// (per aggregate for the restriction, whose rows and therefore nonzeros are consecutive) walk
+// the row's (col, val) pairs in shared memory; a column inside the tile's own row range (most,
+// in the aggregate-contiguous numbering) reads the staged x slice -- neighbouring lanes hold
+// neighbouring rows, so these reads are nearly contiguous -- the others are gathered through
+// L1/L2.  No product array, no CTA-wide barrier: a warp releases the stage when it is done and
+// may run ahead into the next tile.  (ncu on the earlier quad-per-thread variant showed the
+// shared-memory data pipe at 64-80 % of its peak: val/col read, products written and read back,
+// scattered x reads; the row walk needs ~2.5x fewer wavefronts per nonzero.)
 // ------------------------------------------------------------------------------------------
 namespace rt {
-constexpr int align16(int b) { return (b + 15) & ~15; }
-constexpr int OFF_VAL = 0;
-constexpr int OFF_COL = OFF_VAL + RT_TN * 8;
-constexpr int OFF_RP = OFF_COL + RT_TN * 4;
-constexpr int OFF_X = OFF_RP + align16((RT_TR + 8) * 4);
-constexpr int OFF_B = OFF_X + (RT_TR + 4) * 8;
-constexpr int OFF_D = OFF_B + (RT_TR + 4) * 8;
-constexpr int OFF_AGG = OFF_D + (RT_TR + 4) * 8;
-constexpr int OFF_EC = OFF_AGG + align16((RT_TR + 8) * 4);
-constexpr int OFF_DESC = OFF_EC + (RT_TR + 4) * 8;
-constexpr int STAGE_BYTES = (OFF_DESC + 32 + 127) & ~127;
-constexpr int HEADER_BYTES = 128;  // mbarriers
-constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * STAGE_BYTES;
-static_assert(RT_TN % 4 == 0 && RT_TR % 4 == 0, "tile caps must be multiples of 4");
-static_assert(RT_STAGES * 8 <= HEADER_BYTES, "too many stages");
+constexpr int HEADER_BYTES = 128;  // full[RT_STAGES], empty[RT_STAGES] mbarriers
+constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * RT_STAGE_BYTES;
+static_assert(RT_STAGES >= 2 && 2 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
+static_assert(RT_STAGE_BYTES % 128 == 0, "stage size must keep 128-byte alignment");
 static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
 }  // namespace rt
+
+struct StageDesc {  // RT_DESC_BYTES at the start of a stage, written by the producer
+  int r0, nrows, k0, k1;
+  int I0, I1, o_col, o_rp;
+  int o_x, o_b, o_d, o_agg;
+  int o_ec, ka, roff, ioff;  // roff = r0 - ra, ioff = I0 - Ia
+};
+static_assert(sizeof(StageDesc) == RT_DESC_BYTES, "stage header size");
 
 // which operands of the tile are staged for which operation
 template <int OP>
@@ -334,158 +337,180 @@ struct TileOps {
   static constexpr bool AGG = (OP == OP_JACOBI_PROLONG);
   static constexpr bool EC = (OP == OP_JACOBI_PROLONG);
   static constexpr bool AGGPTR = (OP == OP_RESTRICT);
-  static constexpr bool PRE = (OP == OP_JACOBI0 || OP == OP_JACOBI_PROLONG);
 };
 
-// out-of-tile value of the gathered vector
+template <int OP, int NDOT, bool STREAM>
+__device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
+                                           uint64_t pol) {
+  using T = TileOps<OP>;
+  const TileLayout t = tile_layout(d.r0, d.r1, d.k0, d.k1, d.I0, d.I1);
+  StageDesc sd;
+  sd.r0 = d.r0, sd.nrows = d.r1 - d.r0, sd.k0 = d.k0, sd.k1 = d.k1;
+  sd.I0 = d.I0, sd.I1 = d.I1, sd.o_col = t.o_col, sd.o_rp = t.o_rp;
+  sd.o_x = t.o_x, sd.o_b = t.o_b, sd.o_d = t.o_d, sd.o_agg = t.o_agg;
+  sd.o_ec = t.o_ec, sd.ka = t.ka, sd.roff = d.r0 - t.ra, sd.ioff = d.I0 - t.Ia;
+  int4* dst = reinterpret_cast<int4*>(stage);
+  const int4* src = reinterpret_cast<const int4*>(&sd);
+  dst[0] = src[0], dst[1] = src[1], dst[2] = src[2], dst[3] = src[3];
+  if (sd.nrows <= 0) {
+    mbar_arrive(bar);
+    return;
+  }
+  unsigned char* base = stage + RT_DESC_BYTES;
+  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
+  const uint32_t nk = (uint32_t)t.nk, nrp = (uint32_t)t.nrp, nrv = (uint32_t)t.nrv, nec = (uint32_t)t.nec,
+                 nap = (uint32_t)t.nap;
+  uint32_t bytes = nk * 12u + nrp * 4u;
+  if (T::X) bytes += nrv * 8u;
+  if (T::B || d0_staged) bytes += nrv * 8u;
+  if (T::D) bytes += nrv * 8u;
+  if (T::AGG) bytes += nrv * 4u;
+  if (T::EC) bytes += nec * 8u;
+  if (T::AGGPTR) bytes += nap * 4u;
+  mbar_arrive_expect_tx(bar, bytes);
+  bulk_g2s<STREAM>(base, a.val + t.ka, nk * 8u, bar, pol);
+  bulk_g2s<STREAM>(base + t.o_col, a.col + t.ka, nk * 4u, bar, pol);
+  bulk_g2s<false>(base + t.o_rp, a.rowptr + t.ra, nrp * 4u, bar, pol);
+  if (T::X) bulk_g2s<false>(base + t.o_x, a.x + t.ra, nrv * 8u, bar, pol);
+  if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra, nrv * 8u, bar, pol);
+  if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra, nrv * 8u, bar, pol);
+  if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra, nrv * 8u, bar, pol);
+  if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra, nrv * 4u, bar, pol);
+  if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia, nec * 8u, bar, pol);
+  if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia, nap * 4u, bar, pol);
+}
+
+// value of the gathered vector at column c: from the staged slices when c lies in the tile's own
+// row range, else through L1/L2
 template <int OP>
-__device__ __forceinline__ double gather_far(const RowArgs& a, int c) {
+__device__ __forceinline__ double tile_x(const RowArgs& a, int c, int r0, int nrows, const double* xs,
+                                         const double* bs, const double* ds, const int* as, const double* es) {
+  const unsigned dd = (unsigned)(c - r0);
+  if (dd < (unsigned)nrows) {
+    if (OP == OP_JACOBI0) return ds[dd] * bs[dd];
+    if (OP == OP_JACOBI_PROLONG) return xs[dd] + a.gamma * es[as[dd]];
+    return xs[dd];
+  }
   if (OP == OP_JACOBI0) return __ldg(a.dinv + c) * __ldg(a.b + c);
   if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.agg + c));
   return __ldg(a.x + c);
 }
 
 template <int OP, int NDOT, bool STREAM>
-__device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
-                                           uint64_t pol) {
-  using T = TileOps<OP>;
-  *reinterpret_cast<int4*>(stage + rt::OFF_DESC) = make_int4(d.r0, d.r1, d.k0, d.k1);
-  *reinterpret_cast<int4*>(stage + rt::OFF_DESC + 16) = make_int4(d.I0, d.I1, 0, 0);
-  const int nrows = d.r1 - d.r0;
-  if (nrows <= 0) {
-    mbar_arrive(bar);
-    return;
-  }
-  const int ka = d.k0 & ~3, nk = (d.k1 - ka + 3) & ~3;
-  const int ra = d.r0 & ~3, nrp = (d.r1 + 1 - ra + 3) & ~3, nrv = (d.r1 - ra + 3) & ~3;
-  const int Ia = d.I0 & ~3;
-  const int nec = (d.I1 + 1 - Ia + 3) & ~3, nap = (d.I1 + 2 - Ia + 3) & ~3;
-  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
-  uint32_t bytes = (uint32_t)nk * 12u + (uint32_t)nrp * 4u;
-  if (T::X) bytes += (uint32_t)nrv * 8u;
-  if (T::B || d0_staged) bytes += (uint32_t)nrv * 8u;
-  if (T::D) bytes += (uint32_t)nrv * 8u;
-  if (T::AGG) bytes += (uint32_t)nrv * 4u;
-  if (T::EC) bytes += (uint32_t)nec * 8u;
-  if (T::AGGPTR) bytes += (uint32_t)nap * 4u;
-  fence_proxy_async();
-  mbar_arrive_expect_tx(bar, bytes);
-  bulk_g2s<STREAM>(stage + rt::OFF_VAL, a.val + ka, (uint32_t)nk * 8u, bar, pol);
-  bulk_g2s<STREAM>(stage + rt::OFF_COL, a.col + ka, (uint32_t)nk * 4u, bar, pol);
-  bulk_g2s<false>(stage + rt::OFF_RP, a.rowptr + ra, (uint32_t)nrp * 4u, bar, pol);
-  if (T::X) bulk_g2s<false>(stage + rt::OFF_X, a.x + ra, (uint32_t)nrv * 8u, bar, pol);
-  if (T::B) bulk_g2s<false>(stage + rt::OFF_B, a.b + ra, (uint32_t)nrv * 8u, bar, pol);
-  if (d0_staged) bulk_g2s<false>(stage + rt::OFF_B, a.d0 + ra, (uint32_t)nrv * 8u, bar, pol);
-  if (T::D) bulk_g2s<false>(stage + rt::OFF_D, a.dinv + ra, (uint32_t)nrv * 8u, bar, pol);
-  if (T::AGG) bulk_g2s<false>(stage + rt::OFF_AGG, a.agg + ra, (uint32_t)nrv * 4u, bar, pol);
-  if (T::EC) bulk_g2s<false>(stage + rt::OFF_EC, a.ec + Ia, (uint32_t)nec * 8u, bar, pol);
-  if (T::AGGPTR) bulk_g2s<false>(stage + rt::OFF_AGG, a.agg_ptr + Ia, (uint32_t)nap * 4u, bar, pol);
-}
-
-template <int OP, int NDOT, bool STREAM>
 __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (a.ctl != nullptr && a.ctl->done) return;
-  using T = TileOps<OP>;
   extern __shared__ __align__(128) unsigned char smem[];
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty = full + RT_STAGES;
   unsigned char* stage0 = smem + rt::HEADER_BYTES;
   const int tid = threadIdx.x;
   const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
   const int t_end = (int)((int64_t)(blockIdx.x + 1) * a.ntiles / gridDim.x);
   const int my = t_end - t_begin;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
-  uint64_t pol = 0;
-  TileDesc next{};  // descriptor prefetched by the issuing thread
   if (tid == 0) {
-    for (int s = 0; s < RT_STAGES; ++s) mbar_init(bars + s, 1);
+    for (int s = 0; s < RT_STAGES; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, RT_CONSUMERS / 32);
+    }
     fence_mbar_init();
-    if (STREAM) pol = l2_policy_evict_first();
-    const int pre = my < RT_STAGES ? my : RT_STAGES;
-    for (int s = 0; s < pre; ++s)
-      tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + s], stage0 + s * rt::STAGE_BYTES, bars + s, pol);
-    if (my > RT_STAGES) next = a.tiles[t_begin + RT_STAGES];
   }
   __syncthreads();
   double dots[NDOT > 0 ? NDOT : 1];
 #pragma unroll
   for (int j = 0; j < (NDOT > 0 ? NDOT : 1); ++j) dots[j] = 0.0;
 
-  for (int it = 0; it < my; ++it) {
-    const int s = it % RT_STAGES;
-    unsigned char* stage = stage0 + s * rt::STAGE_BYTES;
-    mbar_wait(bars + s, (uint32_t)((it / RT_STAGES) & 1));
-    const int4 dsc = *reinterpret_cast<const int4*>(stage + rt::OFF_DESC);
-    const int r0 = dsc.x, nrows = dsc.y - dsc.x, k0 = dsc.z, k1 = dsc.w;
-    const int ka = k0 & ~3, ra = r0 & ~3, roff = r0 - ra;
-    double* prod = reinterpret_cast<double*>(stage + rt::OFF_VAL);
-    const int* srp = reinterpret_cast<const int*>(stage + rt::OFF_RP) + roff;  // srp[lr] = rowptr[r0 + lr]
-    double* xs = reinterpret_cast<double*>(stage + rt::OFF_X) + roff;          // tile-local row operands
-    const double* bs = reinterpret_cast<const double*>(stage + rt::OFF_B) + roff;
-    const double* ds = reinterpret_cast<const double*>(stage + rt::OFF_D) + roff;
-    if (T::PRE && nrows > 0) {
-      if (OP == OP_JACOBI0) {
-        for (int lr = tid; lr < nrows; lr += RT_THREADS) xs[lr] = ds[lr] * bs[lr];
-      } else {
-        const int2 ii = *reinterpret_cast<const int2*>(stage + rt::OFF_DESC + 16);
-        const int* as = reinterpret_cast<const int*>(stage + rt::OFF_AGG) + roff;
-        const double* es = reinterpret_cast<const double*>(stage + rt::OFF_EC) - (ii.x & ~3);
-        for (int lr = tid; lr < nrows; lr += RT_THREADS) xs[lr] = xs[lr] + a.gamma * es[as[lr]];
-      }
-      __syncthreads();
-    }
-    if (nrows > 0) {
-      const int nq = (k1 - ka + 3) >> 2;
-      const int4* col4 = reinterpret_cast<const int4*>(stage + rt::OFF_COL);
-      double2* val2 = reinterpret_cast<double2*>(prod);
-#pragma unroll 2
-      for (int q = tid; q < nq; q += RT_THREADS) {
-        const int4 c = col4[q];
-        const double2 v01 = val2[2 * q], v23 = val2[2 * q + 1];
-        const unsigned d0 = (unsigned)(c.x - r0), d1 = (unsigned)(c.y - r0), d2 = (unsigned)(c.z - r0),
-                       d3 = (unsigned)(c.w - r0);
-        double x0, x1, x2, x3;
-        if (d0 < (unsigned)nrows) x0 = xs[d0]; else x0 = gather_far<OP>(a, c.x);
-        if (d1 < (unsigned)nrows) x1 = xs[d1]; else x1 = gather_far<OP>(a, c.y);
-        if (d2 < (unsigned)nrows) x2 = xs[d2]; else x2 = gather_far<OP>(a, c.z);
-        if (d3 < (unsigned)nrows) x3 = xs[d3]; else x3 = gather_far<OP>(a, c.w);
-        val2[2 * q] = make_double2(v01.x * x0, v01.y * x1);
-        val2[2 * q + 1] = make_double2(v23.x * x2, v23.y * x3);
+  if (tid >= RT_CONSUMERS) {
+    // ---------------- producer warp ----------------
+    if (tid == RT_CONSUMERS && my > 0) {
+      const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
+      TileDesc d = a.tiles[t_begin];
+      for (int it = 0; it < my; ++it) {
+        const int s = it % RT_STAGES;
+        TileDesc dn = d;
+        if (it + 1 < my) dn = a.tiles[t_begin + it + 1];
+        if (it >= RT_STAGES) mbar_wait(empty + s, (uint32_t)(((it / RT_STAGES) - 1) & 1));
+        tile_issue<OP, NDOT, STREAM>(a, d, stage0 + s * RT_STAGE_BYTES, full + s, pol);
+        d = dn;
       }
     }
-    __syncthreads();  // products complete; every thread has left phase 2 of the previous tile
-    if (tid == 0 && it >= 1 && it - 1 + RT_STAGES < my) {
-      const int sp = (it - 1) % RT_STAGES;
-      tile_issue<OP, NDOT, STREAM>(a, next, stage0 + sp * rt::STAGE_BYTES, bars + sp, pol);
-      if (it + RT_STAGES < my) next = a.tiles[t_begin + it + RT_STAGES];
-    }
-    if (nrows > 0) {
-      if (OP == OP_RESTRICT) {
-        const int2 ii = *reinterpret_cast<const int2*>(stage + rt::OFF_DESC + 16);
-        const int nA = ii.y - ii.x + 1;
-        const int* aps = reinterpret_cast<const int*>(stage + rt::OFF_AGG) + (ii.x - (ii.x & ~3));
-        for (int al = tid; al < nA; al += RT_THREADS) {
-          double acc = 0.0;
-          for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) {
+  } else {
+    // ---------------- consumers ----------------
+    // No CTA-wide barrier: every warp walks its own units (rows, or aggregates for the
+    // restriction) of a tile and releases the stage when it is done with it.
+    const int lane = tid & 31;
+    const int lpr = (OP == OP_RESTRICT) ? a.lpr2 * 2 : a.lpr2;  // lanes per unit
+    const int lsh = 31 - __clz(lpr);
+    for (int it = 0; it < my; ++it) {
+      const int s = it % RT_STAGES;
+      unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
+      mbar_wait(full + s, (uint32_t)((it / RT_STAGES) & 1));
+      const StageDesc sd = *reinterpret_cast<const StageDesc*>(stage);
+      unsigned char* base = stage + RT_DESC_BYTES;
+      const int r0 = sd.r0, nrows = sd.nrows, ka = sd.ka;
+      const double* sval = reinterpret_cast<const double*>(base) - ka;            // sval[k] = val[k]
+      const int* scol = reinterpret_cast<const int*>(base + sd.o_col) - ka;       // scol[k] = col[k]
+      const int* srp = reinterpret_cast<const int*>(base + sd.o_rp) + sd.roff;    // srp[lr] = rowptr[r0 + lr]
+      const double* xs = reinterpret_cast<const double*>(base + sd.o_x) + sd.roff;  // tile-local row operands
+      const double* bs = reinterpret_cast<const double*>(base + sd.o_b) + sd.roff;
+      const double* ds = reinterpret_cast<const double*>(base + sd.o_d) + sd.roff;
+      const int* as = reinterpret_cast<const int*>(base + sd.o_agg) + sd.roff;    // as[lr] = agg[r0 + lr]
+      const double* es = reinterpret_cast<const double*>(base + sd.o_ec) - (sd.I0 - sd.ioff);  // es[I] = ec[I]
+      if (nrows > 0) {
+        if (OP == OP_RESTRICT) {
+          const int nA = sd.I1 - sd.I0 + 1;
+          const int* aps = reinterpret_cast<const int*>(base + sd.o_agg) + sd.ioff;  // aps[al] = agg_ptr[I0 + al]
+          const int nunits = nA << lsh;
+          for (int ubase = 0; ubase < nunits; ubase += RT_CONSUMERS) {
+            const int u = ubase + tid;
+            const int al = u >> lsh, sub = u & (lpr - 1);
             double sum = 0.0;
-            for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) sum += prod[k];
-            acc += bs[lr] - sum;
+            if (al < nA) {
+              const int la = aps[al] - r0, lb = aps[al + 1] - r0;  // the rows of an aggregate are consecutive:
+#pragma unroll 4
+              for (int k = srp[la] + sub, e = srp[lb]; k < e; k += lpr)  // ... so are their nonzeros
+                sum -= sval[k] * tile_x<OP>(a, scol[k], r0, nrows, xs, bs, ds, as, es);
+              for (int lr = la + sub; lr < lb; lr += lpr) sum += bs[lr];
+            }
+            for (int o = lpr >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            if (al < nA && sub == 0) a.out[sd.I0 + al] = sum;
           }
-          a.out[ii.x + al] = acc;
-        }
-      } else {
-        for (int lr = tid; lr < nrows; lr += RT_THREADS) {
-          double sum = 0.0;
-          for (int k = srp[lr] - ka, e = srp[lr + 1] - ka; k < e; ++k) sum += prod[k];
-          double o;
-          if (OP == OP_SPMV)
-            o = sum;
-          else
-            o = xs[lr] + ds[lr] * (bs[lr] - sum);
-          a.out[r0 + lr] = o;
-          if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? (d0_staged ? bs[lr] : xs[lr]) : bs[lr]) * o;
-          if (NDOT >= 2) dots[1] += o * o;
+        } else {
+          const int nunits = nrows << lsh;
+          for (int ubase = 0; ubase < nunits; ubase += RT_CONSUMERS) {
+            const int u = ubase + tid;
+            const int lr = u >> lsh, sub = u & (lpr - 1);
+            double sum = 0.0;
+            if (lr < nrows) {
+#pragma unroll 4
+              for (int k = srp[lr] + sub, e = srp[lr + 1]; k < e; k += lpr)
+                sum += sval[k] * tile_x<OP>(a, scol[k], r0, nrows, xs, bs, ds, as, es);
+            }
+            for (int o = lpr >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            if (lr < nrows && sub == 0) {
+              double o;
+              if (OP == OP_SPMV) {
+                o = sum;
+              } else {
+                double xi;
+                if (OP == OP_JACOBI0)
+                  xi = ds[lr] * bs[lr];
+                else if (OP == OP_JACOBI_PROLONG)
+                  xi = xs[lr] + a.gamma * es[as[lr]];
+                else
+                  xi = xs[lr];
+                o = xi + ds[lr] * (bs[lr] - sum);
+              }
+              a.out[r0 + lr] = o;
+              if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? (d0_staged ? bs[lr] : xs[lr]) : bs[lr]) * o;
+              if (NDOT >= 2) dots[1] += o * o;
+            }
+          }
         }
       }
+      // ---- this warp is done with the stage ----
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + s);
     }
   }
   if (NDOT > 0) grid_reduce_finalize<(NDOT > 0 ? NDOT : 1), RT_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);

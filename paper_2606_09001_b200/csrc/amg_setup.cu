@@ -550,8 +550,13 @@ __global__ void k_gather_double(int n, const double* __restrict__ src, const int
   if (p < n) dst[p] = src[idx[p]];
 }
 
-// row-block partition: block k starts at the first unit (aggregate, or row if unit_ptr == null)
-// whose first nonzero is at or beyond k * target
+// Row-tile partition by shared-memory bytes: a row weighs RT_ROW_WEIGHT bytes of staged row
+// operands plus 12 bytes per nonzero.  Tile k starts at the first unit (aggregate, or row if
+// unit_ptr == null) whose cumulative weight is at or beyond k * target.
+constexpr int RT_ROW_WEIGHT = 40;
+__device__ __forceinline__ int64_t tile_weight(const int* __restrict__ rowptr, int r) {
+  return 12 * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
+}
 __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __restrict__ unit_ptr,
                                 const int* __restrict__ rowptr, int n, int* __restrict__ blk_ptr) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -565,7 +570,7 @@ __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __r
   while (lo < hi) {
     int mid = (lo + hi) >> 1;
     int r = unit_ptr ? unit_ptr[mid] : mid;
-    if (rowptr[r] >= want)
+    if (tile_weight(rowptr, r) >= want)
       hi = mid;
     else
       lo = mid + 1;
@@ -573,14 +578,16 @@ __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __r
   blk_ptr[k] = lo == nunits ? n : (unit_ptr ? unit_ptr[lo] : lo);
 }
 
-__global__ void k_blk_stats(int nblk, const int* __restrict__ blk_ptr, const int* __restrict__ rowptr,
-                            int* __restrict__ stats) {
+// stats[0] = largest stage footprint of a tile (bytes), stats[1] = most nonzero slots, stats[2] = most rows
+__global__ void k_blk_stats(int nblk, const TileDesc* __restrict__ tiles, int* __restrict__ stats) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= nblk) return;
-  int r0 = blk_ptr[k], r1 = blk_ptr[k + 1];
-  int k0 = rowptr[r0], k1 = rowptr[r1];
-  atomicMax(&stats[0], r1 - r0);
-  atomicMax(&stats[1], k1 - (k0 & ~3));
+  const TileDesc d = tiles[k];
+  if (d.r1 <= d.r0) return;
+  const TileLayout t = tile_layout(d.r0, d.r1, d.k0, d.k1, d.I0, d.I1);
+  atomicMax(&stats[0], t.end + RT_DESC_BYTES);
+  atomicMax(&stats[1], t.nk);
+  atomicMax(&stats[2], d.r1 - d.r0);
 }
 
 __global__ void k_tile_desc(int nblk, const int* __restrict__ blk_ptr, const int* __restrict__ rowptr,
@@ -920,26 +927,41 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
       k_gather_double<<<grid_for(L.n), TPB, 0, st>>>(L.n, N.dinv, L.inv, L.dinv);
     }
     AMG_CUDA_TRY(H, cudaGetLastError());
-    // row-tile partition: aim at one row per thread of the row phase and at most RT_TARGET nonzeros
+    // row-tile partition by stage bytes; a unit (aggregate) may overshoot the target, so the target
+    // is lowered until every tile fits a ring stage and RT_MAX_SLOTS nonzero slots
     double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
-    int target = (int)(mean_len * RT_ROWS_TARGET);
-    if (target > RT_TARGET) target = RT_TARGET;
-    if (target < 64) target = 64;
-    L.nblk = L.nnz > 0 ? div_up(L.nnz, target) : 1;
-    AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
-    AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
-    k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
-                                                         q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
-    k_tile_desc<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, q < Lc ? L.agg : nullptr, L.tiles);
-    int* stats;
-    AMG_ALLOC(H, stats, int, 2, st);
-    AMG_CUDA_TRY(H, cudaMemsetAsync(stats, 0, 2 * sizeof(int), st));
-    k_blk_stats<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, stats);
-    int h_stats[2];
-    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_stats, stats, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-    amg_dev_free(H, stats);
-    L.fast = (!o.force_generic && h_stats[0] <= RT_TR && h_stats[1] + 4 <= RT_TN) ? 1 : 0;
+    L.fast = 0;
+    const int64_t total_w = 12 * (int64_t)L.nnz + (int64_t)RT_ROW_WEIGHT * L.n;
+    const double shrink[4] = {0.92, 0.80, 0.65, 0.5};
+    for (int attempt = 0; attempt < 4 && !L.fast; ++attempt) {
+      int target = (int)((RT_STAGE_BYTES - RT_DESC_BYTES - 256) * shrink[attempt]);
+      const int slot_target = (int)(12.0 * RT_MAX_SLOTS * shrink[attempt] * (1.0 + RT_ROW_WEIGHT / (12.0 * mean_len)));
+      if (target > slot_target) target = slot_target;
+      if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
+      if (L.tiles) amg_dev_free(H, L.tiles);
+      L.nblk = total_w > 0 ? div_up(total_w, target) : 1;
+      AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
+      AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
+      k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
+                                                           q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
+      k_tile_desc<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, q < Lc ? L.agg : nullptr, L.tiles);
+      int* stats;
+      AMG_ALLOC(H, stats, int, 4, st);
+      AMG_CUDA_TRY(H, cudaMemsetAsync(stats, 0, 4 * sizeof(int), st));
+      k_blk_stats<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.tiles, stats);
+      int h_stats[4];
+      AMG_CUDA_TRY(H, cudaMemcpyAsync(h_stats, stats, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+      amg_dev_free(H, stats);
+      if (o.force_generic) break;
+      if (h_stats[0] <= RT_STAGE_BYTES && h_stats[1] <= RT_MAX_SLOTS) {
+        L.fast = 1;
+        // lanes per row of the row phase: fill the 256 consumer threads
+        const double rows_per_tile = (double)L.n / L.nblk;
+        L.lpr2 = 1;
+        while (L.lpr2 < 8 && rows_per_tile * (L.lpr2 * 2) <= 250.0 && mean_len >= 3.0 * L.lpr2) L.lpr2 *= 2;
+      }
+    }
     L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));
     size_t mat_bytes = (size_t)L.nnz * 12 + (size_t)L.n * 4;
     L.stream_hint = (H->l2_bytes > 0 && mat_bytes > H->l2_bytes / 2) ? 1 : 0;
