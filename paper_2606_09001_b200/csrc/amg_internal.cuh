@@ -9,66 +9,33 @@
 #include "amg_b200.h"
 
 // ------------------------------------------------------------------------------------------
-// tuning constants of the row-tile streaming kernels; the -D overrides
-// exist for tuning sweeps only
+// tuning constants of the row-tile streaming kernels; the -D overrides exist for
+// tuning sweeps only
 // ------------------------------------------------------------------------------------------
 #ifndef RT_STAGES_CFG
 #define RT_STAGES_CFG 3
 #endif
 #ifndef RT_CTAS_CFG
-#define RT_CTAS_CFG 4
+#define RT_CTAS_CFG 2
 #endif
 #ifndef RT_STAGE_BYTES_CFG
-#define RT_STAGE_BYTES_CFG 16384
+#define RT_STAGE_BYTES_CFG 36864
 #endif
-constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA: one quad of nonzeros each per tile
-constexpr int RT_THREADS = RT_CONSUMERS + 32;      // + one producer warp (issues the bulk copies)
+constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA (8 warps walk the ELL slices)
+constexpr int RT_GATHERERS = 64;                   // 2 warps fetch the halo values one tile ahead
+constexpr int RT_THREADS = RT_CONSUMERS + 32 + RT_GATHERERS;  // + one producer warp (issues the bulk copies)
 constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA
 constexpr int RT_CTAS = RT_CTAS_CFG;               // persistent CTAs per SM
 constexpr int RT_STAGE_BYTES = RT_STAGE_BYTES_CFG; // shared memory of one ring stage (descriptor + operands of one tile)
-constexpr int RT_DESC_BYTES = 64;                  // stage header written by the producer
-constexpr int RT_MAX_SLOTS = RT_CONSUMERS * 4;     // nonzero slots of a tile (incl. alignment slop)
+constexpr int RT_MAX_NNZ = 4096;                   // most entries / halo columns of a tile (packer scratch)
+constexpr int RT_MAX_ROWS = 1024;                  // most rows of a tile
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
                                   // the bulk copies round their slices out to 16-byte boundaries
 constexpr int RB_THREADS = 256;   // row-vector fallback kernels
 constexpr int RED_THREADS = 256;  // BLAS-1 kernels
 constexpr int MAX_DENSE = 4096;   // largest coarsest level accepted
 
-// one tile of a level: rows [r0, r1) (boundaries on aggregate starts), nonzeros [k0, k1),
-// coarse rows [I0, I1] (I1 < I0 on the coarsest level)
-struct alignas(32) TileDesc {
-  int r0, r1, k0, k1, I0, I1, pad0, pad1;
-};
-
-// Placement of a tile's operands inside its ring stage (after the RT_DESC_BYTES header).  Every
-// slice is rounded out to 16-byte boundaries of the source array (bulk copies need 16-byte
-// aligned addresses and sizes), so every section is a multiple of 16 bytes.
-struct TileLayout {
-  int ka, nk;        // first staged nonzero slot (multiple of 4), slots staged
-  int ra, nrp, nrv;  // first staged row (multiple of 4), rowptr entries, row-vector entries
-  int Ia, nec, nap;  // first staged coarse row, coarse-vector entries, agg_ptr entries
-  int o_col, o_rp, o_x, o_b, o_d, o_agg, o_ec, end;  // byte offsets (val at 0)
-};
-__host__ __device__ inline TileLayout tile_layout(int r0, int r1, int k0, int k1, int I0, int I1) {
-  TileLayout t;
-  t.ka = k0 & ~3;
-  t.nk = (k1 - t.ka + 3) & ~3;
-  t.ra = r0 & ~3;
-  t.nrp = (r1 + 1 - t.ra + 3) & ~3;
-  t.nrv = (r1 - t.ra + 3) & ~3;
-  t.Ia = I0 & ~3;
-  t.nec = I1 >= I0 ? ((I1 + 1 - t.Ia + 3) & ~3) : 0;
-  t.nap = I1 >= I0 ? ((I1 + 2 - t.Ia + 3) & ~3) : 0;
-  t.o_col = 8 * t.nk;
-  t.o_rp = t.o_col + 4 * t.nk;
-  t.o_x = t.o_rp + 4 * t.nrp;
-  t.o_b = t.o_x + 8 * t.nrv;
-  t.o_d = t.o_b + 8 * t.nrv;
-  t.o_agg = t.o_d + 8 * t.nrv;
-  t.o_ec = t.o_agg + 4 * (t.nrv > t.nap ? t.nrv : t.nap);
-  t.end = t.o_ec + 8 * t.nec;
-  return t;
-}
+#include "amg_tilepack.cuh"
 
 // ------------------------------------------------------------------------------------------
 // device-resident Krylov scalars and loop control (S7-S9: no host round trip inside the loop)
@@ -112,10 +79,11 @@ struct Level {
   // row-tile partition (boundaries aligned to aggregate starts)
   int* blk_ptr = nullptr;   // [nblk+1]
   TileDesc* tiles = nullptr;  // [nblk]
+  unsigned char* blob = nullptr;  // tile-packed operator (amg_tilepack.cuh), fast levels only
+  size_t blob_bytes = 0;
   int nblk = 0;
   int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback
   int lpr = 8;              // lanes per row of the fallback kernels
-  int lpr2 = 1;             // lanes per row of the row phase of the row-tile kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary
   int* nat_agg = nullptr;   // [n] aggregate ids in natural numbering of levels l, l+1

@@ -29,7 +29,7 @@ struct RowArgs {
   double* out;
   const int* agg;       // prolongation / restriction
   const int* agg_ptr;
-  int lpr2;             // lanes per row of the row phase (row-tile kernels)
+  const unsigned char* blob;  // tile-packed operator (row-tile kernels)
   const double* ec;
   double gamma;
   const double* d0;     // second operand of the fused dot (SpMV)
@@ -294,39 +294,48 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // ------------------------------------------------------------------------------------------
-// Row-tile streaming kernel (S1-S4).  Persistent and warp-specialised: RT_CTAS CTAs per SM, each
-// owning a contiguous run of tiles; 8 consumer warps + 1 producer warp per CTA.
+// Row-tile streaming kernel (S1-S4) over the sorted-ELL tile blobs (amg_tilepack.cuh).
+// Persistent and warp-specialised: RT_CTAS CTAs per SM, each owning a contiguous run of tiles;
+// per CTA 8 consumer warps + 1 producer warp + 2 gather warps around a ring of RT_STAGES stages.
 //
-// One tile = rows [r0, r1) on aggregate boundaries, at most RT_MAX_SLOTS nonzero slots and
-// RT_STAGE_BYTES of operands.  Everything a tile reads with unit stride -- its slices of val /
-// col / rowptr, of x, b, dinv, of agg / agg_ptr and of the coarse vector -- arrives in shared
-// memory by bulk-async copies (TMA) that the producer warp issues up to RT_STAGES tiles ahead,
-// throttled only by the consumers' "stage empty" mbarriers: HBM keeps streaming whatever the
-// consumers are doing.  The consumers read the stage and never write it: LPR2 lanes per row
-// (per aggregate for the restriction, whose rows and therefore nonzeros are consecutive) walk
-// the row's (col, val) pairs in shared memory; a column inside the tile's own row range (most,
-// in the aggregate-contiguous numbering) reads the staged x slice -- neighbouring lanes hold
-// neighbouring rows, so these reads are nearly contiguous -- the others are gathered through
-// L1/L2.  No product array, no CTA-wide barrier: a warp releases the stage when it is done and
-// may run ahead into the next tile.  (ncu on the earlier quad-per-thread variant showed the
-// shared-memory data pipe at 64-80 % of its peak: val/col read, products written and read back,
-// scattered x reads; the row walk needs ~2.5x fewer wavefronts per nonzero.)
+//   producer (1 thread)  waits for "empty", writes the stage header and issues the bulk-async
+//                        copies (TMA) of the tile: its blob (one copy) and its slices of x, b,
+//                        dinv, agg / agg_ptr and of the coarse vector -> mbarrier "full"
+//   gather warps         wait for "full", fetch the x value of every distinct halo column of the
+//                        tile (once per column, independent loads, L2) into the stage, apply
+//                        the per-row transform of the fused operations to the tile's own rows
+//                        (x1 = dinv o b;  x~ = x + gamma ec[agg]) -> mbarrier "ready"
+//   consumer warps       wait for "ready"; slices of 32 storage rows are dealt round-robin to
+//                        the warps ACROSS tiles; one lane per row walks the slice's k-major slots:
+//                        three shared-memory reads and one DFMA per entry, no divergence, no
+//                        global gather, no row pointers; epilogue per row; -> mbarrier "empty"
+//
+// There is no CTA-wide barrier: HBM keeps streaming whatever the consumers are doing, the gather
+// latency is hidden one stage ahead, and warps drift across tiles (the round-robin deal balances
+// them).  Only the restriction needs the tile's rows together (sum over an aggregate's rows): its
+// consumers meet on a fourth mbarrier per tile.
 // ------------------------------------------------------------------------------------------
 namespace rt {
-constexpr int HEADER_BYTES = 128;  // full[RT_STAGES], empty[RT_STAGES] mbarriers
+constexpr int HEADER_BYTES = 256;  // full / ready / empty / resdone mbarriers, RT_STAGES each
 constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * RT_STAGE_BYTES;
-static_assert(RT_STAGES >= 2 && 2 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
+constexpr int NCW = RT_CONSUMERS / 32;  // consumer warps
+constexpr int NGW = RT_GATHERERS / 32;  // gather warps
+static_assert(RT_STAGES >= 2 && 4 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
 static_assert(RT_STAGE_BYTES % 128 == 0, "stage size must keep 128-byte alignment");
 static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
+static_assert((NCW & (NCW - 1)) == 0, "consumer warps must be a power of two");
 }  // namespace rt
 
-struct StageDesc {  // RT_DESC_BYTES at the start of a stage, written by the producer
-  int r0, nrows, k0, k1;
-  int I0, I1, o_col, o_rp;
-  int o_x, o_b, o_d, o_agg;
-  int o_ec, ka, roff, ioff;  // roff = r0 - ra, ioff = I0 - Ia
+struct StageDesc {  // TP_DESC_BYTES at the start of a stage, written by the producer
+  int r0, nr, I0, nA;
+  int nsl, nhalo, roff, pad0;
+  int o_halo, o_perm, o_col, o_val;
+  int o_cagg, o_b, o_d, o_agg;  // o_agg: agg slice (prolongation) or agg_ptr slice (restriction)
+  int o_ec, o_xcat, o_out, aoff;  // aoff: r0 - ra4 (agg slice) or I0 - Ia4 (agg_ptr slice)
+  int eoff, pad1, pad2, pad3;     // eoff: Ia2 (es[I - eoff] = ec[I])
+  int pad4[8];
 };
-static_assert(sizeof(StageDesc) == RT_DESC_BYTES, "stage header size");
+static_assert(sizeof(StageDesc) == TP_DESC_BYTES, "stage header size");
 
 // which operands of the tile are staged for which operation
 template <int OP>
@@ -337,63 +346,53 @@ struct TileOps {
   static constexpr bool AGG = (OP == OP_JACOBI_PROLONG);
   static constexpr bool EC = (OP == OP_JACOBI_PROLONG);
   static constexpr bool AGGPTR = (OP == OP_RESTRICT);
+  static constexpr int FLAGS = (B ? TP_B : 0) | (D ? TP_D : 0) | (AGG ? TP_AGG | TP_CAGG : 0) | (EC ? TP_EC : 0) |
+                               (AGGPTR ? TP_AGGPTR | TP_OUT : 0);
 };
 
 template <int OP, int NDOT, bool STREAM>
 __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
                                            uint64_t pol) {
   using T = TileOps<OP>;
-  const TileLayout t = tile_layout(d.r0, d.r1, d.k0, d.k1, d.I0, d.I1);
+  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
+  const int flags = T::FLAGS | (d0_staged ? TP_B : 0);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  const StageLayout t = tp_stage(d, flags);
   StageDesc sd;
-  sd.r0 = d.r0, sd.nrows = d.r1 - d.r0, sd.k0 = d.k0, sd.k1 = d.k1;
-  sd.I0 = d.I0, sd.I1 = d.I1, sd.o_col = t.o_col, sd.o_rp = t.o_rp;
-  sd.o_x = t.o_x, sd.o_b = t.o_b, sd.o_d = t.o_d, sd.o_agg = t.o_agg;
-  sd.o_ec = t.o_ec, sd.ka = t.ka, sd.roff = d.r0 - t.ra, sd.ioff = d.I0 - t.Ia;
+  sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
+  sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.pad0 = 0;
+  sd.o_halo = p.o_halo, sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val;
+  sd.o_cagg = p.o_cagg, sd.o_b = t.o_b, sd.o_d = t.o_d, sd.o_agg = t.o_agg;
+  sd.o_ec = t.o_ec, sd.o_xcat = t.o_xcat, sd.o_out = t.o_out;
+  sd.aoff = T::AGGPTR ? d.I0 - t.Ia4 : d.r0 - t.ra4;
+  sd.eoff = t.Ia2, sd.pad1 = sd.pad2 = sd.pad3 = 0;
   int4* dst = reinterpret_cast<int4*>(stage);
   const int4* src = reinterpret_cast<const int4*>(&sd);
-  dst[0] = src[0], dst[1] = src[1], dst[2] = src[2], dst[3] = src[3];
-  if (sd.nrows <= 0) {
+#pragma unroll
+  for (int q = 0; q < 6; ++q) dst[q] = src[q];
+  if (d.nr <= 0) {
     mbar_arrive(bar);
     return;
   }
-  unsigned char* base = stage + RT_DESC_BYTES;
-  const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
-  const uint32_t nk = (uint32_t)t.nk, nrp = (uint32_t)t.nrp, nrv = (uint32_t)t.nrv, nec = (uint32_t)t.nec,
-                 nap = (uint32_t)t.nap;
-  uint32_t bytes = nk * 12u + nrp * 4u;
-  if (T::X) bytes += nrv * 8u;
-  if (T::B || d0_staged) bytes += nrv * 8u;
-  if (T::D) bytes += nrv * 8u;
-  if (T::AGG) bytes += nrv * 4u;
-  if (T::EC) bytes += nec * 8u;
-  if (T::AGGPTR) bytes += nap * 4u;
+  unsigned char* base = stage + TP_DESC_BYTES;
+  const uint32_t nblob = (uint32_t)(T::AGG ? p.endB : p.endA);
+  const uint32_t nrv8 = 8u * (uint32_t)t.nrv;
+  uint32_t bytes = nblob;
+  if (T::X) bytes += nrv8;
+  if (T::B || d0_staged) bytes += nrv8;
+  if (T::D) bytes += nrv8;
+  if (T::AGG) bytes += 4u * (uint32_t)t.nr4;
+  if (T::EC) bytes += 8u * (uint32_t)t.nec;
+  if (T::AGGPTR) bytes += 4u * (uint32_t)t.nap;
   mbar_arrive_expect_tx(bar, bytes);
-  bulk_g2s<STREAM>(base, a.val + t.ka, nk * 8u, bar, pol);
-  bulk_g2s<STREAM>(base + t.o_col, a.col + t.ka, nk * 4u, bar, pol);
-  bulk_g2s<false>(base + t.o_rp, a.rowptr + t.ra, nrp * 4u, bar, pol);
-  if (T::X) bulk_g2s<false>(base + t.o_x, a.x + t.ra, nrv * 8u, bar, pol);
-  if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra, nrv * 8u, bar, pol);
-  if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra, nrv * 8u, bar, pol);
-  if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra, nrv * 8u, bar, pol);
-  if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra, nrv * 4u, bar, pol);
-  if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia, nec * 8u, bar, pol);
-  if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia, nap * 4u, bar, pol);
-}
-
-// value of the gathered vector at column c: from the staged slices when c lies in the tile's own
-// row range, else through L1/L2
-template <int OP>
-__device__ __forceinline__ double tile_x(const RowArgs& a, int c, int r0, int nrows, const double* xs,
-                                         const double* bs, const double* ds, const int* as, const double* es) {
-  const unsigned dd = (unsigned)(c - r0);
-  if (dd < (unsigned)nrows) {
-    if (OP == OP_JACOBI0) return ds[dd] * bs[dd];
-    if (OP == OP_JACOBI_PROLONG) return xs[dd] + a.gamma * es[as[dd]];
-    return xs[dd];
-  }
-  if (OP == OP_JACOBI0) return __ldg(a.dinv + c) * __ldg(a.b + c);
-  if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.agg + c));
-  return __ldg(a.x + c);
+  bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, nblob, bar, pol);
+  if (T::X) bulk_g2s<false>(base + t.o_xcat, a.x + t.ra2, nrv8, bar, pol);
+  if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra2, nrv8, bar, pol);
+  if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra2, nrv8, bar, pol);
+  if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, nrv8, bar, pol);
+  if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra4, 4u * (uint32_t)t.nr4, bar, pol);
+  if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
+  if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
 }
 
 template <int OP, int NDOT, bool STREAM>
@@ -401,7 +400,9 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (a.ctl != nullptr && a.ctl->done) return;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
-  uint64_t* empty = full + RT_STAGES;
+  uint64_t* ready = full + RT_STAGES;
+  uint64_t* empty = ready + RT_STAGES;
+  uint64_t* resdone = empty + RT_STAGES;
   unsigned char* stage0 = smem + rt::HEADER_BYTES;
   const int tid = threadIdx.x;
   const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
@@ -411,7 +412,9 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (tid == 0) {
     for (int s = 0; s < RT_STAGES; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, RT_CONSUMERS / 32);
+      mbar_init(ready + s, rt::NGW);
+      mbar_init(empty + s, rt::NCW);
+      mbar_init(resdone + s, rt::NCW);
     }
     fence_mbar_init();
   }
@@ -420,7 +423,75 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
 #pragma unroll
   for (int j = 0; j < (NDOT > 0 ? NDOT : 1); ++j) dots[j] = 0.0;
 
-  if (tid >= RT_CONSUMERS) {
+  if (tid >= RT_CONSUMERS + 32) {
+    // ---------------- gather warps ----------------
+    const int g = tid - (RT_CONSUMERS + 32);
+    for (int it = 0; it < my; ++it) {
+      const int s = it % RT_STAGES;
+      unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
+      mbar_wait(full + s, (uint32_t)((it / RT_STAGES) & 1));
+      const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
+      const int nr = sd->nr, nhalo = sd->nhalo;
+      if (nr > 0) {
+        unsigned char* base = stage + TP_DESC_BYTES;
+        const int* hl = reinterpret_cast<const int*>(base + sd->o_halo);
+        double* xc = reinterpret_cast<double*>(base + sd->o_xcat) + sd->roff;  // xc[col]
+        double* xh = xc + nr;
+        if (OP == OP_JACOBI_PROLONG) {
+          const int* hc = reinterpret_cast<const int*>(base + sd->o_cagg);
+          const double gamma = a.gamma;
+          int h = g;
+          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
+            double v[4], e[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              v[q] = __ldg(a.x + hl[h + q * RT_GATHERERS]);
+              e[q] = __ldg(a.ec + hc[h + q * RT_GATHERERS]);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q] + gamma * e[q];
+          }
+          for (; h < nhalo; h += RT_GATHERERS) xh[h] = __ldg(a.x + hl[h]) + gamma * __ldg(a.ec + hc[h]);
+          const int* as = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;    // as[lr] = agg[r0 + lr]
+          const double* es = reinterpret_cast<const double*>(base + sd->o_ec) - sd->eoff;  // es[I] = ec[I]
+          for (int lr = g; lr < nr; lr += RT_GATHERERS) xc[lr] += gamma * es[as[lr]];
+        } else if (OP == OP_JACOBI0) {
+          int h = g;
+          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
+            double v[4], e[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int c = hl[h + q * RT_GATHERERS];
+              v[q] = __ldg(a.dinv + c);
+              e[q] = __ldg(a.b + c);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q] * e[q];
+          }
+          for (; h < nhalo; h += RT_GATHERERS) {
+            const int c = hl[h];
+            xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
+          }
+          const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
+          const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
+          for (int lr = g; lr < nr; lr += RT_GATHERERS) xc[lr] = ds[lr] * bs[lr];
+        } else {
+          int h = g;
+          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
+            double v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) v[q] = __ldg(a.x + hl[h + q * RT_GATHERERS]);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q];
+          }
+          for (; h < nhalo; h += RT_GATHERERS) xh[h] = __ldg(a.x + hl[h]);
+        }
+        fence_proxy_async();  // generic writes into a region a later bulk copy overwrites
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(ready + s);
+    }
+  } else if (tid >= RT_CONSUMERS) {
     // ---------------- producer warp ----------------
     if (tid == RT_CONSUMERS && my > 0) {
       const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
@@ -436,78 +507,64 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     }
   } else {
     // ---------------- consumers ----------------
-    // No CTA-wide barrier: every warp walks its own units (rows, or aggregates for the
-    // restriction) of a tile and releases the stage when it is done with it.
-    const int lane = tid & 31;
-    const int lpr = (OP == OP_RESTRICT) ? a.lpr2 * 2 : a.lpr2;  // lanes per unit
-    const int lsh = 31 - __clz(lpr);
+    const int lane = tid & 31, w = tid >> 5;
+    int sbase = 0;  // slices of the tiles so far: the round-robin deal continues across tiles
     for (int it = 0; it < my; ++it) {
       const int s = it % RT_STAGES;
+      const uint32_t par = (uint32_t)((it / RT_STAGES) & 1);
       unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
-      mbar_wait(full + s, (uint32_t)((it / RT_STAGES) & 1));
-      const StageDesc sd = *reinterpret_cast<const StageDesc*>(stage);
-      unsigned char* base = stage + RT_DESC_BYTES;
-      const int r0 = sd.r0, nrows = sd.nrows, ka = sd.ka;
-      const double* sval = reinterpret_cast<const double*>(base) - ka;            // sval[k] = val[k]
-      const int* scol = reinterpret_cast<const int*>(base + sd.o_col) - ka;       // scol[k] = col[k]
-      const int* srp = reinterpret_cast<const int*>(base + sd.o_rp) + sd.roff;    // srp[lr] = rowptr[r0 + lr]
-      const double* xs = reinterpret_cast<const double*>(base + sd.o_x) + sd.roff;  // tile-local row operands
-      const double* bs = reinterpret_cast<const double*>(base + sd.o_b) + sd.roff;
-      const double* ds = reinterpret_cast<const double*>(base + sd.o_d) + sd.roff;
-      const int* as = reinterpret_cast<const int*>(base + sd.o_agg) + sd.roff;    // as[lr] = agg[r0 + lr]
-      const double* es = reinterpret_cast<const double*>(base + sd.o_ec) - (sd.I0 - sd.ioff);  // es[I] = ec[I]
-      if (nrows > 0) {
-        if (OP == OP_RESTRICT) {
-          const int nA = sd.I1 - sd.I0 + 1;
-          const int* aps = reinterpret_cast<const int*>(base + sd.o_agg) + sd.ioff;  // aps[al] = agg_ptr[I0 + al]
-          const int nunits = nA << lsh;
-          for (int ubase = 0; ubase < nunits; ubase += RT_CONSUMERS) {
-            const int u = ubase + tid;
-            const int al = u >> lsh, sub = u & (lpr - 1);
-            double sum = 0.0;
-            if (al < nA) {
-              const int la = aps[al] - r0, lb = aps[al + 1] - r0;  // the rows of an aggregate are consecutive:
+      mbar_wait(full + s, par);   // the bulk copies have landed ...
+      mbar_wait(ready + s, par);  // ... and the gather warps are done with the stage
+      const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
+      const int nr = sd->nr, nsl = sd->nsl, r0 = sd->r0;
+      if (nr > 0) {
+        unsigned char* base = stage + TP_DESC_BYTES;
+        const int2* slices = reinterpret_cast<const int2*>(base);
+        const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + sd->o_perm);
+        const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
+        const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
+        const double* xc = reinterpret_cast<const double*>(base + sd->o_xcat) + sd->roff;
+        const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
+        const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
+        double* outs = reinterpret_cast<double*>(base + sd->o_out);
+        for (int j = (w - sbase) & (rt::NCW - 1); j < nsl; j += rt::NCW) {
+          const int2 sl = slices[j];
+          const unsigned short* cp = scol + sl.x;
+          const double* vp = sval + sl.x;
+          double sum = 0.0;
 #pragma unroll 4
-              for (int k = srp[la] + sub, e = srp[lb]; k < e; k += lpr)  // ... so are their nonzeros
-                sum -= sval[k] * tile_x<OP>(a, scol[k], r0, nrows, xs, bs, ds, as, es);
-              for (int lr = la + sub; lr < lb; lr += lpr) sum += bs[lr];
-            }
-            for (int o = lpr >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            if (al < nA && sub == 0) a.out[sd.I0 + al] = sum;
-          }
-        } else {
-          const int nunits = nrows << lsh;
-          for (int ubase = 0; ubase < nunits; ubase += RT_CONSUMERS) {
-            const int u = ubase + tid;
-            const int lr = u >> lsh, sub = u & (lpr - 1);
-            double sum = 0.0;
-            if (lr < nrows) {
-#pragma unroll 4
-              for (int k = srp[lr] + sub, e = srp[lr + 1]; k < e; k += lpr)
-                sum += sval[k] * tile_x<OP>(a, scol[k], r0, nrows, xs, bs, ds, as, es);
-            }
-            for (int o = lpr >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            if (lr < nrows && sub == 0) {
+          for (int k = 0; k < sl.y; ++k) sum += vp[k * 32] * xc[cp[k * 32]];
+          const int lr = perm[j * 32 + lane];
+          if (lr != 0xFFFF) {
+            if (OP == OP_RESTRICT) {
+              outs[lr] = bs[lr] - sum;
+            } else {
               double o;
-              if (OP == OP_SPMV) {
+              if (OP == OP_SPMV)
                 o = sum;
-              } else {
-                double xi;
-                if (OP == OP_JACOBI0)
-                  xi = ds[lr] * bs[lr];
-                else if (OP == OP_JACOBI_PROLONG)
-                  xi = xs[lr] + a.gamma * es[as[lr]];
-                else
-                  xi = xs[lr];
-                o = xi + ds[lr] * (bs[lr] - sum);
-              }
+              else
+                o = xc[lr] + ds[lr] * (bs[lr] - sum);
               a.out[r0 + lr] = o;
-              if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? (d0_staged ? bs[lr] : xs[lr]) : bs[lr]) * o;
+              if (NDOT >= 1) dots[0] += (OP == OP_SPMV ? (d0_staged ? bs[lr] : xc[lr]) : bs[lr]) * o;
               if (NDOT >= 2) dots[1] += o * o;
             }
           }
         }
+        if (OP == OP_RESTRICT) {
+          // the rows of an aggregate are consecutive tile rows: all residuals of the tile first
+          __syncwarp();
+          if (lane == 0) mbar_arrive(resdone + s);
+          mbar_wait(resdone + s, par);
+          const int nA = sd->nA, I0 = sd->I0;
+          const int* aps = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;  // aps[al] = agg_ptr[I0 + al]
+          for (int al = tid; al < nA; al += RT_CONSUMERS) {
+            double sum = 0.0;
+            for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) sum += outs[lr];
+            a.out[I0 + al] = sum;
+          }
+        }
       }
+      sbase = (sbase + nsl) & (rt::NCW - 1);
       // ---- this warp is done with the stage ----
       __syncwarp();
       if (lane == 0) mbar_arrive(empty + s);

@@ -551,11 +551,12 @@ __global__ void k_gather_double(int n, const double* __restrict__ src, const int
 }
 
 // Row-tile partition by shared-memory bytes: a row weighs RT_ROW_WEIGHT bytes of staged row
-// operands plus 12 bytes per nonzero.  Tile k starts at the first unit (aggregate, or row if
+// operands, a nonzero RT_NNZ_WEIGHT (value, 16-bit column, its share of the halo list and values).  Tile k starts at the first unit (aggregate, or row if
 // unit_ptr == null) whose cumulative weight is at or beyond k * target.
-constexpr int RT_ROW_WEIGHT = 40;
+constexpr int RT_ROW_WEIGHT = 44;
+constexpr int RT_NNZ_WEIGHT = 13;
 __device__ __forceinline__ int64_t tile_weight(const int* __restrict__ rowptr, int r) {
-  return 12 * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
+  return RT_NNZ_WEIGHT * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
 }
 __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __restrict__ unit_ptr,
                                 const int* __restrict__ rowptr, int n, int* __restrict__ blk_ptr) {
@@ -578,31 +579,193 @@ __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __r
   blk_ptr[k] = lo == nunits ? n : (unit_ptr ? unit_ptr[lo] : lo);
 }
 
-// stats[0] = largest stage footprint of a tile (bytes), stats[1] = most nonzero slots, stats[2] = most rows
-__global__ void k_blk_stats(int nblk, const TileDesc* __restrict__ tiles, int* __restrict__ stats) {
-  int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= nblk) return;
-  const TileDesc d = tiles[k];
-  if (d.r1 <= d.r0) return;
-  const TileLayout t = tile_layout(d.r0, d.r1, d.k0, d.k1, d.I0, d.I1);
-  atomicMax(&stats[0], t.end + RT_DESC_BYTES);
-  atomicMax(&stats[1], t.nk);
-  atomicMax(&stats[2], d.r1 - d.r0);
-}
-
-__global__ void k_tile_desc(int nblk, const int* __restrict__ blk_ptr, const int* __restrict__ rowptr,
-                            const int* __restrict__ agg, TileDesc* __restrict__ tiles) {
-  int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= nblk) return;
+// ------------------------------------------------------------------------------------------
+// Tile packer (amg_tilepack.cuh): one CTA per tile.  Pass 1 (write == 0) sizes every tile: rows
+// sorted by descending length (stable), slice widths, the sorted list of distinct out-of-tile
+// columns; pass 2 (after a scan of the blob sizes) repeats that and writes the blob.
+// info[0] = largest stage footprint (bytes), info[1] = a tile exceeds the packer's scratch
+// ------------------------------------------------------------------------------------------
+constexpr int PK_THREADS = 256;
+constexpr int PK_MAX_LEN = 512;
+__global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int* __restrict__ blk_ptr,
+                                                           const int* __restrict__ rowptr, const int* __restrict__ col,
+                                                           const double* __restrict__ val, const int* __restrict__ agg,
+                                                           int write, const int* __restrict__ blob_off16,
+                                                           int* __restrict__ size16, int* __restrict__ info,
+                                                           TileDesc* __restrict__ tiles, unsigned char* __restrict__ blob) {
+  __shared__ int ext[RT_MAX_NNZ];
+  __shared__ int halo[RT_MAX_NNZ];
+  __shared__ int len[RT_MAX_ROWS];
+  __shared__ int srow[RT_MAX_ROWS];
+  __shared__ int hist[PK_MAX_LEN + 1];
+  __shared__ int sl_off[RT_MAX_ROWS / 32 + 1], sl_w[RT_MAX_ROWS / 32 + 1];
+  __shared__ int cnts[PK_THREADS];
+  __shared__ int s_cnt, s_nhalo, s_maxlen, s_nslots;
+  const int t = blockIdx.x, tid = threadIdx.x;
+  if (t >= ntiles) return;
+  const int r0 = blk_ptr[t], r1 = blk_ptr[t + 1], nr = r1 - r0;
   TileDesc d;
-  d.r0 = blk_ptr[k];
-  d.r1 = blk_ptr[k + 1];
-  d.k0 = rowptr[d.r0];
-  d.k1 = rowptr[d.r1];
-  d.I0 = (agg && d.r1 > d.r0) ? agg[d.r0] : 0;
-  d.I1 = (agg && d.r1 > d.r0) ? agg[d.r1 - 1] : -1;
-  d.pad0 = d.pad1 = 0;
-  tiles[k] = d;
+  d.r0 = r0, d.nr = nr, d.I0 = 0, d.nA = 0, d.nsl = 0, d.nslots = 0, d.nhalo = 0, d.blob16 = 0;
+  if (nr <= 0) {
+    if (tid == 0) {
+      if (write) tiles[t] = d;
+      else size16[t] = 0;
+    }
+    return;
+  }
+  const int k0 = rowptr[r0], k1 = rowptr[r1];
+  if (nr > RT_MAX_ROWS || k1 - k0 > RT_MAX_NNZ) {
+    if (tid == 0) {
+      info[1] = 1;
+      if (!write) size16[t] = 0;
+    }
+    return;
+  }
+  if (agg != nullptr) {
+    d.I0 = agg[r0];
+    d.nA = agg[r1 - 1] - d.I0 + 1;
+  }
+  if (tid == 0) s_cnt = 0, s_maxlen = 0;
+  for (int q = tid; q <= PK_MAX_LEN; q += PK_THREADS) hist[q] = 0;
+  __syncthreads();
+  for (int lr = tid; lr < nr; lr += PK_THREADS) {
+    const int l = rowptr[r0 + lr + 1] - rowptr[r0 + lr];
+    len[lr] = l;
+    atomicMax(&s_maxlen, l);
+    if (l <= PK_MAX_LEN) atomicAdd(&hist[l], 1);
+  }
+  for (int k = k0 + tid; k < k1; k += PK_THREADS) {
+    const int c = col[k];
+    if (c < r0 || c >= r1) ext[atomicAdd(&s_cnt, 1)] = c;
+  }
+  __syncthreads();
+  if (s_maxlen > PK_MAX_LEN) {
+    if (tid == 0) {
+      info[1] = 1;
+      if (!write) size16[t] = 0;
+    }
+    return;
+  }
+  const int nsl = (nr + 31) >> 5;
+  if (tid == 0) {
+    // stable counting sort by descending length; slice widths = length of the slice's first row
+    int acc = 0;
+    for (int l = s_maxlen; l >= 0; --l) {
+      const int c = hist[l];
+      hist[l] = acc;
+      acc += c;
+    }
+    for (int lr = 0; lr < nr; ++lr) srow[hist[len[lr]]++] = lr;
+    int off = 0;
+    for (int j = 0; j < nsl; ++j) {
+      const int w = len[srow[j * 32]];
+      sl_off[j] = off;
+      sl_w[j] = w;
+      off += 32 * w;
+    }
+    sl_off[nsl] = off;
+    s_nslots = off;
+  }
+  // sort the out-of-tile columns (bitonic, padded with INT_MAX), then keep the distinct ones
+  const int cnt = s_cnt;
+  int N = 1;
+  while (N < cnt) N <<= 1;
+  for (int i = cnt + tid; i < N; i += PK_THREADS) ext[i] = 0x7fffffff;
+  __syncthreads();
+  for (int k = 2; k <= N; k <<= 1)
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = tid; i < N; i += PK_THREADS) {
+        const int p = i ^ j;
+        if (p > i) {
+          const int a = ext[i], b = ext[p];
+          const bool asc = (i & k) == 0;
+          if ((a > b) == asc) {
+            ext[i] = b;
+            ext[p] = a;
+          }
+        }
+      }
+      __syncthreads();
+    }
+  {
+    const int chunk = (cnt + PK_THREADS - 1) / PK_THREADS;
+    const int b = tid * chunk, e = min(cnt, b + chunk);
+    int c = 0;
+    for (int i = b; i < e; ++i) c += (i == 0 || ext[i] != ext[i - 1]);
+    cnts[tid] = c;
+    __syncthreads();
+    if (tid == 0) {
+      int acc = 0;
+      for (int q = 0; q < PK_THREADS; ++q) {
+        const int v = cnts[q];
+        cnts[q] = acc;
+        acc += v;
+      }
+      s_nhalo = acc;
+    }
+    __syncthreads();
+    int o = cnts[tid];
+    for (int i = b; i < e; ++i)
+      if (i == 0 || ext[i] != ext[i - 1]) halo[o++] = ext[i];
+  }
+  __syncthreads();
+  d.nsl = nsl, d.nslots = s_nslots, d.nhalo = s_nhalo;
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  if (!write) {
+    if (tid == 0) {
+      size16[t] = p.endB / 16;
+      atomicMax(&info[0], tp_stage_need(d));
+    }
+    return;
+  }
+  d.blob16 = (uint32_t)blob_off16[t];
+  unsigned char* base = blob + (size_t)d.blob16 * 16u;
+  if (tid == 0) tiles[t] = d;
+  int2* o_sl = reinterpret_cast<int2*>(base);
+  for (int j = tid; j < nsl; j += PK_THREADS) o_sl[j] = make_int2(sl_off[j], sl_w[j]);
+  int* o_halo = reinterpret_cast<int*>(base + p.o_halo);
+  int* o_cagg = reinterpret_cast<int*>(base + p.o_cagg);
+  const int nh4 = tp_up(d.nhalo, 4);
+  for (int h = tid; h < nh4; h += PK_THREADS) {
+    const int c = h < d.nhalo ? halo[h] : 0;
+    o_halo[h] = c;
+    o_cagg[h] = (h < d.nhalo && agg != nullptr) ? agg[c] : 0;
+  }
+  unsigned short* o_perm = reinterpret_cast<unsigned short*>(base + p.o_perm);
+  for (int s = tid; s < nsl * 32; s += PK_THREADS) o_perm[s] = s < nr ? (unsigned short)srow[s] : (unsigned short)0xFFFF;
+  unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
+  double* o_val = reinterpret_cast<double*>(base + p.o_val);
+  for (int j = 0; j < nsl; ++j) {
+    const int off = sl_off[j], w = sl_w[j];
+    for (int q = tid; q < 32 * w; q += PK_THREADS) {
+      const int k = q >> 5, lane = q & 31, s = j * 32 + lane;
+      unsigned short c16 = 0;
+      double v = 0.0;
+      if (s < nr) {
+        const int lr = srow[s];
+        if (k < len[lr]) {
+          const int kk = rowptr[r0 + lr] + k;
+          const int c = col[kk];
+          v = val[kk];
+          if (c >= r0 && c < r1) {
+            c16 = (unsigned short)(c - r0);
+          } else {
+            int lo = 0, hi = d.nhalo;  // first entry >= c
+            while (lo < hi) {
+              const int mid = (lo + hi) >> 1;
+              if (halo[mid] < c) lo = mid + 1;
+              else hi = mid;
+            }
+            c16 = (unsigned short)(nr + lo);
+          }
+        }
+      }
+      o_col[off + q] = c16;
+      o_val[off + q] = v;
+    }
+  }
+  // tail of the u16 column section up to its 16-byte rounding
+  for (int q = d.nslots + tid; q < tp_up(2 * d.nslots, 16) / 2; q += PK_THREADS) o_col[q] = 0;
 }
 
 __global__ void k_pad_tail(int nnz, int nnz_alloc, int* __restrict__ col, double* __restrict__ val) {
@@ -927,39 +1090,64 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
       k_gather_double<<<grid_for(L.n), TPB, 0, st>>>(L.n, N.dinv, L.inv, L.dinv);
     }
     AMG_CUDA_TRY(H, cudaGetLastError());
-    // row-tile partition by stage bytes; a unit (aggregate) may overshoot the target, so the target
-    // is lowered until every tile fits a ring stage and RT_MAX_SLOTS nonzero slots
+    // row-tile partition by stage bytes, then the tile packer.  The byte model of the partition is
+    // approximate (the halo of a tile is only known once it is cut), so the target is rescaled
+    // until every tile fits a ring stage.
     double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
     L.fast = 0;
-    const int64_t total_w = 12 * (int64_t)L.nnz + (int64_t)RT_ROW_WEIGHT * L.n;
-    const double shrink[4] = {0.92, 0.80, 0.65, 0.5};
-    for (int attempt = 0; attempt < 4 && !L.fast; ++attempt) {
-      int target = (int)((RT_STAGE_BYTES - RT_DESC_BYTES - 256) * shrink[attempt]);
-      const int slot_target = (int)(12.0 * RT_MAX_SLOTS * shrink[attempt] * (1.0 + RT_ROW_WEIGHT / (12.0 * mean_len)));
-      if (target > slot_target) target = slot_target;
-      if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
-      if (L.tiles) amg_dev_free(H, L.tiles);
-      L.nblk = total_w > 0 ? div_up(total_w, target) : 1;
-      AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
-      AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
-      k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
-                                                           q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
-      k_tile_desc<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, q < Lc ? L.agg : nullptr, L.tiles);
-      int* stats;
-      AMG_ALLOC(H, stats, int, 4, st);
-      AMG_CUDA_TRY(H, cudaMemsetAsync(stats, 0, 4 * sizeof(int), st));
-      k_blk_stats<<<grid_for(L.nblk), TPB, 0, st>>>(L.nblk, L.tiles, stats);
-      int h_stats[4];
-      AMG_CUDA_TRY(H, cudaMemcpyAsync(h_stats, stats, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
-      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-      amg_dev_free(H, stats);
-      if (o.force_generic) break;
-      if (h_stats[0] <= RT_STAGE_BYTES && h_stats[1] <= RT_MAX_SLOTS) {
-        L.fast = 1;
-        // lanes per row of the row phase: fill the 256 consumer threads
-        const double rows_per_tile = (double)L.n / L.nblk;
-        L.lpr2 = 1;
-        while (L.lpr2 < 8 && rows_per_tile * (L.lpr2 * 2) <= 250.0 && mean_len >= 3.0 * L.lpr2) L.lpr2 *= 2;
+    if (!o.force_generic && L.n > 0) {
+      const int64_t total_w = RT_NNZ_WEIGHT * (int64_t)L.nnz + (int64_t)RT_ROW_WEIGHT * L.n;
+      double scale = 1.0;
+      for (int attempt = 0; attempt < 6 && !L.fast; ++attempt) {
+        const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
+        if (target < 512) break;
+        if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
+        if (L.tiles) amg_dev_free(H, L.tiles);
+        L.blk_ptr = nullptr, L.tiles = nullptr;
+        L.nblk = div_up(total_w, target);
+        int *size16, *off16, *info;
+        AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
+        AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
+        AMG_ALLOC(H, size16, int, L.nblk + 1, st);
+        AMG_ALLOC(H, off16, int, L.nblk + 1, st);
+        AMG_ALLOC(H, info, int, 2, st);
+        AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 2 * sizeof(int), st));
+        k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
+                                                             q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
+        k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr,
+                                                   0, nullptr, size16, info, L.tiles, nullptr);
+        AMG_CUDA_TRY(H, cudaGetLastError());
+        int h_info[2];
+        AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+        if (h_info[1]) {
+          scale *= 0.5;
+        } else if (h_info[0] > RT_STAGE_BYTES) {
+          scale *= 0.96 * (double)RT_STAGE_BYTES / (double)h_info[0];
+        } else {
+          AMG_TRY(amg_exclusive_scan(H, size16, off16, L.nblk, st));
+          int total16 = 0;
+          AMG_TRY(read_int(H, off16 + L.nblk, &total16, st));
+          L.blob_bytes = (size_t)total16 * 16u;
+          L.blob = (unsigned char*)amg_dev_alloc(H, L.blob_bytes + 16, st);
+          if (!L.blob) {
+            H->err = "device allocation failed: tile blobs";
+            return AMG_ERR_OOM;
+          }
+          k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val,
+                                                     q < Lc ? L.agg : nullptr, 1, off16, size16, info, L.tiles, L.blob);
+          AMG_CUDA_TRY(H, cudaGetLastError());
+          AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+          L.fast = 1;
+        }
+        amg_dev_free(H, size16);
+        amg_dev_free(H, off16);
+        amg_dev_free(H, info);
+      }
+      if (!L.fast) {
+        if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
+        if (L.tiles) amg_dev_free(H, L.tiles);
+        L.blk_ptr = nullptr, L.tiles = nullptr, L.nblk = 0;
       }
     }
     L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));

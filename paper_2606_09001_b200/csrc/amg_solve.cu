@@ -68,7 +68,7 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
   a.dinv = L.dinv;
   a.agg = L.agg;
   a.agg_ptr = L.agg_ptr;
-  a.lpr2 = L.lpr2;
+  a.blob = L.blob;
   a.gamma = H->opt.coarse_scale;
   a.partials = H->partials;
   a.counter = H->counter;

@@ -1,69 +1,101 @@
-// Tile-packed operator format of a level ("TP-CSR") -- the HBM layout the solve-phase row kernels
-// stream.  Shared by the packer (amg_pack.cu) and the kernels (amg_kernels.cuh).
+// Tile-packed operator format of a level ("sorted-ELL tiles") -- the HBM layout the solve-phase
+// row kernels stream (DESIGN.md §5/§6).  Shared by the packer (amg_setup.cu) and the kernels
+// (amg_kernels.cuh); nothing here is part of the C ABI.
 //
-// A level's rows are cut into tiles of consecutive rows (boundaries on aggregate starts).  Each
-// tile owns ONE contiguous, 16-byte aligned blob, fetched by a single bulk-async copy (TMA):
+// A level's rows (aggregate-contiguous numbering) are cut into tiles of consecutive rows with
+// boundaries on aggregate starts.  Each tile owns ONE contiguous, 16-byte aligned blob that a single
+// bulk-async copy (TMA) brings into a ring stage:
 //
-//   section A  val   f64[nnz]      matrix values, row-major, ascending columns within a row
-//              col   u16[nnz]      LOCAL column: < nrows -> row r0+col of this tile,
-//                                  >= nrows -> entry (col - nrows) of the tile's halo list
-//              roff  u16[nrows+1]  local row offsets into val / col
-//              halo  i32[nhalo]    level index of every distinct out-of-tile column, ascending
-//              aoff  u16[nagg+1]   local first row of every aggregate of the tile (restriction)
-//   section B  dinv  f64[nrows]    smoother diagonal
-//   section C  aggl  u16[nrows]    local aggregate of every row   (prolongation)
-//              hagg  i32[nhalo]    coarse index of every halo column (prolongation)
+//   slices  int2[nsl]      {first slot, width} of every slice of 32 storage rows
+//   halo    i32[nhalo]     level index of every distinct out-of-tile column, ascending
+//   perm    u16[32 nsl]    storage row -> tile-local row (0xFFFF: padding).  Storage rows are the
+//                          tile's rows sorted by descending length (stable), so the 32 rows of a
+//                          slice have (almost) the same length and the padding stays at a few %
+//   col     u16[nslots]    TILE-LOCAL column of every slot: < nr -> row r0+col of this tile,
+//                          >= nr -> entry (col - nr) of the halo list.  Slice-major; inside a slice
+//                          k-major: slot = first + 32 k + lane  (conflict-free shared-memory reads)
+//   val     f64[nslots]    matrix values, same order; padding slots are {col 0, val 0}
+//   cagg    i32[nhalo]     coarse index of every halo column (prolongation-fused sweep only)
 //
-// SpMV / residual+restriction copy A, the Jacobi sweeps A+B, the prolongation-fused sweep A+B+C:
-// always one prefix of the blob.  Every sub-array starts on a 16-byte boundary.
-// 10 bytes per nonzero instead of CSR's 12, and the out-of-tile x values are fetched once per
-// distinct column into shared memory, so the inner loop reads shared memory only.
+// 10 bytes per stored entry instead of CSR's 12 (+4 per row), no row pointers; the x values of
+// the halo columns are fetched ONCE per distinct column into shared memory by dedicated warps, one
+// tile ahead of the row walk, so the inner loop reads shared memory only.  Within a row the
+// entries keep their CSR order (ascending column of the level numbering), so a row sum is
+// accumulated in the same order as by the CSR kernels and by the oracle.
 #pragma once
 #include <stdint.h>
 
-#ifndef __host__
-#define __host__
-#define __device__
-#endif
-
-struct alignas(16) PackDesc {   // 32 bytes per tile, read by the issuing thread one tile ahead
-  uint32_t off16;               // blob offset in 16-byte units
-  int32_t r0;                   // first row
-  int32_t I0;                   // first coarse row (aggregate) of the tile
-  int32_t nnz;
-  uint16_t nrows, nhalo, nagg, pad0;
-  int32_t pad1, pad2;
-};
-
-struct PackLayout {             // byte offsets inside the blob; all multiples of 16
-  int o_val, o_col, o_roff, o_halo, o_aoff, endA;
-  int o_dinv, endB;
-  int o_aggl, o_hagg, endC;
+struct alignas(16) TileDesc {  // 32 bytes per tile, read by the issuing thread
+  int32_t r0, nr;              // rows [r0, r0 + nr)
+  int32_t I0, nA;              // coarse rows [I0, I0 + nA); nA = 0 on the coarsest level
+  int32_t nsl, nslots;         // slices; stored slots (= sum of 32 * width)
+  int32_t nhalo;
+  uint32_t blob16;             // blob offset in 16-byte units
 };
 
 __host__ __device__ inline int tp_up(int x, int m) { return (x + m - 1) / m * m; }
 
-__host__ __device__ inline PackLayout tp_layout(int nnz, int nrows, int nhalo, int nagg) {
-  PackLayout p;
-  p.o_val = 0;
-  p.o_col = p.o_val + tp_up(nnz, 2) * 8;
-  p.o_roff = p.o_col + tp_up(nnz, 8) * 2;
-  p.o_halo = p.o_roff + tp_up(nrows + 1, 8) * 2;
-  p.o_aoff = p.o_halo + tp_up(nhalo, 4) * 4;
-  p.endA = p.o_aoff + tp_up(nagg + 1, 8) * 2;
-  p.o_dinv = p.endA;
-  p.endB = p.o_dinv + tp_up(nrows, 2) * 8;
-  p.o_aggl = p.endB;
-  p.o_hagg = p.o_aggl + tp_up(nrows, 8) * 2;
-  p.endC = p.o_hagg + tp_up(nhalo, 4) * 4;
+struct BlobLayout {  // byte offsets inside the blob; all multiples of 16
+  int o_halo, o_perm, o_col, o_val, endA, o_cagg, endB;
+};
+__host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots, int nhalo) {
+  BlobLayout p;
+  p.o_halo = tp_up(8 * nsl, 16);
+  p.o_perm = p.o_halo + tp_up(4 * nhalo, 16);
+  p.o_col = p.o_perm + 64 * nsl;
+  p.o_val = p.o_col + tp_up(2 * nslots, 16);
+  p.endA = p.o_val + 8 * nslots;
+  p.o_cagg = p.endA;
+  p.endB = p.o_cagg + tp_up(4 * nhalo, 16);
   return p;
 }
 
-// Shared-memory bytes one ring stage needs for a tile, for the most demanding operation (the
-// prolongation-fused sweep): blob prefix A+B+C, then xs[nrows+nhalo] (+2: the 16-byte rounding
-// of the x slice), h2[nhalo], b[nrows] (+2), ec[nagg] (+2).  The partitioner keeps this below
-// the stage size; other operations need less.
-__host__ __device__ inline int tp_stage_need(int nnz, int nrows, int nhalo, int nagg) {
-  const PackLayout p = tp_layout(nnz, nrows, nhalo, nagg);
-  return p.endC + 8 * (tp_up(nrows + nhalo + 2, 2) + tp_up(nhalo, 2) + tp_up(nrows + 2, 2) + tp_up(nagg + 2, 2));
+// Placement of a tile inside its ring stage, after the TP_DESC_BYTES stage header.  Row-vector
+// slices are rounded out to 16-byte boundaries of their source arrays (bulk copies need 16-byte
+// aligned addresses and sizes): ra2 / ra4 / Ia2 / Ia4 are the rounded-down first elements.
+constexpr int TP_DESC_BYTES = 128;
+struct StageLayout {
+  int ra2, nrv;    // first staged row of the f64 row vectors (even), entries staged (even)
+  int ra4, nr4;    // same for the i32 agg slice (multiple of 4)
+  int Ia2, nec;    // coarse-vector slice
+  int Ia4, nap;    // agg_ptr slice (nA + 1 entries from I0)
+  int o_b, o_d, o_agg, o_ec, o_xcat, o_out, end;  // byte offsets (blob at 0)
+};
+// flags: which operands the operation stages
+enum { TP_B = 1, TP_D = 2, TP_AGG = 4, TP_EC = 8, TP_AGGPTR = 16, TP_CAGG = 32, TP_OUT = 64 };
+__host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
+  StageLayout t;
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  const int r1 = d.r0 + d.nr;
+  t.ra2 = d.r0 & ~1;
+  t.nrv = tp_up(r1 - t.ra2, 2);
+  t.ra4 = d.r0 & ~3;
+  t.nr4 = tp_up(r1 - t.ra4, 4);
+  t.Ia2 = d.I0 & ~1;
+  t.nec = tp_up(d.I0 + d.nA - t.Ia2, 2);
+  t.Ia4 = d.I0 & ~3;
+  t.nap = tp_up(d.I0 + d.nA + 1 - t.Ia4, 4);
+  int o = (flags & TP_CAGG) ? p.endB : p.endA;
+  t.o_b = o;
+  if (flags & TP_B) o += 8 * t.nrv;
+  t.o_d = o;
+  if (flags & TP_D) o += 8 * t.nrv;
+  t.o_agg = o;
+  if (flags & TP_AGG) o += 4 * t.nr4;
+  if (flags & TP_AGGPTR) o += 4 * t.nap;
+  t.o_ec = o;
+  if (flags & TP_EC) o += 8 * t.nec;
+  t.o_xcat = o;  // [x slice (nrv, rounded) | halo values]: index roff + col
+  o += 8 * tp_up(t.nrv + d.nhalo, 2);
+  t.o_out = o;
+  if (flags & TP_OUT) o += 8 * tp_up(d.nr, 2);
+  t.end = o;
+  return t;
+}
+constexpr int TP_FLAGS_JACP = TP_B | TP_D | TP_AGG | TP_EC | TP_CAGG;  // prolongation-fused sweep
+constexpr int TP_FLAGS_RESTRICT = TP_B | TP_AGGPTR | TP_OUT;           // residual + restriction
+// shared-memory bytes one ring stage needs for a tile, for the most demanding operations
+__host__ __device__ inline int tp_stage_need(const TileDesc& d) {
+  const int a = tp_stage(d, TP_FLAGS_JACP).end, b = tp_stage(d, TP_FLAGS_RESTRICT).end;
+  return TP_DESC_BYTES + (a > b ? a : b);
 }
