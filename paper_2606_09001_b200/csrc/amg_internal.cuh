@@ -123,6 +123,11 @@ struct amg_handle_s {
   int tail_grid = 0;
   void* d_tail = nullptr;            // TailLevel[levels] on the device
   unsigned long long* tail_bar = nullptr;
+  void* d_tail_chunk = nullptr;      // TailChunk[levels][tail_grid]
+  int tail_dense_level = -1;         // levels >= this are applied as the dense operator tail_dense_B
+  double* tail_dense_B = nullptr;
+  int tail_lu_smem = 0;              // dynamic shared memory: LU scratch, then the staged operator chunks
+  int tail_smem = 0;
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
   cudaGraphExec_t graph_exec[4] = {nullptr, nullptr, nullptr, nullptr};
   int64_t graph_launches[4] = {0, 0, 0, 0};  // kernel nodes per replay

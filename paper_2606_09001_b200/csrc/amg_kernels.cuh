@@ -676,12 +676,13 @@ __global__ void k_lu_solve(int n, const double* __restrict__ lu, const int* __re
 // memory and ONE warp runs both substitutions, lane i owning rows i, i+32, ...: no block-wide
 // barrier inside the 2n dependent steps.  `sm` holds n*(n+1) + n doubles.
 constexpr int LU_SMALL_MAX = 72;  // 72*73*8 + 72*8 bytes < 48 KB
+template <bool CG>  // CG: b was written by other CTAs of this kernel (read through L2)
 __device__ __forceinline__ void lu_solve_small_cta(int n, const double* __restrict__ lu, const int* __restrict__ piv,
                                                    const double* b, double* x, double* sm) {
   const int tid = threadIdx.x, T = blockDim.x, P = n + 1;
   double* y = sm + (size_t)n * P;
   for (int t = tid; t < n * n; t += T) sm[(t / n) * P + (t % n)] = __ldg(lu + t);
-  for (int i = tid; i < n; i += T) y[i] = __ldcg(b + i);
+  for (int i = tid; i < n; i += T) y[i] = CG ? __ldcg(b + i) : b[i];
   __syncthreads();
   if (tid < 32) {
     const int lane = tid;
@@ -718,7 +719,7 @@ __global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __r
                                                         double* __restrict__ x, const KrylovCtl* ctl) {
   if (ctl != nullptr && ctl->done) return;
   extern __shared__ double lu_sm[];
-  lu_solve_small_cta(n, lu, piv, b, x, lu_sm);
+  lu_solve_small_cta<true>(n, lu, piv, b, x, lu_sm);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -162,6 +162,7 @@ double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin
   TailArgs a;
   memset(&a, 0, sizeof(a));
   a.lv = (const TailLevel*)H->d_tail;
+  a.chunk = (const TailChunk*)H->d_tail_chunk;
   a.first = l;
   a.last = Lc;
   a.b_first = b;
@@ -171,13 +172,17 @@ double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin
   a.nL = H->nL;
   a.lu = H->lu;
   a.piv = H->piv;
+  a.dense_level = H->tail_dense_level;
+  a.dense_B = H->tail_dense_B;
   a.bar = H->tail_bar;
   a.partials = H->partials;
   a.ctl = ctl;
   a.fin = fin;
-  ++g_nlaunch, k_vcycle_tail<<<H->tail_grid, TAIL_THREADS, tail_smem_bytes(H->nL), st>>>(a);
+  a.lu_smem = H->tail_lu_smem;
+  ++g_nlaunch, k_vcycle_tail<<<H->tail_grid, TAIL_THREADS, H->tail_smem, st>>>(a);
   Level& L = H->lv[l];
-  if (l == Lc) return L.x;
+  const bool dense = H->tail_dense_level >= 0 && l <= H->tail_dense_level;
+  if (l == (dense ? H->tail_dense_level : Lc)) return L.x;
   return tail_result_in_x2(a.nu1, a.nu2) ? L.x2 : L.x;
 }
 
@@ -185,12 +190,26 @@ double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin
 
 amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
   H->tail_first = -1;
+  H->tail_dense_level = -1;
   const int nlev = (int)H->lv.size();
+  const int Lc = nlev - 1;
   if (H->opt.tail_max_rows <= 0 || H->opt.force_generic || nlev > TAIL_MAX_LEVELS) return AMG_OK;
   int first = nlev;
   while (first > 0 && H->lv[first - 1].n <= H->opt.tail_max_rows) --first;
   if (first >= nlev) return AMG_OK;
+  const int G = H->sm_count;  // one resident CTA per SM: the grid barrier needs co-residency
+  // the dense collapsed operator replaces the levels from D down
+  int D = -1;
+  if (H->opt.tail_dense_rows > 0)
+    for (int l = first; l < nlev; ++l)
+      if (H->lv[l].n <= H->opt.tail_dense_rows && H->lv[l].n <= MAX_DENSE) {
+        D = l;
+        break;
+      }
+  // ---- per level: row chunks of the CTAs (aggregate boundaries, balanced by nonzeros) ----
   std::vector<TailLevel> h(nlev);
+  std::vector<TailChunk> hc((size_t)nlev * G);
+  memset(hc.data(), 0, sizeof(TailChunk) * hc.size());
   for (int l = 0; l < nlev; ++l) {
     const Level& L = H->lv[l];
     TailLevel& T = h[l];
@@ -208,15 +227,88 @@ amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
     T.b = L.b;
     T.x = L.x;
     T.x2 = L.x2;
+    T.s_rp = T.s_col = T.s_val = T.s_dinv = -1;
   }
+  H->tail_lu_smem = (int)((tail_smem_bytes(H->nL) + 127) & ~(size_t)127);
+  int stage_used = 0;
+  std::vector<int> rp, ap;
+  for (int l = first; l < Lc; ++l) {
+    const Level& L = H->lv[l];
+    rp.resize(L.n + 1);
+    ap.resize(L.nc + 1);
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(rp.data(), L.rowptr, sizeof(int) * (L.n + 1), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(ap.data(), L.agg_ptr, sizeof(int) * (L.nc + 1), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    int I = 0;
+    int m_rp = 0, m_k4 = 0, m_k2 = 0, m_r2 = 0;
+    for (int c = 0; c < G; ++c) {
+      TailChunk& ch = hc[(size_t)l * G + c];
+      const int64_t want_end = (int64_t)(c + 1) * L.nnz / G;
+      ch.A0 = I;
+      while (I < L.nc && (c == G - 1 || rp[ap[I]] < want_end)) ++I;
+      ch.A1 = I;
+      ch.R0 = ap[ch.A0];
+      ch.R1 = ap[ch.A1];
+      ch.K0 = rp[ch.R0];
+      ch.K1 = rp[ch.R1];
+      const TailSlices s = tail_slices(ch);
+      m_rp = std::max(m_rp, s.nrp), m_k4 = std::max(m_k4, s.nk4), m_k2 = std::max(m_k2, s.nk2), m_r2 = std::max(m_r2, s.nr2);
+    }
+    // staging offsets (the same in every CTA); levels the dense operator replaces are only staged
+    // for calls that start below it, which are hooks: not worth shared memory
+    const int need = 4 * m_rp + 4 * m_k4 + 8 * m_k2 + 8 * m_r2 + 64;
+    if ((D < 0 || l < D) && stage_used + need <= TAIL_STAGE_BUDGET) {
+      TailLevel& T = h[l];
+      int o = stage_used;
+      T.s_val = o, o += 8 * m_k2;
+      T.s_dinv = o, o += 8 * m_r2;
+      T.s_rp = o, o += 4 * m_rp;
+      T.s_col = o, o += 4 * m_k4;
+      stage_used = (o + 15) & ~15;
+    }
+  }
+  H->tail_smem = H->tail_lu_smem + stage_used;
   TailLevel* d;
+  TailChunk* dc;
   AMG_ALLOC(H, d, TailLevel, nlev, st);
+  AMG_ALLOC(H, dc, TailChunk, hc.size(), st);
   AMG_CUDA_TRY(H, cudaMemcpyAsync(d, h.data(), sizeof(TailLevel) * nlev, cudaMemcpyHostToDevice, st));
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(dc, hc.data(), sizeof(TailChunk) * hc.size(), cudaMemcpyHostToDevice, st));
   AMG_ALLOC(H, H->tail_bar, unsigned long long, 32, st);
   AMG_CUDA_TRY(H, cudaMemsetAsync(H->tail_bar, 0, sizeof(unsigned long long) * 32, st));
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));  // h goes out of scope
+  // the attribute is per function, not per handle: opt in to the most any handle can ask for
+  AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_vcycle_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
   H->d_tail = d;
-  H->tail_grid = H->sm_count;  // one resident CTA per SM: the grid barrier needs co-residency
+  H->d_tail_chunk = dc;
+  H->tail_grid = G;
+  // ---- dense collapsed operator: column j = V-cycle of levels D.. on e_j ----
+  if (D >= 0) {
+    const int nD = H->lv[D].n;
+    size_t vec_bytes = 0;
+    for (int l = D; l < nlev; ++l) vec_bytes += 3 * sizeof(double) * (size_t)H->lv[l].n;
+    const size_t smem = (size_t)H->tail_lu_smem + vec_bytes;
+    if (smem <= 200 * 1024) {
+      AMG_ALLOC(H, H->tail_dense_B, double, (size_t)nD * nD, st);
+      TailBuildArgs ba;
+      memset(&ba, 0, sizeof(ba));
+      ba.lv = d;
+      ba.D = D;
+      ba.last = Lc;
+      ba.nu1 = H->opt.pre_sweeps;
+      ba.nu2 = H->opt.post_sweeps;
+      ba.gamma = H->opt.coarse_scale;
+      ba.nL = H->nL;
+      ba.lu = H->lu;
+      ba.piv = H->piv;
+      ba.B = H->tail_dense_B;
+      ba.lu_smem = H->tail_lu_smem;
+      AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_tail_dense_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+      k_tail_dense_build<<<nD, TAILB_THREADS, smem, st>>>(ba);
+      AMG_CUDA_TRY(H, cudaGetLastError());
+      H->tail_dense_level = D;
+    }
+  }
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));  // h / hc go out of scope
   H->tail_first = first;
   return AMG_OK;
 }

@@ -1,20 +1,28 @@
 // Coarse tail of the V-cycle (S2-S6 on the small levels): ONE persistent kernel runs every level
 // from `first` down to the coarsest solve and back up.  The levels below ~64 k rows hold < 3 % of
-// the V-cycle's bytes but three quarters of its kernel launches; each of those launches costs
-// 8-11 us (launch + pipeline fill + reduction tail) for < 1 us of memory time.  Here the CTAs
-// stay resident (one per SM), the operators are read from L2, and the dependency between two
-// passes is a grid-wide barrier (~1 us: one atomic arrival per CTA, one polled release flag)
-// instead of a kernel boundary.
+// the V-cycle's bytes but three quarters of its kernel launches, and every pass over them is a
+// chain of dependent memory round trips, not a bandwidth problem.  Three measures:
 //
-// Work split: LPR lanes per row (per aggregate for the restriction: its rows are contiguous, so
-// its nonzeros are ONE contiguous range); rows are dealt round-robin to the sub-warps of the grid.
-// Vectors written inside the kernel are read with ld.global.cg (L2) -- L1 is not coherent across
-// CTAs; the operator arrays are read-only for the whole kernel and go through L1.
+//  * the CTAs stay resident (one per SM) and the dependency between two passes is a grid-wide
+//    barrier (one atomic arrival per CTA, one polled release flag) instead of a kernel boundary;
+//  * every CTA owns a FIXED contiguous chunk of each level's rows (cut on aggregate starts,
+//    balanced by nonzeros) and copies its slice of that level's operator (rowptr / col / val /
+//    dinv) into shared memory once, at kernel start, with bulk-async copies (TMA): the four passes
+//    over a level then read the operator at shared-memory latency, and only the x gathers (values
+//    written by other CTAs in the previous pass) go to L2;
+//  * the levels with at most `tail_dense_rows` rows are not visited at all: the V-cycle from level
+//    D down is a fixed linear operator z = B_D r, assembled once at setup as a dense matrix (by
+//    running that V-cycle on the unit vectors) and applied as one dense matrix-vector product
+//    spread over all CTAs -- 1 pass instead of 4 passes x 5 levels + the LU solve.
+//
+// Vectors written inside the kernel are read with ld.global.cg (L2): L1 is not coherent across
+// CTAs.  No floating-point atomics: every sum has a fixed order for a fixed grid.
 #pragma once
 #include "amg_kernels.cuh"
 
-constexpr int TAIL_THREADS = 512;
+constexpr int TAIL_THREADS = 1024;
 constexpr int TAIL_MAX_LEVELS = 32;
+constexpr int TAIL_STAGE_BUDGET = 176 * 1024;  // shared memory for the staged operator chunks
 
 struct TailLevel {
   int n, nc, nnz, lpr;
@@ -27,21 +35,31 @@ struct TailLevel {
   double* b;   // right-hand side buffer of this level (unused for the level the call starts at)
   double* x;
   double* x2;
+  // staging of this level's chunks (same offsets in every CTA; -1: not staged, read through L1)
+  int s_rp, s_col, s_val, s_dinv;
+};
+
+struct TailChunk {  // rows [R0, R1), nonzeros [K0, K1), aggregates [A0, A1) of one CTA on one level
+  int R0, R1, K0, K1, A0, A1, pad0, pad1;
 };
 
 struct TailArgs {
-  const TailLevel* lv;   // device array indexed by level
-  int first, last;       // first level of the call, coarsest level
-  const double* b_first; // right-hand side of level `first`
+  const TailLevel* lv;     // device array indexed by level
+  const TailChunk* chunk;  // [level][gridDim.x]
+  int first, last;         // first level of the call, coarsest level
+  const double* b_first;   // right-hand side of level `first`
   int nu1, nu2;
   double gamma;
   int nL;
   const double* lu;
   const int* piv;
+  int dense_level;         // -1: none; else levels >= dense_level are applied as dense_B
+  const double* dense_B;   // [nD x nD] row-major
   unsigned long long* bar;  // [0] arrival counter, [16] release generation
   double* partials;
   KrylovCtl* ctl;           // may be null (hooks)
   int fin;                  // FIN_RZ: b_first . result is reduced and finalised (first == 0 only)
+  int lu_smem;              // bytes reserved at the start of dynamic shared memory for the LU solve
 };
 
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
@@ -75,43 +93,68 @@ __device__ __forceinline__ void tail_grid_barrier(unsigned long long* bar) {
 
 enum TailOp { T_JAC0 = 0, T_JAC = 1, T_JACP = 2, T_SCALE = 3, T_ZERO = 4, T_PROLONG = 5 };
 
-// one smoother-type pass over the rows of a level; returns this thread's share of b . out
-template <int OP>
-__device__ __forceinline__ double tail_row_pass(const TailLevel& L, const double* b, const double* x,
-                                                const double* ec, double gamma, double* out, bool want_dot) {
-  const int lpr = L.lpr;
-  const int gsub = (blockIdx.x * TAIL_THREADS + threadIdx.x) / lpr;
-  const int sub = threadIdx.x & (lpr - 1);
-  const int nsub = gridDim.x * TAIL_THREADS / lpr;
-  const int n = L.n;
+// vector loads: CG = written by other CTAs during this kernel (L2); else plain (shared memory /
+// CTA-private data)
+template <bool CG>
+__device__ __forceinline__ double tl_ld(const double* p) {
+  return CG ? __ldcg(p) : *p;
+}
+
+// Operator of one level as seen by one group of threads: generic pointers, indexed by the
+// level's own row / nonzero numbers (shared-memory copies are biased accordingly).  rp / col /
+// val / dinv may point into shared memory (the group's own rows only); dinv_g / agg are the
+// level's global arrays (read-only during the kernel: L1), used for the column gathers.
+struct TailOpView {
+  const int* rp;
+  const int* col;
+  const double* val;
+  const double* dinv;
+  const double* dinv_g;
+  const int* agg;
+  const int* agg_ptr;
+  int lpr;
+};
+
+// one smoother-type pass over rows [R0, R1) by the T threads of a group (this thread is t);
+// returns this thread's share of b . out
+template <int OP, bool CG>
+__device__ __forceinline__ double tl_row_pass(const TailOpView& A, int R0, int R1, int t, int T, const double* b,
+                                              const double* x, const double* ec, double gamma, double* out,
+                                              bool want_dot) {
+  const int lpr = A.lpr;
+  const int g = t / lpr, sub = t & (lpr - 1), ng = T / lpr;
   double dot = 0.0;
-  const int trips = (n + nsub - 1) / nsub;  // every lane of a warp runs the same number of trips
-  for (int t = 0; t < trips; ++t) {
-    const int i = gsub + t * nsub;
-    double s = 0.0;
-    if (i < n) {
-      for (int k = __ldg(L.rowptr + i) + sub, e = __ldg(L.rowptr + i + 1); k < e; k += lpr) {
-        const int c = __ldg(L.col + k);
+  const int trips = (R1 - R0 + ng - 1) / ng;  // every lane of a warp runs the same number of trips
+  for (int q = 0; q < trips; ++q) {
+    const int i = R0 + g + q * ng;
+    const bool act = i < R1;
+    double s = 0.0, di = 0.0, bi = 0.0, xi = 0.0;
+    if (act) {
+      const int k0 = A.rp[i], k1 = A.rp[i + 1];
+      if (sub == 0) {  // own-row operands: issued before the gathers, consumed after the reduction
+        di = A.dinv[i];
+        bi = tl_ld<CG>(b + i);
+        if (OP == T_JAC0)
+          xi = di * bi;
+        else if (OP == T_JACP)
+          xi = tl_ld<CG>(x + i) + gamma * tl_ld<CG>(ec + __ldg(A.agg + i));
+        else
+          xi = tl_ld<CG>(x + i);
+      }
+      for (int k = k0 + sub; k < k1; k += lpr) {
+        const int c = A.col[k];
         double xc;
         if (OP == T_JAC0)
-          xc = __ldg(L.dinv + c) * __ldcg(b + c);
+          xc = __ldg(A.dinv_g + c) * tl_ld<CG>(b + c);
         else if (OP == T_JACP)
-          xc = __ldcg(x + c) + gamma * __ldcg(ec + __ldg(L.agg + c));
+          xc = tl_ld<CG>(x + c) + gamma * tl_ld<CG>(ec + __ldg(A.agg + c));
         else
-          xc = __ldcg(x + c);
-        s += __ldg(L.val + k) * xc;
+          xc = tl_ld<CG>(x + c);
+        s += A.val[k] * xc;
       }
     }
     for (int o = lpr >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (i < n && sub == 0) {
-      const double di = __ldg(L.dinv + i), bi = __ldcg(b + i);
-      double xi;
-      if (OP == T_JAC0)
-        xi = di * bi;
-      else if (OP == T_JACP)
-        xi = __ldcg(x + i) + gamma * __ldcg(ec + __ldg(L.agg + i));
-      else
-        xi = __ldcg(x + i);
+    if (act && sub == 0) {
       const double o = xi + di * (bi - s);
       out[i] = o;
       if (want_dot) dot += bi * o;
@@ -120,53 +163,54 @@ __device__ __forceinline__ double tail_row_pass(const TailLevel& L, const double
   return dot;
 }
 
-// vector-only passes (nu1 < 2 or nu2 == 0)
-template <int OP>
-__device__ __forceinline__ double tail_vec_pass(const TailLevel& L, const double* b, const double* x,
-                                                const double* ec, double gamma, double* out, bool want_dot) {
+// vector-only passes (nu1 < 2 or nu2 == 0) over rows [R0, R1)
+template <int OP, bool CG>
+__device__ __forceinline__ double tl_vec_pass(const TailOpView& A, int R0, int R1, int t, int T, const double* b,
+                                              const double* x, const double* ec, double gamma, double* out,
+                                              bool want_dot) {
   double dot = 0.0;
-  for (int i = blockIdx.x * TAIL_THREADS + threadIdx.x; i < L.n; i += gridDim.x * TAIL_THREADS) {
+  for (int i = R0 + t; i < R1; i += T) {
     double o;
     if (OP == T_SCALE)
-      o = __ldg(L.dinv + i) * __ldcg(b + i);
+      o = A.dinv[i] * tl_ld<CG>(b + i);
     else if (OP == T_ZERO)
       o = 0.0;
     else
-      o = __ldcg(x + i) + gamma * __ldcg(ec + __ldg(L.agg + i));
+      o = tl_ld<CG>(x + i) + gamma * tl_ld<CG>(ec + __ldg(A.agg + i));
     out[i] = o;
-    if (want_dot) dot += __ldcg(b + i) * o;
+    if (want_dot) dot += tl_ld<CG>(b + i) * o;
   }
   return dot;
 }
 
-// rc[I] = sum_{i in I} (b_i - sum_j a_ij x_j): the rows of I are consecutive, so the sum over the
-// nonzeros of all its rows is one contiguous range
-__device__ __forceinline__ void tail_restrict_pass(const TailLevel& L, const double* b, const double* x, double* rc) {
-  const int lpr = L.lpr;
-  const int gsub = (blockIdx.x * TAIL_THREADS + threadIdx.x) / lpr;
-  const int sub = threadIdx.x & (lpr - 1);
-  const int nsub = gridDim.x * TAIL_THREADS / lpr;
-  const int nc = L.nc;
-  const int trips = (nc + nsub - 1) / nsub;
-  for (int t = 0; t < trips; ++t) {
-    const int I = gsub + t * nsub;
+// rc[I] = sum_{i in I} (b_i - sum_j a_ij x_j) for aggregates [A0, A1): the rows of I are
+// consecutive, so the sum over the nonzeros of all its rows is one contiguous range
+template <bool CG>
+__device__ __forceinline__ void tl_restrict_pass(const TailOpView& A, int A0, int A1, int t, int T, const double* b,
+                                                 const double* x, double* rc) {
+  const int lpr = A.lpr;
+  const int g = t / lpr, sub = t & (lpr - 1), ng = T / lpr;
+  const int trips = (A1 - A0 + ng - 1) / ng;
+  for (int q = 0; q < trips; ++q) {
+    const int I = A0 + g + q * ng;
+    const bool act = I < A1;
     double s = 0.0;
-    if (I < nc) {
-      const int ra = __ldg(L.agg_ptr + I), rb = __ldg(L.agg_ptr + I + 1);
-      for (int k = __ldg(L.rowptr + ra) + sub, e = __ldg(L.rowptr + rb); k < e; k += lpr)
-        s -= __ldg(L.val + k) * __ldcg(x + __ldg(L.col + k));
-      for (int i = ra + sub; i < rb; i += lpr) s += __ldcg(b + i);
+    if (act) {
+      const int ra = __ldg(A.agg_ptr + I), rb = __ldg(A.agg_ptr + I + 1);
+      for (int k = A.rp[ra] + sub, e = A.rp[rb]; k < e; k += lpr) s -= A.val[k] * tl_ld<CG>(x + A.col[k]);
+      for (int i = ra + sub; i < rb; i += lpr) s += tl_ld<CG>(b + i);
     }
     for (int o = lpr >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (I < nc && sub == 0) rc[I] = s;
+    if (act && sub == 0) rc[I] = s;
   }
 }
 
 // coarsest solve by one CTA for n > LU_SMALL_MAX: factors stay in global memory (L2), y in shared
+template <bool CG>
 __device__ __forceinline__ void lu_solve_big_cta(int n, const double* __restrict__ lu, const int* __restrict__ piv,
                                                  const double* b, double* x, double* y) {
   const int tid = threadIdx.x, T = blockDim.x;
-  for (int i = tid; i < n; i += T) y[i] = __ldcg(b + i);
+  for (int i = tid; i < n; i += T) y[i] = tl_ld<CG>(b + i);
   __syncthreads();
   if (tid == 0)
     for (int k = 0; k < n; ++k) {
@@ -204,80 +248,180 @@ __host__ __device__ inline bool tail_result_in_x2(int nu1, int nu2) {
   return swaps & 1;
 }
 
+// aligned slices of a chunk (bulk copies need 16-byte aligned sources and sizes)
+struct TailSlices {
+  int ra4, nrp, ka4, nk4, ka2, nk2, ra2, nr2;
+};
+__host__ __device__ inline TailSlices tail_slices(const TailChunk& c) {
+  TailSlices s;
+  s.ra4 = c.R0 & ~3;
+  s.nrp = (c.R1 + 1 - s.ra4 + 3) & ~3;
+  s.ka4 = c.K0 & ~3;
+  s.nk4 = (c.K1 - s.ka4 + 3) & ~3;
+  s.ka2 = c.K0 & ~1;
+  s.nk2 = (c.K1 - s.ka2 + 1) & ~1;
+  s.ra2 = c.R0 & ~1;
+  s.nr2 = (c.R1 - s.ra2 + 1) & ~1;
+  return s;
+}
+
+__device__ __forceinline__ TailOpView tail_view(const TailLevel& L, const TailChunk& ch, unsigned char* stage) {
+  TailOpView A;
+  if (L.s_rp >= 0) {
+    const TailSlices s = tail_slices(ch);
+    A.rp = reinterpret_cast<const int*>(stage + L.s_rp) - s.ra4;
+    A.col = reinterpret_cast<const int*>(stage + L.s_col) - s.ka4;
+    A.val = reinterpret_cast<const double*>(stage + L.s_val) - s.ka2;
+    A.dinv = reinterpret_cast<const double*>(stage + L.s_dinv) - s.ra2;
+  } else {
+    A.rp = L.rowptr, A.col = L.col, A.val = L.val, A.dinv = L.dinv;
+  }
+  A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr;
+  return A;
+}
+
+// z = B b over rows [i0, i1) of the dense operator (row-major, n x n); `tpr` threads per row
+template <bool CG>
+__device__ __forceinline__ double tail_dense_rows(int n, const double* __restrict__ B, const double* b, double* z,
+                                                  int i0, int i1, bool want_dot, double* red /*[TAIL_THREADS/32]*/) {
+  const int tid = threadIdx.x, T = blockDim.x;
+  const int nrows = i1 - i0;
+  int RB = 1;  // rows per batch: the smallest power of two >= nrows, at least one warp per row
+  while (RB < nrows && RB < T / 32) RB <<= 1;
+  const int tpr = T / RB;
+  const int wpr = tpr >> 5;  // warps per row
+  double dot = 0.0;
+  for (int rb = i0; rb < i1; rb += RB) {
+    const int r = rb + tid / tpr, t = tid & (tpr - 1);
+    double s = 0.0;
+    if (r < i1) {
+      const double* row = B + (size_t)r * n;
+      for (int j = t; j < n; j += tpr) s += __ldg(row + j) * tl_ld<CG>(b + j);
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((tid & 31) == 0) red[tid >> 5] = s;
+    __syncthreads();
+    if (tid < RB && rb + tid < i1) {
+      double v = 0.0;
+      for (int q = 0; q < wpr; ++q) v += red[tid * wpr + q];
+      z[rb + tid] = v;
+      if (want_dot) dot += tl_ld<CG>(b + rb + tid) * v;
+    }
+    __syncthreads();
+  }
+  return dot;
+}
+
 __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
   if (a.ctl != nullptr && a.ctl->done) return;
-  extern __shared__ double tail_sm[];
+  extern __shared__ __align__(128) unsigned char tail_sm[];
+  __shared__ uint64_t lvbar[TAIL_MAX_LEVELS];
   __shared__ double red[TAIL_THREADS / 32];
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, G = gridDim.x, cta = blockIdx.x;
+  const bool use_dense = a.dense_level >= 0 && a.first <= a.dense_level;
+  const int E = use_dense ? a.dense_level : a.last;  // sparse levels [first, E), then the bottom solve on E
+  unsigned char* stage = tail_sm + a.lu_smem;
   double dot = 0.0;
 
+  // ---- stage this CTA's operator chunks of every sparse level ----
+  if (tid == 0) {
+    for (int l = a.first; l < E; ++l) mbar_init(&lvbar[l], 1);
+    fence_mbar_init();
+    for (int l = a.first; l < E; ++l) {
+      const TailLevel& L = a.lv[l];
+      if (L.s_rp < 0) continue;
+      const TailChunk ch = a.chunk[l * G + cta];
+      if (ch.R1 <= ch.R0) {
+        mbar_arrive(&lvbar[l]);
+        continue;
+      }
+      const TailSlices s = tail_slices(ch);
+      mbar_arrive_expect_tx(&lvbar[l], 4u * s.nrp + 4u * s.nk4 + 8u * s.nk2 + 8u * s.nr2);
+      bulk_g2s<false>(stage + L.s_rp, L.rowptr + s.ra4, 4u * s.nrp, &lvbar[l], 0);
+      bulk_g2s<false>(stage + L.s_col, L.col + s.ka4, 4u * s.nk4, &lvbar[l], 0);
+      bulk_g2s<false>(stage + L.s_val, L.val + s.ka2, 8u * s.nk2, &lvbar[l], 0);
+      bulk_g2s<false>(stage + L.s_dinv, L.dinv + s.ra2, 8u * s.nr2, &lvbar[l], 0);
+    }
+  }
+  __syncthreads();
+
   // ---- down ----
-  for (int l = a.first; l < a.last; ++l) {
+  for (int l = a.first; l < E; ++l) {
     const TailLevel L = a.lv[l];
+    const TailChunk ch = a.chunk[l * G + cta];
+    if (L.s_rp >= 0) mbar_wait(&lvbar[l], 0);
+    const TailOpView A = tail_view(L, ch, stage);
     const double* b = (l == a.first) ? a.b_first : L.b;
     double* cur = L.x;
     double* oth = L.x2;
     int done;
     if (a.nu1 >= 2) {
-      tail_row_pass<T_JAC0>(L, b, nullptr, nullptr, 0.0, cur, false);
+      tl_row_pass<T_JAC0, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 2;
     } else if (a.nu1 == 1) {
-      tail_vec_pass<T_SCALE>(L, b, nullptr, nullptr, 0.0, cur, false);
+      tl_vec_pass<T_SCALE, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 1;
     } else {
-      tail_vec_pass<T_ZERO>(L, b, nullptr, nullptr, 0.0, cur, false);
+      tl_vec_pass<T_ZERO, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 0;
     }
     tail_grid_barrier(a.bar);
     for (int s = done; s < a.nu1; ++s) {
-      tail_row_pass<T_JAC>(L, b, cur, nullptr, 0.0, oth, false);
+      tl_row_pass<T_JAC, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, nullptr, 0.0, oth, false);
       double* t = cur;
       cur = oth;
       oth = t;
       tail_grid_barrier(a.bar);
     }
-    tail_restrict_pass(L, b, cur, a.lv[l + 1].b);
+    tl_restrict_pass<true>(A, ch.A0, ch.A1, tid, TAIL_THREADS, b, cur, a.lv[l + 1].b);
     tail_grid_barrier(a.bar);
   }
 
-  // ---- coarsest ----
+  // ---- bottom: the dense collapsed operator of levels >= E, or the LU solve of the coarsest level ----
   {
-    const TailLevel L = a.lv[a.last];
-    const double* b = (a.last == a.first) ? a.b_first : L.b;
-    if (blockIdx.x == 0) {
+    const TailLevel L = a.lv[E];
+    const double* b = (E == a.first) ? a.b_first : L.b;
+    const bool want = (E == a.first) && a.fin != FIN_NONE;
+    if (use_dense) {
+      const int i0 = (int)((int64_t)cta * L.n / G), i1 = (int)((int64_t)(cta + 1) * L.n / G);
+      dot += tail_dense_rows<true>(L.n, a.dense_B, b, L.x, i0, i1, want, red);
+    } else if (cta == 0) {
       if (a.nL <= LU_SMALL_MAX)
-        lu_solve_small_cta(a.nL, a.lu, a.piv, b, L.x, tail_sm);
+        lu_solve_small_cta<true>(a.nL, a.lu, a.piv, b, L.x, reinterpret_cast<double*>(tail_sm));
       else
-        lu_solve_big_cta(a.nL, a.lu, a.piv, b, L.x, tail_sm);
-      if (a.first == a.last && a.fin != FIN_NONE)
+        lu_solve_big_cta<true>(a.nL, a.lu, a.piv, b, L.x, reinterpret_cast<double*>(tail_sm));
+      if (want)
         for (int i = tid; i < L.n; i += TAIL_THREADS) dot += __ldcg(b + i) * L.x[i];
     }
-    if (a.first < a.last) tail_grid_barrier(a.bar);
+    if (a.first < E) tail_grid_barrier(a.bar);
   }
 
   // ---- up ----
-  for (int l = a.last - 1; l >= a.first; --l) {
+  for (int l = E - 1; l >= a.first; --l) {
     const TailLevel L = a.lv[l];
+    const TailChunk ch = a.chunk[l * G + cta];
+    const TailOpView A = tail_view(L, ch, stage);
     const double* b = (l == a.first) ? a.b_first : L.b;
     const bool top = (l == a.first) && a.fin != FIN_NONE;
     double* cur = tail_down_in_x2(a.nu1) ? L.x2 : L.x;
     double* oth = tail_down_in_x2(a.nu1) ? L.x : L.x2;
     const TailLevel& C = a.lv[l + 1];
-    const double* ec = (l + 1 == a.last) ? C.x : (tail_result_in_x2(a.nu1, a.nu2) ? C.x2 : C.x);
+    const double* ec = (l + 1 == E) ? C.x : (tail_result_in_x2(a.nu1, a.nu2) ? C.x2 : C.x);
     if (a.nu2 >= 1) {
-      dot += tail_row_pass<T_JACP>(L, b, cur, ec, a.gamma, oth, top && a.nu2 == 1);
+      dot += tl_row_pass<T_JACP, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, ec, a.gamma, oth, top && a.nu2 == 1);
       double* t = cur;
       cur = oth;
       oth = t;
       for (int s = 1; s < a.nu2; ++s) {
         tail_grid_barrier(a.bar);
-        dot += tail_row_pass<T_JAC>(L, b, cur, nullptr, 0.0, oth, top && s == a.nu2 - 1);
+        dot += tl_row_pass<T_JAC, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, nullptr, 0.0, oth,
+                                        top && s == a.nu2 - 1);
         t = cur;
         cur = oth;
         oth = t;
       }
     } else {
-      dot += tail_vec_pass<T_PROLONG>(L, b, cur, ec, a.gamma, oth, top);
+      dot += tl_vec_pass<T_PROLONG, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, ec, a.gamma, oth, top);
     }
     if (l > a.first) tail_grid_barrier(a.bar);
   }
@@ -285,6 +429,7 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
   // ---- fused r.z of a cycle that starts at level 0 (small systems: the whole cycle is this kernel) ----
   if (a.fin != FIN_NONE) {
     for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    __syncthreads();
     if ((tid & 31) == 0) red[tid >> 5] = dot;
     __syncthreads();
     if (tid == 0) {
@@ -299,5 +444,118 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
       for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
       if (tid == 0) krylov_finalize(a.ctl, a.fin, s, 0.0);
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Setup of the dense collapsed operator: CTA j runs the V-cycle of levels D..last on the unit
+// vector e_j with every vector in shared memory (operators through L1/L2) and writes column j.
+// B[i][j] = (Vcycle_D e_j)_i, stored row-major, so that z = B r is exactly the V-cycle applied
+// to r up to the rounding of a different summation order.
+// ------------------------------------------------------------------------------------------
+constexpr int TAILB_THREADS = 256;
+struct TailBuildArgs {
+  const TailLevel* lv;
+  int D, last, nu1, nu2;
+  double gamma;
+  int nL;
+  const double* lu;
+  const int* piv;
+  double* B;
+  int lu_smem;
+};
+
+__global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailBuildArgs a) {
+  extern __shared__ __align__(16) unsigned char tb_sm[];
+  double* vec = reinterpret_cast<double*>(tb_sm + a.lu_smem);
+  const int tid = threadIdx.x, j = blockIdx.x;
+  auto vb = [&](int l) {  // b_l, then x_l, x2_l
+    int off = 0;
+    for (int q = a.D; q < l; ++q) off += 3 * a.lv[q].n;
+    return vec + off;
+  };
+  const int nD = a.lv[a.D].n;
+  {
+    double* b = vb(a.D);
+    for (int i = tid; i < nD; i += TAILB_THREADS) b[i] = (i == j) ? 1.0 : 0.0;
+  }
+  __syncthreads();
+  for (int l = a.D; l < a.last; ++l) {
+    const TailLevel L = a.lv[l];
+    TailOpView A;
+    A.rp = L.rowptr, A.col = L.col, A.val = L.val, A.dinv = L.dinv;
+    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr;
+    double* b = vb(l);
+    double* cur = b + L.n;
+    double* oth = cur + L.n;
+    int done;
+    if (a.nu1 >= 2) {
+      tl_row_pass<T_JAC0, false>(A, 0, L.n, tid, TAILB_THREADS, b, nullptr, nullptr, 0.0, cur, false);
+      done = 2;
+    } else if (a.nu1 == 1) {
+      tl_vec_pass<T_SCALE, false>(A, 0, L.n, tid, TAILB_THREADS, b, nullptr, nullptr, 0.0, cur, false);
+      done = 1;
+    } else {
+      tl_vec_pass<T_ZERO, false>(A, 0, L.n, tid, TAILB_THREADS, b, nullptr, nullptr, 0.0, cur, false);
+      done = 0;
+    }
+    __syncthreads();
+    for (int s = done; s < a.nu1; ++s) {
+      tl_row_pass<T_JAC, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, nullptr, 0.0, oth, false);
+      double* t = cur;
+      cur = oth;
+      oth = t;
+      __syncthreads();
+    }
+    tl_restrict_pass<false>(A, 0, L.nc, tid, TAILB_THREADS, b, cur, vb(l + 1));
+    __syncthreads();
+  }
+  {
+    double* b = vb(a.last);
+    double* x = b + a.lv[a.last].n;
+    if (a.nL <= LU_SMALL_MAX)
+      lu_solve_small_cta<false>(a.nL, a.lu, a.piv, b, x, reinterpret_cast<double*>(tb_sm));
+    else
+      lu_solve_big_cta<false>(a.nL, a.lu, a.piv, b, x, reinterpret_cast<double*>(tb_sm));
+    __syncthreads();
+  }
+  for (int l = a.last - 1; l >= a.D; --l) {
+    const TailLevel L = a.lv[l];
+    TailOpView A;
+    A.rp = L.rowptr, A.col = L.col, A.val = L.val, A.dinv = L.dinv;
+    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr;
+    double* b = vb(l);
+    double* x = b + L.n;
+    double* x2 = x + L.n;
+    double* cur = tail_down_in_x2(a.nu1) ? x2 : x;
+    double* oth = tail_down_in_x2(a.nu1) ? x : x2;
+    double* cb = vb(l + 1);
+    const int ncn = a.lv[l + 1].n;
+    const double* ec = (l + 1 == a.last) ? cb + ncn : (tail_result_in_x2(a.nu1, a.nu2) ? cb + 2 * ncn : cb + ncn);
+    if (a.nu2 >= 1) {
+      tl_row_pass<T_JACP, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, ec, a.gamma, oth, false);
+      double* t = cur;
+      cur = oth;
+      oth = t;
+      for (int s = 1; s < a.nu2; ++s) {
+        __syncthreads();
+        tl_row_pass<T_JAC, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, nullptr, 0.0, oth, false);
+        t = cur;
+        cur = oth;
+        oth = t;
+      }
+    } else {
+      tl_vec_pass<T_PROLONG, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, ec, a.gamma, oth, false);
+    }
+    __syncthreads();
+  }
+  {
+    const double* b = vb(a.D);
+    const double* z;
+    if (a.D == a.last)
+      z = b + nD;
+    else
+      z = tail_result_in_x2(a.nu1, a.nu2) ? b + 2 * nD : b + nD;
+    for (int i = tid; i < nD; i += TAILB_THREADS) a.B[(size_t)i * nD + j] = z[i];
   }
 }
