@@ -93,7 +93,7 @@ typedef struct {
                                65536, 0 = off                                                            */
   int32_t tail_dense_rows;  /* inside that kernel, the V-cycle from the first level with at most this many
                                rows down to the coarsest solve is applied as ONE dense operator assembled
-                               at setup (the same linear map); default 1280, 0 = off         */
+                               at setup (the same linear map); default 2304, 0 = off         */
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */

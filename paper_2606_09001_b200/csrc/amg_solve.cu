@@ -2,6 +2,7 @@
 // iteration replayed as a CUDA graph and the convergence test on the device, per-level hooks,
 // gradient (G2), algorithmic byte counts.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "amg_kernels.cuh"
@@ -179,7 +180,23 @@ double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin
   a.ctl = ctl;
   a.fin = fin;
   a.lu_smem = H->tail_lu_smem;
+#ifdef AMG_TAIL_PROFILE
+  static unsigned long long* d_prof = nullptr;
+  if (!d_prof) cudaMalloc(&d_prof, 256 * sizeof(unsigned long long));
+  cudaMemsetAsync(d_prof, 0, 256 * sizeof(unsigned long long), st);
+  a.prof = d_prof;
+#endif
   ++g_nlaunch, k_vcycle_tail<<<H->tail_grid, TAIL_THREADS, H->tail_smem, st>>>(a);
+#ifdef AMG_TAIL_PROFILE
+  if (getenv("AMG_TAIL_PROF")) {
+    unsigned long long hp[256];
+    cudaMemcpyAsync(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost, st);
+    cudaStreamSynchronize(st);
+    fprintf(stderr, "tail first=%d:", l);
+    for (int q = 1; q < 256 && hp[q]; ++q) fprintf(stderr, " %llu", hp[q] - hp[q - 1]);
+    fprintf(stderr, "\n");
+  }
+#endif
   Level& L = H->lv[l];
   const bool dense = H->tail_dense_level >= 0 && l <= H->tail_dense_level;
   if (l == (dense ? H->tail_dense_level : Lc)) return L.x;
@@ -274,8 +291,8 @@ amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
   AMG_ALLOC(H, dc, TailChunk, hc.size(), st);
   AMG_CUDA_TRY(H, cudaMemcpyAsync(d, h.data(), sizeof(TailLevel) * nlev, cudaMemcpyHostToDevice, st));
   AMG_CUDA_TRY(H, cudaMemcpyAsync(dc, hc.data(), sizeof(TailChunk) * hc.size(), cudaMemcpyHostToDevice, st));
-  AMG_ALLOC(H, H->tail_bar, unsigned long long, 32, st);
-  AMG_CUDA_TRY(H, cudaMemsetAsync(H->tail_bar, 0, sizeof(unsigned long long) * 32, st));
+  AMG_ALLOC(H, H->tail_bar, unsigned long long, G + 64, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(H->tail_bar, 0, sizeof(unsigned long long) * (G + 64), st));
   // the attribute is per function, not per handle: opt in to the most any handle can ask for
   AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_vcycle_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
   H->d_tail = d;

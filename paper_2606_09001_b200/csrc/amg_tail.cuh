@@ -22,6 +22,9 @@
 
 constexpr int TAIL_THREADS = 1024;
 constexpr int TAIL_MAX_LEVELS = 32;
+#ifndef TAIL_POLL_NS
+#define TAIL_POLL_NS 100
+#endif
 constexpr int TAIL_STAGE_BUDGET = 176 * 1024;  // shared memory for the staged operator chunks
 
 struct TailLevel {
@@ -55,12 +58,25 @@ struct TailArgs {
   const int* piv;
   int dense_level;         // -1: none; else levels >= dense_level are applied as dense_B
   const double* dense_B;   // [nD x nD] row-major
-  unsigned long long* bar;  // [0] arrival counter, [16] release generation
+  unsigned long long* bar;  // [gridDim.x] generation flags of the grid barrier
   double* partials;
   KrylovCtl* ctl;           // may be null (hooks)
   int fin;                  // FIN_RZ: b_first . result is reduced and finalised (first == 0 only)
   int lu_smem;              // bytes reserved at the start of dynamic shared memory for the LU solve
+  unsigned long long* prof; // -DAMG_TAIL_PROFILE: CTA 0 stamps %globaltimer after every phase
 };
+#ifdef AMG_TAIL_PROFILE
+#define TAIL_STAMP(a, slot)                                                         \
+  do {                                                                              \
+    if ((a).prof != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {               \
+      unsigned long long _t;                                                        \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(_t));                        \
+      (a).prof[(slot)] = _t;                                                        \
+    }                                                                               \
+  } while (0)
+#else
+#define TAIL_STAMP(a, slot) do { } while (0)
+#endif
 
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
   unsigned long long v;
@@ -71,23 +87,71 @@ __device__ __forceinline__ void st_release_u64(unsigned long long* p, unsigned l
   asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// All CTAs of the grid are co-resident (grid <= number of SMs, one CTA each).  The arrival
-// counter only grows: every launch performs whole barriers, so it stays a multiple of gridDim.x.
-__device__ __forceinline__ void tail_grid_barrier(unsigned long long* bar) {
+// Grid barrier without atomics.  All CTAs of the grid are co-resident (grid <= number of SMs, one
+// CTA each).  CTA c publishes its generation in flags[c]; warp 0 of every CTA polls all flags with
+// coalesced loads until every one has reached the generation.  One store and one load round trip,
+// no serialised same-address atomics (148 atomic arrivals + 147 pollers on one line cost 3-5 us per
+// barrier, measured).  Generations only grow; every launch performs whole barriers, so a CTA picks
+// up its generation from its own flag at kernel start.
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+// SASS on sm_100a: st.release.gpu = MEMBAR.ALL.GPU + STG.STRONG; ld.relaxed.gpu = LDG.STRONG alone;
+// fence.acq_rel.gpu = MEMBAR.ALL.GPU + CCTL.IVALL.  __threadfence() would be MEMBAR.SC.GPU and
+// ld.acquire.gpu a CCTL.IVALL (L1 invalidation) per poll: neither belongs in the polling loop.
+#ifndef TAIL_BAR_VARIANT
+#define TAIL_BAR_VARIANT 1
+#endif
+__device__ __forceinline__ void tail_grid_barrier(unsigned long long* flags, unsigned long long& gen) {
   __syncthreads();
+#if TAIL_BAR_VARIANT == 0
+  // per-CTA generation flags, warp 0 polls all of them
+  if (threadIdx.x < 32) {
+    gen += 1ULL;
+    if (threadIdx.x == 0) st_release_u64(flags + 32 + blockIdx.x, gen);
+    const unsigned G = gridDim.x;
+    for (;;) {
+      bool ok = true;
+      for (unsigned q = threadIdx.x; q < G; q += 32) ok &= (ld_relaxed_u64(flags + 32 + q) >= gen);
+      if (__all_sync(0xffffffffu, ok)) break;
+    }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+  }
+#elif TAIL_BAR_VARIANT == 1
+  // one arrival counter (only grows: every launch performs whole barriers, so it stays a multiple
+  // of gridDim.x) and one release word; thread 0 of every CTA arrives and polls
   if (threadIdx.x == 0) {
     const unsigned long long G = gridDim.x;
     __threadfence();
-    const unsigned long long t = atomicAdd(bar, 1ULL);
-    const unsigned long long gen = t / G + 1ULL;
+    const unsigned long long t = atomicAdd(flags, 1ULL);
+    const unsigned long long g = t / G + 1ULL;
     if (t % G == G - 1ULL) {
-      st_release_u64(bar + 16, gen);
+      st_release_u64(flags + 16, g);
     } else {
-      while (ld_acquire_u64(bar + 16) < gen) {
+      while (ld_acquire_u64(flags + 16) < g) {
       }
     }
     __threadfence();
   }
+#else
+  // as 1 with the lightest fences that are still a release / acquire pair
+  if (threadIdx.x == 0) {
+    const unsigned long long G = gridDim.x;
+    unsigned long long t;
+    asm volatile("atom.add.release.gpu.global.u64 %0, [%1], 1;" : "=l"(t) : "l"(flags) : "memory");
+    const unsigned long long g = t / G + 1ULL;
+    if (t % G == G - 1ULL) {
+      asm volatile("fence.acq_rel.gpu;" ::: "memory");
+      asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(flags + 16), "l"(g) : "memory");
+    } else {
+      while (ld_relaxed_u64(flags + 16) < g) {
+      }
+      asm volatile("fence.acq_rel.gpu;" ::: "memory");
+    }
+  }
+#endif
   __syncthreads();
 }
 
@@ -322,6 +386,9 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
   const int E = use_dense ? a.dense_level : a.last;  // sparse levels [first, E), then the bottom solve on E
   unsigned char* stage = tail_sm + a.lu_smem;
   double dot = 0.0;
+  unsigned long long gen = ld_acquire_u64(a.bar + 32 + blockIdx.x);  // flag variant: warp 0 keeps it current
+  int pslot = 0;
+  TAIL_STAMP(a, pslot++);
 
   // ---- stage this CTA's operator chunks of every sparse level ----
   if (tid == 0) {
@@ -350,6 +417,7 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
     const TailLevel L = a.lv[l];
     const TailChunk ch = a.chunk[l * G + cta];
     if (L.s_rp >= 0) mbar_wait(&lvbar[l], 0);
+    TAIL_STAMP(a, pslot++);
     const TailOpView A = tail_view(L, ch, stage);
     const double* b = (l == a.first) ? a.b_first : L.b;
     double* cur = L.x;
@@ -365,16 +433,20 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
       tl_vec_pass<T_ZERO, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 0;
     }
-    tail_grid_barrier(a.bar);
+    TAIL_STAMP(a, pslot++);
+    tail_grid_barrier(a.bar, gen);
+    TAIL_STAMP(a, pslot++);
     for (int s = done; s < a.nu1; ++s) {
       tl_row_pass<T_JAC, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, nullptr, 0.0, oth, false);
       double* t = cur;
       cur = oth;
       oth = t;
-      tail_grid_barrier(a.bar);
+      tail_grid_barrier(a.bar, gen);
     }
     tl_restrict_pass<true>(A, ch.A0, ch.A1, tid, TAIL_THREADS, b, cur, a.lv[l + 1].b);
-    tail_grid_barrier(a.bar);
+    TAIL_STAMP(a, pslot++);
+    tail_grid_barrier(a.bar, gen);
+    TAIL_STAMP(a, pslot++);
   }
 
   // ---- bottom: the dense collapsed operator of levels >= E, or the LU solve of the coarsest level ----
@@ -393,7 +465,9 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
       if (want)
         for (int i = tid; i < L.n; i += TAIL_THREADS) dot += __ldcg(b + i) * L.x[i];
     }
-    if (a.first < E) tail_grid_barrier(a.bar);
+    TAIL_STAMP(a, pslot++);
+    if (a.first < E) tail_grid_barrier(a.bar, gen);
+    TAIL_STAMP(a, pslot++);
   }
 
   // ---- up ----
@@ -413,7 +487,9 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
       cur = oth;
       oth = t;
       for (int s = 1; s < a.nu2; ++s) {
-        tail_grid_barrier(a.bar);
+        TAIL_STAMP(a, pslot++);
+        tail_grid_barrier(a.bar, gen);
+        TAIL_STAMP(a, pslot++);
         dot += tl_row_pass<T_JAC, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, nullptr, 0.0, oth,
                                         top && s == a.nu2 - 1);
         t = cur;
@@ -423,7 +499,9 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
     } else {
       dot += tl_vec_pass<T_PROLONG, true>(A, ch.R0, ch.R1, tid, TAIL_THREADS, b, cur, ec, a.gamma, oth, top);
     }
-    if (l > a.first) tail_grid_barrier(a.bar);
+    TAIL_STAMP(a, pslot++);
+    if (l > a.first) tail_grid_barrier(a.bar, gen);
+    TAIL_STAMP(a, pslot++);
   }
 
   // ---- fused r.z of a cycle that starts at level 0 (small systems: the whole cycle is this kernel) ----
@@ -437,7 +515,7 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
       for (int q = 0; q < TAIL_THREADS / 32; ++q) s += red[q];
       a.partials[blockIdx.x] = s;
     }
-    tail_grid_barrier(a.bar);
+    tail_grid_barrier(a.bar, gen);
     if (blockIdx.x == 0 && tid < 32) {
       double s = 0.0;
       for (unsigned q = tid; q < gridDim.x; q += 32) s += __ldcg(a.partials + q);
