@@ -94,6 +94,8 @@ typedef struct {
   int32_t tail_dense_rows;  /* inside that kernel, the V-cycle from the first level with at most this many
                                rows down to the coarsest solve is applied as ONE dense operator assembled
                                at setup (the same linear map); default 2304, 0 = off         */
+  int32_t use_pdl;          /* 1 = the kernels of a captured iteration are chained by programmatic dependent
+                               launches (a kernel becomes resident while its predecessor drains); default 1 */
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */

@@ -161,6 +161,7 @@ amg_status amg_options_default(amg_options* o) {
   o->use_graph = 1;
   o->tail_max_rows = 65536;
   o->tail_dense_rows = 2304;
+  o->use_pdl = 1;
   o->omega = 2.0 / 3.0;
   o->strong_beta = 0.25;
   o->coarse_scale = 1.0;

@@ -22,7 +22,13 @@
 #define RT_STAGE_BYTES_CFG 36864
 #endif
 constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA (8 warps walk the ELL slices)
-constexpr int RT_GATHERERS = 64;                   // 2 warps fetch the halo values one tile ahead
+#ifndef RT_GATHERERS_CFG
+#define RT_GATHERERS_CFG 192
+#endif
+#ifndef RT_GATHER_UNROLL
+#define RT_GATHER_UNROLL 4
+#endif
+constexpr int RT_GATHERERS = RT_GATHERERS_CFG;      // warps x 32 that fetch the halo values one tile ahead
 constexpr int RT_THREADS = RT_CONSUMERS + 32 + RT_GATHERERS;  // + one producer warp (issues the bulk copies)
 constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA
 constexpr int RT_CTAS = RT_CTAS_CFG;               // persistent CTAs per SM

@@ -5,6 +5,20 @@
 #include "amg_internal.cuh"
 
 // ------------------------------------------------------------------------------------------
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic-serialization
+// attribute may become resident while its predecessor in the stream / graph is still draining.
+// griddepcontrol.wait blocks until every prerequisite grid has completed and its writes are
+// visible; without the attribute both instructions are no-ops.  Everything before pdl_wait()
+// may only touch data no earlier kernel of the solve writes (tile descriptors, operator blobs).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_sync() {
+  pdl_launch_dependents();
+  pdl_wait();
+}
+
+// ------------------------------------------------------------------------------------------
 // operations of the row kernels
 // ------------------------------------------------------------------------------------------
 enum RowOp {
@@ -397,6 +411,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
 
 template <int OP, int NDOT, bool STREAM>
 __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
+  pdl_sync();
   if (a.ctl != nullptr && a.ctl->done) return;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
@@ -437,54 +452,55 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
         const int* hl = reinterpret_cast<const int*>(base + sd->o_halo);
         double* xc = reinterpret_cast<double*>(base + sd->o_xcat) + sd->roff;  // xc[col]
         double* xh = xc + nr;
+        constexpr int GU = RT_GATHER_UNROLL, GS = RT_GATHERERS;
         if (OP == OP_JACOBI_PROLONG) {
           const int* hc = reinterpret_cast<const int*>(base + sd->o_cagg);
           const double gamma = a.gamma;
           int h = g;
-          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
-            double v[4], e[4];
+          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
+            double v[GU], e[GU];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              v[q] = __ldg(a.x + hl[h + q * RT_GATHERERS]);
-              e[q] = __ldg(a.ec + hc[h + q * RT_GATHERERS]);
+            for (int q = 0; q < GU; ++q) {
+              v[q] = __ldg(a.x + hl[h + q * GS]);
+              e[q] = __ldg(a.ec + hc[h + q * GS]);
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q] + gamma * e[q];
+            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q] + gamma * e[q];
           }
-          for (; h < nhalo; h += RT_GATHERERS) xh[h] = __ldg(a.x + hl[h]) + gamma * __ldg(a.ec + hc[h]);
+          for (; h < nhalo; h += GS) xh[h] = __ldg(a.x + hl[h]) + gamma * __ldg(a.ec + hc[h]);
           const int* as = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;    // as[lr] = agg[r0 + lr]
           const double* es = reinterpret_cast<const double*>(base + sd->o_ec) - sd->eoff;  // es[I] = ec[I]
-          for (int lr = g; lr < nr; lr += RT_GATHERERS) xc[lr] += gamma * es[as[lr]];
+          for (int lr = g; lr < nr; lr += GS) xc[lr] += gamma * es[as[lr]];
         } else if (OP == OP_JACOBI0) {
           int h = g;
-          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
-            double v[4], e[4];
+          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
+            double v[GU], e[GU];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int c = hl[h + q * RT_GATHERERS];
+            for (int q = 0; q < GU; ++q) {
+              const int c = hl[h + q * GS];
               v[q] = __ldg(a.dinv + c);
               e[q] = __ldg(a.b + c);
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q] * e[q];
+            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q] * e[q];
           }
-          for (; h < nhalo; h += RT_GATHERERS) {
+          for (; h < nhalo; h += GS) {
             const int c = hl[h];
             xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
           }
           const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
           const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
-          for (int lr = g; lr < nr; lr += RT_GATHERERS) xc[lr] = ds[lr] * bs[lr];
+          for (int lr = g; lr < nr; lr += GS) xc[lr] = ds[lr] * bs[lr];
         } else {
           int h = g;
-          for (; h + 3 * RT_GATHERERS < nhalo; h += 4 * RT_GATHERERS) {
-            double v[4];
+          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
+            double v[GU];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) v[q] = __ldg(a.x + hl[h + q * RT_GATHERERS]);
+            for (int q = 0; q < GU; ++q) v[q] = __ldg(a.x + hl[h + q * GS]);
 #pragma unroll
-            for (int q = 0; q < 4; ++q) xh[h + q * RT_GATHERERS] = v[q];
+            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q];
           }
-          for (; h < nhalo; h += RT_GATHERERS) xh[h] = __ldg(a.x + hl[h]);
+          for (; h < nhalo; h += GS) xh[h] = __ldg(a.x + hl[h]);
         }
         fence_proxy_async();  // generic writes into a region a later bulk copy overwrites
       }
@@ -578,6 +594,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
 // ------------------------------------------------------------------------------------------
 template <int OP, int NDOT, int LPR>
 __global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
+  pdl_sync();
   if (a.ctl != nullptr && a.ctl->done) return;
   const int tid = threadIdx.x;
   const int sub = tid & (LPR - 1);
@@ -608,6 +625,7 @@ __global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
 // restriction of a stored residual (fallback path): rc[I] = sum of r over the contiguous rows of I
 __global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const double* __restrict__ r,
                                 double* __restrict__ rc, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int I = blockIdx.x * blockDim.x + threadIdx.x;
   if (I >= nc) return;
@@ -619,6 +637,7 @@ __global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const d
 // S4 standalone: x_i += gamma * ec[agg_i]
 __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* __restrict__ ec, double gamma,
                               const double* __restrict__ xin, double* __restrict__ xout, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) xout[i] = xin[i] + gamma * ec[agg[i]];
@@ -626,12 +645,14 @@ __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* 
 
 __global__ void k_scale_dinv(int n, const double* __restrict__ dinv, const double* __restrict__ b,
                              double* __restrict__ x, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) x[i] = dinv[i] * b[i];
 }
 
 __global__ void k_zero(int n, double* __restrict__ x, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) x[i] = 0.0;
@@ -642,6 +663,7 @@ __global__ void k_zero(int n, double* __restrict__ x, const KrylovCtl* ctl) {
 // ------------------------------------------------------------------------------------------
 __global__ void k_lu_solve(int n, const double* __restrict__ lu, const int* __restrict__ piv,
                            const double* __restrict__ b, double* __restrict__ x, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   extern __shared__ double y[];
   const int tid = threadIdx.x, T = blockDim.x;
@@ -717,6 +739,7 @@ __device__ __forceinline__ void lu_solve_small_cta(int n, const double* __restri
 __global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __restrict__ lu,
                                                         const int* __restrict__ piv, const double* __restrict__ b,
                                                         double* __restrict__ x, const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   extern __shared__ double lu_sm[];
   lu_solve_small_cta<true>(n, lu, piv, b, x, lu_sm);
@@ -748,6 +771,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const double
 // p = z + beta p
 __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __restrict__ z, double* __restrict__ p,
                                                        const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl->done) return;
   const double beta = ctl->beta;
   for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
@@ -759,6 +783,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __r
                                                         const double* __restrict__ q, double* __restrict__ x,
                                                         double* __restrict__ r, double* partials, unsigned* counter,
                                                         KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl->done) return;
   const double alpha = ctl->alpha;
   double acc[1] = {0.0};
@@ -771,9 +796,20 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __r
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, FIN_RR);
 }
 
+// dst = src (keeps phat across the second V-cycle of a BiCGSTAB iteration; a kernel, not a memcpy
+// node, so that the captured iteration is a chain of kernels with programmatic edges)
+__global__ void __launch_bounds__(RED_THREADS) k_copy(int n, const double* __restrict__ src, double* __restrict__ dst,
+                                                      const KrylovCtl* ctl) {
+  pdl_sync();
+  if (ctl->done) return;
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
+    dst[i] = src[i];
+}
+
 // sum a.b  (used when no smoother sweep can carry the r.z product)
 __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __restrict__ a, const double* __restrict__ b,
                                                      double* partials, unsigned* counter, KrylovCtl* ctl, int fin) {
+  pdl_sync();
   if (ctl->done) return;
   double acc[1] = {0.0};
   for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
@@ -785,6 +821,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __rest
 __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ p,
                                                         const KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl->done) return;
   const double beta = ctl->beta, omega = ctl->omega;
   for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
@@ -795,6 +832,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __r
 __global__ void __launch_bounds__(RED_THREADS) k_bicg_s(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ s,
                                                         double* partials, unsigned* counter, KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl->done) return;
   const double alpha = ctl->alpha;
   double acc[1] = {0.0};
@@ -812,6 +850,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const double* __
                                                          const double* __restrict__ t, const double* __restrict__ rhat,
                                                          double* __restrict__ x, double* __restrict__ r,
                                                          double* partials, unsigned* counter, KrylovCtl* ctl) {
+  pdl_sync();
   if (ctl->done) return;
   const double alpha = ctl->alpha, omega = ctl->omega;
   double acc[2] = {0.0, 0.0};

@@ -12,6 +12,34 @@ namespace {
 
 thread_local int64_t g_nlaunch = 0;  // kernel launches enqueued by this thread (amg_get_last_launches)
 
+thread_local bool g_pdl = false;     // true while an iteration is being captured with programmatic edges
+
+// kernel launch; with g_pdl the kernel may become resident while its predecessor drains
+// (programmatic dependent launch: every kernel of the solve calls griddepcontrol.wait first)
+template <typename... KArgs>
+struct Launcher {
+  void (*k)(KArgs...);
+  dim3 g, b;
+  size_t sm;
+  cudaStream_t st;
+  template <typename... A>
+  void operator()(A&&... a) const {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = g, cfg.blockDim = b, cfg.dynamicSmemBytes = sm, cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, k, KArgs(a)...);
+  }
+};
+template <typename... KArgs>
+Launcher<KArgs...> launch(void (*k)(KArgs...), dim3 g, dim3 b, size_t sm, cudaStream_t st) {
+  return Launcher<KArgs...>{k, g, b, sm, st};
+}
+
 constexpr int TPB = 256;
 inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
 
@@ -33,7 +61,7 @@ void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaSt
   }
   int grid = H->sm_count * RT_CTAS;
   if (grid > L.nblk) grid = L.nblk;
-  ++g_nlaunch, k_rowtile<OP, NDOT, STREAM><<<grid, RT_THREADS, rt::SMEM_BYTES, st>>>(a);
+  ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM>, grid, RT_THREADS, rt::SMEM_BYTES, st)(a);
 }
 
 template <int OP, int NDOT>
@@ -49,10 +77,10 @@ void launch_row(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStr
     if (NDOT > 0 && g > 4096) g = 4096;  // bounded partials; the kernel strides over rows
     if (g < 1) g = 1;
     switch (L.lpr) {
-      case 4: ++g_nlaunch; k_rowvec<OP, NDOT, 4><<<g, RB_THREADS, 0, st>>>(a); break;
-      case 8: ++g_nlaunch; k_rowvec<OP, NDOT, 8><<<g, RB_THREADS, 0, st>>>(a); break;
-      case 16: ++g_nlaunch; k_rowvec<OP, NDOT, 16><<<g, RB_THREADS, 0, st>>>(a); break;
-      default: ++g_nlaunch; k_rowvec<OP, NDOT, 32><<<g, RB_THREADS, 0, st>>>(a); break;
+      case 4: ++g_nlaunch; launch(k_rowvec<OP, NDOT, 4>, g, RB_THREADS, 0, st)(a); break;
+      case 8: ++g_nlaunch; launch(k_rowvec<OP, NDOT, 8>, g, RB_THREADS, 0, st)(a); break;
+      case 16: ++g_nlaunch; launch(k_rowvec<OP, NDOT, 16>, g, RB_THREADS, 0, st)(a); break;
+      default: ++g_nlaunch; launch(k_rowvec<OP, NDOT, 32>, g, RB_THREADS, 0, st)(a); break;
     }
   }
 }
@@ -142,7 +170,7 @@ void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, cons
   } else {
     a.out = L.rtmp;
     launch_row<OP_RESID, 0>(H, L, a, st);
-    ++g_nlaunch, k_restrict_rows<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
+    ++g_nlaunch, launch(k_restrict_rows, grid_for(L.nc), TPB, 0, st)(L.nc, L.agg_ptr, L.rtmp, rc, ctl);
   }
 }
 
@@ -150,11 +178,11 @@ void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl
   const int n = H->nL;
   if (n <= LU_SMALL_MAX) {
     const size_t sm = sizeof(double) * ((size_t)n * (n + 1) + n);
-    ++g_nlaunch, k_lu_solve_small<<<1, 256, sm, st>>>(n, H->lu, H->piv, b, x, ctl);
+    ++g_nlaunch, launch(k_lu_solve_small, 1, 256, sm, st)(n, H->lu, H->piv, b, x, ctl);
     return;
   }
   int T = n <= 32 ? 32 : (n <= 64 ? 64 : (n <= 256 ? 256 : 1024));
-  ++g_nlaunch, k_lu_solve<<<1, T, sizeof(double) * n, st>>>(n, H->lu, H->piv, b, x, ctl);
+  ++g_nlaunch, launch(k_lu_solve, 1, T, sizeof(double) * n, st)(n, H->lu, H->piv, b, x, ctl);
 }
 
 // levels l..coarsest in one persistent kernel (amg_tail.cuh); returns the result buffer of level l
@@ -186,7 +214,7 @@ double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin
   cudaMemsetAsync(d_prof, 0, 256 * sizeof(unsigned long long), st);
   a.prof = d_prof;
 #endif
-  ++g_nlaunch, k_vcycle_tail<<<H->tail_grid, TAIL_THREADS, H->tail_smem, st>>>(a);
+  ++g_nlaunch, launch(k_vcycle_tail, H->tail_grid, TAIL_THREADS, H->tail_smem, st)(a);
 #ifdef AMG_TAIL_PROFILE
   if (getenv("AMG_TAIL_PROF")) {
     unsigned long long hp[256];
@@ -320,7 +348,7 @@ amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
       ba.B = H->tail_dense_B;
       ba.lu_smem = H->tail_lu_smem;
       AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_tail_dense_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-      k_tail_dense_build<<<nD, TAILB_THREADS, smem, st>>>(ba);
+      launch(k_tail_dense_build, nD, TAILB_THREADS, smem, st)(ba);
       AMG_CUDA_TRY(H, cudaGetLastError());
       H->tail_dense_level = D;
     }
@@ -347,7 +375,7 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     op_coarse_solve(H, b, L.x, ctl, st);
     *x_out = L.x;
     if (fuse_rz && l == 0)
-      ++g_nlaunch, k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
+      ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
     AMG_CUDA_TRY(H, cudaGetLastError());
     return AMG_OK;
   }
@@ -359,10 +387,10 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     op_jacobi0(H, L, b, cur, ctl, st);
     done_sweeps = 2;
   } else if (nu1 == 1) {
-    ++g_nlaunch, k_scale_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.dinv, b, cur, ctl);
+    ++g_nlaunch, launch(k_scale_dinv, grid_for(L.n), TPB, 0, st)(L.n, L.dinv, b, cur, ctl);
     done_sweeps = 1;
   } else {
-    ++g_nlaunch, k_zero<<<grid_for(L.n), TPB, 0, st>>>(L.n, cur, ctl);
+    ++g_nlaunch, launch(k_zero, grid_for(L.n), TPB, 0, st)(L.n, cur, ctl);
   }
   for (int s = done_sweeps; s < nu1; ++s) {
     op_jacobi(H, L, b, cur, oth, false, ctl, st);
@@ -381,9 +409,9 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       std::swap(cur, oth);
     }
   } else {
-    ++g_nlaunch, k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
+    ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
     std::swap(cur, oth);
-    if (want_dot) ++g_nlaunch, k_dot<<<red_grid(H, L.n), RED_THREADS, 0, st>>>(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
+    if (want_dot) ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
   }
   *x_out = cur;
   AMG_CUDA_TRY(H, cudaGetLastError());
@@ -406,14 +434,14 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *q = H->kv[3];
   op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
-  ++g_nlaunch, k_pcg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, p, q, x, r, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, H->partials, H->counter, H->ctl);
   double* z = r;
   if (precond) {
     AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
   } else {
-    ++g_nlaunch, k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+    ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
   }
-  ++g_nlaunch, k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+  ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, z, p, H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -423,21 +451,21 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4], *s = H->kv[5],
          *t = H->kv[6], *ph = H->kv[7];
-  ++g_nlaunch, k_bicg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, p, H->ctl);
+  ++g_nlaunch, launch(k_bicg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, p, H->ctl);
   double* phat = p;
   if (precond) {
     double* zz = nullptr;
     AMG_TRY(amg_vcycle(H, 0, p, &zz, H->ctl, false, st));
     // the second V-cycle of this iteration overwrites the level-0 buffers: keep phat
-    AMG_CUDA_TRY(H, cudaMemcpyAsync(ph, zz, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    ++g_nlaunch, launch(k_copy, red_grid(H, n), RED_THREADS, 0, st)(n, zz, ph, H->ctl);
     phat = ph;
   }
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
-  ++g_nlaunch, k_bicg_s<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, v, s, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, H->partials, H->counter, H->ctl);
   double* shat = s;
   if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st));
   op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
-  ++g_nlaunch, k_bicg_xr<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
+  ++g_nlaunch, launch(k_bicg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
                                                    H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
@@ -458,7 +486,9 @@ amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStr
   if (!H->cap_stream) AMG_CUDA_TRY(H, cudaStreamCreateWithFlags(&H->cap_stream, cudaStreamNonBlocking));
   AMG_CUDA_TRY(H, cudaStreamBeginCapture(H->cap_stream, cudaStreamCaptureModeThreadLocal));
   const int64_t launches0 = g_nlaunch;
+  g_pdl = H->opt.use_pdl != 0;
   amg_status s = enqueue_iteration(H, krylov, precond, H->cap_stream);
+  g_pdl = false;
   H->graph_launches[slot] = g_nlaunch - launches0;  // kernel nodes of one replay
   g_nlaunch = launches0;                            // capturing enqueues nothing
   cudaError_t e = cudaStreamEndCapture(H->cap_stream, &g);
@@ -505,17 +535,17 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   H->h_ctl[5] = init;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
   if (krylov == 0) {
-    ++g_nlaunch, k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
+    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
                                                          H->counter, H->ctl, FIN_INIT_PCG);
     double* z = r;
     if (precond) {
       AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
     } else {
-      ++g_nlaunch, k_dot<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+      ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
     }
-    ++g_nlaunch, k_pcg_p<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, z, p, H->ctl);
+    ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, z, p, H->ctl);
   } else {
-    ++g_nlaunch, k_krylov_init<<<red_grid(H, n), RED_THREADS, 0, st>>>(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
+    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
                                                          H->ctl, FIN_INIT_BICG);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
@@ -543,7 +573,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   }
   const bool half = (krylov == 1);
   const double* phat = half ? (precond ? H->kv[7] : p) : nullptr;
-  ++g_nlaunch, k_krylov_output<<<grid_for(n), TPB, 0, st>>>(n, x, phat, L0.inv, d_x, H->ctl);
+  ++g_nlaunch, launch(k_krylov_output, grid_for(n), TPB, 0, st)(n, x, phat, L0.inv, d_x, H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
@@ -575,10 +605,10 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
     return AMG_ERR_INVALID_ARG;
   }
   auto perm_in = [&](const Level& Lv, const double* nat, double* out) {
-    ++g_nlaunch, k_permute_in<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, nat, Lv.inv, out);
+    ++g_nlaunch, launch(k_permute_in, grid_for(Lv.n), TPB, 0, st)(Lv.n, nat, Lv.inv, out);
   };
   auto perm_out = [&](const Level& Lv, const double* in, double* nat) {
-    ++g_nlaunch, k_permute_out<<<grid_for(Lv.n), TPB, 0, st>>>(Lv.n, in, Lv.inv, nat);
+    ++g_nlaunch, launch(k_permute_out, grid_for(Lv.n), TPB, 0, st)(Lv.n, in, Lv.inv, nat);
   };
   switch (op) {
     case 0:
@@ -608,7 +638,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       perm_in(L, d_in0, t0);
       perm_in(C, d_in1, t1);
       for (int r = 0; r < reps; ++r)
-        ++g_nlaunch, k_prolong_add<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
+        ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
       perm_out(L, t2, d_out);
     } break;
     case 4:
@@ -643,11 +673,11 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
   const double mean = n > 0 ? (double)H->nnz / n : 1.0;
   if (mean <= 12.0) {
     const int64_t threads = (int64_t)n * 8;
-    ++g_nlaunch, k_grad_values<8><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+    ++g_nlaunch, launch(k_grad_values<8>, div_up(threads, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
                                                           d_gA, accumulate);
   } else {
     const int64_t threads = (int64_t)n * 32;
-    ++g_nlaunch, k_grad_values<32><<<div_up(threads, 256), 256, 0, st>>>(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
+    ++g_nlaunch, launch(k_grad_values<32>, div_up(threads, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
                                                            d_gA, accumulate);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());

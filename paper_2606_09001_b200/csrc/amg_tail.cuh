@@ -377,6 +377,7 @@ __device__ __forceinline__ double tail_dense_rows(int n, const double* __restric
 }
 
 __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
+  pdl_sync();
   if (a.ctl != nullptr && a.ctl->done) return;
   extern __shared__ __align__(128) unsigned char tail_sm[];
   __shared__ uint64_t lvbar[TAIL_MAX_LEVELS];
