@@ -23,9 +23,23 @@ void* amg_dev_alloc(amg_handle_s* H, size_t bytes, cudaStream_t st) {
   void* p = nullptr;
   if (g_alloc_fn) {
     p = g_alloc_fn(bytes, (void*)st, g_alloc_user);
-  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
-    cudaGetLastError();
-    p = nullptr;
+  } else {
+    // stream-ordered pool: the setup allocates and frees hundreds of temporaries; cudaMalloc /
+    // cudaFree would each synchronise the device and map / unmap memory (hundreds of ms per setup)
+    static bool pool_ready = false;
+    if (!pool_ready) {
+      int dev = 0;
+      cudaMemPool_t pool;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        uint64_t keep = ~0ULL;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      }
+      pool_ready = true;
+    }
+    if (cudaMallocAsync(&p, bytes, st) != cudaSuccess) {
+      cudaGetLastError();
+      p = nullptr;
+    }
   }
   if (p) H->allocs.push_back(p);
   return p;
@@ -35,7 +49,7 @@ static void raw_free(void* p) {
   if (g_free_fn)
     g_free_fn(p, g_alloc_user);
   else
-    cudaFree(p);
+    cudaFreeAsync(p, nullptr);  // callers have synchronised the stream that last used p
 }
 
 void amg_dev_free(amg_handle_s* H, void* p) {
