@@ -90,7 +90,9 @@ typedef struct {
   int32_t use_graph;        /* 1 = replay one Krylov iteration as a CUDA graph (default), 0 = plain launches */
   int32_t tail_max_rows;    /* levels with at most this many rows (and everything below them) run inside ONE
                                persistent kernel per V-cycle (grid barriers instead of launches); default
-                               65536, 0 = off                                                            */
+                               2304 (= tail_dense_rows: measured on B200, a grid-barrier phase costs more
+                               than a row-tile launch, so by default the tail is the dense operator alone);
+                               0 = off                                                                   */
   int32_t tail_dense_rows;  /* inside that kernel, the V-cycle from the first level with at most this many
                                rows down to the coarsest solve is applied as ONE dense operator assembled
                                at setup (the same linear map); default 2304, 0 = off         */

@@ -173,7 +173,7 @@ amg_status amg_options_default(amg_options* o) {
   o->max_match_rounds = 0;
   o->force_generic = 0;
   o->use_graph = 1;
-  o->tail_max_rows = 65536;
+  o->tail_max_rows = 2304;
   o->tail_dense_rows = 2304;
   o->use_pdl = 1;
   o->omega = 2.0 / 3.0;

@@ -123,9 +123,9 @@ def test_level_kernels(cases, name, generic):
 
 
 # tail_max_rows: the levels at or below this size run inside the persistent coarse-tail kernel
-# (default 65536: almost every level of these small cases); 0 = one kernel per pass on every
-# level; 600 = a mixed cycle
-@pytest.mark.parametrize("tail", [65536, 0, 600])
+# (65536: almost every level of these small cases, sparse phases + the dense collapsed operator);
+# 0 = one kernel per pass on every level; 600 = a mixed cycle; 2304 = the default
+@pytest.mark.parametrize("tail", [65536, 0, 600, 2304])
 @pytest.mark.parametrize("name", list(CASES))
 def test_apply_preconditioner(cases, name, tail):
     c = cases(name, tail_max_rows=tail)
@@ -317,6 +317,89 @@ def test_options(oracle_mod, B, opts):
     assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) / np.linalg.norm(b) <= 1e-8
     s.close()
     o.close()
+
+
+@pytest.mark.parametrize("gpu_opts", [
+    dict(tail_max_rows=65536, tail_dense_rows=0),      # persistent tail, sparse phases down to the LU solve
+    dict(tail_max_rows=65536, tail_dense_rows=300),    # dense collapsed operator deep inside the tail
+    dict(tail_max_rows=65536, tail_dense_rows=4000),   # ... and near its top
+    dict(tail_max_rows=0, tail_dense_rows=0),          # no tail at all
+    dict(use_pdl=0), dict(use_graph=0, use_pdl=0),
+])
+def test_launch_structure_options(cases, gpu_opts):
+    """Options that change how the cycle is launched, never what it computes: same V-cycle operator
+    (1e-12), same iteration count and solution as the oracle on the identical hierarchy."""
+    c = cases("cfg3_40", **gpu_opts)
+    r = np.random.default_rng(17).standard_normal(c.A.n)
+    assert rel(c.s.apply_preconditioner(r).cpu().numpy(), c.o.vcycle(r, 0)) <= 1e-12
+    for l in range(1, c.s.num_levels):  # cycles that start inside / below the collapsed levels
+        n = c.s.level_info(l)[0]
+        bl = np.random.default_rng(100 + l).standard_normal(n)
+        assert rel(c.s.level_op(l, 5, None, bl, n).cpu().numpy(), c.o.vcycle(bl, l)) <= 1e-12
+    for krylov in (0, 1):
+        xg, ig = c.s.solve(c.b, 1e-8, 1000, krylov)
+        xo, io = c.o.solve(c.b, 1e-8, 1000, krylov, 1)
+        assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        assert np.linalg.norm(c.b - c.Asp @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(c.b)
+
+
+def _irregular_spd(n, seed, hub_rows=0, hub_deg=0):
+    """Weighted graph Laplacian + positive diagonal shift of a random graph with very uneven degrees
+    (bit-symmetric values): rows of 2..40 entries, optionally a few hub rows with hub_deg entries."""
+    import scipy.sparse as sp
+
+    rng = np.random.default_rng(seed)
+    deg = np.minimum(1 + rng.zipf(1.7, n), 40)
+    src = np.repeat(np.arange(n), deg)
+    dst = (src + rng.integers(1, 200, src.size) * rng.choice([-1, 1], src.size)) % n  # mostly near the diagonal
+    if hub_rows:
+        hubs = rng.choice(n, hub_rows, replace=False)
+        hs = np.repeat(hubs, hub_deg)
+        src = np.concatenate([src, hs])
+        dst = np.concatenate([dst, rng.integers(0, n, hs.size)])
+    keep = src != dst
+    lo, hi = np.minimum(src[keep], dst[keep]), np.maximum(src[keep], dst[keep])
+    key = np.unique(lo.astype(np.int64) * n + hi)
+    lo, hi = (key // n).astype(np.int64), (key % n).astype(np.int64)
+    w = np.random.default_rng(seed + 1).uniform(0.1, 1.0, lo.size)
+    W = sp.coo_matrix((np.concatenate([w, w]), (np.concatenate([lo, hi]), np.concatenate([hi, lo]))), shape=(n, n)).tocsr()
+    d = np.asarray(W.sum(axis=1)).ravel() + 0.05
+    A = (sp.diags(d) - W).tocsr()
+    A.sort_indices()
+    return A
+
+
+@pytest.mark.parametrize("hubs", [0, 3])
+def test_irregular_rows_tile_packer(oracle_mod, B, hubs):
+    """The tile packer on rows of very different lengths (sorted-ELL slices, halo lists across the whole
+    matrix); with hub rows longer than the packer's 512-entry limit level 0 falls back to the
+    row-vector kernels, the coarser levels stay on the tile path.  Same parity bars as the PDE cases."""
+    A = _irregular_spd(30000, 5, hub_rows=hubs, hub_deg=700)
+    rp, cl, vl = A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(np.float64)
+    o = oracle_mod.Oracle(rp, cl, vl)
+    s = B.AmgSolver(rp, cl, vl)
+    try:
+        assert s.num_levels == o.num_levels
+        for l in range(s.num_levels - 1):
+            assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l)), f"level {l}"
+        assert s.level_path(0) == (0 if hubs else 1)
+        rng = np.random.default_rng(23)
+        for l in range(s.num_levels - 1):
+            n, nc = s.level_info(l)[0], s.level_info(l + 1)[0]
+            x, bb = rng.standard_normal(n), rng.standard_normal(n)
+            assert rel(s.level_op(l, 0, x, None, n).cpu().numpy(), o.spmv(l, x)) <= 1e-12
+            assert rel(s.level_op(l, 1, x, bb, n).cpu().numpy(), o.smooth(l, bb, x)) <= 1e-12
+            assert rel(s.level_op(l, 2, x, bb, nc).cpu().numpy(), o.residual_restrict(l, bb, x)) <= 1e-12
+        r = rng.standard_normal(A.shape[0])
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+        b = rng.uniform(-1, 1, A.shape[0])
+        xg, ig = s.solve(b, 1e-8, 2000, 0)
+        xo, io = o.solve(b, 1e-8, 2000, 0, 1)
+        assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        assert np.linalg.norm(b - A @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+    finally:
+        s.close()
+        o.close()
 
 
 def test_imported_aggregates_1d_closed_form(oracle_mod, B):
