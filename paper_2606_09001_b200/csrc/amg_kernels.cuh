@@ -330,11 +330,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // consumers meet on a fourth mbarrier per tile.
 // ------------------------------------------------------------------------------------------
 namespace rt {
-constexpr int HEADER_BYTES = 256;  // full / ready / empty / resdone mbarriers, RT_STAGES each
+constexpr int HEADER_BYTES = 256;  // full / ready / empty / resdone / pre mbarriers, RT_STAGES each
 constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * RT_STAGE_BYTES;
 constexpr int NCW = RT_CONSUMERS / 32;  // consumer warps
 constexpr int NGW = RT_GATHERERS / 32;  // gather warps
-static_assert(RT_STAGES >= 2 && 4 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
+static_assert(RT_STAGES >= 2 && 5 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
 static_assert(RT_STAGE_BYTES % 128 == 0, "stage size must keep 128-byte alignment");
 static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
 static_assert((NCW & (NCW - 1)) == 0, "consumer warps must be a power of two");
@@ -364,9 +364,11 @@ struct TileOps {
                                (AGGPTR ? TP_AGGPTR | TP_OUT : 0);
 };
 
+// mode 0: header + every copy, all on `bar`;  mode 1: header + the blob copy only, on `bar` (issued
+// before the grid dependency: the blob is setup data);  mode 2: the vector slices only, on `bar`
 template <int OP, int NDOT, bool STREAM>
 __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
-                                           uint64_t pol) {
+                                           uint64_t pol, int mode) {
   using T = TileOps<OP>;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
   const int flags = T::FLAGS | (d0_staged ? TP_B : 0);
@@ -380,10 +382,12 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
   sd.o_ec = t.o_ec, sd.o_xcat = t.o_xcat, sd.o_out = t.o_out;
   sd.aoff = T::AGGPTR ? d.I0 - t.Ia4 : d.r0 - t.ra4;
   sd.eoff = t.Ia2, sd.pad1 = sd.pad2 = sd.pad3 = 0;
-  int4* dst = reinterpret_cast<int4*>(stage);
-  const int4* src = reinterpret_cast<const int4*>(&sd);
+  if (mode != 2) {
+    int4* dst = reinterpret_cast<int4*>(stage);
+    const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
-  for (int q = 0; q < 6; ++q) dst[q] = src[q];
+    for (int q = 0; q < 6; ++q) dst[q] = src[q];
+  }
   if (d.nr <= 0) {
     mbar_arrive(bar);
     return;
@@ -391,49 +395,67 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
   unsigned char* base = stage + TP_DESC_BYTES;
   const uint32_t nblob = (uint32_t)(T::AGG ? p.endB : p.endA);
   const uint32_t nrv8 = 8u * (uint32_t)t.nrv;
-  uint32_t bytes = nblob;
-  if (T::X) bytes += nrv8;
-  if (T::B || d0_staged) bytes += nrv8;
-  if (T::D) bytes += nrv8;
-  if (T::AGG) bytes += 4u * (uint32_t)t.nr4;
-  if (T::EC) bytes += 8u * (uint32_t)t.nec;
-  if (T::AGGPTR) bytes += 4u * (uint32_t)t.nap;
+  uint32_t bytes = 0;
+  if (mode != 2) bytes += nblob;
+  if (mode != 1) {
+    if (T::X) bytes += nrv8;
+    if (T::B || d0_staged) bytes += nrv8;
+    if (T::D) bytes += nrv8;
+    if (T::AGG) bytes += 4u * (uint32_t)t.nr4;
+    if (T::EC) bytes += 8u * (uint32_t)t.nec;
+    if (T::AGGPTR) bytes += 4u * (uint32_t)t.nap;
+  }
   mbar_arrive_expect_tx(bar, bytes);
-  bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, nblob, bar, pol);
-  if (T::X) bulk_g2s<false>(base + t.o_xcat, a.x + t.ra2, nrv8, bar, pol);
-  if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra2, nrv8, bar, pol);
-  if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra2, nrv8, bar, pol);
-  if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, nrv8, bar, pol);
-  if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra4, 4u * (uint32_t)t.nr4, bar, pol);
-  if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
-  if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
+  if (mode != 2) bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, nblob, bar, pol);
+  if (mode != 1) {
+    if (T::X) bulk_g2s<false>(base + t.o_xcat, a.x + t.ra2, nrv8, bar, pol);
+    if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra2, nrv8, bar, pol);
+    if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra2, nrv8, bar, pol);
+    if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, nrv8, bar, pol);
+    if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra4, 4u * (uint32_t)t.nr4, bar, pol);
+    if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
+    if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
+  }
 }
 
 template <int OP, int NDOT, bool STREAM>
 __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
-  pdl_sync();
-  if (a.ctl != nullptr && a.ctl->done) return;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
   uint64_t* ready = full + RT_STAGES;
   uint64_t* empty = ready + RT_STAGES;
   uint64_t* resdone = empty + RT_STAGES;
+  uint64_t* pre = resdone + RT_STAGES;  // blobs of the first RT_STAGES tiles, issued before the grid dependency
   unsigned char* stage0 = smem + rt::HEADER_BYTES;
   const int tid = threadIdx.x;
   const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
   const int t_end = (int)((int64_t)(blockIdx.x + 1) * a.ntiles / gridDim.x);
   const int my = t_end - t_begin;
+  const int npre = my < RT_STAGES ? my : RT_STAGES;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
+  // ---- before the grid dependency: nothing here reads what an earlier kernel of the solve wrote ----
   if (tid == 0) {
     for (int s = 0; s < RT_STAGES; ++s) {
       mbar_init(full + s, 1);
       mbar_init(ready + s, rt::NGW);
       mbar_init(empty + s, rt::NCW);
       mbar_init(resdone + s, rt::NCW);
+      mbar_init(pre + s, 1);
     }
     fence_mbar_init();
   }
   __syncthreads();
+  pdl_launch_dependents();
+  const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
+  if (tid == RT_CONSUMERS)
+    for (int it = 0; it < npre; ++it)
+      tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, pre + it, pol, 1);
+  pdl_wait();
+  if (a.ctl != nullptr && a.ctl->done) {
+    if (tid == RT_CONSUMERS)  // the copies in flight target this CTA's shared memory: let them land
+      for (int it = 0; it < npre; ++it) mbar_wait(pre + it, 0);
+    return;
+  }
   double dots[NDOT > 0 ? NDOT : 1];
 #pragma unroll
   for (int j = 0; j < (NDOT > 0 ? NDOT : 1); ++j) dots[j] = 0.0;
@@ -444,6 +466,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     for (int it = 0; it < my; ++it) {
       const int s = it % RT_STAGES;
       unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
+      if (it < RT_STAGES) mbar_wait(pre + s, 0);
       mbar_wait(full + s, (uint32_t)((it / RT_STAGES) & 1));
       const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
       const int nr = sd->nr, nhalo = sd->nhalo;
@@ -510,15 +533,13 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   } else if (tid >= RT_CONSUMERS) {
     // ---------------- producer warp ----------------
     if (tid == RT_CONSUMERS && my > 0) {
-      const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
-      TileDesc d = a.tiles[t_begin];
-      for (int it = 0; it < my; ++it) {
+      for (int it = 0; it < npre; ++it)  // their blobs are already on the way
+        tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, full + it, pol, 2);
+      for (int it = npre; it < my; ++it) {
         const int s = it % RT_STAGES;
-        TileDesc dn = d;
-        if (it + 1 < my) dn = a.tiles[t_begin + it + 1];
-        if (it >= RT_STAGES) mbar_wait(empty + s, (uint32_t)(((it / RT_STAGES) - 1) & 1));
-        tile_issue<OP, NDOT, STREAM>(a, d, stage0 + s * RT_STAGE_BYTES, full + s, pol);
-        d = dn;
+        const TileDesc d = a.tiles[t_begin + it];
+        mbar_wait(empty + s, (uint32_t)(((it / RT_STAGES) - 1) & 1));
+        tile_issue<OP, NDOT, STREAM>(a, d, stage0 + s * RT_STAGE_BYTES, full + s, pol, 0);
       }
     }
   } else {
@@ -529,6 +550,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
       const int s = it % RT_STAGES;
       const uint32_t par = (uint32_t)((it / RT_STAGES) & 1);
       unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
+      if (it < RT_STAGES) mbar_wait(pre + s, 0);
       mbar_wait(full + s, par);   // the bulk copies have landed ...
       mbar_wait(ready + s, par);  // ... and the gather warps are done with the stage
       const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
