@@ -377,7 +377,19 @@ __device__ __forceinline__ double tail_dense_rows(int n, const double* __restric
 }
 
 __global__ void __launch_bounds__(TAIL_THREADS, 1) k_vcycle_tail(TailArgs a) {
-  pdl_sync();
+  pdl_launch_dependents();
+  {  // before the grid dependency: pull this CTA's rows of the dense operator (setup data) into L2
+    const bool dense0 = a.dense_level >= 0 && a.first <= a.dense_level;
+    if (dense0) {
+      const int nD = a.lv[a.dense_level].n;
+      const int i0 = (int)((int64_t)blockIdx.x * nD / gridDim.x), i1 = (int)((int64_t)(blockIdx.x + 1) * nD / gridDim.x);
+      const char* p0 = reinterpret_cast<const char*>(a.dense_B + (size_t)i0 * nD);
+      const size_t bytes = (size_t)(i1 - i0) * nD * sizeof(double);
+      for (size_t o = (size_t)threadIdx.x * 128; o < bytes; o += (size_t)TAIL_THREADS * 128)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + o));
+    }
+  }
+  pdl_wait();
   if (a.ctl != nullptr && a.ctl->done) return;
   extern __shared__ __align__(128) unsigned char tail_sm[];
   __shared__ uint64_t lvbar[TAIL_MAX_LEVELS];
