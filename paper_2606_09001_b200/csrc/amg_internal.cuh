@@ -19,7 +19,13 @@
 #define RT_CTAS_CFG 2
 #endif
 #ifndef RT_STAGE_BYTES_CFG
-#define RT_STAGE_BYTES_CFG 36864
+#define RT_STAGE_BYTES_CFG 29696
+#endif
+#ifndef RT_XSLOTS_CFG
+#define RT_XSLOTS_CFG 4
+#endif
+#ifndef RT_XSLOT_BYTES_CFG
+#define RT_XSLOT_BYTES_CFG 5632
 #endif
 constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA (8 warps walk the ELL slices)
 #ifndef RT_GATHERERS_CFG
@@ -33,6 +39,8 @@ constexpr int RT_THREADS = RT_CONSUMERS + 32 + RT_GATHERERS;  // + one producer 
 constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA
 constexpr int RT_CTAS = RT_CTAS_CFG;               // persistent CTAs per SM
 constexpr int RT_STAGE_BYTES = RT_STAGE_BYTES_CFG; // shared memory of one ring stage (descriptor + operands of one tile)
+constexpr int RT_XSLOTS = RT_XSLOTS_CFG;           // x slots (side ring): how many tiles the gather warps run ahead
+constexpr int RT_XSLOT_BYTES = RT_XSLOT_BYTES_CFG; // one x slot: 8 bytes x (rows + halo columns of a tile)
 constexpr int RT_MAX_NNZ = 4096;                   // most entries / halo columns of a tile (packer scratch)
 constexpr int RT_MAX_ROWS = 1024;                  // most rows of a tile
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
@@ -86,6 +94,8 @@ struct Level {
   int* blk_ptr = nullptr;   // [nblk+1]
   TileDesc* tiles = nullptr;  // [nblk]
   unsigned char* blob = nullptr;  // tile-packed operator (amg_tilepack.cuh), fast levels only
+  int* halo_idx = nullptr;        // halo lists of all tiles, concatenated
+  int* halo_cagg = nullptr;       // coarse index of every halo entry
   size_t blob_bytes = 0;
   int nblk = 0;
   int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback

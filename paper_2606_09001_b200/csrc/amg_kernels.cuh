@@ -44,6 +44,8 @@ struct RowArgs {
   const int* agg;       // prolongation / restriction
   const int* agg_ptr;
   const unsigned char* blob;  // tile-packed operator (row-tile kernels)
+  const int* halo_idx;        // halo lists of the tiles
+  const int* halo_cagg;
   const double* ec;
   double gamma;
   const double* d0;     // second operand of the fused dot (SpMV)
@@ -310,58 +312,56 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // ------------------------------------------------------------------------------------------
 // Row-tile streaming kernel (S1-S4) over the sorted-ELL tile blobs (amg_tilepack.cuh).
 // Persistent and warp-specialised: RT_CTAS CTAs per SM, each owning a contiguous run of tiles;
-// per CTA 8 consumer warps + 1 producer warp + 2 gather warps around a ring of RT_STAGES stages.
+// per CTA 8 consumer warps + 1 producer warp + 6 gather warps, a ring of RT_STAGES operator
+// stages and a side ring of RT_XSLOTS x slots.
 //
-//   producer (1 thread)  waits for "empty", writes the stage header and issues the bulk-async
-//                        copies (TMA) of the tile: its blob (one copy) and its slices of x, b,
-//                        dinv, agg / agg_ptr and of the coarse vector -> mbarrier "full"
-//   gather warps         wait for "full", fetch the x value of every distinct halo column of the
-//                        tile (once per column, independent loads, L2) into the stage, apply
-//                        the per-row transform of the fused operations to the tile's own rows
-//                        (x1 = dinv o b;  x~ = x + gamma ec[agg]) -> mbarrier "ready"
-//   consumer warps       wait for "ready"; slices of 32 storage rows are dealt round-robin to
-//                        the warps ACROSS tiles; one lane per row walks the slice's k-major slots:
-//                        three shared-memory reads and one DFMA per entry, no divergence, no
-//                        global gather, no row pointers; epilogue per row; -> mbarrier "empty"
+//   producer (1 thread)  waits for a stage's "empty", writes its header and issues the bulk-async
+//                        copies (TMA) of the tile: its blob (one copy) and its slices of b, dinv
+//                        / agg_ptr -> mbarrier "full"
+//   gather warps         assemble the tile's x slot [x of its rows | x of its halo columns]: they
+//                        read the tile descriptor and its halo list straight from global memory,
+//                        gather once per distinct column (independent loads) and apply the per-row
+//                        transform of the fused operations (x1 = dinv o b;  x~ = x + gamma
+//                        ec[agg]) -> "xready".  They do not touch the operator ring, so they run
+//                        up to RT_XSLOTS tiles ahead of the row walk: the gather latency is off the
+//                        critical path of a stage (bulk copy -> row walk -> refill)
+//   consumer warps       wait for "full" and "xready"; slices of 32 storage rows are dealt
+//                        round-robin to the warps ACROSS tiles; one lane per row walks the slice's
+//                        k-major slots: three shared-memory reads and one DFMA per entry, no
+//                        divergence, no global gather, no row pointers; epilogue per row;
+//                        -> "empty", "xempty"
 //
-// There is no CTA-wide barrier: HBM keeps streaming whatever the consumers are doing, the gather
-// latency is hidden one stage ahead, and warps drift across tiles (the round-robin deal balances
-// them).  Only the restriction needs the tile's rows together (sum over an aggregate's rows): its
-// consumers meet on a fourth mbarrier per tile.
+// There is no CTA-wide barrier: HBM keeps streaming whatever the consumers are doing and warps
+// drift across tiles (the round-robin deal balances them).  Only the restriction needs the tile's
+// rows together (sum over an aggregate's rows): its consumers meet on one more mbarrier per tile.
 // ------------------------------------------------------------------------------------------
 namespace rt {
-constexpr int HEADER_BYTES = 256;  // full / ready / empty / resdone / pre mbarriers, RT_STAGES each
-constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * RT_STAGE_BYTES;
+constexpr int HEADER_BYTES = 256;  // full / empty / resdone / pre [RT_STAGES], xready / xempty [RT_XSLOTS]
+constexpr int SMEM_BYTES = HEADER_BYTES + RT_STAGES * RT_STAGE_BYTES + RT_XSLOTS * RT_XSLOT_BYTES;
 constexpr int NCW = RT_CONSUMERS / 32;  // consumer warps
 constexpr int NGW = RT_GATHERERS / 32;  // gather warps
-static_assert(RT_STAGES >= 2 && 5 * RT_STAGES * 8 <= HEADER_BYTES, "2..8 stages");
-static_assert(RT_STAGE_BYTES % 128 == 0, "stage size must keep 128-byte alignment");
+static_assert(RT_STAGES >= 2 && (4 * RT_STAGES + 2 * RT_XSLOTS) * 8 <= HEADER_BYTES, "too many stages / slots");
+static_assert(RT_STAGE_BYTES % 128 == 0 && RT_XSLOT_BYTES % 128 == 0, "stage / slot sizes must keep 128-byte alignment");
 static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
 static_assert((NCW & (NCW - 1)) == 0, "consumer warps must be a power of two");
 }  // namespace rt
 
 struct StageDesc {  // TP_DESC_BYTES at the start of a stage, written by the producer
   int r0, nr, I0, nA;
-  int nsl, nhalo, roff, pad0;
-  int o_halo, o_perm, o_col, o_val;
-  int o_cagg, o_b, o_d, o_agg;  // o_agg: agg slice (prolongation) or agg_ptr slice (restriction)
-  int o_ec, o_xcat, o_out, aoff;  // aoff: r0 - ra4 (agg slice) or I0 - Ia4 (agg_ptr slice)
-  int eoff, pad1, pad2, pad3;     // eoff: Ia2 (es[I - eoff] = ec[I])
-  int pad4[8];
+  int nsl, nhalo, roff, aoff;    // roff = r0 - ra2 (b / dinv slices), aoff = I0 - Ia4 (agg_ptr slice)
+  int o_perm, o_col, o_val, o_b;
+  int o_d, o_agg, o_out, pad0;
+  int pad1[16];
 };
 static_assert(sizeof(StageDesc) == TP_DESC_BYTES, "stage header size");
 
-// which operands of the tile are staged for which operation
+// which operands of the tile are staged in the ring for which operation
 template <int OP>
 struct TileOps {
-  static constexpr bool X = (OP != OP_JACOBI0);
   static constexpr bool B = (OP != OP_SPMV);
   static constexpr bool D = (OP == OP_JACOBI || OP == OP_JACOBI0 || OP == OP_JACOBI_PROLONG);
-  static constexpr bool AGG = (OP == OP_JACOBI_PROLONG);
-  static constexpr bool EC = (OP == OP_JACOBI_PROLONG);
   static constexpr bool AGGPTR = (OP == OP_RESTRICT);
-  static constexpr int FLAGS = (B ? TP_B : 0) | (D ? TP_D : 0) | (AGG ? TP_AGG | TP_CAGG : 0) | (EC ? TP_EC : 0) |
-                               (AGGPTR ? TP_AGGPTR | TP_OUT : 0);
+  static constexpr int FLAGS = (B ? TP_B : 0) | (D ? TP_D : 0) | (AGGPTR ? TP_AGGPTR | TP_OUT : 0);
 };
 
 // mode 0: header + every copy, all on `bar`;  mode 1: header + the blob copy only, on `bar` (issued
@@ -372,61 +372,78 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
   using T = TileOps<OP>;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
   const int flags = T::FLAGS | (d0_staged ? TP_B : 0);
-  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
   const StageLayout t = tp_stage(d, flags);
-  StageDesc sd;
-  sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
-  sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.pad0 = 0;
-  sd.o_halo = p.o_halo, sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val;
-  sd.o_cagg = p.o_cagg, sd.o_b = t.o_b, sd.o_d = t.o_d, sd.o_agg = t.o_agg;
-  sd.o_ec = t.o_ec, sd.o_xcat = t.o_xcat, sd.o_out = t.o_out;
-  sd.aoff = T::AGGPTR ? d.I0 - t.Ia4 : d.r0 - t.ra4;
-  sd.eoff = t.Ia2, sd.pad1 = sd.pad2 = sd.pad3 = 0;
   if (mode != 2) {
+    StageDesc sd;
+    sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
+    sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
+    sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_b = t.o_b;
+    sd.o_d = t.o_d, sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.pad0 = 0;
     int4* dst = reinterpret_cast<int4*>(stage);
     const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
-    for (int q = 0; q < 6; ++q) dst[q] = src[q];
+    for (int q = 0; q < 4; ++q) dst[q] = src[q];
   }
   if (d.nr <= 0) {
     mbar_arrive(bar);
     return;
   }
   unsigned char* base = stage + TP_DESC_BYTES;
-  const uint32_t nblob = (uint32_t)(T::AGG ? p.endB : p.endA);
+  const uint32_t nblob = (uint32_t)p.end;
   const uint32_t nrv8 = 8u * (uint32_t)t.nrv;
+  const bool has_vec = T::B || d0_staged || T::D || T::AGGPTR;
   uint32_t bytes = 0;
   if (mode != 2) bytes += nblob;
   if (mode != 1) {
-    if (T::X) bytes += nrv8;
     if (T::B || d0_staged) bytes += nrv8;
     if (T::D) bytes += nrv8;
-    if (T::AGG) bytes += 4u * (uint32_t)t.nr4;
-    if (T::EC) bytes += 8u * (uint32_t)t.nec;
     if (T::AGGPTR) bytes += 4u * (uint32_t)t.nap;
+  }
+  if (mode == 2 && !has_vec) {  // nothing but the blob is staged (SpMV without a second dot operand)
+    mbar_arrive(bar);
+    return;
   }
   mbar_arrive_expect_tx(bar, bytes);
   if (mode != 2) bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, nblob, bar, pol);
   if (mode != 1) {
-    if (T::X) bulk_g2s<false>(base + t.o_xcat, a.x + t.ra2, nrv8, bar, pol);
     if (T::B) bulk_g2s<false>(base + t.o_b, a.b + t.ra2, nrv8, bar, pol);
     if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra2, nrv8, bar, pol);
     if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, nrv8, bar, pol);
-    if (T::AGG) bulk_g2s<false>(base + t.o_agg, a.agg + t.ra4, 4u * (uint32_t)t.nr4, bar, pol);
-    if (T::EC) bulk_g2s<false>(base + t.o_ec, a.ec + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
     if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
   }
 }
+
+// value of the gathered vector at index i of the level (the fused operations transform it on the fly)
+template <int OP>
+__device__ __forceinline__ double xvalue_local(const RowArgs& a, int i) {
+  if (OP == OP_JACOBI0) return __ldg(a.dinv + i) * __ldg(a.b + i);
+  if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + i) + a.gamma * __ldg(a.ec + __ldg(a.agg + i));
+  return __ldg(a.x + i);
+}
+
+struct GTile {  // what the gather warps need of a tile descriptor
+  int r0, nr, nhalo, hoff;
+  __device__ __forceinline__ void load(const RowArgs& a, int t_begin, int my, int it) {
+    r0 = nr = nhalo = hoff = 0;
+    if (it < my) {
+      const TileDesc* d = a.tiles + t_begin + it;
+      r0 = __ldg(&d->r0), nr = __ldg(&d->nr), nhalo = __ldg(&d->nhalo), hoff = __ldg(&d->halo_off);
+    }
+  }
+};
 
 template <int OP, int NDOT, bool STREAM>
 __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
-  uint64_t* ready = full + RT_STAGES;
-  uint64_t* empty = ready + RT_STAGES;
+  uint64_t* empty = full + RT_STAGES;
   uint64_t* resdone = empty + RT_STAGES;
   uint64_t* pre = resdone + RT_STAGES;  // blobs of the first RT_STAGES tiles, issued before the grid dependency
+  uint64_t* xready = pre + RT_STAGES;
+  uint64_t* xempty = xready + RT_XSLOTS;
   unsigned char* stage0 = smem + rt::HEADER_BYTES;
+  unsigned char* xslot0 = stage0 + RT_STAGES * RT_STAGE_BYTES;
   const int tid = threadIdx.x;
   const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
   const int t_end = (int)((int64_t)(blockIdx.x + 1) * a.ntiles / gridDim.x);
@@ -437,10 +454,13 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (tid == 0) {
     for (int s = 0; s < RT_STAGES; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(ready + s, rt::NGW);
       mbar_init(empty + s, rt::NCW);
       mbar_init(resdone + s, rt::NCW);
       mbar_init(pre + s, 1);
+    }
+    for (int q = 0; q < RT_XSLOTS; ++q) {
+      mbar_init(xready + q, rt::NGW);
+      mbar_init(xempty + q, rt::NCW);
     }
     fence_mbar_init();
   }
@@ -450,6 +470,21 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   if (tid == RT_CONSUMERS)
     for (int it = 0; it < npre; ++it)
       tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, pre + it, pol, 1);
+  // gather warps: descriptors of their first two tiles and the halo indices of the first (setup data too)
+  constexpr int GU = RT_GATHER_UNROLL, GS = RT_GATHERERS;
+  const int g = tid - (RT_CONSUMERS + 32);
+  GTile gc, gn;
+  int idx[GU], cag[GU];
+  gc.load(a, t_begin, my, 0);
+  gn.load(a, t_begin, my, 1);
+  if (g >= 0) {
+#pragma unroll
+    for (int u = 0; u < GU; ++u) {
+      const int h = g + u * GS;
+      idx[u] = h < gc.nhalo ? __ldg(a.halo_idx + gc.hoff + h) : -1;
+      if (OP == OP_JACOBI_PROLONG) cag[u] = h < gc.nhalo ? __ldg(a.halo_cagg + gc.hoff + h) : 0;
+    }
+  }
   pdl_wait();
   if (a.ctl != nullptr && a.ctl->done) {
     if (tid == RT_CONSUMERS)  // the copies in flight target this CTA's shared memory: let them land
@@ -461,74 +496,67 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   for (int j = 0; j < (NDOT > 0 ? NDOT : 1); ++j) dots[j] = 0.0;
 
   if (tid >= RT_CONSUMERS + 32) {
-    // ---------------- gather warps ----------------
-    const int g = tid - (RT_CONSUMERS + 32);
+    // ---------------- gather warps: x slots, up to RT_XSLOTS tiles ahead ----------------
+    // software pipeline: while tile `it` is gathered, the halo indices of tile it+1 and the
+    // descriptor of tile it+2 are already on their way
     for (int it = 0; it < my; ++it) {
-      const int s = it % RT_STAGES;
-      unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
-      if (it < RT_STAGES) mbar_wait(pre + s, 0);
-      mbar_wait(full + s, (uint32_t)((it / RT_STAGES) & 1));
-      const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
-      const int nr = sd->nr, nhalo = sd->nhalo;
-      if (nr > 0) {
-        unsigned char* base = stage + TP_DESC_BYTES;
-        const int* hl = reinterpret_cast<const int*>(base + sd->o_halo);
-        double* xc = reinterpret_cast<double*>(base + sd->o_xcat) + sd->roff;  // xc[col]
-        double* xh = xc + nr;
-        constexpr int GU = RT_GATHER_UNROLL, GS = RT_GATHERERS;
-        if (OP == OP_JACOBI_PROLONG) {
-          const int* hc = reinterpret_cast<const int*>(base + sd->o_cagg);
-          const double gamma = a.gamma;
-          int h = g;
-          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
-            double v[GU], e[GU];
+      const int q = it % RT_XSLOTS;
+      GTile gnn;
+      gnn.load(a, t_begin, my, it + 2);
+      int idxn[GU], cagn[GU];
 #pragma unroll
-            for (int q = 0; q < GU; ++q) {
-              v[q] = __ldg(a.x + hl[h + q * GS]);
-              e[q] = __ldg(a.ec + hc[h + q * GS]);
-            }
-#pragma unroll
-            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q] + gamma * e[q];
-          }
-          for (; h < nhalo; h += GS) xh[h] = __ldg(a.x + hl[h]) + gamma * __ldg(a.ec + hc[h]);
-          const int* as = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;    // as[lr] = agg[r0 + lr]
-          const double* es = reinterpret_cast<const double*>(base + sd->o_ec) - sd->eoff;  // es[I] = ec[I]
-          for (int lr = g; lr < nr; lr += GS) xc[lr] += gamma * es[as[lr]];
-        } else if (OP == OP_JACOBI0) {
-          int h = g;
-          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
-            double v[GU], e[GU];
-#pragma unroll
-            for (int q = 0; q < GU; ++q) {
-              const int c = hl[h + q * GS];
-              v[q] = __ldg(a.dinv + c);
-              e[q] = __ldg(a.b + c);
-            }
-#pragma unroll
-            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q] * e[q];
-          }
-          for (; h < nhalo; h += GS) {
-            const int c = hl[h];
-            xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
-          }
-          const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
-          const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
-          for (int lr = g; lr < nr; lr += GS) xc[lr] = ds[lr] * bs[lr];
-        } else {
-          int h = g;
-          for (; h + (GU - 1) * GS < nhalo; h += GU * GS) {
-            double v[GU];
-#pragma unroll
-            for (int q = 0; q < GU; ++q) v[q] = __ldg(a.x + hl[h + q * GS]);
-#pragma unroll
-            for (int q = 0; q < GU; ++q) xh[h + q * GS] = v[q];
-          }
-          for (; h < nhalo; h += GS) xh[h] = __ldg(a.x + hl[h]);
-        }
-        fence_proxy_async();  // generic writes into a region a later bulk copy overwrites
+      for (int u = 0; u < GU; ++u) {
+        const int h = g + u * GS;
+        idxn[u] = h < gn.nhalo ? __ldg(a.halo_idx + gn.hoff + h) : -1;
+        if (OP == OP_JACOBI_PROLONG) cagn[u] = h < gn.nhalo ? __ldg(a.halo_cagg + gn.hoff + h) : 0;
       }
+      if (it >= RT_XSLOTS) mbar_wait(xempty + q, (uint32_t)(((it / RT_XSLOTS) - 1) & 1));
+      double* xc = reinterpret_cast<double*>(xslot0 + q * RT_XSLOT_BYTES);  // xc[col]: rows, then halo
+      double* xh = xc + gc.nr;
+      {
+        double v[GU], e[GU];
+#pragma unroll
+        for (int u = 0; u < GU; ++u) {
+          const int c = idx[u];
+          v[u] = 0.0, e[u] = 0.0;
+          if (c >= 0) {
+            if (OP == OP_JACOBI_PROLONG) {
+              v[u] = __ldg(a.x + c);
+              e[u] = __ldg(a.ec + cag[u]);
+            } else if (OP == OP_JACOBI0) {
+              v[u] = __ldg(a.dinv + c);
+              e[u] = __ldg(a.b + c);
+            } else {
+              v[u] = __ldg(a.x + c);
+            }
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < GU; ++u)
+          if (idx[u] >= 0) {
+            if (OP == OP_JACOBI_PROLONG)
+              xh[g + u * GS] = v[u] + a.gamma * e[u];
+            else if (OP == OP_JACOBI0)
+              xh[g + u * GS] = v[u] * e[u];
+            else
+              xh[g + u * GS] = v[u];
+          }
+        for (int h = g + GU * GS; h < gc.nhalo; h += GS) {  // more halo columns than the index registers hold
+          const int c = __ldg(a.halo_idx + gc.hoff + h);
+          if (OP == OP_JACOBI_PROLONG)
+            xh[h] = __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.halo_cagg + gc.hoff + h));
+          else if (OP == OP_JACOBI0)
+            xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
+          else
+            xh[h] = __ldg(a.x + c);
+        }
+      }
+      for (int lr = g; lr < gc.nr; lr += GS) xc[lr] = xvalue_local<OP>(a, gc.r0 + lr);
       __syncwarp();
-      if ((tid & 31) == 0) mbar_arrive(ready + s);
+      if ((tid & 31) == 0) mbar_arrive(xready + q);
+      gc = gn, gn = gnn;
+#pragma unroll
+      for (int u = 0; u < GU; ++u) idx[u] = idxn[u], cag[u] = cagn[u];
     }
   } else if (tid >= RT_CONSUMERS) {
     // ---------------- producer warp ----------------
@@ -547,12 +575,12 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     const int lane = tid & 31, w = tid >> 5;
     int sbase = 0;  // slices of the tiles so far: the round-robin deal continues across tiles
     for (int it = 0; it < my; ++it) {
-      const int s = it % RT_STAGES;
+      const int s = it % RT_STAGES, q = it % RT_XSLOTS;
       const uint32_t par = (uint32_t)((it / RT_STAGES) & 1);
       unsigned char* stage = stage0 + s * RT_STAGE_BYTES;
       if (it < RT_STAGES) mbar_wait(pre + s, 0);
-      mbar_wait(full + s, par);   // the bulk copies have landed ...
-      mbar_wait(ready + s, par);  // ... and the gather warps are done with the stage
+      mbar_wait(full + s, par);                                      // the bulk copies have landed ...
+      mbar_wait(xready + q, (uint32_t)((it / RT_XSLOTS) & 1));       // ... and the tile's x slot is assembled
       const StageDesc* sd = reinterpret_cast<const StageDesc*>(stage);
       const int nr = sd->nr, nsl = sd->nsl, r0 = sd->r0;
       if (nr > 0) {
@@ -561,7 +589,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
         const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + sd->o_perm);
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
-        const double* xc = reinterpret_cast<const double*>(base + sd->o_xcat) + sd->roff;
+        const double* xc = reinterpret_cast<const double*>(xslot0 + q * RT_XSLOT_BYTES);
         const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
         double* outs = reinterpret_cast<double*>(base + sd->o_out);
@@ -603,9 +631,13 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
         }
       }
       sbase = (sbase + nsl) & (rt::NCW - 1);
-      // ---- this warp is done with the stage ----
+      // ---- this warp is done with the stage and the x slot ----
+      if (OP == OP_RESTRICT) fence_proxy_async();  // residuals were written into a region the next bulk copy overwrites
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty + s);
+      if (lane == 0) {
+        mbar_arrive(empty + s);
+        mbar_arrive(xempty + q);
+      }
     }
   }
   if (NDOT > 0) grid_reduce_finalize<(NDOT > 0 ? NDOT : 1), RT_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);

@@ -553,8 +553,8 @@ __global__ void k_gather_double(int n, const double* __restrict__ src, const int
 // Row-tile partition by shared-memory bytes: a row weighs RT_ROW_WEIGHT bytes of staged row
 // operands, a nonzero RT_NNZ_WEIGHT (value, 16-bit column, its share of the halo list and values).  Tile k starts at the first unit (aggregate, or row if
 // unit_ptr == null) whose cumulative weight is at or beyond k * target.
-constexpr int RT_ROW_WEIGHT = 44;
-constexpr int RT_NNZ_WEIGHT = 13;
+constexpr int RT_ROW_WEIGHT = 24;
+constexpr int RT_NNZ_WEIGHT = 10;
 __device__ __forceinline__ int64_t tile_weight(const int* __restrict__ rowptr, int r) {
   return RT_NNZ_WEIGHT * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
 }
@@ -591,8 +591,10 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
                                                            const int* __restrict__ rowptr, const int* __restrict__ col,
                                                            const double* __restrict__ val, const int* __restrict__ agg,
                                                            int write, const int* __restrict__ blob_off16,
-                                                           int* __restrict__ size16, int* __restrict__ info,
-                                                           TileDesc* __restrict__ tiles, unsigned char* __restrict__ blob) {
+                                                           const int* __restrict__ halo_off, int* __restrict__ size16,
+                                                           int* __restrict__ nhalo_out, int* __restrict__ info,
+                                                           TileDesc* __restrict__ tiles, unsigned char* __restrict__ blob,
+                                                           int* __restrict__ halo_idx, int* __restrict__ halo_cagg) {
   __shared__ int ext[RT_MAX_NNZ];
   __shared__ int halo[RT_MAX_NNZ];
   __shared__ int len[RT_MAX_ROWS];
@@ -606,10 +608,11 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   const int r0 = blk_ptr[t], r1 = blk_ptr[t + 1], nr = r1 - r0;
   TileDesc d;
   d.r0 = r0, d.nr = nr, d.I0 = 0, d.nA = 0, d.nsl = 0, d.nslots = 0, d.nhalo = 0, d.blob16 = 0;
+  d.halo_off = 0, d.pad0 = d.pad1 = d.pad2 = 0;
   if (nr <= 0) {
     if (tid == 0) {
       if (write) tiles[t] = d;
-      else size16[t] = 0;
+      else size16[t] = 0, nhalo_out[t] = 0;
     }
     return;
   }
@@ -617,7 +620,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   if (nr > RT_MAX_ROWS || k1 - k0 > RT_MAX_NNZ) {
     if (tid == 0) {
       info[1] = 1;
-      if (!write) size16[t] = 0;
+      if (!write) size16[t] = 0, nhalo_out[t] = 0;
     }
     return;
   }
@@ -642,7 +645,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   if (s_maxlen > PK_MAX_LEN) {
     if (tid == 0) {
       info[1] = 1;
-      if (!write) size16[t] = 0;
+      if (!write) size16[t] = 0, nhalo_out[t] = 0;
     }
     return;
   }
@@ -710,26 +713,26 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   }
   __syncthreads();
   d.nsl = nsl, d.nslots = s_nslots, d.nhalo = s_nhalo;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
   if (!write) {
     if (tid == 0) {
-      size16[t] = p.endB / 16;
+      size16[t] = p.end / 16;
+      nhalo_out[t] = d.nhalo;
       atomicMax(&info[0], tp_stage_need(d));
+      atomicMax(&info[2], tp_xslot_need(d));
     }
     return;
   }
   d.blob16 = (uint32_t)blob_off16[t];
+  d.halo_off = halo_off[t];
   unsigned char* base = blob + (size_t)d.blob16 * 16u;
   if (tid == 0) tiles[t] = d;
   int2* o_sl = reinterpret_cast<int2*>(base);
   for (int j = tid; j < nsl; j += PK_THREADS) o_sl[j] = make_int2(sl_off[j], sl_w[j]);
-  int* o_halo = reinterpret_cast<int*>(base + p.o_halo);
-  int* o_cagg = reinterpret_cast<int*>(base + p.o_cagg);
-  const int nh4 = tp_up(d.nhalo, 4);
-  for (int h = tid; h < nh4; h += PK_THREADS) {
-    const int c = h < d.nhalo ? halo[h] : 0;
-    o_halo[h] = c;
-    o_cagg[h] = (h < d.nhalo && agg != nullptr) ? agg[c] : 0;
+  for (int h = tid; h < d.nhalo; h += PK_THREADS) {
+    const int c = halo[h];
+    halo_idx[d.halo_off + h] = c;
+    halo_cagg[d.halo_off + h] = agg != nullptr ? agg[c] : 0;
   }
   unsigned short* o_perm = reinterpret_cast<unsigned short*>(base + p.o_perm);
   for (int s = tid; s < nsl * 32; s += PK_THREADS) o_perm[s] = s < nr ? (unsigned short)srow[s] : (unsigned short)0xFFFF;
@@ -1105,43 +1108,54 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
         if (L.tiles) amg_dev_free(H, L.tiles);
         L.blk_ptr = nullptr, L.tiles = nullptr;
         L.nblk = div_up(total_w, target);
-        int *size16, *off16, *info;
+        int *size16, *off16, *nh, *hoff, *info;
         AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
         AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
         AMG_ALLOC(H, size16, int, L.nblk + 1, st);
         AMG_ALLOC(H, off16, int, L.nblk + 1, st);
-        AMG_ALLOC(H, info, int, 2, st);
-        AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 2 * sizeof(int), st));
+        AMG_ALLOC(H, nh, int, L.nblk + 1, st);
+        AMG_ALLOC(H, hoff, int, L.nblk + 1, st);
+        AMG_ALLOC(H, info, int, 4, st);
+        AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 4 * sizeof(int), st));
         k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
                                                              q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
         k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr,
-                                                   0, nullptr, size16, info, L.tiles, nullptr);
+                                                   0, nullptr, nullptr, size16, nh, info, L.tiles, nullptr, nullptr,
+                                                   nullptr);
         AMG_CUDA_TRY(H, cudaGetLastError());
-        int h_info[2];
-        AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        int h_info[4];
+        AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
         AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
         if (h_info[1]) {
           scale *= 0.5;
-        } else if (h_info[0] > RT_STAGE_BYTES) {
-          scale *= 0.96 * (double)RT_STAGE_BYTES / (double)h_info[0];
+        } else if (h_info[0] > RT_STAGE_BYTES || h_info[2] > RT_XSLOT_BYTES) {
+          const double f1 = (double)RT_STAGE_BYTES / (double)h_info[0], f2 = (double)RT_XSLOT_BYTES / (double)h_info[2];
+          scale *= 0.96 * (f1 < f2 ? f1 : f2);
         } else {
           AMG_TRY(amg_exclusive_scan(H, size16, off16, L.nblk, st));
-          int total16 = 0;
+          AMG_TRY(amg_exclusive_scan(H, nh, hoff, L.nblk, st));
+          int total16 = 0, total_h = 0;
           AMG_TRY(read_int(H, off16 + L.nblk, &total16, st));
+          AMG_TRY(read_int(H, hoff + L.nblk, &total_h, st));
           L.blob_bytes = (size_t)total16 * 16u;
           L.blob = (unsigned char*)amg_dev_alloc(H, L.blob_bytes + 16, st);
           if (!L.blob) {
             H->err = "device allocation failed: tile blobs";
             return AMG_ERR_OOM;
           }
+          AMG_ALLOC(H, L.halo_idx, int, total_h + 4, st);
+          AMG_ALLOC(H, L.halo_cagg, int, total_h + 4, st);
           k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val,
-                                                     q < Lc ? L.agg : nullptr, 1, off16, size16, info, L.tiles, L.blob);
+                                                     q < Lc ? L.agg : nullptr, 1, off16, hoff, size16, nh, info, L.tiles,
+                                                     L.blob, L.halo_idx, L.halo_cagg);
           AMG_CUDA_TRY(H, cudaGetLastError());
           AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
           L.fast = 1;
         }
         amg_dev_free(H, size16);
         amg_dev_free(H, off16);
+        amg_dev_free(H, nh);
+        amg_dev_free(H, hoff);
         amg_dev_free(H, info);
       }
       if (!L.fast) {

@@ -98,6 +98,8 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
   a.agg = L.agg;
   a.agg_ptr = L.agg_ptr;
   a.blob = L.blob;
+  a.halo_idx = L.halo_idx;
+  a.halo_cagg = L.halo_cagg;
   a.gamma = H->opt.coarse_scale;
   a.partials = H->partials;
   a.counter = H->counter;

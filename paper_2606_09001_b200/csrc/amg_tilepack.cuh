@@ -7,95 +7,90 @@
 // bulk-async copy (TMA) brings into a ring stage:
 //
 //   slices  int2[nsl]      {first slot, width} of every slice of 32 storage rows
-//   halo    i32[nhalo]     level index of every distinct out-of-tile column, ascending
 //   perm    u16[32 nsl]    storage row -> tile-local row (0xFFFF: padding).  Storage rows are the
 //                          tile's rows sorted by descending length (stable), so the 32 rows of a
 //                          slice have (almost) the same length and the padding stays at a few %
 //   col     u16[nslots]    TILE-LOCAL column of every slot: < nr -> row r0+col of this tile,
-//                          >= nr -> entry (col - nr) of the halo list.  Slice-major; inside a slice
-//                          k-major: slot = first + 32 k + lane  (conflict-free shared-memory reads)
+//                          >= nr -> entry (col - nr) of the tile's halo list.  Slice-major; inside a
+//                          slice k-major: slot = first + 32 k + lane  (conflict-free shared-memory reads)
 //   val     f64[nslots]    matrix values, same order; padding slots are {col 0, val 0}
-//   cagg    i32[nhalo]     coarse index of every halo column (prolongation-fused sweep only)
 //
-// 10 bytes per stored entry instead of CSR's 12 (+4 per row), no row pointers; the x values of
-// the halo columns are fetched ONCE per distinct column into shared memory by dedicated warps, one
-// tile ahead of the row walk, so the inner loop reads shared memory only.  Within a row the
-// entries keep their CSR order (ascending column of the level numbering), so a row sum is
-// accumulated in the same order as by the CSR kernels and by the oracle.
+// and a range [halo_off, halo_off + nhalo) of the level's halo arrays
+//
+//   halo_idx  i32[]        level index of every distinct out-of-tile column of the tile, ascending
+//   halo_cagg i32[]        its coarse index (prolongation-fused sweep only)
+//
+// 10 bytes per stored entry instead of CSR's 12 (+4 per row), no row pointers.  The x values a
+// tile needs -- its own rows and its halo columns, once per distinct column -- are assembled in
+// shared memory by dedicated warps that run several tiles AHEAD of the row walk (they read the
+// halo lists straight from global memory and do not depend on the ring), so the inner loop reads
+// shared memory only.  Within a row the entries keep their CSR order (ascending column of the
+// level numbering), so a row sum is accumulated in the same order as by the CSR kernels and by
+// the oracle.
 #pragma once
 #include <stdint.h>
 
-struct alignas(16) TileDesc {  // 32 bytes per tile, read by the issuing thread
+struct alignas(16) TileDesc {  // 48 bytes per tile
   int32_t r0, nr;              // rows [r0, r0 + nr)
   int32_t I0, nA;              // coarse rows [I0, I0 + nA); nA = 0 on the coarsest level
   int32_t nsl, nslots;         // slices; stored slots (= sum of 32 * width)
   int32_t nhalo;
   uint32_t blob16;             // blob offset in 16-byte units
+  int32_t halo_off;            // first entry of the tile in the level's halo arrays
+  int32_t pad0, pad1, pad2;
 };
 
 __host__ __device__ inline int tp_up(int x, int m) { return (x + m - 1) / m * m; }
 
 struct BlobLayout {  // byte offsets inside the blob; all multiples of 16
-  int o_halo, o_perm, o_col, o_val, endA, o_cagg, endB;
+  int o_perm, o_col, o_val, end;
 };
-__host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots, int nhalo) {
+__host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots) {
   BlobLayout p;
-  p.o_halo = tp_up(8 * nsl, 16);
-  p.o_perm = p.o_halo + tp_up(4 * nhalo, 16);
+  p.o_perm = tp_up(8 * nsl, 16);
   p.o_col = p.o_perm + 64 * nsl;
   p.o_val = p.o_col + tp_up(2 * nslots, 16);
-  p.endA = p.o_val + 8 * nslots;
-  p.o_cagg = p.endA;
-  p.endB = p.o_cagg + tp_up(4 * nhalo, 16);
+  p.end = p.o_val + 8 * nslots;
   return p;
 }
 
 // Placement of a tile inside its ring stage, after the TP_DESC_BYTES stage header.  Row-vector
 // slices are rounded out to 16-byte boundaries of their source arrays (bulk copies need 16-byte
-// aligned addresses and sizes): ra2 / ra4 / Ia2 / Ia4 are the rounded-down first elements.
+// aligned addresses and sizes): ra2 / Ia4 are the rounded-down first elements.
 constexpr int TP_DESC_BYTES = 128;
 struct StageLayout {
   int ra2, nrv;    // first staged row of the f64 row vectors (even), entries staged (even)
-  int ra4, nr4;    // same for the i32 agg slice (multiple of 4)
-  int Ia2, nec;    // coarse-vector slice
   int Ia4, nap;    // agg_ptr slice (nA + 1 entries from I0)
-  int o_b, o_d, o_agg, o_ec, o_xcat, o_out, end;  // byte offsets (blob at 0)
+  int o_b, o_d, o_agg, o_out, end;  // byte offsets (blob at 0)
 };
-// flags: which operands the operation stages
-enum { TP_B = 1, TP_D = 2, TP_AGG = 4, TP_EC = 8, TP_AGGPTR = 16, TP_CAGG = 32, TP_OUT = 64 };
+// flags: which operands the operation stages in the ring
+enum { TP_B = 1, TP_D = 2, TP_AGGPTR = 16, TP_OUT = 64 };
 __host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
   StageLayout t;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.nhalo);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
   const int r1 = d.r0 + d.nr;
   t.ra2 = d.r0 & ~1;
   t.nrv = tp_up(r1 - t.ra2, 2);
-  t.ra4 = d.r0 & ~3;
-  t.nr4 = tp_up(r1 - t.ra4, 4);
-  t.Ia2 = d.I0 & ~1;
-  t.nec = tp_up(d.I0 + d.nA - t.Ia2, 2);
   t.Ia4 = d.I0 & ~3;
   t.nap = tp_up(d.I0 + d.nA + 1 - t.Ia4, 4);
-  int o = (flags & TP_CAGG) ? p.endB : p.endA;
+  int o = p.end;
   t.o_b = o;
   if (flags & TP_B) o += 8 * t.nrv;
   t.o_d = o;
   if (flags & TP_D) o += 8 * t.nrv;
   t.o_agg = o;
-  if (flags & TP_AGG) o += 4 * t.nr4;
   if (flags & TP_AGGPTR) o += 4 * t.nap;
-  t.o_ec = o;
-  if (flags & TP_EC) o += 8 * t.nec;
-  t.o_xcat = o;  // [x slice (nrv, rounded) | halo values]: index roff + col
-  o += 8 * tp_up(t.nrv + d.nhalo, 2);
   t.o_out = o;
   if (flags & TP_OUT) o += 8 * tp_up(d.nr, 2);
   t.end = o;
   return t;
 }
-constexpr int TP_FLAGS_JACP = TP_B | TP_D | TP_AGG | TP_EC | TP_CAGG;  // prolongation-fused sweep
+constexpr int TP_FLAGS_SWEEP = TP_B | TP_D;                            // Jacobi sweeps
 constexpr int TP_FLAGS_RESTRICT = TP_B | TP_AGGPTR | TP_OUT;           // residual + restriction
 // shared-memory bytes one ring stage needs for a tile, for the most demanding operations
 __host__ __device__ inline int tp_stage_need(const TileDesc& d) {
-  const int a = tp_stage(d, TP_FLAGS_JACP).end, b = tp_stage(d, TP_FLAGS_RESTRICT).end;
+  const int a = tp_stage(d, TP_FLAGS_SWEEP).end, b = tp_stage(d, TP_FLAGS_RESTRICT).end;
   return TP_DESC_BYTES + (a > b ? a : b);
 }
+// bytes of the tile's x slot (side ring): [x of the tile's rows | x of its halo columns]
+__host__ __device__ inline int tp_xslot_need(const TileDesc& d) { return 8 * (d.nr + d.nhalo); }
