@@ -510,48 +510,83 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
         idxn[u] = h < gn.nhalo ? __ldg(a.halo_idx + gn.hoff + h) : -1;
         if (OP == OP_JACOBI_PROLONG) cagn[u] = h < gn.nhalo ? __ldg(a.halo_cagg + gn.hoff + h) : 0;
       }
+      // every load of the tile is issued before anything is consumed: the slot is assembled in two
+      // memory round trips (one for the plain operations) however many rows and halo columns it has
+      constexpr int LU = (RT_XSLOT_BYTES / 8 + GS - 1) / GS;  // rows per gather thread, at most
+      double v[GU], e[GU], lv[LU], le[LU];
+      int la[LU];
+#pragma unroll
+      for (int u = 0; u < GU; ++u) {
+        const int c = idx[u];
+        v[u] = 0.0, e[u] = 0.0;
+        if (c >= 0) {
+          if (OP == OP_JACOBI_PROLONG) {
+            v[u] = __ldg(a.x + c);
+            e[u] = __ldg(a.ec + cag[u]);
+          } else if (OP == OP_JACOBI0) {
+            v[u] = __ldg(a.dinv + c);
+            e[u] = __ldg(a.b + c);
+          } else {
+            v[u] = __ldg(a.x + c);
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < LU; ++u) {
+        const int lr = g + u * GS;
+        lv[u] = 0.0, le[u] = 0.0, la[u] = 0;
+        if (lr < gc.nr) {
+          const int i = gc.r0 + lr;
+          if (OP == OP_JACOBI_PROLONG) {
+            lv[u] = __ldg(a.x + i);
+            la[u] = __ldg(a.agg + i);
+          } else if (OP == OP_JACOBI0) {
+            lv[u] = __ldg(a.dinv + i);
+            le[u] = __ldg(a.b + i);
+          } else {
+            lv[u] = __ldg(a.x + i);
+          }
+        }
+      }
+      if (OP == OP_JACOBI_PROLONG) {
+#pragma unroll
+        for (int u = 0; u < LU; ++u)
+          if (g + u * GS < gc.nr) le[u] = __ldg(a.ec + la[u]);
+      }
       if (it >= RT_XSLOTS) mbar_wait(xempty + q, (uint32_t)(((it / RT_XSLOTS) - 1) & 1));
       double* xc = reinterpret_cast<double*>(xslot0 + q * RT_XSLOT_BYTES);  // xc[col]: rows, then halo
       double* xh = xc + gc.nr;
-      {
-        double v[GU], e[GU];
 #pragma unroll
-        for (int u = 0; u < GU; ++u) {
-          const int c = idx[u];
-          v[u] = 0.0, e[u] = 0.0;
-          if (c >= 0) {
-            if (OP == OP_JACOBI_PROLONG) {
-              v[u] = __ldg(a.x + c);
-              e[u] = __ldg(a.ec + cag[u]);
-            } else if (OP == OP_JACOBI0) {
-              v[u] = __ldg(a.dinv + c);
-              e[u] = __ldg(a.b + c);
-            } else {
-              v[u] = __ldg(a.x + c);
-            }
-          }
+      for (int u = 0; u < GU; ++u)
+        if (idx[u] >= 0) {
+          if (OP == OP_JACOBI_PROLONG)
+            xh[g + u * GS] = v[u] + a.gamma * e[u];
+          else if (OP == OP_JACOBI0)
+            xh[g + u * GS] = v[u] * e[u];
+          else
+            xh[g + u * GS] = v[u];
         }
 #pragma unroll
-        for (int u = 0; u < GU; ++u)
-          if (idx[u] >= 0) {
-            if (OP == OP_JACOBI_PROLONG)
-              xh[g + u * GS] = v[u] + a.gamma * e[u];
-            else if (OP == OP_JACOBI0)
-              xh[g + u * GS] = v[u] * e[u];
-            else
-              xh[g + u * GS] = v[u];
-          }
-        for (int h = g + GU * GS; h < gc.nhalo; h += GS) {  // more halo columns than the index registers hold
-          const int c = __ldg(a.halo_idx + gc.hoff + h);
+      for (int u = 0; u < LU; ++u) {
+        const int lr = g + u * GS;
+        if (lr < gc.nr) {
           if (OP == OP_JACOBI_PROLONG)
-            xh[h] = __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.halo_cagg + gc.hoff + h));
+            xc[lr] = lv[u] + a.gamma * le[u];
           else if (OP == OP_JACOBI0)
-            xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
+            xc[lr] = lv[u] * le[u];
           else
-            xh[h] = __ldg(a.x + c);
+            xc[lr] = lv[u];
         }
       }
-      for (int lr = g; lr < gc.nr; lr += GS) xc[lr] = xvalue_local<OP>(a, gc.r0 + lr);
+      for (int h = g + GU * GS; h < gc.nhalo; h += GS) {  // more halo columns than the index registers hold
+        const int c = __ldg(a.halo_idx + gc.hoff + h);
+        if (OP == OP_JACOBI_PROLONG)
+          xh[h] = __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.halo_cagg + gc.hoff + h));
+        else if (OP == OP_JACOBI0)
+          xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
+        else
+          xh[h] = __ldg(a.x + c);
+      }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(xready + q);
       gc = gn, gn = gnn;
