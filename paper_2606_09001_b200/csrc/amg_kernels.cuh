@@ -876,10 +876,33 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __r
   if (ctl->done) return;
   const double alpha = ctl->alpha;
   double acc[1] = {0.0};
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
-    x[i] += alpha * p[i];
-    const double ri = r[i] - alpha * q[i];
-    r[i] = ri;
+  // 128-bit accesses, two independent pairs per thread and trip (the work vectors are 16-byte aligned)
+  const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* p2 = reinterpret_cast<const double2*>(p);
+  const double2* q2 = reinterpret_cast<const double2*>(q);
+  double2* x2 = reinterpret_cast<double2*>(x);
+  double2* r2 = reinterpret_cast<double2*>(r);
+  int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x;
+  for (; i + stride < n2; i += 2 * stride) {
+    const double2 pa = p2[i], pb = p2[i + stride], qa = q2[i], qb = q2[i + stride];
+    double2 xa = x2[i], xb = x2[i + stride], ra = r2[i], rb = r2[i + stride];
+    xa.x += alpha * pa.x, xa.y += alpha * pa.y, xb.x += alpha * pb.x, xb.y += alpha * pb.y;
+    ra.x -= alpha * qa.x, ra.y -= alpha * qa.y, rb.x -= alpha * qb.x, rb.y -= alpha * qb.y;
+    x2[i] = xa, x2[i + stride] = xb, r2[i] = ra, r2[i + stride] = rb;
+    acc[0] += (ra.x * ra.x + ra.y * ra.y) + (rb.x * rb.x + rb.y * rb.y);
+  }
+  for (; i < n2; i += stride) {
+    const double2 pa = p2[i], qa = q2[i];
+    double2 xa = x2[i], ra = r2[i];
+    xa.x += alpha * pa.x, xa.y += alpha * pa.y;
+    ra.x -= alpha * qa.x, ra.y -= alpha * qa.y;
+    x2[i] = xa, r2[i] = ra;
+    acc[0] += ra.x * ra.x + ra.y * ra.y;
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+    x[n - 1] += alpha * p[n - 1];
+    const double ri = r[n - 1] - alpha * q[n - 1];
+    r[n - 1] = ri;
     acc[0] += ri * ri;
   }
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, FIN_RR);

@@ -7,6 +7,7 @@
 // program following the same definition produces the same integers.
 #include <chrono>
 #include <cstdio>
+#include <cstdlib>
 
 #include "amg_internal.cuh"
 
@@ -1151,6 +1152,10 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
           AMG_CUDA_TRY(H, cudaGetLastError());
           AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
           L.fast = 1;
+          if (getenv("AMG_DEBUG_TILES"))
+            fprintf(stderr, "level %d: n %d nnz %d tiles %d (%.0f rows, %.0f halo per tile) blob %.1f MB stage need %d / %d, x slot need %d / %d, attempt %d\n",
+                    q, L.n, L.nnz, L.nblk, (double)L.n / L.nblk, (double)total_h / L.nblk, L.blob_bytes / 1e6, h_info[0],
+                    RT_STAGE_BYTES, h_info[2], RT_XSLOT_BYTES, attempt);
         }
         amg_dev_free(H, size16);
         amg_dev_free(H, off16);
