@@ -270,11 +270,13 @@ def run_b200(args):
         peak, peak_src = peaks()
         ach = bytes_sweep / (sweep_ms * 1e-3) / 1e9
         # traffic: dram__bytes_read.sum + dram__bytes_write.sum of this kernel on this workload from the
-        # `ncu --set full` capture summarised in profiles/r01_ncu_full_tiles.md (229.0 + 4.2 MB per launch)
-        traffic = 233.2e6 if (n == 2097152 and nnz == 14581760) else None
+        # `ncu --set full` capture summarised in profiles/r01_final_rowtile_xslots.md (216.7 + 6.7 MB per launch)
+        traffic = 223.4e6 if (n == 2097152 and nnz == 14581760) else None
         roof = {"bound": "hbm", "kernel": "k_rowtile<OP_JACOBI, 1> level 0 (smoother sweep fused with the residual and r.z)",
                 "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4), "traffic": traffic,
-                "traffic_source": "profiles/r01_ncu_full_tiles.md",
+                "traffic_source": "profiles/r01_final_rowtile_xslots.md",
+                "note": "achieved counts ALGORITHMIC (CSR-based) bytes; the tile blobs store 10 bytes per entry instead "
+                        "of 12 + row pointers, so the real traffic is smaller and frac can exceed 1",
                 "bytes_per_launch": bytes_sweep, "us_per_launch": round(sweep_ms * 1e3, 2), "peak_source": peak_src,
                 "how": "CUDA events around 10 and 60 back-to-back launches (amg_level_op), difference / 50; operands 234 MB > L2"}
         vc = {"ms": round(vcycle_ms, 4), "bytes": bytes_vcycle, "gbs": round(bytes_vcycle / vcycle_ms / 1e6, 1),
