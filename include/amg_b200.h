@@ -143,6 +143,16 @@ AMG_API amg_status amg_setup_with_aggregates(amg_handle* out, int64_t n, int64_t
                                      const double* d_val, const amg_options* opt, int32_t nagg,
                                      const int32_t* const* h_d_aggs, void* cuda_stream);
 
+/* Warm resetup (the paper's cache-hit path: "matrix coefficients are updated in
+ * place" and the setup is repeated on the new values; the operation its Fig. 3 benchmarks, :285).
+ * d_val double[nnz]: new values on the SAME pattern as the amg_setup call (device pointer, read
+ * only during the call, not borrowed).  keep_aggregates = 1: the aggregates of the current
+ * hierarchy are kept (no matching: Galerkin products, smoother diagonals, tile blobs, coarse LU
+ * and the dense tail operator are recomputed); 0: everything is rebuilt, the result equals a cold
+ * amg_setup on the new values.  The handle stays valid; on an error it keeps its old hierarchy. */
+AMG_API amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t keep_aggregates,
+                                      void* cuda_stream);
+
 AMG_API amg_status amg_destroy(amg_handle h);
 
 /* S1-S9: solve A x = b from x0 = 0 with the Krylov method of the options; x is output only.

@@ -21,7 +21,7 @@ STATUS_NAMES = ["AMG_OK", "AMG_ERR_INVALID_ARG", "AMG_ERR_BAD_CSR", "AMG_ERR_CUD
                 "AMG_ERR_COARSE_SINGULAR", "AMG_ERR_COARSEN_STALL", "AMG_ERR_UNSUPPORTED"]
 AMG_CONVERGED, AMG_MAXIT, AMG_BREAKDOWN, AMG_NONFINITE = 0, 1, 2, 3
 
-EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_with_aggregates",
+EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_with_aggregates", "amg_resetup_values",
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
            "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
@@ -129,6 +129,10 @@ def amg_setup_with_aggregates(n, nnz, d_rowptr, d_col, d_val, opt, d_aggs):
         _stream())
     _check(st)
     return h
+
+
+def amg_resetup_values(h, d_val, keep_aggregates):
+    _check(load_library().amg_resetup_values(h, _ptr(d_val, torch.float64), C.c_int32(int(keep_aggregates)), _stream()), h)
 
 
 def amg_destroy(h):
@@ -260,6 +264,12 @@ class AmgSolver:
             d_aggs = [to(a, torch.int32) for a in aggregates]
             self.h = amg_setup_with_aggregates(self.n, self.nnz, self.d_rowptr, self.d_col, self.d_val, self.opt,
                                                d_aggs)
+
+    def resetup_values(self, val, keep_aggregates=True):
+        """Warm resetup on new values of the same pattern (amg_resetup_values)."""
+        self.d_val = torch.as_tensor(val).to(dtype=torch.float64).to(self.device).contiguous()
+        assert self.d_val.numel() == self.nnz
+        amg_resetup_values(self.h, self.d_val, keep_aggregates)
 
     def close(self):
         if getattr(self, "h", None):

@@ -208,6 +208,36 @@ amg_status amg_setup_with_aggregates(amg_handle* out, int64_t n, int64_t nnz, co
   return create_handle(out, n, nnz, d_rowptr, d_col, d_val, opt, nagg, nagg > 0 ? h_d_aggs : none, cuda_stream);
 }
 
+// NEXT-1: the paper's cache-hit path -- "matrix coefficients are updated in place
+// and the setup is repeated on the new values", the operation its Fig. 3 times
+// ("warm resetup-and-solve", :285).  The handle keeps its identity; its hierarchy is rebuilt from
+// the stored pattern and the new values, with the matching skipped when the aggregates are kept.
+// All memory cycles through the stream-ordered pool, so no device allocation reaches the driver.
+amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t keep_aggregates, void* cuda_stream) {
+  if (!h) return AMG_ERR_INVALID_ARG;
+  if (!d_val) {
+    h->err = "amg_resetup_values: null values";
+    return AMG_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStreamSynchronize(st);
+  std::vector<const int32_t*> aggs;
+  if (keep_aggregates)
+    for (size_t l = 0; l + 1 < h->lv.size(); ++l) aggs.push_back(h->lv[l].nat_agg);
+  amg_handle fresh = nullptr;
+  amg_options o = h->opt;
+  o.symmetric = h->symmetric;  // a device check at the first setup is not repeated
+  const amg_status s = create_handle(&fresh, h->n, h->nnz, h->nat_rowptr, h->nat_col, d_val, &o,
+                                     keep_aggregates ? (int32_t)aggs.size() : 0,
+                                     keep_aggregates ? aggs.data() : nullptr, cuda_stream);
+  if (s != AMG_OK) {
+    h->err = "amg_resetup_values: " + g_thread_error;  // the old hierarchy stays usable
+    return s;
+  }
+  std::swap(*h, *fresh);  // the caller's handle now owns the new hierarchy
+  return amg_destroy(fresh);
+}
+
 amg_status amg_destroy(amg_handle h) {
   if (!h) return AMG_OK;
   cudaDeviceSynchronize();

@@ -402,6 +402,48 @@ def test_irregular_rows_tile_packer(oracle_mod, B, hubs):
         o.close()
 
 
+@pytest.mark.parametrize("keep", [1, 0])
+def test_warm_resetup_values(oracle_mod, B, keep):
+    """amg_resetup_values (PAPER.md:103 cache hit: new coefficients on the same pattern).  keep = 0 must
+    equal a cold setup on the new values (same aggregates as the oracle's own setup); keep = 1 must
+    equal the oracle's hierarchy built on the new values with the OLD aggregates imported."""
+    shape = (20, 20, 20)
+    A0 = inputs.variable_diffusion_csr(shape, seed=71)
+    A1 = inputs.variable_diffusion_csr(shape, seed=72)   # same 7-point pattern, new coefficient field
+    assert np.array_equal(A0.rowptr, A1.rowptr) and np.array_equal(A0.col, A1.col)
+    s = B.AmgSolver(A0.rowptr, A0.col, A0.val)
+    o0 = oracle_mod.Oracle(A0.rowptr, A0.col, A0.val)
+    old_aggs = [o0.aggregates(l) for l in range(o0.num_levels - 1)]
+    for l, a in enumerate(old_aggs):
+        assert np.array_equal(s.aggregates(l).cpu().numpy(), a)
+    b = inputs.rhs_uniform(A0.n, 5)
+    x0, i0 = s.solve(b, 1e-8, 500, 0)   # also instantiates the iteration graph of the old hierarchy
+    s.resetup_values(A1.val, keep_aggregates=bool(keep))
+    o1 = oracle_mod.Oracle(A1.rowptr, A1.col, A1.val, aggregates=old_aggs if keep else None)
+    try:
+        assert s.num_levels == o1.num_levels
+        for l in range(s.num_levels - 1):
+            assert np.array_equal(s.aggregates(l).cpu().numpy(), o1.aggregates(l)), f"level {l}"
+        for l in range(s.num_levels):
+            rg, cg, vg = s.level_csr(l)
+            ro, co, vo = o1.level_csr(l)
+            assert np.array_equal(rg.cpu().numpy(), ro) and np.array_equal(cg.cpu().numpy(), co)
+            assert np.max(np.abs(vg.cpu().numpy() - vo)) <= 1e-13 * np.max(np.abs(vo))
+        r = np.random.default_rng(9).standard_normal(A1.n)
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o1.vcycle(r, 0)) <= 1e-12
+        xg, ig = s.solve(b, 1e-8, 500, 0)
+        xo, io = o1.solve(b, 1e-8, 500, 0, 1)
+        assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        assert np.linalg.norm(b - A1.to_scipy() @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+        xg, _ = s.solve(b, 1e-11, 500, 0)
+        xo, _ = o1.solve(b, 1e-13, 500, 0, 1)
+        assert rel(xg.cpu().numpy(), xo) <= 1e-6
+    finally:
+        s.close()
+        o0.close()
+        o1.close()
+
+
 def test_imported_aggregates_1d_closed_form(oracle_mod, B):
     # P5(i): pairs {2I, 2I+1} of tridiag(-1,2,-1) give exactly tridiag(-1,2,-1) of half the size
     n = 4096
