@@ -126,6 +126,17 @@ def dist_env():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
 
 
+def all_max(dist, v, device):
+    """MAX over ranks of a per-rank timing (replicas only: the one collective of the bench, none on the data path)."""
+    if dist is None:
+        return v
+    import torch
+
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def make_workload(cfg, edge):
     from paper_2606_09001_b200 import inputs
 
@@ -176,11 +187,7 @@ def run_b200(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return all_max(dist, v, dev)
 
     def ev():
         return torch.cuda.Event(enable_timing=True)
