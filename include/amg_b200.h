@@ -98,6 +98,10 @@ typedef struct {
                                at setup (the same linear map); default 2304, 0 = off         */
   int32_t use_pdl;          /* 1 = the kernels of a captured iteration are chained by programmatic dependent
                                launches (a kernel becomes resident while its predecessor drains); default 1 */
+  int32_t split_prolong_rows; /* levels with at least this many rows apply the coarse correction x += gamma P e_c
+                               as its own unit-stride pass instead of fusing it into the first post-sweep
+                               (the fused sweep gathers two values per halo column); default 1500000, 0 = never */
+  int32_t reserved0;
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */
@@ -212,6 +216,8 @@ AMG_API amg_status amg_get_last_launches(amg_handle h, int64_t* launches);
  *   op 3: xout = x + gamma * P e_c                (d_in0 = x, d_in1 = e_c rows(l+1), d_out rows(l))
  *   op 4: two fused sweeps from zero: x2 of b     (d_in1 = b,           d_out rows(l))
  *   op 5: V-cycle started at level l              (d_in1 = b,           d_out rows(l))
+ *   op 6: xout = x~ + dinv o (b - A_l x~), x~ = x + gamma * P e_c
+ *                                                 (d_in0 = x, d_in1 = [b rows(l) | e_c rows(l+1)], d_out rows(l))
  * `reps` > 1 repeats the kernel back to back (timing); results are those of one application. */
 AMG_API amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0,
                         const double* d_in1, double* d_out, int32_t reps, void* cuda_stream);

@@ -34,6 +34,12 @@ constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA (
 #ifndef RT_GATHER_UNROLL
 #define RT_GATHER_UNROLL 4
 #endif
+#ifndef RT_GGROUPS
+#define RT_GGROUPS 2   // groups of gather warps working on alternate tiles
+#endif
+#ifndef RT_GATHER_ROWS
+#define RT_GATHER_ROWS 2
+#endif
 constexpr int RT_GATHERERS = RT_GATHERERS_CFG;      // warps x 32 that fetch the halo values one tile ahead
 constexpr int RT_THREADS = RT_CONSUMERS + 32 + RT_GATHERERS;  // + one producer warp (issues the bulk copies)
 constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA

@@ -344,6 +344,7 @@ static_assert(RT_STAGES >= 2 && (4 * RT_STAGES + 2 * RT_XSLOTS) * 8 <= HEADER_BY
 static_assert(RT_STAGE_BYTES % 128 == 0 && RT_XSLOT_BYTES % 128 == 0, "stage / slot sizes must keep 128-byte alignment");
 static_assert(SMEM_BYTES <= 227 * 1024, "tile ring exceeds shared memory");
 static_assert((NCW & (NCW - 1)) == 0, "consumer warps must be a power of two");
+static_assert(NGW % RT_GGROUPS == 0 && RT_XSLOTS >= 2 * RT_GGROUPS, "gather groups");
 }  // namespace rt
 
 struct StageDesc {  // TP_DESC_BYTES at the start of a stage, written by the producer
@@ -459,7 +460,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
       mbar_init(pre + s, 1);
     }
     for (int q = 0; q < RT_XSLOTS; ++q) {
-      mbar_init(xready + q, rt::NGW);
+      mbar_init(xready + q, rt::NGW / RT_GGROUPS);
       mbar_init(xempty + q, rt::NCW);
     }
     fence_mbar_init();
@@ -471,18 +472,26 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     for (int it = 0; it < npre; ++it)
       tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, pre + it, pol, 1);
   // gather warps: descriptors of their first two tiles and the halo indices of the first (setup data too)
-  constexpr int GU = RT_GATHER_UNROLL, GS = RT_GATHERERS;
-  const int g = tid - (RT_CONSUMERS + 32);
+  // The gather warps form RT_GGROUPS groups that take the tiles in turn: a group assembles a slot in
+  // one memory round trip (HBM latency when the coarse vector is cold), and the groups overlap theirs.
+  constexpr int NG = RT_GGROUPS, GU = RT_GATHER_UNROLL, GS = RT_GATHERERS / NG;
+  const int g = (tid - (RT_CONSUMERS + 32)) % GS;  // lane of the group
+  const int gg = (tid - (RT_CONSUMERS + 32)) / GS; // group
+  constexpr int LU = RT_GATHER_ROWS;  // own rows per gather thread held in registers (more rows: fallback loop)
   GTile gc, gn;
-  int idx[GU], cag[GU];
-  gc.load(a, t_begin, my, 0);
-  gn.load(a, t_begin, my, 1);
-  if (g >= 0) {
+  int idx[GU], cag[GU], la[LU];  // halo columns, their coarse indices, coarse indices of the tile's own rows
+  gc.load(a, t_begin, my, tid >= RT_CONSUMERS + 32 ? gg : my);
+  gn.load(a, t_begin, my, tid >= RT_CONSUMERS + 32 ? gg + NG : my);
+  if (tid >= RT_CONSUMERS + 32) {
 #pragma unroll
     for (int u = 0; u < GU; ++u) {
       const int h = g + u * GS;
       idx[u] = h < gc.nhalo ? __ldg(a.halo_idx + gc.hoff + h) : -1;
       if (OP == OP_JACOBI_PROLONG) cag[u] = h < gc.nhalo ? __ldg(a.halo_cagg + gc.hoff + h) : 0;
+    }
+    if (OP == OP_JACOBI_PROLONG) {
+#pragma unroll
+      for (int u = 0; u < LU; ++u) la[u] = (g + u * GS < gc.nr) ? __ldg(a.agg + gc.r0 + g + u * GS) : 0;
     }
   }
   pdl_wait();
@@ -499,22 +508,24 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     // ---------------- gather warps: x slots, up to RT_XSLOTS tiles ahead ----------------
     // software pipeline: while tile `it` is gathered, the halo indices of tile it+1 and the
     // descriptor of tile it+2 are already on their way
-    for (int it = 0; it < my; ++it) {
+    for (int it = gg; it < my; it += NG) {
       const int q = it % RT_XSLOTS;
       GTile gnn;
-      gnn.load(a, t_begin, my, it + 2);
-      int idxn[GU], cagn[GU];
+      gnn.load(a, t_begin, my, it + 2 * NG);
+      int idxn[GU], cagn[GU], lan[LU];
 #pragma unroll
       for (int u = 0; u < GU; ++u) {
         const int h = g + u * GS;
         idxn[u] = h < gn.nhalo ? __ldg(a.halo_idx + gn.hoff + h) : -1;
         if (OP == OP_JACOBI_PROLONG) cagn[u] = h < gn.nhalo ? __ldg(a.halo_cagg + gn.hoff + h) : 0;
       }
+      if (OP == OP_JACOBI_PROLONG) {
+#pragma unroll
+        for (int u = 0; u < LU; ++u) lan[u] = (g + u * GS < gn.nr) ? __ldg(a.agg + gn.r0 + g + u * GS) : 0;
+      }
       // every load of the tile is issued before anything is consumed: the slot is assembled in two
       // memory round trips (one for the plain operations) however many rows and halo columns it has
-      constexpr int LU = (RT_XSLOT_BYTES / 8 + GS - 1) / GS;  // rows per gather thread, at most
       double v[GU], e[GU], lv[LU], le[LU];
-      int la[LU];
 #pragma unroll
       for (int u = 0; u < GU; ++u) {
         const int c = idx[u];
@@ -534,12 +545,12 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
 #pragma unroll
       for (int u = 0; u < LU; ++u) {
         const int lr = g + u * GS;
-        lv[u] = 0.0, le[u] = 0.0, la[u] = 0;
+        lv[u] = 0.0, le[u] = 0.0;
         if (lr < gc.nr) {
           const int i = gc.r0 + lr;
           if (OP == OP_JACOBI_PROLONG) {
             lv[u] = __ldg(a.x + i);
-            la[u] = __ldg(a.agg + i);
+            le[u] = __ldg(a.ec + la[u]);
           } else if (OP == OP_JACOBI0) {
             lv[u] = __ldg(a.dinv + i);
             le[u] = __ldg(a.b + i);
@@ -547,11 +558,6 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
             lv[u] = __ldg(a.x + i);
           }
         }
-      }
-      if (OP == OP_JACOBI_PROLONG) {
-#pragma unroll
-        for (int u = 0; u < LU; ++u)
-          if (g + u * GS < gc.nr) le[u] = __ldg(a.ec + la[u]);
       }
       if (it >= RT_XSLOTS) mbar_wait(xempty + q, (uint32_t)(((it / RT_XSLOTS) - 1) & 1));
       double* xc = reinterpret_cast<double*>(xslot0 + q * RT_XSLOT_BYTES);  // xc[col]: rows, then halo
@@ -578,6 +584,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
             xc[lr] = lv[u];
         }
       }
+      for (int lr = g + LU * GS; lr < gc.nr; lr += GS) xc[lr] = xvalue_local<OP>(a, gc.r0 + lr);  // more rows than registers
       for (int h = g + GU * GS; h < gc.nhalo; h += GS) {  // more halo columns than the index registers hold
         const int c = __ldg(a.halo_idx + gc.hoff + h);
         if (OP == OP_JACOBI_PROLONG)
@@ -592,6 +599,10 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
       gc = gn, gn = gnn;
 #pragma unroll
       for (int u = 0; u < GU; ++u) idx[u] = idxn[u], cag[u] = cagn[u];
+      if (OP == OP_JACOBI_PROLONG) {
+#pragma unroll
+        for (int u = 0; u < LU; ++u) la[u] = lan[u];
+      }
     }
   } else if (tid >= RT_CONSUMERS) {
     // ---------------- producer warp ----------------
@@ -725,7 +736,7 @@ __global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const d
 
 // S4 standalone: x_i += gamma * ec[agg_i]
 __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* __restrict__ ec, double gamma,
-                              const double* __restrict__ xin, double* __restrict__ xout, const KrylovCtl* ctl) {
+                              const double* xin, double* xout /* may be xin */, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;

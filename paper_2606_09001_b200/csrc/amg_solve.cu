@@ -404,7 +404,15 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
   AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st));
   const bool want_dot = fuse_rz && l == 0;
   if (nu2 >= 1) {
-    op_jacobi_prolong(H, L, b, cur, ec, oth, want_dot && nu2 == 1, ctl, st);
+    if (L.fast && L.n >= H->opt.split_prolong_rows && H->opt.split_prolong_rows > 0) {
+      // Two scattered loads per halo column make the fused sweep L1-bound on the largest levels
+      // (level 0 of cfg 3: 53 us against 33 us for a plain sweep); there a separate unit-stride
+      // correction pass (8 us) followed by the plain sweep is cheaper.
+      ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, cur, ctl);
+      op_jacobi(H, L, b, cur, oth, want_dot && nu2 == 1, ctl, st);
+    } else {
+      op_jacobi_prolong(H, L, b, cur, ec, oth, want_dot && nu2 == 1, ctl, st);
+    }
     std::swap(cur, oth);
     for (int s = 1; s < nu2; ++s) {
       op_jacobi(H, L, b, cur, oth, want_dot && s == nu2 - 1, ctl, st);
@@ -601,7 +609,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
   if (reps < 1) reps = 1;
   const int64_t launches0 = g_nlaunch;
   double *t0 = H->io_tmp, *t1 = H->io_tmp2, *t2 = H->io_tmp3;
-  const bool needs_coarse = (op >= 1 && op <= 4);
+  const bool needs_coarse = (op >= 1 && op <= 4) || op == 6;
   if (needs_coarse && level >= Lc) {
     H->err = "level op needs a level below the coarsest";
     return AMG_ERR_INVALID_ARG;
@@ -655,6 +663,15 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       double* z = nullptr;
       for (int r = 0; r < reps; ++r) AMG_TRY(amg_vcycle(H, level, t1, &z, nullptr, false, st));
       perm_out(L, z, d_out);
+    } break;
+    case 6: {  // prolongation-fused sweep: d_in1 = [b (rows of this level) | e_c (rows of the next)]
+      if (!d_in0 || !d_in1) return AMG_ERR_INVALID_ARG;
+      Level& C = H->lv[level + 1];
+      perm_in(L, d_in0, t0);
+      perm_in(L, d_in1, t1);
+      perm_in(C, d_in1 + L.n, C.x2);
+      for (int r = 0; r < reps; ++r) op_jacobi_prolong(H, L, t1, t0, C.x2, t2, false, nullptr, st);
+      perm_out(L, t2, d_out);
     } break;
     default:
       H->err = "unknown level op";

@@ -120,6 +120,9 @@ def test_level_kernels(cases, name, generic):
         y = c.s.level_op(l, 5, None, b, n).cpu().numpy()
         z = c.o.vcycle(b, l)
         assert rel(y, z) <= 1e-12
+        # prolongation fused into the first post-sweep: smooth(b, x + gamma P e_c), gamma = 1
+        y = c.s.level_op(l, 6, x, np.concatenate([b, ec]), n).cpu().numpy()
+        assert np.max(np.abs(y - c.o.smooth(l, b, x + ec[agg]))) <= 1e-13 * 4
 
 
 # tail_max_rows: the levels at or below this size run inside the persistent coarse-tail kernel
@@ -325,6 +328,8 @@ def test_options(oracle_mod, B, opts):
     dict(tail_max_rows=65536, tail_dense_rows=4000),   # ... and near its top
     dict(tail_max_rows=0, tail_dense_rows=0),          # no tail at all
     dict(use_pdl=0), dict(use_graph=0, use_pdl=0),
+    dict(split_prolong_rows=1),                         # coarse correction as its own pass on every level
+    dict(split_prolong_rows=0),
 ])
 def test_launch_structure_options(cases, gpu_opts):
     """Options that change how the cycle is launched, never what it computes: same V-cycle operator
