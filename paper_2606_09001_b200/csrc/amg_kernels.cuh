@@ -1027,3 +1027,62 @@ __global__ void __launch_bounds__(256) k_grad_values(int n, const int* __restric
     gA[k] = accumulate ? gA[k] - s : -s;
   }
 }
+
+// Batched G2 (nrhs > 1).  With the right-hand sides stored one after the other, the gather
+// x_s[col[k]] touches a different 32-byte sector for every s: 16 sectors per stored entry on the
+// permuted systems (cfg 5: 14 ms, 170 GB/s).  X is therefore first interleaved to XT[j][s] (one
+// coalesced pass), so that all nrhs values of a column are ONE contiguous gather; lambda_s[i] is
+// unit-stride along the rows as it stands.
+constexpr int GT_ROWS = 64;  // rows per CTA of the interleave kernel
+__global__ void __launch_bounds__(256) k_interleave_rhs(int n, int nrhs, int64_t ld, const double* __restrict__ X,
+                                                        double* __restrict__ XT) {
+  extern __shared__ double tile[];  // [nrhs][GT_ROWS + 1]
+  const int i0 = blockIdx.x * GT_ROWS;
+  for (int t = threadIdx.x; t < nrhs * GT_ROWS; t += blockDim.x) {
+    const int s = t / GT_ROWS, r = t % GT_ROWS;
+    if (i0 + r < n) tile[s * (GT_ROWS + 1) + r] = X[(size_t)s * ld + i0 + r];
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < nrhs * GT_ROWS; t += blockDim.x) {
+    const int r = t / nrhs, s = t % nrhs;
+    if (i0 + r < n) XT[(size_t)(i0 + r) * nrhs + s] = tile[s * (GT_ROWS + 1) + r];
+  }
+}
+
+template <int LPR, int NR>  // NR > 0: nrhs known at compile time (registers for lambda); 0: generic
+__global__ void __launch_bounds__(256) k_grad_values_batched(int n, const int* __restrict__ rowptr,
+                                                             const int* __restrict__ col,
+                                                             const double* __restrict__ lam, int64_t ld,
+                                                             const double* __restrict__ XT, int nrhs_rt,
+                                                             double* __restrict__ gA, int accumulate) {
+  const int64_t gt = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t i = gt / LPR;
+  const int sub = (int)(gt % LPR);
+  if (i >= n) return;
+  const int nrhs = NR > 0 ? NR : nrhs_rt;
+  double l[NR > 0 ? NR : 1];
+  if (NR > 0) {
+#pragma unroll
+    for (int s = 0; s < NR; ++s) l[s] = __ldg(lam + (size_t)s * ld + i);
+  }
+  for (int k = rowptr[i] + sub, e = rowptr[i + 1]; k < e; k += LPR) {
+    const double* xj = XT + (size_t)col[k] * nrhs;
+    double acc = 0.0;
+    if (NR > 0 && (NR % 2) == 0) {
+      const double2* x2 = reinterpret_cast<const double2*>(xj);  // rows of XT are 16-byte aligned for even nrhs
+#pragma unroll
+      for (int s = 0; s < NR / 2; ++s) {
+        const double2 v = __ldg(x2 + s);
+        acc += l[2 * s] * v.x;
+        acc += l[2 * s + 1] * v.y;
+      }
+    } else if (NR > 0) {
+#pragma unroll
+      for (int s = 0; s < NR; ++s) acc += l[s] * __ldg(xj + s);
+    } else {
+      for (int s = 0; s < nrhs; ++s) acc += __ldg(lam + (size_t)s * ld + i) * __ldg(xj + s);
+    }
+    gA[k] = accumulate ? gA[k] - acc : -acc;
+  }
+}
+

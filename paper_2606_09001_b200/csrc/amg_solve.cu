@@ -690,6 +690,43 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
                                 double* d_gA, int accumulate, cudaStream_t st) {
   const int n = (int)H->n;
   const double mean = n > 0 ? (double)H->nnz / n : 1.0;
+  if (nrhs > 1) {
+    // interleave X once, then one contiguous gather of nrhs values per stored entry
+    double* XT = (double*)amg_dev_alloc(H, sizeof(double) * (size_t)n * nrhs, st);
+    if (!XT) {
+      H->err = "device allocation failed: interleaved right-hand sides";
+      return AMG_ERR_OOM;
+    }
+    const size_t sm = sizeof(double) * (size_t)nrhs * (GT_ROWS + 1);
+    if (sm > 48 * 1024) {
+      amg_dev_free(H, XT);
+      H->err = "amg_grad_values: nrhs too large (at most 94 right-hand sides per call; accumulate over calls)";
+      return AMG_ERR_UNSUPPORTED;
+    }
+    ++g_nlaunch, launch(k_interleave_rhs, div_up(n, GT_ROWS), 256, sm, st)(n, nrhs, ld, d_x, XT);
+    const int g8 = div_up((int64_t)n * 8, 256), g32 = div_up((int64_t)n * 32, 256);
+    const bool wide = mean > 12.0;
+#define AMG_GRAD_CASE(NR)                                                                                          \
+  if (wide)                                                                                                       \
+    ++g_nlaunch, launch(k_grad_values_batched<32, NR>, g32, 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, ld, \
+                                                                        XT, nrhs, d_gA, accumulate);                \
+  else                                                                                                            \
+    ++g_nlaunch, launch(k_grad_values_batched<8, NR>, g8, 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, ld,   \
+                                                                      XT, nrhs, d_gA, accumulate);
+    switch (nrhs) {
+      case 2: AMG_GRAD_CASE(2) break;
+      case 4: AMG_GRAD_CASE(4) break;
+      case 8: AMG_GRAD_CASE(8) break;
+      case 16: AMG_GRAD_CASE(16) break;
+      default: AMG_GRAD_CASE(0) break;
+    }
+#undef AMG_GRAD_CASE
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, XT);
+    H->last_launches = 2;
+    return AMG_OK;
+  }
   if (mean <= 12.0) {
     const int64_t threads = (int64_t)n * 8;
     ++g_nlaunch, launch(k_grad_values<8>, div_up(threads, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,

@@ -289,6 +289,28 @@ def test_adjoint_gradients(cases, name):
     assert rel(acc.cpu().numpy(), gO2) <= 1e-14
 
 
+@pytest.mark.parametrize("nrhs", [2, 4, 5, 8, 16])
+@pytest.mark.parametrize("name", ["cfg3_40", "cfg4_28"])
+def test_grad_values_batched_kernel(cases, B, name, nrhs):
+    """G2 with several right-hand sides (interleaved-X kernel, compile-time and generic nrhs), a leading
+    dimension larger than n, and accumulation: gA[k] = -sum_s lambda_s[i] x_s[col[k]] (Eq. 2 on the pattern)."""
+    c = cases(name)
+    n, ld = c.A.n, c.A.n + 37
+    rng = np.random.default_rng(300 + nrhs)
+    lam = np.zeros((nrhs, ld))
+    x = np.zeros((nrhs, ld))
+    lam[:, :n] = rng.standard_normal((nrhs, n))
+    x[:, :n] = rng.standard_normal((nrhs, n))
+    want = c.o.grad_values(np.ascontiguousarray(lam[:, :n]), np.ascontiguousarray(x[:, :n]))
+    d_lam, d_x = torch.as_tensor(lam).cuda().contiguous(), torch.as_tensor(x).cuda().contiguous()
+    gA = torch.empty(c.A.nnz, dtype=torch.float64, device="cuda")
+    B.amg_grad_values(c.s.h, d_lam, d_x, nrhs, ld, gA, 0)
+    scale = np.max(np.abs(want))
+    assert np.max(np.abs(gA.cpu().numpy() - want)) <= 1e-14 * scale * nrhs
+    B.amg_grad_values(c.s.h, d_lam, d_x, nrhs, ld, gA, 1)  # accumulate: twice the gradient
+    assert np.max(np.abs(gA.cpu().numpy() - 2 * want)) <= 1e-14 * scale * nrhs * 2
+
+
 # ------------------------------------------------------------------------------------------
 # options, imported aggregates, edge cases
 # ------------------------------------------------------------------------------------------
