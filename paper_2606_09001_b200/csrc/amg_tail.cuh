@@ -4,7 +4,9 @@
 // chain of dependent memory round trips, not a bandwidth problem.  Three measures:
 //
 //  * the CTAs stay resident (one per SM) and the dependency between two passes is a grid-wide
-//    barrier (one atomic arrival per CTA, one polled release flag) instead of a kernel boundary;
+//    barrier (one atomic arrival per CTA, one polled release flag) instead of a kernel boundary
+//    (measured: such a phase costs MORE than a row-tile launch in the PDL-chained graph, so by
+//    default only the third measure is active: tail_max_rows = tail_dense_rows);
 //  * every CTA owns a FIXED contiguous chunk of each level's rows (cut on aggregate starts,
 //    balanced by nonzeros) and copies its slice of that level's operator (rowptr / col / val /
 //    dinv) into shared memory once, at kernel start, with bulk-async copies (TMA): the four passes
@@ -58,7 +60,7 @@ struct TailArgs {
   const int* piv;
   int dense_level;         // -1: none; else levels >= dense_level are applied as dense_B
   const double* dense_B;   // [nD x nD] row-major
-  unsigned long long* bar;  // [gridDim.x] generation flags of the grid barrier
+  unsigned long long* bar;  // [0] arrival counter, [16] release word, [32 + cta] generation flags (variant 0)
   double* partials;
   KrylovCtl* ctl;           // may be null (hooks)
   int fin;                  // FIN_RZ: b_first . result is reduced and finalised (first == 0 only)
@@ -87,20 +89,20 @@ __device__ __forceinline__ void st_release_u64(unsigned long long* p, unsigned l
   asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// Grid barrier without atomics.  All CTAs of the grid are co-resident (grid <= number of SMs, one
-// CTA each).  CTA c publishes its generation in flags[c]; warp 0 of every CTA polls all flags with
-// coalesced loads until every one has reached the generation.  One store and one load round trip,
-// no serialised same-address atomics (148 atomic arrivals + 147 pollers on one line cost 3-5 us per
-// barrier, measured).  Generations only grow; every launch performs whole barriers, so a CTA picks
-// up its generation from its own flag at kernel start.
 __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
   unsigned long long v;
   asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
 }
+// Grid barrier.  All CTAs of the grid are co-resident (grid <= number of SMs, one CTA each).
+// Three variants were measured on B200 (cfg 3, 21 barriers per V-cycle at the time):
+//   1 (default) one arrival counter + one polled release word, thread 0 of every CTA:   136 us per tail
+//   2           the same with the lightest fences that still form a release / acquire pair: 135 us
+//   0           per-CTA generation flags, warp 0 of every CTA polls all of them (no atomics): 172 us
+// A barrier costs 3-5 us whichever way: 1.5-4 us of it is the arrival skew between the CTAs.
 // SASS on sm_100a: st.release.gpu = MEMBAR.ALL.GPU + STG.STRONG; ld.relaxed.gpu = LDG.STRONG alone;
-// fence.acq_rel.gpu = MEMBAR.ALL.GPU + CCTL.IVALL.  __threadfence() would be MEMBAR.SC.GPU and
-// ld.acquire.gpu a CCTL.IVALL (L1 invalidation) per poll: neither belongs in the polling loop.
+// fence.acq_rel.gpu = MEMBAR.ALL.GPU + CCTL.IVALL; __threadfence() = MEMBAR.SC.GPU + CCTL.IVALL;
+// ld.acquire.gpu = LDG.STRONG + CCTL.IVALL (an L1 invalidation per poll).
 #ifndef TAIL_BAR_VARIANT
 #define TAIL_BAR_VARIANT 1
 #endif
