@@ -565,7 +565,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
 
   // The host runs at most LAG iterations ahead of the device's convergence flag; iterations
   // enqueued after convergence return at their first instruction.
-  constexpr int NSLOT = 4, LAG = 2;
+  constexpr int NSLOT = 4, LAG = 1;
   for (int it = 0; it < maxit; ++it) {
     if (gexec) {
       AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
