@@ -23,14 +23,17 @@
  * POINTERS.  Arguments prefixed d_ are DEVICE pointers, h_ are HOST pointers; `opt`, `info`,
  * `out` scalars are host pointers.  The caller owns every buffer it passes; the library never
  * frees or reallocates them and copies what it needs during amg_setup (the CSR arrays may be
- * released after amg_setup returns).  Library-owned memory (hierarchy, work vectors) comes
- * from cudaMalloc, or from the allocator hook if one is installed, and is released by
- * amg_destroy.
+ * released after amg_setup returns).  Library-owned memory (hierarchy, work vectors, setup
+ * temporaries) comes from the device's default stream-ordered memory pool (cudaMallocAsync,
+ * release threshold raised so that repeated setups reuse it), or from the allocator hook if
+ * one is installed, and is released by amg_destroy.
  *
  * STREAMS.  Every call enqueues its work on `cuda_stream` (a cudaStream_t passed as void*;
  * NULL = the legacy default stream) and returns after that work has completed (one
  * synchronisation at the end of a solve; none inside the Krylov loop, whose scalars and
- * convergence test live on the device).
+ * convergence test live on the device: the host only waits on the event of the previous
+ * iteration before it enqueues the next-but-one).  The iteration is replayed as a CUDA graph
+ * captured on an internal stream and launched into `cuda_stream`.
  *
  * ERRORS.  Every function returns amg_status; no exception crosses the ABI.  On a failed
  * amg_setup *out is NULL and amg_last_error(NULL) holds a message (thread-local).
