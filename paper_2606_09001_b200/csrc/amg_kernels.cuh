@@ -311,7 +311,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 
 // ------------------------------------------------------------------------------------------
 // Row-tile streaming kernel (S1-S4) over the sorted-ELL tile blobs (amg_tilepack.cuh).
-// Persistent and warp-specialised: RT_CTAS CTAs per SM, each owning a contiguous run of tiles;
+// Persistent and warp-specialised: RT_CTAS CTAs per SM, tiles dealt round-robin to the CTAs;
 // per CTA 8 consumer warps + 1 producer warp + 6 gather warps, a ring of RT_STAGES operator
 // stages and a side ring of RT_XSLOTS x slots.
 //
@@ -423,12 +423,16 @@ __device__ __forceinline__ double xvalue_local(const RowArgs& a, int i) {
   return __ldg(a.x + i);
 }
 
+// Tiles are dealt to the CTAs round-robin (tile = blockIdx.x + it * gridDim.x): at any moment the grid works
+// on one window of consecutive tiles, so halo columns are in L2 and HBM is read as a few sequential streams
+// (measured 1 % faster than one contiguous run of tiles per CTA).
+#define RT_TILE(t0, it) ((t0) + (it) * (int)gridDim.x)
 struct GTile {  // what the gather warps need of a tile descriptor
   int r0, nr, nhalo, hoff;
   __device__ __forceinline__ void load(const RowArgs& a, int t_begin, int my, int it) {
     r0 = nr = nhalo = hoff = 0;
     if (it < my) {
-      const TileDesc* d = a.tiles + t_begin + it;
+      const TileDesc* d = a.tiles + RT_TILE(t_begin, it);
       r0 = __ldg(&d->r0), nr = __ldg(&d->nr), nhalo = __ldg(&d->nhalo), hoff = __ldg(&d->halo_off);
     }
   }
@@ -446,9 +450,8 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   unsigned char* stage0 = smem + rt::HEADER_BYTES;
   unsigned char* xslot0 = stage0 + RT_STAGES * RT_STAGE_BYTES;
   const int tid = threadIdx.x;
-  const int t_begin = (int)((int64_t)blockIdx.x * a.ntiles / gridDim.x);
-  const int t_end = (int)((int64_t)(blockIdx.x + 1) * a.ntiles / gridDim.x);
-  const int my = t_end - t_begin;
+  const int t_begin = blockIdx.x;
+  const int my = ((int)a.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;  // this CTA's tiles
   const int npre = my < RT_STAGES ? my : RT_STAGES;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
   // ---- before the grid dependency: nothing here reads what an earlier kernel of the solve wrote ----
@@ -470,7 +473,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
   if (tid == RT_CONSUMERS)
     for (int it = 0; it < npre; ++it)
-      tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, pre + it, pol, 1);
+      tile_issue<OP, NDOT, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + it * RT_STAGE_BYTES, pre + it, pol, 1);
   // gather warps: descriptors of their first two tiles and the halo indices of the first (setup data too)
   // The gather warps form RT_GGROUPS groups that take the tiles in turn: a group assembles a slot in
   // one memory round trip (HBM latency when the coarse vector is cold), and the groups overlap theirs.
@@ -608,10 +611,10 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
     // ---------------- producer warp ----------------
     if (tid == RT_CONSUMERS && my > 0) {
       for (int it = 0; it < npre; ++it)  // their blobs are already on the way
-        tile_issue<OP, NDOT, STREAM>(a, a.tiles[t_begin + it], stage0 + it * RT_STAGE_BYTES, full + it, pol, 2);
+        tile_issue<OP, NDOT, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + it * RT_STAGE_BYTES, full + it, pol, 2);
       for (int it = npre; it < my; ++it) {
         const int s = it % RT_STAGES;
-        const TileDesc d = a.tiles[t_begin + it];
+        const TileDesc d = a.tiles[RT_TILE(t_begin, it)];
         mbar_wait(empty + s, (uint32_t)(((it / RT_STAGES) - 1) & 1));
         tile_issue<OP, NDOT, STREAM>(a, d, stage0 + s * RT_STAGE_BYTES, full + s, pol, 0);
       }
