@@ -742,8 +742,19 @@ __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* 
                               const double* xin, double* xout /* may be xin */, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) xout[i] = xin[i] + gamma * ec[agg[i]];
+  // two rows per thread and trip: 128-bit accesses of x, 64-bit of agg (all arrays are 16-byte aligned)
+  const int n2 = n >> 1;
+  const int2* agg2 = reinterpret_cast<const int2*>(agg);
+  const double2* xi2 = reinterpret_cast<const double2*>(xin);
+  double2* xo2 = reinterpret_cast<double2*>(xout);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += gridDim.x * blockDim.x) {
+    const int2 a = agg2[i];
+    double2 v = xi2[i];
+    v.x += gamma * ec[a.x];
+    v.y += gamma * ec[a.y];
+    xo2[i] = v;
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) xout[n - 1] = xin[n - 1] + gamma * ec[agg[n - 1]];
 }
 
 __global__ void k_scale_dinv(int n, const double* __restrict__ dinv, const double* __restrict__ b,
@@ -877,8 +888,17 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __re
   pdl_sync();
   if (ctl->done) return;
   const double beta = ctl->beta;
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
-    p[i] = z[i] + beta * p[i];
+  const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* z2 = reinterpret_cast<const double2*>(z);
+  double2* p2 = reinterpret_cast<double2*>(p);
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n2; i += stride) {
+    const double2 a = z2[i];
+    double2 b = p2[i];
+    b.x = a.x + beta * b.x;
+    b.y = a.y + beta * b.y;
+    p2[i] = b;
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) p[n - 1] = z[n - 1] + beta * p[n - 1];
 }
 
 // x += alpha p ; r -= alpha q ; ||r||^2

@@ -408,7 +408,7 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       // Two scattered loads per halo column make the fused sweep L1-bound on the largest levels
       // (level 0 of cfg 3: 53 us against 33 us for a plain sweep); there a separate unit-stride
       // correction pass (8 us) followed by the plain sweep is cheaper.
-      ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, cur, ctl);
+      ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, cur, ctl);
       op_jacobi(H, L, b, cur, oth, want_dot && nu2 == 1, ctl, st);
     } else {
       op_jacobi_prolong(H, L, b, cur, ec, oth, want_dot && nu2 == 1, ctl, st);
@@ -419,7 +419,7 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       std::swap(cur, oth);
     }
   } else {
-    ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
+    ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
     std::swap(cur, oth);
     if (want_dot) ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
   }
@@ -648,7 +648,7 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       perm_in(L, d_in0, t0);
       perm_in(C, d_in1, t1);
       for (int r = 0; r < reps; ++r)
-        ++g_nlaunch, launch(k_prolong_add, grid_for(L.n), TPB, 0, st)(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
+        ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, t1, H->opt.coarse_scale, t0, t2, nullptr);
       perm_out(L, t2, d_out);
     } break;
     case 4:
