@@ -103,7 +103,7 @@ typedef struct {
                                launches (a kernel becomes resident while its predecessor drains); default 1 */
   int32_t split_prolong_rows; /* levels with at least this many rows apply the coarse correction x += gamma P e_c
                                as its own unit-stride pass instead of fusing it into the first post-sweep
-                               (the fused sweep gathers two values per halo column); default 1500000, 0 = never */
+                               (the fused sweep gathers two values per halo column); default 800000, 0 = never */
   int32_t reserved0;
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */

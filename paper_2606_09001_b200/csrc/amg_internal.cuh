@@ -151,8 +151,9 @@ struct amg_handle_s {
   int tail_lu_smem = 0;              // dynamic shared memory: LU scratch, then the staged operator chunks
   int tail_smem = 0;
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
-  cudaGraphExec_t graph_exec[4] = {nullptr, nullptr, nullptr, nullptr};
-  int64_t graph_launches[4] = {0, 0, 0, 0};  // kernel nodes per replay
+  // [krylov * 2 + precond]: one iteration; [4]: the start of an AMG-PCG solve (first V-cycle + p = z)
+  cudaGraphExec_t graph_exec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  int64_t graph_launches[5] = {0, 0, 0, 0, 0};  // kernel nodes per replay
   int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;  // graphs are captured here (the legacy stream cannot capture)

@@ -485,8 +485,18 @@ amg_status enqueue_iteration(amg_handle_s* H, int krylov, int precond, cudaStrea
   return krylov == 0 ? enqueue_pcg_iteration(H, precond, st) : enqueue_bicg_iteration(H, precond, st);
 }
 
+// the start of an AMG-PCG solve after k_krylov_init: z = B r (r.z on the last sweep), p = z
+amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
+  double* z = nullptr;
+  AMG_TRY(amg_vcycle(H, 0, H->kv[1], &z, H->ctl, true, st));
+  ++g_nlaunch, launch(k_pcg_p, red_grid(H, H->lv[0].n), RED_THREADS, 0, st)(H->lv[0].n, z, H->kv[2], H->ctl);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
+
+// krylov < 0: the start graph (slot 4)
 amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStream_t st, cudaGraphExec_t* out) {
-  const int slot = krylov * 2 + precond;
+  const int slot = krylov < 0 ? 4 : krylov * 2 + precond;
   if (H->graph_exec[slot]) {
     *out = H->graph_exec[slot];
     return AMG_OK;
@@ -497,7 +507,7 @@ amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStr
   AMG_CUDA_TRY(H, cudaStreamBeginCapture(H->cap_stream, cudaStreamCaptureModeThreadLocal));
   const int64_t launches0 = g_nlaunch;
   g_pdl = H->opt.use_pdl != 0;
-  amg_status s = enqueue_iteration(H, krylov, precond, H->cap_stream);
+  amg_status s = krylov < 0 ? enqueue_pcg_start(H, H->cap_stream) : enqueue_iteration(H, krylov, precond, H->cap_stream);
   g_pdl = false;
   H->graph_launches[slot] = g_nlaunch - launches0;  // kernel nodes of one replay
   g_nlaunch = launches0;                            // capturing enqueues nothing
@@ -547,13 +557,17 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   if (krylov == 0) {
     ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
                                                          H->counter, H->ctl, FIN_INIT_PCG);
-    double* z = r;
-    if (precond) {
-      AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
+    if (precond && H->opt.use_graph && maxit > 0) {
+      cudaGraphExec_t gstart = nullptr;
+      AMG_TRY(get_iteration_graph(H, -1, 1, st, &gstart));
+      AMG_CUDA_TRY(H, cudaGraphLaunch(gstart, st));
+      g_nlaunch += H->graph_launches[4];
+    } else if (precond) {
+      AMG_TRY(enqueue_pcg_start(H, st));
     } else {
       ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
+      ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, p, H->ctl);
     }
-    ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, z, p, H->ctl);
   } else {
     ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
                                                          H->ctl, FIN_INIT_BICG);
