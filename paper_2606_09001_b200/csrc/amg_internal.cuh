@@ -154,6 +154,7 @@ struct amg_handle_s {
   // [krylov * 2 + precond]: one iteration; [4]: the start of an AMG-PCG solve (first V-cycle + p = z)
   cudaGraphExec_t graph_exec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int64_t graph_launches[5] = {0, 0, 0, 0, 0};  // kernel nodes per replay
+  double* vcycle_final_out = nullptr;        // if set: the last post-sweep of a cycle started at level 0 writes here
   int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;  // graphs are captured here (the legacy stream cannot capture)

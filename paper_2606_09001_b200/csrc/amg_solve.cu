@@ -415,8 +415,14 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     }
     std::swap(cur, oth);
     for (int s = 1; s < nu2; ++s) {
-      op_jacobi(H, L, b, cur, oth, want_dot && s == nu2 - 1, ctl, st);
-      std::swap(cur, oth);
+      // the caller may ask for the result of a level-0 cycle in a buffer of its own (BiCGSTAB keeps phat
+      // across the second V-cycle of an iteration: no copy)
+      double* out = (l == 0 && s == nu2 - 1 && H->vcycle_final_out) ? H->vcycle_final_out : oth;
+      op_jacobi(H, L, b, cur, out, want_dot && s == nu2 - 1, ctl, st);
+      if (out == oth)
+        std::swap(cur, oth);
+      else
+        cur = out;
     }
   } else {
     ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
@@ -465,9 +471,12 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   double* phat = p;
   if (precond) {
     double* zz = nullptr;
-    AMG_TRY(amg_vcycle(H, 0, p, &zz, H->ctl, false, st));
+    H->vcycle_final_out = ph;
+    const amg_status sv = amg_vcycle(H, 0, p, &zz, H->ctl, false, st);
+    H->vcycle_final_out = nullptr;
+    AMG_TRY(sv);
     // the second V-cycle of this iteration overwrites the level-0 buffers: keep phat
-    ++g_nlaunch, launch(k_copy, red_grid(H, n), RED_THREADS, 0, st)(n, zz, ph, H->ctl);
+    if (zz != ph) ++g_nlaunch, launch(k_copy, red_grid(H, n), RED_THREADS, 0, st)(n, zz, ph, H->ctl);
     phat = ph;
   }
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
