@@ -210,7 +210,7 @@ amg_status amg_exclusive_scan(amg_handle_s* H, const int* d_in, int* d_out, int 
 
 // solve.cu
 amg_status amg_vcycle(amg_handle_s* H, int level, const double* b, double** x_out, KrylovCtl* ctl,
-                      bool fuse_rz, cudaStream_t st);
+                      bool fuse_rz, cudaStream_t st, bool x1_ready = false);
 amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, double rtol, int maxit,
                             int krylov, int precond, amg_info* info, cudaStream_t st);
 amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d_in0,

@@ -41,6 +41,8 @@ struct RowArgs {
   const double* b;
   const double* dinv;
   double* out;
+  const double* dinv_c; // restriction, optional: smoother diagonal of the coarse level ...
+  double* out2;         // ... then out2[I] = dinv_c[I] * out[I] (the first sweep of the coarse level from zero)
   const int* agg;       // prolongation / restriction
   const int* agg_ptr;
   const unsigned char* blob;  // tile-packed operator (row-tile kernels)
@@ -351,8 +353,9 @@ struct StageDesc {  // TP_DESC_BYTES at the start of a stage, written by the pro
   int r0, nr, I0, nA;
   int nsl, nhalo, roff, aoff;    // roff = r0 - ra2 (b / dinv slices), aoff = I0 - Ia4 (agg_ptr slice)
   int o_perm, o_col, o_val, o_b;
-  int o_d, o_agg, o_out, pad0;
-  int pad1[16];
+  int o_d, o_agg, o_out, o_dc;
+  int eoff, pad0, pad2, pad3;    // eoff = Ia2 (coarse slice: dcs[I - eoff] = dinv_c[I])
+  int pad1[12];
 };
 static_assert(sizeof(StageDesc) == TP_DESC_BYTES, "stage header size");
 
@@ -372,7 +375,8 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
                                            uint64_t pol, int mode) {
   using T = TileOps<OP>;
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
-  const int flags = T::FLAGS | (d0_staged ? TP_B : 0);
+  const bool dc = T::AGGPTR && a.dinv_c != nullptr;
+  const int flags = T::FLAGS | (d0_staged ? TP_B : 0) | (dc ? TP_DC : 0);
   const BlobLayout p = tp_blob(d.nsl, d.nslots);
   const StageLayout t = tp_stage(d, flags);
   if (mode != 2) {
@@ -380,11 +384,12 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
     sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
     sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
     sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_b = t.o_b;
-    sd.o_d = t.o_d, sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.pad0 = 0;
+    sd.o_d = t.o_d, sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.o_dc = t.o_dc;
+    sd.eoff = t.Ia2, sd.pad0 = sd.pad2 = sd.pad3 = 0;
     int4* dst = reinterpret_cast<int4*>(stage);
     const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) dst[q] = src[q];
+    for (int q = 0; q < 5; ++q) dst[q] = src[q];
   }
   if (d.nr <= 0) {
     mbar_arrive(bar);
@@ -400,6 +405,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
     if (T::B || d0_staged) bytes += nrv8;
     if (T::D) bytes += nrv8;
     if (T::AGGPTR) bytes += 4u * (uint32_t)t.nap;
+    if (dc) bytes += 8u * (uint32_t)t.nec;
   }
   if (mode == 2 && !has_vec) {  // nothing but the blob is staged (SpMV without a second dot operand)
     mbar_arrive(bar);
@@ -412,6 +418,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
     if (d0_staged) bulk_g2s<false>(base + t.o_b, a.d0 + t.ra2, nrv8, bar, pol);
     if (T::D) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, nrv8, bar, pol);
     if (T::AGGPTR) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
+    if (dc) bulk_g2s<false>(base + t.o_dc, a.dinv_c + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
   }
 }
 
@@ -672,10 +679,12 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
           mbar_wait(resdone + s, par);
           const int nA = sd->nA, I0 = sd->I0;
           const int* aps = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;  // aps[al] = agg_ptr[I0 + al]
+          const double* dcs = reinterpret_cast<const double*>(base + sd->o_dc) - sd->eoff;  // dcs[I] = dinv_c[I]
           for (int al = tid; al < nA; al += RT_CONSUMERS) {
             double sum = 0.0;
             for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) sum += outs[lr];
             a.out[I0 + al] = sum;
+            if (a.out2 != nullptr) a.out2[I0 + al] = dcs[I0 + al] * sum;
           }
         }
       }

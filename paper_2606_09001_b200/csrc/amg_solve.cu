@@ -158,13 +158,17 @@ void op_jacobi_prolong(amg_handle_s* H, const Level& L, const double* b, const d
     launch_row<OP_JACOBI_PROLONG, 0>(H, L, a, st);
 }
 
+// rc = R (b - A x); with dinv_c / x1c also x1c = dinv_c o rc, the first sweep of the coarse level from zero
+// (row-tile path only)
 void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, const double* x, double* rc,
-                          KrylovCtl* ctl, cudaStream_t st) {
+                          KrylovCtl* ctl, cudaStream_t st, const double* dinv_c = nullptr, double* x1c = nullptr) {
   RowArgs a = base_args(H, L, ctl);
   a.x = x;
   a.b = b;
   if (L.fast) {
     a.out = rc;
+    a.dinv_c = x1c ? dinv_c : nullptr;
+    a.out2 = dinv_c ? x1c : nullptr;
     if (L.stream_hint)
       launch_tile<OP_RESTRICT, 0, true>(H, L, a, st);
     else
@@ -365,7 +369,7 @@ amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
 // fuse_rz: the last smoother sweep of level 0 also produces r.z (FIN_RZ).
 // ------------------------------------------------------------------------------------------
 amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, KrylovCtl* ctl, bool fuse_rz,
-                      cudaStream_t st) {
+                      cudaStream_t st, bool x1_ready) {
   const int Lc = (int)H->lv.size() - 1;
   Level& L = H->lv[l];
   if (H->tail_first >= 0 && l >= H->tail_first) {
@@ -385,7 +389,12 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
   double* cur = L.x;
   double* oth = L.x2;
   int done_sweeps = 0;
-  if (nu1 >= 2) {
+  if (nu1 >= 2 && x1_ready) {
+    // the restriction of the level above left x1 = dinv o b in L.x2: the second sweep is a plain one
+    // (one gather per halo column instead of the two of the fused pair)
+    op_jacobi(H, L, b, L.x2, cur, false, ctl, st);
+    done_sweeps = 2;
+  } else if (nu1 >= 2) {
     op_jacobi0(H, L, b, cur, ctl, st);
     done_sweeps = 2;
   } else if (nu1 == 1) {
@@ -399,9 +408,11 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
     std::swap(cur, oth);
   }
   Level& C = H->lv[l + 1];
-  op_residual_restrict(H, L, b, cur, C.b, ctl, st);
+  // the coarse level starts with two sweeps from zero on the row-tile path: hand it its first one
+  const bool give_x1 = L.fast && C.fast && nu1 >= 2 && l + 1 < Lc && !(H->tail_first >= 0 && l + 1 >= H->tail_first);
+  op_residual_restrict(H, L, b, cur, C.b, ctl, st, give_x1 ? C.dinv : nullptr, give_x1 ? C.x2 : nullptr);
   double* ec = nullptr;
-  AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st));
+  AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st, give_x1));
   const bool want_dot = fuse_rz && l == 0;
   if (nu2 >= 1) {
     if (L.fast && L.n >= H->opt.split_prolong_rows && H->opt.split_prolong_rows > 0) {

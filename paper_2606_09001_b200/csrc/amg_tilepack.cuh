@@ -61,10 +61,11 @@ constexpr int TP_DESC_BYTES = 128;
 struct StageLayout {
   int ra2, nrv;    // first staged row of the f64 row vectors (even), entries staged (even)
   int Ia4, nap;    // agg_ptr slice (nA + 1 entries from I0)
-  int o_b, o_d, o_agg, o_out, end;  // byte offsets (blob at 0)
+  int Ia2, nec;    // coarse-vector slice (nA entries from I0)
+  int o_b, o_d, o_agg, o_dc, o_out, end;  // byte offsets (blob at 0)
 };
 // flags: which operands the operation stages in the ring
-enum { TP_B = 1, TP_D = 2, TP_AGGPTR = 16, TP_OUT = 64 };
+enum { TP_B = 1, TP_D = 2, TP_DC = 8, TP_AGGPTR = 16, TP_OUT = 64 };
 __host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
   StageLayout t;
   const BlobLayout p = tp_blob(d.nsl, d.nslots);
@@ -73,6 +74,8 @@ __host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
   t.nrv = tp_up(r1 - t.ra2, 2);
   t.Ia4 = d.I0 & ~3;
   t.nap = tp_up(d.I0 + d.nA + 1 - t.Ia4, 4);
+  t.Ia2 = d.I0 & ~1;
+  t.nec = tp_up(d.I0 + d.nA - t.Ia2, 2);
   int o = p.end;
   t.o_b = o;
   if (flags & TP_B) o += 8 * t.nrv;
@@ -80,13 +83,15 @@ __host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
   if (flags & TP_D) o += 8 * t.nrv;
   t.o_agg = o;
   if (flags & TP_AGGPTR) o += 4 * t.nap;
+  t.o_dc = o;
+  if (flags & TP_DC) o += 8 * t.nec;
   t.o_out = o;
   if (flags & TP_OUT) o += 8 * tp_up(d.nr, 2);
   t.end = o;
   return t;
 }
 constexpr int TP_FLAGS_SWEEP = TP_B | TP_D;                            // Jacobi sweeps
-constexpr int TP_FLAGS_RESTRICT = TP_B | TP_AGGPTR | TP_OUT;           // residual + restriction
+constexpr int TP_FLAGS_RESTRICT = TP_B | TP_AGGPTR | TP_DC | TP_OUT;   // residual + restriction (+ x1 of the coarse level)
 // shared-memory bytes one ring stage needs for a tile, for the most demanding operations
 __host__ __device__ inline int tp_stage_need(const TileDesc& d) {
   const int a = tp_stage(d, TP_FLAGS_SWEEP).end, b = tp_stage(d, TP_FLAGS_RESTRICT).end;
