@@ -35,7 +35,7 @@ class Options(C.Structure):
                 ("coarse_max_rows", C.c_int32), ("max_levels", C.c_int32),
                 ("max_match_rounds", C.c_int32), ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double),
-                ("hash_seed", C.c_uint64)]
+                ("hash_seed", C.c_uint64), ("agg_passes", C.c_int32), ("symmetric", C.c_int32)]
 
 
 class Info(C.Structure):
@@ -179,6 +179,12 @@ class Oracle:
         _check(lib().oracle_vcycle(self._h, C.c_int32(level), _p(r), _p(z)), "vcycle")
         return z
 
+    def vcycle_transpose(self, r, level=0) -> np.ndarray:
+        r = _f64(r)
+        z = np.empty_like(r)
+        _check(lib().oracle_vcycle_transpose(self._h, C.c_int32(level), _p(r), _p(z)), "vcycle_transpose")
+        return z
+
     def solve(self, b, rtol=1e-8, maxit=1000, krylov=0, precond=1):
         b = _f64(b)
         x = np.empty_like(b)
@@ -195,6 +201,14 @@ class Oracle:
                                             C.c_int32(maxit), C.c_int32(krylov), C.c_int32(precond),
                                             C.c_int32(symmetric), C.byref(info)), "solve_transpose")
         return lam, info
+
+    def residual_history(self) -> np.ndarray:
+        """||r_k|| / ||b||, k = 1 … iterations, of the last solve / solve_transpose on this handle."""
+        m = int(lib().oracle_get_residual_history(self._h, None, C.c_int32(0)))
+        out = np.empty(max(m, 0))
+        if m > 0:
+            lib().oracle_get_residual_history(self._h, _p(out), C.c_int32(m))
+        return out
 
     def grad_values(self, lam, x, accumulate_into=None) -> np.ndarray:
         """lam, x: arrays of shape (nrhs, n) (row b = vector b) or (n,)."""
@@ -213,8 +227,9 @@ class Oracle:
         return gA
 
 
-def aggregate(rowptr, col, val, beta=0.25, salt=0, max_rounds=0, mode=0):
-    """O-2 on its own.  Returns (match, agg, nc, rounds).  mode 0 handshake, 1 greedy."""
+def aggregate(rowptr, col, val, beta=0.25, salt=0, max_rounds=0, mode=0, symmetric=1):
+    """O-2 on its own.  Returns (match, agg, nc, rounds).  mode 0 handshake, 1 greedy.
+    symmetric = 0: the matching runs on (A + A^T)/2 (A1, nonsymmetric case)."""
     rowptr, col, val = _i32(rowptr), _i32(col), _f64(val)
     n = len(rowptr) - 1
     match = np.empty(n, dtype=np.int32)
@@ -222,7 +237,7 @@ def aggregate(rowptr, col, val, beta=0.25, salt=0, max_rounds=0, mode=0):
     nc, rounds = C.c_int32(), C.c_int32()
     _check(lib().oracle_aggregate(C.c_int32(n), _p(rowptr), _p(col), _p(val), C.c_double(beta),
                                   C.c_uint64(salt), C.c_int32(max_rounds), C.c_int32(mode),
-                                  _p(match), _p(agg), C.byref(nc), C.byref(rounds)), "aggregate")
+                                  C.c_int32(symmetric), _p(match), _p(agg), C.byref(nc), C.byref(rounds)), "aggregate")
     return match, agg, nc.value, rounds.value
 
 

@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <climits>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -45,6 +46,7 @@ struct oracle_handle_s {
   std::vector<int> pivt;
   bool have_t = false;
   bool have_lu = false;  // with imported aggregates the coarsest LU is factored at first use
+  std::vector<double> hist;  // ||r_k|| / ||b|| of the last solve, k = 1 … iterations (PAPER.md:125 diagnostics)
 };
 
 namespace {
@@ -83,6 +85,30 @@ Csr transpose(const Csr& A) {
       T.val[p] = A.val[k];
     }
   return T;
+}
+
+// S = (A + A^T) / 2 on the union of the two patterns (A1, nonsymmetric case: the strength of the
+// pair {i,j} is w_ij = -(a_ij + a_ji)/2; the sum is commutative, so S is bitwise symmetric and
+// S(A) == S(A^T); a missing entry counts as 0).  For a bitwise symmetric A, S == A bitwise.
+Csr symmetrise(const Csr& A) {
+  Csr T = transpose(A);
+  Csr S;
+  S.n = A.n;
+  S.rowptr.assign(A.n + 1, 0);
+  for (int i = 0; i < A.n; ++i) {
+    int ka = A.rowptr[i], ea = A.rowptr[i + 1], kt = T.rowptr[i], et = T.rowptr[i + 1];
+    while (ka < ea || kt < et) {  // two sorted lists: ascending union
+      int ca = ka < ea ? A.col[ka] : INT32_MAX, ct = kt < et ? T.col[kt] : INT32_MAX;
+      int c = std::min(ca, ct);
+      double a = 0.0, t = 0.0;
+      if (ca == c) a = A.val[ka++];
+      if (ct == c) t = T.val[kt++];
+      S.col.push_back(c);
+      S.val.push_back((a + t) / 2);
+    }
+    S.rowptr[i + 1] = (int)S.col.size();
+  }
+  return S;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -233,8 +259,13 @@ int number_aggregates(const Csr& A, const std::vector<double>& m, double beta, u
   return nc;
 }
 
-int aggregate(const Csr& A, double beta, uint64_t salt, int max_rounds, int mode,
+// symmetric != 0: w_ij = -a_ij read from row i (A1; the generators make a_ij == a_ji bitwise);
+// symmetric == 0: the matching runs on S = (A + A^T)/2 (A1, nonsymmetric case)
+int aggregate(const Csr& A0, double beta, uint64_t salt, int max_rounds, int mode, int symmetric,
               std::vector<int>& match, std::vector<int>& agg, int* rounds) {
+  Csr S;
+  if (!symmetric) S = symmetrise(A0);
+  const Csr& A = symmetric ? A0 : S;
   std::vector<double> m = row_maxima(A);
   *rounds = mode == 0 ? match_handshake(A, m, beta, salt, max_rounds, match)
                       : match_greedy(A, m, beta, salt, match);
@@ -341,11 +372,14 @@ bool dense_lu(int n, std::vector<double>& a, std::vector<int>& piv) {
 
 void dense_lu_solve(int n, const std::vector<double>& a, const std::vector<int>& piv,
                     const double* b, double* x) {
+  // dense_lu exchanges WHOLE rows (the multipliers of the earlier columns move with them), so the
+  // factors are those of P A with P = the product of all exchanges: P is applied to b first, then
+  // L y = P b and U x = y  (O-1: "factor A_L = P L U"; pinned by test_dense_lu_row_swaps)
   for (int i = 0; i < n; ++i) x[i] = b[i];
-  for (int k = 0; k < n; ++k) {
+  for (int k = 0; k < n; ++k)
     if (piv[k] != k) std::swap(x[k], x[piv[k]]);
+  for (int k = 0; k < n; ++k)
     for (int i = k + 1; i < n; ++i) x[i] -= a[(size_t)i * n + k] * x[k];
-  }
   for (int i = n - 1; i >= 0; --i) {
     double s = x[i];
     for (int j = i + 1; j < n; ++j) s -= a[(size_t)i * n + j] * x[j];
@@ -410,8 +444,20 @@ int setup(oracle_handle_s* H, Csr A0, int nagg, const int32_t* const* aggs) {
     } else {
       if (nl <= o.coarse_max_rows || l == o.max_levels - 1) break;
       std::vector<int> match;
-      nc = aggregate(cur.A, o.strong_beta, o.hash_seed + (uint64_t)l, o.max_match_rounds, 0, match,
-                     agg, &cur.rounds);
+      nc = aggregate(cur.A, o.strong_beta, o.hash_seed + (uint64_t)l, o.max_match_rounds, 0,
+                     o.symmetric, match, agg, &cur.rounds);
+      // agg_passes > 1 (O-1): aggregate the intermediate Galerkin matrix again and compose
+      // (pass p uses the salt hash_seed + l + 1000 p; size-4 aggregates for agg_passes = 2)
+      for (int p = 1; p < o.agg_passes; ++p) {
+        Csr mid = galerkin(cur.A, agg, nc);
+        std::vector<int> match2, agg2;
+        int r2 = 0;
+        int nc2 = aggregate(mid, o.strong_beta, o.hash_seed + (uint64_t)l + 1000ull * (uint64_t)p,
+                            o.max_match_rounds, 0, o.symmetric, match2, agg2, &r2);
+        for (int i = 0; i < nl; ++i) agg[i] = agg2[agg[i]];
+        nc = nc2;
+        cur.rounds = std::max(cur.rounds, r2);
+      }
       if ((double)nc > 0.8 * (double)nl) break;  // stall => this level is the coarsest (A6)
     }
     cur.agg = agg;
@@ -495,9 +541,10 @@ void apply_precond(const oracle_handle_s* H, int precond, bool T, const double* 
 // ------------------------------------------------------------------------------------------
 // O-5  PCG (textbook, x0 = 0, recurrence residual, Euclidean norm; A10)
 // ------------------------------------------------------------------------------------------
-void pcg(const oracle_handle_s* H, const Csr& A, bool T, const double* b, double* x, double rtol,
+void pcg(oracle_handle_s* H, const Csr& A, bool T, const double* b, double* x, double rtol,
          int maxit, int precond, oracle_info* info) {
   int n = A.n;
+  H->hist.clear();
   std::vector<double> r(b, b + n), z(n), p(n), q(n);
   for (int i = 0; i < n; ++i) x[i] = 0.0;
   double nb = std::sqrt(dot(n, b, b));
@@ -524,6 +571,7 @@ void pcg(const oracle_handle_s* H, const Csr& A, bool T, const double* b, double
     double nr = std::sqrt(dot(n, r.data(), r.data()));
     info->iterations = k;
     info->rel_residual = nr / nb;
+    H->hist.push_back(nr / nb);
     if (!std::isfinite(nr)) {
       info->status = ORACLE_NONFINITE;
       break;
@@ -543,9 +591,10 @@ void pcg(const oracle_handle_s* H, const Csr& A, bool T, const double* b, double
 // ------------------------------------------------------------------------------------------
 // O-6  right-preconditioned BiCGSTAB (x0 = 0, rhat = r0 = b; A11)
 // ------------------------------------------------------------------------------------------
-void bicgstab(const oracle_handle_s* H, const Csr& A, bool T, const double* b, double* x,
+void bicgstab(oracle_handle_s* H, const Csr& A, bool T, const double* b, double* x,
               double rtol, int maxit, int precond, oracle_info* info) {
   int n = A.n;
+  H->hist.clear();
   std::vector<double> r(b, b + n), rhat(b, b + n), p(n, 0.0), v(n, 0.0), s(n), t(n), ph(n), sh(n);
   for (int i = 0; i < n; ++i) x[i] = 0.0;
   double nb = std::sqrt(dot(n, b, b));
@@ -581,6 +630,7 @@ void bicgstab(const oracle_handle_s* H, const Csr& A, bool T, const double* b, d
       for (int i = 0; i < n; ++i) x[i] += alpha * ph[i];
       info->rel_residual = ns / nb;
       info->status = ORACLE_CONVERGED;
+      H->hist.push_back(ns / nb);
       break;
     }
     apply_precond(H, precond, T, s.data(), sh.data());
@@ -592,6 +642,7 @@ void bicgstab(const oracle_handle_s* H, const Csr& A, bool T, const double* b, d
     for (int i = 0; i < n; ++i) r[i] = s[i] - omega * t[i];
     double nr = std::sqrt(dot(n, r.data(), r.data()));
     info->rel_residual = nr / nb;
+    H->hist.push_back(nr / nb);
     if (!std::isfinite(nr)) {
       info->status = ORACLE_NONFINITE;
       break;
@@ -634,6 +685,8 @@ void oracle_options_default(oracle_options* o) {
   o->strong_beta = 0.25;
   o->coarse_scale = 1.0;
   o->hash_seed = 0;
+  o->agg_passes = 1;
+  o->symmetric = 1;
 }
 
 void oracle_set_threads(int nthreads) { g_threads = nthreads > 0 ? nthreads : 1; }
@@ -717,8 +770,8 @@ int oracle_match_rounds(oracle_handle h, int32_t level) {
 }
 
 int oracle_aggregate(int32_t n, const int32_t* rowptr, const int32_t* col, const double* val,
-                     double beta, uint64_t salt, int32_t max_rounds, int32_t mode, int32_t* match,
-                     int32_t* agg, int32_t* nc, int32_t* rounds) {
+                     double beta, uint64_t salt, int32_t max_rounds, int32_t mode, int32_t symmetric,
+                     int32_t* match, int32_t* agg, int32_t* nc, int32_t* rounds) {
   if (n <= 0 || !rowptr || !col || !val || !nc) return ORACLE_ERR_INVALID_ARG;
   Csr A;
   A.n = n;
@@ -727,7 +780,7 @@ int oracle_aggregate(int32_t n, const int32_t* rowptr, const int32_t* col, const
   A.val.assign(val, val + rowptr[n]);
   std::vector<int> m, a;
   int r = 0;
-  *nc = aggregate(A, beta, salt, max_rounds, mode, m, a, &r);
+  *nc = aggregate(A, beta, salt, max_rounds, mode, symmetric, m, a, &r);
   if (match) std::copy(m.begin(), m.end(), match);
   if (agg) std::copy(a.begin(), a.end(), agg);
   if (rounds) *rounds = r;
@@ -780,6 +833,14 @@ int oracle_vcycle(oracle_handle h, int32_t level, const double* r, double* z) {
   return ORACLE_OK;
 }
 
+int oracle_vcycle_transpose(oracle_handle h, int32_t level, const double* r, double* z) {
+  if (!h || level < 0 || level >= (int)h->lv.size()) return ORACLE_ERR_INVALID_ARG;
+  if (int rc = ensure_lu(h)) return rc;
+  ensure_transposed(h);
+  vcycle(h, level, true, r, z);
+  return ORACLE_OK;
+}
+
 int oracle_solve(oracle_handle h, const double* b, double* x, double rtol, int32_t maxit,
                  int32_t krylov, int32_t precond, oracle_info* info) {
   if (!h || !b || !x || !info || maxit < 0) return ORACLE_ERR_INVALID_ARG;
@@ -805,6 +866,14 @@ int oracle_solve_transpose(oracle_handle h, const double* g, double* lambda, dou
   else
     bicgstab(h, h->lv[0].At, true, g, lambda, rtol, maxit, precond, info);
   return ORACLE_OK;
+}
+
+int oracle_get_residual_history(oracle_handle h, double* out, int32_t cap) {
+  if (!h) return ORACLE_ERR_INVALID_ARG;
+  int m = (int)h->hist.size();
+  if (out)
+    for (int k = 0; k < m && k < cap; ++k) out[k] = h->hist[k];
+  return m;
 }
 
 int oracle_grad_values(oracle_handle h, const double* lambda, const double* x, int32_t nrhs,

@@ -54,6 +54,12 @@ typedef struct {
   double strong_beta;       /* beta, default 0.25 (A2)                                      */
   double coarse_scale;      /* gamma, default 1.0 (A9)                                      */
   uint64_t hash_seed;       /* tie-break salt; level l uses hash_seed + l (A4)              */
+  int32_t agg_passes;       /* 1 = pairwise; 2 = the intermediate Galerkin matrix is aggregated
+                               again and the maps composed (size-4 aggregates; O-1, NEXT-4);
+                               pass p uses the salt hash_seed + l + 1000 p.  default 1       */
+  int32_t symmetric;        /* 1 (default): w_ij = -a_ij read from row i (A1);  0: the matching
+                               of every level runs on (A_l + A_l^T)/2, union pattern (A1,
+                               nonsymmetric case; bitwise equal to 1 for a bitwise symmetric A) */
 } oracle_options;
 
 typedef struct {
@@ -93,7 +99,7 @@ int oracle_match_rounds(oracle_handle h, int32_t level);                 /* roun
  * candidate edges sorted by descending key (must give the same result on a bitwise
  * symmetric matrix; pin P8).  match[i] = partner or -1; agg[i] in [0, *nc). */
 int oracle_aggregate(int32_t n, const int32_t* rowptr, const int32_t* col, const double* val,
-                     double beta, uint64_t salt, int32_t max_rounds, int32_t mode,
+                     double beta, uint64_t salt, int32_t max_rounds, int32_t mode, int32_t symmetric,
                      int32_t* match, int32_t* agg, int32_t* nc, int32_t* rounds);
 /* O-3 on its own: sizes the output (call with crowptr=NULL to get *cnnz only). */
 int oracle_galerkin(int32_t n, const int32_t* rowptr, const int32_t* col, const double* val,
@@ -110,6 +116,10 @@ int oracle_residual_restrict(oracle_handle h, int32_t level, const double* b, co
 /* O-4: z = B r, one V-cycle from a zero guess, starting at `level` (0 = the preconditioner) */
 int oracle_vcycle(oracle_handle h, int32_t level, const double* r, double* z);
 
+/* O-7: z = B^T r, the same cycle on the transposed level operators A_l^T (same aggregates, same
+ * dinv, LU of A_L^T): exactly the transpose of the linear map of oracle_vcycle when nu1 = nu2. */
+int oracle_vcycle_transpose(oracle_handle h, int32_t level, const double* r, double* z);
+
 /* O-5 / O-6.  krylov: 0 = PCG, 1 = right-preconditioned BiCGSTAB.  precond: 1 = AMG V-cycle,
  * 0 = identity.  x0 = 0.  x is output only. */
 int oracle_solve(oracle_handle h, const double* b, double* x, double rtol, int32_t maxit,
@@ -120,6 +130,11 @@ int oracle_solve(oracle_handle h, const double* b, double* x, double rtol, int32
 int oracle_solve_transpose(oracle_handle h, const double* g, double* lambda, double rtol,
                            int32_t maxit, int32_t krylov, int32_t precond, int32_t symmetric,
                            oracle_info* info);
+/* ||r_k||_2 / ||b||_2 of the last oracle_solve / oracle_solve_transpose on this handle for
+ * k = 1 … iterations (the value the convergence test of iteration k saw).
+ * Returns the number of entries; copies at most `cap` of them into `out` (may be NULL). */
+int oracle_get_residual_history(oracle_handle h, double* out, int32_t cap);
+
 /* O-8: gA[k] (+)= - sum_b lambda_b[i] x_b[col[k]],  rowptr[i] <= k < rowptr[i+1];  columns of
  * Lambda / X are ld apart. */
 int oracle_grad_values(oracle_handle h, const double* lambda, const double* x, int32_t nrhs,

@@ -618,3 +618,325 @@ def test_setup_rules(oracle_mod):
     o5 = oracle_mod.Oracle(A.rowptr, A.col, A.val, hash_seed=99)
     assert not np.array_equal(o5.aggregates(0), o.aggregates(0))
     assert abs(o5.level_info(1)[0] - o.level_info(1)[0]) < 0.05 * o.level_info(1)[0]
+
+
+# ------------------------------------------------------------------------------------------
+# Round-2 pins of branches no earlier pin exercised: LU row swaps, the singleton-merge target (A5),
+# the stall rule (A6); then the readings added in round 2 (nonsymmetric strength A1, agg_passes,
+# residual history)
+# ------------------------------------------------------------------------------------------
+def _csr_from_dense(D):
+    import scipy.sparse as sp
+
+    S = sp.csr_matrix(D)
+    S.sort_indices()
+    return S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64)
+
+
+def _needs_pivoting_matrix(n, seed):
+    """Dense nonsymmetric matrix with a tiny positive diagonal and O(1) off-diagonals: LU without row
+    exchanges loses every digit (pivots ~1e-13), partial pivoting swaps in almost every column."""
+    rng = np.random.default_rng(seed)
+    D = rng.uniform(-1.0, 1.0, (n, n))
+    D[np.abs(D) < 0.05] = 0.05
+    np.fill_diagonal(D, 1e-13 * rng.uniform(1.0, 2.0, n))
+    return D
+
+
+def _lu_nopivot_solve(D, b):
+    a = D.copy()
+    n = len(b)
+    x = b.copy()
+    for k in range(n):
+        for i in range(k + 1, n):
+            l = a[i, k] / a[k, k]
+            a[i, k:] -= l * a[k, k:]
+            x[i] -= l * x[k]
+    for i in range(n - 1, -1, -1):
+        x[i] = (x[i] - a[i, i + 1:] @ x[i + 1:]) / a[i, i]
+    return x
+
+
+@pytest.mark.parametrize("n", [12, 61])
+def test_dense_lu_row_swaps(oracle_mod, n):
+    """S5/U6 with piv[k] != k: a coarsest operator that NEEDS partial pivoting (every earlier case was
+    SPD and diagonally dominant, so the row-swap branch of dense_lu / dense_lu_solve never ran).
+    coarse_max_rows >= n makes the V-cycle the LU solve alone: compare with numpy.linalg.solve."""
+    D = _needs_pivoting_matrix(n, 31 + n)
+    rp, cl, vl = _csr_from_dense(D)
+    o = oracle_mod.Oracle(rp, cl, vl, coarse_max_rows=n)
+    assert o.num_levels == 1
+    rng = np.random.default_rng(5)
+    r = rng.standard_normal(n)
+    want = np.linalg.solve(D, r)
+    z = o.vcycle(r)
+    assert np.linalg.norm(z - want) <= 1e-10 * np.linalg.norm(want)
+    # the case really exercises the swaps: the same elimination without them is useless here
+    bad = _lu_nopivot_solve(D, r)
+    assert not np.linalg.norm(bad - want) <= 1e-6 * np.linalg.norm(want)
+    # the exact preconditioner gives one Krylov iteration, also for the transposed factors (O-7)
+    x, info = o.solve(r, rtol=1e-9, maxit=5, krylov=1)
+    assert info.iterations == 1 and info.status == 0 and np.linalg.norm(x - want) <= 1e-9 * np.linalg.norm(want)
+    lam, info = o.solve_transpose(r, rtol=1e-9, maxit=5, krylov=1, symmetric=0)
+    want_t = np.linalg.solve(D.T, r)
+    assert info.iterations == 1 and np.linalg.norm(lam - want_t) <= 1e-9 * np.linalg.norm(want_t)
+
+
+_M64 = (1 << 64) - 1
+
+
+def _py_mix64(z):
+    z ^= z >> 30
+    z = (z * 0xBF58476D1CE4E5B9) & _M64
+    z ^= z >> 27
+    z = (z * 0x94D049BB133111EB) & _M64
+    z ^= z >> 31
+    return z
+
+
+def py_aggregate(D, beta, salt, merge="max"):
+    """O-2 from its definition with python integers / floats on a dense matrix: handshake rounds to the
+    fix-point, singleton merge into the matched neighbour with the LARGEST key (A5), numbering by
+    ascending root.  merge="min" is the plausible mistake the pin has to catch."""
+    n = D.shape[0]
+    W = -(D - np.diag(np.diag(D)))
+    m = np.maximum(W, 0).max(axis=1)
+    cand = (W > 0) & (W >= beta * np.minimum.outer(m, m))
+
+    def key(i, j):
+        lo, hi = min(i, j), max(i, j)
+        M = max(m[i], m[j])
+        q = 0 if 2 * W[i, j] > M else (1 if 4 * W[i, j] > M else 2)
+        return (-q, _py_mix64((lo * 0x9E3779B97F4A7C15 + hi * 0xBF58476D1CE4E5B9 + salt) & _M64), -lo, -hi)
+
+    match = [-1] * n
+    while True:
+        ptr = [-1] * n
+        for i in range(n):
+            if match[i] < 0:
+                nb = [j for j in range(n) if cand[i, j] and match[j] < 0]
+                if nb:
+                    ptr[i] = max(nb, key=lambda j: key(i, j))
+        added = 0
+        for i in range(n):
+            if ptr[i] >= 0 and ptr[ptr[i]] == i:
+                match[i] = ptr[i]
+                added += 1
+        if not added:
+            break
+    root = [min(i, match[i]) if match[i] >= 0 else i for i in range(n)]
+    root2 = list(root)
+    choices = 0  # singletons whose matched candidate neighbours sit in more than one aggregate
+    for i in range(n):
+        if match[i] < 0:
+            nb = [j for j in range(n) if cand[i, j] and match[j] >= 0]
+            if nb:
+                pick = max if merge == "max" else min
+                root2[i] = root[pick(nb, key=lambda j: key(i, j))]
+                choices += len({root[j] for j in nb}) > 1
+    ids = {r: t for t, r in enumerate(sorted(set(root2)))}
+    return np.array(match), np.array([ids[r] for r in root2]), len(ids), choices
+
+
+def _random_mesh_matrix(n, seed, k=4):
+    """SPD M-matrix of a random planar-ish point cloud (k nearest neighbours, weights over two decades)."""
+    rng = np.random.default_rng(seed)
+    pts = rng.uniform(0, 1, (n, 2))
+    d2 = ((pts[:, None, :] - pts[None, :, :]) ** 2).sum(-1)
+    W = np.zeros((n, n))
+    for i in range(n):
+        for j in np.argsort(d2[i])[1:k + 1]:
+            w = 10.0 ** rng.uniform(-1.0, 1.0)
+            W[i, j] = W[j, i] = max(W[i, j], w)
+    return np.diag(W.sum(axis=1) + 0.1) - W
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_p8_whole_aggregation_bruteforce(oracle_mod, seed):
+    """The WHOLE of O-2 on a 56-vertex graph against python integers: matching to the fix-point, and
+    which matched neighbour a leftover vertex joins (A5: the one with the largest key)."""
+    D = _random_mesh_matrix(56, seed)
+    rp, cl, vl = _csr_from_dense(D)
+    salt = 777 + seed
+    match, agg, nc, _ = oracle_mod.aggregate(rp, cl, vl, 0.25, salt, 0, 0)
+    pm, pa, pnc, choices = py_aggregate(D, 0.25, salt)
+    assert np.array_equal(match, pm) and np.array_equal(agg, pa) and nc == pnc
+    wm, wa, _, _ = py_aggregate(D, 0.25, salt, merge="min")
+    assert choices >= 1 and not np.array_equal(wa, pa)  # the case can tell "largest" from "smallest"
+
+
+def test_stall_rule_and_coarsen_stall(oracle_mod):
+    """A6: n_{l+1} > 0.8 n_l  =>  level l is the coarsest (strict, factor 0.8); n_L > 4096 => error."""
+    def matrix(npairs, nlone):
+        # npairs strongly coupled pairs + nlone rows without any negative off-diagonal (never candidates)
+        n = 2 * npairs + nlone
+        D = np.diag(np.full(n, 4.0))
+        for p in range(npairs):
+            D[2 * p, 2 * p + 1] = D[2 * p + 1, 2 * p] = -1.0
+        for i in range(2 * npairs, n - 1):  # positive couplings keep the lone rows connected but weak (A1)
+            D[i, i + 1] = D[i + 1, i] = 0.5
+        return D
+
+    # 100 rows: 20 pairs + 60 lone -> n_c = 80 = 0.8 n: NOT a stall (strict inequality): one coarse level
+    rp, cl, vl = _csr_from_dense(matrix(20, 60))
+    o = oracle_mod.Oracle(rp, cl, vl)
+    assert o.level_info(0)[0] == 100 and o.num_levels >= 2 and o.level_info(1)[0] == 80
+    # 19 pairs + 62 lone -> n_c = 81 > 80: stall, level 0 is the coarsest and is solved densely
+    D = matrix(19, 62)
+    rp, cl, vl = _csr_from_dense(D)
+    o = oracle_mod.Oracle(rp, cl, vl)
+    assert o.num_levels == 1
+    r = np.random.default_rng(3).standard_normal(100)
+    assert np.allclose(o.vcycle(r), np.linalg.solve(D, r), rtol=1e-12, atol=1e-14)
+    x, info = o.solve(r, rtol=1e-10, maxit=5)
+    assert info.iterations == 1 and info.status == 0
+    # the second level of the first matrix stalls (80 rows > 64, no candidates left but the lone chain)
+    o = oracle_mod.Oracle(*_csr_from_dense(matrix(20, 60)))
+    assert o.num_levels == 2
+    # a stalled coarsest level above 4096 rows is an error (O-1), at 4096 + 1 exactly
+    n = 4097
+    rp = np.arange(n + 1, dtype=np.int32)
+    with pytest.raises(RuntimeError, match="-4"):
+        oracle_mod.Oracle(rp, np.arange(n, dtype=np.int32), np.full(n, 2.0))
+    n = 300  # ... and fine below
+    o = oracle_mod.Oracle(np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32), np.full(n, 2.0))
+    assert o.num_levels == 1 and np.allclose(o.vcycle(np.ones(n)), 0.5)
+
+
+def _row_scaled(S, seed):
+    """A = diag(s) S: nonsymmetric values on a symmetric pattern (the pressure-Poisson-like D^-1 S form)."""
+    n = S.n
+    scale = np.random.default_rng(seed).uniform(0.5, 2.0, n)
+    rows = np.repeat(np.arange(n), np.diff(S.rowptr))
+    return inputs.Csr(n, S.rowptr, S.col, S.val * scale[rows])
+
+
+def _transpose_csr(A):
+    T = A.to_scipy().T.tocsr()
+    T.sort_indices()
+    return inputs.Csr(A.n, T.indptr.astype(np.int32), T.indices.astype(np.int32), T.data.astype(np.float64))
+
+
+def test_nonsymmetric_strength(oracle_mod):
+    """A1, nonsymmetric case: the matching runs on (A + A^T)/2.  Pins: bitwise no-op on a bitwise
+    symmetric matrix; A and A^T get the SAME aggregates; handshake == greedy still holds (the key is
+    symmetric again); structurally nonsymmetric patterns (union pattern) work."""
+    S = inputs.variable_diffusion_csr((7, 6, 5), seed=21, sigma=1.5, ell=2.0)
+    a1 = oracle_mod.aggregate(S.rowptr, S.col, S.val, 0.25, 3, 0, 0, symmetric=1)
+    a0 = oracle_mod.aggregate(S.rowptr, S.col, S.val, 0.25, 3, 0, 0, symmetric=0)
+    assert np.array_equal(a1[0], a0[0]) and np.array_equal(a1[1], a0[1])
+    A = _row_scaled(S, 22)
+    At = _transpose_csr(A)
+    m, agg, nc, _ = oracle_mod.aggregate(A.rowptr, A.col, A.val, 0.25, 3, 0, 0, symmetric=0)
+    mt, aggt, nct, _ = oracle_mod.aggregate(At.rowptr, At.col, At.val, 0.25, 3, 0, 0, symmetric=0)
+    assert np.array_equal(m, mt) and np.array_equal(agg, aggt) and nc == nct
+    mg, aggg, _, _ = oracle_mod.aggregate(A.rowptr, A.col, A.val, 0.25, 3, 0, 1, symmetric=0)
+    assert np.array_equal(m, mg) and np.array_equal(agg, aggg)
+    # the same from the definition: python-integer O-2 on the dense (A + A^T)/2
+    D = A.to_dense()
+    pm, pa, pnc, _ = py_aggregate((D + D.T) / 2, 0.25, 3)
+    assert np.array_equal(m, pm) and np.array_equal(agg, pa) and nc == pnc
+    assert 1.8 <= A.n / nc <= 2.6
+    # structurally nonsymmetric: drop some (i, j) entries but keep (j, i)
+    rng = np.random.default_rng(23)
+    Dn = D.copy()
+    iu = np.argwhere(np.triu(D, 1) != 0)
+    for i, j in iu[rng.choice(len(iu), len(iu) // 4, replace=False)]:
+        Dn[i, j] = 0.0
+    rp, cl, vl = _csr_from_dense(Dn)
+    m2, agg2, nc2, _ = oracle_mod.aggregate(rp, cl, vl, 0.25, 3, 0, 0, symmetric=0)
+    pm2, pa2, pnc2, _ = py_aggregate((Dn + Dn.T) / 2, 0.25, 3)
+    assert np.array_equal(m2, pm2) and np.array_equal(agg2, pa2) and nc2 == pnc2
+
+
+def test_nonsymmetric_hierarchy_and_adjoint(oracle_mod):
+    """O-7 with symmetric = 0 in the options: (P^T A P)^T = P^T A^T P level by level (the transposed
+    hierarchy is the Galerkin hierarchy of A^T on the same aggregates), lambda = A^-T g against numpy,
+    g.x = lambda.b, and the gradient against central finite differences."""
+    S = inputs.variable_diffusion_csr((5, 5, 4), seed=31, sigma=1.0, ell=2.0)
+    A = _row_scaled(S, 32)
+    At = _transpose_csr(A)
+    n = A.n
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, coarse_max_rows=8, symmetric=0)
+    ot = oracle_mod.Oracle(At.rowptr, At.col, At.val, coarse_max_rows=8, symmetric=0)
+    assert o.num_levels == ot.num_levels >= 3
+    for l in range(o.num_levels):
+        if l < o.num_levels - 1:
+            assert np.array_equal(o.aggregates(l), ot.aggregates(l))
+        rp, cl, vl = o.level_csr(l)
+        Tl = _transpose_csr(inputs.Csr(len(rp) - 1, rp, cl, vl))
+        rpt, clt, vlt = ot.level_csr(l)
+        assert np.array_equal(Tl.rowptr, rpt) and np.array_equal(Tl.col, clt)  # pattern: bitwise
+        assert np.max(np.abs(Tl.val - vlt)) <= 1e-14 * np.max(np.abs(vlt))     # values: summation order only
+    D = A.to_dense()
+    rng = np.random.default_rng(33)
+    b, xt = rng.standard_normal(n), rng.standard_normal(n)
+    x, i1 = o.solve(b, rtol=1e-13, maxit=300, krylov=1)
+    lam, i2 = o.solve_transpose(x - xt, rtol=1e-13, maxit=300, krylov=1, symmetric=0)
+    assert i1.status == 0 and i2.status == 0
+    assert np.allclose(x, np.linalg.solve(D, b), rtol=1e-9, atol=1e-11)
+    assert np.allclose(lam, np.linalg.solve(D.T, x - xt), rtol=1e-9, atol=1e-11)
+    g = x - xt
+    assert abs(g @ x - lam @ b) <= 1e-9 * np.linalg.norm(g) * np.linalg.norm(x)
+    # the transposed V-cycle is the transpose of the V-cycle operator (nu1 = nu2): <B^T u, v> = <u, B v>
+    u, v = rng.standard_normal(n), rng.standard_normal(n)
+    Bv = o.vcycle(v)
+    Btu = o.vcycle_transpose(u)  # A_l^T, same aggregates, same dinv (A16)
+    assert abs(Btu @ v - u @ Bv) <= 1e-12 * np.linalg.norm(u) * np.linalg.norm(Bv)
+    assert not abs(o.vcycle(u) @ v - u @ Bv) <= 1e-6 * np.linalg.norm(u) * np.linalg.norm(Bv)  # B itself is not symmetric
+    gA = o.grad_values(lam, x)
+    rows = np.repeat(np.arange(n), np.diff(A.rowptr))
+    loss = lambda Dm: 0.5 * np.sum((np.linalg.solve(Dm, b) - xt) ** 2)
+    ks = rng.choice(A.nnz, 40, replace=False)
+    fd = np.empty(len(ks))
+    for t, k in enumerate(ks):
+        Dp, Dm = D.copy(), D.copy()
+        Dp[rows[k], A.col[k]] += 1e-5
+        Dm[rows[k], A.col[k]] -= 1e-5
+        fd[t] = (loss(Dp) - loss(Dm)) / 2e-5
+    assert np.linalg.norm(gA[ks] - fd) <= 1e-7 * np.linalg.norm(fd)
+
+
+def test_agg_passes_two(oracle_mod):
+    """agg_passes = 2 (O-1; north_star "pairwise or size-4"): the aggregates are the composition of two
+    pairwise matchings, the second one on the intermediate Galerkin matrix with salt hash_seed + l + 1000."""
+    A = inputs.config_matrix(3, 14)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, agg_passes=2, hash_seed=4)
+    _, agg1, nc1, _ = oracle_mod.aggregate(A.rowptr, A.col, A.val, 0.25, 4, 0, 0)
+    mid = oracle_mod.galerkin(A.rowptr, A.col, A.val, agg1, nc1)
+    _, agg2, nc2, _ = oracle_mod.aggregate(mid[0], mid[1], mid[2], 0.25, 4 + 1000, 0, 0)
+    assert np.array_equal(o.aggregates(0), agg2[agg1]) and o.level_info(1)[0] == nc2
+    sizes = np.bincount(o.aggregates(0))
+    assert 3.5 <= A.n / nc2 <= 5.5 and sizes.max() <= 12 and np.median(sizes) == 4
+    # the coarse operator is the Galerkin product on the composed map (dense P^T A P)
+    P = np.zeros((A.n, nc2))
+    P[np.arange(A.n), o.aggregates(0)] = 1.0
+    rp, cl, vl = o.level_csr(1)
+    assert np.allclose(inputs.Csr(nc2, rp, cl, vl).to_dense(), P.T @ dense(A) @ P, rtol=1e-13, atol=1e-13)
+    # fewer levels than pairwise, still an SPD preconditioner that PCG converges with
+    o1 = oracle_mod.Oracle(A.rowptr, A.col, A.val, hash_seed=4)
+    assert o.num_levels < o1.num_levels
+    b = inputs.config_rhs(3, A.n)
+    x, info = o.solve(b, rtol=1e-10, maxit=200)
+    assert info.status == 0 and info.iterations <= 2 * o1.solve(b, rtol=1e-10, maxit=200)[1].iterations
+    assert np.linalg.norm(b - A.to_scipy() @ x) <= 1.01e-10 * np.linalg.norm(b)
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_residual_history(oracle_mod, krylov):
+    """PAPER.md:125 diagnostics: ||r_k|| / ||b|| per iteration; the iterates do not depend on rtol, so the
+    history of a looser solve is a bitwise prefix of a tighter one (what the full-size goldens rely on)."""
+    A = inputs.config_matrix(3, 12)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    b = inputs.config_rhs(3, A.n)
+    _, i12 = o.solve(b, rtol=1e-12, maxit=200, krylov=krylov)
+    h12 = o.residual_history()
+    _, i8 = o.solve(b, rtol=1e-8, maxit=200, krylov=krylov)
+    h8 = o.residual_history()
+    assert len(h12) == i12.iterations and len(h8) == i8.iterations < i12.iterations
+    assert h8[-1] == i8.rel_residual <= 1e-8 < h8[-2]
+    if krylov == 0:
+        assert np.array_equal(h8, h12[:len(h8)])
+        assert int(np.argmax(h12 <= 1e-8)) + 1 == i8.iterations
+    else:  # BiCGSTAB: the last entry of the looser solve may be its half-step exit ||s|| / ||b|| (A11)
+        assert np.array_equal(h8[:-1], h12[:len(h8) - 1])
