@@ -80,9 +80,13 @@ typedef enum { AMG_CONVERGED = 0, AMG_MAXIT = 1, AMG_BREAKDOWN = 2, AMG_NONFINIT
 typedef struct {
   int32_t struct_size;
   int32_t krylov;           /* 0 = PCG, 1 = right-preconditioned BiCGSTAB (paper default)   */
-  int32_t symmetric;        /* 1 = caller asserts A == A^T (no transposition for the adjoint, :95, :114);
-                               0 = not symmetric (amg_solve_transpose -> AMG_ERR_UNSUPPORTED for now);
-                              -1 = check on the device at setup (bitwise a_ij == a_ji)                   */
+  int32_t symmetric;        /* -1 (default) = check on the device at setup, bitwise a_ij == a_ji, one cheap kernel;
+                                1 = caller asserts A == A^T (no check; no transposition for the adjoint, :95, :114);
+                                0 = not symmetric: the matching of every level runs on (A_l + A_l^T)/2 and
+                                    amg_solve_transpose uses the transposed hierarchy            */
+  int32_t agg_passes;       /* 1 = pairwise aggregation (default); 2 = the intermediate Galerkin matrix is
+                               aggregated again and the maps composed (size-4 aggregates); pass p of level l
+                               uses the salt hash_seed + l + 1000 p                                          */
   int32_t pre_sweeps;       /* nu1, default 2                                                            */
   int32_t post_sweeps;      /* nu2, default 2                                                            */
   int32_t smoother;         /* 0 = L1-Jacobi (d_i = sum_j |a_ij|), 1 = damped Jacobi (omega / a_ii)      */
@@ -91,14 +95,9 @@ typedef struct {
   int32_t max_match_rounds; /* 0 = handshake rounds until the fix-point                                  */
   int32_t force_generic;    /* 1 = use the row-vector fallback kernels on every level (tests)            */
   int32_t use_graph;        /* 1 = replay one Krylov iteration as a CUDA graph (default), 0 = plain launches */
-  int32_t tail_max_rows;    /* levels with at most this many rows (and everything below them) run inside ONE
-                               persistent kernel per V-cycle (grid barriers instead of launches); default
-                               2304 (= tail_dense_rows: measured on B200, a grid-barrier phase costs more
-                               than a row-tile launch, so by default the tail is the dense operator alone);
-                               0 = off                                                                   */
-  int32_t tail_dense_rows;  /* inside that kernel, the V-cycle from the first level with at most this many
-                               rows down to the coarsest solve is applied as ONE dense operator assembled
-                               at setup (the same linear map); default 2304, 0 = off         */
+  int32_t tail_dense_rows;  /* the V-cycle from the first level with at most this many rows down to the
+                               coarsest solve is applied as ONE dense operator assembled at setup (the same
+                               linear map); default 2304, 0 = off                            */
   int32_t use_pdl;          /* 1 = the kernels of a captured iteration are chained by programmatic dependent
                                launches (a kernel becomes resident while its predecessor drains); default 1 */
   int32_t split_prolong_rows; /* levels with at least this many rows apply the coarse correction x += gamma P e_c
@@ -162,16 +161,24 @@ AMG_API amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t
 
 AMG_API amg_status amg_destroy(amg_handle h);
 
-/* S1-S9: solve A x = b from x0 = 0 with the Krylov method of the options; x is output only.
- * ||b|| = 0 gives x = 0, 0 iterations, converged.  info may be NULL. */
+/* S1-S9: solve A x = b from x0 = 0 with the Krylov method of the options (a nonsymmetric handle
+ * always uses BiCGSTAB: PCG needs A = A^T); x is output only.  ||b|| = 0 gives x = 0, 0 iterations,
+ * converged.  info == NULL: nothing is reported and the call does not wait for the end of the solve
+ * (it returns with at most the last iteration and the output kernel still in the stream; x is
+ * valid in stream order). */
 AMG_API amg_status amg_solve(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit,
                      amg_info* info, void* cuda_stream);
 /* Same with an explicit Krylov method (0 PCG, 1 BiCGSTAB) and preconditioner switch
  * (1 = AMG V-cycle, 0 = identity: plain CG / BiCGSTAB as in PAPER.md:277). */
 AMG_API amg_status amg_solve_ex(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit,
                         int32_t krylov, int32_t precond, amg_info* info, void* cuda_stream);
-/* G1: A^T lambda = g on the same hierarchy (Eq. 1).  symmetric = 1: the transposition is
- * skipped and this is amg_solve on A. */
+/* G1: A^T lambda = g on the same hierarchy (Eq. 1).  Symmetric handle: the transposition is
+ * skipped and this is amg_solve on A.  Nonsymmetric handle ("forms
+ * A^T ... then solves the adjoint system"): right-preconditioned BiCGSTAB on A^T with the
+ * preconditioner B^T -- the same V-cycle on the transposed level operators A_l^T (= the Galerkin
+ * hierarchy of A^T on the same aggregates), same smoother diagonals, LU of A_L^T; the transposed
+ * operators are built on the device at setup (hand-written CSR transpose) and tile-packed like
+ * the forward ones. */
 AMG_API amg_status amg_solve_transpose(amg_handle h, const double* d_g, double* d_lambda, double rtol,
                                int32_t maxit, amg_info* info, void* cuda_stream);
 /* S10: nrhs independent solves on one hierarchy; column s of B / X starts at s * ld.
@@ -197,7 +204,9 @@ AMG_API amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, dou
 /* ---- introspection / parity hooks (natural numbering) ---- */
 AMG_API amg_status amg_get_num_levels(amg_handle h, int32_t* num_levels);
 AMG_API amg_status amg_get_level_info(amg_handle h, int32_t level, int64_t* rows, int64_t* nnz);
-AMG_API amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out);
+AMG_API amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out, void* cuda_stream);
+/* 1 / 0: what the setup decided (the caller's flag, or the result of the device check for -1). */
+AMG_API amg_status amg_get_symmetric(amg_handle h, int32_t* symmetric);
 AMG_API amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int32_t* d_col,
                              double* d_val, void* cuda_stream);
 AMG_API amg_status amg_get_setup_stats(amg_handle h, amg_setup_stats* stats);
@@ -221,6 +230,9 @@ AMG_API amg_status amg_get_last_launches(amg_handle h, int64_t* launches);
  *   op 5: V-cycle started at level l              (d_in1 = b,           d_out rows(l))
  *   op 6: xout = x~ + dinv o (b - A_l x~), x~ = x + gamma * P e_c
  *                                                 (d_in0 = x, d_in1 = [b rows(l) | e_c rows(l+1)], d_out rows(l))
+ *   op 7: y = A_l^T x   (nonsymmetric handles)    (d_in0 = x,           d_out rows(l))
+ *   op 8: transposed V-cycle started at level l   (d_in1 = b,           d_out rows(l))
+ * The calls are stream-ordered (no synchronisation).
  * `reps` > 1 repeats the kernel back to back (timing); results are those of one application. */
 AMG_API amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0,
                         const double* d_in1, double* d_out, int32_t reps, void* cuda_stream);

@@ -25,15 +25,16 @@ EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_w
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
            "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
-           "amg_get_level_path", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error"]
+           "amg_get_level_path", "amg_get_symmetric", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error"]
 
 
 class amg_options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("krylov", C.c_int32), ("symmetric", C.c_int32),
+                ("agg_passes", C.c_int32),
                 ("pre_sweeps", C.c_int32), ("post_sweeps", C.c_int32), ("smoother", C.c_int32),
                 ("coarse_max_rows", C.c_int32), ("max_levels", C.c_int32),
                 ("max_match_rounds", C.c_int32), ("force_generic", C.c_int32),
-                ("use_graph", C.c_int32), ("tail_max_rows", C.c_int32), ("tail_dense_rows", C.c_int32), ("use_pdl", C.c_int32),
+                ("use_graph", C.c_int32), ("tail_dense_rows", C.c_int32), ("use_pdl", C.c_int32),
                 ("split_prolong_rows", C.c_int32), ("reserved0", C.c_int32),
                 ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double), ("hash_seed", C.c_uint64)]
@@ -206,7 +207,13 @@ def amg_get_level_info(h, level):
 
 
 def amg_get_aggregates(h, level, d_agg_out):
-    _check(load_library().amg_get_aggregates(h, C.c_int32(level), _ptr(d_agg_out, torch.int32)), h)
+    _check(load_library().amg_get_aggregates(h, C.c_int32(level), _ptr(d_agg_out, torch.int32), _stream()), h)
+
+
+def amg_get_symmetric(h) -> int:
+    v = C.c_int32()
+    _check(load_library().amg_get_symmetric(h, C.byref(v)), h)
+    return v.value
 
 
 def amg_get_level_csr(h, level, d_rowptr, d_col, d_val):
@@ -285,6 +292,10 @@ class AmgSolver:
 
     def _dev(self, a):
         return torch.as_tensor(a).to(dtype=torch.float64).to(self.device).contiguous()
+
+    @property
+    def symmetric(self):
+        return amg_get_symmetric(self.h)
 
     @property
     def num_levels(self):

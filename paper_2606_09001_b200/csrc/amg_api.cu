@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "amg_internal.cuh"
 
@@ -10,46 +11,54 @@ namespace {
 
 thread_local std::string g_thread_error;
 
+std::mutex g_alloc_mutex;  // guards the three words below (handles copy them at creation)
 void* (*g_alloc_fn)(size_t, void*, void*) = nullptr;
 void (*g_free_fn)(void*, void*) = nullptr;
 void* g_alloc_user = nullptr;
+
+// Every entry point that takes a handle: the handle's device is made current for the call (and
+// restored), and the stream is remembered (amg_destroy waits for the last one only).
+struct Enter {
+  int prev = -1;
+  Enter(amg_handle_s* h, void* st, bool has_stream = true) {
+    int cur = 0;
+    if (cudaGetDevice(&cur) == cudaSuccess && cur != h->device) {
+      prev = cur;
+      cudaSetDevice(h->device);
+    }
+    if (has_stream) h->last_stream = (cudaStream_t)st;
+  }
+  ~Enter() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
 
 }  // namespace
 
 void amg_set_thread_error(const std::string& s) { g_thread_error = s; }
 
+// Library-owned device memory.  A handle uses the allocator that was installed when it was created
+// (amg_set_allocator) for its whole life, else the device's default stream-ordered pool.
 void* amg_dev_alloc(amg_handle_s* H, size_t bytes, cudaStream_t st) {
   bytes += VEC_PAD * sizeof(double);  // slack for the 16-byte-rounded bulk copies of the row-tile kernels
   void* p = nullptr;
-  if (g_alloc_fn) {
-    p = g_alloc_fn(bytes, (void*)st, g_alloc_user);
-  } else {
+  if (H->alloc_fn) {
+    p = H->alloc_fn(bytes, (void*)st, H->alloc_user);
+  } else if (cudaMallocAsync(&p, bytes, st) != cudaSuccess) {
     // stream-ordered pool: the setup allocates and frees hundreds of temporaries; cudaMalloc /
     // cudaFree would each synchronise the device and map / unmap memory (hundreds of ms per setup)
-    static bool pool_ready = false;
-    if (!pool_ready) {
-      int dev = 0;
-      cudaMemPool_t pool;
-      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        uint64_t keep = ~0ULL;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-      }
-      pool_ready = true;
-    }
-    if (cudaMallocAsync(&p, bytes, st) != cudaSuccess) {
-      cudaGetLastError();
-      p = nullptr;
-    }
+    cudaGetLastError();
+    p = nullptr;
   }
   if (p) H->allocs.push_back(p);
   return p;
 }
 
-static void raw_free(void* p) {
-  if (g_free_fn)
-    g_free_fn(p, g_alloc_user);
+static void raw_free(amg_handle_s* H, void* p) {
+  if (H->free_fn)
+    H->free_fn(p, H->alloc_user);
   else
-    cudaFreeAsync(p, nullptr);  // callers have synchronised the stream that last used p
+    cudaFreeAsync(p, H->last_stream);  // stream-ordered after the last work of the handle
 }
 
 void amg_dev_free(amg_handle_s* H, void* p) {
@@ -57,11 +66,11 @@ void amg_dev_free(amg_handle_s* H, void* p) {
   auto it = std::find(H->allocs.rbegin(), H->allocs.rend(), p);
   if (it == H->allocs.rend()) return;  // not ours (e.g. the caller's val array)
   H->allocs.erase(std::next(it).base());
-  raw_free(p);
+  raw_free(H, p);
 }
 
 void amg_free_all(amg_handle_s* H) {
-  for (void* p : H->allocs) raw_free(p);
+  for (void* p : H->allocs) raw_free(H, p);
   H->allocs.clear();
 }
 
@@ -92,7 +101,7 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
   }
   if (o.pre_sweeps < 0 || o.post_sweeps < 0 || o.max_levels < 1 || o.coarse_max_rows < 1 ||
       (o.smoother != 0 && o.smoother != 1) || (o.krylov != 0 && o.krylov != 1) || !(o.strong_beta >= 0.0) ||
-      o.symmetric < -1 || o.symmetric > 1 || nagg < 0) {
+      o.symmetric < -1 || o.symmetric > 1 || o.agg_passes < 1 || o.agg_passes > 4 || nagg < 0) {
     amg_set_thread_error("amg_setup: option out of range");
     return AMG_ERR_INVALID_ARG;
   }
@@ -108,8 +117,22 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
     delete H;
     return AMG_ERR_CUDA;
   }
+  H->device = dev;
+  H->last_stream = st;
   H->sm_count = prop.multiProcessorCount;
   H->l2_bytes = (size_t)prop.l2CacheSize;
+  {
+    std::lock_guard<std::mutex> lk(g_alloc_mutex);
+    H->alloc_fn = g_alloc_fn, H->free_fn = g_free_fn, H->alloc_user = g_alloc_user;
+  }
+  if (!H->alloc_fn) {  // per device, idempotent: freed blocks stay in the pool, repeated setups reuse them
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      uint64_t keep = ~0ULL;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+  }
+  amg_configure_kernels();  // per-device function attributes (dynamic shared memory opt-in)
 
   auto fail = [&](amg_status s) {
     amg_set_thread_error(H->err.empty() ? "amg_setup failed" : H->err);
@@ -142,7 +165,8 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
     AMG_ALLOC(H, H->partials, double, 2 * (size_t)cap, st);
     AMG_ALLOC(H, H->counter, unsigned, 1, st);
     AMG_CUDA_TRY(H, cudaMemsetAsync(H->counter, 0, sizeof(unsigned), st));
-    AMG_TRY(amg_setup_tail(H, st));
+    AMG_TRY(amg_setup_tail(H, 0, st));
+    if (!H->symmetric) AMG_TRY(amg_ensure_transposed(H, st));
     AMG_CUDA_TRY(H, cudaMemsetAsync(H->ctl, 0, sizeof(KrylovCtl), st));
     AMG_CUDA_TRY(H, cudaMallocHost((void**)&H->h_ctl, sizeof(KrylovCtl) * 8));
     for (auto& e : H->ev) AMG_CUDA_TRY(H, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -164,7 +188,8 @@ amg_status amg_options_default(amg_options* o) {
   memset(o, 0, sizeof(*o));
   o->struct_size = (int32_t)sizeof(amg_options);
   o->krylov = 0;
-  o->symmetric = 1;
+  o->symmetric = -1;
+  o->agg_passes = 1;
   o->pre_sweeps = 2;
   o->post_sweeps = 2;
   o->smoother = 0;
@@ -173,7 +198,6 @@ amg_status amg_options_default(amg_options* o) {
   o->max_match_rounds = 0;
   o->force_generic = 0;
   o->use_graph = 1;
-  o->tail_max_rows = 2304;
   o->tail_dense_rows = 2304;
   o->use_pdl = 1;
   o->split_prolong_rows = 800000;
@@ -186,6 +210,7 @@ amg_status amg_options_default(amg_options* o) {
 
 amg_status amg_set_allocator(void* (*alloc_fn)(size_t, void*, void*), void (*free_fn)(void*, void*), void* user) {
   if ((alloc_fn == nullptr) != (free_fn == nullptr)) return AMG_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lk(g_alloc_mutex);
   g_alloc_fn = alloc_fn;
   g_free_fn = free_fn;
   g_alloc_user = user;
@@ -220,14 +245,14 @@ amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t keep_ag
     h->err = "amg_resetup_values: null values";
     return AMG_ERR_INVALID_ARG;
   }
+  Enter e(h, cuda_stream);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaStreamSynchronize(st);
   std::vector<const int32_t*> aggs;
   if (keep_aggregates)
     for (size_t l = 0; l + 1 < h->lv.size(); ++l) aggs.push_back(h->lv[l].nat_agg);
   amg_handle fresh = nullptr;
-  amg_options o = h->opt;
-  o.symmetric = h->symmetric;  // a device check at the first setup is not repeated
+  amg_options o = h->opt;  // symmetric = -1 repeats the device check on the new values
   const amg_status s = create_handle(&fresh, h->n, h->nnz, h->nat_rowptr, h->nat_col, d_val, &o,
                                      keep_aggregates ? (int32_t)aggs.size() : 0,
                                      keep_aggregates ? aggs.data() : nullptr, cuda_stream);
@@ -241,12 +266,15 @@ amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t keep_ag
 
 amg_status amg_destroy(amg_handle h) {
   if (!h) return AMG_OK;
-  cudaDeviceSynchronize();
-  amg_destroy_graphs(h);
-  for (auto& e : h->ev)
-    if (e) cudaEventDestroy(e);
-  if (h->h_ctl) cudaFreeHost(h->h_ctl);
-  amg_free_all(h);
+  {
+    Enter e(h, nullptr, false);
+    cudaStreamSynchronize(h->last_stream);  // the handle runs one call at a time: its last stream is enough
+    amg_destroy_graphs(h);
+    for (auto& ev : h->ev)
+      if (ev) cudaEventDestroy(ev);
+    if (h->h_ctl) cudaFreeHost(h->h_ctl);
+    amg_free_all(h);
+  }
   delete h;
   return AMG_OK;
 }
@@ -258,24 +286,31 @@ amg_status amg_solve_ex(amg_handle h, const double* d_b, double* d_x, double rto
     h->err = "amg_solve: bad argument";
     return AMG_ERR_INVALID_ARG;
   }
-  return amg_krylov_solve(h, d_b, d_x, rtol, maxit, krylov, precond ? 1 : 0, info, (cudaStream_t)cuda_stream);
+  Enter e(h, cuda_stream);
+  return amg_krylov_solve(h, d_b, d_x, rtol, maxit, krylov, precond ? 1 : 0, 0, info, (cudaStream_t)cuda_stream);
 }
 
 amg_status amg_solve(amg_handle h, const double* d_b, double* d_x, double rtol, int32_t maxit, amg_info* info,
                      void* cuda_stream) {
   if (!h) return AMG_ERR_INVALID_ARG;
-  return amg_solve_ex(h, d_b, d_x, rtol, maxit, h->opt.krylov, 1, info, cuda_stream);
+  // PCG needs A = A^T: a nonsymmetric handle solves with BiCGSTAB (the paper's default)
+  return amg_solve_ex(h, d_b, d_x, rtol, maxit, h->symmetric ? h->opt.krylov : 1, 1, info, cuda_stream);
 }
 
 amg_status amg_solve_transpose(amg_handle h, const double* d_g, double* d_lambda, double rtol, int32_t maxit,
                                amg_info* info, void* cuda_stream) {
   if (!h) return AMG_ERR_INVALID_ARG;
-  if (!h->symmetric) {
-    h->err = "amg_solve_transpose: nonsymmetric matrices are not supported yet";
-    return AMG_ERR_UNSUPPORTED;
-  }
   // symmetric: the transposition is skipped, A lambda = g is solved on the same hierarchy
-  return amg_solve(h, d_g, d_lambda, rtol, maxit, info, cuda_stream);
+  if (h->symmetric) return amg_solve(h, d_g, d_lambda, rtol, maxit, info, cuda_stream);
+  if (!d_g || !d_lambda || maxit < 0 || !(rtol >= 0.0)) {
+    h->err = "amg_solve_transpose: bad argument";
+    return AMG_ERR_INVALID_ARG;
+  }
+  // nonsymmetric: operator A^T, preconditioner B^T (transposed level operators on the same aggregates,
+  // same smoother diagonals), right-preconditioned BiCGSTAB
+  Enter e(h, cuda_stream);
+  AMG_TRY(amg_ensure_transposed(h, (cudaStream_t)cuda_stream));
+  return amg_krylov_solve(h, d_g, d_lambda, rtol, maxit, 1, 1, 1, info, (cudaStream_t)cuda_stream);
 }
 
 amg_status amg_solve_batched(amg_handle h, int32_t transpose, const double* d_B, double* d_X, int32_t nrhs,
@@ -303,6 +338,7 @@ amg_status amg_solve_host(amg_handle h, const double* h_b, double* h_x, double r
     h->err = "amg_solve_host: null pointer";
     return AMG_ERR_INVALID_ARG;
   }
+  Enter e(h, cuda_stream);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t bytes = sizeof(double) * (size_t)h->n;
   AMG_CUDA_TRY(h, cudaMemcpyAsync(h->io_tmp, h_b, bytes, cudaMemcpyHostToDevice, st));
@@ -319,12 +355,14 @@ amg_status amg_grad_values(amg_handle h, const double* d_lambda, const double* d
     h->err = "amg_grad_values: bad argument";
     return AMG_ERR_INVALID_ARG;
   }
+  Enter e(h, cuda_stream);
   return amg_grad_values_impl(h, d_lambda, d_x, nrhs, ld, d_gA, accumulate, (cudaStream_t)cuda_stream);
 }
 
 amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, double* d_z, void* cuda_stream) {
   if (!h) return AMG_ERR_INVALID_ARG;
   if (!d_r || !d_z) return AMG_ERR_INVALID_ARG;
+  Enter e(h, cuda_stream);
   return amg_level_op_impl(h, 0, 5, nullptr, d_r, d_z, 1, (cudaStream_t)cuda_stream);
 }
 
@@ -341,10 +379,11 @@ amg_status amg_get_level_info(amg_handle h, int32_t level, int64_t* rows, int64_
   return AMG_OK;
 }
 
-amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out) {
+amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out, void* cuda_stream) {
   if (!h || level < 0 || level >= (int32_t)h->lv.size() - 1 || !d_agg_out) return AMG_ERR_INVALID_ARG;
-  AMG_CUDA_TRY(h, cudaMemcpy(d_agg_out, h->lv[level].nat_agg, sizeof(int) * (size_t)h->lv[level].n,
-                             cudaMemcpyDeviceToDevice));
+  Enter e(h, cuda_stream);
+  AMG_CUDA_TRY(h, cudaMemcpyAsync(d_agg_out, h->lv[level].nat_agg, sizeof(int) * (size_t)h->lv[level].n,
+                                  cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
   return AMG_OK;
 }
 
@@ -352,6 +391,7 @@ amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int
                              void* cuda_stream) {
   if (!h || level < 0 || level >= (int32_t)h->lv.size() || !d_rowptr || !d_col || !d_val)
     return AMG_ERR_INVALID_ARG;
+  Enter e(h, cuda_stream);
   return amg_natural_level_csr(h, level, d_rowptr, d_col, d_val, (cudaStream_t)cuda_stream);
 }
 
@@ -379,9 +419,16 @@ amg_status amg_get_last_launches(amg_handle h, int64_t* launches) {
   return AMG_OK;
 }
 
+amg_status amg_get_symmetric(amg_handle h, int32_t* symmetric) {
+  if (!h || !symmetric) return AMG_ERR_INVALID_ARG;
+  *symmetric = h->symmetric;
+  return AMG_OK;
+}
+
 amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0, const double* d_in1,
                         double* d_out, int32_t reps, void* cuda_stream) {
   if (!h || level < 0 || level >= (int32_t)h->lv.size() || !d_out) return AMG_ERR_INVALID_ARG;
+  Enter e(h, cuda_stream);
   return amg_level_op_impl(h, level, op, d_in0, d_in1, d_out, reps, (cudaStream_t)cuda_stream);
 }
 

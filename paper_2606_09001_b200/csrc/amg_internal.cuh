@@ -9,44 +9,19 @@
 #include "amg_b200.h"
 
 // ------------------------------------------------------------------------------------------
-// tuning constants of the row-tile streaming kernels; the -D overrides exist for
-// tuning sweeps only
+// tuning constants of the row-tile streaming kernels
 // ------------------------------------------------------------------------------------------
-#ifndef RT_STAGES_CFG
-#define RT_STAGES_CFG 3
-#endif
-#ifndef RT_CTAS_CFG
-#define RT_CTAS_CFG 2
-#endif
-#ifndef RT_STAGE_BYTES_CFG
-#define RT_STAGE_BYTES_CFG 29696
-#endif
-#ifndef RT_XSLOTS_CFG
-#define RT_XSLOTS_CFG 4
-#endif
-#ifndef RT_XSLOT_BYTES_CFG
-#define RT_XSLOT_BYTES_CFG 5632
-#endif
-constexpr int RT_CONSUMERS = 256;                  // consumer threads per CTA (8 warps walk the ELL slices)
-#ifndef RT_GATHERERS_CFG
-#define RT_GATHERERS_CFG 192
-#endif
-#ifndef RT_GATHER_UNROLL
-#define RT_GATHER_UNROLL 4
-#endif
-#ifndef RT_GGROUPS
-#define RT_GGROUPS 2   // groups of gather warps working on alternate tiles
-#endif
-#ifndef RT_GATHER_ROWS
-#define RT_GATHER_ROWS 2
-#endif
-constexpr int RT_GATHERERS = RT_GATHERERS_CFG;      // warps x 32 that fetch the halo values one tile ahead
+constexpr int RT_CONSUMERS = 256;     // consumer threads per CTA (8 warps walk the ELL slices)
+constexpr int RT_GATHERERS = 192;     // gather threads (6 warps) that assemble the x slots ahead of the row walk
+constexpr int RT_GATHER_UNROLL = 4;   // halo columns per gather thread held in registers
+constexpr int RT_GGROUPS = 2;         // groups of gather warps working on alternate tiles
+constexpr int RT_GATHER_ROWS = 2;     // own rows per gather thread held in registers
 constexpr int RT_THREADS = RT_CONSUMERS + 32 + RT_GATHERERS;  // + one producer warp (issues the bulk copies)
-constexpr int RT_STAGES = RT_STAGES_CFG;           // tiles in the bulk-async ring of a CTA
-constexpr int RT_CTAS = RT_CTAS_CFG;               // persistent CTAs per SM
-constexpr int RT_STAGE_BYTES = RT_STAGE_BYTES_CFG; // shared memory of one ring stage (descriptor + operands of one tile)
-constexpr int RT_XSLOTS = RT_XSLOTS_CFG;           // x slots (side ring): how many tiles the gather warps run ahead
-constexpr int RT_XSLOT_BYTES = RT_XSLOT_BYTES_CFG; // one x slot: 8 bytes x (rows + halo columns of a tile)
+constexpr int RT_STAGES = 3;          // tiles in the bulk-async ring of a CTA
+constexpr int RT_CTAS = 2;            // persistent CTAs per SM
+constexpr int RT_STAGE_BYTES = 29696; // shared memory of one ring stage (descriptor + operands of one tile)
+constexpr int RT_XSLOTS = 4;          // x slots (side ring): how many tiles the gather warps run ahead
+constexpr int RT_XSLOT_BYTES = 5632;  // one x slot: 8 bytes x (rows + halo columns of a tile)
 constexpr int RT_MAX_NNZ = 4096;                   // most entries / halo columns of a tile (packer scratch)
 constexpr int RT_MAX_ROWS = 1024;                  // most rows of a tile
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
@@ -84,6 +59,23 @@ enum FinalizeId {
 // ------------------------------------------------------------------------------------------
 // one level of the hierarchy, stored in aggregate-contiguous ("permuted") numbering
 // ------------------------------------------------------------------------------------------
+// transposed operator A_l^T of a level (nonsymmetric adjoint): same rows, same
+// aggregates, same permuted numbering, its own tile partition and blobs
+struct LevelOpT {
+  int* rowptr = nullptr;
+  int* col = nullptr;
+  double* val = nullptr;
+  int* src = nullptr;       // [nnz] position in the level's own val[] every entry came from (value-only resetup)
+  int* blk_ptr = nullptr;
+  TileDesc* tiles = nullptr;
+  unsigned char* blob = nullptr;
+  int* halo_idx = nullptr;
+  int* halo_cagg = nullptr;
+  size_t blob_bytes = 0;
+  int nblk = 0;
+  int fast = 0;
+};
+
 struct Level {
   int n = 0;        // rows
   int nc = 0;       // rows of the next level (0 on the coarsest)
@@ -105,6 +97,7 @@ struct Level {
   size_t blob_bytes = 0;
   int nblk = 0;
   int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback
+  LevelOpT T;               // A_l^T (only when the handle is nonsymmetric)
   int lpr = 8;              // lanes per row of the fallback kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary
@@ -126,10 +119,13 @@ struct amg_handle_s {
   // natural level-0 pattern for amg_grad_values
   int* nat_rowptr = nullptr;
   int* nat_col = nullptr;
-  // coarsest dense LU
+  // coarsest dense LU (of A_L; luT / pivT: of A_L^T, nonsymmetric handles only)
   int nL = 0;
   double* lu = nullptr;
   int* piv = nullptr;
+  double* luT = nullptr;
+  int* pivT = nullptr;
+  bool have_T = false;
   // Krylov work vectors (level-0 size, permuted numbering)
   double* kv[10] = {nullptr};
   double* io_tmp = nullptr;  // staging for amg_solve_host / hooks
@@ -140,24 +136,27 @@ struct amg_handle_s {
   double* partials = nullptr;     // [2 * partials_cap]
   int partials_cap = 0;
   unsigned* counter = nullptr;
-  // coarse tail of the V-cycle: levels >= tail_first run inside one persistent kernel (amg_tail.cuh)
-  int tail_first = -1;               // -1: off
+  // coarse tail of the V-cycle: the cycle from level tail_dense_level down is one dense operator (amg_tail.cuh)
   int tail_grid = 0;
-  void* d_tail = nullptr;            // TailLevel[levels] on the device
-  unsigned long long* tail_bar = nullptr;
-  void* d_tail_chunk = nullptr;      // TailChunk[levels][tail_grid]
-  int tail_dense_level = -1;         // levels >= this are applied as the dense operator tail_dense_B
+  int tail_dense_level = -1;         // -1: off
   double* tail_dense_B = nullptr;
-  int tail_lu_smem = 0;              // dynamic shared memory: LU scratch, then the staged operator chunks
-  int tail_smem = 0;
+  double* tail_dense_BT = nullptr;   // the same for the transposed hierarchy
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
   // [krylov * 2 + precond]: one iteration; [4]: the start of an AMG-PCG solve (first V-cycle + p = z)
-  cudaGraphExec_t graph_exec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-  int64_t graph_launches[5] = {0, 0, 0, 0, 0};  // kernel nodes per replay
+  // [5]: one BiCGSTAB + AMG iteration on the transposed hierarchy
+  cudaGraphExec_t graph_exec[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  int64_t graph_launches[6] = {0, 0, 0, 0, 0, 0};  // kernel nodes per replay
   double* vcycle_final_out = nullptr;        // if set: the last post-sweep of a cycle started at level 0 writes here
   int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;  // graphs are captured here (the legacy stream cannot capture)
+  int device = 0;                     // the device the handle lives on
+  cudaStream_t last_stream = nullptr; // stream of the last call (amg_destroy waits for it)
+  void* (*alloc_fn)(size_t, void*, void*) = nullptr;  // allocator captured at creation (amg_set_allocator)
+  void (*free_fn)(void*, void*) = nullptr;
+  void* alloc_user = nullptr;
+  double* grad_xt = nullptr;          // interleaved right-hand sides of amg_grad_values (grown on demand)
+  size_t grad_xt_cap = 0;
   int sm_count = 148;
   size_t l2_bytes = 0;
   int symmetric = 1;
@@ -212,11 +211,14 @@ amg_status amg_exclusive_scan(amg_handle_s* H, const int* d_in, int* d_out, int 
 amg_status amg_vcycle(amg_handle_s* H, int level, const double* b, double** x_out, KrylovCtl* ctl,
                       bool fuse_rz, cudaStream_t st, bool x1_ready = false);
 amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, double rtol, int maxit,
-                            int krylov, int precond, amg_info* info, cudaStream_t st);
+                            int krylov, int precond, int transposed, amg_info* info, cudaStream_t st);
 amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d_in0,
                              const double* d_in1, double* d_out, int reps, cudaStream_t st);
 amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const double* d_x, int nrhs,
                                 int64_t ld, double* d_gA, int accumulate, cudaStream_t st);
 double amg_algorithmic_bytes(amg_handle_s* H, int which);
 void amg_destroy_graphs(amg_handle_s* H);
-amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st);
+amg_status amg_setup_tail(amg_handle_s* H, int transposed, cudaStream_t st);
+void amg_configure_kernels();
+// setup.cu: transposed level operators, their tile blobs, LU of A_L^T, dense tail of B^T
+amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st);

@@ -951,16 +951,6 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __r
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, FIN_RR);
 }
 
-// dst = src (keeps phat across the second V-cycle of a BiCGSTAB iteration; a kernel, not a memcpy
-// node, so that the captured iteration is a chain of kernels with programmatic edges)
-__global__ void __launch_bounds__(RED_THREADS) k_copy(int n, const double* __restrict__ src, double* __restrict__ dst,
-                                                      const KrylovCtl* ctl) {
-  pdl_sync();
-  if (ctl->done) return;
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
-    dst[i] = src[i];
-}
-
 // sum a.b  (used when no smoother sweep can carry the r.z product)
 __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __restrict__ a, const double* __restrict__ b,
                                                      double* partials, unsigned* counter, KrylovCtl* ctl, int fin) {

@@ -780,6 +780,110 @@ __global__ void k_pad_tail(int nnz, int nnz_alloc, int* __restrict__ col, double
   }
 }
 
+inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
+
+amg_status read_int(amg_handle_s* H, const int* d, int* h, cudaStream_t st) {
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(h, d, sizeof(int), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  return AMG_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// CSR transpose on the device (NEXT-2; the paper calls cuSPARSE for it): count ->
+// scan -> fill (atomic cursors: arbitrary order inside a row) -> per-row sort by column, which makes
+// the result unique.  src[p] = position in the input the entry p came from: a value-only update
+// re-transposes with one gather.
+// ------------------------------------------------------------------------------------------
+__global__ void k_tr_count(int nnz, const int* __restrict__ col, int* __restrict__ cnt) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < nnz) atomicAdd(&cnt[col[k]], 1);
+}
+__global__ void k_tr_fill(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                          const int* __restrict__ tptr, int* __restrict__ cursor, int* __restrict__ tcol,
+                          int* __restrict__ tsrc) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+    const int j = col[k];
+    const int p = tptr[j] + atomicAdd(&cursor[j], 1);
+    tcol[p] = i;
+    tsrc[p] = k;
+  }
+}
+__global__ void k_tr_sort(int n, const int* __restrict__ tptr, int* __restrict__ tcol, int* __restrict__ tsrc) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const int s = tptr[j], e = tptr[j + 1];
+  for (int a = s + 1; a < e; ++a) {
+    const int c = tcol[a], k = tsrc[a];
+    int b = a - 1;
+    while (b >= s && tcol[b] > c) {
+      tcol[b + 1] = tcol[b];
+      tsrc[b + 1] = tsrc[b];
+      --b;
+    }
+    tcol[b + 1] = c;
+    tsrc[b + 1] = k;
+  }
+}
+__global__ void k_gather_vals(int nnz, const double* __restrict__ val, const int* __restrict__ src,
+                              double* __restrict__ out) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < nnz) out[p] = val[src[p]];
+}
+
+// outputs are allocated here: trowptr[n+1], tcol / tval [nnz_alloc], tsrc[nnz]
+amg_status transpose_csr(amg_handle_s* H, int n, int nnz, int nnz_alloc, const int* rowptr, const int* col,
+                         const double* val, int** trowptr, int** tcol, double** tval, int** tsrc, cudaStream_t st) {
+  int* cnt;
+  AMG_ALLOC(H, cnt, int, n + 1, st);
+  AMG_ALLOC(H, *trowptr, int, n + 1, st);
+  AMG_ALLOC(H, *tcol, int, nnz_alloc, st);
+  AMG_ALLOC(H, *tval, double, nnz_alloc, st);
+  AMG_ALLOC(H, *tsrc, int, nnz, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
+  k_tr_count<<<grid_for(nnz), TPB, 0, st>>>(nnz, col, cnt);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_exclusive_scan(H, cnt, *trowptr, n, st));
+  AMG_CUDA_TRY(H, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
+  k_tr_fill<<<grid_for(n), TPB, 0, st>>>(n, rowptr, col, *trowptr, cnt, *tcol, *tsrc);
+  k_tr_sort<<<grid_for(n), TPB, 0, st>>>(n, *trowptr, *tcol, *tsrc);
+  k_gather_vals<<<grid_for(nnz), TPB, 0, st>>>(nnz, val, *tsrc, *tval);
+  if (nnz_alloc > nnz) k_pad_tail<<<1, 32, 0, st>>>(nnz, nnz_alloc, *tcol, *tval);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  amg_dev_free(H, cnt);
+  return AMG_OK;
+}
+
+// S = (A + A^T) / 2 on the union of the two patterns (reading A1, nonsymmetric case: the strength of
+// the pair {i,j} is w_ij = -(a_ij + a_ji)/2; commutative, so S is bitwise symmetric; a missing
+// entry counts as 0).  Two sorted lists per row: ascending union.
+__global__ void k_sym_rows(int n, const int* __restrict__ rp, const int* __restrict__ col,
+                           const double* __restrict__ val, const int* __restrict__ trp,
+                           const int* __restrict__ tcol, const double* __restrict__ tval,
+                           const int* __restrict__ srp, int* __restrict__ scol, double* __restrict__ sval,
+                           int* __restrict__ len) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int ka = rp[i], kt = trp[i], m = 0;
+  const int ea = rp[i + 1], et = trp[i + 1];
+  const int d = srp ? srp[i] : 0;
+  while (ka < ea || kt < et) {
+    const int ca = ka < ea ? col[ka] : 0x7fffffff, ct = kt < et ? tcol[kt] : 0x7fffffff;
+    const int c = ca < ct ? ca : ct;
+    double a = 0.0, t = 0.0;
+    if (ca == c) a = val[ka++];
+    if (ct == c) t = tval[kt++];
+    if (srp) {
+      scol[d + m] = c;
+      sval[d + m] = (a + t) / 2;
+    }
+    ++m;
+  }
+  if (!srp) len[i] = m;
+}
+
 // natural-numbering CSR of one level while the hierarchy is being built
 struct NatCsr {
   int n = 0, nnz = 0;
@@ -793,18 +897,32 @@ struct NatCsr {
   int nc = 0;
 };
 
-inline int grid_for(int n) { return n > 0 ? div_up(n, TPB) : 1; }
-
-amg_status read_int(amg_handle_s* H, const int* d, int* h, cudaStream_t st) {
-  AMG_CUDA_TRY(H, cudaMemcpyAsync(h, d, sizeof(int), cudaMemcpyDeviceToHost, st));
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  return AMG_OK;
+__global__ void k_compose_agg(int n, int* __restrict__ agg, const int* __restrict__ agg2) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) agg[i] = agg2[agg[i]];
 }
 
-// U1-U3 on one level: fills N.agg / N.nc
-amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* rounds_out, cudaStream_t st) {
-  const int n = N.n;
+// U1-U3 on one matrix: *agg_out (allocated here), *nc_out.  Nonsymmetric handles match on S = (A + A^T)/2.
+amg_status aggregate_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
+                         uint64_t salt, int** agg_out, int* nc_out, int* rounds_out, cudaStream_t st) {
   const amg_options& o = H->opt;
+  int *trp = nullptr, *tcol = nullptr, *tsrc = nullptr, *srp = nullptr, *scol = nullptr, *slen = nullptr;
+  double *tval = nullptr, *sval = nullptr;
+  if (!H->symmetric) {
+    AMG_TRY(transpose_csr(H, n, nnz, nnz, rowptr, col, val, &trp, &tcol, &tval, &tsrc, st));
+    AMG_ALLOC(H, slen, int, n, st);
+    AMG_ALLOC(H, srp, int, n + 1, st);
+    k_sym_rows<<<grid_for(n), TPB, 0, st>>>(n, rowptr, col, val, trp, tcol, tval, nullptr, nullptr, nullptr, slen);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_TRY(amg_exclusive_scan(H, slen, srp, n, st));
+    int snnz = 0;
+    AMG_TRY(read_int(H, srp + n, &snnz, st));
+    AMG_ALLOC(H, scol, int, snnz, st);
+    AMG_ALLOC(H, sval, double, snnz, st);
+    k_sym_rows<<<grid_for(n), TPB, 0, st>>>(n, rowptr, col, val, trp, tcol, tval, srp, scol, sval, nullptr);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    rowptr = srp, col = scol, val = sval;
+  }
   double* m;
   int *match, *ptr, *root, *isroot, *id, *added;
   AMG_ALLOC(H, m, double, n, st);
@@ -815,13 +933,13 @@ amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* round
   AMG_ALLOC(H, id, int, n + 1, st);
   AMG_ALLOC(H, added, int, 1, st);
   const int g = grid_for(n);
-  k_row_max<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m);
+  k_row_max<<<g, TPB, 0, st>>>(n, rowptr, col, val, m);
   k_fill_int<<<g, TPB, 0, st>>>(n, match, -1);
   int rounds = 0;
   for (;;) {
     if (o.max_match_rounds > 0 && rounds >= o.max_match_rounds) break;
     AMG_CUDA_TRY(H, cudaMemsetAsync(added, 0, sizeof(int), st));
-    k_propose<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m, o.strong_beta, salt, match, ptr);
+    k_propose<<<g, TPB, 0, st>>>(n, rowptr, col, val, m, o.strong_beta, salt, match, ptr);
     k_handshake<<<g, TPB, 0, st>>>(n, ptr, match, added);
     AMG_CUDA_TRY(H, cudaGetLastError());
     int h_added = 0;
@@ -830,21 +948,44 @@ amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* round
     if (h_added == 0) break;
   }
   *rounds_out = rounds;
-  k_roots<<<g, TPB, 0, st>>>(n, N.rowptr, N.col, N.val, m, o.strong_beta, salt, match, root, isroot);
+  k_roots<<<g, TPB, 0, st>>>(n, rowptr, col, val, m, o.strong_beta, salt, match, root, isroot);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_TRY(amg_exclusive_scan(H, isroot, id, n, st));
-  AMG_TRY(read_int(H, id + n, &N.nc, st));
-  AMG_ALLOC(H, N.agg, int, n, st);
-  k_assign_agg<<<g, TPB, 0, st>>>(n, root, id, N.agg);
+  AMG_TRY(read_int(H, id + n, nc_out, st));
+  AMG_ALLOC(H, *agg_out, int, n, st);
+  k_assign_agg<<<g, TPB, 0, st>>>(n, root, id, *agg_out);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  amg_dev_free(H, m);
-  amg_dev_free(H, match);
-  amg_dev_free(H, ptr);
-  amg_dev_free(H, root);
-  amg_dev_free(H, isroot);
-  amg_dev_free(H, id);
-  amg_dev_free(H, added);
+  for (void* q : {(void*)m, (void*)match, (void*)ptr, (void*)root, (void*)isroot, (void*)id, (void*)added, (void*)trp,
+                  (void*)tcol, (void*)tval, (void*)tsrc, (void*)srp, (void*)scol, (void*)sval, (void*)slen})
+    amg_dev_free(H, q);
+  return AMG_OK;
+}
+
+amg_status build_members(amg_handle_s* H, NatCsr& N, cudaStream_t st);
+amg_status galerkin_level(amg_handle_s* H, const NatCsr& N, NatCsr& C, cudaStream_t st);
+
+// U1-U3 on one level: fills N.agg / N.nc.  agg_passes = 2: the intermediate Galerkin matrix is aggregated
+// again (salt + 1000) and the two maps are composed (size-4 aggregates)
+amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* rounds_out, cudaStream_t st) {
+  AMG_TRY(aggregate_csr(H, N.n, N.nnz, N.rowptr, N.col, N.val, salt, &N.agg, &N.nc, rounds_out, st));
+  for (int p = 1; p < H->opt.agg_passes; ++p) {
+    NatCsr mid;
+    AMG_TRY(build_members(H, N, st));
+    AMG_TRY(galerkin_level(H, N, mid, st));
+    int* agg2 = nullptr;
+    int nc2 = 0, r2 = 0;
+    AMG_TRY(aggregate_csr(H, mid.n, mid.nnz, mid.rowptr, mid.col, mid.val, salt + 1000ull * (uint64_t)p, &agg2, &nc2,
+                          &r2, st));
+    k_compose_agg<<<grid_for(N.n), TPB, 0, st>>>(N.n, N.agg, agg2);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    N.nc = nc2;
+    if (r2 > *rounds_out) *rounds_out = r2;
+    for (void* q : {(void*)agg2, (void*)mid.rowptr, (void*)mid.col, (void*)mid.val, (void*)N.mptr, (void*)N.mem})
+      amg_dev_free(H, q);
+    N.mptr = N.mem = nullptr;
+  }
   return AMG_OK;
 }
 
@@ -916,6 +1057,108 @@ amg_status permute_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   amg_dev_free(H, len);
   (void)nnz;
+  return AMG_OK;
+}
+
+// U6: dense LU with partial pivoting of a (coarsest) operator given in CSR; *lu / *piv allocated here
+amg_status dense_lu_of(amg_handle_s* H, int n, const int* rowptr, const int* col, const double* val, double** lu,
+                       int** piv, cudaStream_t st) {
+  AMG_ALLOC(H, *lu, double, (size_t)n * n, st);
+  AMG_ALLOC(H, *piv, int, n, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(*lu, 0, sizeof(double) * (size_t)n * n, st));
+  k_csr_to_dense<<<grid_for(n), TPB, 0, st>>>(n, rowptr, col, val, *lu);
+  int* info;
+  AMG_ALLOC(H, info, int, 1, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, sizeof(int), st));
+  k_dense_lu<<<1, n <= 64 ? 256 : 1024, 0, st>>>(n, *lu, *piv, info);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  int h_info = 0;
+  AMG_TRY(read_int(H, info, &h_info, st));
+  amg_dev_free(H, info);
+  if (h_info) {
+    H->err = "coarsest operator is singular";
+    return AMG_ERR_COARSE_SINGULAR;
+  }
+  return AMG_OK;
+}
+
+// Row-tile partition by stage bytes, then the tile packer (amg_tilepack.cuh) for one operator of a
+// level (A_l or A_l^T) in permuted numbering.  The byte model of the partition is approximate (the
+// halo of a tile is only known once it is cut), so the target is rescaled until every tile fits a
+// ring stage.  fast = 0: no partition fits (very long rows): the level runs the row-vector kernels.
+struct TilePack {
+  int* blk_ptr = nullptr;
+  TileDesc* tiles = nullptr;
+  unsigned char* blob = nullptr;
+  int* halo_idx = nullptr;
+  int* halo_cagg = nullptr;
+  size_t blob_bytes = 0;
+  int nblk = 0, fast = 0;
+};
+
+amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
+                      const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st) {
+  const int64_t total_w = RT_NNZ_WEIGHT * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
+  double scale = 1.0;
+  for (int attempt = 0; attempt < 6 && !P.fast; ++attempt) {
+    const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
+    if (target < 512) break;
+    if (P.blk_ptr) amg_dev_free(H, P.blk_ptr);
+    if (P.tiles) amg_dev_free(H, P.tiles);
+    P.blk_ptr = nullptr, P.tiles = nullptr;
+    P.nblk = div_up(total_w, target);
+    int *size16, *off16, *nh, *hoff, *info;
+    AMG_ALLOC(H, P.blk_ptr, int, P.nblk + 1, st);
+    AMG_ALLOC(H, P.tiles, TileDesc, P.nblk, st);
+    AMG_ALLOC(H, size16, int, P.nblk + 1, st);
+    AMG_ALLOC(H, off16, int, P.nblk + 1, st);
+    AMG_ALLOC(H, nh, int, P.nblk + 1, st);
+    AMG_ALLOC(H, hoff, int, P.nblk + 1, st);
+    AMG_ALLOC(H, info, int, 4, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 4 * sizeof(int), st));
+    k_blk_partition<<<grid_for(P.nblk + 1), TPB, 0, st>>>(P.nblk, target, agg_ptr ? nc : n, agg_ptr, rowptr, n, P.blk_ptr);
+    k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, 0, nullptr, nullptr, size16, nh,
+                                               info, P.tiles, nullptr, nullptr, nullptr);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    int h_info[4];
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    if (h_info[1]) {
+      scale *= 0.5;
+    } else if (h_info[0] > RT_STAGE_BYTES || h_info[2] > RT_XSLOT_BYTES) {
+      const double f1 = (double)RT_STAGE_BYTES / (double)h_info[0], f2 = (double)RT_XSLOT_BYTES / (double)h_info[2];
+      scale *= 0.96 * (f1 < f2 ? f1 : f2);
+    } else {
+      AMG_TRY(amg_exclusive_scan(H, size16, off16, P.nblk, st));
+      AMG_TRY(amg_exclusive_scan(H, nh, hoff, P.nblk, st));
+      int total16 = 0, total_h = 0;
+      AMG_TRY(read_int(H, off16 + P.nblk, &total16, st));
+      AMG_TRY(read_int(H, hoff + P.nblk, &total_h, st));
+      P.blob_bytes = (size_t)total16 * 16u;
+      P.blob = (unsigned char*)amg_dev_alloc(H, P.blob_bytes + 16, st);
+      if (!P.blob) {
+        H->err = "device allocation failed: tile blobs";
+        return AMG_ERR_OOM;
+      }
+      AMG_ALLOC(H, P.halo_idx, int, total_h + 4, st);
+      AMG_ALLOC(H, P.halo_cagg, int, total_h + 4, st);
+      k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, 1, off16, hoff, size16, nh, info,
+                                                 P.tiles, P.blob, P.halo_idx, P.halo_cagg);
+      AMG_CUDA_TRY(H, cudaGetLastError());
+      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+      P.fast = 1;
+    }
+    amg_dev_free(H, size16);
+    amg_dev_free(H, off16);
+    amg_dev_free(H, nh);
+    amg_dev_free(H, hoff);
+    amg_dev_free(H, info);
+  }
+  if (!P.fast) {
+    if (P.blk_ptr) amg_dev_free(H, P.blk_ptr);
+    if (P.tiles) amg_dev_free(H, P.tiles);
+    P.blk_ptr = nullptr, P.tiles = nullptr, P.nblk = 0;
+  }
   return AMG_OK;
 }
 
@@ -1094,81 +1337,15 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
       k_gather_double<<<grid_for(L.n), TPB, 0, st>>>(L.n, N.dinv, L.inv, L.dinv);
     }
     AMG_CUDA_TRY(H, cudaGetLastError());
-    // row-tile partition by stage bytes, then the tile packer.  The byte model of the partition is
-    // approximate (the halo of a tile is only known once it is cut), so the target is rescaled
-    // until every tile fits a ring stage.
-    double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
     L.fast = 0;
     if (!o.force_generic && L.n > 0) {
-      const int64_t total_w = RT_NNZ_WEIGHT * (int64_t)L.nnz + (int64_t)RT_ROW_WEIGHT * L.n;
-      double scale = 1.0;
-      for (int attempt = 0; attempt < 6 && !L.fast; ++attempt) {
-        const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
-        if (target < 512) break;
-        if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
-        if (L.tiles) amg_dev_free(H, L.tiles);
-        L.blk_ptr = nullptr, L.tiles = nullptr;
-        L.nblk = div_up(total_w, target);
-        int *size16, *off16, *nh, *hoff, *info;
-        AMG_ALLOC(H, L.blk_ptr, int, L.nblk + 1, st);
-        AMG_ALLOC(H, L.tiles, TileDesc, L.nblk, st);
-        AMG_ALLOC(H, size16, int, L.nblk + 1, st);
-        AMG_ALLOC(H, off16, int, L.nblk + 1, st);
-        AMG_ALLOC(H, nh, int, L.nblk + 1, st);
-        AMG_ALLOC(H, hoff, int, L.nblk + 1, st);
-        AMG_ALLOC(H, info, int, 4, st);
-        AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 4 * sizeof(int), st));
-        k_blk_partition<<<grid_for(L.nblk + 1), TPB, 0, st>>>(L.nblk, target, q < Lc ? L.nc : L.n,
-                                                             q < Lc ? L.agg_ptr : nullptr, L.rowptr, L.n, L.blk_ptr);
-        k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr,
-                                                   0, nullptr, nullptr, size16, nh, info, L.tiles, nullptr, nullptr,
-                                                   nullptr);
-        AMG_CUDA_TRY(H, cudaGetLastError());
-        int h_info[4];
-        AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
-        AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-        if (h_info[1]) {
-          scale *= 0.5;
-        } else if (h_info[0] > RT_STAGE_BYTES || h_info[2] > RT_XSLOT_BYTES) {
-          const double f1 = (double)RT_STAGE_BYTES / (double)h_info[0], f2 = (double)RT_XSLOT_BYTES / (double)h_info[2];
-          scale *= 0.96 * (f1 < f2 ? f1 : f2);
-        } else {
-          AMG_TRY(amg_exclusive_scan(H, size16, off16, L.nblk, st));
-          AMG_TRY(amg_exclusive_scan(H, nh, hoff, L.nblk, st));
-          int total16 = 0, total_h = 0;
-          AMG_TRY(read_int(H, off16 + L.nblk, &total16, st));
-          AMG_TRY(read_int(H, hoff + L.nblk, &total_h, st));
-          L.blob_bytes = (size_t)total16 * 16u;
-          L.blob = (unsigned char*)amg_dev_alloc(H, L.blob_bytes + 16, st);
-          if (!L.blob) {
-            H->err = "device allocation failed: tile blobs";
-            return AMG_ERR_OOM;
-          }
-          AMG_ALLOC(H, L.halo_idx, int, total_h + 4, st);
-          AMG_ALLOC(H, L.halo_cagg, int, total_h + 4, st);
-          k_pack_tiles<<<L.nblk, PK_THREADS, 0, st>>>(L.nblk, L.blk_ptr, L.rowptr, L.col, L.val,
-                                                     q < Lc ? L.agg : nullptr, 1, off16, hoff, size16, nh, info, L.tiles,
-                                                     L.blob, L.halo_idx, L.halo_cagg);
-          AMG_CUDA_TRY(H, cudaGetLastError());
-          AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-          L.fast = 1;
-          if (getenv("AMG_DEBUG_TILES"))
-            fprintf(stderr, "level %d: n %d nnz %d tiles %d (%.0f rows, %.0f halo per tile) blob %.1f MB stage need %d / %d, x slot need %d / %d, attempt %d\n",
-                    q, L.n, L.nnz, L.nblk, (double)L.n / L.nblk, (double)total_h / L.nblk, L.blob_bytes / 1e6, h_info[0],
-                    RT_STAGE_BYTES, h_info[2], RT_XSLOT_BYTES, attempt);
-        }
-        amg_dev_free(H, size16);
-        amg_dev_free(H, off16);
-        amg_dev_free(H, nh);
-        amg_dev_free(H, hoff);
-        amg_dev_free(H, info);
-      }
-      if (!L.fast) {
-        if (L.blk_ptr) amg_dev_free(H, L.blk_ptr);
-        if (L.tiles) amg_dev_free(H, L.tiles);
-        L.blk_ptr = nullptr, L.tiles = nullptr, L.nblk = 0;
-      }
+      TilePack P;
+      AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
+                         q < Lc ? L.nc : 0, P, st));
+      L.blk_ptr = P.blk_ptr, L.tiles = P.tiles, L.blob = P.blob, L.halo_idx = P.halo_idx, L.halo_cagg = P.halo_cagg;
+      L.blob_bytes = P.blob_bytes, L.nblk = P.nblk, L.fast = P.fast;
     }
+    const double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
     L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));
     size_t mat_bytes = (size_t)L.nnz * 12 + (size_t)L.n * 4;
     L.stream_hint = (H->l2_bytes > 0 && mat_bytes > H->l2_bytes / 2) ? 1 : 0;
@@ -1185,23 +1362,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
   {
     Level& L = H->lv[Lc];
     H->nL = L.n;
-    AMG_ALLOC(H, H->lu, double, (size_t)L.n * L.n, st);
-    AMG_ALLOC(H, H->piv, int, L.n, st);
-    AMG_CUDA_TRY(H, cudaMemsetAsync(H->lu, 0, sizeof(double) * (size_t)L.n * L.n, st));
-    k_csr_to_dense<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, H->lu);
-    int* info;
-    AMG_ALLOC(H, info, int, 1, st);
-    AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, sizeof(int), st));
-    int T = L.n <= 64 ? 256 : 1024;
-    k_dense_lu<<<1, T, 0, st>>>(L.n, H->lu, H->piv, info);
-    AMG_CUDA_TRY(H, cudaGetLastError());
-    int h_info = 0;
-    AMG_TRY(read_int(H, info, &h_info, st));
-    amg_dev_free(H, info);
-    if (h_info) {
-      H->err = "coarsest operator is singular";
-      return AMG_ERR_COARSE_SINGULAR;
-    }
+    AMG_TRY(dense_lu_of(H, L.n, L.rowptr, L.col, L.val, &H->lu, &H->piv, st));
   }
   H->stats.lu_ms = now_ms() - t_lu0;
 
@@ -1223,6 +1384,35 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
   H->stats.galerkin_ms = t_rap;
   H->stats.match_rounds_max = rounds_max;
   H->stats.total_ms = now_ms() - t_start;
+  return AMG_OK;
+}
+
+// NEXT-2 ("forms A^T ... then solves the adjoint system"): the
+// transposed hierarchy IS the Galerkin hierarchy of A^T on the same aggregates ((P^T A P)^T =
+// P^T A^T P), so every level operator is transposed in place (permuted numbering), tile-packed like
+// the forward one, the coarsest A_L^T factored, and the dense tail of B^T assembled.
+amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st) {
+  if (H->have_T) return AMG_OK;
+  const int Lc = (int)H->lv.size() - 1;
+  for (int q = 0; q <= Lc; ++q) {
+    Level& L = H->lv[q];
+    LevelOpT& T = L.T;
+    AMG_TRY(transpose_csr(H, L.n, L.nnz, L.nnz_alloc, L.rowptr, L.col, L.val, &T.rowptr, &T.col, &T.val, &T.src, st));
+    if (!H->opt.force_generic && L.n > 0) {
+      TilePack P;
+      AMG_TRY(pack_tiles(H, L.n, L.nnz, T.rowptr, T.col, T.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
+                         q < Lc ? L.nc : 0, P, st));
+      T.blk_ptr = P.blk_ptr, T.tiles = P.tiles, T.blob = P.blob, T.halo_idx = P.halo_idx, T.halo_cagg = P.halo_cagg;
+      T.blob_bytes = P.blob_bytes, T.nblk = P.nblk, T.fast = P.fast;
+    }
+    if (!T.fast && !L.rtmp && q < Lc) AMG_ALLOC(H, L.rtmp, double, L.n, st);
+  }
+  {
+    Level& L = H->lv[Lc];
+    AMG_TRY(dense_lu_of(H, L.n, L.T.rowptr, L.T.col, L.T.val, &H->luT, &H->pivT, st));
+  }
+  H->have_T = true;
+  AMG_TRY(amg_setup_tail(H, 1, st));
   return AMG_OK;
 }
 

@@ -13,6 +13,7 @@ namespace {
 thread_local int64_t g_nlaunch = 0;  // kernel launches enqueued by this thread (amg_get_last_launches)
 
 thread_local bool g_pdl = false;     // true while an iteration is being captured with programmatic edges
+thread_local int g_tr = 0;           // 1: the level operators are the transposed ones (A_l^T, nonsymmetric adjoint)
 
 // kernel launch; with g_pdl the kernel may become resident while its predecessor drains
 // (programmatic dependent launch: every kernel of the solve calls griddepcontrol.wait first)
@@ -52,21 +53,19 @@ inline int red_grid(const amg_handle_s* H, int n) {
 }
 
 // ---- dispatch of the row kernels ---------------------------------------------------------
+inline int lv_fast(const Level& L) { return g_tr ? L.T.fast : L.fast; }
+inline int lv_nblk(const Level& L) { return g_tr ? L.T.nblk : L.nblk; }
+
 template <int OP, int NDOT, bool STREAM>
 void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
-  static bool attr_set = false;  // opt in to > 48 KB of dynamic shared memory, once per instantiation
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_rowtile<OP, NDOT, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
-    attr_set = true;
-  }
   int grid = H->sm_count * RT_CTAS;
-  if (grid > L.nblk) grid = L.nblk;
+  if (grid > lv_nblk(L)) grid = lv_nblk(L);
   ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM>, grid, RT_THREADS, rt::SMEM_BYTES, st)(a);
 }
 
 template <int OP, int NDOT>
 void launch_row(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
-  if (L.fast) {
+  if (lv_fast(L)) {
     if (L.stream_hint)
       launch_tile<OP, NDOT, true>(H, L, a, st);
     else
@@ -85,21 +84,28 @@ void launch_row(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStr
   }
 }
 
+template <int OP, int NDOT>
+void set_tile_attr() {
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
+}
+
 RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
   RowArgs a;
   memset(&a, 0, sizeof(a));
   a.n = L.n;
-  a.rowptr = L.rowptr;
-  a.col = L.col;
-  a.val = L.val;
-  a.tiles = L.tiles;
-  a.ntiles = L.nblk;
+  if (g_tr) {
+    a.rowptr = L.T.rowptr, a.col = L.T.col, a.val = L.T.val;
+    a.tiles = L.T.tiles, a.ntiles = L.T.nblk, a.blob = L.T.blob;
+    a.halo_idx = L.T.halo_idx, a.halo_cagg = L.T.halo_cagg;
+  } else {
+    a.rowptr = L.rowptr, a.col = L.col, a.val = L.val;
+    a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob;
+    a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
+  }
   a.dinv = L.dinv;
   a.agg = L.agg;
   a.agg_ptr = L.agg_ptr;
-  a.blob = L.blob;
-  a.halo_idx = L.halo_idx;
-  a.halo_cagg = L.halo_cagg;
   a.gamma = H->opt.coarse_scale;
   a.partials = H->partials;
   a.counter = H->counter;
@@ -165,7 +171,7 @@ void op_residual_restrict(amg_handle_s* H, const Level& L, const double* b, cons
   RowArgs a = base_args(H, L, ctl);
   a.x = x;
   a.b = b;
-  if (L.fast) {
+  if (lv_fast(L)) {
     a.out = rc;
     a.dinv_c = x1c ? dinv_c : nullptr;
     a.out2 = dinv_c ? x1c : nullptr;
@@ -184,83 +190,55 @@ void op_coarse_solve(amg_handle_s* H, const double* b, double* x, KrylovCtl* ctl
   const int n = H->nL;
   if (n <= LU_SMALL_MAX) {
     const size_t sm = sizeof(double) * ((size_t)n * (n + 1) + n);
-    ++g_nlaunch, launch(k_lu_solve_small, 1, 256, sm, st)(n, H->lu, H->piv, b, x, ctl);
+    ++g_nlaunch, launch(k_lu_solve_small, 1, 256, sm, st)(n, g_tr ? H->luT : H->lu, g_tr ? H->pivT : H->piv, b, x, ctl);
     return;
   }
   int T = n <= 32 ? 32 : (n <= 64 ? 64 : (n <= 256 ? 256 : 1024));
-  ++g_nlaunch, launch(k_lu_solve, 1, T, sizeof(double) * n, st)(n, H->lu, H->piv, b, x, ctl);
+  ++g_nlaunch, launch(k_lu_solve, 1, T, sizeof(double) * n, st)(n, g_tr ? H->luT : H->lu, g_tr ? H->pivT : H->piv, b, x, ctl);
 }
 
-// levels l..coarsest in one persistent kernel (amg_tail.cuh); returns the result buffer of level l
-double* op_tail(amg_handle_s* H, int l, const double* b, KrylovCtl* ctl, int fin, cudaStream_t st) {
-  const int Lc = (int)H->lv.size() - 1;
+// V-cycle from level D down as the dense collapsed operator (amg_tail.cuh); returns the result buffer
+double* op_tail(amg_handle_s* H, const double* b, double* out, KrylovCtl* ctl, int fin, cudaStream_t st) {
+  Level& L = H->lv[H->tail_dense_level];
+  if (!out) out = L.x;
   TailArgs a;
   memset(&a, 0, sizeof(a));
-  a.lv = (const TailLevel*)H->d_tail;
-  a.chunk = (const TailChunk*)H->d_tail_chunk;
-  a.first = l;
-  a.last = Lc;
-  a.b_first = b;
-  a.nu1 = H->opt.pre_sweeps;
-  a.nu2 = H->opt.post_sweeps;
-  a.gamma = H->opt.coarse_scale;
-  a.nL = H->nL;
-  a.lu = H->lu;
-  a.piv = H->piv;
-  a.dense_level = H->tail_dense_level;
-  a.dense_B = H->tail_dense_B;
-  a.bar = H->tail_bar;
+  a.n = L.n;
+  a.dense_B = g_tr ? H->tail_dense_BT : H->tail_dense_B;
+  a.b = b;
+  a.z = out;
   a.partials = H->partials;
+  a.counter = H->counter;
   a.ctl = ctl;
   a.fin = fin;
-  a.lu_smem = H->tail_lu_smem;
-#ifdef AMG_TAIL_PROFILE
-  static unsigned long long* d_prof = nullptr;
-  if (!d_prof) cudaMalloc(&d_prof, 256 * sizeof(unsigned long long));
-  cudaMemsetAsync(d_prof, 0, 256 * sizeof(unsigned long long), st);
-  a.prof = d_prof;
-#endif
-  ++g_nlaunch, launch(k_vcycle_tail, H->tail_grid, TAIL_THREADS, H->tail_smem, st)(a);
-#ifdef AMG_TAIL_PROFILE
-  if (getenv("AMG_TAIL_PROF")) {
-    unsigned long long hp[256];
-    cudaMemcpyAsync(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost, st);
-    cudaStreamSynchronize(st);
-    fprintf(stderr, "tail first=%d:", l);
-    for (int q = 1; q < 256 && hp[q]; ++q) fprintf(stderr, " %llu", hp[q] - hp[q - 1]);
-    fprintf(stderr, "\n");
-  }
-#endif
-  Level& L = H->lv[l];
-  const bool dense = H->tail_dense_level >= 0 && l <= H->tail_dense_level;
-  if (l == (dense ? H->tail_dense_level : Lc)) return L.x;
-  return tail_result_in_x2(a.nu1, a.nu2) ? L.x2 : L.x;
+  ++g_nlaunch, launch(k_dense_tail, H->tail_grid, TAIL_THREADS, 0, st)(a);
+  return out;
 }
 
 }  // namespace
 
-amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
-  H->tail_first = -1;
-  H->tail_dense_level = -1;
+// Dense collapsed operator of the coarse tail: column j = V-cycle of levels D.. on e_j
+// (transposed = 1: the same for the transposed hierarchy, after the forward one)
+amg_status amg_setup_tail(amg_handle_s* H, int transposed, cudaStream_t st) {
+  if (!transposed) H->tail_dense_level = -1;
   const int nlev = (int)H->lv.size();
   const int Lc = nlev - 1;
-  if (H->opt.tail_max_rows <= 0 || H->opt.force_generic || nlev > TAIL_MAX_LEVELS) return AMG_OK;
-  int first = nlev;
-  while (first > 0 && H->lv[first - 1].n <= H->opt.tail_max_rows) --first;
-  if (first >= nlev) return AMG_OK;
-  const int G = H->sm_count;  // one resident CTA per SM: the grid barrier needs co-residency
-  // the dense collapsed operator replaces the levels from D down
+  if (H->opt.tail_dense_rows <= 0 || H->opt.force_generic || nlev > TAIL_MAX_LEVELS) return AMG_OK;
   int D = -1;
-  if (H->opt.tail_dense_rows > 0)
-    for (int l = first; l < nlev; ++l)
-      if (H->lv[l].n <= H->opt.tail_dense_rows && H->lv[l].n <= MAX_DENSE) {
-        D = l;
-        break;
-      }
-  // ---- per level: row chunks of the CTAs (aggregate boundaries, balanced by nonzeros) ----
+  for (int l = 0; l < nlev; ++l)
+    if (H->lv[l].n <= H->opt.tail_dense_rows && H->lv[l].n <= MAX_DENSE) {
+      D = l;
+      break;
+    }
+  if (D < 0) return AMG_OK;
+  const int nD = H->lv[D].n;
+  const size_t lu_smem = (tail_smem_bytes(H->nL) + 127) & ~(size_t)127;
+  size_t vec_bytes = 0;
+  for (int l = D; l < nlev; ++l) vec_bytes += 3 * sizeof(double) * (size_t)H->lv[l].n;
+  const size_t smem = lu_smem + vec_bytes;
+  if (smem > 200 * 1024) return AMG_OK;
+  if (transposed && H->tail_dense_level != D) return AMG_OK;  // no forward operator: levels are visited
   std::vector<TailLevel> h(nlev);
-  std::vector<TailChunk> hc((size_t)nlev * G);
-  memset(hc.data(), 0, sizeof(TailChunk) * hc.size());
   for (int l = 0; l < nlev; ++l) {
     const Level& L = H->lv[l];
     TailLevel& T = h[l];
@@ -269,98 +247,37 @@ amg_status amg_setup_tail(amg_handle_s* H, cudaStream_t st) {
     T.nnz = L.nnz;
     const double mean = L.n > 0 ? (double)L.nnz / L.n : 1.0;
     T.lpr = mean <= 6.0 ? 4 : (mean <= 24.0 ? 8 : 16);
-    T.rowptr = L.rowptr;
-    T.col = L.col;
-    T.val = L.val;
+    T.rowptr = transposed ? L.T.rowptr : L.rowptr;
+    T.col = transposed ? L.T.col : L.col;
+    T.val = transposed ? L.T.val : L.val;
     T.dinv = L.dinv;
     T.agg = L.agg;
     T.agg_ptr = L.agg_ptr;
-    T.b = L.b;
-    T.x = L.x;
-    T.x2 = L.x2;
-    T.s_rp = T.s_col = T.s_val = T.s_dinv = -1;
   }
-  H->tail_lu_smem = (int)((tail_smem_bytes(H->nL) + 127) & ~(size_t)127);
-  int stage_used = 0;
-  std::vector<int> rp, ap;
-  for (int l = first; l < Lc; ++l) {
-    const Level& L = H->lv[l];
-    rp.resize(L.n + 1);
-    ap.resize(L.nc + 1);
-    AMG_CUDA_TRY(H, cudaMemcpyAsync(rp.data(), L.rowptr, sizeof(int) * (L.n + 1), cudaMemcpyDeviceToHost, st));
-    AMG_CUDA_TRY(H, cudaMemcpyAsync(ap.data(), L.agg_ptr, sizeof(int) * (L.nc + 1), cudaMemcpyDeviceToHost, st));
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-    int I = 0;
-    int m_rp = 0, m_k4 = 0, m_k2 = 0, m_r2 = 0;
-    for (int c = 0; c < G; ++c) {
-      TailChunk& ch = hc[(size_t)l * G + c];
-      const int64_t want_end = (int64_t)(c + 1) * L.nnz / G;
-      ch.A0 = I;
-      while (I < L.nc && (c == G - 1 || rp[ap[I]] < want_end)) ++I;
-      ch.A1 = I;
-      ch.R0 = ap[ch.A0];
-      ch.R1 = ap[ch.A1];
-      ch.K0 = rp[ch.R0];
-      ch.K1 = rp[ch.R1];
-      const TailSlices s = tail_slices(ch);
-      m_rp = std::max(m_rp, s.nrp), m_k4 = std::max(m_k4, s.nk4), m_k2 = std::max(m_k2, s.nk2), m_r2 = std::max(m_r2, s.nr2);
-    }
-    // staging offsets (the same in every CTA); levels the dense operator replaces are only staged
-    // for calls that start below it, which are hooks: not worth shared memory
-    const int need = 4 * m_rp + 4 * m_k4 + 8 * m_k2 + 8 * m_r2 + 64;
-    if ((D < 0 || l < D) && stage_used + need <= TAIL_STAGE_BUDGET) {
-      TailLevel& T = h[l];
-      int o = stage_used;
-      T.s_val = o, o += 8 * m_k2;
-      T.s_dinv = o, o += 8 * m_r2;
-      T.s_rp = o, o += 4 * m_rp;
-      T.s_col = o, o += 4 * m_k4;
-      stage_used = (o + 15) & ~15;
-    }
-  }
-  H->tail_smem = H->tail_lu_smem + stage_used;
   TailLevel* d;
-  TailChunk* dc;
   AMG_ALLOC(H, d, TailLevel, nlev, st);
-  AMG_ALLOC(H, dc, TailChunk, hc.size(), st);
   AMG_CUDA_TRY(H, cudaMemcpyAsync(d, h.data(), sizeof(TailLevel) * nlev, cudaMemcpyHostToDevice, st));
-  AMG_CUDA_TRY(H, cudaMemcpyAsync(dc, hc.data(), sizeof(TailChunk) * hc.size(), cudaMemcpyHostToDevice, st));
-  AMG_ALLOC(H, H->tail_bar, unsigned long long, G + 64, st);
-  AMG_CUDA_TRY(H, cudaMemsetAsync(H->tail_bar, 0, sizeof(unsigned long long) * (G + 64), st));
-  // the attribute is per function, not per handle: opt in to the most any handle can ask for
-  AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_vcycle_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-  H->d_tail = d;
-  H->d_tail_chunk = dc;
-  H->tail_grid = G;
-  // ---- dense collapsed operator: column j = V-cycle of levels D.. on e_j ----
-  if (D >= 0) {
-    const int nD = H->lv[D].n;
-    size_t vec_bytes = 0;
-    for (int l = D; l < nlev; ++l) vec_bytes += 3 * sizeof(double) * (size_t)H->lv[l].n;
-    const size_t smem = (size_t)H->tail_lu_smem + vec_bytes;
-    if (smem <= 200 * 1024) {
-      AMG_ALLOC(H, H->tail_dense_B, double, (size_t)nD * nD, st);
-      TailBuildArgs ba;
-      memset(&ba, 0, sizeof(ba));
-      ba.lv = d;
-      ba.D = D;
-      ba.last = Lc;
-      ba.nu1 = H->opt.pre_sweeps;
-      ba.nu2 = H->opt.post_sweeps;
-      ba.gamma = H->opt.coarse_scale;
-      ba.nL = H->nL;
-      ba.lu = H->lu;
-      ba.piv = H->piv;
-      ba.B = H->tail_dense_B;
-      ba.lu_smem = H->tail_lu_smem;
-      AMG_CUDA_TRY(H, cudaFuncSetAttribute(k_tail_dense_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-      launch(k_tail_dense_build, nD, TAILB_THREADS, smem, st)(ba);
-      AMG_CUDA_TRY(H, cudaGetLastError());
-      H->tail_dense_level = D;
-    }
-  }
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));  // h / hc go out of scope
-  H->tail_first = first;
+  double*& Bd = transposed ? H->tail_dense_BT : H->tail_dense_B;
+  if (!Bd) AMG_ALLOC(H, Bd, double, (size_t)nD * nD, st);
+  TailBuildArgs ba;
+  memset(&ba, 0, sizeof(ba));
+  ba.lv = d;
+  ba.D = D;
+  ba.last = Lc;
+  ba.nu1 = H->opt.pre_sweeps;
+  ba.nu2 = H->opt.post_sweeps;
+  ba.gamma = H->opt.coarse_scale;
+  ba.nL = H->nL;
+  ba.lu = transposed ? H->luT : H->lu;
+  ba.piv = transposed ? H->pivT : H->piv;
+  ba.B = Bd;
+  ba.lu_smem = (int)lu_smem;
+  launch(k_tail_dense_build, nD, TAILB_THREADS, smem, st)(ba);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));  // h goes out of scope
+  amg_dev_free(H, d);
+  H->tail_dense_level = D;
+  H->tail_grid = H->sm_count;
   return AMG_OK;
 }
 
@@ -372,16 +289,20 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
                       cudaStream_t st, bool x1_ready) {
   const int Lc = (int)H->lv.size() - 1;
   Level& L = H->lv[l];
-  if (H->tail_first >= 0 && l >= H->tail_first) {
-    *x_out = op_tail(H, l, b, ctl, (fuse_rz && l == 0) ? FIN_RZ : FIN_NONE, st);
+  // the caller may ask for the result of a level-0 cycle in a buffer of its own (BiCGSTAB keeps phat
+  // across the second V-cycle of an iteration: no copy)
+  double* const fo = (l == 0) ? H->vcycle_final_out : nullptr;
+  if (l == H->tail_dense_level) {
+    *x_out = op_tail(H, b, fo, ctl, (fuse_rz && l == 0) ? FIN_RZ : FIN_NONE, st);
     AMG_CUDA_TRY(H, cudaGetLastError());
     return AMG_OK;
   }
   if (l == Lc) {
-    op_coarse_solve(H, b, L.x, ctl, st);
-    *x_out = L.x;
+    double* out = fo ? fo : L.x;
+    op_coarse_solve(H, b, out, ctl, st);
+    *x_out = out;
     if (fuse_rz && l == 0)
-      ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, L.x, H->partials, H->counter, ctl, FIN_RZ);
+      ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, out, H->partials, H->counter, ctl, FIN_RZ);
     AMG_CUDA_TRY(H, cudaGetLastError());
     return AMG_OK;
   }
@@ -409,26 +330,28 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
   }
   Level& C = H->lv[l + 1];
   // the coarse level starts with two sweeps from zero on the row-tile path: hand it its first one
-  const bool give_x1 = L.fast && C.fast && nu1 >= 2 && l + 1 < Lc && !(H->tail_first >= 0 && l + 1 >= H->tail_first);
+  const bool give_x1 = lv_fast(L) && lv_fast(C) && nu1 >= 2 && l + 1 < Lc && l + 1 != H->tail_dense_level;
   op_residual_restrict(H, L, b, cur, C.b, ctl, st, give_x1 ? C.dinv : nullptr, give_x1 ? C.x2 : nullptr);
   double* ec = nullptr;
   AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st, give_x1));
   const bool want_dot = fuse_rz && l == 0;
   if (nu2 >= 1) {
-    if (L.fast && L.n >= H->opt.split_prolong_rows && H->opt.split_prolong_rows > 0) {
+    double* out = (fo && nu2 == 1) ? fo : oth;
+    if (lv_fast(L) && L.n >= H->opt.split_prolong_rows && H->opt.split_prolong_rows > 0) {
       // Two scattered loads per halo column make the fused sweep L1-bound on the largest levels
       // (level 0 of cfg 3: 53 us against 33 us for a plain sweep); there a separate unit-stride
       // correction pass (8 us) followed by the plain sweep is cheaper.
       ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, cur, ctl);
-      op_jacobi(H, L, b, cur, oth, want_dot && nu2 == 1, ctl, st);
+      op_jacobi(H, L, b, cur, out, want_dot && nu2 == 1, ctl, st);
     } else {
-      op_jacobi_prolong(H, L, b, cur, ec, oth, want_dot && nu2 == 1, ctl, st);
+      op_jacobi_prolong(H, L, b, cur, ec, out, want_dot && nu2 == 1, ctl, st);
     }
-    std::swap(cur, oth);
+    if (out == oth)
+      std::swap(cur, oth);
+    else
+      cur = out;
     for (int s = 1; s < nu2; ++s) {
-      // the caller may ask for the result of a level-0 cycle in a buffer of its own (BiCGSTAB keeps phat
-      // across the second V-cycle of an iteration: no copy)
-      double* out = (l == 0 && s == nu2 - 1 && H->vcycle_final_out) ? H->vcycle_final_out : oth;
+      out = (fo && s == nu2 - 1) ? fo : oth;
       op_jacobi(H, L, b, cur, out, want_dot && s == nu2 - 1, ctl, st);
       if (out == oth)
         std::swap(cur, oth);
@@ -436,8 +359,9 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
         cur = out;
     }
   } else {
-    ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, oth, ctl);
-    std::swap(cur, oth);
+    double* out = fo ? fo : oth;
+    ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, out, ctl);
+    cur = out;
     if (want_dot) ++g_nlaunch, launch(k_dot, red_grid(H, L.n), RED_THREADS, 0, st)(L.n, b, cur, H->partials, H->counter, ctl, FIN_RZ);
   }
   *x_out = cur;
@@ -486,9 +410,7 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
     const amg_status sv = amg_vcycle(H, 0, p, &zz, H->ctl, false, st);
     H->vcycle_final_out = nullptr;
     AMG_TRY(sv);
-    // the second V-cycle of this iteration overwrites the level-0 buffers: keep phat
-    if (zz != ph) ++g_nlaunch, launch(k_copy, red_grid(H, n), RED_THREADS, 0, st)(n, zz, ph, H->ctl);
-    phat = ph;
+    phat = zz;  // == ph on every path of the cycle: the second V-cycle of this iteration may overwrite the level-0 buffers
   }
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
   ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, H->partials, H->counter, H->ctl);
@@ -514,9 +436,11 @@ amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
   return AMG_OK;
 }
 
-// krylov < 0: the start graph (slot 4)
+// krylov < 0: the start graph (slot 4); g_tr: the transposed BiCGSTAB + AMG iteration (slot 5)
+inline int graph_slot(int krylov, int precond) { return krylov < 0 ? 4 : (g_tr ? 5 : krylov * 2 + precond); }
+
 amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStream_t st, cudaGraphExec_t* out) {
-  const int slot = krylov < 0 ? 4 : krylov * 2 + precond;
+  const int slot = graph_slot(krylov, precond);
   if (H->graph_exec[slot]) {
     *out = H->graph_exec[slot];
     return AMG_OK;
@@ -561,7 +485,11 @@ void amg_destroy_graphs(amg_handle_s* H) {
 }
 
 amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, double rtol, int maxit, int krylov,
-                            int precond, amg_info* info, cudaStream_t st) {
+                            int precond, int transposed, amg_info* info, cudaStream_t st) {
+  struct TrScope {  // the enqueue helpers read g_tr
+    TrScope(int t) { g_tr = t; }
+    ~TrScope() { g_tr = 0; }
+  } tr_scope(transposed);
   Level& L0 = H->lv[0];
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4];
@@ -603,7 +531,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   for (int it = 0; it < maxit; ++it) {
     if (gexec) {
       AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
-      g_nlaunch += H->graph_launches[krylov * 2 + precond];
+      g_nlaunch += H->graph_launches[graph_slot(krylov, precond)];
     } else
       AMG_TRY(enqueue_iteration(H, krylov, precond, st));
     const int slot = it % NSLOT;
@@ -619,18 +547,29 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   const double* phat = half ? (precond ? H->kv[7] : p) : nullptr;
   ++g_nlaunch, launch(k_krylov_output, grid_for(n), TPB, 0, st)(n, x, phat, L0.inv, d_x, H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
+  H->last_launches = g_nlaunch - launches0;
+  // info == NULL: the call returns here, with the last iteration and the output kernel still in the
+  // stream (x is valid in stream order; nothing is reported)
+  if (!info) return AMG_OK;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  H->last_launches = g_nlaunch - launches0;
-  if (info) {
-    const KrylovCtl& c = H->h_ctl[4];
-    info->iterations = c.iter;
-    info->status = c.status;
-    info->b_norm = sqrt(c.bnorm2);
-    info->rel_residual = c.bnorm2 > 0.0 ? sqrt(c.rr) / sqrt(c.bnorm2) : 0.0;
-    if (c.status == AMG_MAXIT && c.iter == 0) info->rel_residual = c.bnorm2 > 0.0 ? 1.0 : 0.0;
-  }
+  const KrylovCtl& c = H->h_ctl[4];
+  info->iterations = c.iter;
+  info->status = c.status;
+  info->b_norm = sqrt(c.bnorm2);
+  info->rel_residual = c.bnorm2 > 0.0 ? sqrt(c.rr) / sqrt(c.bnorm2) : 0.0;
+  if (c.status == AMG_MAXIT && c.iter == 0) info->rel_residual = c.bnorm2 > 0.0 ? 1.0 : 0.0;
   return AMG_OK;
+}
+
+void amg_configure_kernels() {
+  // opt in to > 48 KB of dynamic shared memory: a per-device attribute of every instantiation in use
+  set_tile_attr<OP_SPMV, 0>(), set_tile_attr<OP_SPMV, 1>(), set_tile_attr<OP_SPMV, 2>();
+  set_tile_attr<OP_JACOBI, 0>(), set_tile_attr<OP_JACOBI, 1>();
+  set_tile_attr<OP_JACOBI0, 0>();
+  set_tile_attr<OP_JACOBI_PROLONG, 0>(), set_tile_attr<OP_JACOBI_PROLONG, 1>();
+  set_tile_attr<OP_RESTRICT, 0>();
+  cudaFuncSetAttribute(k_tail_dense_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -707,13 +646,34 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       for (int r = 0; r < reps; ++r) op_jacobi_prolong(H, L, t1, t0, C.x2, t2, false, nullptr, st);
       perm_out(L, t2, d_out);
     } break;
+    case 7:  // y = A_l^T x (nonsymmetric handles)
+    case 8: {  // V-cycle of the transposed hierarchy started at this level: z = B_l^T b
+      if (!H->have_T) {
+        H->err = "level op 7 / 8: the handle has no transposed hierarchy (symmetric matrix)";
+        return AMG_ERR_INVALID_ARG;
+      }
+      const double* in = op == 7 ? d_in0 : d_in1;
+      if (!in) return AMG_ERR_INVALID_ARG;
+      perm_in(L, in, t1);
+      g_tr = 1;
+      amg_status sv = AMG_OK;
+      double* z = t2;
+      for (int r = 0; r < reps && sv == AMG_OK; ++r) {
+        if (op == 7)
+          op_spmv(H, L, t1, t2, 0, nullptr, FIN_NONE, nullptr, st);
+        else
+          sv = amg_vcycle(H, level, t1, &z, nullptr, false, st);
+      }
+      g_tr = 0;
+      AMG_TRY(sv);
+      perm_out(L, z, d_out);
+    } break;
     default:
       H->err = "unknown level op";
       return AMG_ERR_INVALID_ARG;
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  H->last_launches = g_nlaunch - launches0;
+  H->last_launches = g_nlaunch - launches0;  // stream-ordered: no synchronisation
   return AMG_OK;
 }
 
@@ -725,15 +685,25 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
   const int n = (int)H->n;
   const double mean = n > 0 ? (double)H->nnz / n : 1.0;
   if (nrhs > 1) {
-    // interleave X once, then one contiguous gather of nrhs values per stored entry
-    double* XT = (double*)amg_dev_alloc(H, sizeof(double) * (size_t)n * nrhs, st);
-    if (!XT) {
-      H->err = "device allocation failed: interleaved right-hand sides";
-      return AMG_ERR_OOM;
+    // interleave X once, then one contiguous gather of nrhs values per stored entry; the scratch stays on
+    // the handle (grown on demand), so that a call allocates nothing and does not synchronise
+    const size_t need = sizeof(double) * (size_t)n * nrhs;
+    if (H->grad_xt_cap < need) {
+      if (H->grad_xt) {
+        AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+        amg_dev_free(H, H->grad_xt);
+        H->grad_xt = nullptr, H->grad_xt_cap = 0;
+      }
+      H->grad_xt = (double*)amg_dev_alloc(H, need, st);
+      if (!H->grad_xt) {
+        H->err = "device allocation failed: interleaved right-hand sides";
+        return AMG_ERR_OOM;
+      }
+      H->grad_xt_cap = need;
     }
+    double* XT = H->grad_xt;
     const size_t sm = sizeof(double) * (size_t)nrhs * (GT_ROWS + 1);
     if (sm > 48 * 1024) {
-      amg_dev_free(H, XT);
       H->err = "amg_grad_values: nrhs too large (at most 94 right-hand sides per call; accumulate over calls)";
       return AMG_ERR_UNSUPPORTED;
     }
@@ -756,8 +726,6 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
     }
 #undef AMG_GRAD_CASE
     AMG_CUDA_TRY(H, cudaGetLastError());
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-    amg_dev_free(H, XT);
     H->last_launches = 2;
     return AMG_OK;
   }
@@ -771,7 +739,6 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
                                                            d_gA, accumulate);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   H->last_launches = 1;
   return AMG_OK;
 }

@@ -95,6 +95,30 @@ def _stencil_csr(shape, k_cell=None) -> Csr:
         lo_ok.append(ok_lo)
         up_ok.append(ok_up)
 
+    return _assemble_stencil(shape, lo_coef, up_coef)
+
+
+def _assemble_stencil(shape, lo_coef, up_coef, row_scale=None) -> Csr:
+    """CSR of the (2d+1)-point operator with the given face coefficients per axis ("towards the lower
+    neighbour" / "towards the upper neighbour", full-shape arrays; a boundary face has no neighbour
+    entry but still counts in the diagonal: Dirichlet ghost).  row_scale (optional, full shape)
+    multiplies every entry of a row (e.g. 1 / cell volume: a nonsymmetric matrix)."""
+    d = len(shape)
+    n = int(np.prod(shape))
+    idx = np.arange(n, dtype=np.int64).reshape(shape)
+    strides = [int(np.prod(shape[a + 1:])) for a in range(d)]
+    lo_ok, up_ok = [], []
+    for a in range(d):
+        ok_lo = np.ones(shape, dtype=bool)
+        ok_up = np.ones(shape, dtype=bool)
+        sl_first = [slice(None)] * d
+        sl_first[a] = slice(0, 1)
+        sl_last = [slice(None)] * d
+        sl_last[a] = slice(shape[a] - 1, shape[a])
+        ok_lo[tuple(sl_first)] = False
+        ok_up[tuple(sl_last)] = False
+        lo_ok.append(ok_lo)
+        up_ok.append(ok_up)
     # slots in ascending column order: lower neighbours from the slowest axis to the fastest,
     # the diagonal, upper neighbours from the fastest axis to the slowest.
     nslot = 2 * d + 1
@@ -121,6 +145,8 @@ def _stencil_csr(shape, k_cell=None) -> Csr:
     cols[:, sd] = flat
     vals[:, sd] = diag
     mask[:, sd] = True
+    if row_scale is not None:
+        vals = vals * np.asarray(row_scale, dtype=np.float64).reshape(-1, 1)
 
     rowlen = mask.sum(axis=1)
     rowptr = np.zeros(n + 1, dtype=np.int64)
@@ -129,6 +155,44 @@ def _stencil_csr(shape, k_cell=None) -> Csr:
         raise ValueError("nnz too large for int32 indices")
     return Csr(n, rowptr.astype(np.int32), cols[mask].astype(np.int32), vals[mask],
                {"shape": shape})
+
+
+def stretched_channel_csr(shape, stretch: float = 2.0) -> Csr:
+    """Nonsymmetric "pressure-Poisson-like" system: the 7-point finite-volume Laplacian on a box grid
+    whose axis 1 (wall-normal, shape = (nz, ny, nx)) is stretched by y_j = tanh(stretch (2j/ny - 1)) /
+    tanh(stretch) (cells cluster at both walls; widths normalised to mean 1), the other axes uniform
+    with width 1, Dirichlet ghost cells on every boundary, EVERY ROW DIVIDED BY ITS CELL VOLUME:
+    A = D^-1 S with S symmetric, so a_ij != a_ji across the stretched axis while the pattern stays
+    symmetric.  Stands in for the stretched-grid channel matrix of PAPER.md:293 (100 x 260 x 256,
+    "nonsymmetric stored matrix"), which is not available.  Face coefficient = face area / distance
+    between the cell centres (boundary face: distance to the wall = half a cell)."""
+    shape = tuple(int(s) for s in shape)
+    assert len(shape) == 3
+    nz, ny, nx = shape
+    edges = np.tanh(stretch * (2.0 * np.arange(ny + 1) / ny - 1.0)) / np.tanh(stretch)
+    hy = np.diff(edges)
+    hy = hy * (ny / hy.sum())
+    widths = [np.ones(nz), hy, np.ones(nx)]
+    vol = widths[0][:, None, None] * widths[1][None, :, None] * widths[2][None, None, :]
+    lo_coef, up_coef = [], []
+    for a in range(3):
+        w = widths[a]
+        sh = [1, 1, 1]
+        sh[a] = shape[a]
+        area = vol / w.reshape(sh)                       # face area normal to axis a
+        d_lo = np.empty(shape[a])
+        d_up = np.empty(shape[a])
+        d_lo[0] = 0.5 * w[0]
+        d_lo[1:] = 0.5 * (w[:-1] + w[1:])               # the same expression on both sides of a face
+        d_up[-1] = 0.5 * w[-1]
+        d_up[:-1] = 0.5 * (w[:-1] + w[1:])
+        lo_coef.append(area / d_lo.reshape(sh))
+        up_coef.append(area / d_up.reshape(sh))
+    a_ = _assemble_stencil(shape, lo_coef, up_coef, row_scale=1.0 / vol)
+    a_.meta["stretch"] = stretch
+    a_.meta["hy_min"] = float(hy.min())
+    a_.meta["hy_max"] = float(hy.max())
+    return a_
 
 
 def poisson_csr(shape) -> Csr:

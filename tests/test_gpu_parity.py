@@ -125,26 +125,26 @@ def test_level_kernels(cases, name, generic):
         assert np.max(np.abs(y - c.o.smooth(l, b, x + ec[agg]))) <= 1e-13 * 4
 
 
-# tail_max_rows: the levels at or below this size run inside the persistent coarse-tail kernel
-# (65536: almost every level of these small cases, sparse phases + the dense collapsed operator);
-# 0 = one kernel per pass on every level; 600 = a mixed cycle; 2304 = the default
-@pytest.mark.parametrize("tail", [65536, 0, 600, 2304])
+# tail_dense_rows: the V-cycle from the first level at or below this size down is one dense operator
+# (4000: near the top of these small cases; 0 = one kernel per pass on every level + the LU solve;
+# 300 = deep down; 2304 = the default)
+@pytest.mark.parametrize("tail", [4000, 0, 300, 2304])
 @pytest.mark.parametrize("name", list(CASES))
 def test_apply_preconditioner(cases, name, tail):
-    c = cases(name, tail_max_rows=tail)
+    c = cases(name, tail_dense_rows=tail)
     r = np.random.default_rng(11).standard_normal(c.A.n)
     z = c.s.apply_preconditioner(r).cpu().numpy()
     assert rel(z, c.o.vcycle(r, 0)) <= 1e-12
 
 
 @pytest.mark.parametrize("sweeps", [(1, 1), (3, 2), (0, 1), (2, 0), (1, 3)])
-@pytest.mark.parametrize("tail", [65536, 0, 600])
+@pytest.mark.parametrize("tail", [4000, 0, 300])
 def test_vcycle_sweep_counts(cases, oracle_mod, B, sweeps, tail):
     """V(nu1, nu2) for sweep counts other than the default (2, 2), every kernel family."""
     nu1, nu2 = sweeps
     A = inputs.config_matrix(3, 20)
     o = oracle_mod.Oracle(A.rowptr, A.col, A.val, pre_sweeps=nu1, post_sweeps=nu2)
-    s = B.AmgSolver(A.rowptr, A.col, A.val, pre_sweeps=nu1, post_sweeps=nu2, tail_max_rows=tail)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, pre_sweeps=nu1, post_sweeps=nu2, tail_dense_rows=tail)
     try:
         r = np.random.default_rng(13).standard_normal(A.n)
         z = s.apply_preconditioner(r).cpu().numpy()
@@ -165,11 +165,11 @@ def test_vcycle_sweep_counts(cases, oracle_mod, B, sweeps, tail):
 # ------------------------------------------------------------------------------------------
 # S6-S9: whole solves
 # ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("graph,tail", [(1, 65536), (0, 65536), (1, 0), (1, 600)])
+@pytest.mark.parametrize("graph,tail", [(1, 2304), (0, 2304), (1, 0), (1, 300)])
 @pytest.mark.parametrize("krylov", [0, 1])
 @pytest.mark.parametrize("name", list(CASES))
 def test_solve_parity(cases, name, krylov, graph, tail):
-    c = cases(name, use_graph=graph, tail_max_rows=tail)
+    c = cases(name, use_graph=graph, tail_dense_rows=tail)
     bn = np.linalg.norm(c.b)
     # timed tolerance: residual and iteration count
     xg, ig = c.s.solve(c.b, 1e-8, 1000, krylov)
@@ -345,10 +345,9 @@ def test_options(oracle_mod, B, opts):
 
 
 @pytest.mark.parametrize("gpu_opts", [
-    dict(tail_max_rows=65536, tail_dense_rows=0),      # persistent tail, sparse phases down to the LU solve
-    dict(tail_max_rows=65536, tail_dense_rows=300),    # dense collapsed operator deep inside the tail
-    dict(tail_max_rows=65536, tail_dense_rows=4000),   # ... and near its top
-    dict(tail_max_rows=0, tail_dense_rows=0),          # no tail at all
+    dict(tail_dense_rows=0),      # every level visited, LU solve at the bottom
+    dict(tail_dense_rows=300),    # dense collapsed operator deep down
+    dict(tail_dense_rows=4000),   # ... and near the top
     dict(use_pdl=0), dict(use_graph=0, use_pdl=0),
     dict(split_prolong_rows=1),                         # coarse correction as its own pass on every level
     dict(split_prolong_rows=0),
@@ -564,13 +563,14 @@ def test_error_returns(B):
     with pytest.raises(B.AmgError) as e:
         B.AmgSolver(T.rowptr, T.col, v)
     assert e.value.status == 5
-    # nonsymmetric matrix: detected on the device, transpose solve refused (NEXT-2)
+    # nonsymmetric values: detected on the device by default (tests/test_gpu_nonsymmetric.py has the solves)
     v = A.val.copy()
     v[1] = -0.5
-    s = B.AmgSolver(A.rowptr, A.col, v, symmetric=-1)
-    with pytest.raises(B.AmgError) as e:
-        s.solve_transpose(np.ones(A.n))
-    assert e.value.status == 7
+    s = B.AmgSolver(A.rowptr, A.col, v)
+    assert s.symmetric == 0
+    s.close()
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    assert s.symmetric == 1
     s.close()
     with pytest.raises(AttributeError):
         B.amg_options_default(no_such_option=1)
