@@ -1,13 +1,18 @@
 """bench.py — AMG-PCG solve time + V-cycle HBM GB/s on the 3D 128^3 fp64 Poisson system (one B200).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--cfg 3] [--edge E]
+                    [--configs 1,2,4,5,ns | none] [--roofline-only]
 
 A "step" is one pass of the solve-phase hot path on the cached hierarchy: one AMG-PCG solve of
 A x = b from x0 = 0 to ||r|| <= 1e-8 ||b|| (BASELINE.json configs[2], the
 configuration the metric is quoted on).  The other rows of §8(a) are timed beside it in the same
 run and reported under "phases": the cold device setup (U1-U7, "timed separately and amortized
-by the cache"), one V-cycle, the BiCGSTAB solve, the adjoint solve + matrix-value gradient
-(G1-G3).  Inputs are seeded synthetic PDE matrices (paper_2606_09001_b200/inputs.py).
+by the cache"), the warm resetup, one V-cycle, the BiCGSTAB solve, the adjoint solve + matrix-value
+gradient (G1-G3).  The other BASELINE.json configurations (1, 2 with its 8 right-hand sides on one
+hierarchy, 4, 5 with its 16 + 16 solves and the fused gradient) and the nonsymmetric
+pressure-Poisson-like system of NEXT-2 are measured through the same C ABI in the same run and
+reported under "configs" (rank 0, N = 1).  Inputs are seeded synthetic PDE matrices
+(paper_2606_09001_b200/inputs.py).
 
 One JSON line on stdout (rank 0).  N > 1: "replicas only": every rank
 solves the same system on its own GPU; no data-path collective.
@@ -18,6 +23,7 @@ the same workload and metric; rank 0 only.
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import statistics
@@ -38,7 +44,12 @@ WORKLOADS = {
     2: "cfg2: 2D 5-point Poisson 1024x1024, b=A*N(0,1)",
     3: "cfg3: 3D 7-point Poisson 128^3 (N=2097152, nnz=14581760), b~U[-1,1], AMG-PCG rtol 1e-8",
     4: "cfg4: 3D 7-point variable-coefficient diffusion 192^3, randomly permuted rows, b~U[-1,1]",
+    5: "cfg5: differentiable solve on the cfg4 system, 16 right-hand sides forward + 16 adjoint + gradient",
 }
+# NEXT-2: nonsymmetric pressure-Poisson-like system, the size of the paper's channel grid
+NONSYM_SHAPE = (100, 260, 256)
+# ncu capture of the roofline rep loop (profiles/r02_roofline.md names the command that wrote it)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_level0_sweep_dram.csv")
 
 
 def parse_args():
@@ -49,11 +60,42 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--edge", type=int, default=None, help="grid edge (default: the config's full size)")
+    ap.add_argument("--configs", default="1,2,4,5,ns",
+                    help="other configurations measured beside the headline one (rank 0, N = 1); 'none' skips them")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-phases", action="store_true", help="skip the setup / BiCGSTAB / adjoint extras")
-    ap.add_argument("--ncu-window", action="store_true",
-                    help="bracket the first timed step with cudaProfilerStart/Stop (ncu --profile-from-start off)")
+    ap.add_argument("--roofline-only", action="store_true",
+                    help="setup + the level-0 sweep rep loop of the roofline leg only (the command ncu captures)")
     return ap.parse_args()
+
+
+def config_dict(cfg, edge, n, nnz):
+    """The workload description, identical for both arms of the bench."""
+    return {"workload": WORKLOADS.get(cfg, str(cfg)) + (f" [edge {edge}]" if edge else ""), "n": n, "nnz": nnz,
+            "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi"}
+
+
+def roofline_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the level-0 sweep, averaged over the launches of
+    the committed ncu capture of `bench.py --roofline-only` (None if there is no capture)."""
+    try:
+        rows = list(csv.reader(open(TRAFFIC_CSV)))
+    except OSError:
+        return None
+    hdr = next((r for r in rows if "Kernel Name" in r), None)
+    if hdr is None:
+        return None
+    ik, im, iv, iu = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value"), hdr.index("Metric Unit")
+    per = {}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for r in rows[rows.index(hdr) + 1:]:
+        if len(r) <= iv or "k_rowtile" not in r[ik] or not r[im].startswith("dram__bytes_"):
+            continue
+        per.setdefault(r[0], 0.0)
+        per[r[0]] += float(r[iv].replace(",", "")) * scale.get(r[iu], 1.0)
+    if not per:
+        return None
+    return sum(per.values()) / len(per)
 
 
 def peaks():
@@ -163,6 +205,166 @@ def oracle_run(A, b, threads, maxit=MAXIT):
     return t_setup, t_solve, info, used
 
 
+def extra_configs(which, B, inputs, dev, peak):
+    """The other BASELINE.json configurations + the nonsymmetric system, through the C ABI (rank 0, N = 1).
+    Device times with CUDA events, 1 warm-up + best of 3; residuals recomputed on the host in fp64."""
+    import numpy as np
+    import torch
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, reps=3, warm=1):
+        out = None
+        for _ in range(warm):
+            out = fn()
+        ts = []
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record()
+            out = fn()
+            b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return min(ts), out
+
+    def setup(A, **opts):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **opts)
+        torch.cuda.synchronize()
+        first = (time.perf_counter() - t0) * 1e3
+        ts = []
+        for _ in range(2):  # device setup alone: the CSR is already resident, the pool is warm
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            h2 = B.amg_setup(s.n, s.nnz, s.d_rowptr, s.d_col, s.d_val, s.opt)
+            torch.cuda.synchronize()
+            ts.append((time.perf_counter() - t0) * 1e3)
+            B.amg_destroy(h2)
+        return s, round(first, 1), round(min(ts), 2)
+
+    def solve_phase(s, ms, its, krylov=0):
+        by = B.amg_get_algorithmic_bytes(s.h, 3 if krylov else 2) * its
+        gbs = by / (ms * 1e-3) / 1e9
+        return {"algorithmic_gb": round(by / 1e9, 2), "achieved_gbs": round(gbs, 1), "frac": round(gbs / peak, 4)}
+
+    def hres(Asp, b, x):
+        return float(np.linalg.norm(b - Asp @ x) / np.linalg.norm(b))
+
+    out = {}
+    if "1" in which:
+        A = inputs.config_matrix(1)
+        b = inputs.config_rhs(1, A.n)
+        s, first, sms = setup(A)
+        db, dx = torch.as_tensor(b).to(dev), torch.empty(A.n, dtype=torch.float64, device=dev)
+        ms, info = timed(lambda: B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1), reps=5)
+        out["cfg1"] = {"workload": WORKLOADS[1], "n": A.n, "nnz": A.nnz, "levels": s.num_levels, "setup_ms": sms,
+                       "solve_ms": round(ms, 4), "iterations": info.iterations,
+                       "true_rel_residual_host_fp64": hres(A.to_scipy(), b, dx.cpu().numpy()),
+                       "note": "0.26 MB working set: launch/latency bound, time only"}
+        s.close()
+    if "2" in which:
+        A = inputs.config_matrix(2)
+        Asp = A.to_scipy()
+        Bh = np.stack([Asp @ inputs.config_rhs(2, A.n, k) for k in range(8)])
+        s, first, sms = setup(A)
+        Bd = torch.as_tensor(Bh).to(dev).contiguous()
+        X = torch.empty_like(Bd)
+        ms, infos = timed(lambda: B.amg_solve_batched(s.h, 0, Bd, X, 8, A.n, RTOL, MAXIT))
+        Xh = X.cpu().numpy()
+        its = [i.iterations for i in infos]
+        out["cfg2"] = {"workload": WORKLOADS[2] + ", 8 right-hand sides on one hierarchy (amg_solve_batched)",
+                       "n": A.n, "nnz": A.nnz, "levels": s.num_levels, "setup_ms": sms, "solve_ms_8rhs": round(ms, 3),
+                       "solve_ms_per_rhs": round(ms / 8, 3), "iterations": its,
+                       "setup_plus_8_solves_ms": round(sms + ms, 2),
+                       "true_rel_residual_host_fp64_max": max(hres(Asp, Bh[k], Xh[k]) for k in range(8)),
+                       "solve_phase": solve_phase(s, ms, sum(its)),
+                       "note": "67 MB level-0 operator: L2-resident levels, algorithmic GB/s may exceed the HBM peak"}
+        s.close()
+        del Bd, X
+    if "4" in which or "5" in which:
+        A = inputs.config_matrix(4)
+        Asp = A.to_scipy()
+        n, nnz = A.n, A.nnz
+        s, first, sms = setup(A)
+        if "4" in which:
+            b = inputs.config_rhs(4, n)
+            db, dx = torch.as_tensor(b).to(dev), torch.empty(n, dtype=torch.float64, device=dev)
+            ms, info = timed(lambda: B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1))
+            vms, _ = timed(lambda: B.amg_level_op(s.h, 0, 5, None, db, dx, 10))
+            rs = []
+            for keep in (1, 0):
+                t = []
+                for _ in range(2):
+                    torch.cuda.synchronize()
+                    t0 = time.perf_counter()
+                    B.amg_resetup_values(s.h, s.d_val, keep)
+                    torch.cuda.synchronize()
+                    t.append((time.perf_counter() - t0) * 1e3)
+                rs.append(round(min(t), 2))
+            B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1)
+            out["cfg4"] = {"workload": WORKLOADS[4], "n": n, "nnz": nnz, "levels": s.num_levels, "setup_ms": sms,
+                           "setup_first_call_ms": first, "resetup_keep_aggregates_ms": rs[0], "resetup_full_ms": rs[1],
+                           "solve_ms": round(ms, 3), "iterations": info.iterations,
+                           "true_rel_residual_host_fp64": hres(Asp, b, dx.cpu().numpy()),
+                           "solve_phase": solve_phase(s, ms, info.iterations),
+                           "vcycle_ms": round(vms / 10, 4),
+                           "vcycle_frac": round(B.amg_get_algorithmic_bytes(s.h, 1) / (vms / 10 * 1e-3) / 1e9 / peak, 4)}
+        if "5" in which:
+            R = 16
+            Bd = torch.as_tensor(np.stack([inputs.config_rhs(5, n, k) for k in range(R)])).to(dev).contiguous()
+            Td = torch.as_tensor(np.stack([inputs.config_target(n, k) for k in range(R)])).to(dev).contiguous()
+            X, Lam = torch.empty_like(Bd), torch.empty_like(Bd)
+            gA = torch.empty(nnz, dtype=torch.float64, device=dev)
+            fms, fi = timed(lambda: B.amg_solve_batched(s.h, 0, Bd, X, R, n, RTOL, MAXIT), reps=2)
+            G = (X - Td).contiguous()
+            ams, ai = timed(lambda: B.amg_solve_batched(s.h, 1, G, Lam, R, n, RTOL, MAXIT), reps=2)
+            gms, _ = timed(lambda: B.amg_grad_values(s.h, Lam, X, R, n, gA, 0), reps=5)
+            gbytes = 12.0 * nnz + 4.0 * (n + 1) + 2 * R * 8.0 * n
+            x0, l0, g0, b0 = X[0].cpu().numpy(), Lam[0].cpu().numpy(), G[0].cpu().numpy(), Bd[0].cpu().numpy()
+            out["cfg5"] = {"workload": WORKLOADS[5], "n": n, "nnz": nnz, "nrhs": R,
+                           "forward_ms_16rhs": round(fms, 2), "forward_ms_per_rhs": round(fms / R, 3),
+                           "forward_iterations": [i.iterations for i in fi],
+                           "adjoint_ms_16rhs": round(ams, 2), "adjoint_ms_per_rhs": round(ams / R, 3),
+                           "adjoint_iterations": [i.iterations for i in ai],
+                           "grad_values_ms": round(gms, 4), "grad_values_gbs": round(gbytes / gms / 1e6, 1),
+                           "grad_values_frac": round(gbytes / gms / 1e6 / peak, 4),
+                           "total_ms": round(fms + ams + gms, 2),
+                           "true_rel_residual_host_fp64_rhs0": hres(Asp, b0, x0),
+                           "adjoint_true_rel_residual_host_fp64_rhs0": hres(Asp, g0, l0),  # A = A^T bitwise here
+                           "forward_solve_phase": solve_phase(s, fms, sum(i.iterations for i in fi)),
+                           "adjoint_solve_phase": solve_phase(s, ams, sum(i.iterations for i in ai))}
+            del Bd, Td, X, Lam, gA, G
+        s.close()
+    if "ns" in which:
+        A = inputs.stretched_channel_csr(NONSYM_SHAPE, 2.0)
+        Asp = A.to_scipy()
+        n = A.n
+        s, first, sms = setup(A)
+        b = inputs.rhs_uniform(n, 6001)
+        g = inputs.rhs_uniform(n, 6002)
+        db, dg = torch.as_tensor(b).to(dev), torch.as_tensor(g).to(dev)
+        dx, dl = torch.empty_like(db), torch.empty_like(db)
+        fms, fi = timed(lambda: B.amg_solve(s.h, db, dx, RTOL, MAXIT))
+        ams, ai = timed(lambda: B.amg_solve_transpose(s.h, dg, dl, RTOL, MAXIT))
+        out["nonsymmetric"] = {
+            "workload": f"NEXT-2: 7-point Laplacian on a {NONSYM_SHAPE[0]}x{NONSYM_SHAPE[1]}x{NONSYM_SHAPE[2]} grid, wall-normal "
+                        "tanh stretching (2.0), rows divided by the cell volume (A = D^-1 S, nonsymmetric), b,g~U[-1,1]; "
+                        "BiCGSTAB + AMG forward, BiCGSTAB + B^T on A^T for the adjoint",
+            "n": n, "nnz": A.nnz, "levels": s.num_levels, "symmetric_detected": s.symmetric,
+            "setup_ms_incl_transposed_hierarchy": sms, "forward_ms": round(fms, 3), "forward_iterations": fi.iterations,
+            "adjoint_ms": round(ams, 3), "adjoint_iterations": ai.iterations,
+            "true_rel_residual_host_fp64": hres(Asp, b, dx.cpu().numpy()),
+            "adjoint_true_rel_residual_host_fp64": hres(Asp.T.tocsr(), g, dl.cpu().numpy()),
+            "forward_solve_phase": solve_phase(s, fms, fi.iterations, 1),
+            "adjoint_solve_phase": solve_phase(s, ams, ai.iterations, 1),
+            "paper_context": "PAPER.md:303 Table 3: 3.88 s per solve (JAX-AMG/AmgX, 1x RTX A6000, 6.66 M unknowns, tol 1e-5)"}
+        s.close()
+    return out
+
+
 def run_b200(args):
     import numpy as np
     import torch
@@ -208,6 +410,30 @@ def run_b200(args):
     bytes_spmv, bytes_vcycle, bytes_pcg_it, bytes_bicg_it, bytes_sweep = (B.amg_get_algorithmic_bytes(h, w) for w in range(5))
     hier_bytes = sum(12 * z + 4 * (r + 1) for r, z in levels)
 
+    # ---- dominant kernel: the level-0 smoother sweep (k_rowtile<OP_JACOBI>) --------------
+    def timed_level_op(level, op, in0, in1, out, reps):
+        c0, c1 = ev(), ev()
+        torch.cuda.synchronize()
+        c0.record()
+        B.amg_level_op(h, level, op, in0, in1, out, reps)
+        c1.record()
+        torch.cuda.synchronize()
+        return c0.elapsed_time(c1)
+
+    def per_rep_ms(level, op, in0, in1, out, r1, r2):
+        timed_level_op(level, op, in0, in1, out, r1)
+        t1 = min(timed_level_op(level, op, in0, in1, out, r1) for _ in range(3))
+        t2 = min(timed_level_op(level, op, in0, in1, out, r2) for _ in range(3))
+        return (t2 - t1) / (r2 - r1)
+
+    if args.roofline_only:  # the command the ncu capture of profiles/r02_roofline.md runs
+        tmp = torch.empty_like(d_b)
+        d_x.copy_(d_b)
+        sweep_ms = per_rep_ms(0, 1, d_x, d_b, tmp, 10, 60)
+        print(json.dumps({"roofline_only": True, "us_per_launch": round(sweep_ms * 1e3, 2), "bytes_per_launch": bytes_sweep}))
+        s.close()
+        return
+
     # ---- the timed region: K PCG solves -------------------------------------------------
     for _ in range(W):
         info = B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 0, 1)
@@ -219,14 +445,9 @@ def run_b200(args):
     launches = 0
     barrier()
     for i in range(K):
-        if args.ncu_window and i == 0:
-            torch.cuda.profiler.start()
         e0[i].record()
         info = B.amg_solve_ex(h, d_b, d_x, RTOL, MAXIT, 0, 1)
         e1[i].record()
-        if args.ncu_window and i == 0:
-            torch.cuda.synchronize()
-            torch.cuda.profiler.stop()
         launches += B.amg_get_last_launches(h)
     barrier()
     total_ms = e0[0].elapsed_time(e1[-1])
@@ -251,22 +472,6 @@ def run_b200(args):
     barrier()
     e2e_ms = max_over_ranks(a0.elapsed_time(a1) / K)
 
-    # ---- dominant kernel: the level-0 smoother sweep (k_rowtile<OP_JACOBI>) --------------
-    def timed_level_op(level, op, in0, in1, out, reps):
-        c0, c1 = ev(), ev()
-        torch.cuda.synchronize()
-        c0.record()
-        B.amg_level_op(h, level, op, in0, in1, out, reps)
-        c1.record()
-        torch.cuda.synchronize()
-        return c0.elapsed_time(c1)
-
-    def per_rep_ms(level, op, in0, in1, out, r1, r2):
-        timed_level_op(level, op, in0, in1, out, r1)
-        t1 = min(timed_level_op(level, op, in0, in1, out, r1) for _ in range(3))
-        t2 = min(timed_level_op(level, op, in0, in1, out, r2) for _ in range(3))
-        return (t2 - t1) / (r2 - r1)
-
     roof = None
     vc = None
     if nlev > 1:
@@ -276,16 +481,20 @@ def run_b200(args):
         vcycle_ms = per_rep_ms(0, 5, None, d_b, tmp, 3, 13)
         peak, peak_src = peaks()
         ach = bytes_sweep / (sweep_ms * 1e-3) / 1e9
-        # traffic: dram__bytes_read.sum + dram__bytes_write.sum of this kernel on this workload from the
-        # `ncu --set full` capture summarised in profiles/r01_final_rowtile_xslots.md (216.7 + 6.7 MB per launch)
-        traffic = 223.4e6 if (n == 2097152 and nnz == 14581760) else None
-        roof = {"bound": "hbm", "kernel": "k_rowtile<OP_JACOBI, 1> level 0 (smoother sweep fused with the residual and r.z)",
-                "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4), "traffic": traffic,
-                "traffic_source": "profiles/r01_final_rowtile_xslots.md",
-                "note": "achieved counts ALGORITHMIC (CSR-based) bytes; the tile blobs store 10 bytes per entry instead "
-                        "of 12 + row pointers, so the real traffic is smaller and frac can exceed 1",
+        # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of this kernel in the committed ncu
+        # capture of this same rep loop (`bench.py --roofline-only`, profiles/r02_roofline.md)
+        traffic = roofline_traffic() if (n == 2097152 and nnz == 14581760) else None
+        roof = {"bound": "hbm", "kernel": "k_rowtile<OP_JACOBI, 0> level 0 (smoother sweep fused with the residual)",
+                "achieved": round(ach, 1), "peak": peak, "unit": "GB/s", "frac": round(ach / peak, 4),
+                "traffic": traffic, "traffic_source": "profiles/r02_level0_sweep_dram.csv (profiles/r02_roofline.md)",
+                "traffic_gbs": round(traffic / (sweep_ms * 1e-3) / 1e9, 1) if traffic else None,
+                "traffic_frac": round(traffic / (sweep_ms * 1e-3) / 1e9 / peak, 4) if traffic else None,
+                "note": "achieved / frac count ALGORITHMIC (CSR-based) bytes: M_0 + 4 V_0; the tile blobs store 10 bytes per "
+                        "entry instead of 12 + row pointers, so the DRAM traffic is smaller (traffic_frac = traffic / time / peak)",
                 "bytes_per_launch": bytes_sweep, "us_per_launch": round(sweep_ms * 1e3, 2), "peak_source": peak_src,
-                "how": "CUDA events around 10 and 60 back-to-back launches (amg_level_op), difference / 50; operands 234 MB > L2"}
+                "how": "CUDA events around 10 and 60 back-to-back launches (amg_level_op op 1), difference / 50; the launches "
+                       "rotate over 3 sets of x, b, dinv, out (12 vectors, 201 MB) + the 146 MB operator (evict-first): no "
+                       "operand of a launch is still in the 126 MB L2 from the launch before"}
         vc = {"ms": round(vcycle_ms, 4), "bytes": bytes_vcycle, "gbs": round(bytes_vcycle / vcycle_ms / 1e6, 1),
               "frac_of_peak": round(bytes_vcycle / vcycle_ms / 1e6 / peak, 4),
               "spmv_l0_us": round(spmv_ms * 1e3, 2), "spmv_l0_gbs": round(bytes_spmv / spmv_ms / 1e6, 1)}
@@ -356,6 +565,12 @@ def run_b200(args):
         phases["match_rounds_max"] = st.match_rounds_max
         B.amg_destroy(h2)
 
+    configs = None
+    if rank == 0 and world == 1 and args.configs != "none" and args.cfg == 3 and args.edge is None:
+        s.close()  # frees the headline hierarchy first
+        s = None
+        configs = extra_configs(set(args.configs.split(",")), B, inputs, dev, peak)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
@@ -370,10 +585,9 @@ def run_b200(args):
             "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": round(ms_per_step, 4), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOADS.get(args.cfg, str(args.cfg)) + (f" [edge {args.edge}]" if args.edge else ""),
-                       "n": n, "nnz": nnz, "levels": nlev, "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": f"no flush: one iteration streams the {hier_bytes / 1e6:.0f} MB hierarchy (> 126 MB L2)"},
+            "config": config_dict(args.cfg, args.edge, n, nnz),
+            "levels": nlev, "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2": f"no flush: one iteration streams the {hier_bytes / 1e6:.0f} MB hierarchy (> 126 MB L2)",
             "iterations": iters, "rel_residual": info.rel_residual, "true_rel_residual_host_fp64": true_res,
             "status": info.status, "step_ms_median": round(statistics.median(step_ms), 4),
             "step_ms_min": round(min(step_ms), 4),
@@ -384,10 +598,11 @@ def run_b200(args):
             "solve_phase": {"algorithmic_bytes": solve_bytes, "achieved_gbs": round(solve_gbs, 1), "peak": peak,
                             "frac": round(solve_gbs / peak, 4), "frac_of_8000_nominal": round(solve_gbs / 8000.0, 4),
                             "bytes_per_iteration": bytes_pcg_it, "peak_source": peak_src},
-            "vcycle": vc, "phases": phases, "cpu_baseline": cpu, "clocks": clocks,
+            "vcycle": vc, "phases": phases, "configs": configs, "cpu_baseline": cpu, "clocks": clocks,
         }
         print(json.dumps(out), flush=True)
-    s.close()
+    if s is not None:
+        s.close()
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -432,9 +647,7 @@ def run_reference(args):
     out = {"impl": "reference", "metric": METRIC, "value": round(ms, 2), "unit": "ms", "n_gpus": args.gpus, "steps": K,
            "warmup": W, "ms_per_step": round(ms, 2), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": WORKLOADS.get(args.cfg, str(args.cfg)) + (f" [edge {args.edge}]" if args.edge else ""),
-                      "n": A.n, "nnz": A.nnz, "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi",
-                      "parallelism": "host cores (OpenMP row loops)"},
+           "config": config_dict(args.cfg, args.edge, A.n, A.nnz), "parallelism": "host cores (OpenMP row loops)",
            "iterations": full.iterations, "rel_residual": full.rel_residual,
            "cpu_baseline": {"value": round(ms, 2), "unit": "ms", "cores": used, "kind": "oracle", "sample": sample,
                             "setup_ms": round(setup_s * 1e3, 1)},

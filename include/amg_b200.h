@@ -233,7 +233,9 @@ AMG_API amg_status amg_get_last_launches(amg_handle h, int64_t* launches);
  *   op 7: y = A_l^T x   (nonsymmetric handles)    (d_in0 = x,           d_out rows(l))
  *   op 8: transposed V-cycle started at level l   (d_in1 = b,           d_out rows(l))
  * The calls are stream-ordered (no synchronisation).
- * `reps` > 1 repeats the kernel back to back (timing); results are those of one application. */
+ * `reps` > 1 repeats the kernel back to back (timing); results are those of one application.  For op 1
+ * on level 0 the repetitions rotate over three internal copies of the operands (x, b, dinv, out: 12
+ * level-0 vectors), so that no operand of a launch is still in L2 from the launch before. */
 AMG_API amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0,
                         const double* d_in1, double* d_out, int32_t reps, void* cuda_stream);
 

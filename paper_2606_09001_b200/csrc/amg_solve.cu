@@ -131,8 +131,9 @@ void op_spmv(amg_handle_s* H, const Level& L, const double* x, double* y, int nd
 }
 
 void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x, double* out, bool dot,
-               KrylovCtl* ctl, cudaStream_t st) {
+               KrylovCtl* ctl, cudaStream_t st, const double* dinv = nullptr) {
   RowArgs a = base_args(H, L, ctl);
+  if (dinv) a.dinv = dinv;  // a copy of the level's smoother diagonal (timing hook)
   a.x = x;
   a.b = b;
   a.out = out;
@@ -604,7 +605,26 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       if (!d_in0 || !d_in1) return AMG_ERR_INVALID_ARG;
       perm_in(L, d_in0, t0);
       perm_in(L, d_in1, t1);
-      for (int r = 0; r < reps; ++r) op_jacobi(H, L, t1, t0, t2, false, nullptr, st);
+      if (level == 0 && reps > 1) {
+        // timing of back-to-back sweeps: the launches rotate over three operand sets (x, b, dinv, out:
+        // 12 level-0 vectors) so that no operand of a launch can still sit in L2 from the launch before
+        double* set[3][4] = {{t0, t1, H->kv[0], t2}, {H->kv[1], H->kv[2], H->kv[3], H->kv[4]},
+                             {H->kv[5], H->kv[6], H->kv[7], H->kv[8]}};
+        const size_t bytes = sizeof(double) * (size_t)L.n;
+        for (int q = 0; q < 3; ++q) {
+          if (q > 0) {
+            AMG_CUDA_TRY(H, cudaMemcpyAsync(set[q][0], t0, bytes, cudaMemcpyDeviceToDevice, st));
+            AMG_CUDA_TRY(H, cudaMemcpyAsync(set[q][1], t1, bytes, cudaMemcpyDeviceToDevice, st));
+          }
+          AMG_CUDA_TRY(H, cudaMemcpyAsync(set[q][2], L.dinv, bytes, cudaMemcpyDeviceToDevice, st));
+        }
+        for (int r = 0; r < reps; ++r) {
+          double** q = set[(reps - 1 - r) % 3];  // the last launch works on set 0: its result goes out
+          op_jacobi(H, L, q[1], q[0], q[3], false, nullptr, st, q[2]);
+        }
+      } else {
+        for (int r = 0; r < reps; ++r) op_jacobi(H, L, t1, t0, t2, false, nullptr, st);
+      }
       perm_out(L, t2, d_out);
       break;
     case 2: {

@@ -640,56 +640,3 @@ def test_full_size_cfg3_properties(full3):
     ks = rng.integers(0, A.nnz, 2000)
     rows = np.searchsorted(A.rowptr, ks, side="right") - 1
     assert np.array_equal(gA[ks], -(ls[rows] * xs[A.col[ks]]))
-
-
-# ------------------------------------------------------------------------------------------
-# full-size cfg 4 / cfg 5 system (192^3 variable coefficients, permuted rows): the oracle needs minutes
-# there, so its results are stored (tests/golden/full_size_oracle.txt, written by
-# tests/golden/make_full_size_golden.py from the oracle alone); the residual is recomputed here
-# ------------------------------------------------------------------------------------------
-def _golden_full():
-    import os
-
-    p = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "full_size_oracle.txt")
-    g = {}
-    with open(p) as f:
-        for line in f:
-            if line.startswith("#") or not line.strip():
-                continue
-            key, name, *vals = line.split()
-            g[(key, name)] = vals
-    return g
-
-
-def test_full_size_cfg4_against_stored_oracle(B):
-    g = _golden_full()
-    A = inputs.config_matrix(4)
-    b = inputs.config_rhs(4, A.n)
-    s = B.AmgSolver(A.rowptr, A.col, A.val)
-    try:
-        assert s.num_levels == int(g[("cfg4_192", "levels")][0])
-        rows = [int(v) for v in g[("cfg4_192", "rows")]]
-        nnzs = [int(v) for v in g[("cfg4_192", "nnz")]]
-        assert [s.level_info(l) for l in range(s.num_levels)] == list(zip(rows, nnzs))  # integer work: exact
-        xg, ig = s.solve(b, 1e-8, 1000, 0)
-        assert ig.status == 0 and abs(ig.iterations - int(g[("cfg4_192", "iterations")][0])) <= 2
-        Asp = A.to_scipy()
-        xg = xg.cpu().numpy()
-        assert np.linalg.norm(b - Asp @ xg) / np.linalg.norm(b) <= 1e-8
-        # differentiable solve on the same handle (cfg 5, one right-hand side): adjoint identity g.x = lambda.b and the
-        # gradient on sampled entries recomputed from lambda, x one by one
-        xt = inputs.config_target(A.n, 0)
-        xg11, _ = s.solve(b, 1e-11, 1000, 0)
-        gvec = xg11 - torch.as_tensor(xt).cuda()
-        lam, il = s.solve_transpose(gvec, 1e-11, 1000)
-        assert il.status == 0
-        x_h, lam_h, g_h = xg11.cpu().numpy(), lam.cpu().numpy(), gvec.cpu().numpy()
-        assert abs(g_h @ x_h - lam_h @ b) <= 1e-8 * np.linalg.norm(g_h) * np.linalg.norm(x_h)
-        assert np.linalg.norm(g_h - Asp.T @ lam_h) / np.linalg.norm(g_h) <= 1e-10   # A^T lambda = g (Eq. 1)
-        gA = s.grad_values(lam, xg11).cpu().numpy()
-        ks = np.random.default_rng(8).integers(0, A.nnz, 200000)
-        rows_of = np.searchsorted(A.rowptr, ks, side="right") - 1
-        want = -lam_h[rows_of] * x_h[A.col[ks]]                                      # Eq. 2 on the pattern
-        assert np.max(np.abs(gA[ks] - want)) <= 1e-14 * np.max(np.abs(want))
-    finally:
-        s.close()
