@@ -205,6 +205,11 @@ AMG_API amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, dou
 AMG_API amg_status amg_get_num_levels(amg_handle h, int32_t* num_levels);
 AMG_API amg_status amg_get_level_info(amg_handle h, int32_t level, int64_t* rows, int64_t* nnz);
 AMG_API amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_agg_out, void* cuda_stream);
+/* Diagnostics: ||r_k||_2 / ||b||_2 for k = 1 .. iterations of the last solve on this handle
+ * that was called with info != NULL -- the value the convergence test of iteration k saw (BiCGSTAB: ||s|| of a
+ * half-step exit, else ||r||).  *count = number of entries; at most `cap` are copied to the HOST array h_out. */
+AMG_API amg_status amg_get_residual_history(amg_handle h, double* h_out, int32_t cap, int32_t* count,
+                                            void* cuda_stream);
 /* 1 / 0: what the setup decided (the caller's flag, or the result of the device check for -1). */
 AMG_API amg_status amg_get_symmetric(amg_handle h, int32_t* symmetric);
 AMG_API amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int32_t* d_col,
@@ -238,6 +243,25 @@ AMG_API amg_status amg_get_last_launches(amg_handle h, int64_t* launches);
  * level-0 vectors), so that no operand of a launch is still in L2 from the launch before. */
 AMG_API amg_status amg_level_op(amg_handle h, int32_t level, int32_t op, const double* d_in0,
                         const double* d_in1, double* d_out, int32_t reps, void* cuda_stream);
+
+/* ---- keyed LRU cache of hierarchies ("LRU cache of solver handles keyed by a hash of the
+ * sparsity pattern"; :121; :287 reuse_setup) ----
+ * amg_cache_get looks the matrix up by a 64-bit hash of (n, nnz, rowptr, col, options), computed on the device.
+ *   miss: amg_setup; the handle is inserted and the least recently used one beyond `capacity` is destroyed.
+ *   hit:  on_hit = 0 the cached handle is returned as it is (same values: reuse_setup);
+ *         on_hit = 1 amg_resetup_values(h, d_val, keep_aggregates = 0): "coefficients are updated in place and
+ *                    the setup is repeated"; on_hit = 2 the same with the aggregates kept.
+ * The handles belong to the cache (amg_cache_destroy destroys them; never call amg_destroy on one); a handle
+ * stays valid until it is evicted.  *hit (may be NULL) reports which case it was.  One call at a time per cache
+ * (an internal mutex serialises them). */
+typedef struct amg_cache_s* amg_cache;
+AMG_API amg_status amg_cache_create(amg_cache* out, int32_t capacity);
+AMG_API amg_status amg_cache_get(amg_cache c, int64_t n, int64_t nnz, const int32_t* d_rowptr, const int32_t* d_col,
+                                 const double* d_val, const amg_options* opt, int32_t on_hit, amg_handle* out,
+                                 int32_t* hit, void* cuda_stream);
+AMG_API amg_status amg_cache_stats(amg_cache c, int64_t* entries, int64_t* hits, int64_t* misses,
+                                   int64_t* evictions);
+AMG_API amg_status amg_cache_destroy(amg_cache c);
 
 /* Message of the last error on this handle; NULL handle: last failed setup on this thread. */
 AMG_API const char* amg_last_error(amg_handle h);

@@ -25,7 +25,8 @@ EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_w
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
            "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
-           "amg_get_level_path", "amg_get_symmetric", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error"]
+           "amg_get_level_path", "amg_get_symmetric", "amg_get_residual_history", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error",
+           "amg_cache_create", "amg_cache_get", "amg_cache_stats", "amg_cache_destroy"]
 
 
 class amg_options(C.Structure):
@@ -210,6 +211,19 @@ def amg_get_aggregates(h, level, d_agg_out):
     _check(load_library().amg_get_aggregates(h, C.c_int32(level), _ptr(d_agg_out, torch.int32), _stream()), h)
 
 
+def amg_get_residual_history(h):
+    """||r_k|| / ||b||, k = 1 .. iterations, of the last solve on this handle (numpy array)."""
+    import numpy as np
+
+    cnt = C.c_int32()
+    _check(load_library().amg_get_residual_history(h, None, C.c_int32(0), C.byref(cnt), _stream()), h)
+    out = np.empty(max(cnt.value, 0))
+    if cnt.value > 0:
+        _check(load_library().amg_get_residual_history(h, C.c_void_p(out.ctypes.data), C.c_int32(cnt.value),
+                                                       C.byref(cnt), _stream()), h)
+    return out
+
+
 def amg_get_symmetric(h) -> int:
     v = C.c_int32()
     _check(load_library().amg_get_symmetric(h, C.byref(v)), h)
@@ -249,6 +263,33 @@ def amg_level_op(h, level, op, d_in0, d_in1, d_out, reps=1):
     _check(load_library().amg_level_op(h, C.c_int32(level), C.c_int32(op), _ptr(d_in0, torch.float64),
                                        _ptr(d_in1, torch.float64), _ptr(d_out, torch.float64), C.c_int32(reps),
                                        _stream()), h)
+
+
+def amg_cache_create(capacity):
+    c = C.c_void_p()
+    _check(load_library().amg_cache_create(C.byref(c), C.c_int32(capacity)))
+    return c
+
+
+def amg_cache_get(c, n, nnz, d_rowptr, d_col, d_val, opt=None, on_hit=1):
+    """Returns (handle, hit).  The handle belongs to the cache."""
+    h, hit = C.c_void_p(), C.c_int32()
+    _check(load_library().amg_cache_get(c, C.c_int64(n), C.c_int64(nnz), _ptr(d_rowptr, torch.int32),
+                                        _ptr(d_col, torch.int32), _ptr(d_val, torch.float64),
+                                        C.byref(opt) if opt is not None else None, C.c_int32(on_hit), C.byref(h),
+                                        C.byref(hit), _stream()))
+    return h, hit.value
+
+
+def amg_cache_stats(c):
+    v = [C.c_int64() for _ in range(4)]
+    _check(load_library().amg_cache_stats(c, *[C.byref(x) for x in v]))
+    return dict(zip(("entries", "hits", "misses", "evictions"), (x.value for x in v)))
+
+
+def amg_cache_destroy(c):
+    if c:
+        load_library().amg_cache_destroy(c)
 
 
 # ---- small convenience wrapper (owns the handle and the device copy of the matrix) ---------
@@ -292,6 +333,9 @@ class AmgSolver:
 
     def _dev(self, a):
         return torch.as_tensor(a).to(dtype=torch.float64).to(self.device).contiguous()
+
+    def residual_history(self):
+        return amg_get_residual_history(self.h)
 
     @property
     def symmetric(self):

@@ -419,6 +419,19 @@ amg_status amg_get_last_launches(amg_handle h, int64_t* launches) {
   return AMG_OK;
 }
 
+amg_status amg_get_residual_history(amg_handle h, double* h_out, int32_t cap, int32_t* count, void* cuda_stream) {
+  if (!h || !count || cap < 0 || (cap > 0 && !h_out)) return AMG_ERR_INVALID_ARG;
+  Enter e(h, cuda_stream);
+  *count = h->hist_len;
+  const int m = h->hist_len < cap ? h->hist_len : cap;
+  if (m > 0) {
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    AMG_CUDA_TRY(h, cudaMemcpyAsync(h_out, h->hist, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(h, cudaStreamSynchronize(st));
+  }
+  return AMG_OK;
+}
+
 amg_status amg_get_symmetric(amg_handle h, int32_t* symmetric) {
   if (!h || !symmetric) return AMG_ERR_INVALID_ARG;
   *symmetric = h->symmetric;

@@ -40,7 +40,8 @@ struct KrylovCtl {
   double rr, ss, ts, tt, rv;
   double bnorm2, rtol;
   int iter, status, done, maxit;
-  int first, halfstep, pad0, pad1;
+  int first, halfstep, hist_cap, pad1;
+  double* hist;  // [hist_cap] ||r_k|| / ||b|| of iteration k = 1.. (the value its convergence test saw), or null
 };
 
 enum FinalizeId {
@@ -155,6 +156,9 @@ struct amg_handle_s {
   void* (*alloc_fn)(size_t, void*, void*) = nullptr;  // allocator captured at creation (amg_set_allocator)
   void (*free_fn)(void*, void*) = nullptr;
   void* alloc_user = nullptr;
+  double* hist = nullptr;             // residual history of the last solve (device), hist_cap entries
+  int hist_cap = 0;
+  int hist_len = 0;                   // iterations of the last solve that reported (info != NULL)
   double* grad_xt = nullptr;          // interleaved right-hand sides of amg_grad_values (grown on demand)
   size_t grad_xt_cap = 0;
   int sm_count = 148;

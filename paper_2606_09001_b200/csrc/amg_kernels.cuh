@@ -145,6 +145,7 @@ __device__ inline void krylov_finalize(KrylovCtl* c, int fin, double s0, double 
       c->iter += 1;
       c->rr = s0;
       double nr = sqrt(s0);
+      if (c->hist != nullptr && c->iter <= c->hist_cap) c->hist[c->iter - 1] = nr / sqrt(c->bnorm2);
       if (!isfinite(nr)) {
         c->status = AMG_NONFINITE;
         c->done = 1;
@@ -170,6 +171,7 @@ __device__ inline void krylov_finalize(KrylovCtl* c, int fin, double s0, double 
       c->ss = s0;
       double ns = sqrt(s0);
       if (ns <= c->rtol * sqrt(c->bnorm2)) {  // half-step exit: x += alpha * phat in the output kernel
+        if (c->hist != nullptr && c->iter <= c->hist_cap) c->hist[c->iter - 1] = ns / sqrt(c->bnorm2);
         c->rr = s0;
         c->status = AMG_CONVERGED;
         c->halfstep = 1;
@@ -184,6 +186,7 @@ __device__ inline void krylov_finalize(KrylovCtl* c, int fin, double s0, double 
     case FIN_RR_RHO: {
       c->rr = s0;
       double nr = sqrt(s0);
+      if (c->hist != nullptr && c->iter <= c->hist_cap) c->hist[c->iter - 1] = nr / sqrt(c->bnorm2);
       if (!isfinite(nr)) {
         c->status = AMG_NONFINITE;
         c->done = 1;

@@ -501,6 +501,22 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   init.rtol = rtol;
   init.maxit = maxit;
   init.status = AMG_MAXIT;
+  if (H->hist_cap < maxit) {  // residual history (PAPER.md:125 diagnostics): one entry per iteration
+    if (H->hist) {
+      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+      amg_dev_free(H, H->hist);
+    }
+    H->hist_cap = maxit < 256 ? 256 : maxit;
+    H->hist = (double*)amg_dev_alloc(H, sizeof(double) * (size_t)H->hist_cap, st);
+    if (!H->hist) {
+      H->hist_cap = 0;
+      H->err = "device allocation failed: residual history";
+      return AMG_ERR_OOM;
+    }
+  }
+  init.hist = H->hist;
+  init.hist_cap = H->hist_cap;
+  H->hist_len = 0;
   H->h_ctl[5] = init;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
   if (krylov == 0) {
@@ -555,6 +571,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   const KrylovCtl& c = H->h_ctl[4];
+  H->hist_len = c.iter < H->hist_cap ? c.iter : H->hist_cap;
   info->iterations = c.iter;
   info->status = c.status;
   info->b_norm = sqrt(c.bnorm2);

@@ -1,0 +1,135 @@
+"""GPU parity of the NEXT-4 variants: size-4 aggregation (agg_passes = 2; north_star
+"pairwise or size-4"), the residual-history diagnostics, the keyed LRU cache of
+hierarchies -- each against the oracle option of the same name, through the C ABI.
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from paper_2606_09001_b200 import inputs  # noqa: E402
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / max(np.linalg.norm(np.asarray(b)), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_09001_b200 import binding
+
+    assert torch.cuda.is_available()
+    binding.load_library()
+    return binding
+
+
+@pytest.mark.parametrize("case", [(3, 40), (4, 28), (2, 96)])
+def test_size4_aggregation_matches_the_oracle(oracle_mod, B, case):
+    cfg, edge = case
+    A = inputs.config_matrix(cfg, edge)
+    v = inputs.config_rhs(cfg, A.n)
+    b = A.to_scipy() @ v if cfg == 2 else v
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, agg_passes=2, hash_seed=4)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, agg_passes=2, hash_seed=4)
+    o1 = oracle_mod.Oracle(A.rowptr, A.col, A.val, hash_seed=4)
+    try:
+        assert s.num_levels == o.num_levels < o1.num_levels
+        for l in range(s.num_levels - 1):  # composed map of two matchings: the same integers
+            assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l)), l
+            sizes = np.bincount(o.aggregates(l))
+            assert np.median(sizes) == 4 or l >= s.num_levels - 3
+        for l in range(s.num_levels):
+            rp, cl, vl = (t.cpu().numpy() for t in s.level_csr(l))
+            orp, ocl, ovl = o.level_csr(l)
+            assert np.array_equal(rp, orp) and np.array_equal(cl, ocl)
+            assert np.max(np.abs(vl - ovl)) <= 1e-13 * np.max(np.abs(ovl))
+        r = np.random.default_rng(3).standard_normal(A.n)
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+        xg, ig = s.solve(b, 1e-8, 500, 0)
+        xo, io = o.solve(b, 1e-8, 500, 0, 1)
+        assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+        xg, _ = s.solve(b, 1e-11, 500, 0)
+        xo, _ = o.solve(b, 1e-13, 500, 0, 1)
+        assert rel(xg.cpu().numpy(), xo) <= 1e-6
+    finally:
+        s.close()
+        o.close()
+        o1.close()
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_residual_history_matches_the_oracle(oracle_mod, B, krylov):
+    A = inputs.config_matrix(3, 24)
+    b = inputs.config_rhs(3, A.n)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    try:
+        _, ig = s.solve(b, 1e-10, 200, krylov)
+        hg = s.residual_history()
+        _, io = o.solve(b, 1e-10, 200, krylov, 1)
+        ho = o.residual_history()
+        assert len(hg) == ig.iterations and hg[-1] == ig.rel_residual <= 1e-10
+        m = min(len(hg), len(ho))
+        assert abs(len(hg) - len(ho)) <= 2
+        # the same residual curve, iteration by iteration (rounding order differs: relative 1e-6 on values
+        # that fall by ten orders of magnitude)
+        assert np.max(np.abs(hg[:m] - ho[:m]) / ho[:m]) <= 1e-6
+        # the iterates do not depend on rtol: the history of a looser solve is a bitwise prefix
+        _, i6 = s.solve(b, 1e-6, 200, krylov)
+        h6 = s.residual_history()
+        assert len(h6) == i6.iterations < len(hg)
+        if krylov == 0:
+            assert np.array_equal(h6, hg[:len(h6)])
+        else:
+            assert np.array_equal(h6[:-1], hg[:len(h6) - 1])
+        # maxit stop
+        _, i3 = s.solve(b, 1e-30, 3, krylov)
+        assert i3.status == 1 and len(s.residual_history()) == 3
+    finally:
+        s.close()
+        o.close()
+
+
+def test_lru_cache_of_hierarchies(oracle_mod, B):
+    dev = torch.device("cuda:0")
+    to = lambda a, dt: torch.as_tensor(a).to(dtype=dt, device=dev).contiguous()
+    mats = [inputs.config_matrix(3, 20), inputs.config_matrix(1, 48), inputs.config_matrix(3, 24)]
+    dm = [(A.n, A.nnz, to(A.rowptr, torch.int32), to(A.col, torch.int32), to(A.val, torch.float64)) for A in mats]
+    c = B.amg_cache_create(2)
+    try:
+        h0, hit = B.amg_cache_get(c, *dm[0])
+        assert hit == 0
+        h0b, hit = B.amg_cache_get(c, *dm[0], on_hit=0)           # same pattern: the same handle, untouched
+        assert hit == 1 and h0b.value == h0.value
+        h1, hit = B.amg_cache_get(c, *dm[1])
+        assert hit == 0 and h1.value != h0.value
+        assert B.amg_cache_stats(c) == {"entries": 2, "hits": 1, "misses": 2, "evictions": 0}
+        # new values on the pattern of matrix 0 (variable coefficients on the same 20^3 stencil): a hit with a
+        # warm resetup; the solve equals the oracle built on the new values
+        A0 = mats[0]
+        Anew = inputs.variable_diffusion_csr((20, 20, 20), seed=77, sigma=1.0, ell=4.0)
+        assert np.array_equal(Anew.col, A0.col)
+        h0c, hit = B.amg_cache_get(c, A0.n, A0.nnz, dm[0][2], dm[0][3], to(Anew.val, torch.float64), on_hit=1)
+        assert hit == 1 and h0c.value == h0.value
+        b = torch.as_tensor(inputs.rhs_uniform(A0.n, 1)).to(dev)
+        x = torch.empty_like(b)
+        info = B.amg_solve(h0c, b, x, 1e-8, 500)
+        o = oracle_mod.Oracle(Anew.rowptr, Anew.col, Anew.val)
+        xo, io = o.solve(b.cpu().numpy(), 1e-8, 500, 0, 1)
+        assert info.status == 0 and abs(info.iterations - io.iterations) <= 2
+        assert np.linalg.norm(b.cpu().numpy() - Anew.to_scipy() @ x.cpu().numpy()) <= 1e-8 * torch.linalg.norm(b).item()
+        o.close()
+        # a third pattern evicts the least recently used entry (matrix 1), not matrix 0
+        h2, hit = B.amg_cache_get(c, *dm[2])
+        assert hit == 0 and B.amg_cache_stats(c)["evictions"] == 1
+        _, hit = B.amg_cache_get(c, *dm[0], on_hit=0)
+        assert hit == 1
+        _, hit = B.amg_cache_get(c, *dm[1])
+        assert hit == 0                                           # it was evicted: set up again
+        # different options on the same pattern are a different key
+        _, hit = B.amg_cache_get(c, *dm[1], opt=B.amg_options_default(pre_sweeps=1, post_sweeps=1))
+        assert hit == 0
+    finally:
+        B.amg_cache_destroy(c)
