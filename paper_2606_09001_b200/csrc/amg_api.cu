@@ -9,6 +9,8 @@
 
 namespace {
 
+constexpr int AMG_BATCH_MIN = 4;  // fewer right-hand sides than this: a loop of single solves is cheaper
+
 thread_local std::string g_thread_error;
 
 std::mutex g_alloc_mutex;  // guards the three words below (handles copy them at creation)
@@ -138,6 +140,7 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
     amg_set_thread_error(H->err.empty() ? "amg_setup failed" : H->err);
     cudaStreamSynchronize(st);
     amg_destroy_graphs(H);
+    amg_batch_release(H);
     for (auto& e : H->ev)
       if (e) cudaEventDestroy(e);
     if (H->h_ctl) cudaFreeHost(H->h_ctl);
@@ -270,6 +273,7 @@ amg_status amg_destroy(amg_handle h) {
     Enter e(h, nullptr, false);
     cudaStreamSynchronize(h->last_stream);  // the handle runs one call at a time: its last stream is enough
     amg_destroy_graphs(h);
+    amg_batch_release(h);
     for (auto& ev : h->ev)
       if (ev) cudaEventDestroy(ev);
     if (h->h_ctl) cudaFreeHost(h->h_ctl);
@@ -320,7 +324,22 @@ amg_status amg_solve_batched(amg_handle h, int32_t transpose, const double* d_B,
     h->err = "amg_solve_batched: bad argument";
     return AMG_ERR_INVALID_ARG;
   }
-  for (int32_t s = 0; s < nrhs; ++s) {
+  int32_t s0 = 0;
+  if (h->opt.krylov == 0 && h->symmetric && nrhs >= AMG_BATCH_MIN) {
+    // NEXT-3: one operator pass serves 8 right-hand sides (PCG + AMG on a symmetric handle; the transposed
+    // systems are the same systems).  Chunks of 8; a remainder of fewer than AMG_BATCH_MIN columns is looped.
+    Enter e(h, cuda_stream);
+    if (amg_batch_prepare(h, (cudaStream_t)cuda_stream)) {
+      h->last_launches = 0;
+      while (nrhs - s0 >= AMG_BATCH_MIN) {
+        const int32_t m = nrhs - s0 < 8 ? nrhs - s0 : 8;
+        AMG_TRY(amg_solve_batch_chunk(h, d_B + (size_t)s0 * ld, d_X + (size_t)s0 * ld, m, ld, rtol, maxit,
+                                      infos ? infos + s0 : nullptr, (cudaStream_t)cuda_stream));
+        s0 += m;
+      }
+    }
+  }
+  for (int32_t s = s0; s < nrhs; ++s) {
     amg_info* inf = infos ? infos + s : nullptr;
     amg_status st = transpose ? amg_solve_transpose(h, d_B + (size_t)s * ld, d_X + (size_t)s * ld, rtol, maxit, inf,
                                                     cuda_stream)

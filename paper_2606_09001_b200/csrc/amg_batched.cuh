@@ -1,0 +1,639 @@
+// Batched multi-right-hand-side solve (NEXT-3; "the matrix is shared
+// across the batch"): ONE pass over a level operator serves NB = 8 right-hand sides.  ~75 % of the
+// bytes of a single-RHS iteration are the operator stream (4 M_l of 4 M_l + 13 V_l); with 8 vectors
+// riding on one stream the per-RHS traffic drops to M/8 + vectors.
+//
+// Vectors are interleaved [row][NB] (64 contiguous bytes per row), so that the gather of a halo column
+// fetches all 8 right-hand sides as two full 32-byte sectors, and a row's operands / results are one
+// 64-byte access.  The row-tile kernel is the single-RHS one (amg_kernels.cuh) with
+//   - the same tile blobs (one bulk-async copy per tile), nothing else of the operator;
+//   - x slots [NB/2 planes][columns] of double2: the consumer's per-entry reads are NB/2 LDS.128;
+//   - 8 accumulators per row in registers; b rows are read straight from global memory before the
+//     row walk (64 B per lane, latency hidden behind the walk), results written straight to global;
+//   - one CTA per SM (the x slots are 8 x larger), 14 gather warps in two groups;
+//   - per-column Krylov scalars and convergence flags (KrylovCtlB): a converged column keeps riding
+//     with alpha = beta = 0 (its x, r stay as they are) until every column is done.
+// The fused operations with two gathers per column are split in batched mode where that is simpler:
+// the first sweep from zero (x1 = dinv o r) is emitted by the kernel that produces r (level 0) or by
+// the restriction above (other levels), as in the single-RHS path.
+#pragma once
+#include "amg_kernels.cuh"
+
+constexpr int NB = 8;        // right-hand sides per batch
+constexpr int NB2 = NB / 2;  // double2 per row
+constexpr int RTB_CONSUMERS = 256;
+constexpr int RTB_GATHERERS = 448;  // 14 warps in RTB_GGROUPS groups
+constexpr int RTB_GGROUPS = 2;
+constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
+constexpr int RTB_GU = 12;          // columns per gather thread whose indices are held in registers
+constexpr int RTB_MAXS = 4;         // most ring stages / x slots
+constexpr int RTB_HEADER = 256;
+constexpr int RTB_SMEM_MAX = 224 * 1024;  // dynamic part: the reductions keep ~2 KB of static shared memory
+
+struct KrylovCtlB {
+  KrylovCtl c[NB];
+  int all_done, pad0, pad1, pad2;
+};
+
+struct RowArgsB {
+  int n;
+  const TileDesc* tiles;
+  int ntiles;
+  const unsigned char* blob;
+  const int* halo_idx;
+  const int* halo_cagg;
+  const double* x;       // gathered vector, [n][NB]
+  const double* b;
+  const double* dinv;    // [n]
+  double* out;
+  const double* dinv_c;  // restriction, optional: smoother diagonal of the coarse level ...
+  double* out2;          // ... then out2[I][s] = dinv_c[I] * out[I][s]
+  const int* agg;
+  const int* agg_ptr;
+  const double* ec;      // [nc][NB]
+  double gamma;
+  double* partials;      // [NB][gridDim.x]
+  unsigned* counter;
+  KrylovCtlB* ctl;       // may be null (hooks)
+  int fin;
+  int stages, xslots, stage_bytes, xslot_bytes;  // shared-memory ring geometry (host: fits RTB_SMEM_MAX)
+};
+
+// ---- placement of a tile inside its ring stage (after the TP_DESC_BYTES header); blob at 0 ----
+struct StageLayoutB {
+  int ra2, nrv;  // dinv slice (even start / count)
+  int Ia4, nap;  // agg_ptr slice
+  int Ia2, nec;  // dinv_c slice
+  int o_d, o_agg, o_dc, o_out, end;
+};
+enum { TPB_D = 1, TPB_RESTRICT = 2 };
+__host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) {
+  StageLayoutB t;
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const int r1 = d.r0 + d.nr;
+  t.ra2 = d.r0 & ~1;
+  t.nrv = tp_up(r1 - t.ra2, 2);
+  t.Ia4 = d.I0 & ~3;
+  t.nap = tp_up(d.I0 + d.nA + 1 - t.Ia4, 4);
+  t.Ia2 = d.I0 & ~1;
+  t.nec = tp_up(d.I0 + d.nA - t.Ia2, 2);
+  int o = p.end;
+  t.o_d = o;
+  if (flags & TPB_D) o += 8 * t.nrv;
+  t.o_agg = o;
+  if (flags & TPB_RESTRICT) o += 4 * t.nap;
+  t.o_dc = o;
+  if (flags & TPB_RESTRICT) o += 8 * t.nec;
+  t.o_out = o;
+  if (flags & TPB_RESTRICT) o += 8 * NB * d.nr;
+  t.end = o;
+  return t;
+}
+__host__ __device__ inline int tpb_stage_need(const TileDesc& d) {
+  const int a = tpb_stage(d, TPB_D).end, b = tpb_stage(d, TPB_RESTRICT).end;
+  return TP_DESC_BYTES + (a > b ? a : b);
+}
+__host__ __device__ inline int tpb_ncolp(int nr, int nhalo) { return (nr + nhalo) | 1; }  // odd plane pitch
+__host__ __device__ inline int tpb_xslot_need(const TileDesc& d) { return 16 * NB2 * tpb_ncolp(d.nr, d.nhalo); }
+
+// ---- per-column finalisation of a reduction; a finished column is frozen ----
+__device__ inline void krylov_finalize_b(KrylovCtlB* cb, int fin, const double* s0) {
+  int all = 1;
+#pragma unroll 1
+  for (int s = 0; s < NB; ++s) {
+    KrylovCtl& c = cb->c[s];
+    if (!c.done) krylov_finalize(&c, fin, s0[s], 0.0);
+    if (c.done) {  // no further update of x, r; p = z
+      c.alpha = 0.0;
+      c.beta = 0.0;
+    }
+    all &= c.done;
+  }
+  cb->all_done = all;
+}
+
+template <int THREADS>
+__device__ __forceinline__ void grid_reduce_finalize_b(double (&v)[NB], double* partials, unsigned* counter,
+                                                       KrylovCtlB* ctl, int fin) {
+  __shared__ double sh[NB][THREADS / 32];
+  __shared__ bool is_last;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    double s = v[j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) sh[j][w] = s;
+  }
+  __syncthreads();
+  if (tid < NB) {
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < THREADS / 32; ++q) s += sh[tid][q];
+    partials[(size_t)tid * gridDim.x + blockIdx.x] = s;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    unsigned t = atomicAdd(counter, 1u);
+    is_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    double s = 0.0;
+    for (unsigned q = tid; q < gridDim.x; q += THREADS) s += __ldcg(partials + (size_t)j * gridDim.x + q);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) sh[j][w] = s;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double tot[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      double s = 0.0;
+#pragma unroll
+      for (int q = 0; q < THREADS / 32; ++q) s += sh[j][q];
+      tot[j] = s;
+    }
+    *counter = 0;
+    krylov_finalize_b(ctl, fin, tot);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Batched row-tile kernel.  OP: OP_SPMV (dot: x.out per column), OP_JACOBI (dot: b.out),
+// OP_RESTRICT, OP_JACOBI_PROLONG (dot: b.out).  Everything the producer stages (blob, dinv,
+// agg_ptr, dinv_c) is setup data, so its first copies are issued before the grid dependency.
+// ------------------------------------------------------------------------------------------
+struct StageDescB {  // TP_DESC_BYTES at the start of a stage, written by the producer
+  int r0, nr, I0, nA;
+  int nsl, nhalo, roff, aoff;  // roff = r0 - ra2 (dinv slice), aoff = I0 - Ia4 (agg_ptr slice)
+  int o_perm, o_col, o_val, o_d;
+  int o_agg, o_out, o_dc, eoff;  // eoff = Ia2 (dcs[I - eoff] = dinv_c[I])
+  int pad[16];
+};
+static_assert(sizeof(StageDescB) == TP_DESC_BYTES, "stage header size");
+
+template <int OP, bool STREAM>
+__device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
+                                             uint64_t pol) {
+  constexpr bool SWEEP = (OP == OP_JACOBI || OP == OP_JACOBI_PROLONG);
+  constexpr bool RES = (OP == OP_RESTRICT);
+  const bool dc = RES && a.dinv_c != nullptr;
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const StageLayoutB t = tpb_stage(d, (SWEEP ? TPB_D : 0) | (RES ? TPB_RESTRICT : 0));
+  StageDescB sd;
+  sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
+  sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
+  sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_d = t.o_d;
+  sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.o_dc = t.o_dc, sd.eoff = t.Ia2;
+  int4* dst = reinterpret_cast<int4*>(stage);
+  const int4* src = reinterpret_cast<const int4*>(&sd);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) dst[q] = src[q];
+  if (d.nr <= 0) {
+    mbar_arrive(bar);
+    return;
+  }
+  unsigned char* base = stage + TP_DESC_BYTES;
+  uint32_t bytes = (uint32_t)p.end;
+  if (SWEEP) bytes += 8u * (uint32_t)t.nrv;
+  if (RES) bytes += 4u * (uint32_t)t.nap;
+  if (dc) bytes += 8u * (uint32_t)t.nec;
+  mbar_arrive_expect_tx(bar, bytes);
+  bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, (uint32_t)p.end, bar, pol);
+  if (SWEEP) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, 8u * (uint32_t)t.nrv, bar, pol);
+  if (RES) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
+  if (dc) bulk_g2s<false>(base + t.o_dc, a.dinv_c + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
+}
+
+struct GTileB {
+  int r0, nr, nhalo, hoff;
+  __device__ __forceinline__ void load(const RowArgsB& a, int t_begin, int my, int it) {
+    r0 = nr = nhalo = hoff = 0;
+    if (it < my) {
+      const TileDesc* d = a.tiles + RT_TILE(t_begin, it);
+      r0 = __ldg(&d->r0), nr = __ldg(&d->nr), nhalo = __ldg(&d->nhalo), hoff = __ldg(&d->halo_off);
+    }
+  }
+};
+
+template <int OP, int NDOT, bool STREAM>
+static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+  uint64_t* empty = full + RTB_MAXS;
+  uint64_t* resdone = empty + RTB_MAXS;
+  uint64_t* xready = resdone + RTB_MAXS;
+  uint64_t* xempty = xready + RTB_MAXS;
+  const int S = a.stages, XS = a.xslots;
+  unsigned char* stage0 = smem + RTB_HEADER;
+  unsigned char* xslot0 = stage0 + (size_t)S * a.stage_bytes;
+  constexpr int NCW = RTB_CONSUMERS / 32, NGW = RTB_GATHERERS / 32, NG = RTB_GGROUPS;
+  const int tid = threadIdx.x;
+  const int t_begin = blockIdx.x;
+  const int my = ((int)a.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;  // this CTA's tiles
+  const int npre = my < S ? my : S;
+  // ---- before the grid dependency: nothing here reads what an earlier kernel of the solve wrote ----
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, NCW);
+      mbar_init(resdone + s, NCW);
+    }
+    for (int q = 0; q < XS; ++q) {
+      mbar_init(xready + q, NGW / NG);
+      mbar_init(xempty + q, NCW);
+    }
+    fence_mbar_init();
+  }
+  __syncthreads();
+  pdl_launch_dependents();
+  const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
+  if (tid == RTB_CONSUMERS)  // the first ring stages: operator blobs and setup vectors only
+    for (int it = 0; it < npre; ++it)
+      tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, full + it, pol);
+  // gather warps: descriptor and column indices of their first tile
+  constexpr int GS = RTB_GATHERERS / NG;  // threads of a group
+  constexpr int CL = GS / NB2;            // column lanes of a group
+  constexpr int GU = RTB_GU;
+  const int gt = tid - (RTB_CONSUMERS + 32);
+  const int g = gt % GS, gg = gt / GS;
+  const int sub = g & (NB2 - 1), cl = g / NB2;
+  const bool is_gather = tid >= RTB_CONSUMERS + 32;
+  GTileB gc, gn;
+  int src[GU], cag[GU];  // level index of this thread's columns (own rows, then halo), their coarse indices
+  gc.load(a, t_begin, my, is_gather ? gg : my);
+  gn.load(a, t_begin, my, is_gather ? gg + NG : my);
+  auto load_indices = [&](const GTileB& t, int (&si)[GU], int (&ci)[GU]) {
+#pragma unroll
+    for (int u = 0; u < GU; ++u) {
+      const int c = cl + u * CL;
+      si[u] = -1, ci[u] = 0;
+      if (c < t.nr) {
+        si[u] = t.r0 + c;
+        if (OP == OP_JACOBI_PROLONG) ci[u] = __ldg(a.agg + t.r0 + c);
+      } else if (c < t.nr + t.nhalo) {
+        si[u] = __ldg(a.halo_idx + t.hoff + c - t.nr);
+        if (OP == OP_JACOBI_PROLONG) ci[u] = __ldg(a.halo_cagg + t.hoff + c - t.nr);
+      }
+    }
+  };
+  if (is_gather) load_indices(gc, src, cag);
+  pdl_wait();
+  if (a.ctl != nullptr && a.ctl->all_done) {
+    if (tid == RTB_CONSUMERS)  // the copies in flight target this CTA's shared memory: let them land
+      for (int it = 0; it < npre; ++it) mbar_wait(full + it, 0);
+    return;
+  }
+  double dots[NB];
+#pragma unroll
+  for (int j = 0; j < NB; ++j) dots[j] = 0.0;
+  const double2* x2g = reinterpret_cast<const double2*>(a.x);
+  const double2* e2g = reinterpret_cast<const double2*>(a.ec);
+
+  if (is_gather) {
+    // ---------------- gather warps: x slots [plane h][column], up to XS tiles ahead ----------------
+    for (int it = gg; it < my; it += NG) {
+      const int q = it % XS;
+      GTileB gnn;
+      gnn.load(a, t_begin, my, it + 2 * NG);
+      int srcn[GU], cagn[GU];
+      load_indices(gn, srcn, cagn);  // the next tile's indices travel while this tile is gathered
+      const int ncol = gc.nr + gc.nhalo, ncolp = tpb_ncolp(gc.nr, gc.nhalo);
+      double2 v[GU];
+#pragma unroll
+      for (int u = 0; u < GU; ++u) {
+        v[u] = make_double2(0.0, 0.0);
+        if (src[u] >= 0) {
+          v[u] = __ldg(x2g + (size_t)src[u] * NB2 + sub);
+          if (OP == OP_JACOBI_PROLONG) {
+            const double2 e = __ldg(e2g + (size_t)cag[u] * NB2 + sub);
+            v[u].x += a.gamma * e.x, v[u].y += a.gamma * e.y;
+          }
+        }
+      }
+      if (it >= XS) mbar_wait(xempty + q, (uint32_t)(((it / XS) - 1) & 1));
+      double2* xc = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes) + (size_t)sub * ncolp;
+#pragma unroll
+      for (int u = 0; u < GU; ++u)
+        if (src[u] >= 0) xc[cl + u * CL] = v[u];
+      for (int c = cl + GU * CL; c < ncol; c += CL) {  // more columns than the index registers hold
+        int s_, c_ = 0;
+        if (c < gc.nr) {
+          s_ = gc.r0 + c;
+          if (OP == OP_JACOBI_PROLONG) c_ = __ldg(a.agg + s_);
+        } else {
+          s_ = __ldg(a.halo_idx + gc.hoff + c - gc.nr);
+          if (OP == OP_JACOBI_PROLONG) c_ = __ldg(a.halo_cagg + gc.hoff + c - gc.nr);
+        }
+        double2 w = __ldg(x2g + (size_t)s_ * NB2 + sub);
+        if (OP == OP_JACOBI_PROLONG) {
+          const double2 e = __ldg(e2g + (size_t)c_ * NB2 + sub);
+          w.x += a.gamma * e.x, w.y += a.gamma * e.y;
+        }
+        xc[c] = w;
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(xready + q);
+      gc = gn, gn = gnn;
+#pragma unroll
+      for (int u = 0; u < GU; ++u) src[u] = srcn[u], cag[u] = cagn[u];
+    }
+  } else if (tid >= RTB_CONSUMERS) {
+    // ---------------- producer warp ----------------
+    if (tid == RTB_CONSUMERS)
+      for (int it = npre; it < my; ++it) {
+        const int s = it % S;
+        const TileDesc d = a.tiles[RT_TILE(t_begin, it)];
+        mbar_wait(empty + s, (uint32_t)(((it / S) - 1) & 1));
+        tile_issue_b<OP, STREAM>(a, d, stage0 + (size_t)s * a.stage_bytes, full + s, pol);
+      }
+  } else {
+    // ---------------- consumers ----------------
+    const int lane = tid & 31, w = tid >> 5;
+    const double2* b2g = reinterpret_cast<const double2*>(a.b);
+    double2* o2g = reinterpret_cast<double2*>(a.out);
+    int sbase = 0;  // slices of the tiles so far: the round-robin deal continues across tiles
+    for (int it = 0; it < my; ++it) {
+      const int s = it % S, q = it % XS;
+      const uint32_t par = (uint32_t)((it / S) & 1);
+      unsigned char* stage = stage0 + (size_t)s * a.stage_bytes;
+      mbar_wait(full + s, par);                                // the bulk copies have landed ...
+      mbar_wait(xready + q, (uint32_t)((it / XS) & 1));        // ... and the tile's x slot is assembled
+      const StageDescB* sd = reinterpret_cast<const StageDescB*>(stage);
+      const int nr = sd->nr, nsl = sd->nsl, r0 = sd->r0;
+      if (nr > 0) {
+        unsigned char* base = stage + TP_DESC_BYTES;
+        const int2* slices = reinterpret_cast<const int2*>(base);
+        const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + sd->o_perm);
+        const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
+        const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
+        const int ncolp = tpb_ncolp(nr, sd->nhalo);
+        const double2* xc = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes);
+        const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
+        double2* outs = reinterpret_cast<double2*>(base + sd->o_out);  // [row][NB2]: residuals of the tile
+        for (int j = (w - sbase) & (NCW - 1); j < nsl; j += NCW) {
+          const int2 sl = slices[j];
+          const int lr = perm[j * 32 + lane];
+          const bool valid = lr != 0xFFFF;
+          double2 bv[NB2];
+#pragma unroll
+          for (int h = 0; h < NB2; ++h) bv[h] = make_double2(0.0, 0.0);
+          if (OP != OP_SPMV && valid) {  // 64 contiguous bytes of b, consumed after the row walk
+#pragma unroll
+            for (int h = 0; h < NB2; ++h) bv[h] = __ldg(b2g + (size_t)(r0 + lr) * NB2 + h);
+          }
+          const unsigned short* cp = scol + sl.x;
+          const double* vp = sval + sl.x;
+          double acc[NB];
+#pragma unroll
+          for (int t = 0; t < NB; ++t) acc[t] = 0.0;
+#pragma unroll 2
+          for (int k = 0; k < sl.y; ++k) {
+            const double av = vp[k * 32];
+            const double2* xp = xc + cp[k * 32];
+#pragma unroll
+            for (int h = 0; h < NB2; ++h) {
+              const double2 xv = xp[(size_t)h * ncolp];
+              acc[2 * h] += av * xv.x;
+              acc[2 * h + 1] += av * xv.y;
+            }
+          }
+          if (valid) {
+            if (OP == OP_RESTRICT) {
+#pragma unroll
+              for (int h = 0; h < NB2; ++h)
+                outs[lr * NB2 + h] = make_double2(bv[h].x - acc[2 * h], bv[h].y - acc[2 * h + 1]);
+            } else {
+              const double di = (OP == OP_SPMV) ? 0.0 : ds[lr];
+#pragma unroll
+              for (int h = 0; h < NB2; ++h) {
+                double2 o;
+                const double2 xo = xc[(size_t)h * ncolp + lr];  // the row's own x (SpMV: for the dot)
+                if (OP == OP_SPMV) {
+                  o = make_double2(acc[2 * h], acc[2 * h + 1]);
+                  if (NDOT) dots[2 * h] += xo.x * o.x, dots[2 * h + 1] += xo.y * o.y;
+                } else {
+                  o.x = xo.x + di * (bv[h].x - acc[2 * h]);
+                  o.y = xo.y + di * (bv[h].y - acc[2 * h + 1]);
+                  if (NDOT) dots[2 * h] += bv[h].x * o.x, dots[2 * h + 1] += bv[h].y * o.y;
+                }
+                o2g[(size_t)(r0 + lr) * NB2 + h] = o;
+              }
+            }
+          }
+        }
+        if (OP == OP_RESTRICT) {
+          // the rows of an aggregate are consecutive tile rows: all residuals of the tile first
+          __syncwarp();
+          if (lane == 0) mbar_arrive(resdone + s);
+          mbar_wait(resdone + s, par);
+          const int nA = sd->nA, I0 = sd->I0;
+          const int* aps = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;      // aps[al] = agg_ptr[I0 + al]
+          const double* dcs = reinterpret_cast<const double*>(base + sd->o_dc) - sd->eoff;  // dcs[I] = dinv_c[I]
+          double2* o22g = reinterpret_cast<double2*>(a.out2);
+          for (int t = tid; t < nA * NB2; t += RTB_CONSUMERS) {
+            const int al = t / NB2, h = t % NB2;
+            double2 sum = make_double2(0.0, 0.0);
+            for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) {
+              const double2 rv = outs[lr * NB2 + h];
+              sum.x += rv.x, sum.y += rv.y;
+            }
+            o2g[(size_t)(I0 + al) * NB2 + h] = sum;
+            if (a.out2 != nullptr) {
+              const double dcv = dcs[I0 + al];
+              o22g[(size_t)(I0 + al) * NB2 + h] = make_double2(dcv * sum.x, dcv * sum.y);
+            }
+          }
+        }
+      }
+      sbase = (sbase + nsl) & (NCW - 1);
+      // ---- this warp is done with the stage and the x slot ----
+      if (OP == OP_RESTRICT) fence_proxy_async();  // residuals were written into a region the next bulk copy overwrites
+      __syncwarp();
+      if (lane == 0) {
+        mbar_arrive(empty + s);
+        mbar_arrive(xempty + q);
+      }
+    }
+  }
+  if (NDOT > 0) grid_reduce_finalize_b<RTB_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);
+}
+
+// ------------------------------------------------------------------------------------------
+// Batched Krylov vector kernels (interleaved [row][NB] vectors, per-column scalars)
+// ------------------------------------------------------------------------------------------
+// r[i][s] = b_s[inv[i]] (columns >= ncols: 0), x = 0, x1 = dinv o r (first sweep of level 0 from zero);
+// ||b_s||^2 per column
+static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init_b(int n, int ncols, int64_t ld,
+                                                               const double* __restrict__ b_nat,
+                                                               const int* __restrict__ inv,
+                                                               const double* __restrict__ dinv, double* __restrict__ r,
+                                                               double* __restrict__ x, double* __restrict__ x1,
+                                                               double* partials, unsigned* counter, KrylovCtlB* ctl) {
+  double acc[NB];
+#pragma unroll
+  for (int s = 0; s < NB; ++s) acc[s] = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
+    const int src = inv[i];
+    const double di = x1 ? dinv[i] : 0.0;
+    double v[NB];
+#pragma unroll
+    for (int s = 0; s < NB; ++s) v[s] = s < ncols ? __ldg(b_nat + (size_t)s * ld + src) : 0.0;
+    double2* r2 = reinterpret_cast<double2*>(r) + i * NB2;
+    double2* x2 = reinterpret_cast<double2*>(x) + i * NB2;
+#pragma unroll
+    for (int h = 0; h < NB2; ++h) {
+      r2[h] = make_double2(v[2 * h], v[2 * h + 1]);
+      x2[h] = make_double2(0.0, 0.0);
+      if (x1) reinterpret_cast<double2*>(x1)[i * NB2 + h] = make_double2(di * v[2 * h], di * v[2 * h + 1]);
+      acc[2 * h] += v[2 * h] * v[2 * h];
+      acc[2 * h + 1] += v[2 * h + 1] * v[2 * h + 1];
+    }
+  }
+  grid_reduce_finalize_b<RED_THREADS>(acc, partials, counter, ctl, FIN_INIT_PCG);
+}
+
+// x += alpha_s p ; r -= alpha_s q ; ||r_s||^2 ; x1 = dinv o r (first sweep of the next V-cycle on level 0)
+static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr_b(int n, const double* __restrict__ p,
+                                                          const double* __restrict__ q, double* __restrict__ x,
+                                                          double* __restrict__ r, const double* __restrict__ dinv,
+                                                          double* __restrict__ x1, double* partials, unsigned* counter,
+                                                          KrylovCtlB* ctl) {
+  pdl_sync();
+  if (ctl->all_done) return;
+  // gridDim.x * RED_THREADS is a multiple of NB2: a thread keeps its pair of columns over the loop
+  const int h = threadIdx.x & (NB2 - 1);
+  const double a0 = ctl->c[2 * h].done ? 0.0 : ctl->c[2 * h].alpha;
+  const double a1 = ctl->c[2 * h + 1].done ? 0.0 : ctl->c[2 * h + 1].alpha;
+  double s0 = 0.0, s1 = 0.0;
+  const int64_t m = (int64_t)n * NB2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* p2 = reinterpret_cast<const double2*>(p);
+  const double2* q2 = reinterpret_cast<const double2*>(q);
+  double2* x2 = reinterpret_cast<double2*>(x);
+  double2* r2 = reinterpret_cast<double2*>(r);
+  double2* y2 = reinterpret_cast<double2*>(x1);
+  for (int64_t t = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; t < m; t += stride) {
+    const double2 pv = p2[t], qv = q2[t];
+    double2 xv = x2[t], rv = r2[t];
+    xv.x += a0 * pv.x, xv.y += a1 * pv.y;
+    rv.x -= a0 * qv.x, rv.y -= a1 * qv.y;
+    x2[t] = xv, r2[t] = rv;
+    if (x1) {
+      const double di = __ldg(dinv + t / NB2);
+      y2[t] = make_double2(di * rv.x, di * rv.y);
+    }
+    s0 += rv.x * rv.x, s1 += rv.y * rv.y;
+  }
+  double acc[NB];
+#pragma unroll
+  for (int s = 0; s < NB; ++s) acc[s] = (s == 2 * h) ? s0 : ((s == 2 * h + 1) ? s1 : 0.0);
+  grid_reduce_finalize_b<RED_THREADS>(acc, partials, counter, ctl, FIN_RR);
+}
+
+// p = z + beta_s p
+static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p_b(int n, const double* __restrict__ z, double* __restrict__ p,
+                                                         const KrylovCtlB* ctl) {
+  pdl_sync();
+  if (ctl->all_done) return;
+  const int h = threadIdx.x & (NB2 - 1);
+  const double b0 = ctl->c[2 * h].beta, b1 = ctl->c[2 * h + 1].beta;
+  const int64_t m = (int64_t)n * NB2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* z2 = reinterpret_cast<const double2*>(z);
+  double2* p2 = reinterpret_cast<double2*>(p);
+  for (int64_t t = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; t < m; t += stride) {
+    const double2 zv = z2[t];
+    double2 pv = p2[t];
+    // beta = 0 (first iteration, frozen column): p = z exactly, whatever the buffer held (it is not initialised)
+    pv.x = b0 != 0.0 ? zv.x + b0 * pv.x : zv.x;
+    pv.y = b1 != 0.0 ? zv.y + b1 * pv.y : zv.y;
+    p2[t] = pv;
+  }
+}
+
+// x_nat column s (s < ncols), natural numbering
+static __global__ void k_krylov_output_b(int n, int ncols, int64_t ld, const double* __restrict__ x,
+                                  const int* __restrict__ inv, double* __restrict__ x_nat) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int dst = inv[i];
+  const double2* x2 = reinterpret_cast<const double2*>(x) + i * NB2;
+#pragma unroll
+  for (int h = 0; h < NB2; ++h) {
+    const double2 v = x2[h];
+    if (2 * h < ncols) x_nat[(size_t)(2 * h) * ld + dst] = v.x;
+    if (2 * h + 1 < ncols) x_nat[(size_t)(2 * h + 1) * ld + dst] = v.y;
+  }
+}
+
+// interleave / de-interleave of a level vector batch for the hooks: nat[s * ld + inv[i]] <-> v[i][s]
+static __global__ void k_permute_in_b(int n, int ncols, int64_t ld, const double* __restrict__ nat,
+                               const int* __restrict__ inv, double* __restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int src = inv[i];
+#pragma unroll
+  for (int s = 0; s < NB; ++s) out[i * NB + s] = s < ncols ? nat[(size_t)s * ld + src] : 0.0;
+}
+
+// z[i][s] = sum_j B[i][j] b[j][s]: the dense collapsed tail for NB right-hand sides; one warp per row
+struct TailArgsB {
+  int n;
+  const double* dense_B;
+  const double* b;
+  double* z;
+  double* partials;
+  unsigned* counter;
+  KrylovCtlB* ctl;
+  int fin;
+};
+constexpr int TAILB_T = 1024;
+static __global__ void __launch_bounds__(TAILB_T, 1) k_dense_tail_b(TailArgsB a) {
+  pdl_launch_dependents();
+  const int G = gridDim.x, cta = blockIdx.x;
+  const int i0 = (int)((int64_t)cta * a.n / G), i1 = (int)((int64_t)(cta + 1) * a.n / G);
+  {
+    const char* p0 = reinterpret_cast<const char*>(a.dense_B + (size_t)i0 * a.n);
+    const size_t bytes = (size_t)(i1 - i0) * a.n * sizeof(double);
+    for (size_t o = (size_t)threadIdx.x * 128; o < bytes; o += (size_t)TAILB_T * 128)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + o));
+  }
+  pdl_wait();
+  if (a.ctl != nullptr && a.ctl->all_done) return;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const double2* b2 = reinterpret_cast<const double2*>(a.b);
+  double dots[NB];
+#pragma unroll
+  for (int s = 0; s < NB; ++s) dots[s] = 0.0;
+  for (int i = i0 + w; i < i1; i += TAILB_T / 32) {
+    const double* row = a.dense_B + (size_t)i * a.n;
+    double acc[NB];
+#pragma unroll
+    for (int s = 0; s < NB; ++s) acc[s] = 0.0;
+    for (int j = lane; j < a.n; j += 32) {
+      const double v = __ldg(row + j);
+#pragma unroll
+      for (int h = 0; h < NB2; ++h) {
+        const double2 bv = b2[(size_t)j * NB2 + h];
+        acc[2 * h] += v * bv.x, acc[2 * h + 1] += v * bv.y;
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < NB; ++s)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc[s] += __shfl_xor_sync(0xffffffffu, acc[s], o);
+    if (lane == 0) {
+#pragma unroll
+      for (int s = 0; s < NB; ++s) {
+        a.z[(size_t)i * NB + s] = acc[s];
+        if (a.fin != FIN_NONE) dots[s] += a.b[(size_t)i * NB + s] * acc[s];
+      }
+    }
+  }
+  if (a.fin != FIN_NONE) grid_reduce_finalize_b<TAILB_T>(dots, a.partials, a.counter, a.ctl, a.fin);
+}

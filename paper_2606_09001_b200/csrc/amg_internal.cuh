@@ -113,6 +113,8 @@ struct Level {
   int match_rounds = 0;
 };
 
+struct AmgBatch;  // batched multi-RHS state (amg_batched.cu)
+
 struct amg_handle_s {
   amg_options opt;
   int64_t n = 0, nnz = 0;
@@ -159,6 +161,7 @@ struct amg_handle_s {
   double* hist = nullptr;             // residual history of the last solve (device), hist_cap entries
   int hist_cap = 0;
   int hist_len = 0;                   // iterations of the last solve that reported (info != NULL)
+  AmgBatch* batch = nullptr;          // work vectors / graphs of the batched solve, built on first use
   double* grad_xt = nullptr;          // interleaved right-hand sides of amg_grad_values (grown on demand)
   size_t grad_xt_cap = 0;
   int sm_count = 148;
@@ -224,5 +227,10 @@ double amg_algorithmic_bytes(amg_handle_s* H, int which);
 void amg_destroy_graphs(amg_handle_s* H);
 amg_status amg_setup_tail(amg_handle_s* H, int transposed, cudaStream_t st);
 void amg_configure_kernels();
+// batched.cu (NEXT-3)
+int amg_batch_prepare(amg_handle_s* H, cudaStream_t st);
+amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X, int ncols, int64_t ld, double rtol,
+                                 int maxit, amg_info* infos, cudaStream_t st);
+void amg_batch_release(amg_handle_s* H);
 // setup.cu: transposed level operators, their tile blobs, LU of A_L^T, dense tail of B^T
 amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st);

@@ -449,7 +449,7 @@ struct GTile {  // what the gather warps need of a tile descriptor
 };
 
 template <int OP, int NDOT, bool STREAM>
-__global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
+static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty = full + RT_STAGES;
@@ -708,7 +708,7 @@ __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
 // Row-vector fallback: LPR lanes per row (any row length, any aggregate size).
 // ------------------------------------------------------------------------------------------
 template <int OP, int NDOT, int LPR>
-__global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
+static __global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
   pdl_sync();
   if (a.ctl != nullptr && a.ctl->done) return;
   const int tid = threadIdx.x;
@@ -738,7 +738,7 @@ __global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
 }
 
 // restriction of a stored residual (fallback path): rc[I] = sum of r over the contiguous rows of I
-__global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const double* __restrict__ r,
+static __global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const double* __restrict__ r,
                                 double* __restrict__ rc, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
@@ -750,7 +750,7 @@ __global__ void k_restrict_rows(int nc, const int* __restrict__ agg_ptr, const d
 }
 
 // S4 standalone: x_i += gamma * ec[agg_i]
-__global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* __restrict__ ec, double gamma,
+static __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* __restrict__ ec, double gamma,
                               const double* xin, double* xout /* may be xin */, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
@@ -769,7 +769,7 @@ __global__ void k_prolong_add(int n, const int* __restrict__ agg, const double* 
   if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) xout[n - 1] = xin[n - 1] + gamma * ec[agg[n - 1]];
 }
 
-__global__ void k_scale_dinv(int n, const double* __restrict__ dinv, const double* __restrict__ b,
+static __global__ void k_scale_dinv(int n, const double* __restrict__ dinv, const double* __restrict__ b,
                              double* __restrict__ x, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
@@ -777,7 +777,7 @@ __global__ void k_scale_dinv(int n, const double* __restrict__ dinv, const doubl
   if (i < n) x[i] = dinv[i] * b[i];
 }
 
-__global__ void k_zero(int n, double* __restrict__ x, const KrylovCtl* ctl) {
+static __global__ void k_zero(int n, double* __restrict__ x, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -787,7 +787,7 @@ __global__ void k_zero(int n, double* __restrict__ x, const KrylovCtl* ctl) {
 // ------------------------------------------------------------------------------------------
 // S5: coarsest solve with the dense LU factors (one CTA; y in shared memory)
 // ------------------------------------------------------------------------------------------
-__global__ void k_lu_solve(int n, const double* __restrict__ lu, const int* __restrict__ piv,
+static __global__ void k_lu_solve(int n, const double* __restrict__ lu, const int* __restrict__ piv,
                            const double* __restrict__ b, double* __restrict__ x, const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl != nullptr && ctl->done) return;
@@ -862,7 +862,7 @@ __device__ __forceinline__ void lu_solve_small_cta(int n, const double* __restri
   for (int i = tid; i < n; i += T) x[i] = y[i];
 }
 
-__global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __restrict__ lu,
+static __global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __restrict__ lu,
                                                         const int* __restrict__ piv, const double* __restrict__ b,
                                                         double* __restrict__ x, const KrylovCtl* ctl) {
   pdl_sync();
@@ -875,7 +875,7 @@ __global__ void __launch_bounds__(256) k_lu_solve_small(int n, const double* __r
 // S7/S8: fused Krylov vector kernels (grid-stride, one pass each, scalars read from KrylovCtl)
 // ------------------------------------------------------------------------------------------
 // r = b (permuted in), x = 0, optional extra vectors zeroed / copied; ||b||^2
-__global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const double* __restrict__ b_nat,
+static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const double* __restrict__ b_nat,
                                                              const int* __restrict__ inv, double* __restrict__ r,
                                                              double* __restrict__ x, double* __restrict__ z0,
                                                              double* __restrict__ z1, double* __restrict__ rhat,
@@ -895,7 +895,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const double
 }
 
 // p = z + beta p
-__global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __restrict__ z, double* __restrict__ p,
+static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __restrict__ z, double* __restrict__ p,
                                                        const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl->done) return;
@@ -914,7 +914,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __re
 }
 
 // x += alpha p ; r -= alpha q ; ||r||^2
-__global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __restrict__ p,
+static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __restrict__ p,
                                                         const double* __restrict__ q, double* __restrict__ x,
                                                         double* __restrict__ r, double* partials, unsigned* counter,
                                                         KrylovCtl* ctl) {
@@ -955,7 +955,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __r
 }
 
 // sum a.b  (used when no smoother sweep can carry the r.z product)
-__global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __restrict__ a, const double* __restrict__ b,
+static __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __restrict__ a, const double* __restrict__ b,
                                                      double* partials, unsigned* counter, KrylovCtl* ctl, int fin) {
   pdl_sync();
   if (ctl->done) return;
@@ -966,7 +966,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double* __rest
 }
 
 // p = r + beta (p - omega v)
-__global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __restrict__ r,
+static __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ p,
                                                         const KrylovCtl* ctl) {
   pdl_sync();
@@ -977,7 +977,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __r
 }
 
 // s = r - alpha v ; ||s||^2
-__global__ void __launch_bounds__(RED_THREADS) k_bicg_s(int n, const double* __restrict__ r,
+static __global__ void __launch_bounds__(RED_THREADS) k_bicg_s(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ s,
                                                         double* partials, unsigned* counter, KrylovCtl* ctl) {
   pdl_sync();
@@ -993,7 +993,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_s(int n, const double* __r
 }
 
 // x += alpha phat + omega shat ; r = s - omega t ; ||r||^2 , rhat.r
-__global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const double* __restrict__ ph,
+static __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const double* __restrict__ ph,
                                                          const double* __restrict__ sh, const double* __restrict__ s,
                                                          const double* __restrict__ t, const double* __restrict__ rhat,
                                                          double* __restrict__ x, double* __restrict__ r,
@@ -1013,7 +1013,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const double* __
 }
 
 // x_out (natural numbering) = x [+ alpha * phat after a BiCGSTAB half-step exit]
-__global__ void k_krylov_output(int n, const double* __restrict__ x, const double* __restrict__ ph,
+static __global__ void k_krylov_output(int n, const double* __restrict__ x, const double* __restrict__ ph,
                                 const int* __restrict__ inv, double* __restrict__ x_nat, const KrylovCtl* ctl) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -1022,12 +1022,12 @@ __global__ void k_krylov_output(int n, const double* __restrict__ x, const doubl
   x_nat[inv[i]] = v;
 }
 
-__global__ void k_permute_in(int n, const double* __restrict__ nat, const int* __restrict__ inv,
+static __global__ void k_permute_in(int n, const double* __restrict__ nat, const int* __restrict__ inv,
                              double* __restrict__ out) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = nat[inv[i]];
 }
-__global__ void k_permute_out(int n, const double* __restrict__ in, const int* __restrict__ inv,
+static __global__ void k_permute_out(int n, const double* __restrict__ in, const int* __restrict__ inv,
                               double* __restrict__ nat) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) nat[inv[i]] = in[i];
@@ -1037,7 +1037,7 @@ __global__ void k_permute_out(int n, const double* __restrict__ in, const int* _
 // G2: gA[k] (+)= - sum_s lambda_s[i] x_s[col[k]]  on the natural pattern; LPR lanes per row
 // ------------------------------------------------------------------------------------------
 template <int LPR>
-__global__ void __launch_bounds__(256) k_grad_values(int n, const int* __restrict__ rowptr,
+static __global__ void __launch_bounds__(256) k_grad_values(int n, const int* __restrict__ rowptr,
                                                      const int* __restrict__ col, const double* __restrict__ lam,
                                                      const double* __restrict__ x, int nrhs, int64_t ld,
                                                      double* __restrict__ gA, int accumulate) {
@@ -1059,7 +1059,7 @@ __global__ void __launch_bounds__(256) k_grad_values(int n, const int* __restric
 // coalesced pass), so that all nrhs values of a column are ONE contiguous gather; lambda_s[i] is
 // unit-stride along the rows as it stands.
 constexpr int GT_ROWS = 64;  // rows per CTA of the interleave kernel
-__global__ void __launch_bounds__(256) k_interleave_rhs(int n, int nrhs, int64_t ld, const double* __restrict__ X,
+static __global__ void __launch_bounds__(256) k_interleave_rhs(int n, int nrhs, int64_t ld, const double* __restrict__ X,
                                                         double* __restrict__ XT) {
   extern __shared__ double tile[];  // [nrhs][GT_ROWS + 1]
   const int i0 = blockIdx.x * GT_ROWS;
@@ -1075,7 +1075,7 @@ __global__ void __launch_bounds__(256) k_interleave_rhs(int n, int nrhs, int64_t
 }
 
 template <int LPR, int NR>  // NR > 0: nrhs known at compile time (registers for lambda); 0: generic
-__global__ void __launch_bounds__(256) k_grad_values_batched(int n, const int* __restrict__ rowptr,
+static __global__ void __launch_bounds__(256) k_grad_values_batched(int n, const int* __restrict__ rowptr,
                                                              const int* __restrict__ col,
                                                              const double* __restrict__ lam, int64_t ld,
                                                              const double* __restrict__ XT, int nrhs_rt,

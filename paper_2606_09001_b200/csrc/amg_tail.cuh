@@ -229,7 +229,7 @@ struct TailArgs {
   int fin;                 // FIN_RZ: b . z is reduced and finalised (cycles that start at level D = 0)
 };
 
-__global__ void __launch_bounds__(TAIL_THREADS, 1) k_dense_tail(TailArgs a) {
+static __global__ void __launch_bounds__(TAIL_THREADS, 1) k_dense_tail(TailArgs a) {
   pdl_launch_dependents();
   const int G = gridDim.x, cta = blockIdx.x;
   const int i0 = (int)((int64_t)cta * a.n / G), i1 = (int)((int64_t)(cta + 1) * a.n / G);
@@ -267,7 +267,7 @@ struct TailBuildArgs {
   int lu_smem;
 };
 
-__global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailBuildArgs a) {
+static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailBuildArgs a) {
   extern __shared__ __align__(16) unsigned char tb_sm[];
   double* vec = reinterpret_cast<double*>(tb_sm + a.lu_smem);
   const int tid = threadIdx.x, j = blockIdx.x;
