@@ -250,6 +250,12 @@ amg_status amg_resetup_values(amg_handle h, const double* d_val, int32_t keep_ag
   }
   Enter e(h, cuda_stream);
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (keep_aggregates) {
+    // warm: values only, on the kept hierarchy (patterns, partitions, blobs' index sections, graphs stay)
+    int fallback = 0;
+    const amg_status sw = amg_resetup_values_warm(h, d_val, &fallback, st);
+    if (sw != AMG_OK || !fallback) return sw;
+  }
   cudaStreamSynchronize(st);
   std::vector<const int32_t*> aggs;
   if (keep_aggregates)

@@ -111,6 +111,10 @@ struct Level {
   double* x2 = nullptr;     // pong
   double* rtmp = nullptr;   // fine residual (fallback path only)
   int match_rounds = 0;
+  // value-only (warm) resetup maps, built on the first amg_resetup_values(keep_aggregates = 1):
+  int* src0 = nullptr;         // level 0 only: [nnz] position in the caller's val[] of every permuted entry
+  int* contrib_ptr = nullptr;  // [nnz_{l+1} + 1] per entry of A_{l+1}: its fine contributions ...
+  int* contrib_idx = nullptr;  // [nnz_l] ... as ascending positions in this level's val[] (fixed summation order)
 };
 
 struct AmgBatch;  // batched multi-RHS state (amg_batched.cu)
@@ -129,6 +133,7 @@ struct amg_handle_s {
   double* luT = nullptr;
   int* pivT = nullptr;
   bool have_T = false;
+  bool have_maps = false;  // warm-resetup maps built
   // Krylov work vectors (level-0 size, permuted numbering)
   double* kv[10] = {nullptr};
   double* io_tmp = nullptr;  // staging for amg_solve_host / hooks
@@ -234,3 +239,5 @@ amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X
 void amg_batch_release(amg_handle_s* H);
 // setup.cu: transposed level operators, their tile blobs, LU of A_L^T, dense tail of B^T
 amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st);
+// setup.cu: NEXT-1 value-only resetup on the kept hierarchy; *fallback = 1: the caller has to rebuild (symmetry changed)
+amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fallback, cudaStream_t st);

@@ -1060,11 +1060,11 @@ amg_status permute_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const
   return AMG_OK;
 }
 
-// U6: dense LU with partial pivoting of a (coarsest) operator given in CSR; *lu / *piv allocated here
+// U6: dense LU with partial pivoting of a (coarsest) operator given in CSR; *lu / *piv allocated here if null
 amg_status dense_lu_of(amg_handle_s* H, int n, const int* rowptr, const int* col, const double* val, double** lu,
                        int** piv, cudaStream_t st) {
-  AMG_ALLOC(H, *lu, double, (size_t)n * n, st);
-  AMG_ALLOC(H, *piv, int, n, st);
+  if (!*lu) AMG_ALLOC(H, *lu, double, (size_t)n * n, st);  // a warm resetup refactors in place
+  if (!*piv) AMG_ALLOC(H, *piv, int, n, st);
   AMG_CUDA_TRY(H, cudaMemsetAsync(*lu, 0, sizeof(double) * (size_t)n * n, st));
   k_csr_to_dense<<<grid_for(n), TPB, 0, st>>>(n, rowptr, col, val, *lu);
   int* info;
@@ -1422,4 +1422,223 @@ amg_status amg_natural_level_csr(amg_handle_s* H, int level, int32_t* d_rowptr, 
   Level& L = H->lv[level];
   // natural row i = permuted row pos[i]; permuted column c -> natural inv[c]
   return permute_csr(H, L.n, L.nnz, L.rowptr, L.col, L.val, L.pos, L.inv, d_rowptr, d_col, d_val, st);
+}
+
+// ------------------------------------------------------------------------------------------
+// NEXT-1, warm: amg_resetup_values(keep_aggregates = 1) on the KEPT hierarchy ("matrix
+// coefficients are updated in place"; :285 "warm resetup-and-solve ... dominates").  Nothing
+// structural is redone: aggregates, numbering, level patterns, tile partitions, halo lists, the
+// slice / perm / column sections of the blobs, work vectors, CUDA graphs all stay.  Recomputed,
+// each as one bandwidth-trivial pass: level-0 values (gather through src0), coarse values (numeric
+// Galerkin: every coarse entry sums its fine contributions in ascending position, a fixed order),
+// smoother diagonals, the value sections of the tile blobs, the coarsest LU, the dense tail, and
+// the same for the transposed hierarchy.  The maps are built on the first warm resetup.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+// src0[k] for the permuted level-0 entry k = (row p, column c): position of (inv[p], inv[c]) in the caller's CSR
+__global__ void k_build_src0(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                             const int* __restrict__ inv, const int* __restrict__ nat_rowptr,
+                             const int* __restrict__ nat_col, int* __restrict__ src0) {
+  int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  const int i = inv[p];
+  const int s = nat_rowptr[i], e = nat_rowptr[i + 1];
+  for (int k = rowptr[p]; k < rowptr[p + 1]; ++k) {
+    const int j = inv[col[k]];
+    int lo = s, hi = e - 1, pos = s;
+    while (lo <= hi) {
+      const int mid = (lo + hi) >> 1;
+      const int c = nat_col[mid];
+      if (c == j) {
+        pos = mid;
+        break;
+      }
+      if (c < j) lo = mid + 1;
+      else hi = mid - 1;
+    }
+    src0[k] = pos;
+  }
+}
+
+// coarse entry of every fine entry: tgt[k] = position of (agg[i], agg[col[k]]) in the coarse CSR; cnt[tgt]++
+__global__ void k_rap_target(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                             const int* __restrict__ agg, const int* __restrict__ crowptr,
+                             const int* __restrict__ ccol, int* __restrict__ tgt, int* __restrict__ cnt) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int I = agg[i];
+  const int s = crowptr[I], e = crowptr[I + 1];
+  for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+    const int J = agg[col[k]];
+    int lo = s, hi = e - 1, pos = s;
+    while (lo <= hi) {
+      const int mid = (lo + hi) >> 1;
+      const int c = ccol[mid];
+      if (c == J) {
+        pos = mid;
+        break;
+      }
+      if (c < J) lo = mid + 1;
+      else hi = mid - 1;
+    }
+    tgt[k] = pos;
+    atomicAdd(&cnt[pos], 1);
+  }
+}
+__global__ void k_contrib_fill(int nnz, const int* __restrict__ tgt, const int* __restrict__ cptr,
+                               int* __restrict__ cursor, int* __restrict__ cidx) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nnz) return;
+  const int t = tgt[k];
+  cidx[cptr[t] + atomicAdd(&cursor[t], 1)] = k;
+}
+__global__ void k_contrib_sort(int m, const int* __restrict__ cptr, int* __restrict__ cidx) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= m) return;
+  const int s = cptr[e], t = cptr[e + 1];
+  for (int a = s + 1; a < t; ++a) {
+    const int v = cidx[a];
+    int b = a - 1;
+    while (b >= s && cidx[b] > v) {
+      cidx[b + 1] = cidx[b];
+      --b;
+    }
+    cidx[b + 1] = v;
+  }
+}
+// numeric Galerkin: cval[e] = sum of val[] over the contributions of e, ascending position
+__global__ void k_rap_numeric(int m, const int* __restrict__ cptr, const int* __restrict__ cidx,
+                              const double* __restrict__ val, double* __restrict__ cval) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= m) return;
+  double s = 0.0;
+  for (int t = cptr[e]; t < cptr[e + 1]; ++t) s += val[cidx[t]];
+  cval[e] = s;
+}
+
+// value section of every tile blob from the level's CSR values (the slices / perm sections say where)
+__global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc* __restrict__ tiles,
+                                                     const int* __restrict__ rowptr, const double* __restrict__ val,
+                                                     unsigned char* __restrict__ blob) {
+  const int t = blockIdx.x;
+  if (t >= ntiles) return;
+  const TileDesc d = tiles[t];
+  if (d.nr <= 0) return;
+  unsigned char* base = blob + (size_t)d.blob16 * 16u;
+  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const int2* slices = reinterpret_cast<const int2*>(base);
+  const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + p.o_perm);
+  double* o_val = reinterpret_cast<double*>(base + p.o_val);
+  for (int j = 0; j < d.nsl; ++j) {
+    const int2 sl = slices[j];
+    for (int q = threadIdx.x; q < 32 * sl.y; q += blockDim.x) {
+      const int k = q >> 5, lane = q & 31;
+      const int lr = perm[j * 32 + lane];
+      double v = 0.0;
+      if (lr != 0xFFFF) {
+        const int r = d.r0 + lr;
+        const int s = rowptr[r];
+        if (k < rowptr[r + 1] - s) v = val[s + k];
+      }
+      o_val[sl.x + q] = v;
+    }
+  }
+}
+
+amg_status build_resetup_maps(amg_handle_s* H, cudaStream_t st) {
+  const int Lc = (int)H->lv.size() - 1;
+  Level& L0 = H->lv[0];
+  AMG_ALLOC(H, L0.src0, int, L0.nnz, st);
+  k_build_src0<<<grid_for(L0.n), TPB, 0, st>>>(L0.n, L0.rowptr, L0.col, L0.inv, H->nat_rowptr, H->nat_col, L0.src0);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  for (int l = 0; l < Lc; ++l) {
+    Level& L = H->lv[l];
+    Level& C = H->lv[l + 1];
+    int *tgt, *cnt;
+    AMG_ALLOC(H, tgt, int, L.nnz, st);
+    AMG_ALLOC(H, cnt, int, C.nnz + 1, st);
+    AMG_ALLOC(H, L.contrib_ptr, int, C.nnz + 1, st);
+    AMG_ALLOC(H, L.contrib_idx, int, L.nnz, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(cnt, 0, sizeof(int) * (C.nnz + 1), st));
+    k_rap_target<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.agg, C.rowptr, C.col, tgt, cnt);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_TRY(amg_exclusive_scan(H, cnt, L.contrib_ptr, C.nnz, st));
+    AMG_CUDA_TRY(H, cudaMemsetAsync(cnt, 0, sizeof(int) * (C.nnz + 1), st));
+    k_contrib_fill<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, tgt, L.contrib_ptr, cnt, L.contrib_idx);
+    k_contrib_sort<<<grid_for(C.nnz), TPB, 0, st>>>(C.nnz, L.contrib_ptr, L.contrib_idx);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, tgt);
+    amg_dev_free(H, cnt);
+  }
+  H->have_maps = true;
+  return AMG_OK;
+}
+
+}  // namespace
+
+amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fallback, cudaStream_t st) {
+  *fallback = 0;
+  const amg_options& o = H->opt;
+  const int n0 = (int)H->n, nnz0 = (int)H->nnz;
+  const int Lc = (int)H->lv.size() - 1;
+  // ---- the new values must keep the CSR valid; symmetric = -1 repeats the device check ----
+  {
+    int* bad;
+    AMG_ALLOC(H, bad, int, 2, st);
+    AMG_CUDA_TRY(H, cudaMemsetAsync(bad, 0, 2 * sizeof(int), st));
+    k_validate_csr<<<grid_for(n0), TPB, 0, st>>>(n0, nnz0, H->nat_rowptr, H->nat_col, d_val, bad);
+    if (o.symmetric < 0) k_check_symmetric<<<grid_for(n0), TPB, 0, st>>>(n0, H->nat_rowptr, H->nat_col, d_val, bad + 1);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    int h_bad[2] = {0, 0};
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_bad, bad, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    amg_dev_free(H, bad);
+    if (h_bad[0]) {
+      H->err = "bad CSR: the new values must keep a positive diagonal in every row";
+      return AMG_ERR_BAD_CSR;
+    }
+    const int sym = o.symmetric < 0 ? (h_bad[1] ? 0 : 1) : o.symmetric;
+    if (sym != H->symmetric) {  // symmetric <-> nonsymmetric: the matching and the transposed hierarchy change
+      *fallback = 1;
+      return AMG_OK;
+    }
+  }
+  const double t0 = now_ms();
+  if (!H->have_maps) AMG_TRY(build_resetup_maps(H, st));
+  // ---- values of every level: gather on level 0, numeric Galerkin below ----
+  Level& L0 = H->lv[0];
+  k_gather_vals<<<grid_for(L0.nnz), TPB, 0, st>>>(L0.nnz, d_val, L0.src0, L0.val);
+  for (int l = 0; l < Lc; ++l) {
+    Level& L = H->lv[l];
+    Level& C = H->lv[l + 1];
+    k_rap_numeric<<<grid_for(C.nnz), TPB, 0, st>>>(C.nnz, L.contrib_ptr, L.contrib_idx, L.val, C.val);
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  // ---- smoother diagonals, blob value sections, transposed values ----
+  for (int l = 0; l <= Lc; ++l) {
+    Level& L = H->lv[l];
+    if (l < Lc) k_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, o.smoother, o.omega, L.dinv);
+    if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.val, L.blob);
+    if (H->have_T) {
+      k_gather_vals<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, L.val, L.T.src, L.T.val);
+      if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.val, L.T.blob);
+    }
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  // ---- coarsest LU (factors rebuilt in place), dense tail ----
+  {
+    Level& L = H->lv[Lc];
+    AMG_TRY(dense_lu_of(H, L.n, L.rowptr, L.col, L.val, &H->lu, &H->piv, st));
+    if (H->have_T) AMG_TRY(dense_lu_of(H, L.n, L.T.rowptr, L.T.col, L.T.val, &H->luT, &H->pivT, st));
+  }
+  if (H->tail_dense_level >= 0) {
+    AMG_TRY(amg_setup_tail(H, 0, st));
+    if (H->have_T) AMG_TRY(amg_setup_tail(H, 1, st));
+  }
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  H->stats.total_ms = now_ms() - t0;
+  H->stats.aggregate_ms = H->stats.galerkin_ms = H->stats.reorder_ms = 0.0;
+  return AMG_OK;
 }

@@ -133,3 +133,81 @@ def test_lru_cache_of_hierarchies(oracle_mod, B):
         assert hit == 0
     finally:
         B.amg_cache_destroy(c)
+
+
+def test_warm_resetup_keeps_graphs_batches_and_the_transposed_hierarchy(oracle_mod, B):
+    """NEXT-1 warm path: amg_resetup_values(keep_aggregates = 1) rewrites values only.  Repeated resetups on one
+    handle (A0 -> A1 -> A2 -> A0), each followed by single solves (cached CUDA graphs), a batched solve (cached
+    work vectors / ring geometry) -- against the oracle built on the same values with the kept aggregates."""
+    shape = (24, 24, 24)
+    mats = [inputs.variable_diffusion_csr(shape, seed=s, sigma=1.5, ell=4.0) for s in (81, 82, 83)]
+    A0 = mats[0]
+    n = A0.n
+    s = B.AmgSolver(A0.rowptr, A0.col, A0.val)
+    o0 = oracle_mod.Oracle(A0.rowptr, A0.col, A0.val)
+    aggs = [o0.aggregates(l) for l in range(o0.num_levels - 1)]
+    b = inputs.rhs_uniform(n, 5)
+    Bh = np.stack([inputs.rhs_uniform(n, 50 + k) for k in range(8)])
+    Bd = torch.as_tensor(Bh).cuda().contiguous()
+    X = torch.empty_like(Bd)
+    x_first, _ = s.solve(b, 1e-8, 500, 0)
+    B.amg_solve_batched(s.h, 0, Bd, X, 8, n, 1e-8, 500)
+    try:
+        for A in (mats[1], mats[2], mats[0]):
+            s.resetup_values(A.val, keep_aggregates=True)
+            o = oracle_mod.Oracle(A.rowptr, A.col, A.val, aggregates=aggs)
+            for l in range(s.num_levels):
+                _, _, vg = s.level_csr(l)
+                _, _, vo = o.level_csr(l)
+                assert np.max(np.abs(vg.cpu().numpy() - vo)) <= 1e-13 * np.max(np.abs(vo)), l
+            r = np.random.default_rng(9).standard_normal(n)
+            assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+            for krylov in (0, 1):
+                xg, ig = s.solve(b, 1e-8, 500, krylov)
+                xo, io = o.solve(b, 1e-8, 500, krylov, 1)
+                assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+                assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+            infos = B.amg_solve_batched(s.h, 0, Bd, X, 8, n, 1e-8, 500)
+            for k in (0, 5):
+                xo, io = o.solve(Bh[k], 1e-8, 500, 0, 1)
+                assert infos[k].status == 0 and abs(infos[k].iterations - io.iterations) <= 2
+                assert np.linalg.norm(Bh[k] - A.to_scipy() @ X[k].cpu().numpy()) <= 1e-8 * np.linalg.norm(Bh[k])
+            o.close()
+        # back on the first values: the first solution again, bitwise (nothing structural moved)
+        x_again, _ = s.solve(b, 1e-8, 500, 0)
+        assert rel(x_again.cpu().numpy(), x_first.cpu().numpy()) <= 1e-12
+    finally:
+        s.close()
+        o0.close()
+
+
+def test_warm_resetup_of_a_nonsymmetric_handle(oracle_mod, B):
+    A0 = inputs.stretched_channel_csr((10, 16, 12), 2.0)
+    A1 = inputs.stretched_channel_csr((10, 16, 12), 1.2)  # same pattern, other stretching: new values
+    assert np.array_equal(A0.col, A1.col)
+    s = B.AmgSolver(A0.rowptr, A0.col, A0.val)
+    o0 = oracle_mod.Oracle(A0.rowptr, A0.col, A0.val, symmetric=0)
+    aggs = [o0.aggregates(l) for l in range(o0.num_levels - 1)]
+    g = inputs.rhs_uniform(A0.n, 3)
+    s.solve_transpose(g, 1e-8, 300)
+    s.resetup_values(A1.val, keep_aggregates=True)
+    o1 = oracle_mod.Oracle(A1.rowptr, A1.col, A1.val, aggregates=aggs, symmetric=0)
+    try:
+        assert s.symmetric == 0
+        rows = s.level_info(1)[0]
+        x = np.random.default_rng(2).standard_normal(rows)
+        import scipy.sparse as sp
+
+        rp, cl, vl = o1.level_csr(1)
+        A1c = sp.csr_matrix((vl, cl, rp), shape=(rows, rows))
+        assert rel(s.level_op(1, 7, x, None, rows).cpu().numpy(), A1c.T @ x) <= 1e-13
+        r = np.random.default_rng(4).standard_normal(A0.n)
+        assert rel(s.level_op(0, 8, None, r, A0.n).cpu().numpy(), o1.vcycle_transpose(r, 0)) <= 1e-12
+        lam, il = s.solve_transpose(g, 1e-8, 300)
+        lo, ilo = o1.solve_transpose(g, 1e-8, 300, 1, 1, 0)
+        assert il.status == ilo.status == 0 and abs(il.iterations - ilo.iterations) <= 2
+        assert np.linalg.norm(g - A1.to_scipy().T @ lam.cpu().numpy()) <= 1e-8 * np.linalg.norm(g)
+    finally:
+        s.close()
+        o0.close()
+        o1.close()
