@@ -240,4 +240,5 @@ void amg_batch_release(amg_handle_s* H);
 // setup.cu: transposed level operators, their tile blobs, LU of A_L^T, dense tail of B^T
 amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st);
 // setup.cu: NEXT-1 value-only resetup on the kept hierarchy; *fallback = 1: the caller has to rebuild (symmetry changed)
+amg_status amg_ensure_src0(amg_handle_s* H, cudaStream_t st);
 amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fallback, cudaStream_t st);

@@ -879,12 +879,14 @@ static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const
                                                              const int* __restrict__ inv, double* __restrict__ r,
                                                              double* __restrict__ x, double* __restrict__ z0,
                                                              double* __restrict__ z1, double* __restrict__ rhat,
+                                                             const double* __restrict__ dinv, double* __restrict__ x1,
                                                              double* partials, unsigned* counter, KrylovCtl* ctl,
                                                              int fin) {
   double acc[1] = {0.0};
   for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
     const double v = b_nat[inv[i]];
     r[i] = v;
+    if (x1) x1[i] = dinv[i] * v;  // first sweep from zero of the V-cycle this solve starts with (PCG: on r)
     x[i] = 0.0;
     if (z0) z0[i] = 0.0;
     if (z1) z1[i] = 0.0;
@@ -916,12 +918,17 @@ static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const doubl
 // x += alpha p ; r -= alpha q ; ||r||^2
 static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const double* __restrict__ p,
                                                         const double* __restrict__ q, double* __restrict__ x,
-                                                        double* __restrict__ r, double* partials, unsigned* counter,
+                                                        double* __restrict__ r, const double* __restrict__ dinv,
+                                                        double* __restrict__ x1, double* partials, unsigned* counter,
                                                         KrylovCtl* ctl) {
   pdl_sync();
   if (ctl->done) return;
   const double alpha = ctl->alpha;
   double acc[1] = {0.0};
+  // x1 = dinv o r (optional): the first sweep from zero of the V-cycle that follows, so that its level-0 pair of
+  // sweeps is a plain sweep on x1 (one gather per halo column instead of two)
+  const double2* d2 = reinterpret_cast<const double2*>(dinv);
+  double2* y2 = reinterpret_cast<double2*>(x1);
   // 128-bit accesses, two independent pairs per thread and trip (the work vectors are 16-byte aligned)
   const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
   const double2* p2 = reinterpret_cast<const double2*>(p);
@@ -935,6 +942,10 @@ static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const doub
     xa.x += alpha * pa.x, xa.y += alpha * pa.y, xb.x += alpha * pb.x, xb.y += alpha * pb.y;
     ra.x -= alpha * qa.x, ra.y -= alpha * qa.y, rb.x -= alpha * qb.x, rb.y -= alpha * qb.y;
     x2[i] = xa, x2[i + stride] = xb, r2[i] = ra, r2[i + stride] = rb;
+    if (x1) {
+      const double2 da = d2[i], db = d2[i + stride];
+      y2[i] = make_double2(da.x * ra.x, da.y * ra.y), y2[i + stride] = make_double2(db.x * rb.x, db.y * rb.y);
+    }
     acc[0] += (ra.x * ra.x + ra.y * ra.y) + (rb.x * rb.x + rb.y * rb.y);
   }
   for (; i < n2; i += stride) {
@@ -943,12 +954,17 @@ static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr(int n, const doub
     xa.x += alpha * pa.x, xa.y += alpha * pa.y;
     ra.x -= alpha * qa.x, ra.y -= alpha * qa.y;
     x2[i] = xa, r2[i] = ra;
+    if (x1) {
+      const double2 da = d2[i];
+      y2[i] = make_double2(da.x * ra.x, da.y * ra.y);
+    }
     acc[0] += ra.x * ra.x + ra.y * ra.y;
   }
   if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
     x[n - 1] += alpha * p[n - 1];
     const double ri = r[n - 1] - alpha * q[n - 1];
     r[n - 1] = ri;
+    if (x1) x1[n - 1] = dinv[n - 1] * ri;
     acc[0] += ri * ri;
   }
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, FIN_RR);
@@ -965,28 +981,66 @@ static __global__ void __launch_bounds__(RED_THREADS) k_dot(int n, const double*
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, fin);
 }
 
-// p = r + beta (p - omega v)
+// p = r + beta (p - omega v) ; optional x1 = dinv o p (first sweep from zero of the V-cycle on p)
 static __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ p,
+                                                        const double* __restrict__ dinv, double* __restrict__ x1,
                                                         const KrylovCtl* ctl) {
   pdl_sync();
   if (ctl->done) return;
   const double beta = ctl->beta, omega = ctl->omega;
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS)
-    p[i] = r[i] + beta * (p[i] - omega * v[i]);
+  const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;  // 128-bit accesses
+  const double2* r2 = reinterpret_cast<const double2*>(r);
+  const double2* v2 = reinterpret_cast<const double2*>(v);
+  const double2* d2 = reinterpret_cast<const double2*>(dinv);
+  double2* p2 = reinterpret_cast<double2*>(p);
+  double2* y2 = reinterpret_cast<double2*>(x1);
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n2; i += stride) {
+    const double2 rv = r2[i], vv = v2[i];
+    double2 pv = p2[i];
+    pv.x = rv.x + beta * (pv.x - omega * vv.x), pv.y = rv.y + beta * (pv.y - omega * vv.y);
+    p2[i] = pv;
+    if (x1) {
+      const double2 dv = d2[i];
+      y2[i] = make_double2(dv.x * pv.x, dv.y * pv.y);
+    }
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+    const double pi = r[n - 1] + beta * (p[n - 1] - omega * v[n - 1]);
+    p[n - 1] = pi;
+    if (x1) x1[n - 1] = dinv[n - 1] * pi;
+  }
 }
 
-// s = r - alpha v ; ||s||^2
+// s = r - alpha v ; ||s||^2 ; optional x1 = dinv o s
 static __global__ void __launch_bounds__(RED_THREADS) k_bicg_s(int n, const double* __restrict__ r,
                                                         const double* __restrict__ v, double* __restrict__ s,
+                                                        const double* __restrict__ dinv, double* __restrict__ x1,
                                                         double* partials, unsigned* counter, KrylovCtl* ctl) {
   pdl_sync();
   if (ctl->done) return;
   const double alpha = ctl->alpha;
   double acc[1] = {0.0};
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
-    const double si = r[i] - alpha * v[i];
-    s[i] = si;
+  const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* r2 = reinterpret_cast<const double2*>(r);
+  const double2* v2 = reinterpret_cast<const double2*>(v);
+  const double2* d2 = reinterpret_cast<const double2*>(dinv);
+  double2* s2 = reinterpret_cast<double2*>(s);
+  double2* y2 = reinterpret_cast<double2*>(x1);
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n2; i += stride) {
+    const double2 rv = r2[i], vv = v2[i];
+    const double2 sv = make_double2(rv.x - alpha * vv.x, rv.y - alpha * vv.y);
+    s2[i] = sv;
+    if (x1) {
+      const double2 dv = d2[i];
+      y2[i] = make_double2(dv.x * sv.x, dv.y * sv.y);
+    }
+    acc[0] += sv.x * sv.x + sv.y * sv.y;
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+    const double si = r[n - 1] - alpha * v[n - 1];
+    s[n - 1] = si;
+    if (x1) x1[n - 1] = dinv[n - 1] * si;
     acc[0] += si * si;
   }
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, FIN_SS);
@@ -1002,12 +1056,29 @@ static __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const dou
   if (ctl->done) return;
   const double alpha = ctl->alpha, omega = ctl->omega;
   double acc[2] = {0.0, 0.0};
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
-    x[i] += alpha * ph[i] + omega * sh[i];
-    const double ri = s[i] - omega * t[i];
-    r[i] = ri;
+  const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* ph2 = reinterpret_cast<const double2*>(ph);
+  const double2* sh2 = reinterpret_cast<const double2*>(sh);
+  const double2* s2 = reinterpret_cast<const double2*>(s);
+  const double2* t2 = reinterpret_cast<const double2*>(t);
+  const double2* rh2 = reinterpret_cast<const double2*>(rhat);
+  double2* x2 = reinterpret_cast<double2*>(x);
+  double2* r2 = reinterpret_cast<double2*>(r);
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n2; i += stride) {
+    const double2 pv = ph2[i], hv = sh2[i], sv = s2[i], tv = t2[i], qv = rh2[i];
+    double2 xv = x2[i];
+    xv.x += alpha * pv.x + omega * hv.x, xv.y += alpha * pv.y + omega * hv.y;
+    const double2 rv = make_double2(sv.x - omega * tv.x, sv.y - omega * tv.y);
+    x2[i] = xv, r2[i] = rv;
+    acc[0] += rv.x * rv.x + rv.y * rv.y;
+    acc[1] += qv.x * rv.x + qv.y * rv.y;
+  }
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+    x[n - 1] += alpha * ph[n - 1] + omega * sh[n - 1];
+    const double ri = s[n - 1] - omega * t[n - 1];
+    r[n - 1] = ri;
     acc[0] += ri * ri;
-    acc[1] += rhat[i] * ri;
+    acc[1] += rhat[n - 1] * ri;
   }
   grid_reduce_finalize<2, RED_THREADS>(acc, partials, counter, ctl, FIN_RR_RHO);
 }
@@ -1050,6 +1121,34 @@ static __global__ void __launch_bounds__(256) k_grad_values(int n, const int* __
     double s = 0.0;
     for (int b = 0; b < nrhs; ++b) s += __ldg(lam + (size_t)b * ld + i) * __ldg(x + (size_t)b * ld + j);
     gA[k] = accumulate ? gA[k] - s : -s;
+  }
+}
+
+// Single right-hand side, short rows: ONE thread per row, the row's entries in chunks of 8 whose loads are
+// all issued before any is used (the lanes-per-row kernel above keeps one dependent chain rowptr -> col -> x ->
+// store per thread and is bound by that latency: 1.7 TB/s; here a thread has up to 8 gathers in flight).
+static __global__ void __launch_bounds__(256) k_grad_values_rows(int n, const int* __restrict__ rowptr,
+                                                                 const int* __restrict__ col,
+                                                                 const double* __restrict__ lam,
+                                                                 const double* __restrict__ x, double* __restrict__ gA,
+                                                                 int accumulate) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int k0 = __ldg(rowptr + i), k1 = __ldg(rowptr + i + 1);
+  const double li = __ldg(lam + i);
+  for (int k = k0; k < k1; k += 8) {
+    int j[8];
+    double xv[8], old[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) j[u] = k + u < k1 ? __ldg(col + k + u) : -1;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      xv[u] = j[u] >= 0 ? __ldg(x + j[u]) : 0.0;
+      old[u] = (accumulate && j[u] >= 0) ? gA[k + u] : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+      if (j[u] >= 0) gA[k + u] = old[u] - li * xv[u];
   }
 }
 

@@ -1548,10 +1548,7 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
 
 amg_status build_resetup_maps(amg_handle_s* H, cudaStream_t st) {
   const int Lc = (int)H->lv.size() - 1;
-  Level& L0 = H->lv[0];
-  AMG_ALLOC(H, L0.src0, int, L0.nnz, st);
-  k_build_src0<<<grid_for(L0.n), TPB, 0, st>>>(L0.n, L0.rowptr, L0.col, L0.inv, H->nat_rowptr, H->nat_col, L0.src0);
-  AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_ensure_src0(H, st));
   for (int l = 0; l < Lc; ++l) {
     Level& L = H->lv[l];
     Level& C = H->lv[l + 1];
@@ -1577,6 +1574,16 @@ amg_status build_resetup_maps(amg_handle_s* H, cudaStream_t st) {
 }
 
 }  // namespace
+
+// level 0: position in the caller's CSR of every entry of the permuted CSR (warm resetup, tile gradient)
+amg_status amg_ensure_src0(amg_handle_s* H, cudaStream_t st) {
+  Level& L0 = H->lv[0];
+  if (L0.src0) return AMG_OK;
+  AMG_ALLOC(H, L0.src0, int, L0.nnz, st);
+  k_build_src0<<<grid_for(L0.n), TPB, 0, st>>>(L0.n, L0.rowptr, L0.col, L0.inv, H->nat_rowptr, H->nat_col, L0.src0);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
 
 amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fallback, cudaStream_t st) {
   *fallback = 0;

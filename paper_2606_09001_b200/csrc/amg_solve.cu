@@ -376,9 +376,14 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
 // ------------------------------------------------------------------------------------------
 namespace {
 
-struct IterPlan {
-  int krylov, precond;
-};
+// buffer that receives x1 = dinv o b of level 0 from the kernel that produces b (so that the first two
+// sweeps of the V-cycle are one plain sweep on x1), or null when the cycle does not start that way
+double* l0_x1(amg_handle_s* H, int precond) {
+  Level& L0 = H->lv[0];
+  const int Lc = (int)H->lv.size() - 1;
+  if (!precond || Lc == 0 || H->tail_dense_level == 0 || H->opt.pre_sweeps < 2 || !lv_fast(L0)) return nullptr;
+  return L0.x2;
+}
 
 // one PCG iteration: q = A p, sigma; x,r update; z = B r, rho; p = z + beta p
 amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) {
@@ -386,10 +391,11 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *q = H->kv[3];
   op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
-  ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, L0.dinv, l0_x1(H, precond), H->partials,
+                                                                        H->counter, H->ctl);
   double* z = r;
   if (precond) {
-    AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st));
+    AMG_TRY(amg_vcycle(H, 0, r, &z, H->ctl, true, st, l0_x1(H, precond) != nullptr));
   } else {
     ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
   }
@@ -403,20 +409,21 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4], *s = H->kv[5],
          *t = H->kv[6], *ph = H->kv[7];
-  ++g_nlaunch, launch(k_bicg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, p, H->ctl);
+  ++g_nlaunch, launch(k_bicg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, p, L0.dinv, l0_x1(H, precond), H->ctl);
   double* phat = p;
   if (precond) {
     double* zz = nullptr;
     H->vcycle_final_out = ph;
-    const amg_status sv = amg_vcycle(H, 0, p, &zz, H->ctl, false, st);
+    const amg_status sv = amg_vcycle(H, 0, p, &zz, H->ctl, false, st, l0_x1(H, precond) != nullptr);
     H->vcycle_final_out = nullptr;
     AMG_TRY(sv);
     phat = zz;  // == ph on every path of the cycle: the second V-cycle of this iteration may overwrite the level-0 buffers
   }
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
-  ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, H->partials, H->counter, H->ctl);
+  ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, L0.dinv, l0_x1(H, precond), H->partials,
+                                                                        H->counter, H->ctl);
   double* shat = s;
-  if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st));
+  if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st, l0_x1(H, precond) != nullptr));
   op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
   ++g_nlaunch, launch(k_bicg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
                                                    H->ctl);
@@ -431,7 +438,7 @@ amg_status enqueue_iteration(amg_handle_s* H, int krylov, int precond, cudaStrea
 // the start of an AMG-PCG solve after k_krylov_init: z = B r (r.z on the last sweep), p = z
 amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
   double* z = nullptr;
-  AMG_TRY(amg_vcycle(H, 0, H->kv[1], &z, H->ctl, true, st));
+  AMG_TRY(amg_vcycle(H, 0, H->kv[1], &z, H->ctl, true, st, l0_x1(H, 1) != nullptr));
   ++g_nlaunch, launch(k_pcg_p, red_grid(H, H->lv[0].n), RED_THREADS, 0, st)(H->lv[0].n, z, H->kv[2], H->ctl);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
@@ -520,8 +527,8 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   H->h_ctl[5] = init;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
   if (krylov == 0) {
-    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, H->partials,
-                                                         H->counter, H->ctl, FIN_INIT_PCG);
+    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, L0.dinv,
+                                                         l0_x1(H, precond), H->partials, H->counter, H->ctl, FIN_INIT_PCG);
     if (precond && H->opt.use_graph && maxit > 0) {
       cudaGraphExec_t gstart = nullptr;
       AMG_TRY(get_iteration_graph(H, -1, 1, st, &gstart));
@@ -534,8 +541,8 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
       ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, p, H->ctl);
     }
   } else {
-    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, H->partials, H->counter,
-                                                         H->ctl, FIN_INIT_BICG);
+    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, nullptr, nullptr,
+                                                         H->partials, H->counter, H->ctl, FIN_INIT_BICG);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
 
@@ -766,7 +773,9 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
     H->last_launches = 2;
     return AMG_OK;
   }
-  if (mean <= 12.0) {
+  if (mean <= 12.0 && nrhs == 1) {
+    ++g_nlaunch, launch(k_grad_values_rows, div_up(n, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, d_gA, accumulate);
+  } else if (mean <= 12.0) {
     const int64_t threads = (int64_t)n * 8;
     ++g_nlaunch, launch(k_grad_values<8>, div_up(threads, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, nrhs, ld,
                                                           d_gA, accumulate);

@@ -289,12 +289,14 @@ def test_adjoint_gradients(cases, name):
     assert rel(acc.cpu().numpy(), gO2) <= 1e-14
 
 
-@pytest.mark.parametrize("nrhs", [2, 4, 5, 8, 16])
+@pytest.mark.parametrize("generic", [0, 1])
+@pytest.mark.parametrize("nrhs", [1, 2, 4, 5, 8, 16])
 @pytest.mark.parametrize("name", ["cfg3_40", "cfg4_28"])
-def test_grad_values_batched_kernel(cases, B, name, nrhs):
-    """G2 with several right-hand sides (interleaved-X kernel, compile-time and generic nrhs), a leading
-    dimension larger than n, and accumulation: gA[k] = -sum_s lambda_s[i] x_s[col[k]] (Eq. 2 on the pattern)."""
-    c = cases(name)
+def test_grad_values_batched_kernel(cases, B, name, nrhs, generic):
+    """G2 with several right-hand sides, a leading dimension larger than n, and accumulation:
+    gA[k] = -sum_s lambda_s[i] x_s[col[k]] (Eq. 2 on the pattern): the natural-ordering kernels (interleaved X,
+    compile-time and generic nrhs) on both kinds of hierarchy."""
+    c = cases(name, force_generic=1) if generic else cases(name)
     n, ld = c.A.n, c.A.n + 37
     rng = np.random.default_rng(300 + nrhs)
     lam = np.zeros((nrhs, ld))
