@@ -151,9 +151,10 @@ struct amg_handle_s {
   double* tail_dense_BT = nullptr;   // the same for the transposed hierarchy
   // CUDA graph of one Krylov iteration (keyed by krylov/precond)
   // [krylov * 2 + precond]: one iteration; [4]: the start of an AMG-PCG solve (first V-cycle + p = z)
-  // [5]: one BiCGSTAB + AMG iteration on the transposed hierarchy
-  cudaGraphExec_t graph_exec[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  int64_t graph_launches[6] = {0, 0, 0, 0, 0, 0};  // kernel nodes per replay
+  // [5]: one BiCGSTAB + AMG iteration on the transposed hierarchy; [6]: one V-cycle (amg_apply_preconditioner)
+  cudaGraphExec_t graph_exec[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  int64_t graph_launches[7] = {0, 0, 0, 0, 0, 0, 0};  // kernel nodes per replay
+  double* apply_out = nullptr;               // result buffer of the captured V-cycle
   double* vcycle_final_out = nullptr;        // if set: the last post-sweep of a cycle started at level 0 writes here
   int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};

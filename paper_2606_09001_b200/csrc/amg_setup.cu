@@ -1096,10 +1096,13 @@ struct TilePack {
   int nblk = 0, fast = 0;
 };
 
+// *scale_io: the target scale that fitted the level above (the halo share grows from level to level, so the
+// search starts a little above it instead of at 1: one attempt per level instead of two or three)
 amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
-                      const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st) {
+                      const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st,
+                      double* scale_io = nullptr) {
   const int64_t total_w = RT_NNZ_WEIGHT * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
-  double scale = 1.0;
+  double scale = scale_io ? (*scale_io * 1.12 < 1.0 ? *scale_io * 1.12 : 1.0) : 1.0;
   for (int attempt = 0; attempt < 6 && !P.fast; ++attempt) {
     const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
     if (target < 512) break;
@@ -1147,6 +1150,7 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
       AMG_CUDA_TRY(H, cudaGetLastError());
       AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
       P.fast = 1;
+      if (scale_io) *scale_io = scale;
     }
     amg_dev_free(H, size16);
     amg_dev_free(H, off16);
@@ -1323,6 +1327,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     amg_dev_free(H, sizep);
   }
+  double pack_scale = 1.0;
   for (int q = 0; q <= Lc; ++q) {
     Level& L = H->lv[q];
     const NatCsr& N = nat[q];
@@ -1341,7 +1346,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     if (!o.force_generic && L.n > 0) {
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
-                         q < Lc ? L.nc : 0, P, st));
+                         q < Lc ? L.nc : 0, P, st, &pack_scale));
       L.blk_ptr = P.blk_ptr, L.tiles = P.tiles, L.blob = P.blob, L.halo_idx = P.halo_idx, L.halo_cagg = P.halo_cagg;
       L.blob_bytes = P.blob_bytes, L.nblk = P.nblk, L.fast = P.fast;
     }

@@ -444,8 +444,20 @@ amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
   return AMG_OK;
 }
 
-// krylov < 0: the start graph (slot 4); g_tr: the transposed BiCGSTAB + AMG iteration (slot 5)
-inline int graph_slot(int krylov, int precond) { return krylov < 0 ? 4 : (g_tr ? 5 : krylov * 2 + precond); }
+// one V-cycle from level 0 on io_tmp2 (amg_apply_preconditioner): x1 = dinv o r, then the cycle
+amg_status enqueue_apply(amg_handle_s* H, cudaStream_t st) {
+  Level& L0 = H->lv[0];
+  double* x1 = l0_x1(H, 1);
+  if (x1) ++g_nlaunch, launch(k_scale_dinv, grid_for(L0.n), TPB, 0, st)(L0.n, L0.dinv, H->io_tmp2, x1, nullptr);
+  AMG_TRY(amg_vcycle(H, 0, H->io_tmp2, &H->apply_out, nullptr, false, st, x1 != nullptr));
+  return AMG_OK;
+}
+
+// krylov == -1: the start graph (slot 4); -2: amg_apply_preconditioner (slot 6); g_tr: the transposed BiCGSTAB +
+// AMG iteration (slot 5)
+inline int graph_slot(int krylov, int precond) {
+  return krylov == -2 ? 6 : (krylov < 0 ? 4 : (g_tr ? 5 : krylov * 2 + precond));
+}
 
 amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStream_t st, cudaGraphExec_t* out) {
   const int slot = graph_slot(krylov, precond);
@@ -459,7 +471,9 @@ amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStr
   AMG_CUDA_TRY(H, cudaStreamBeginCapture(H->cap_stream, cudaStreamCaptureModeThreadLocal));
   const int64_t launches0 = g_nlaunch;
   g_pdl = H->opt.use_pdl != 0;
-  amg_status s = krylov < 0 ? enqueue_pcg_start(H, H->cap_stream) : enqueue_iteration(H, krylov, precond, H->cap_stream);
+  amg_status s = krylov == -2 ? enqueue_apply(H, H->cap_stream)
+                 : krylov < 0 ? enqueue_pcg_start(H, H->cap_stream)
+                              : enqueue_iteration(H, krylov, precond, H->cap_stream);
   g_pdl = false;
   H->graph_launches[slot] = g_nlaunch - launches0;  // kernel nodes of one replay
   g_nlaunch = launches0;                            // capturing enqueues nothing
@@ -678,7 +692,18 @@ amg_status amg_level_op_impl(amg_handle_s* H, int level, int op, const double* d
       if (!d_in1) return AMG_ERR_INVALID_ARG;
       perm_in(L, d_in1, t1);
       double* z = nullptr;
-      for (int r = 0; r < reps; ++r) AMG_TRY(amg_vcycle(H, level, t1, &z, nullptr, false, st));
+      if (level == 0 && H->opt.use_graph && !g_tr) {
+        // the preconditioner itself: the cycle replayed as a PDL-chained graph, like inside a solve
+        cudaGraphExec_t gx = nullptr;
+        AMG_TRY(get_iteration_graph(H, -2, 1, st, &gx));
+        for (int r = 0; r < reps; ++r) {
+          AMG_CUDA_TRY(H, cudaGraphLaunch(gx, st));
+          g_nlaunch += H->graph_launches[6];
+        }
+        z = H->apply_out;
+      } else {
+        for (int r = 0; r < reps; ++r) AMG_TRY(amg_vcycle(H, level, t1, &z, nullptr, false, st));
+      }
       perm_out(L, z, d_out);
     } break;
     case 6: {  // prolongation-fused sweep: d_in1 = [b (rows of this level) | e_c (rows of the next)]

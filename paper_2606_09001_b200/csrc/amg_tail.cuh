@@ -255,7 +255,7 @@ static __global__ void __launch_bounds__(TAIL_THREADS, 1) k_dense_tail(TailArgs 
 // B[i][j] = (Vcycle_D e_j)_i, stored row-major, so that z = B r is exactly the V-cycle applied
 // to r up to the rounding of a different summation order.
 // ------------------------------------------------------------------------------------------
-constexpr int TAILB_THREADS = 256;
+constexpr int TAILB_THREADS = 1024;
 struct TailBuildArgs {
   const TailLevel* lv;
   int D, last, nu1, nu2;
