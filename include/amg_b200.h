@@ -29,10 +29,11 @@
  * one is installed, and is released by amg_destroy.
  *
  * STREAMS.  Every call enqueues its work on `cuda_stream` (a cudaStream_t passed as void*;
- * NULL = the legacy default stream) and returns after that work has completed (one
- * synchronisation at the end of a solve; none inside the Krylov loop, whose scalars and
- * convergence test live on the device: the host only waits on the event of the previous
- * iteration before it enqueues the next-but-one).  The iteration is replayed as a CUDA graph
+ * NULL = the legacy default stream).  A solve is: one init kernel, one graph whose conditional
+ * WHILE node repeats the iteration until the device-side convergence test says stop, one output
+ * kernel -- nothing of the loop involves the host.  With info != NULL the call then waits for
+ * the stream and reports; with info == NULL it returns at once (fully asynchronous).  Hooks,
+ * gradients and amg_get_aggregates are stream-ordered and do not synchronise.  Graphs are
  * captured on an internal stream and launched into `cuda_stream`.
  *
  * ERRORS.  Every function returns amg_status; no exception crosses the ABI.  On a failed
@@ -103,7 +104,10 @@ typedef struct {
   int32_t split_prolong_rows; /* levels with at least this many rows apply the coarse correction x += gamma P e_c
                                as its own unit-stride pass instead of fusing it into the first post-sweep
                                (the fused sweep gathers two values per halo column); default 800000, 0 = never */
-  int32_t reserved0;
+  int32_t use_while;        /* 1 = the whole Krylov loop is ONE graph launch: a conditional WHILE node whose body is one
+                               iteration, the loop condition set on the device from the convergence flag (no host
+                               polling, no surplus iteration); default 1; falls back to replaying the iteration
+                               graph under host control if the driver refuses the node; 0 = host-controlled loop   */
   double omega;             /* damped Jacobi weight, default 2/3                                         */
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */

@@ -36,7 +36,7 @@ class amg_options(C.Structure):
                 ("coarse_max_rows", C.c_int32), ("max_levels", C.c_int32),
                 ("max_match_rounds", C.c_int32), ("force_generic", C.c_int32),
                 ("use_graph", C.c_int32), ("tail_dense_rows", C.c_int32), ("use_pdl", C.c_int32),
-                ("split_prolong_rows", C.c_int32), ("reserved0", C.c_int32),
+                ("split_prolong_rows", C.c_int32), ("use_while", C.c_int32),
                 ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double), ("hash_seed", C.c_uint64)]
 

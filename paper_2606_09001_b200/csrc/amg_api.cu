@@ -204,6 +204,7 @@ amg_status amg_options_default(amg_options* o) {
   o->tail_dense_rows = 2304;
   o->use_pdl = 1;
   o->split_prolong_rows = 800000;
+  o->use_while = 1;
   o->omega = 2.0 / 3.0;
   o->strong_beta = 0.25;
   o->coarse_scale = 1.0;

@@ -20,8 +20,9 @@ struct AmgBatch {
   double* partials = nullptr;
   int partials_cap = 0;
   unsigned* counter = nullptr;
-  cudaGraphExec_t g_start = nullptr, g_iter = nullptr;
+  cudaGraphExec_t g_start = nullptr, g_iter = nullptr, g_while = nullptr;  // g_while: the loop as one WHILE-node graph
   int64_t nl_start = 0, nl_iter = 0;
+  bool while_failed = false;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
@@ -29,6 +30,7 @@ namespace {
 
 thread_local int64_t gb_nlaunch = 0;
 thread_local bool gb_pdl = false;
+thread_local cudaGraphConditionalHandle gb_loop = 0;  // != 0 while the body of a WHILE node is captured
 
 template <typename... KArgs, typename... A>
 void launch_b(void (*k)(KArgs...), dim3 g, dim3 b, size_t sm, cudaStream_t st, A&&... a) {
@@ -145,7 +147,7 @@ amg_status enqueue_start_b(amg_handle_s* H, cudaStream_t st) {
   AMG_TRY(vcycle_b(H, 0, Bt.kv[1], &z, Bt.ctl, true, st));
   const int n = H->lv[0].n;
   launch_b(k_pcg_p_b, red_grid_b(H, (int64_t)n * NB2), RED_THREADS, 0, st, n, (const double*)z, Bt.kv[2],
-           (const KrylovCtlB*)Bt.ctl);
+           (const KrylovCtlB*)Bt.ctl, (cudaGraphConditionalHandle)0);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -170,7 +172,7 @@ amg_status enqueue_iteration_b(amg_handle_s* H, cudaStream_t st) {
   double* z = nullptr;
   AMG_TRY(vcycle_b(H, 0, r, &z, Bt.ctl, true, st));
   launch_b(k_pcg_p_b, red_grid_b(H, (int64_t)n * NB2), RED_THREADS, 0, st, n, (const double*)z, p,
-           (const KrylovCtlB*)Bt.ctl);
+           (const KrylovCtlB*)Bt.ctl, gb_loop);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -197,6 +199,40 @@ amg_status capture_b(amg_handle_s* H, bool start, cudaGraphExec_t* out, int64_t*
   return AMG_OK;
 }
 
+// the whole loop as one graph: conditional WHILE node, body = one batched iteration (see get_while_graph)
+bool capture_while_b(amg_handle_s* H, cudaGraphExec_t* out) {
+  if (!H->cap_stream && cudaStreamCreateWithFlags(&H->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
+  cudaGraph_t g = nullptr;
+  bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
+  cudaGraphConditionalHandle hd = 0;
+  ok = ok && cudaGraphConditionalHandleCreate(&hd, g, 1, cudaGraphCondAssignDefault) == cudaSuccess;
+  cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+  np.conditional.handle = hd;
+  np.conditional.type = cudaGraphCondTypeWhile;
+  np.conditional.size = 1;
+  cudaGraphNode_t node = nullptr;
+  ok = ok && cudaGraphAddNode(&node, g, nullptr, 0, &np) == cudaSuccess;
+  if (ok) {
+    ok = cudaStreamBeginCaptureToGraph(H->cap_stream, np.conditional.phGraph_out[0], nullptr, nullptr, 0,
+                                       cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+      const int64_t l0 = gb_nlaunch;
+      gb_pdl = H->opt.use_pdl != 0;
+      gb_loop = hd;
+      const amg_status s = enqueue_iteration_b(H, H->cap_stream);
+      gb_loop = 0;
+      gb_pdl = false;
+      gb_nlaunch = l0;
+      cudaGraph_t cap = nullptr;
+      ok = cudaStreamEndCapture(H->cap_stream, &cap) == cudaSuccess && s == AMG_OK;
+    }
+  }
+  ok = ok && cudaGraphInstantiate(out, g, 0) == cudaSuccess;
+  if (g) cudaGraphDestroy(g);
+  if (!ok) cudaGetLastError();
+  return ok;
+}
+
 }  // namespace
 
 void amg_batch_release(amg_handle_s* H) {  // device memory is tracked by the handle (amg_free_all)
@@ -204,6 +240,7 @@ void amg_batch_release(amg_handle_s* H) {  // device memory is tracked by the ha
   if (!B) return;
   if (B->g_start) cudaGraphExecDestroy(B->g_start);
   if (B->g_iter) cudaGraphExecDestroy(B->g_iter);
+  if (B->g_while) cudaGraphExecDestroy(B->g_while);
   for (auto& e : B->ev)
     if (e) cudaEventDestroy(e);
   if (B->h_ctl) cudaFreeHost(B->h_ctl);
@@ -298,8 +335,16 @@ amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X
   } else if (maxit > 0) {
     AMG_TRY(enqueue_start_b(H, st));
   }
+  bool looped = false;
+  if (graph && H->opt.use_while && !B.while_failed) {
+    if (!B.g_while && !capture_while_b(H, &B.g_while)) B.while_failed = true, B.g_while = nullptr;
+    if (B.g_while) {
+      AMG_CUDA_TRY(H, cudaGraphLaunch(B.g_while, st));
+      looped = true;
+    }
+  }
   constexpr int NSLOT = 4, LAG = 1;
-  for (int it = 0; it < maxit; ++it) {
+  for (int it = 0; it < maxit && !looped; ++it) {
     if (graph) {
       AMG_CUDA_TRY(H, cudaGraphLaunch(B.g_iter, st));
       gb_nlaunch += B.nl_iter;
@@ -320,6 +365,11 @@ amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X
   if (!infos) return AMG_OK;
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&B.h_ctl[4], B.ctl, sizeof(KrylovCtlB), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  if (looped) {  // kernels the device-side loop launched
+    int itmax = 1;
+    for (int s = 0; s < NB; ++s) itmax = std::max(itmax, B.h_ctl[4].c[s].iter);
+    H->last_launches += (int64_t)itmax * B.nl_iter;
+  }
   for (int s = 0; s < ncols; ++s) {
     const KrylovCtl& c = B.h_ctl[4].c[s];
     infos[s].iterations = c.iter;

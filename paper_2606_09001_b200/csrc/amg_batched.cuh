@@ -538,8 +538,10 @@ static __global__ void __launch_bounds__(RED_THREADS) k_pcg_xr_b(int n, const do
 
 // p = z + beta_s p
 static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p_b(int n, const double* __restrict__ z, double* __restrict__ p,
-                                                         const KrylovCtlB* ctl) {
+                                                         const KrylovCtlB* ctl, cudaGraphConditionalHandle loop) {
   pdl_sync();
+  // the last kernel of an iteration: inside a conditional WHILE node it sets the loop condition (0 = outside)
+  if (loop != 0 && blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(loop, ctl->all_done ? 0u : 1u);
   if (ctl->all_done) return;
   const int h = threadIdx.x & (NB2 - 1);
   const double b0 = ctl->c[2 * h].beta, b1 = ctl->c[2 * h + 1].beta;

@@ -154,6 +154,10 @@ struct amg_handle_s {
   // [5]: one BiCGSTAB + AMG iteration on the transposed hierarchy; [6]: one V-cycle (amg_apply_preconditioner)
   cudaGraphExec_t graph_exec[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   int64_t graph_launches[7] = {0, 0, 0, 0, 0, 0, 0};  // kernel nodes per replay
+  // the Krylov loop as one graph with a conditional WHILE node ([krylov * 2 + precond], [4]: transposed BiCGSTAB)
+  cudaGraphExec_t while_exec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  int64_t while_launches[5] = {0, 0, 0, 0, 0};  // kernel nodes of the body
+  bool while_failed = false, while_used = false;
   double* apply_out = nullptr;               // result buffer of the captured V-cycle
   double* vcycle_final_out = nullptr;        // if set: the last post-sweep of a cycle started at level 0 writes here
   int64_t last_launches = 0;                 // kernels enqueued by the last solve / hook / gradient call

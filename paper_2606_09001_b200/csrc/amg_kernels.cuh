@@ -896,10 +896,12 @@ static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const
   grid_reduce_finalize<1, RED_THREADS>(acc, partials, counter, ctl, fin);
 }
 
-// p = z + beta p
+// p = z + beta p.  The last kernel of a PCG iteration: inside a conditional WHILE graph node it also sets the
+// loop condition (continue while the solve is not done; `loop` = 0 outside such a graph)
 static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p(int n, const double* __restrict__ z, double* __restrict__ p,
-                                                       const KrylovCtl* ctl) {
+                                                       const KrylovCtl* ctl, cudaGraphConditionalHandle loop) {
   pdl_sync();
+  if (loop != 0 && blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(loop, ctl->done ? 0u : 1u);
   if (ctl->done) return;
   const double beta = ctl->beta;
   const int64_t n2 = n / 2, stride = (int64_t)gridDim.x * RED_THREADS;
@@ -1081,6 +1083,13 @@ static __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(int n, const dou
     acc[1] += rhat[n - 1] * ri;
   }
   grid_reduce_finalize<2, RED_THREADS>(acc, partials, counter, ctl, FIN_RR_RHO);
+}
+
+// loop condition of a conditional WHILE graph node whose body is one Krylov iteration (BiCGSTAB: its last kernel
+// finalises the convergence test itself, so the condition is set by this one-thread kernel after it)
+static __global__ void k_while_ctl(const KrylovCtl* ctl, cudaGraphConditionalHandle loop) {
+  pdl_sync();
+  cudaGraphSetConditional(loop, ctl->done ? 0u : 1u);
 }
 
 // x_out (natural numbering) = x [+ alpha * phat after a BiCGSTAB half-step exit]

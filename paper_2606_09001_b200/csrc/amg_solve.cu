@@ -13,6 +13,7 @@ namespace {
 thread_local int64_t g_nlaunch = 0;  // kernel launches enqueued by this thread (amg_get_last_launches)
 
 thread_local bool g_pdl = false;     // true while an iteration is being captured with programmatic edges
+thread_local cudaGraphConditionalHandle g_loop = 0;  // != 0 while the body of a WHILE node is being captured
 thread_local int g_tr = 0;           // 1: the level operators are the transposed ones (A_l^T, nonsymmetric adjoint)
 
 // kernel launch; with g_pdl the kernel may become resident while its predecessor drains
@@ -399,7 +400,7 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   } else {
     ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
   }
-  ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, z, p, H->ctl);
+  ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, z, p, H->ctl, g_loop);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -427,6 +428,7 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
   ++g_nlaunch, launch(k_bicg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
                                                    H->ctl);
+  if (g_loop) ++g_nlaunch, launch(k_while_ctl, 1, 1, 0, st)((const KrylovCtl*)H->ctl, g_loop);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -439,7 +441,7 @@ amg_status enqueue_iteration(amg_handle_s* H, int krylov, int precond, cudaStrea
 amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
   double* z = nullptr;
   AMG_TRY(amg_vcycle(H, 0, H->kv[1], &z, H->ctl, true, st, l0_x1(H, 1) != nullptr));
-  ++g_nlaunch, launch(k_pcg_p, red_grid(H, H->lv[0].n), RED_THREADS, 0, st)(H->lv[0].n, z, H->kv[2], H->ctl);
+  ++g_nlaunch, launch(k_pcg_p, red_grid(H, H->lv[0].n), RED_THREADS, 0, st)(H->lv[0].n, z, H->kv[2], H->ctl, (cudaGraphConditionalHandle)0);
   AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
 }
@@ -492,9 +494,68 @@ amg_status get_iteration_graph(amg_handle_s* H, int krylov, int precond, cudaStr
   return AMG_OK;
 }
 
+// The whole Krylov loop as ONE graph: a conditional WHILE node whose body is one iteration (PDL-chained
+// kernels); the body's last kernel sets the condition from the device-side convergence flag.  No host polling,
+// no copy between iterations, no surplus iteration.  Returns AMG_ERR_UNSUPPORTED (once, remembered) if the driver
+// refuses any step: the caller falls back to replaying the iteration graph under host control.
+amg_status get_while_graph(amg_handle_s* H, int krylov, int precond, cudaGraphExec_t* out) {
+  const int slot = g_tr ? 4 : krylov * 2 + precond;
+  if (H->while_exec[slot]) {
+    *out = H->while_exec[slot];
+    return AMG_OK;
+  }
+  if (H->while_failed) return AMG_ERR_UNSUPPORTED;
+  if (!H->cap_stream && cudaStreamCreateWithFlags(&H->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return AMG_ERR_CUDA;
+  cudaGraph_t g = nullptr;
+  cudaGraphExec_t ex = nullptr;
+  bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
+  cudaGraphConditionalHandle hd = 0;
+  ok = ok && cudaGraphConditionalHandleCreate(&hd, g, 1, cudaGraphCondAssignDefault) == cudaSuccess;
+  cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = hd;
+  np.conditional.type = cudaGraphCondTypeWhile;
+  np.conditional.size = 1;
+  cudaGraphNode_t node = nullptr;
+  ok = ok && cudaGraphAddNode(&node, g, nullptr, 0, &np) == cudaSuccess;
+  amg_status s = AMG_OK;
+  if (ok) {
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    ok = cudaStreamBeginCaptureToGraph(H->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) ==
+         cudaSuccess;
+    if (ok) {
+      const int64_t launches0 = g_nlaunch;
+      g_pdl = H->opt.use_pdl != 0;
+      g_loop = hd;
+      s = enqueue_iteration(H, krylov, precond, H->cap_stream);
+      g_loop = 0;
+      g_pdl = false;
+      H->while_launches[slot] = g_nlaunch - launches0;
+      g_nlaunch = launches0;
+      cudaGraph_t cap = nullptr;
+      ok = cudaStreamEndCapture(H->cap_stream, &cap) == cudaSuccess && s == AMG_OK;
+    }
+  }
+  ok = ok && cudaGraphInstantiate(&ex, g, 0) == cudaSuccess;
+  if (g) cudaGraphDestroy(g);
+  if (!ok) {
+    cudaGetLastError();
+    H->while_failed = true;
+    return s != AMG_OK ? s : AMG_ERR_UNSUPPORTED;
+  }
+  H->while_exec[slot] = ex;
+  *out = ex;
+  return AMG_OK;
+}
+
 }  // namespace
 
 void amg_destroy_graphs(amg_handle_s* H) {
+  for (auto& g : H->while_exec)
+    if (g) {
+      cudaGraphExecDestroy(g);
+      g = nullptr;
+    }
   for (auto& g : H->graph_exec)
     if (g) {
       cudaGraphExecDestroy(g);
@@ -552,7 +613,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
       AMG_TRY(enqueue_pcg_start(H, st));
     } else {
       ++g_nlaunch, launch(k_dot, red_grid(H, n), RED_THREADS, 0, st)(n, r, r, H->partials, H->counter, H->ctl, FIN_RZ);
-      ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, p, H->ctl);
+      ++g_nlaunch, launch(k_pcg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, p, H->ctl, (cudaGraphConditionalHandle)0);
     }
   } else {
     ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, nullptr, nullptr,
@@ -560,25 +621,36 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
 
-  cudaGraphExec_t gexec = nullptr;
-  if (H->opt.use_graph && maxit > 0) AMG_TRY(get_iteration_graph(H, krylov, precond, st, &gexec));
-
-  // The host runs at most LAG iterations ahead of the device's convergence flag; iterations
-  // enqueued after convergence return at their first instruction.
-  constexpr int NSLOT = 4, LAG = 1;
-  for (int it = 0; it < maxit; ++it) {
-    if (gexec) {
-      AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
-      g_nlaunch += H->graph_launches[graph_slot(krylov, precond)];
-    } else
-      AMG_TRY(enqueue_iteration(H, krylov, precond, st));
-    const int slot = it % NSLOT;
-    AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[slot], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
-    AMG_CUDA_TRY(H, cudaEventRecord(H->ev[slot], st));
-    if (it >= LAG) {
-      const int old = (it - LAG) % NSLOT;
-      AMG_CUDA_TRY(H, cudaEventSynchronize(H->ev[old]));
-      if (H->h_ctl[old].done) break;
+  // the loop: one graph with a conditional WHILE node (device-side loop control), else the iteration graph
+  // replayed under host control
+  cudaGraphExec_t gwhile = nullptr;
+  if (H->opt.use_graph && H->opt.use_while && maxit > 0) {
+    const amg_status sw = get_while_graph(H, krylov, precond, &gwhile);
+    if (sw != AMG_OK && sw != AMG_ERR_UNSUPPORTED) return sw;
+  }
+  if (gwhile) {
+    AMG_CUDA_TRY(H, cudaGraphLaunch(gwhile, st));
+    H->while_used = true;
+  } else {
+    cudaGraphExec_t gexec = nullptr;
+    if (H->opt.use_graph && maxit > 0) AMG_TRY(get_iteration_graph(H, krylov, precond, st, &gexec));
+    // The host runs at most LAG iterations ahead of the device's convergence flag; iterations
+    // enqueued after convergence return at their first instruction.
+    constexpr int NSLOT = 4, LAG = 1;
+    for (int it = 0; it < maxit; ++it) {
+      if (gexec) {
+        AMG_CUDA_TRY(H, cudaGraphLaunch(gexec, st));
+        g_nlaunch += H->graph_launches[graph_slot(krylov, precond)];
+      } else
+        AMG_TRY(enqueue_iteration(H, krylov, precond, st));
+      const int slot = it % NSLOT;
+      AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[slot], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
+      AMG_CUDA_TRY(H, cudaEventRecord(H->ev[slot], st));
+      if (it >= LAG) {
+        const int old = (it - LAG) % NSLOT;
+        AMG_CUDA_TRY(H, cudaEventSynchronize(H->ev[old]));
+        if (H->h_ctl[old].done) break;
+      }
     }
   }
   const bool half = (krylov == 1);
@@ -592,6 +664,11 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   AMG_CUDA_TRY(H, cudaMemcpyAsync(&H->h_ctl[4], H->ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, st));
   AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   const KrylovCtl& c = H->h_ctl[4];
+  if (gwhile) {  // kernels the device-side loop launched: iterations passed x kernel nodes of the body
+    const int slot = g_tr ? 4 : krylov * 2 + precond;
+    g_nlaunch += (int64_t)(c.iter > 0 ? c.iter : 1) * H->while_launches[slot];
+    H->last_launches = g_nlaunch - launches0;
+  }
   H->hist_len = c.iter < H->hist_cap ? c.iter : H->hist_cap;
   info->iterations = c.iter;
   info->status = c.status;

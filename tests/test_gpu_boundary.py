@@ -135,3 +135,24 @@ def test_distinct_handles_on_distinct_threads_and_streams(B):
     assert not errs, errs
     for (x, it), (xr, itr) in zip(out, ref):
         assert it == itr and torch.equal(x, xr)  # bitwise: no cross-talk between handles
+
+
+@pytest.mark.parametrize("krylov", [0, 1])
+def test_device_side_loop_equals_host_controlled_loop(B, krylov):
+    """use_while = 1 (default): the Krylov loop is one graph with a conditional WHILE node; use_while = 0: the
+    iteration graph replayed under host control with a one-behind poll.  Same kernels in the same order: bitwise
+    equal solutions and counts; the device-side loop launches no surplus iteration."""
+    A = inputs.config_matrix(3, 40)
+    b = inputs.config_rhs(3, A.n)
+    res = {}
+    for w in (1, 0):
+        s = B.AmgSolver(A.rowptr, A.col, A.val, use_while=w)
+        x, info = s.solve(b, 1e-8, 500, krylov)
+        res[w] = (x.clone(), info.iterations, info.rel_residual, B.amg_get_last_launches(s.h))
+        x3, i3 = s.solve(b, 1e-30, 3, krylov)          # maxit stop inside the device-side loop
+        assert i3.status == 1 and i3.iterations == 3
+        x0, i0 = s.solve(np.zeros(A.n), 1e-8, 500, krylov)  # zero right-hand side: the loop body exits at once
+        assert i0.status == 0 and i0.iterations == 0 and not bool(x0.any())
+        s.close()
+    assert torch.equal(res[1][0], res[0][0]) and res[1][1] == res[0][1] and res[1][2] == res[0][2]
+    assert res[1][3] < res[0][3]  # one surplus look-ahead iteration less
