@@ -35,7 +35,8 @@ class Options(C.Structure):
                 ("coarse_max_rows", C.c_int32), ("max_levels", C.c_int32),
                 ("max_match_rounds", C.c_int32), ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double),
-                ("hash_seed", C.c_uint64), ("agg_passes", C.c_int32), ("symmetric", C.c_int32)]
+                ("hash_seed", C.c_uint64), ("agg_passes", C.c_int32), ("symmetric", C.c_int32),
+                ("hierarchy_fp32", C.c_int32)]
 
 
 class Info(C.Structure):

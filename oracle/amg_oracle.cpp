@@ -28,6 +28,7 @@ struct Csr {
 struct Level {
   Csr A;                     // A_l
   Csr At;                    // A_l^T, built lazily for the nonsymmetric adjoint (O-7)
+  Csr A32, At32;             // hierarchy_fp32: the same operators with every value rounded to fp32 (V-cycle only)
   std::vector<double> dinv;  // smoother diagonal (A7)
   std::vector<int> agg;      // agg_l[i] in [0, n_{l+1})
   std::vector<int> agg_ptr, agg_mem;  // members of every aggregate, ascending fine index
@@ -45,6 +46,7 @@ struct oracle_handle_s {
   std::vector<double> lut;  // dense LU of A_L^T
   std::vector<int> pivt;
   bool have_t = false;
+  bool have_32 = false, have_t32 = false;
   bool have_lu = false;  // with imported aggregates the coarsest LU is factored at first use
   std::vector<double> hist;  // ||r_k|| / ||b|| of the last solve, k = 1 … iterations (PAPER.md:125 diagnostics)
 };
@@ -504,7 +506,10 @@ void residual_restrict(const Csr& A, const Level& L, const double* b, const doub
 void vcycle(const oracle_handle_s* H, int l, bool T, const double* b, double* x) {
   int Lc = (int)H->lv.size() - 1;
   const Level& lev = H->lv[l];
-  const Csr& A = T ? lev.At : lev.A;
+  // hierarchy_fp32 (NEXT-4): inside the V-cycle the sparse level operators are the fp64 ones
+  // rounded to fp32, used in fp64 arithmetic; dinv, the coarsest LU and every vector stay fp64
+  const bool f32 = H->opt.hierarchy_fp32 != 0 && l < Lc;
+  const Csr& A = T ? (f32 ? lev.At32 : lev.At) : (f32 ? lev.A32 : lev.A);
   int n = A.n;
   if (l == Lc) {
     dense_lu_solve(n, T ? H->lut : H->lu, T ? H->pivt : H->piv, b, x);
@@ -658,6 +663,24 @@ void bicgstab(oracle_handle_s* H, const Csr& A, bool T, const double* b, double*
   }
 }
 
+Csr rounded_to_fp32(const Csr& A) {
+  Csr R = A;
+  for (double& v : R.val) v = (double)(float)v;
+  return R;
+}
+
+void ensure_fp32(oracle_handle_s* H) {
+  if (!H->opt.hierarchy_fp32) return;
+  if (!H->have_32) {
+    for (Level& L : H->lv) L.A32 = rounded_to_fp32(L.A);
+    H->have_32 = true;
+  }
+  if (H->have_t && !H->have_t32) {
+    for (Level& L : H->lv) L.At32 = rounded_to_fp32(L.At);
+    H->have_t32 = true;
+  }
+}
+
 void ensure_transposed(oracle_handle_s* H) {
   if (H->have_t) return;
   for (Level& L : H->lv) L.At = transpose(L.A);  // (P^T A P)^T = P^T A^T P on the same aggregates
@@ -687,6 +710,7 @@ void oracle_options_default(oracle_options* o) {
   o->hash_seed = 0;
   o->agg_passes = 1;
   o->symmetric = 1;
+  o->hierarchy_fp32 = 0;
 }
 
 void oracle_set_threads(int nthreads) { g_threads = nthreads > 0 ? nthreads : 1; }
@@ -829,6 +853,7 @@ int oracle_residual_restrict(oracle_handle h, int32_t level, const double* b, co
 int oracle_vcycle(oracle_handle h, int32_t level, const double* r, double* z) {
   if (!h || level < 0 || level >= (int)h->lv.size()) return ORACLE_ERR_INVALID_ARG;
   if (int rc = ensure_lu(h)) return rc;
+  ensure_fp32(h);
   vcycle(h, level, false, r, z);
   return ORACLE_OK;
 }
@@ -837,6 +862,7 @@ int oracle_vcycle_transpose(oracle_handle h, int32_t level, const double* r, dou
   if (!h || level < 0 || level >= (int)h->lv.size()) return ORACLE_ERR_INVALID_ARG;
   if (int rc = ensure_lu(h)) return rc;
   ensure_transposed(h);
+  ensure_fp32(h);
   vcycle(h, level, true, r, z);
   return ORACLE_OK;
 }
@@ -846,6 +872,7 @@ int oracle_solve(oracle_handle h, const double* b, double* x, double rtol, int32
   if (!h || !b || !x || !info || maxit < 0) return ORACLE_ERR_INVALID_ARG;
   if (precond)
     if (int rc = ensure_lu(h)) return rc;
+  ensure_fp32(h);
   if (krylov == 0)
     pcg(h, h->lv[0].A, false, b, x, rtol, maxit, precond, info);
   else
@@ -861,6 +888,7 @@ int oracle_solve_transpose(oracle_handle h, const double* g, double* lambda, dou
   if (precond)
     if (int rc = ensure_lu(h)) return rc;
   ensure_transposed(h);
+  ensure_fp32(h);
   if (krylov == 0)
     pcg(h, h->lv[0].At, true, g, lambda, rtol, maxit, precond, info);
   else

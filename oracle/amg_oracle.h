@@ -60,6 +60,10 @@ typedef struct {
   int32_t symmetric;        /* 1 (default): w_ij = -a_ij read from row i (A1);  0: the matching
                                of every level runs on (A_l + A_l^T)/2, union pattern (A1,
                                nonsymmetric case; bitwise equal to 1 for a bitwise symmetric A) */
+  int32_t hierarchy_fp32;   /* 1: mixed-precision hierarchy (NEXT-4; "single and double precision"):
+                               inside the V-cycle every sparse level operator A_l, l < L, is the fp64 operator with
+                               each value rounded to fp32, used in fp64 arithmetic; dinv, the coarsest LU, the Krylov
+                               operator A, all vectors and all sums stay fp64.  default 0                        */
 } oracle_options;
 
 typedef struct {

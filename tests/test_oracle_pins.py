@@ -940,3 +940,69 @@ def test_residual_history(oracle_mod, krylov):
         assert int(np.argmax(h12 <= 1e-8)) + 1 == i8.iterations
     else:  # BiCGSTAB: the last entry of the looser solve may be its half-step exit ||s|| / ||b|| (A11)
         assert np.array_equal(h8[:-1], h12[:len(h8) - 1])
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-4: mixed-precision hierarchy (hierarchy_fp32): the V-cycle on fp32-rounded level operators
+# ------------------------------------------------------------------------------------------
+def py_vcycle(o, l, b, round32, nu1=2, nu2=2, gamma=1.0):
+    """O-4 written out with scipy matrices taken from the oracle's level CSRs (plain definition, recursion)."""
+    import scipy.sparse as sp
+
+    L = o.num_levels - 1
+    rp, cl, vl = o.level_csr(l)
+    n = len(rp) - 1
+    if l == L:
+        return np.linalg.solve(sp.csr_matrix((vl, cl, rp), shape=(n, n)).toarray(), b)
+    v = vl.astype(np.float32).astype(np.float64) if round32 else vl
+    A = sp.csr_matrix((v, cl, rp), shape=(n, n))
+    dinv = o.dinv(l)
+    agg = o.aggregates(l)
+    nc = o.level_info(l + 1)[0]
+    x = dinv * b if nu1 > 0 else np.zeros(n)
+    for _ in range(1, nu1):
+        x = x + dinv * (b - A @ x)
+    rc = np.bincount(agg, weights=b - A @ x, minlength=nc)
+    x = x + gamma * py_vcycle(o, l + 1, rc, round32, nu1, nu2, gamma)[agg]
+    for _ in range(nu2):
+        x = x + dinv * (b - A @ x)
+    return x
+
+
+def test_mixed_precision_hierarchy(oracle_mod):
+    """hierarchy_fp32 = 1: inside the V-cycle every sparse level operator is the fp64 one rounded to fp32 (used
+    in fp64 arithmetic); dinv, the coarsest LU and the Krylov operator stay fp64.  Pinned by the recursion
+    written out with scipy on the rounded matrices; the fp64 cycle is pinned by the same recursion unrounded."""
+    A = inputs.variable_diffusion_csr((12, 12, 12), seed=9, sigma=1.5, ell=3.0)
+    o64 = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    o32 = oracle_mod.Oracle(A.rowptr, A.col, A.val, hierarchy_fp32=1)
+    assert o64.num_levels == o32.num_levels >= 4
+    for l in range(o64.num_levels):  # the hierarchy itself (aggregates, Galerkin values, dinv) is the fp64 one
+        assert all(np.array_equal(a, b) for a, b in zip(o64.level_csr(l), o32.level_csr(l)))
+    r = np.random.default_rng(3).standard_normal(A.n)
+    z64, z32 = o64.vcycle(r), o32.vcycle(r)
+    rel = lambda a, b: np.linalg.norm(a - b) / np.linalg.norm(b)
+    assert rel(z64, py_vcycle(o64, 0, r, False)) <= 1e-13
+    assert rel(z32, py_vcycle(o32, 0, r, True)) <= 1e-13
+    assert 1e-10 < rel(z32, z64) < 1e-6          # a perturbation of fp32 size, not the same operator
+    for l in (1, 2):                             # cycles started below level 0
+        nl = o32.level_info(l)[0]
+        rl = np.random.default_rng(l).standard_normal(nl)
+        assert rel(o32.vcycle(rl, l), py_vcycle(o32, l, rl, True)) <= 1e-13
+    # rounding a bitwise symmetric matrix keeps it symmetric: B stays symmetric, PCG applies and converges to the
+    # fp64 tolerance with the fp64 operator A in the Krylov recurrences
+    u, v = np.random.default_rng(5).standard_normal((2, A.n))
+    assert abs(o32.vcycle(u) @ v - u @ o32.vcycle(v)) <= 1e-13 * np.linalg.norm(u) * np.linalg.norm(v)
+    b = inputs.rhs_uniform(A.n, 4)
+    x64, i64 = o64.solve(b, rtol=1e-10, maxit=200)
+    x32, i32 = o32.solve(b, rtol=1e-10, maxit=200)
+    assert i32.status == 0 and abs(i32.iterations - i64.iterations) <= 1
+    assert np.linalg.norm(b - A.to_scipy() @ x32) <= 1.01e-10 * np.linalg.norm(b)
+    assert rel(x32, x64) <= 1e-8
+    # the solve of a nonsymmetric system and its adjoint with the rounded transposed operators
+    N = inputs.stretched_channel_csr((6, 8, 6), 2.0)
+    on = oracle_mod.Oracle(N.rowptr, N.col, N.val, symmetric=0, hierarchy_fp32=1, coarse_max_rows=16)
+    D = N.to_dense()
+    g = np.random.default_rng(6).standard_normal(N.n)
+    lam, il = on.solve_transpose(g, rtol=1e-11, maxit=300, krylov=1, symmetric=0)
+    assert il.status == 0 and np.allclose(lam, np.linalg.solve(D.T, g), rtol=1e-7, atol=1e-9)
