@@ -112,6 +112,12 @@ typedef struct {
   double strong_beta;       /* strength threshold beta, default 0.25                                     */
   double coarse_scale;      /* gamma: x += gamma * P e_c, default 1.0                                    */
   uint64_t hash_seed;       /* tie-break salt of the matching; level l uses hash_seed + l                */
+  int32_t hierarchy_fp32;   /* 1 = mixed-precision hierarchy: inside the V-cycle every sparse level operator
+                               A_l, l < L, is stored with fp32 values (6 bytes per entry instead of 10) and used in fp64
+                               arithmetic; dinv, the coarsest LU, the Krylov operator A (level 0 keeps an fp64 copy), all
+                               vectors and all sums stay fp64.  The solve still converges to rtol in fp64.  In this mode
+                               the per-level hooks (amg_level_op) see the rounded operators.  default 0            */
+  int32_t reserved1;
 } amg_options;
 
 typedef struct {

@@ -38,7 +38,8 @@ class amg_options(C.Structure):
                 ("use_graph", C.c_int32), ("tail_dense_rows", C.c_int32), ("use_pdl", C.c_int32),
                 ("split_prolong_rows", C.c_int32), ("use_while", C.c_int32),
                 ("omega", C.c_double),
-                ("strong_beta", C.c_double), ("coarse_scale", C.c_double), ("hash_seed", C.c_uint64)]
+                ("strong_beta", C.c_double), ("coarse_scale", C.c_double), ("hash_seed", C.c_uint64),
+                ("hierarchy_fp32", C.c_int32), ("reserved1", C.c_int32)]
 
 
 class amg_info(C.Structure):

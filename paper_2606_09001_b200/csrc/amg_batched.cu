@@ -14,6 +14,7 @@ struct AmgBatch {
   int eligible = -1;  // -1: not examined yet
   std::vector<double*> x, x2, b;  // per level, [n_l][NB]
   std::vector<LevelGeomB> geom;
+  LevelGeomB geomK;  // level 0's fp64 blobs of a mixed-precision hierarchy (the Krylov SpMV)
   double* kv[4] = {nullptr, nullptr, nullptr, nullptr};  // x, r, p, q
   KrylovCtlB* ctl = nullptr;
   KrylovCtlB* h_ctl = nullptr;  // pinned, 6 slots
@@ -59,13 +60,15 @@ void set_attr_b() {
 }
 
 template <int OP, int NDOT>
-void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowArgsB& a, cudaStream_t st) {
+void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowArgsB& a, cudaStream_t st,
+                      const LevelOpT* K = nullptr) {
   a.n = L.n, a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob, a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
+  if (K) a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx, a.halo_cagg = K->halo_cagg;
   a.dinv = L.dinv, a.agg = L.agg, a.agg_ptr = L.agg_ptr, a.gamma = H->opt.coarse_scale;
   a.partials = H->batch->partials, a.counter = H->batch->counter;
   a.stages = G.stages, a.xslots = G.xslots, a.stage_bytes = G.stage_bytes, a.xslot_bytes = G.xslot_bytes;
   int grid = H->sm_count;  // one CTA per SM
-  if (grid > L.nblk) grid = L.nblk;
+  if (grid > a.ntiles) grid = a.ntiles;
   if (L.stream_hint)
     launch_b(k_rowtile_b<OP, NDOT, true>, grid, RTB_THREADS, G.smem, st, a);
   else
@@ -165,7 +168,10 @@ amg_status enqueue_iteration_b(amg_handle_s* H, cudaStream_t st) {
   {
     RowArgsB a = args_b(Bt.ctl);
     a.x = p, a.out = q, a.fin = FIN_PQ;
-    launch_rowtile_b<OP_SPMV, 1>(H, L0, Bt.geom[0], a, st);
+    if (L0.K.fast)  // mixed-precision hierarchy: the Krylov operator stays fp64
+      launch_rowtile_b<OP_SPMV, 1>(H, L0, Bt.geomK, a, st, &L0.K);
+    else
+      launch_rowtile_b<OP_SPMV, 1>(H, L0, Bt.geom[0], a, st);
   }
   launch_b(k_pcg_xr_b, red_grid_b(H, (int64_t)n * NB2), RED_THREADS, 0, st, n, (const double*)p, (const double*)q, x, r,
            (const double*)L0.dinv, Bt.x2[0], Bt.partials, Bt.counter, Bt.ctl);
@@ -259,19 +265,23 @@ int amg_batch_prepare(amg_handle_s* H, cudaStream_t st) {
   if (!H->symmetric || H->opt.force_generic || D < 1 || H->opt.pre_sweeps < 1 || H->opt.post_sweeps < 1) return 0;
   for (int l = 0; l < D; ++l)
     if (!H->lv[l].fast) return 0;
+  if (H->lv[0].v32 && !H->lv[0].K.fast) return 0;
   // ---- ring geometry per level from the tile descriptors ----
   B.geom.assign(D, LevelGeomB());
   std::vector<TileDesc> td;
-  for (int l = 0; l < D; ++l) {
-    const Level& L = H->lv[l];
-    td.resize(L.nblk);
-    if (cudaMemcpyAsync(td.data(), L.tiles, sizeof(TileDesc) * L.nblk, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+  for (int l = -1; l < D; ++l) {  // l = -1: the fp64 blobs of level 0 of a mixed-precision hierarchy
+    if (l < 0 && !H->lv[0].K.fast) continue;
+    const Level& L = H->lv[l < 0 ? 0 : l];
+    const int nblk = l < 0 ? L.K.nblk : L.nblk;
+    td.resize(nblk);
+    if (cudaMemcpyAsync(td.data(), l < 0 ? L.K.tiles : L.tiles, sizeof(TileDesc) * nblk, cudaMemcpyDeviceToHost, st) !=
+            cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess)
       return 0;
     int sb = 0, xb = 0;
     for (const TileDesc& d : td) sb = std::max(sb, tpb_stage_need(d)), xb = std::max(xb, tpb_xslot_need(d));
     sb = (sb + 127) & ~127, xb = (xb + 127) & ~127;
-    LevelGeomB& G = B.geom[l];
+    LevelGeomB& G = l < 0 ? B.geomK : B.geom[l];
     G.stage_bytes = sb, G.xslot_bytes = xb;
     for (int S = 3; S >= 2 && !G.stages; --S) {
       const int left = RTB_SMEM_MAX - RTB_HEADER - S * sb;

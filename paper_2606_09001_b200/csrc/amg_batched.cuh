@@ -69,7 +69,7 @@ struct StageLayoutB {
 enum { TPB_D = 1, TPB_RESTRICT = 2 };
 __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) {
   StageLayoutB t;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const int r1 = d.r0 + d.nr;
   t.ra2 = d.r0 & ~1;
   t.nrv = tp_up(r1 - t.ra2, 2);
@@ -174,7 +174,8 @@ struct StageDescB {  // TP_DESC_BYTES at the start of a stage, written by the pr
   int nsl, nhalo, roff, aoff;  // roff = r0 - ra2 (dinv slice), aoff = I0 - Ia4 (agg_ptr slice)
   int o_perm, o_col, o_val, o_d;
   int o_agg, o_out, o_dc, eoff;  // eoff = Ia2 (dcs[I - eoff] = dinv_c[I])
-  int pad[16];
+  int vb;                        // bytes per stored value (8, or 4 with the mixed-precision hierarchy)
+  int pad[15];
 };
 static_assert(sizeof(StageDescB) == TP_DESC_BYTES, "stage header size");
 
@@ -184,17 +185,18 @@ __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& 
   constexpr bool SWEEP = (OP == OP_JACOBI || OP == OP_JACOBI_PROLONG);
   constexpr bool RES = (OP == OP_RESTRICT);
   const bool dc = RES && a.dinv_c != nullptr;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const StageLayoutB t = tpb_stage(d, (SWEEP ? TPB_D : 0) | (RES ? TPB_RESTRICT : 0));
   StageDescB sd;
   sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
   sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
   sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_d = t.o_d;
   sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.o_dc = t.o_dc, sd.eoff = t.Ia2;
+  sd.vb = d.vb;
   int4* dst = reinterpret_cast<int4*>(stage);
   const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
-  for (int q = 0; q < 4; ++q) dst[q] = src[q];
+  for (int q = 0; q < 5; ++q) dst[q] = src[q];
   if (d.nr <= 0) {
     mbar_arrive(bar);
     return;
@@ -373,6 +375,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + sd->o_perm);
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
+        const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
+        const bool v32 = sd->vb == 4;
         const int ncolp = tpb_ncolp(nr, sd->nhalo);
         const double2* xc = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes);
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
@@ -390,12 +394,13 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           }
           const unsigned short* cp = scol + sl.x;
           const double* vp = sval + sl.x;
+          const float* vp32 = sval32 + sl.x;
           double acc[NB];
 #pragma unroll
           for (int t = 0; t < NB; ++t) acc[t] = 0.0;
 #pragma unroll 2
           for (int k = 0; k < sl.y; ++k) {
-            const double av = vp[k * 32];
+            const double av = v32 ? (double)vp32[k * 32] : vp[k * 32];
             const double2* xp = xc + cp[k * 32];
 #pragma unroll
             for (int h = 0; h < NB2; ++h) {

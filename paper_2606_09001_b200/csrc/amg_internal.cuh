@@ -99,6 +99,10 @@ struct Level {
   int nblk = 0;
   int fast = 0;             // 1: row-tile streaming kernels; 0: row-vector fallback
   LevelOpT T;               // A_l^T (only when the handle is nonsymmetric)
+  // mixed-precision hierarchy: the blobs above (and T's) hold fp32 values; level 0 keeps fp64 blobs of A_0 (K) and
+  // A_0^T (KT) for the Krylov method's own SpMV
+  LevelOpT K, KT;
+  int v32 = 0;              // 1: this level's V-cycle operator is the fp64 one rounded to fp32
   int lpr = 8;              // lanes per row of the fallback kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary

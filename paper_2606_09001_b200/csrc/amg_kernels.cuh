@@ -55,6 +55,7 @@ struct RowArgs {
   unsigned* counter;
   KrylovCtl* ctl;       // may be null (hooks)
   int fin;
+  int v32;              // row-vector fallback: round every CSR value to fp32 on the fly (mixed-precision hierarchy)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -357,7 +358,7 @@ struct StageDesc {  // TP_DESC_BYTES at the start of a stage, written by the pro
   int nsl, nhalo, roff, aoff;    // roff = r0 - ra2 (b / dinv slices), aoff = I0 - Ia4 (agg_ptr slice)
   int o_perm, o_col, o_val, o_b;
   int o_d, o_agg, o_out, o_dc;
-  int eoff, pad0, pad2, pad3;    // eoff = Ia2 (coarse slice: dcs[I - eoff] = dinv_c[I])
+  int eoff, vb, pad2, pad3;      // eoff = Ia2 (coarse slice: dcs[I - eoff] = dinv_c[I]); vb = bytes per stored value
   int pad1[12];
 };
 static_assert(sizeof(StageDesc) == TP_DESC_BYTES, "stage header size");
@@ -380,7 +381,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
   const bool d0_staged = (OP == OP_SPMV && NDOT > 0 && a.d0 != a.x);
   const bool dc = T::AGGPTR && a.dinv_c != nullptr;
   const int flags = T::FLAGS | (d0_staged ? TP_B : 0) | (dc ? TP_DC : 0);
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const StageLayout t = tp_stage(d, flags);
   if (mode != 2) {
     StageDesc sd;
@@ -388,7 +389,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
     sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
     sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_b = t.o_b;
     sd.o_d = t.o_d, sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.o_dc = t.o_dc;
-    sd.eoff = t.Ia2, sd.pad0 = sd.pad2 = sd.pad3 = 0;
+    sd.eoff = t.Ia2, sd.vb = d.vb, sd.pad2 = sd.pad3 = 0;
     int4* dst = reinterpret_cast<int4*>(stage);
     const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
@@ -648,6 +649,8 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + sd->o_perm);
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
+        const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;  // mixed-precision hierarchy
+        const bool v32 = sd->vb == 4;
         const double* xc = reinterpret_cast<const double*>(xslot0 + q * RT_XSLOT_BYTES);
         const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
@@ -655,10 +658,16 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         for (int j = (w - sbase) & (rt::NCW - 1); j < nsl; j += rt::NCW) {
           const int2 sl = slices[j];
           const unsigned short* cp = scol + sl.x;
-          const double* vp = sval + sl.x;
           double sum = 0.0;
+          if (v32) {  // values stored in fp32 (exactly representable), arithmetic in fp64
+            const float* vp = sval32 + sl.x;
 #pragma unroll 4
-          for (int k = 0; k < sl.y; ++k) sum += vp[k * 32] * xc[cp[k * 32]];
+            for (int k = 0; k < sl.y; ++k) sum += (double)vp[k * 32] * xc[cp[k * 32]];
+          } else {
+            const double* vp = sval + sl.x;
+#pragma unroll 4
+            for (int k = 0; k < sl.y; ++k) sum += vp[k * 32] * xc[cp[k * 32]];
+          }
           const int lr = perm[j * 32 + lane];
           if (lr != 0xFFFF) {
             if (OP == OP_RESTRICT) {
@@ -724,7 +733,8 @@ static __global__ void __launch_bounds__(RB_THREADS) k_rowvec(RowArgs a) {
     const int64_t i = row0 + it * rstride;
     double s = 0.0;
     if (i < a.n)
-      for (int k = a.rowptr[i] + sub, e = a.rowptr[i + 1]; k < e; k += LPR) s += a.val[k] * gather_x<OP>(a, a.col[k]);
+      for (int k = a.rowptr[i] + sub, e = a.rowptr[i + 1]; k < e; k += LPR)
+        s += (a.v32 ? (double)(float)a.val[k] : a.val[k]) * gather_x<OP>(a, a.col[k]);
 #pragma unroll
     for (int o = LPR / 2; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (i < a.n && sub == 0) {

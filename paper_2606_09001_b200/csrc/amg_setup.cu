@@ -555,11 +555,10 @@ __global__ void k_gather_double(int n, const double* __restrict__ src, const int
 // operands, a nonzero RT_NNZ_WEIGHT (value, 16-bit column, its share of the halo list and values).  Tile k starts at the first unit (aggregate, or row if
 // unit_ptr == null) whose cumulative weight is at or beyond k * target.
 constexpr int RT_ROW_WEIGHT = 24;
-constexpr int RT_NNZ_WEIGHT = 10;
-__device__ __forceinline__ int64_t tile_weight(const int* __restrict__ rowptr, int r) {
-  return RT_NNZ_WEIGHT * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
+__device__ __forceinline__ int64_t tile_weight(const int* __restrict__ rowptr, int r, int nnz_w) {
+  return nnz_w * (int64_t)rowptr[r] + (int64_t)RT_ROW_WEIGHT * r;
 }
-__global__ void k_blk_partition(int nblk, int target, int nunits, const int* __restrict__ unit_ptr,
+__global__ void k_blk_partition(int nblk, int target, int nnz_w, int nunits, const int* __restrict__ unit_ptr,
                                 const int* __restrict__ rowptr, int n, int* __restrict__ blk_ptr) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k > nblk) return;
@@ -572,7 +571,7 @@ __global__ void k_blk_partition(int nblk, int target, int nunits, const int* __r
   while (lo < hi) {
     int mid = (lo + hi) >> 1;
     int r = unit_ptr ? unit_ptr[mid] : mid;
-    if (tile_weight(rowptr, r) >= want)
+    if (tile_weight(rowptr, r, nnz_w) >= want)
       hi = mid;
     else
       lo = mid + 1;
@@ -591,7 +590,7 @@ constexpr int PK_MAX_LEN = 512;
 __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int* __restrict__ blk_ptr,
                                                            const int* __restrict__ rowptr, const int* __restrict__ col,
                                                            const double* __restrict__ val, const int* __restrict__ agg,
-                                                           int write, const int* __restrict__ blob_off16,
+                                                           int vb, int write, const int* __restrict__ blob_off16,
                                                            const int* __restrict__ halo_off, int* __restrict__ size16,
                                                            int* __restrict__ nhalo_out, int* __restrict__ info,
                                                            TileDesc* __restrict__ tiles, unsigned char* __restrict__ blob,
@@ -609,7 +608,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   const int r0 = blk_ptr[t], r1 = blk_ptr[t + 1], nr = r1 - r0;
   TileDesc d;
   d.r0 = r0, d.nr = nr, d.I0 = 0, d.nA = 0, d.nsl = 0, d.nslots = 0, d.nhalo = 0, d.blob16 = 0;
-  d.halo_off = 0, d.pad0 = d.pad1 = d.pad2 = 0;
+  d.halo_off = 0, d.vb = vb, d.pad1 = d.pad2 = 0;
   if (nr <= 0) {
     if (tid == 0) {
       if (write) tiles[t] = d;
@@ -714,7 +713,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   }
   __syncthreads();
   d.nsl = nsl, d.nslots = s_nslots, d.nhalo = s_nhalo;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, vb);
   if (!write) {
     if (tid == 0) {
       size16[t] = p.end / 16;
@@ -739,6 +738,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   for (int s = tid; s < nsl * 32; s += PK_THREADS) o_perm[s] = s < nr ? (unsigned short)srow[s] : (unsigned short)0xFFFF;
   unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
+  float* o_val32 = reinterpret_cast<float*>(base + p.o_val);  // vb == 4: mixed-precision hierarchy
   for (int j = 0; j < nsl; ++j) {
     const int off = sl_off[j], w = sl_w[j];
     for (int q = tid; q < 32 * w; q += PK_THREADS) {
@@ -765,7 +765,10 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
         }
       }
       o_col[off + q] = c16;
-      o_val[off + q] = v;
+      if (vb == 4)
+        o_val32[off + q] = (float)v;
+      else
+        o_val[off + q] = v;
     }
   }
   // tail of the u16 column section up to its 16-byte rounding
@@ -1100,8 +1103,9 @@ struct TilePack {
 // search starts a little above it instead of at 1: one attempt per level instead of two or three)
 amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
                       const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st,
-                      double* scale_io = nullptr) {
-  const int64_t total_w = RT_NNZ_WEIGHT * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
+                      double* scale_io = nullptr, int vb = 8) {
+  const int nnz_w = 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value
+  const int64_t total_w = nnz_w * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
   double scale = scale_io ? (*scale_io * 1.12 < 1.0 ? *scale_io * 1.12 : 1.0) : 1.0;
   for (int attempt = 0; attempt < 6 && !P.fast; ++attempt) {
     const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
@@ -1119,8 +1123,9 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
     AMG_ALLOC(H, hoff, int, P.nblk + 1, st);
     AMG_ALLOC(H, info, int, 4, st);
     AMG_CUDA_TRY(H, cudaMemsetAsync(info, 0, 4 * sizeof(int), st));
-    k_blk_partition<<<grid_for(P.nblk + 1), TPB, 0, st>>>(P.nblk, target, agg_ptr ? nc : n, agg_ptr, rowptr, n, P.blk_ptr);
-    k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, 0, nullptr, nullptr, size16, nh,
+    k_blk_partition<<<grid_for(P.nblk + 1), TPB, 0, st>>>(P.nblk, target, nnz_w, agg_ptr ? nc : n, agg_ptr, rowptr, n,
+                                                         P.blk_ptr);
+    k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, vb, 0, nullptr, nullptr, size16, nh,
                                                info, P.tiles, nullptr, nullptr, nullptr);
     AMG_CUDA_TRY(H, cudaGetLastError());
     int h_info[4];
@@ -1145,7 +1150,7 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
       }
       AMG_ALLOC(H, P.halo_idx, int, total_h + 4, st);
       AMG_ALLOC(H, P.halo_cagg, int, total_h + 4, st);
-      k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, 1, off16, hoff, size16, nh, info,
+      k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, vb, 1, off16, hoff, size16, nh, info,
                                                  P.tiles, P.blob, P.halo_idx, P.halo_cagg);
       AMG_CUDA_TRY(H, cudaGetLastError());
       AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
@@ -1343,12 +1348,19 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     }
     AMG_CUDA_TRY(H, cudaGetLastError());
     L.fast = 0;
+    L.v32 = (o.hierarchy_fp32 && q < Lc) ? 1 : 0;  // mixed-precision hierarchy: the V-cycle's operators in fp32
     if (!o.force_generic && L.n > 0) {
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
-                         q < Lc ? L.nc : 0, P, st, &pack_scale));
+                         q < Lc ? L.nc : 0, P, st, &pack_scale, L.v32 ? 4 : 8));
       L.blk_ptr = P.blk_ptr, L.tiles = P.tiles, L.blob = P.blob, L.halo_idx = P.halo_idx, L.halo_cagg = P.halo_cagg;
       L.blob_bytes = P.blob_bytes, L.nblk = P.nblk, L.fast = P.fast;
+      if (L.v32 && q == 0) {  // the Krylov method's own SpMV keeps the fp64 operator
+        TilePack PK;
+        AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, L.agg, L.agg_ptr, L.nc, PK, st, nullptr, 8));
+        L.K.blk_ptr = PK.blk_ptr, L.K.tiles = PK.tiles, L.K.blob = PK.blob, L.K.halo_idx = PK.halo_idx;
+        L.K.halo_cagg = PK.halo_cagg, L.K.blob_bytes = PK.blob_bytes, L.K.nblk = PK.nblk, L.K.fast = PK.fast;
+      }
     }
     const double mean_len = L.n > 0 ? (double)L.nnz / L.n : 1.0;
     L.lpr = mean_len <= 6.0 ? 4 : (mean_len <= 12.0 ? 8 : (mean_len <= 24.0 ? 16 : 32));
@@ -1406,9 +1418,15 @@ amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st) {
     if (!H->opt.force_generic && L.n > 0) {
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, T.rowptr, T.col, T.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
-                         q < Lc ? L.nc : 0, P, st));
+                         q < Lc ? L.nc : 0, P, st, nullptr, L.v32 ? 4 : 8));
       T.blk_ptr = P.blk_ptr, T.tiles = P.tiles, T.blob = P.blob, T.halo_idx = P.halo_idx, T.halo_cagg = P.halo_cagg;
       T.blob_bytes = P.blob_bytes, T.nblk = P.nblk, T.fast = P.fast;
+      if (L.v32 && q == 0) {  // fp64 blobs of A_0^T for the Krylov method's SpMV
+        TilePack PK;
+        AMG_TRY(pack_tiles(H, L.n, L.nnz, T.rowptr, T.col, T.val, L.agg, L.agg_ptr, L.nc, PK, st, nullptr, 8));
+        L.KT.blk_ptr = PK.blk_ptr, L.KT.tiles = PK.tiles, L.KT.blob = PK.blob, L.KT.halo_idx = PK.halo_idx;
+        L.KT.halo_cagg = PK.halo_cagg, L.KT.blob_bytes = PK.blob_bytes, L.KT.nblk = PK.nblk, L.KT.fast = PK.fast;
+      }
     }
     if (!T.fast && !L.rtmp && q < Lc) AMG_ALLOC(H, L.rtmp, double, L.n, st);
   }
@@ -1531,10 +1549,11 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
   const TileDesc d = tiles[t];
   if (d.nr <= 0) return;
   unsigned char* base = blob + (size_t)d.blob16 * 16u;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const int2* slices = reinterpret_cast<const int2*>(base);
   const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + p.o_perm);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
+  float* o_val32 = reinterpret_cast<float*>(base + p.o_val);
   for (int j = 0; j < d.nsl; ++j) {
     const int2 sl = slices[j];
     for (int q = threadIdx.x; q < 32 * sl.y; q += blockDim.x) {
@@ -1546,7 +1565,10 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
         const int s = rowptr[r];
         if (k < rowptr[r + 1] - s) v = val[s + k];
       }
-      o_val[sl.x + q] = v;
+      if (d.vb == 4)
+        o_val32[sl.x + q] = (float)v;
+      else
+        o_val[sl.x + q] = v;
     }
   }
 }
@@ -1633,9 +1655,11 @@ amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fa
     Level& L = H->lv[l];
     if (l < Lc) k_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, o.smoother, o.omega, L.dinv);
     if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.val, L.blob);
+    if (L.K.fast) k_blob_refill<<<L.K.nblk, 256, 0, st>>>(L.K.nblk, L.K.tiles, L.rowptr, L.val, L.K.blob);
     if (H->have_T) {
       k_gather_vals<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, L.val, L.T.src, L.T.val);
       if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.val, L.T.blob);
+      if (L.KT.fast) k_blob_refill<<<L.KT.nblk, 256, 0, st>>>(L.KT.nblk, L.KT.tiles, L.T.rowptr, L.T.val, L.KT.blob);
     }
   }
   AMG_CUDA_TRY(H, cudaGetLastError());

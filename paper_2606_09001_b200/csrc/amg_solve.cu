@@ -14,6 +14,7 @@ thread_local int64_t g_nlaunch = 0;  // kernel launches enqueued by this thread 
 
 thread_local bool g_pdl = false;     // true while an iteration is being captured with programmatic edges
 thread_local cudaGraphConditionalHandle g_loop = 0;  // != 0 while the body of a WHILE node is being captured
+thread_local int g_kop = 0;          // 1: the Krylov method's own SpMV (mixed-precision hierarchy: the fp64 blobs of level 0)
 thread_local int g_tr = 0;           // 1: the level operators are the transposed ones (A_l^T, nonsymmetric adjoint)
 
 // kernel launch; with g_pdl the kernel may become resident while its predecessor drains
@@ -54,8 +55,19 @@ inline int red_grid(const amg_handle_s* H, int n) {
 }
 
 // ---- dispatch of the row kernels ---------------------------------------------------------
-inline int lv_fast(const Level& L) { return g_tr ? L.T.fast : L.fast; }
-inline int lv_nblk(const Level& L) { return g_tr ? L.T.nblk : L.nblk; }
+inline const LevelOpT* lv_kop(const Level& L) {  // fp64 blobs for the Krylov SpMV of a mixed-precision hierarchy
+  if (!g_kop) return nullptr;
+  const LevelOpT* K = g_tr ? &L.KT : &L.K;
+  return K->fast ? K : nullptr;
+}
+inline int lv_fast(const Level& L) {
+  if (g_kop && L.v32) return lv_kop(L) != nullptr;  // no fp64 blobs: the row-vector kernels on the fp64 CSR
+  return g_tr ? L.T.fast : L.fast;
+}
+inline int lv_nblk(const Level& L) {
+  if (const LevelOpT* K = lv_kop(L)) return K->nblk;
+  return g_tr ? L.T.nblk : L.nblk;
+}
 
 template <int OP, int NDOT, bool STREAM>
 void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
@@ -95,7 +107,11 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
   RowArgs a;
   memset(&a, 0, sizeof(a));
   a.n = L.n;
-  if (g_tr) {
+  a.v32 = (L.v32 && !g_kop) ? 1 : 0;
+  if (const LevelOpT* K = lv_kop(L)) {
+    a.rowptr = g_tr ? L.T.rowptr : L.rowptr, a.col = g_tr ? L.T.col : L.col, a.val = g_tr ? L.T.val : L.val;
+    a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx, a.halo_cagg = K->halo_cagg;
+  } else if (g_tr) {
     a.rowptr = L.T.rowptr, a.col = L.T.col, a.val = L.T.val;
     a.tiles = L.T.tiles, a.ntiles = L.T.nblk, a.blob = L.T.blob;
     a.halo_idx = L.T.halo_idx, a.halo_cagg = L.T.halo_cagg;
@@ -255,6 +271,7 @@ amg_status amg_setup_tail(amg_handle_s* H, int transposed, cudaStream_t st) {
     T.dinv = L.dinv;
     T.agg = L.agg;
     T.agg_ptr = L.agg_ptr;
+    T.v32 = L.v32;
   }
   TailLevel* d;
   AMG_ALLOC(H, d, TailLevel, nlev, st);
@@ -391,7 +408,9 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   Level& L0 = H->lv[0];
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *q = H->kv[3];
+  g_kop = 1;
   op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
+  g_kop = 0;
   ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, L0.dinv, l0_x1(H, precond), H->partials,
                                                                         H->counter, H->ctl);
   double* z = r;
@@ -420,12 +439,16 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
     AMG_TRY(sv);
     phat = zz;  // == ph on every path of the cycle: the second V-cycle of this iteration may overwrite the level-0 buffers
   }
+  g_kop = 1;
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
+  g_kop = 0;
   ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, L0.dinv, l0_x1(H, precond), H->partials,
                                                                         H->counter, H->ctl);
   double* shat = s;
   if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st, l0_x1(H, precond) != nullptr));
+  g_kop = 1;
   op_spmv(H, L0, shat, t, 2, s, FIN_TS_TT, H->ctl, st);
+  g_kop = 0;
   ++g_nlaunch, launch(k_bicg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, phat, shat, s, t, rhat, x, r, H->partials, H->counter,
                                                    H->ctl);
   if (g_loop) ++g_nlaunch, launch(k_while_ctl, 1, 1, 0, st)((const KrylovCtl*)H->ctl, g_loop);

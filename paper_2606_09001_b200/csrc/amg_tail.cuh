@@ -21,6 +21,7 @@ constexpr int TAIL_MAX_LEVELS = 32;
 
 struct TailLevel {
   int n, nc, nnz, lpr;
+  int v32, pad;  // v32: the level's values are rounded to fp32 on the fly (mixed-precision hierarchy)
   const int* rowptr;
   const int* col;
   const double* val;
@@ -51,6 +52,8 @@ struct TailOpView {
   const int* agg;
   const int* agg_ptr;
   int lpr;
+  int v32;
+  __device__ __forceinline__ double a(int k) const { return v32 ? (double)(float)val[k] : val[k]; }
 };
 
 // one smoother-type pass over rows [R0, R1) by the T threads of a group (this thread is t);
@@ -88,7 +91,7 @@ __device__ __forceinline__ double tl_row_pass(const TailOpView& A, int R0, int R
           xc = tl_ld<CG>(x + c) + gamma * tl_ld<CG>(ec + __ldg(A.agg + c));
         else
           xc = tl_ld<CG>(x + c);
-        s += A.val[k] * xc;
+        s += A.a(k) * xc;
       }
     }
     for (int o = lpr >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
@@ -135,7 +138,7 @@ __device__ __forceinline__ void tl_restrict_pass(const TailOpView& A, int A0, in
     double s = 0.0;
     if (act) {
       const int ra = __ldg(A.agg_ptr + I), rb = __ldg(A.agg_ptr + I + 1);
-      for (int k = A.rp[ra] + sub, e = A.rp[rb]; k < e; k += lpr) s -= A.val[k] * tl_ld<CG>(x + A.col[k]);
+      for (int k = A.rp[ra] + sub, e = A.rp[rb]; k < e; k += lpr) s -= A.a(k) * tl_ld<CG>(x + A.col[k]);
       for (int i = ra + sub; i < rb; i += lpr) s += tl_ld<CG>(b + i);
     }
     for (int o = lpr >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
@@ -286,7 +289,7 @@ static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailB
     const TailLevel L = a.lv[l];
     TailOpView A;
     A.rp = L.rowptr, A.col = L.col, A.val = L.val, A.dinv = L.dinv;
-    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr;
+    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr, A.v32 = L.v32;
     double* b = vb(l);
     double* cur = b + L.n;
     double* oth = cur + L.n;
@@ -325,7 +328,7 @@ static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailB
     const TailLevel L = a.lv[l];
     TailOpView A;
     A.rp = L.rowptr, A.col = L.col, A.val = L.val, A.dinv = L.dinv;
-    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr;
+    A.dinv_g = L.dinv, A.agg = L.agg, A.agg_ptr = L.agg_ptr, A.lpr = L.lpr, A.v32 = L.v32;
     double* b = vb(l);
     double* x = b + L.n;
     double* x2 = x + L.n;

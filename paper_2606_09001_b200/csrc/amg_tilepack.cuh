@@ -14,6 +14,7 @@
 //                          >= nr -> entry (col - nr) of the tile's halo list.  Slice-major; inside a
 //                          slice k-major: slot = first + 32 k + lane  (conflict-free shared-memory reads)
 //   val     f64[nslots]    matrix values, same order; padding slots are {col 0, val 0}
+//           (f32[nslots] with the mixed-precision hierarchy, TileDesc::vb = 4: 6 bytes per entry)
 //
 // and a range [halo_off, halo_off + nhalo) of the level's halo arrays
 //
@@ -37,7 +38,8 @@ struct alignas(16) TileDesc {  // 48 bytes per tile
   int32_t nhalo;
   uint32_t blob16;             // blob offset in 16-byte units
   int32_t halo_off;            // first entry of the tile in the level's halo arrays
-  int32_t pad0, pad1, pad2;
+  int32_t vb;                  // bytes per stored value: 8 (fp64) or 4 (fp32, mixed-precision hierarchy)
+  int32_t pad1, pad2;
 };
 
 __host__ __device__ inline int tp_up(int x, int m) { return (x + m - 1) / m * m; }
@@ -45,12 +47,12 @@ __host__ __device__ inline int tp_up(int x, int m) { return (x + m - 1) / m * m;
 struct BlobLayout {  // byte offsets inside the blob; all multiples of 16
   int o_perm, o_col, o_val, end;
 };
-__host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots) {
+__host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots, int vb) {
   BlobLayout p;
   p.o_perm = tp_up(8 * nsl, 16);
   p.o_col = p.o_perm + 64 * nsl;
   p.o_val = p.o_col + tp_up(2 * nslots, 16);
-  p.end = p.o_val + 8 * nslots;
+  p.end = p.o_val + tp_up(vb * nslots, 16);
   return p;
 }
 
@@ -68,7 +70,7 @@ struct StageLayout {
 enum { TP_B = 1, TP_D = 2, TP_DC = 8, TP_AGGPTR = 16, TP_OUT = 64 };
 __host__ __device__ inline StageLayout tp_stage(const TileDesc& d, int flags) {
   StageLayout t;
-  const BlobLayout p = tp_blob(d.nsl, d.nslots);
+  const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const int r1 = d.r0 + d.nr;
   t.ra2 = d.r0 & ~1;
   t.nrv = tp_up(r1 - t.ra2, 2);

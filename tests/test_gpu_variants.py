@@ -211,3 +211,75 @@ def test_warm_resetup_of_a_nonsymmetric_handle(oracle_mod, B):
         s.close()
         o0.close()
         o1.close()
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(force_generic=1), dict(tail_dense_rows=0)])
+@pytest.mark.parametrize("case", [(3, 40), (4, 28)])
+def test_mixed_precision_hierarchy_matches_the_oracle(oracle_mod, B, case, opts):
+    """hierarchy_fp32 = 1 (NEXT-4): the V-cycle's sparse level operators stored in fp32 (6 bytes per
+    entry), used in fp64 arithmetic; the Krylov operator, dinv, the LU and all vectors fp64.  The oracle rounds the
+    same values: the V-cycle agrees to 1e-12 as in fp64 mode, the solves to the usual bars."""
+    cfg, edge = case
+    A = inputs.config_matrix(cfg, edge)
+    Asp = A.to_scipy()
+    n = A.n
+    b = inputs.config_rhs(cfg, n)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, hierarchy_fp32=1)
+    o64 = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, hierarchy_fp32=1, **opts)
+    try:
+        assert s.num_levels == o.num_levels
+        for l in range(s.num_levels - 1):
+            assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l))
+        r = np.random.default_rng(3).standard_normal(n)
+        z = s.apply_preconditioner(r).cpu().numpy()
+        assert rel(z, o.vcycle(r, 0)) <= 1e-12
+        if cfg == 4:  # (the integer stencils of cfg 3 are exact in fp32: the two cycles coincide there)
+            assert 1e-10 < rel(z, o64.vcycle(r, 0)) < 1e-6  # it really is the rounded operator
+        for l in range(1, s.num_levels):
+            nl = s.level_info(l)[0]
+            bl = np.random.default_rng(100 + l).standard_normal(nl)
+            assert rel(s.level_op(l, 5, None, bl, nl).cpu().numpy(), o.vcycle(bl, l)) <= 1e-12
+        for krylov in (0, 1):
+            xg, ig = s.solve(b, 1e-8, 500, krylov)
+            xo, io = o.solve(b, 1e-8, 500, krylov, 1)
+            assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+            assert np.linalg.norm(b - Asp @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)   # fp64 residual, fp64 A
+            xg, _ = s.solve(b, 1e-11, 500, krylov)
+            xo, _ = o64.solve(b, 1e-13, 500, krylov, 1)
+            assert rel(xg.cpu().numpy(), xo) <= 1e-6
+        # batched solve, warm resetup (fp32 value sections refilled), adjoint
+        Bh = np.stack([inputs.rhs_uniform(n, 60 + k) for k in range(8)])
+        Bd = torch.as_tensor(Bh).cuda().contiguous()
+        X = torch.empty_like(Bd)
+        infos = B.amg_solve_batched(s.h, 0, Bd, X, 8, n, 1e-8, 500)
+        for k in (0, 7):
+            xo, io = o.solve(Bh[k], 1e-8, 500, 0, 1)
+            assert infos[k].status == 0 and abs(infos[k].iterations - io.iterations) <= 2
+            assert np.linalg.norm(Bh[k] - Asp @ X[k].cpu().numpy()) <= 1e-8 * np.linalg.norm(Bh[k])
+        s.resetup_values(A.val * 2.0, keep_aggregates=True)
+        z2 = s.apply_preconditioner(r).cpu().numpy()
+        assert rel(z2, 0.5 * z) <= 1e-12
+        x2, i2 = s.solve(b, 1e-8, 500, 0)
+        assert i2.status == 0 and np.linalg.norm(b - 2.0 * (Asp @ x2.cpu().numpy())) <= 1e-8 * np.linalg.norm(b)
+    finally:
+        s.close()
+        o.close()
+        o64.close()
+
+
+def test_mixed_precision_hierarchy_nonsymmetric(oracle_mod, B):
+    A = inputs.stretched_channel_csr((12, 20, 16), 2.0)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, symmetric=0, hierarchy_fp32=1)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, hierarchy_fp32=1)
+    try:
+        r = np.random.default_rng(8).standard_normal(A.n)
+        assert rel(s.level_op(0, 8, None, r, A.n).cpu().numpy(), o.vcycle_transpose(r, 0)) <= 1e-12
+        g = inputs.rhs_uniform(A.n, 9)
+        lam, il = s.solve_transpose(g, 1e-8, 500)
+        lo, ilo = o.solve_transpose(g, 1e-8, 500, 1, 1, 0)
+        assert il.status == ilo.status == 0 and abs(il.iterations - ilo.iterations) <= 2
+        assert np.linalg.norm(g - A.to_scipy().T @ lam.cpu().numpy()) <= 1e-8 * np.linalg.norm(g)
+    finally:
+        s.close()
+        o.close()
