@@ -325,16 +325,10 @@ amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X
   Level& L0 = H->lv[0];
   const int n = L0.n;
   const int64_t launches0 = gb_nlaunch;
-  KrylovCtlB& init = B.h_ctl[5];
-  memset(&init, 0, sizeof(init));
-  for (int s = 0; s < NB; ++s) {
-    init.c[s].rtol = rtol;
-    init.c[s].maxit = maxit;
-    init.c[s].status = AMG_MAXIT;
-  }
-  AMG_CUDA_TRY(H, cudaMemcpyAsync(B.ctl, &init, sizeof(KrylovCtlB), cudaMemcpyHostToDevice, st));
+  CtlInit ci;
+  ci.rtol = rtol, ci.maxit = maxit, ci.hist = nullptr, ci.hist_cap = 0;
   launch_b(k_krylov_init_b, red_grid_b(H, n), RED_THREADS, 0, st, n, ncols, ld, d_B, (const int*)L0.inv,
-           (const double*)L0.dinv, B.kv[1], B.kv[0], B.x2[0], B.partials, B.counter, B.ctl);
+           (const double*)L0.dinv, B.kv[1], B.kv[0], B.x2[0], B.partials, B.counter, B.ctl, ci);
   AMG_CUDA_TRY(H, cudaGetLastError());
   const bool graph = H->opt.use_graph && maxit > 0;
   if (graph) {

@@ -480,7 +480,12 @@ static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init_b(int n, int
                                                                const int* __restrict__ inv,
                                                                const double* __restrict__ dinv, double* __restrict__ r,
                                                                double* __restrict__ x, double* __restrict__ x1,
-                                                               double* partials, unsigned* counter, KrylovCtlB* ctl) {
+                                                               double* partials, unsigned* counter, KrylovCtlB* ctl,
+                                                               CtlInit ci) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {  // loop control of every column (see k_krylov_init)
+    for (int s = 0; s < NB; ++s) ci.apply(&ctl->c[s]);
+    ctl->all_done = 0;
+  }
   double acc[NB];
 #pragma unroll
   for (int s = 0; s < NB; ++s) acc[s] = 0.0;

@@ -881,6 +881,17 @@ static __global__ void __launch_bounds__(256) k_lu_solve_small(int n, const doub
   lu_solve_small_cta<true>(n, lu, piv, b, x, lu_sm);
 }
 
+// rtol / maxit / residual-history buffer of one solve, handed to the init kernel by value
+struct CtlInit {
+  double rtol;
+  double* hist;
+  int maxit, hist_cap;
+  __device__ __forceinline__ void apply(KrylovCtl* c) const {
+    c->rtol = rtol, c->maxit = maxit, c->hist = hist, c->hist_cap = hist_cap;
+    c->done = 0, c->status = AMG_MAXIT, c->iter = 0, c->halfstep = 0;
+  }
+};
+
 // ------------------------------------------------------------------------------------------
 // S7/S8: fused Krylov vector kernels (grid-stride, one pass each, scalars read from KrylovCtl)
 // ------------------------------------------------------------------------------------------
@@ -891,7 +902,10 @@ static __global__ void __launch_bounds__(RED_THREADS) k_krylov_init(int n, const
                                                              double* __restrict__ z1, double* __restrict__ rhat,
                                                              const double* __restrict__ dinv, double* __restrict__ x1,
                                                              double* partials, unsigned* counter, KrylovCtl* ctl,
-                                                             int fin) {
+                                                             int fin, CtlInit ci) {
+  // loop control of this solve: written here (no host-to-device copy that a following call could race with);
+  // ordered before the last block's finalisation by this block's fence + ticket in grid_reduce_finalize
+  if (blockIdx.x == 0 && threadIdx.x == 0) ci.apply(ctl);
   double acc[1] = {0.0};
   for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * RED_THREADS) {
     const double v = b_nat[inv[i]];

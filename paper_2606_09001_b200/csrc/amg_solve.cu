@@ -600,12 +600,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4];
   const int64_t launches0 = g_nlaunch;
-  // loop control: rtol / maxit go to the device once
-  KrylovCtl init;
-  memset(&init, 0, sizeof(init));
-  init.rtol = rtol;
-  init.maxit = maxit;
-  init.status = AMG_MAXIT;
+  // loop control: rtol / maxit / the history buffer go to the device as arguments of the init kernel
   if (H->hist_cap < maxit) {  // residual history (PAPER.md:125 diagnostics): one entry per iteration
     if (H->hist) {
       AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
@@ -619,14 +614,12 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
       return AMG_ERR_OOM;
     }
   }
-  init.hist = H->hist;
-  init.hist_cap = H->hist_cap;
+  CtlInit ci;
+  ci.rtol = rtol, ci.maxit = maxit, ci.hist = H->hist, ci.hist_cap = H->hist_cap;
   H->hist_len = 0;
-  H->h_ctl[5] = init;
-  AMG_CUDA_TRY(H, cudaMemcpyAsync(H->ctl, &H->h_ctl[5], sizeof(KrylovCtl), cudaMemcpyHostToDevice, st));
   if (krylov == 0) {
     ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, L0.dinv,
-                                                         l0_x1(H, precond), H->partials, H->counter, H->ctl, FIN_INIT_PCG);
+                                                         l0_x1(H, precond), H->partials, H->counter, H->ctl, FIN_INIT_PCG, ci);
     if (precond && H->opt.use_graph && maxit > 0) {
       cudaGraphExec_t gstart = nullptr;
       AMG_TRY(get_iteration_graph(H, -1, 1, st, &gstart));
@@ -640,7 +633,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
     }
   } else {
     ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, v, rhat, nullptr, nullptr,
-                                                         H->partials, H->counter, H->ctl, FIN_INIT_BICG);
+                                                         H->partials, H->counter, H->ctl, FIN_INIT_BICG, ci);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
 
