@@ -36,7 +36,7 @@ class Options(C.Structure):
                 ("max_match_rounds", C.c_int32), ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double),
                 ("hash_seed", C.c_uint64), ("agg_passes", C.c_int32), ("symmetric", C.c_int32),
-                ("hierarchy_fp32", C.c_int32)]
+                ("hierarchy_fp32", C.c_int32), ("pad0", C.c_int32), ("cheby_ratio", C.c_double)]
 
 
 class Info(C.Structure):
@@ -226,6 +226,13 @@ class Oracle:
         _check(lib().oracle_grad_values(self._h, _p(lam), _p(x), C.c_int32(nrhs),
                                         C.c_int64(self.n), _p(gA), C.c_int32(acc)), "grad_values")
         return gA
+
+
+def cheby_weights(k: int, ratio: float) -> np.ndarray:
+    """Sweep weights of the Chebyshev-accelerated L1-Jacobi smoother (smoother = 2)."""
+    w = np.empty(k)
+    _check(lib().oracle_cheby_weights(C.c_int32(k), C.c_double(ratio), _p(w)), "cheby_weights")
+    return w
 
 
 def aggregate(rowptr, col, val, beta=0.25, salt=0, max_rounds=0, mode=0, symmetric=1):

@@ -338,9 +338,22 @@ std::vector<double> smoother_diag(const Csr& A, int smoother, double omega) {
       l1 += std::fabs(A.val[k]);
       if (A.col[k] == i) aii = A.val[k];
     }
-    d[i] = smoother == 0 ? 1.0 / l1 : omega / aii;
+    d[i] = smoother == 1 ? omega / aii : 1.0 / l1;  // 0 and 2 (Chebyshev-accelerated L1-Jacobi): the l1 diagonal
   }
   return d;
+}
+
+// Chebyshev-accelerated L1-Jacobi (smoother = 2, NEXT-4).  spec(D_l1^-1 A) lies in (0, 1] for the M-matrix-like
+// operators of the method (Gershgorin), so no eigenvalue estimate is needed: the k sweeps of one smoothing step are
+// Richardson steps x += tau_j D_l1^-1 (b - A x) whose weights are the reciprocals of the roots of the degree-k
+// Chebyshev polynomial of the interval [1/ratio, 1]:  r_j = (1+a)/2 + (1-a)/2 cos(pi (2j+1) / (2k)), a = 1/ratio.
+// The product of the k error factors (1 - tau_j mu) is the polynomial of degree k with p(0) = 1 of least maximum
+// on [a, 1]:  max |p| = 1 / T_k((1+a)/(1-a)).  j ascending: weights ascending (the mildest step first).
+std::vector<double> cheby_weights(int k, double ratio) {
+  std::vector<double> w(k > 0 ? k : 0);
+  const double a = 1.0 / ratio, pi = 3.14159265358979323846;
+  for (int j = 0; j < k; ++j) w[j] = 1.0 / ((1.0 + a) / 2 + (1.0 - a) / 2 * std::cos(pi * (2 * j + 1) / (2.0 * k)));
+  return w;
 }
 
 // dense LU with partial pivoting, in place, row-major; returns false if singular (O-1)
@@ -480,12 +493,12 @@ int setup(oracle_handle_s* H, Csr A0, int nagg, const int32_t* const* aggs) {
 // `T` selects the transposed hierarchy (B^T) for the nonsymmetric adjoint (O-7)
 // ------------------------------------------------------------------------------------------
 void jacobi_sweep(const Csr& A, const std::vector<double>& dinv, const double* b, const double* x,
-                  double* xout) {  // all rows from the old x
+                  double* xout, double w = 1.0) {  // all rows from the old x; w: Chebyshev weight of the sweep
 #pragma omp parallel for num_threads(g_threads) schedule(static) if (A.n > 20000)
   for (int i = 0; i < A.n; ++i) {
     double s = 0.0;
     for (int k = A.rowptr[i]; k < A.rowptr[i + 1]; ++k) s += A.val[k] * x[A.col[k]];
-    xout[i] = x[i] + dinv[i] * (b[i] - s);
+    xout[i] = x[i] + (w * dinv[i]) * (b[i] - s);
   }
 }
 
@@ -517,10 +530,14 @@ void vcycle(const oracle_handle_s* H, int l, bool T, const double* b, double* x)
   }
   const oracle_options& o = H->opt;
   std::vector<double> tmp(n);
+  const std::vector<double> wpre = o.smoother == 2 ? cheby_weights(o.pre_sweeps, o.cheby_ratio)
+                                                   : std::vector<double>(o.pre_sweeps > 0 ? o.pre_sweeps : 0, 1.0);
+  const std::vector<double> wpost = o.smoother == 2 ? cheby_weights(o.post_sweeps, o.cheby_ratio)
+                                                    : std::vector<double>(o.post_sweeps > 0 ? o.post_sweeps : 0, 1.0);
   if (o.pre_sweeps > 0) {
-    for (int i = 0; i < n; ++i) x[i] = lev.dinv[i] * b[i];  // sweep 1 of nu1 from a zero guess
+    for (int i = 0; i < n; ++i) x[i] = (wpre[0] * lev.dinv[i]) * b[i];  // sweep 1 of nu1 from a zero guess
     for (int s = 1; s < o.pre_sweeps; ++s) {
-      jacobi_sweep(A, lev.dinv, b, x, tmp.data());
+      jacobi_sweep(A, lev.dinv, b, x, tmp.data(), wpre[s]);
       std::memcpy(x, tmp.data(), sizeof(double) * n);
     }
   } else {
@@ -530,8 +547,8 @@ void vcycle(const oracle_handle_s* H, int l, bool T, const double* b, double* x)
   residual_restrict(A, lev, b, x, rc.data());
   vcycle(H, l + 1, T, rc.data(), ec.data());
   for (int i = 0; i < n; ++i) x[i] = x[i] + o.coarse_scale * ec[lev.agg[i]];
-  for (int s = 0; s < o.post_sweeps; ++s) {
-    jacobi_sweep(A, lev.dinv, b, x, tmp.data());
+  for (int s = 0; s < o.post_sweeps; ++s) {  // Chebyshev: the weights in reverse order (B stays symmetric for nu1 = nu2)
+    jacobi_sweep(A, lev.dinv, b, x, tmp.data(), wpost[o.post_sweeps - 1 - s]);
     std::memcpy(x, tmp.data(), sizeof(double) * n);
   }
 }
@@ -711,6 +728,7 @@ void oracle_options_default(oracle_options* o) {
   o->agg_passes = 1;
   o->symmetric = 1;
   o->hierarchy_fp32 = 0;
+  o->cheby_ratio = 6.0;
 }
 
 void oracle_set_threads(int nthreads) { g_threads = nthreads > 0 ? nthreads : 1; }
@@ -893,6 +911,13 @@ int oracle_solve_transpose(oracle_handle h, const double* g, double* lambda, dou
     pcg(h, h->lv[0].At, true, g, lambda, rtol, maxit, precond, info);
   else
     bicgstab(h, h->lv[0].At, true, g, lambda, rtol, maxit, precond, info);
+  return ORACLE_OK;
+}
+
+int oracle_cheby_weights(int32_t k, double ratio, double* w) {
+  if (k < 0 || !(ratio > 1.0) || (k > 0 && !w)) return ORACLE_ERR_INVALID_ARG;
+  const std::vector<double> v = cheby_weights(k, ratio);
+  std::copy(v.begin(), v.end(), w);
   return ORACLE_OK;
 }
 

@@ -46,7 +46,10 @@ extern "C" {
 typedef struct {
   int32_t pre_sweeps;       /* nu1, default 2 (BASELINE.json cfg 1)                         */
   int32_t post_sweeps;      /* nu2, default 2                                               */
-  int32_t smoother;         /* 0 = L1-Jacobi  d_i = sum_j |a_ij|  (A7);  1 = damped Jacobi  */
+  int32_t smoother;         /* 0 = L1-Jacobi  d_i = sum_j |a_ij|  (A7);  1 = damped Jacobi;
+                               2 = Chebyshev-accelerated L1-Jacobi (NEXT-4): the nu sweeps of a smoothing step are
+                               x += tau_j D_l1^-1 (b - A x) with tau_j the reciprocal roots of the degree-nu Chebyshev
+                               polynomial of [1/cheby_ratio, 1]; post-sweeps in reverse order                 */
   int32_t coarse_max_rows;  /* stop coarsening at n_l <= this; default 64 (A6)              */
   int32_t max_levels;       /* default 32                                                   */
   int32_t max_match_rounds; /* 0 = until fix-point                                          */
@@ -64,6 +67,8 @@ typedef struct {
                                inside the V-cycle every sparse level operator A_l, l < L, is the fp64 operator with
                                each value rounded to fp32, used in fp64 arithmetic; dinv, the coarsest LU, the Krylov
                                operator A, all vectors and all sums stay fp64.  default 0                        */
+  int32_t pad0;
+  double cheby_ratio;       /* smoother = 2: the smoothing interval of spec(D_l1^-1 A) is [1/cheby_ratio, 1]; default 6 */
 } oracle_options;
 
 typedef struct {
@@ -123,6 +128,10 @@ int oracle_vcycle(oracle_handle h, int32_t level, const double* r, double* z);
 /* O-7: z = B^T r, the same cycle on the transposed level operators A_l^T (same aggregates, same
  * dinv, LU of A_L^T): exactly the transpose of the linear map of oracle_vcycle when nu1 = nu2. */
 int oracle_vcycle_transpose(oracle_handle h, int32_t level, const double* r, double* z);
+
+/* smoother = 2: the k sweep weights tau_0 <= ... <= tau_{k-1} of one smoothing step (pre-sweeps in this order,
+ * post-sweeps reversed). */
+int oracle_cheby_weights(int32_t k, double ratio, double* w);
 
 /* O-5 / O-6.  krylov: 0 = PCG, 1 = right-preconditioned BiCGSTAB.  precond: 1 = AMG V-cycle,
  * 0 = identity.  x0 = 0.  x is output only. */

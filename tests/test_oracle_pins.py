@@ -1006,3 +1006,80 @@ def test_mixed_precision_hierarchy(oracle_mod):
     g = np.random.default_rng(6).standard_normal(N.n)
     lam, il = on.solve_transpose(g, rtol=1e-11, maxit=300, krylov=1, symmetric=0)
     assert il.status == 0 and np.allclose(lam, np.linalg.solve(D.T, g), rtol=1e-7, atol=1e-9)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-4: Chebyshev-accelerated L1-Jacobi (smoother = 2)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ratio", [2.0, 6.0, 30.0])
+@pytest.mark.parametrize("k", [1, 2, 3, 4])
+def test_chebyshev_weights_are_the_minimax_polynomial(oracle_mod, k, ratio):
+    """p(mu) = prod_j (1 - tau_j mu) must be THE degree-k polynomial with p(0) = 1 of least maximum on [1/ratio, 1]:
+    max |p| = 1 / T_k((1+a)/(1-a)), attained k+1 times with alternating sign (equioscillation); a wrong root
+    formula, interval or order of the reciprocal fails one of these."""
+    tau = oracle_mod.cheby_weights(k, ratio)
+    a = 1.0 / ratio
+    assert np.all(np.diff(tau) > 0) and tau[0] > 1.0 and tau[-1] < ratio  # ascending, roots inside (a, 1)
+    mu = np.linspace(a, 1.0, 200001)
+    p = np.prod(1.0 - tau[:, None] * mu[None, :], axis=0)
+    t = (1 + a) / (1 - a)
+    Tk = np.cosh(k * np.arccosh(t))
+    assert abs(np.max(np.abs(p)) - 1.0 / Tk) <= 1e-9 / Tk * 1e3
+    ext = np.cos(np.pi * np.arange(k + 1) / k) * (1 - a) / 2 + (1 + a) / 2  # extrema of T_k mapped to [a, 1]
+    pe = np.prod(1.0 - tau[:, None] * ext[None, :], axis=0)
+    assert np.allclose(np.abs(pe), 1.0 / Tk, rtol=1e-10) and np.all(pe[:-1] * pe[1:] < 0)
+    assert np.all(np.abs(np.prod(1.0 - tau[:, None] * np.linspace(0, a, 1001)[None, :], axis=0)) <= 1.0 + 1e-12)
+
+
+def py_vcycle_w(o, l, b, wpre, wpost, gamma=1.0):
+    """O-4 with per-sweep weights, written out with scipy matrices (post-sweeps take wpost in reverse order)."""
+    import scipy.sparse as sp
+
+    L = o.num_levels - 1
+    rp, cl, vl = o.level_csr(l)
+    n = len(rp) - 1
+    A = sp.csr_matrix((vl, cl, rp), shape=(n, n))
+    if l == L:
+        return np.linalg.solve(A.toarray(), b)
+    dinv, agg, nc = o.dinv(l), o.aggregates(l), o.level_info(l + 1)[0]
+    x = wpre[0] * dinv * b
+    for w in wpre[1:]:
+        x = x + w * dinv * (b - A @ x)
+    rc = np.bincount(agg, weights=b - A @ x, minlength=nc)
+    x = x + gamma * py_vcycle_w(o, l + 1, rc, wpre, wpost, gamma)[agg]
+    for w in wpost[::-1]:
+        x = x + w * dinv * (b - A @ x)
+    return x
+
+
+def test_chebyshev_smoother(oracle_mod):
+    A = inputs.variable_diffusion_csr((10, 10, 10), seed=4, sigma=1.5, ell=3.0)
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, smoother=2, cheby_ratio=6.0)
+    o1 = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+    for l in range(o.num_levels):  # the hierarchy and the l1 diagonal are those of plain L1-Jacobi
+        assert all(np.array_equal(a, b) for a, b in zip(o.level_csr(l), o1.level_csr(l)))
+        if l < o.num_levels - 1:
+            assert np.array_equal(o.dinv(l), o1.dinv(l))
+    # spec(D_l1^-1 A) in (0, 1]: the premise of the fixed interval (Gershgorin), checked densely on level 0
+    D = dense(A)
+    mu = np.linalg.eigvals(np.diag(o.dinv(0)) @ D).real
+    assert mu.min() > 0 and mu.max() <= 1.0 + 1e-12
+    rel = lambda a, b: np.linalg.norm(a - b) / np.linalg.norm(b)
+    w2 = oracle_mod.cheby_weights(2, 6.0)
+    r = np.random.default_rng(2).standard_normal(A.n)
+    assert rel(o.vcycle(r), py_vcycle_w(o, 0, r, w2, w2)) <= 1e-13
+    assert rel(o1.vcycle(r), py_vcycle_w(o1, 0, r, np.ones(2), np.ones(2))) <= 1e-13  # weights 1: the plain cycle
+    # B symmetric positive definite, spec(BA) in (0, 1 + eps]; fewer PCG iterations than plain L1-Jacobi
+    n = A.n
+    Bm = np.column_stack([o.vcycle(e) for e in np.eye(n)[:, :n]])
+    assert np.linalg.norm(Bm - Bm.T) <= 1e-13 * np.linalg.norm(Bm)
+    ev = np.linalg.eigvals(Bm @ D).real
+    assert ev.min() > 0 and ev.max() <= 1.0 + 1e-10
+    b = inputs.rhs_uniform(n, 3)
+    x, ic = o.solve(b, rtol=1e-10, maxit=200)
+    x1, i1 = o1.solve(b, rtol=1e-10, maxit=200)
+    assert ic.status == 0 and ic.iterations < i1.iterations
+    assert np.linalg.norm(b - A.to_scipy() @ x) <= 1.01e-10 * np.linalg.norm(b)
+    # unequal sweep counts: weights of degree nu1 before, degree nu2 (reversed) after
+    o32 = oracle_mod.Oracle(A.rowptr, A.col, A.val, smoother=2, pre_sweeps=3, post_sweeps=1)
+    assert rel(o32.vcycle(r), py_vcycle_w(o32, 0, r, oracle_mod.cheby_weights(3, 6.0), oracle_mod.cheby_weights(1, 6.0))) <= 1e-13
