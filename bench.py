@@ -307,12 +307,22 @@ def extra_configs(which, B, inputs, dev, peak):
                     t.append((time.perf_counter() - t0) * 1e3)
                 rs.append(round(min(t), 2))
             B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1)
+            # the same system with the NEXT-4 options on (Chebyshev-weighted L1-Jacobi, size-4 aggregation, fp32 level
+            # operators inside the V-cycle; Krylov and residual in fp64)
+            st_ = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, smoother=2, agg_passes=2, hierarchy_fp32=1)
+            dxt = torch.empty_like(db)
+            tms, tinfo = timed(lambda: B.amg_solve_ex(st_.h, db, dxt, RTOL, MAXIT, 0, 1))
+            tuned = {"options": "smoother=2, agg_passes=2, hierarchy_fp32=1", "solve_ms": round(tms, 3),
+                     "iterations": tinfo.iterations, "levels": st_.num_levels,
+                     "true_rel_residual_host_fp64": hres(Asp, b, dxt.cpu().numpy())}
+            st_.close()
+            del dxt
             out["cfg4"] = {"workload": WORKLOADS[4], "n": n, "nnz": nnz, "levels": s.num_levels, "setup_ms": sms,
                            "setup_first_call_ms": first, "resetup_keep_aggregates_ms": rs[0], "resetup_full_ms": rs[1],
                            "solve_ms": round(ms, 3), "iterations": info.iterations,
                            "true_rel_residual_host_fp64": hres(Asp, b, dx.cpu().numpy()),
                            "solve_phase": solve_phase(s, ms, info.iterations),
-                           "vcycle_ms": round(vms / 10, 4),
+                           "tuned": tuned, "vcycle_ms": round(vms / 10, 4),
                            "vcycle_frac": round(B.amg_get_algorithmic_bytes(s.h, 1) / (vms / 10 * 1e-3) / 1e9 / peak, 4)}
         if "5" in which:
             R = 16
@@ -580,7 +590,9 @@ def run_b200(args):
         # NEXT-4 variants on the same system: mixed-precision hierarchy (fp32 level operators inside the V-cycle, fp64
         # Krylov; default off) and size-4 aggregation
         for key, opts in (("mixed_precision", dict(hierarchy_fp32=1)), ("size4_aggregation", dict(agg_passes=2)),
-                          ("size4_mixed_precision", dict(agg_passes=2, hierarchy_fp32=1))):
+                          ("size4_mixed_precision", dict(agg_passes=2, hierarchy_fp32=1)),
+                          ("chebyshev_smoother", dict(smoother=2)),
+                          ("chebyshev_size4_mixed_precision", dict(smoother=2, agg_passes=2, hierarchy_fp32=1))):
             sv = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **opts)
             dxv = torch.empty_like(d_b)
             for _ in range(2):
@@ -631,6 +643,10 @@ def run_b200(args):
             "solve_phase": {"algorithmic_bytes": solve_bytes, "achieved_gbs": round(solve_gbs, 1), "peak": peak,
                             "frac": round(solve_gbs / peak, 4), "frac_of_8000_nominal": round(solve_gbs / 8000.0, 4),
                             "bytes_per_iteration": bytes_pcg_it, "peak_source": peak_src},
+            "tuned": ({"options": "smoother=2 (Chebyshev-weighted L1-Jacobi), agg_passes=2 (size-4 aggregates), "
+                                  "hierarchy_fp32=1 (fp32 level operators inside the V-cycle; Krylov, residual, vectors fp64); "
+                                  "all default off, each with its oracle option and parity tests",
+                       **phases["chebyshev_size4_mixed_precision"]} if "chebyshev_size4_mixed_precision" in phases else None),
             "vcycle": vc, "phases": phases, "configs": configs, "cpu_baseline": cpu, "clocks": clocks,
         }
         print(json.dumps(out), flush=True)

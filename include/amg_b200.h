@@ -90,7 +90,11 @@ typedef struct {
                                uses the salt hash_seed + l + 1000 p                                          */
   int32_t pre_sweeps;       /* nu1, default 2                                                            */
   int32_t post_sweeps;      /* nu2, default 2                                                            */
-  int32_t smoother;         /* 0 = L1-Jacobi (d_i = sum_j |a_ij|), 1 = damped Jacobi (omega / a_ii)      */
+  int32_t smoother;         /* 0 = L1-Jacobi (d_i = sum_j |a_ij|), 1 = damped Jacobi (omega / a_ii),
+                               2 = Chebyshev-accelerated L1-Jacobi: the nu sweeps of a smoothing step are
+                                   x += tau_j D_l1^-1 (b - A x), tau_j the reciprocal roots of the degree-nu Chebyshev
+                                   polynomial of [1/cheby_ratio, 1] (spec(D_l1^-1 A) lies in (0, 1]); post-sweeps in
+                                   reverse order                                                          */
   int32_t coarse_max_rows;  /* stop coarsening at n_l <= this (default 64); dense LU there               */
   int32_t max_levels;       /* default 32                                                                */
   int32_t max_match_rounds; /* 0 = handshake rounds until the fix-point                                  */
@@ -118,6 +122,7 @@ typedef struct {
                                vectors and all sums stay fp64.  The solve still converges to rtol in fp64.  In this mode
                                the per-level hooks (amg_level_op) see the rounded operators.  default 0            */
   int32_t reserved1;
+  double cheby_ratio;       /* smoother = 2: smoothing interval [1/cheby_ratio, 1]; default 6                    */
 } amg_options;
 
 typedef struct {

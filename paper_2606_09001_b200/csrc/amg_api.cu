@@ -102,7 +102,7 @@ amg_status create_handle(amg_handle* out, int64_t n, int64_t nnz, const int32_t*
     o.struct_size = (int32_t)sizeof(amg_options);
   }
   if (o.pre_sweeps < 0 || o.post_sweeps < 0 || o.max_levels < 1 || o.coarse_max_rows < 1 ||
-      (o.smoother != 0 && o.smoother != 1) || (o.krylov != 0 && o.krylov != 1) || !(o.strong_beta >= 0.0) ||
+      o.smoother < 0 || o.smoother > 2 || !(o.cheby_ratio > 1.0) || o.pre_sweeps + o.post_sweeps > AMG_MAX_SWEEPS || (o.krylov != 0 && o.krylov != 1) || !(o.strong_beta >= 0.0) ||
       o.symmetric < -1 || o.symmetric > 1 || o.agg_passes < 1 || o.agg_passes > 4 || nagg < 0) {
     amg_set_thread_error("amg_setup: option out of range");
     return AMG_ERR_INVALID_ARG;
@@ -209,6 +209,8 @@ amg_status amg_options_default(amg_options* o) {
   o->strong_beta = 0.25;
   o->coarse_scale = 1.0;
   o->hash_seed = 0;
+  o->hierarchy_fp32 = 0;
+  o->cheby_ratio = 6.0;
   return AMG_OK;
 }
 

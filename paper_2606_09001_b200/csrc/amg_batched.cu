@@ -64,7 +64,8 @@ void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowA
                       const LevelOpT* K = nullptr) {
   a.n = L.n, a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob, a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
   if (K) a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx, a.halo_cagg = K->halo_cagg;
-  a.dinv = L.dinv, a.agg = L.agg, a.agg_ptr = L.agg_ptr, a.gamma = H->opt.coarse_scale;
+  if (!a.dinv) a.dinv = L.dinv;  // (the sweeps pass the diagonal of their own sweep index: Chebyshev weights)
+  a.agg = L.agg, a.agg_ptr = L.agg_ptr, a.gamma = H->opt.coarse_scale;
   a.partials = H->batch->partials, a.counter = H->batch->counter;
   a.stages = G.stages, a.xslots = G.xslots, a.stage_bytes = G.stage_bytes, a.xslot_bytes = G.xslot_bytes;
   int grid = H->sm_count;  // one CTA per SM
@@ -84,9 +85,9 @@ RowArgsB args_b(KrylovCtlB* ctl) {
 }
 
 void op_jacobi_b(amg_handle_s* H, int l, const double* b, const double* x, double* out, bool dot, KrylovCtlB* ctl,
-                 cudaStream_t st) {
+                 cudaStream_t st, int sweep) {
   RowArgsB a = args_b(ctl);
-  a.x = x, a.b = b, a.out = out, a.fin = FIN_RZ;
+  a.x = x, a.b = b, a.out = out, a.fin = FIN_RZ, a.dinv = H->lv[l].dsw[sweep];
   if (dot)
     launch_rowtile_b<OP_JACOBI, 1>(H, H->lv[l], H->batch->geom[l], a, st);
   else
@@ -113,14 +114,14 @@ amg_status vcycle_b(amg_handle_s* H, int l, const double* b, double** out, Krylo
   const int nu1 = H->opt.pre_sweeps, nu2 = H->opt.post_sweeps;
   double *cur = Bt.x2[l], *oth = Bt.x[l];  // cur = x1 (one sweep from zero)
   for (int s = 1; s < nu1; ++s) {
-    op_jacobi_b(H, l, b, cur, oth, false, ctl, st);
+    op_jacobi_b(H, l, b, cur, oth, false, ctl, st, s);
     std::swap(cur, oth);
   }
   const int lc = l + 1;
   {
     RowArgsB a = args_b(ctl);
     a.x = cur, a.b = b, a.out = Bt.b[lc];
-    if (lc != H->tail_dense_level) a.dinv_c = H->lv[lc].dinv, a.out2 = Bt.x2[lc];  // x1 of the coarse level
+    if (lc != H->tail_dense_level) a.dinv_c = H->lv[lc].dsw[0], a.out2 = Bt.x2[lc];  // x1 of the coarse level
     launch_rowtile_b<OP_RESTRICT, 0>(H, L, Bt.geom[l], a, st);
   }
   double* ec = nullptr;
@@ -128,7 +129,7 @@ amg_status vcycle_b(amg_handle_s* H, int l, const double* b, double** out, Krylo
   const bool want_dot = fuse_rz && l == 0;
   {
     RowArgsB a = args_b(ctl);
-    a.x = cur, a.b = b, a.ec = ec, a.out = oth, a.fin = FIN_RZ;
+    a.x = cur, a.b = b, a.ec = ec, a.out = oth, a.fin = FIN_RZ, a.dinv = L.dsw[nu1];
     if (want_dot && nu2 == 1)
       launch_rowtile_b<OP_JACOBI_PROLONG, 1>(H, L, Bt.geom[l], a, st);
     else
@@ -136,7 +137,7 @@ amg_status vcycle_b(amg_handle_s* H, int l, const double* b, double** out, Krylo
     std::swap(cur, oth);
   }
   for (int s = 1; s < nu2; ++s) {
-    op_jacobi_b(H, l, b, cur, oth, want_dot && s == nu2 - 1, ctl, st);
+    op_jacobi_b(H, l, b, cur, oth, want_dot && s == nu2 - 1, ctl, st, nu1 + s);
     std::swap(cur, oth);
   }
   *out = cur;
@@ -174,7 +175,7 @@ amg_status enqueue_iteration_b(amg_handle_s* H, cudaStream_t st) {
       launch_rowtile_b<OP_SPMV, 1>(H, L0, Bt.geom[0], a, st);
   }
   launch_b(k_pcg_xr_b, red_grid_b(H, (int64_t)n * NB2), RED_THREADS, 0, st, n, (const double*)p, (const double*)q, x, r,
-           (const double*)L0.dinv, Bt.x2[0], Bt.partials, Bt.counter, Bt.ctl);
+           (const double*)L0.dsw[0], Bt.x2[0], Bt.partials, Bt.counter, Bt.ctl);
   double* z = nullptr;
   AMG_TRY(vcycle_b(H, 0, r, &z, Bt.ctl, true, st));
   launch_b(k_pcg_p_b, red_grid_b(H, (int64_t)n * NB2), RED_THREADS, 0, st, n, (const double*)z, p,
@@ -328,7 +329,7 @@ amg_status amg_solve_batch_chunk(amg_handle_s* H, const double* d_B, double* d_X
   CtlInit ci;
   ci.rtol = rtol, ci.maxit = maxit, ci.hist = nullptr, ci.hist_cap = 0;
   launch_b(k_krylov_init_b, red_grid_b(H, n), RED_THREADS, 0, st, n, ncols, ld, d_B, (const int*)L0.inv,
-           (const double*)L0.dinv, B.kv[1], B.kv[0], B.x2[0], B.partials, B.counter, B.ctl, ci);
+           (const double*)L0.dsw[0], B.kv[1], B.kv[0], B.x2[0], B.partials, B.counter, B.ctl, ci);
   AMG_CUDA_TRY(H, cudaGetLastError());
   const bool graph = H->opt.use_graph && maxit > 0;
   if (graph) {

@@ -28,6 +28,7 @@ constexpr int VEC_PAD = 8;        // every vector / index array is over-allocate
                                   // the bulk copies round their slices out to 16-byte boundaries
 constexpr int RB_THREADS = 256;   // row-vector fallback kernels
 constexpr int RED_THREADS = 256;  // BLAS-1 kernels
+constexpr int AMG_MAX_SWEEPS = 12; // most pre + post sweeps of a cycle
 constexpr int MAX_DENSE = 4096;   // largest coarsest level accepted
 
 #include "amg_tilepack.cuh"
@@ -87,6 +88,9 @@ struct Level {
   int* col = nullptr;
   double* val = nullptr;
   double* dinv = nullptr;   // smoother diagonal (null on the coarsest)
+  // diagonal of every sweep of a cycle: pre-sweep s -> dsw[s], post-sweep s -> dsw[nu1 + s].  All equal to dinv unless
+  // the smoother is the Chebyshev-accelerated L1-Jacobi (smoother = 2): then tau * dinv with the sweep's weight
+  double* dsw[AMG_MAX_SWEEPS] = {nullptr};
   int* agg = nullptr;       // [n]  coarse id of every row, non-decreasing
   int* agg_ptr = nullptr;   // [nc+1] first row of every aggregate
   // row-tile partition (boundaries aligned to aggregate starts)
@@ -250,4 +254,5 @@ void amg_batch_release(amg_handle_s* H);
 amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st);
 // setup.cu: NEXT-1 value-only resetup on the kept hierarchy; *fallback = 1: the caller has to rebuild (symmetry changed)
 amg_status amg_ensure_src0(amg_handle_s* H, cudaStream_t st);
+amg_status amg_build_sweep_diagonals(amg_handle_s* H, cudaStream_t st);  // Level::dsw from Level::dinv
 amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fallback, cudaStream_t st);

@@ -40,6 +40,8 @@ struct RowArgs {
   const double* x;      // gathered vector
   const double* b;
   const double* dinv;
+  const double* dinv_x1; // OP_JACOBI0: diagonal of the first sweep from zero (x1 = dinv_x1 o b); = dinv unless the
+                         // sweeps carry Chebyshev weights
   double* out;
   const double* dinv_c; // restriction, optional: smoother diagonal of the coarse level ...
   double* out2;         // ... then out2[I] = dinv_c[I] * out[I] (the first sweep of the coarse level from zero)
@@ -72,7 +74,7 @@ __device__ __forceinline__ double2 ld_d2(const double2* p) {
 
 template <int OP>
 __device__ __forceinline__ double gather_x(const RowArgs& a, int c) {
-  if (OP == OP_JACOBI0) return __ldg(a.dinv + c) * __ldg(a.b + c);
+  if (OP == OP_JACOBI0) return __ldg(a.dinv_x1 + c) * __ldg(a.b + c);
   if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.agg + c));
   return __ldg(a.x + c);
 }
@@ -85,7 +87,7 @@ __device__ __forceinline__ double row_epilogue(const RowArgs& a, int i, double s
   const double di = a.dinv[i], bi = a.b[i];
   double xi;
   if (OP == OP_JACOBI0)
-    xi = di * bi;
+    xi = a.dinv_x1[i] * bi;
   else if (OP == OP_JACOBI_PROLONG)
     xi = a.x[i] + a.gamma * a.ec[a.agg[i]];
   else
@@ -429,7 +431,7 @@ __device__ __forceinline__ void tile_issue(const RowArgs& a, const TileDesc& d, 
 // value of the gathered vector at index i of the level (the fused operations transform it on the fly)
 template <int OP>
 __device__ __forceinline__ double xvalue_local(const RowArgs& a, int i) {
-  if (OP == OP_JACOBI0) return __ldg(a.dinv + i) * __ldg(a.b + i);
+  if (OP == OP_JACOBI0) return __ldg(a.dinv_x1 + i) * __ldg(a.b + i);
   if (OP == OP_JACOBI_PROLONG) return __ldg(a.x + i) + a.gamma * __ldg(a.ec + __ldg(a.agg + i));
   return __ldg(a.x + i);
 }
@@ -549,7 +551,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
             v[u] = __ldg(a.x + c);
             e[u] = __ldg(a.ec + cag[u]);
           } else if (OP == OP_JACOBI0) {
-            v[u] = __ldg(a.dinv + c);
+            v[u] = __ldg(a.dinv_x1 + c);
             e[u] = __ldg(a.b + c);
           } else {
             v[u] = __ldg(a.x + c);
@@ -566,7 +568,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
             lv[u] = __ldg(a.x + i);
             le[u] = __ldg(a.ec + la[u]);
           } else if (OP == OP_JACOBI0) {
-            lv[u] = __ldg(a.dinv + i);
+            lv[u] = __ldg(a.dinv_x1 + i);
             le[u] = __ldg(a.b + i);
           } else {
             lv[u] = __ldg(a.x + i);
@@ -604,7 +606,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         if (OP == OP_JACOBI_PROLONG)
           xh[h] = __ldg(a.x + c) + a.gamma * __ldg(a.ec + __ldg(a.halo_cagg + gc.hoff + h));
         else if (OP == OP_JACOBI0)
-          xh[h] = __ldg(a.dinv + c) * __ldg(a.b + c);
+          xh[h] = __ldg(a.dinv_x1 + c) * __ldg(a.b + c);
         else
           xh[h] = __ldg(a.x + c);
       }

@@ -6,6 +6,7 @@
 // pure function of the matrix and the salt, independent of the thread schedule, so a sequential
 // program following the same definition produces the same integers.
 #include <chrono>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 
@@ -393,7 +394,7 @@ __global__ void k_dinv(int n, const int* __restrict__ rowptr, const int* __restr
     l1 += fabs(val[k]);
     if (col[k] == i) aii = val[k];
   }
-  dinv[i] = smoother == 0 ? 1.0 / l1 : omega / aii;
+  dinv[i] = smoother == 1 ? omega / aii : 1.0 / l1;  // 0 and 2 (Chebyshev-accelerated L1-Jacobi): the l1 diagonal
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1372,6 +1373,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     if (q > 0) AMG_ALLOC(H, L.b, double, L.n, st);
     if (!L.fast && q < Lc) AMG_ALLOC(H, L.rtmp, double, L.n, st);
   }
+  AMG_TRY(amg_build_sweep_diagonals(H, st));
   H->stats.reorder_ms = now_ms() - t_reorder0;
 
   // ---- coarsest dense LU ----
@@ -1602,6 +1604,44 @@ amg_status build_resetup_maps(amg_handle_s* H, cudaStream_t st) {
 
 }  // namespace
 
+namespace {
+__global__ void k_scale_vec(int n, double w, const double* __restrict__ in, double* __restrict__ out) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = w * in[i];
+}
+}  // namespace
+
+// Diagonals of the sweeps of a cycle.  Chebyshev-accelerated L1-Jacobi (smoother = 2, NEXT-4): spec(D_l1^-1 A) lies
+// in (0, 1] (Gershgorin), so the nu sweeps of a smoothing step are Richardson steps x += tau_j D_l1^-1 (b - A x) with
+// tau_j the reciprocal roots of the degree-nu Chebyshev polynomial of [1/ratio, 1] (ascending; post-sweeps reversed,
+// so that B stays symmetric for nu1 = nu2).  tau_j * dinv is stored once per sweep: the kernels do not change.
+amg_status amg_build_sweep_diagonals(amg_handle_s* H, cudaStream_t st) {
+  const amg_options& o = H->opt;
+  const int nu1 = o.pre_sweeps, nu2 = o.post_sweeps;
+  const int Lc = (int)H->lv.size() - 1;
+  auto weights = [&](int k) {
+    std::vector<double> w(k > 0 ? k : 0);
+    const double a = 1.0 / o.cheby_ratio, pi = 3.14159265358979323846;
+    for (int j = 0; j < k; ++j) w[j] = 1.0 / ((1.0 + a) / 2 + (1.0 - a) / 2 * cos(pi * (2 * j + 1) / (2.0 * k)));
+    return w;
+  };
+  const std::vector<double> wpre = weights(nu1), wpost = weights(nu2);
+  for (int l = 0; l < Lc; ++l) {
+    Level& L = H->lv[l];
+    for (int s = 0; s < nu1 + nu2; ++s) {
+      if (o.smoother != 2) {
+        L.dsw[s] = L.dinv;
+        continue;
+      }
+      const double w = s < nu1 ? wpre[s] : wpost[nu2 - 1 - (s - nu1)];
+      if (!L.dsw[s] || L.dsw[s] == L.dinv) AMG_ALLOC(H, L.dsw[s], double, L.n, st);
+      k_scale_vec<<<grid_for(L.n), TPB, 0, st>>>(L.n, w, L.dinv, L.dsw[s]);
+    }
+  }
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  return AMG_OK;
+}
+
 // level 0: position in the caller's CSR of every entry of the permuted CSR (warm resetup, tile gradient)
 amg_status amg_ensure_src0(amg_handle_s* H, cudaStream_t st) {
   Level& L0 = H->lv[0];
@@ -1663,6 +1703,7 @@ amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fa
     }
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
+  AMG_TRY(amg_build_sweep_diagonals(H, st));
   // ---- coarsest LU (factors rebuilt in place), dense tail ----
   {
     Level& L = H->lv[Lc];

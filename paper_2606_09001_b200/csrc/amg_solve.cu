@@ -121,6 +121,7 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
     a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
   }
   a.dinv = L.dinv;
+  a.dinv_x1 = L.dinv;
   a.agg = L.agg;
   a.agg_ptr = L.agg_ptr;
   a.gamma = H->opt.coarse_scale;
@@ -150,7 +151,7 @@ void op_spmv(amg_handle_s* H, const Level& L, const double* x, double* y, int nd
 void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x, double* out, bool dot,
                KrylovCtl* ctl, cudaStream_t st, const double* dinv = nullptr) {
   RowArgs a = base_args(H, L, ctl);
-  if (dinv) a.dinv = dinv;  // a copy of the level's smoother diagonal (timing hook)
+  if (dinv) a.dinv = dinv;  // the diagonal of this sweep (Chebyshev weights), or a copy of it (timing hook)
   a.x = x;
   a.b = b;
   a.out = out;
@@ -161,16 +162,20 @@ void op_jacobi(amg_handle_s* H, const Level& L, const double* b, const double* x
     launch_row<OP_JACOBI, 0>(H, L, a, st);
 }
 
-void op_jacobi0(amg_handle_s* H, const Level& L, const double* b, double* out, KrylovCtl* ctl, cudaStream_t st) {
+void op_jacobi0(amg_handle_s* H, const Level& L, const double* b, double* out, KrylovCtl* ctl, cudaStream_t st,
+                const double* d0 = nullptr, const double* d1 = nullptr) {
   RowArgs a = base_args(H, L, ctl);
+  if (d0) a.dinv_x1 = d0;  // diagonals of the first and the second sweep
+  if (d1) a.dinv = d1;
   a.b = b;
   a.out = out;
   launch_row<OP_JACOBI0, 0>(H, L, a, st);
 }
 
 void op_jacobi_prolong(amg_handle_s* H, const Level& L, const double* b, const double* x, const double* ec,
-                       double* out, bool dot, KrylovCtl* ctl, cudaStream_t st) {
+                       double* out, bool dot, KrylovCtl* ctl, cudaStream_t st, const double* dinv = nullptr) {
   RowArgs a = base_args(H, L, ctl);
+  if (dinv) a.dinv = dinv;
   a.x = x;
   a.b = b;
   a.ec = ec;
@@ -269,6 +274,7 @@ amg_status amg_setup_tail(amg_handle_s* H, int transposed, cudaStream_t st) {
     T.col = transposed ? L.T.col : L.col;
     T.val = transposed ? L.T.val : L.val;
     T.dinv = L.dinv;
+    for (int q = 0; q < AMG_MAX_SWEEPS; ++q) T.dsw[q] = L.dsw[q];
     T.agg = L.agg;
     T.agg_ptr = L.agg_ptr;
     T.v32 = L.v32;
@@ -332,25 +338,25 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
   if (nu1 >= 2 && x1_ready) {
     // the restriction of the level above left x1 = dinv o b in L.x2: the second sweep is a plain one
     // (one gather per halo column instead of the two of the fused pair)
-    op_jacobi(H, L, b, L.x2, cur, false, ctl, st);
+    op_jacobi(H, L, b, L.x2, cur, false, ctl, st, L.dsw[1]);
     done_sweeps = 2;
   } else if (nu1 >= 2) {
-    op_jacobi0(H, L, b, cur, ctl, st);
+    op_jacobi0(H, L, b, cur, ctl, st, L.dsw[0], L.dsw[1]);
     done_sweeps = 2;
   } else if (nu1 == 1) {
-    ++g_nlaunch, launch(k_scale_dinv, grid_for(L.n), TPB, 0, st)(L.n, L.dinv, b, cur, ctl);
+    ++g_nlaunch, launch(k_scale_dinv, grid_for(L.n), TPB, 0, st)(L.n, L.dsw[0], b, cur, ctl);
     done_sweeps = 1;
   } else {
     ++g_nlaunch, launch(k_zero, grid_for(L.n), TPB, 0, st)(L.n, cur, ctl);
   }
   for (int s = done_sweeps; s < nu1; ++s) {
-    op_jacobi(H, L, b, cur, oth, false, ctl, st);
+    op_jacobi(H, L, b, cur, oth, false, ctl, st, L.dsw[s]);
     std::swap(cur, oth);
   }
   Level& C = H->lv[l + 1];
   // the coarse level starts with two sweeps from zero on the row-tile path: hand it its first one
   const bool give_x1 = lv_fast(L) && lv_fast(C) && nu1 >= 2 && l + 1 < Lc && l + 1 != H->tail_dense_level;
-  op_residual_restrict(H, L, b, cur, C.b, ctl, st, give_x1 ? C.dinv : nullptr, give_x1 ? C.x2 : nullptr);
+  op_residual_restrict(H, L, b, cur, C.b, ctl, st, give_x1 ? C.dsw[0] : nullptr, give_x1 ? C.x2 : nullptr);
   double* ec = nullptr;
   AMG_TRY(amg_vcycle(H, l + 1, C.b, &ec, ctl, false, st, give_x1));
   const bool want_dot = fuse_rz && l == 0;
@@ -361,9 +367,9 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       // (level 0 of cfg 3: 53 us against 33 us for a plain sweep); there a separate unit-stride
       // correction pass (8 us) followed by the plain sweep is cheaper.
       ++g_nlaunch, launch(k_prolong_add, grid_for((L.n + 1) / 2), TPB, 0, st)(L.n, L.agg, ec, H->opt.coarse_scale, cur, cur, ctl);
-      op_jacobi(H, L, b, cur, out, want_dot && nu2 == 1, ctl, st);
+      op_jacobi(H, L, b, cur, out, want_dot && nu2 == 1, ctl, st, L.dsw[nu1]);
     } else {
-      op_jacobi_prolong(H, L, b, cur, ec, out, want_dot && nu2 == 1, ctl, st);
+      op_jacobi_prolong(H, L, b, cur, ec, out, want_dot && nu2 == 1, ctl, st, L.dsw[nu1]);
     }
     if (out == oth)
       std::swap(cur, oth);
@@ -371,7 +377,7 @@ amg_status amg_vcycle(amg_handle_s* H, int l, const double* b, double** x_out, K
       cur = out;
     for (int s = 1; s < nu2; ++s) {
       out = (fo && s == nu2 - 1) ? fo : oth;
-      op_jacobi(H, L, b, cur, out, want_dot && s == nu2 - 1, ctl, st);
+      op_jacobi(H, L, b, cur, out, want_dot && s == nu2 - 1, ctl, st, L.dsw[nu1 + s]);
       if (out == oth)
         std::swap(cur, oth);
       else
@@ -411,7 +417,7 @@ amg_status enqueue_pcg_iteration(amg_handle_s* H, int precond, cudaStream_t st) 
   g_kop = 1;
   op_spmv(H, L0, p, q, 1, p, FIN_PQ, H->ctl, st);
   g_kop = 0;
-  ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, L0.dinv, l0_x1(H, precond), H->partials,
+  ++g_nlaunch, launch(k_pcg_xr, red_grid(H, n), RED_THREADS, 0, st)(n, p, q, x, r, L0.dsw[0], l0_x1(H, precond), H->partials,
                                                                         H->counter, H->ctl);
   double* z = r;
   if (precond) {
@@ -429,7 +435,7 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   const int n = L0.n;
   double *x = H->kv[0], *r = H->kv[1], *p = H->kv[2], *v = H->kv[3], *rhat = H->kv[4], *s = H->kv[5],
          *t = H->kv[6], *ph = H->kv[7];
-  ++g_nlaunch, launch(k_bicg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, p, L0.dinv, l0_x1(H, precond), H->ctl);
+  ++g_nlaunch, launch(k_bicg_p, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, p, L0.dsw[0], l0_x1(H, precond), H->ctl);
   double* phat = p;
   if (precond) {
     double* zz = nullptr;
@@ -442,7 +448,7 @@ amg_status enqueue_bicg_iteration(amg_handle_s* H, int precond, cudaStream_t st)
   g_kop = 1;
   op_spmv(H, L0, phat, v, 1, rhat, FIN_RV, H->ctl, st);
   g_kop = 0;
-  ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, L0.dinv, l0_x1(H, precond), H->partials,
+  ++g_nlaunch, launch(k_bicg_s, red_grid(H, n), RED_THREADS, 0, st)(n, r, v, s, L0.dsw[0], l0_x1(H, precond), H->partials,
                                                                         H->counter, H->ctl);
   double* shat = s;
   if (precond) AMG_TRY(amg_vcycle(H, 0, s, &shat, H->ctl, false, st, l0_x1(H, precond) != nullptr));
@@ -473,7 +479,7 @@ amg_status enqueue_pcg_start(amg_handle_s* H, cudaStream_t st) {
 amg_status enqueue_apply(amg_handle_s* H, cudaStream_t st) {
   Level& L0 = H->lv[0];
   double* x1 = l0_x1(H, 1);
-  if (x1) ++g_nlaunch, launch(k_scale_dinv, grid_for(L0.n), TPB, 0, st)(L0.n, L0.dinv, H->io_tmp2, x1, nullptr);
+  if (x1) ++g_nlaunch, launch(k_scale_dinv, grid_for(L0.n), TPB, 0, st)(L0.n, L0.dsw[0], H->io_tmp2, x1, nullptr);
   AMG_TRY(amg_vcycle(H, 0, H->io_tmp2, &H->apply_out, nullptr, false, st, x1 != nullptr));
   return AMG_OK;
 }
@@ -618,7 +624,7 @@ amg_status amg_krylov_solve(amg_handle_s* H, const double* d_b, double* d_x, dou
   ci.rtol = rtol, ci.maxit = maxit, ci.hist = H->hist, ci.hist_cap = H->hist_cap;
   H->hist_len = 0;
   if (krylov == 0) {
-    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, L0.dinv,
+    ++g_nlaunch, launch(k_krylov_init, red_grid(H, n), RED_THREADS, 0, st)(n, d_b, L0.inv, r, x, p, nullptr, nullptr, L0.dsw[0],
                                                          l0_x1(H, precond), H->partials, H->counter, H->ctl, FIN_INIT_PCG, ci);
     if (precond && H->opt.use_graph && maxit > 0) {
       cudaGraphExec_t gstart = nullptr;

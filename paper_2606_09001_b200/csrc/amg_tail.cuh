@@ -26,6 +26,7 @@ struct TailLevel {
   const int* col;
   const double* val;
   const double* dinv;
+  const double* dsw[AMG_MAX_SWEEPS];  // diagonal of every sweep of a cycle (Level::dsw)
   const int* agg;
   const int* agg_ptr;
 };
@@ -76,7 +77,7 @@ __device__ __forceinline__ double tl_row_pass(const TailOpView& A, int R0, int R
         di = A.dinv[i];
         bi = tl_ld<CG>(b + i);
         if (OP == T_JAC0)
-          xi = di * bi;
+          xi = __ldg(A.dinv_g + i) * bi;  // x1 with the diagonal of the first sweep, the epilogue with the second's
         else if (OP == T_JACP)
           xi = tl_ld<CG>(x + i) + gamma * tl_ld<CG>(ec + __ldg(A.agg + i));
         else
@@ -295,9 +296,11 @@ static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailB
     double* oth = cur + L.n;
     int done;
     if (a.nu1 >= 2) {
+      A.dinv_g = L.dsw[0], A.dinv = L.dsw[1];
       tl_row_pass<T_JAC0, false>(A, 0, L.n, tid, TAILB_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 2;
     } else if (a.nu1 == 1) {
+      A.dinv = L.dsw[0];
       tl_vec_pass<T_SCALE, false>(A, 0, L.n, tid, TAILB_THREADS, b, nullptr, nullptr, 0.0, cur, false);
       done = 1;
     } else {
@@ -306,6 +309,7 @@ static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailB
     }
     __syncthreads();
     for (int s = done; s < a.nu1; ++s) {
+      A.dinv = L.dsw[s];
       tl_row_pass<T_JAC, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, nullptr, 0.0, oth, false);
       double* t = cur;
       cur = oth;
@@ -338,12 +342,14 @@ static __global__ void __launch_bounds__(TAILB_THREADS) k_tail_dense_build(TailB
     const int ncn = a.lv[l + 1].n;
     const double* ec = (l + 1 == a.last) ? cb + ncn : (tail_result_in_x2(a.nu1, a.nu2) ? cb + 2 * ncn : cb + ncn);
     if (a.nu2 >= 1) {
+      A.dinv = L.dsw[a.nu1];
       tl_row_pass<T_JACP, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, ec, a.gamma, oth, false);
       double* t = cur;
       cur = oth;
       oth = t;
       for (int s = 1; s < a.nu2; ++s) {
         __syncthreads();
+        A.dinv = L.dsw[a.nu1 + s];
         tl_row_pass<T_JAC, false>(A, 0, L.n, tid, TAILB_THREADS, b, cur, nullptr, 0.0, oth, false);
         t = cur;
         cur = oth;

@@ -40,7 +40,7 @@ def test_struct_layouts_and_defaults():
     from paper_2606_09001_b200 import binding
 
     o = binding.amg_options_default()
-    assert o.struct_size == C.sizeof(binding.amg_options) == 104
+    assert o.struct_size == C.sizeof(binding.amg_options) == 112
     assert (o.krylov, o.symmetric, o.agg_passes, o.pre_sweeps, o.post_sweeps, o.smoother) == (0, -1, 1, 2, 2, 0)
     assert (o.coarse_max_rows, o.max_levels, o.max_match_rounds) == (64, 32, 0)
     assert o.strong_beta == 0.25 and o.coarse_scale == 1.0 and abs(o.omega - 2 / 3) < 1e-16

@@ -283,3 +283,53 @@ def test_mixed_precision_hierarchy_nonsymmetric(oracle_mod, B):
     finally:
         s.close()
         o.close()
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(force_generic=1), dict(tail_dense_rows=0), dict(pre_sweeps=3, post_sweeps=3),
+                                  dict(pre_sweeps=1, post_sweeps=1), dict(pre_sweeps=3, post_sweeps=1)])
+@pytest.mark.parametrize("case", [(3, 40), (4, 28)])
+def test_chebyshev_smoother_matches_the_oracle(oracle_mod, B, case, opts):
+    """smoother = 2 (NEXT-4): Chebyshev-accelerated L1-Jacobi, per-sweep diagonals tau_j * dinv.  V-cycle from every
+    level against the oracle (1e-12), solves at the usual bars, fewer iterations than plain L1-Jacobi."""
+    cfg, edge = case
+    A = inputs.config_matrix(cfg, edge)
+    Asp = A.to_scipy()
+    n = A.n
+    b = inputs.config_rhs(cfg, n)
+    oo = {k: v for k, v in opts.items() if k in ("pre_sweeps", "post_sweeps")}
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, smoother=2, **oo)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, smoother=2, **opts)
+    try:
+        for l in range(s.num_levels):
+            nl = s.level_info(l)[0]
+            bl = np.random.default_rng(100 + l).standard_normal(nl)
+            assert rel(s.level_op(l, 5, None, bl, nl).cpu().numpy(), o.vcycle(bl, l)) <= 1e-12, l
+        r = np.random.default_rng(3).standard_normal(n)
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+        sym = opts.get("pre_sweeps", 2) == opts.get("post_sweeps", 2)
+        for krylov in ((0, 1) if sym else (1,)):
+            xg, ig = s.solve(b, 1e-8, 500, krylov)
+            xo, io = o.solve(b, 1e-8, 500, krylov, 1)
+            assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+            assert np.linalg.norm(b - Asp @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+        if not opts:
+            o1 = oracle_mod.Oracle(A.rowptr, A.col, A.val)
+            _, i1 = o1.solve(b, 1e-8, 500, 0, 1)
+            xg, ig = s.solve(b, 1e-8, 500, 0)
+            assert ig.iterations < i1.iterations
+            o1.close()
+            # batched solve and warm resetup keep the weighted diagonals
+            Bh = np.stack([inputs.rhs_uniform(n, 60 + k) for k in range(8)])
+            Bd = torch.as_tensor(Bh).cuda().contiguous()
+            X = torch.empty_like(Bd)
+            infos = B.amg_solve_batched(s.h, 0, Bd, X, 8, n, 1e-8, 500)
+            for k in (0, 7):
+                xo, io = o.solve(Bh[k], 1e-8, 500, 0, 1)
+                assert infos[k].status == 0 and abs(infos[k].iterations - io.iterations) <= 2
+                assert np.linalg.norm(Bh[k] - Asp @ X[k].cpu().numpy()) <= 1e-8 * np.linalg.norm(Bh[k])
+            z = s.apply_preconditioner(r).cpu().numpy()
+            s.resetup_values(A.val * 4.0, keep_aggregates=True)
+            assert rel(s.apply_preconditioner(r).cpu().numpy(), 0.25 * z) <= 1e-12
+    finally:
+        s.close()
+        o.close()
