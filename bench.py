@@ -46,6 +46,14 @@ WORKLOADS = {
     4: "cfg4: 3D 7-point variable-coefficient diffusion 192^3, randomly permuted rows, b~U[-1,1]",
     5: "cfg5: differentiable solve on the cfg4 system, 16 right-hand sides forward + 16 adjoint + gradient",
 }
+# Solver options of the headline run and of configs 2, 4, 5, ns -- all within north_star's description ("pairwise or
+# size-4 aggregation", "L1-Jacobi or damped-Jacobi smoother"), each an option of BOTH the library and the oracle with its
+# own pins and parity tests, everything in fp64: size-4 aggregation (two pairwise passes), Chebyshev-weighted L1-Jacobi
+# sweeps, over-correction gamma = 1.6.  The library defaults (pairwise, plain L1-Jacobi, gamma = 1: BASELINE.json
+# configs[0]) are timed beside it ("phases.default_options") and used for cfg 1, whose text fixes them.
+TUNED = dict(smoother=2, agg_passes=2, coarse_scale=1.6)
+TUNED_TEXT = "V(2,2) Chebyshev-weighted L1-Jacobi (ratio 6), size-4 aggregation, gamma 1.6"
+
 # NEXT-2: nonsymmetric pressure-Poisson-like system, the size of the paper's channel grid
 NONSYM_SHAPE = (100, 260, 256)
 # ncu capture of the roofline rep loop (profiles/r02_roofline.md names the command that wrote it)
@@ -74,7 +82,7 @@ def parse_args():
 def config_dict(cfg, edge, n, nnz):
     """The workload description, identical for both arms of the bench."""
     return {"workload": WORKLOADS.get(cfg, str(cfg)) + (f" [edge {edge}]" if edge else ""), "n": n, "nnz": nnz,
-            "rtol": RTOL, "krylov": "PCG", "cycle": "V(2,2) L1-Jacobi"}
+            "rtol": RTOL, "krylov": "PCG", "cycle": TUNED_TEXT}
 
 
 def roofline_traffic():
@@ -197,7 +205,7 @@ def oracle_run(A, b, threads, maxit=MAXIT):
     oracle.build()
     oracle.set_threads(threads)
     t = time.perf_counter()
-    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    o = oracle.Oracle(A.rowptr, A.col, A.val, **TUNED)
     t_setup = time.perf_counter() - t
     t = time.perf_counter()
     _, info = o.solve(b, RTOL, maxit, 0, 1)
@@ -271,7 +279,7 @@ def extra_configs(which, B, inputs, dev, peak):
         A = inputs.config_matrix(2)
         Asp = A.to_scipy()
         Bh = np.stack([Asp @ inputs.config_rhs(2, A.n, k) for k in range(8)])
-        s, first, sms = setup(A)
+        s, first, sms = setup(A, **TUNED)
         Bd = torch.as_tensor(Bh).to(dev).contiguous()
         X = torch.empty_like(Bd)
         ms, infos = timed(lambda: B.amg_solve_batched(s.h, 0, Bd, X, 8, A.n, RTOL, MAXIT))
@@ -290,7 +298,7 @@ def extra_configs(which, B, inputs, dev, peak):
         A = inputs.config_matrix(4)
         Asp = A.to_scipy()
         n, nnz = A.n, A.nnz
-        s, first, sms = setup(A)
+        s, first, sms = setup(A, **TUNED)
         if "4" in which:
             b = inputs.config_rhs(4, n)
             db, dx = torch.as_tensor(b).to(dev), torch.empty(n, dtype=torch.float64, device=dev)
@@ -307,22 +315,23 @@ def extra_configs(which, B, inputs, dev, peak):
                     t.append((time.perf_counter() - t0) * 1e3)
                 rs.append(round(min(t), 2))
             B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1)
-            # the same system with the NEXT-4 options on (Chebyshev-weighted L1-Jacobi, size-4 aggregation, fp32 level
-            # operators inside the V-cycle; Krylov and residual in fp64)
-            st_ = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, smoother=2, agg_passes=2, hierarchy_fp32=1)
-            dxt = torch.empty_like(db)
-            tms, tinfo = timed(lambda: B.amg_solve_ex(st_.h, db, dxt, RTOL, MAXIT, 0, 1))
-            tuned = {"options": "smoother=2, agg_passes=2, hierarchy_fp32=1", "solve_ms": round(tms, 3),
-                     "iterations": tinfo.iterations, "levels": st_.num_levels,
-                     "true_rel_residual_host_fp64": hres(Asp, b, dxt.cpu().numpy())}
-            st_.close()
-            del dxt
+            # the same system with the library defaults (pairwise, plain L1-Jacobi, gamma 1: the round-1 configuration,
+            # 73 iterations = the stored oracle count), and with the fp32 level operators on top of the tuned options
+            other = {}
+            for key, opts in (("default_options", dict()), ("tuned_mixed_precision", dict(hierarchy_fp32=1, **TUNED))):
+                st_ = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **opts)
+                dxt = torch.empty_like(db)
+                tms, tinfo = timed(lambda: B.amg_solve_ex(st_.h, db, dxt, RTOL, MAXIT, 0, 1))
+                other[key] = {"solve_ms": round(tms, 3), "iterations": tinfo.iterations, "levels": st_.num_levels,
+                              "true_rel_residual_host_fp64": hres(Asp, b, dxt.cpu().numpy())}
+                st_.close()
+                del dxt
             out["cfg4"] = {"workload": WORKLOADS[4], "n": n, "nnz": nnz, "levels": s.num_levels, "setup_ms": sms,
                            "setup_first_call_ms": first, "resetup_keep_aggregates_ms": rs[0], "resetup_full_ms": rs[1],
                            "solve_ms": round(ms, 3), "iterations": info.iterations,
                            "true_rel_residual_host_fp64": hres(Asp, b, dx.cpu().numpy()),
                            "solve_phase": solve_phase(s, ms, info.iterations),
-                           "tuned": tuned, "vcycle_ms": round(vms / 10, 4),
+                           **other, "vcycle_ms": round(vms / 10, 4),
                            "vcycle_frac": round(B.amg_get_algorithmic_bytes(s.h, 1) / (vms / 10 * 1e-3) / 1e9 / peak, 4)}
         if "5" in which:
             R = 16
@@ -354,7 +363,7 @@ def extra_configs(which, B, inputs, dev, peak):
         A = inputs.stretched_channel_csr(NONSYM_SHAPE, 2.0)
         Asp = A.to_scipy()
         n = A.n
-        s, first, sms = setup(A)
+        s, first, sms = setup(A, **TUNED)
         b = inputs.rhs_uniform(n, 6001)
         g = inputs.rhs_uniform(n, 6002)
         db, dg = torch.as_tensor(b).to(dev), torch.as_tensor(g).to(dev)
@@ -411,7 +420,7 @@ def run_b200(args):
     B.load_library()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **TUNED)
     torch.cuda.synchronize()
     setup_first_ms = (time.perf_counter() - t0) * 1e3  # includes the H2D copy of the CSR arrays and context warm-up
     h = s.h
@@ -589,10 +598,9 @@ def run_b200(args):
                                         "reorder": round(st.reorder_ms, 2), "lu": round(st.lu_ms, 2)}
         # NEXT-4 variants on the same system: mixed-precision hierarchy (fp32 level operators inside the V-cycle, fp64
         # Krylov; default off) and size-4 aggregation
-        for key, opts in (("mixed_precision", dict(hierarchy_fp32=1)), ("size4_aggregation", dict(agg_passes=2)),
-                          ("size4_mixed_precision", dict(agg_passes=2, hierarchy_fp32=1)),
-                          ("chebyshev_smoother", dict(smoother=2)),
-                          ("chebyshev_size4_mixed_precision", dict(smoother=2, agg_passes=2, hierarchy_fp32=1))):
+        for key, opts in (("default_options", dict()), ("default_mixed_precision", dict(hierarchy_fp32=1)),
+                          ("size4_aggregation_only", dict(agg_passes=2)), ("chebyshev_smoother_only", dict(smoother=2)),
+                          ("tuned_mixed_precision", dict(hierarchy_fp32=1, **TUNED))):
             sv = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **opts)
             dxv = torch.empty_like(d_b)
             for _ in range(2):
@@ -643,10 +651,9 @@ def run_b200(args):
             "solve_phase": {"algorithmic_bytes": solve_bytes, "achieved_gbs": round(solve_gbs, 1), "peak": peak,
                             "frac": round(solve_gbs / peak, 4), "frac_of_8000_nominal": round(solve_gbs / 8000.0, 4),
                             "bytes_per_iteration": bytes_pcg_it, "peak_source": peak_src},
-            "tuned": ({"options": "smoother=2 (Chebyshev-weighted L1-Jacobi), agg_passes=2 (size-4 aggregates), "
-                                  "hierarchy_fp32=1 (fp32 level operators inside the V-cycle; Krylov, residual, vectors fp64); "
-                                  "all default off, each with its oracle option and parity tests",
-                       **phases["chebyshev_size4_mixed_precision"]} if "chebyshev_size4_mixed_precision" in phases else None),
+            "solver_options": {**TUNED, "cheby_ratio": 6.0, "pre_sweeps": 2, "post_sweeps": 2, "hierarchy_fp32": 0,
+                               "note": "every option exists in the library AND in the oracle (pinned, parity-tested); the "
+                                       "library defaults (pairwise, plain L1-Jacobi, gamma 1) are timed under phases.default_options"},
             "vcycle": vc, "phases": phases, "configs": configs, "cpu_baseline": cpu, "clocks": clocks,
         }
         print(json.dumps(out), flush=True)
@@ -670,7 +677,7 @@ def run_reference(args):
     oracle.build()
     oracle.set_threads(cores)
     t = time.perf_counter()
-    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    o = oracle.Oracle(A.rowptr, A.col, A.val, **TUNED)
     setup_s = time.perf_counter() - t
     t = time.perf_counter()
     _, full = o.solve(b, RTOL, MAXIT, 0, 1)

@@ -333,3 +333,40 @@ def test_chebyshev_smoother_matches_the_oracle(oracle_mod, B, case, opts):
     finally:
         s.close()
         o.close()
+
+
+def test_full_size_headline_options_against_the_oracle(oracle_mod, B):
+    """The options bench.py runs the headline with (cfg 3, 128^3: size-4 aggregation, Chebyshev-weighted L1-Jacobi,
+    gamma = 1.6, all fp64), on the GPU against the oracle with the same options at full size: identical hierarchy
+    (integers), iterations +-2, host fp64 residual, x against the oracle's converged solution."""
+    import os
+
+    opts = dict(smoother=2, agg_passes=2, coarse_scale=1.6)
+    A = inputs.config_matrix(3)
+    b = inputs.config_rhs(3, A.n)
+    oracle_mod.set_threads(os.cpu_count() or 1)
+    try:
+        o = oracle_mod.Oracle(A.rowptr, A.col, A.val, **opts)
+        s = B.AmgSolver(A.rowptr, A.col, A.val, **opts)
+        assert s.num_levels == o.num_levels
+        for l in range(s.num_levels):
+            assert s.level_info(l) == o.level_info(l)
+            if l < s.num_levels - 1:
+                assert np.array_equal(s.aggregates(l).cpu().numpy(), o.aggregates(l)), l
+        xg, ig = s.solve(b, 1e-8, 500, 0)
+        xo, io = o.solve(b, 1e-8, 500, 0, 1)
+        assert ig.status == io.status == 0 and abs(ig.iterations - io.iterations) <= 2
+        assert ig.iterations < 30  # (the library defaults need 42)
+        assert np.linalg.norm(b - A.to_scipy() @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
+        xg, _ = s.solve(b, 1e-11, 500, 0)
+        xo, _ = o.solve(b, 1e-13, 500, 0, 1)
+        assert rel(xg.cpu().numpy(), xo) <= 1e-6
+        r = np.random.default_rng(1).standard_normal(A.n)
+        assert rel(s.apply_preconditioner(r).cpu().numpy(), o.vcycle(r, 0)) <= 1e-12
+        u, v = np.random.default_rng(2).standard_normal((2, A.n))
+        Bu, Bv = s.apply_preconditioner(u).cpu().numpy(), s.apply_preconditioner(v).cpu().numpy()
+        assert abs(Bu @ v - u @ Bv) <= 1e-12 * np.linalg.norm(Bu) * np.linalg.norm(v) and Bu @ u > 0  # B stays SPD
+        s.close()
+        o.close()
+    finally:
+        oracle_mod.set_threads(1)
