@@ -72,6 +72,9 @@ def parse_args():
                     help="other configurations measured beside the headline one (rank 0, N = 1); 'none' skips them")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-phases", action="store_true", help="skip the setup / BiCGSTAB / adjoint extras")
+    ap.add_argument("--host-loop", action="store_true",
+                    help="use_while = 0: the iteration graph replayed under host control (its kernel nodes can be listed by "
+                         "ncu; kernel nodes under a conditional WHILE node cannot)")
     ap.add_argument("--setup-only", action="store_true",
                     help="one warm-up amg_setup, then one more between cudaProfilerStart/Stop (ncu --profile-from-start off)")
     ap.add_argument("--roofline-only", action="store_true",
@@ -420,7 +423,7 @@ def run_b200(args):
     B.load_library()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, **TUNED)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, device=dev, use_while=0 if args.host_loop else 1, **TUNED)
     torch.cuda.synchronize()
     setup_first_ms = (time.perf_counter() - t0) * 1e3  # includes the H2D copy of the CSR arrays and context warm-up
     h = s.h
