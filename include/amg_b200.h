@@ -225,6 +225,11 @@ AMG_API amg_status amg_get_aggregates(amg_handle h, int32_t level, int32_t* d_ag
  * half-step exit, else ||r||).  *count = number of entries; at most `cap` are copied to the HOST array h_out. */
 AMG_API amg_status amg_get_residual_history(amg_handle h, double* h_out, int32_t cap, int32_t* count,
                                             void* cuda_stream);
+/* Diagnostics file ("optional file-based output provides detailed AMG hierarchy statistics and
+ * per-iteration residual histories"): writes a plain-text report to `path` (HOST string) -- per level rows, nonzeros,
+ * entries per row, aggregation rounds, kernel path, tiles; grid / operator complexity; the options in force; the
+ * setup timings; the residual history of the last reporting solve.  Synchronises `cuda_stream`. */
+AMG_API amg_status amg_write_report(amg_handle h, const char* path, void* cuda_stream);
 /* 1 / 0: what the setup decided (the caller's flag, or the result of the device check for -1). */
 AMG_API amg_status amg_get_symmetric(amg_handle h, int32_t* symmetric);
 AMG_API amg_status amg_get_level_csr(amg_handle h, int32_t level, int32_t* d_rowptr, int32_t* d_col,

@@ -25,7 +25,7 @@ EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_w
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
            "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
-           "amg_get_level_path", "amg_get_symmetric", "amg_get_residual_history", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error",
+           "amg_get_level_path", "amg_get_symmetric", "amg_get_residual_history", "amg_write_report", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error",
            "amg_cache_create", "amg_cache_get", "amg_cache_stats", "amg_cache_destroy"]
 
 
@@ -223,6 +223,10 @@ def amg_get_residual_history(h):
         _check(load_library().amg_get_residual_history(h, C.c_void_p(out.ctypes.data), C.c_int32(cnt.value),
                                                        C.byref(cnt), _stream()), h)
     return out
+
+
+def amg_write_report(h, path):
+    _check(load_library().amg_write_report(h, C.c_char_p(str(path).encode()), _stream()), h)
 
 
 def amg_get_symmetric(h) -> int:

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <vector>
 
 #include "amg_internal.cuh"
 
@@ -457,6 +458,47 @@ amg_status amg_get_residual_history(amg_handle h, double* h_out, int32_t cap, in
     AMG_CUDA_TRY(h, cudaMemcpyAsync(h_out, h->hist, sizeof(double) * (size_t)m, cudaMemcpyDeviceToHost, st));
     AMG_CUDA_TRY(h, cudaStreamSynchronize(st));
   }
+  return AMG_OK;
+}
+
+amg_status amg_write_report(amg_handle h, const char* path, void* cuda_stream) {
+  if (!h || !path) return AMG_ERR_INVALID_ARG;
+  Enter e(h, cuda_stream);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  std::vector<double> hist((size_t)(h->hist_len > 0 ? h->hist_len : 0));
+  if (!hist.empty())
+    AMG_CUDA_TRY(h, cudaMemcpyAsync(hist.data(), h->hist, sizeof(double) * hist.size(), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(h, cudaStreamSynchronize(st));
+  FILE* f = fopen(path, "w");
+  if (!f) {
+    h->err = std::string("amg_write_report: cannot open ") + path;
+    return AMG_ERR_INVALID_ARG;
+  }
+  const amg_options& o = h->opt;
+  fprintf(f, "amg_b200 hierarchy report\n");
+  fprintf(f, "rows %lld  nonzeros %lld  symmetric %d  levels %d\n", (long long)h->n, (long long)h->nnz, h->symmetric,
+          (int)h->lv.size());
+  fprintf(f, "options: krylov %d  agg_passes %d  sweeps %d+%d  smoother %d (omega %.6g, cheby_ratio %.6g)  strong_beta %.6g  "
+             "coarse_scale %.6g  coarse_max_rows %d  hierarchy_fp32 %d  tail_dense_rows %d  use_graph %d  use_pdl %d  use_while %d\n",
+          o.krylov, o.agg_passes, o.pre_sweeps, o.post_sweeps, o.smoother, o.omega, o.cheby_ratio, o.strong_beta,
+          o.coarse_scale, o.coarse_max_rows, o.hierarchy_fp32, o.tail_dense_rows, o.use_graph, o.use_pdl, o.use_while);
+  double sn = 0.0, sz = 0.0;
+  fprintf(f, "%5s %12s %14s %9s %7s %6s %8s %12s\n", "level", "rows", "nonzeros", "nnz/row", "rounds", "tiles", "kernels",
+          "blob MB");
+  for (size_t l = 0; l < h->lv.size(); ++l) {
+    const Level& L = h->lv[l];
+    sn += L.n, sz += L.nnz;
+    fprintf(f, "%5d %12d %14d %9.2f %7d %6d %8s %12.2f\n", (int)l, L.n, L.nnz, L.n ? (double)L.nnz / L.n : 0.0,
+            L.match_rounds, L.nblk, L.fast ? "row-tile" : "row-vec", L.blob_bytes / 1e6);
+  }
+  fprintf(f, "grid complexity %.4f  operator complexity %.4f  coarsest dense LU %d x %d  dense tail from level %d\n",
+          h->n ? sn / (double)h->n : 0.0, h->nnz ? sz / (double)h->nnz : 0.0, h->nL, h->nL, h->tail_dense_level);
+  fprintf(f, "setup ms: total %.3f  aggregation %.3f  galerkin %.3f  renumbering+packing %.3f  lu %.3f  (max rounds %d)\n",
+          h->stats.total_ms, h->stats.aggregate_ms, h->stats.galerkin_ms, h->stats.reorder_ms, h->stats.lu_ms,
+          h->stats.match_rounds_max);
+  fprintf(f, "residual history of the last reporting solve (%d iterations): ||r_k|| / ||b||\n", (int)hist.size());
+  for (size_t k = 0; k < hist.size(); ++k) fprintf(f, "%5d %.17g\n", (int)k + 1, hist[k]);
+  fclose(f);
   return AMG_OK;
 }
 

@@ -370,3 +370,23 @@ def test_full_size_headline_options_against_the_oracle(oracle_mod, B):
         o.close()
     finally:
         oracle_mod.set_threads(1)
+
+
+def test_report_file(B, tmp_path):
+    """optional file-based output with the hierarchy statistics and the residual history."""
+    A = inputs.config_matrix(3, 24)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    try:
+        x, info = s.solve(inputs.config_rhs(3, A.n), 1e-8, 200)
+        p = tmp_path / "amg_report.txt"
+        B.amg_write_report(s.h, p)
+        txt = p.read_text().splitlines()
+        assert txt[0].startswith("amg_b200 hierarchy report") and f"levels {s.num_levels}" in txt[1]
+        rows = [l.split() for l in txt if l.split() and l.split()[0].isdigit() and len(l.split()) == 8]
+        assert [(int(r[1]), int(r[2])) for r in rows] == [s.level_info(l) for l in range(s.num_levels)]
+        hist = [float(l.split()[1]) for l in txt[txt.index(next(t for t in txt if t.startswith("residual history"))) + 1:]]
+        assert len(hist) == info.iterations and np.array_equal(np.array(hist), s.residual_history())
+        oc = float(next(t for t in txt if t.startswith("grid complexity")).split()[5])
+        assert abs(oc - sum(s.level_info(l)[1] for l in range(s.num_levels)) / A.nnz) < 1e-3
+    finally:
+        s.close()
