@@ -1,7 +1,7 @@
 """bench.py — AMG-PCG solve time + V-cycle HBM GB/s on the 3D 128^3 fp64 Poisson system (one B200).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--cfg 3] [--edge E]
-                    [--configs 1,2,4,5,ns | none] [--roofline-only]
+                    [--configs 1,2,4,5,ns,tri | none] [--roofline-only]
 
 A "step" is one pass of the solve-phase hot path on the cached hierarchy: one AMG-PCG solve of
 A x = b from x0 = 0 to ||r|| <= 1e-8 ||b|| (BASELINE.json configs[2], the
@@ -68,7 +68,7 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--edge", type=int, default=None, help="grid edge (default: the config's full size)")
-    ap.add_argument("--configs", default="1,2,4,5,ns",
+    ap.add_argument("--configs", default="1,2,4,5,ns,tri",
                     help="other configurations measured beside the headline one (rank 0, N = 1); 'none' skips them")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-phases", action="store_true", help="skip the setup / BiCGSTAB / adjoint extras")
@@ -385,6 +385,27 @@ def extra_configs(which, B, inputs, dev, peak):
             "forward_solve_phase": solve_phase(s, fms, fi.iterations, 1),
             "adjoint_solve_phase": solve_phase(s, ams, ai.iterations, 1),
             "paper_context": "PAPER.md:303 Table 3: 3.88 s per solve (JAX-AMG/AmgX, 1x RTX A6000, 6.66 M unknowns, tol 1e-5)"}
+        s.close()
+    if "tri" in which:
+        # the paper's Fig. 2 workload: a well-conditioned tridiagonal system with n = 1e7, solved
+        # WITHOUT a preconditioner by CG and BiCGSTAB (the paper prints no numbers, only a bar chart on an L40)
+        n = 10_000_000
+        A = inputs.tridiagonal_csr(n, 4.0, -1.0)
+        b = inputs.rhs_ones(n)
+        s, first, sms = setup(A)
+        db, dx = torch.as_tensor(b).to(dev), torch.empty(n, dtype=torch.float64, device=dev)
+        res = {}
+        for name, krylov in (("cg", 0), ("bicgstab", 1)):
+            ms, info = timed(lambda: B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, krylov, 0))
+            it_bytes = B.amg_get_algorithmic_bytes(s.h, 0) * (1 if krylov == 0 else 2) + (11 if krylov == 0 else 17) * 8.0 * n
+            res[name] = {"solve_ms": round(ms, 3), "iterations": info.iterations,
+                         "true_rel_residual_host_fp64": hres(A.to_scipy(), b, dx.cpu().numpy()),
+                         "frac": round(it_bytes * info.iterations / (ms * 1e-3) / 1e9 / peak, 4)}
+        ms, info = timed(lambda: B.amg_solve_ex(s.h, db, dx, RTOL, MAXIT, 0, 1))
+        out["tridiagonal"] = {"workload": "PAPER.md Fig. 2: tridiag(-1, 4, -1), n = 1e7, b = ones; unpreconditioned CG / BiCGSTAB "
+                                          "(amg_solve_ex precond = 0) to rtol 1e-8, library defaults",
+                              "n": n, "nnz": A.nnz, "unpreconditioned": res, "setup_ms": sms,
+                              "amg_pcg": {"solve_ms": round(ms, 3), "iterations": info.iterations}}
         s.close()
     return out
 
