@@ -1,7 +1,10 @@
 """Writes tests/golden/full_size_*.txt: what the CPU oracle (and only the oracle) computes on the
 full-size BASELINE.json configurations that are too slow to re-run inside the GPU test suite.
 
-    python tests/golden/make_full_size_golden.py [cfg4] [cfg5] [cfg2]     (about 90 minutes on 8 cores)
+    python tests/golden/make_full_size_golden.py [cfg4] [cfg5] [cfg2] [tuned]    (about 90 minutes on 8 cores)
+
+"tuned" writes the same files with the suffix _tuned for the solver options bench.py runs these configurations with
+(size-4 aggregation, Chebyshev-weighted L1-Jacobi, gamma = 1.6; oracle options of the same names).
 
 Every solve runs ONCE to rtol 1e-13 ("converged", reading A12); the iteration count at the timed
 tolerance 1e-8 is read off the oracle's residual history (the iterates do not depend on rtol).
@@ -35,6 +38,8 @@ NS, NS2 = 10000, 4096
 SEED_ROWS, SEED_ENTRIES = 9001, 9002
 CFG5_COLUMNS = (0, 7, 15)
 RTOL_TIMED, RTOL_CONVERGED, MAXIT = 1e-8, 1e-13, 600
+OPTS, SUFFIX = {}, ""   # "tuned": the options of bench.py
+TUNED = dict(smoother=2, agg_passes=2, coarse_scale=1.6)
 
 
 def sample_rows(n, count=NS):
@@ -73,7 +78,7 @@ def write(name, lines):
 def cfg4_and_5(do4, do5):
     A = inputs.config_matrix(4, 192)
     t = time.time()
-    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    o = oracle.Oracle(A.rowptr, A.col, A.val, **OPTS)
     ts = time.time() - t
     rows_s, ent_s = sample_rows(A.n), sample_entries(A.nnz)
     row_of = np.searchsorted(A.rowptr, ent_s, side="right") - 1
@@ -81,7 +86,8 @@ def cfg4_and_5(do4, do5):
         b = inputs.config_rhs(4, A.n)
         x, info, k8, r8, tv = converged_solve(o, b)
         shapes = [o.level_info(l) for l in range(o.num_levels)]
-        out = ["# written by tests/golden/make_full_size_golden.py (CPU oracle only); cfg 4 = BASELINE.json configs[3]",
+        out = ["# written by tests/golden/make_full_size_golden.py (CPU oracle only); cfg 4 = BASELINE.json configs[3]" +
+               (f"; oracle options {OPTS}" if OPTS else ""),
                f"# oracle setup {ts:.0f} s, solve to 1e-13 {tv:.0f} s ({info.iterations} iterations) on {os.cpu_count()} cores",
                f"cfg4_192 iterations {k8}", f"cfg4_192 rel_residual {r8:.17g}", f"cfg4_192 levels {o.num_levels}",
                "cfg4_192 rows " + " ".join(str(r) for r, _ in shapes),
@@ -89,7 +95,7 @@ def cfg4_and_5(do4, do5):
                f"cfg4_192 converged_iterations {info.iterations}", f"cfg4_192 converged_status {info.status}",
                f"cfg4_192 sample_rows_seed {SEED_ROWS} {NS}",
                "cfg4_192 x_converged " + fmt(x[rows_s])]
-        write("full_size_oracle.txt", out)
+        write(f"full_size_oracle{SUFFIX}.txt", out)
     if do5:
         out = ["# written by tests/golden/make_full_size_golden.py (CPU oracle only); cfg 5 = BASELINE.json configs[4],",
                f"# right-hand sides {CFG5_COLUMNS} of 16; x, lambda at rows rng({SEED_ROWS}).integers(0, n, {NS}),",
@@ -109,7 +115,7 @@ def cfg4_and_5(do4, do5):
                     f"cfg5_rhs{s} lambda_converged " + fmt(lam[rows_s]),
                     f"cfg5_rhs{s} gA " + fmt(gA[ent_s])]
             assert np.array_equal(gA[ent_s], -(lam[row_of] * x[A.col[ent_s]]))
-            write("full_size_cfg5.txt", out)  # keep what is done so far
+            write(f"full_size_cfg5{SUFFIX}.txt", out)  # keep what is done so far
     o.close()
 
 
@@ -117,7 +123,7 @@ def cfg2():
     A = inputs.config_matrix(2, 1024)
     Asp = A.to_scipy()
     t = time.time()
-    o = oracle.Oracle(A.rowptr, A.col, A.val)
+    o = oracle.Oracle(A.rowptr, A.col, A.val, **OPTS)
     ts = time.time() - t
     rows_s = sample_rows(A.n, NS2)
     shapes = [o.level_info(l) for l in range(o.num_levels)]
@@ -134,11 +140,16 @@ def cfg2():
                 f"cfg2_rhs{s} converged_status {info.status}",
                 f"cfg2_rhs{s} x_converged " + fmt(x[rows_s])]
     o.close()
-    write("full_size_cfg2.txt", out)
+    write(f"full_size_cfg2{SUFFIX}.txt", out)
 
 
 def main():
-    which = set(sys.argv[1:]) or {"cfg4", "cfg5", "cfg2"}
+    global OPTS, SUFFIX
+    which = set(sys.argv[1:])
+    if "tuned" in which:
+        OPTS, SUFFIX = dict(TUNED), "_tuned"
+        which.discard("tuned")
+    which = which or {"cfg4", "cfg5", "cfg2"}
     oracle.build()
     oracle.set_threads(os.cpu_count() or 1)
     if "cfg2" in which:

