@@ -146,7 +146,10 @@ typedef struct {
 AMG_API amg_status amg_options_default(amg_options* opt);
 
 /* Optional: route library-owned device memory through the caller's allocator (e.g. torch's
- * caching allocator).  Process-wide; call before amg_setup.  Pass NULLs to restore cudaMalloc. */
+ * caching allocator).  A handle keeps the allocator that was installed when it was created.  Pass NULLs
+ * to restore the stream-ordered pool.  free_fn may be called while work that uses the block is still queued
+ * on the stream the block was allocated on: the allocator must be stream-ordered on that stream (torch's
+ * caching allocator, cudaFreeAsync) or synchronise itself (cudaFree). */
 AMG_API amg_status amg_set_allocator(void* (*alloc_fn)(size_t bytes, void* cuda_stream, void* user),
                              void (*free_fn)(void* ptr, void* user), void* user);
 

@@ -92,8 +92,7 @@ amg_status amg_exclusive_scan(amg_handle_s* H, const int* d_in, int* d_out, int 
   AMG_TRY(amg_exclusive_scan(H, bsum, bsum, nb, st));  // in place: every block reads before it writes
   k_scan_add<<<div_up(n1, TPB), TPB, 0, st>>>(d_out, n1, bsum);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  amg_dev_free(H, bsum);
+  amg_dev_free(H, bsum);  // (frees are stream-ordered: no synchronisation)
   return AMG_OK;
 }
 
@@ -855,7 +854,6 @@ amg_status transpose_csr(amg_handle_s* H, int n, int nnz, int nnz_alloc, const i
   k_gather_vals<<<grid_for(nnz), TPB, 0, st>>>(nnz, val, *tsrc, *tval);
   if (nnz_alloc > nnz) k_pad_tail<<<1, 32, 0, st>>>(nnz, nnz_alloc, *tcol, *tval);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   amg_dev_free(H, cnt);
   return AMG_OK;
 }
@@ -959,7 +957,6 @@ amg_status aggregate_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, con
   AMG_ALLOC(H, *agg_out, int, n, st);
   k_assign_agg<<<g, TPB, 0, st>>>(n, root, id, *agg_out);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   for (void* q : {(void*)m, (void*)match, (void*)ptr, (void*)root, (void*)isroot, (void*)id, (void*)added, (void*)trp,
                   (void*)tcol, (void*)tval, (void*)tsrc, (void*)srp, (void*)scol, (void*)sval, (void*)slen})
     amg_dev_free(H, q);
@@ -983,7 +980,6 @@ amg_status aggregate_level(amg_handle_s* H, NatCsr& N, uint64_t salt, int* round
                           &r2, st));
     k_compose_agg<<<grid_for(N.n), TPB, 0, st>>>(N.n, N.agg, agg2);
     AMG_CUDA_TRY(H, cudaGetLastError());
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     N.nc = nc2;
     if (r2 > *rounds_out) *rounds_out = r2;
     for (void* q : {(void*)agg2, (void*)mid.rowptr, (void*)mid.col, (void*)mid.val, (void*)N.mptr, (void*)N.mem})
@@ -1007,7 +1003,6 @@ amg_status build_members(amg_handle_s* H, NatCsr& N, cudaStream_t st) {
   k_fill_members<<<grid_for(n), TPB, 0, st>>>(n, N.agg, N.mptr, slot, N.mem);
   k_sort_members<<<grid_for(nc), TPB, 0, st>>>(nc, N.mptr, N.mem);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   amg_dev_free(H, cnt);
   amg_dev_free(H, slot);
   return AMG_OK;
@@ -1037,7 +1032,6 @@ amg_status galerkin_level(amg_handle_s* H, const NatCsr& N, NatCsr& C, cudaStrea
   AMG_ALLOC(H, C.val, double, C.nnz, st);
   k_rap_compact<<<grid_for(nc), TPB, 0, st>>>(nc, segptr, skey, sval, C.rowptr, C.col, C.val);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   amg_dev_free(H, len);
   amg_dev_free(H, segptr);
   amg_dev_free(H, cnt);
@@ -1058,7 +1052,6 @@ amg_status permute_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const
   k_perm_fill<<<div_up(n, 128), 128, 0, st>>>(n, rowptr, col, val, src_row, col_map, rowptr_out, col_out,
                                           val_out);
   AMG_CUDA_TRY(H, cudaGetLastError());
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
   amg_dev_free(H, len);
   (void)nnz;
   return AMG_OK;
@@ -1154,7 +1147,6 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
       k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, vb, 1, off16, hoff, size16, nh, info,
                                                  P.tiles, P.blob, P.halo_idx, P.halo_cagg);
       AMG_CUDA_TRY(H, cudaGetLastError());
-      AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
       P.fast = 1;
       if (scale_io) *scale_io = scale;
     }
@@ -1330,7 +1322,6 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     k_perm_pos<<<grid_for(L.nc), TPB, 0, st>>>(L.nc, N.mptr, N.mem, H->lv[q + 1].pos, L.agg_ptr, L.pos, L.inv,
                                               L.agg);
     AMG_CUDA_TRY(H, cudaGetLastError());
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     amg_dev_free(H, sizep);
   }
   double pack_scale = 1.0;
@@ -1594,7 +1585,6 @@ amg_status build_resetup_maps(amg_handle_s* H, cudaStream_t st) {
     k_contrib_fill<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, tgt, L.contrib_ptr, cnt, L.contrib_idx);
     k_contrib_sort<<<grid_for(C.nnz), TPB, 0, st>>>(C.nnz, L.contrib_ptr, L.contrib_idx);
     AMG_CUDA_TRY(H, cudaGetLastError());
-    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     amg_dev_free(H, tgt);
     amg_dev_free(H, cnt);
   }
