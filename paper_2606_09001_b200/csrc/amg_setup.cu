@@ -207,9 +207,11 @@ __global__ void k_row_max(int n, const int* __restrict__ rowptr, const int* __re
 // every unmatched vertex points to its best unmatched candidate neighbour (state = match[])
 __global__ void k_propose(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
                           const double* __restrict__ val, const double* __restrict__ m, double beta,
-                          uint64_t salt, const int* __restrict__ match, int* __restrict__ ptr) {
+                          uint64_t salt, const int* __restrict__ match, int* __restrict__ ptr,
+                          const int* __restrict__ prev_added) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (prev_added && *prev_added == 0) return;  // the matching was already maximal a round ago (rounds are queued ahead)
   int best_j = -1;
   if (match[i] < 0) {
     EdgeKey best{};
@@ -229,9 +231,10 @@ __global__ void k_propose(int n, const int* __restrict__ rowptr, const int* __re
 }
 
 __global__ void k_handshake(int n, const int* __restrict__ ptr, int* __restrict__ match,
-                            int* __restrict__ added) {
+                            int* __restrict__ added, const int* __restrict__ prev_added) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (prev_added && *prev_added == 0) return;
   int j = ptr[i];
   if (j >= 0 && ptr[j] == i) {
     match[i] = j;
@@ -338,15 +341,11 @@ __global__ void k_rap_len(int nc, const int* __restrict__ mptr, const int* __res
   len[I] = s;
 }
 
-__global__ void k_rap_rows(int nc, const int* __restrict__ mptr, const int* __restrict__ mem,
-                           const int* __restrict__ rowptr, const int* __restrict__ col,
-                           const double* __restrict__ val, const int* __restrict__ agg,
-                           const int* __restrict__ segptr, int* __restrict__ skey,
-                           double* __restrict__ sval, int* __restrict__ cnt) {
-  int I = blockIdx.x * blockDim.x + threadIdx.x;
-  if (I >= nc) return;
-  int* key = skey + segptr[I];
-  double* acc = sval + segptr[I];
+// serial form (one lane): also the path of a coarse row whose segment does not fit the group's shared lists
+__device__ void rap_row_serial(int I, const int* __restrict__ mptr, const int* __restrict__ mem,
+                               const int* __restrict__ rowptr, const int* __restrict__ col,
+                               const double* __restrict__ val, const int* __restrict__ agg, int* __restrict__ key,
+                               double* __restrict__ acc, int* __restrict__ cnt) {
   int m = 0;  // entries in the sorted list
   for (int t = mptr[I]; t < mptr[I + 1]; ++t) {
     int i = mem[t];
@@ -369,6 +368,70 @@ __global__ void k_rap_rows(int nc, const int* __restrict__ mptr, const int* __re
     }
   }
   cnt[I] = m;
+}
+
+// G lanes per coarse row.  The entries (J, a) of the members' rows are listed in shared memory in the fixed order
+// (ascending fine row, ascending position), ranked by a STABLE counting sort on J (every lane compares its entry with
+// all others: the lists are short), and every distinct J is summed by one lane from its first entry on: the same
+// additions in the same order as the serial form, so the values are bit-equal to it.
+constexpr int RAP_THREADS = 128;
+template <int G, int CAP>
+__global__ void __launch_bounds__(RAP_THREADS)
+    k_rap_rows(int nc, const int* __restrict__ mptr, const int* __restrict__ mem, const int* __restrict__ rowptr,
+               const int* __restrict__ col, const double* __restrict__ val, const int* __restrict__ agg,
+               const int* __restrict__ segptr, int* __restrict__ skey, double* __restrict__ sval,
+               int* __restrict__ cnt) {
+  constexpr int GROUPS = RAP_THREADS / G;
+  __shared__ int uk[GROUPS][CAP], sk[GROUPS][CAP];
+  __shared__ double uv[GROUPS][CAP], sv[GROUPS][CAP];
+  const int g = threadIdx.x / G, lane = threadIdx.x % G;
+  constexpr unsigned LOW = (unsigned)((1ull << G) - 1ull);  // G lanes
+  const int shift = (threadIdx.x % 32) / G * G;
+  const unsigned gmask = LOW << shift;
+  const int I = blockIdx.x * GROUPS + g;
+  if (I >= nc) return;  // whole groups leave together
+  const int seg = segptr[I], L = segptr[I + 1] - seg;
+  if (L > CAP) {
+    if (lane == 0) rap_row_serial(I, mptr, mem, rowptr, col, val, agg, skey + seg, sval + seg, cnt);
+    return;
+  }
+  int off = 0;
+  for (int t = mptr[I]; t < mptr[I + 1]; ++t) {
+    const int i = mem[t], r0 = rowptr[i], len = rowptr[i + 1] - r0;
+    for (int k = lane; k < len; k += G) {
+      uk[g][off + k] = agg[col[r0 + k]];
+      uv[g][off + k] = val[r0 + k];
+    }
+    off += len;
+  }
+  __syncwarp(gmask);
+  for (int e = lane; e < L; e += G) {
+    const int J = uk[g][e];
+    int r = 0;
+    for (int f = 0; f < L; ++f) {
+      const int K = uk[g][f];
+      r += (K < J) | ((K == J) & (f < e));
+    }
+    sk[g][r] = J;
+    sv[g][r] = uv[g][e];
+  }
+  __syncwarp(gmask);
+  int base = 0;
+  for (int r0 = 0; r0 < L; r0 += G) {  // uniform trip count inside the group
+    const int r = r0 + lane;
+    const bool head = r < L && (r == 0 || sk[g][r - 1] != sk[g][r]);
+    const unsigned heads = (__ballot_sync(gmask, head) & gmask) >> shift;
+    if (head) {
+      const int J = sk[g][r];
+      double a = sv[g][r];
+      for (int q = r + 1; q < L && sk[g][q] == J; ++q) a += sv[g][q];
+      const int pos = base + __popc(heads & ((1u << lane) - 1u));
+      skey[seg + pos] = J;
+      sval[seg + pos] = a;
+    }
+    base += __popc(heads);
+  }
+  if (lane == 0) cnt[I] = base;
 }
 
 __global__ void k_rap_compact(int nc, const int* __restrict__ segptr, const int* __restrict__ skey,
@@ -521,27 +584,50 @@ __global__ void k_perm_rowlen(int n, const int* __restrict__ rowptr, const int* 
 
 // row p of the output is row src_row[p] of the input with columns relabelled by col_map and
 // re-sorted ascending
-__global__ void k_perm_fill(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
-                            const double* __restrict__ val, const int* __restrict__ src_row,
-                            const int* __restrict__ col_map, const int* __restrict__ rowptr_out,
-                            int* __restrict__ col_out, double* __restrict__ val_out) {
-  int p = blockIdx.x * blockDim.x + threadIdx.x;
+// G lanes per output row: the mapped columns are ranked in shared memory (a permutation keeps them distinct) and
+// written in ascending order; a row longer than CAP is insertion-sorted in place by one lane
+template <int G, int CAP>
+__global__ void __launch_bounds__(128)
+    k_perm_fill(int n, const int* __restrict__ rowptr, const int* __restrict__ col, const double* __restrict__ val,
+                const int* __restrict__ src_row, const int* __restrict__ col_map,
+                const int* __restrict__ rowptr_out, int* __restrict__ col_out, double* __restrict__ val_out) {
+  constexpr int GROUPS = 128 / G;
+  __shared__ int uk[GROUPS][CAP];
+  __shared__ double uv[GROUPS][CAP];
+  const int g = threadIdx.x / G, lane = threadIdx.x % G;
+  constexpr unsigned LOW = (unsigned)((1ull << G) - 1ull);
+  const unsigned gmask = LOW << ((threadIdx.x % 32) / G * G);
+  const int p = blockIdx.x * GROUPS + g;
   if (p >= n) return;
-  int i = src_row[p];
-  int s = rowptr[i], e = rowptr[i + 1], d = rowptr_out[p];
-  int m = 0;
-  for (int k = s; k < e; ++k) {
-    int c = col_map[col[k]];
-    double v = val[k];
-    int q = m;
-    while (q > 0 && col_out[d + q - 1] > c) {
-      col_out[d + q] = col_out[d + q - 1];
-      val_out[d + q] = val_out[d + q - 1];
-      --q;
+  const int i = src_row[p];
+  const int s = rowptr[i], len = rowptr[i + 1] - s, d = rowptr_out[p];
+  if (len > CAP) {
+    if (lane != 0) return;
+    for (int m = 0; m < len; ++m) {
+      int c = col_map[col[s + m]];
+      double v = val[s + m];
+      int q = m;
+      while (q > 0 && col_out[d + q - 1] > c) {
+        col_out[d + q] = col_out[d + q - 1];
+        val_out[d + q] = val_out[d + q - 1];
+        --q;
+      }
+      col_out[d + q] = c;
+      val_out[d + q] = v;
     }
-    col_out[d + q] = c;
-    val_out[d + q] = v;
-    ++m;
+    return;
+  }
+  for (int k = lane; k < len; k += G) {
+    uk[g][k] = col_map[col[s + k]];
+    uv[g][k] = val[s + k];
+  }
+  __syncwarp(gmask);
+  for (int e = lane; e < len; e += G) {
+    const int c = uk[g][e];
+    int r = 0;
+    for (int f = 0; f < len; ++f) r += uk[g][f] < c;
+    col_out[d + r] = c;
+    val_out[d + r] = uv[g][e];
   }
 }
 
@@ -933,21 +1019,33 @@ amg_status aggregate_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, con
   AMG_ALLOC(H, root, int, n, st);
   AMG_ALLOC(H, isroot, int, n, st);
   AMG_ALLOC(H, id, int, n + 1, st);
-  AMG_ALLOC(H, added, int, 1, st);
+  AMG_ALLOC(H, added, int, 8, st);
   const int g = grid_for(n);
   k_row_max<<<g, TPB, 0, st>>>(n, rowptr, col, val, m);
   k_fill_int<<<g, TPB, 0, st>>>(n, match, -1);
+  // U1 rounds until one adds no pair.  MATCH_BATCH rounds are queued before the host looks at the counters (one
+  // synchronisation per batch instead of one per round); a round queued behind the one that added nothing returns
+  // at once on the device, so the matching and the reported round count are those of the round-by-round loop.
+  constexpr int MATCH_BATCH = 6;
   int rounds = 0;
-  for (;;) {
-    if (o.max_match_rounds > 0 && rounds >= o.max_match_rounds) break;
-    AMG_CUDA_TRY(H, cudaMemsetAsync(added, 0, sizeof(int), st));
-    k_propose<<<g, TPB, 0, st>>>(n, rowptr, col, val, m, o.strong_beta, salt, match, ptr);
-    k_handshake<<<g, TPB, 0, st>>>(n, ptr, match, added);
+  for (bool done = false; !done;) {
+    int nb = MATCH_BATCH;
+    if (o.max_match_rounds > 0) nb = std::min(nb, o.max_match_rounds - rounds);
+    if (nb <= 0) break;
+    AMG_CUDA_TRY(H, cudaMemsetAsync(added + 1, 0, sizeof(int) * MATCH_BATCH, st));
+    for (int r = 0; r < nb; ++r) {
+      const int* prev = r > 0 ? added + r : nullptr;  // slot r + 1 counts round r of the batch
+      k_propose<<<g, TPB, 0, st>>>(n, rowptr, col, val, m, o.strong_beta, salt, match, ptr, prev);
+      k_handshake<<<g, TPB, 0, st>>>(n, ptr, match, added + r + 1, prev);
+    }
     AMG_CUDA_TRY(H, cudaGetLastError());
-    int h_added = 0;
-    AMG_TRY(read_int(H, added, &h_added, st));
-    ++rounds;
-    if (h_added == 0) break;
+    int h_added[MATCH_BATCH];
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_added, added + 1, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    for (int r = 0; r < nb && !done; ++r) {
+      ++rounds;
+      done = h_added[r] == 0;
+    }
   }
   *rounds_out = rounds;
   k_roots<<<g, TPB, 0, st>>>(n, rowptr, col, val, m, o.strong_beta, salt, match, root, isroot);
@@ -1021,8 +1119,12 @@ amg_status galerkin_level(amg_handle_s* H, const NatCsr& N, NatCsr& C, cudaStrea
   k_rap_len<<<grid_for(nc), TPB, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, len);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_TRY(amg_exclusive_scan(H, len, segptr, nc, st));
-  k_rap_rows<<<div_up(nc, 128), 128, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, N.col, N.val, N.agg, segptr, skey,
-                                          sval, cnt);
+  if ((long long)N.nnz <= 24ll * nc)  // short merged rows (the fine levels): 8 lanes per coarse row
+    k_rap_rows<8, 64><<<div_up(nc, RAP_THREADS / 8), RAP_THREADS, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, N.col, N.val,
+                                                                         N.agg, segptr, skey, sval, cnt);
+  else
+    k_rap_rows<32, 320><<<div_up(nc, RAP_THREADS / 32), RAP_THREADS, 0, st>>>(nc, N.mptr, N.mem, N.rowptr, N.col,
+                                                                            N.val, N.agg, segptr, skey, sval, cnt);
   AMG_CUDA_TRY(H, cudaGetLastError());
   C.n = nc;
   AMG_ALLOC(H, C.rowptr, int, nc + 1, st);
@@ -1049,7 +1151,11 @@ amg_status permute_csr(amg_handle_s* H, int n, int nnz, const int* rowptr, const
   k_perm_rowlen<<<grid_for(n), TPB, 0, st>>>(n, rowptr, src_row, len);
   AMG_CUDA_TRY(H, cudaGetLastError());
   AMG_TRY(amg_exclusive_scan(H, len, rowptr_out, n, st));
-  k_perm_fill<<<div_up(n, 128), 128, 0, st>>>(n, rowptr, col, val, src_row, col_map, rowptr_out, col_out,
+  if ((long long)nnz <= 12ll * n)
+    k_perm_fill<8, 64><<<div_up(n, 16), 128, 0, st>>>(n, rowptr, col, val, src_row, col_map, rowptr_out, col_out,
+                                          val_out);
+  else
+    k_perm_fill<32, 320><<<div_up(n, 4), 128, 0, st>>>(n, rowptr, col, val, src_row, col_map, rowptr_out, col_out,
                                           val_out);
   AMG_CUDA_TRY(H, cudaGetLastError());
   amg_dev_free(H, len);
