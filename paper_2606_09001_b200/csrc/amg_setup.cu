@@ -384,6 +384,7 @@ __global__ void __launch_bounds__(RAP_THREADS)
   constexpr int GROUPS = RAP_THREADS / G;
   __shared__ int uk[GROUPS][CAP], sk[GROUPS][CAP];
   __shared__ double uv[GROUPS][CAP], sv[GROUPS][CAP];
+  __shared__ int mr0[GROUPS][G], mend[GROUPS][G];
   const int g = threadIdx.x / G, lane = threadIdx.x % G;
   constexpr unsigned LOW = (unsigned)((1ull << G) - 1ull);  // G lanes
   const int shift = (threadIdx.x % 32) / G * G;
@@ -395,14 +396,41 @@ __global__ void __launch_bounds__(RAP_THREADS)
     if (lane == 0) rap_row_serial(I, mptr, mem, rowptr, col, val, agg, skey + seg, sval + seg, cnt);
     return;
   }
-  int off = 0;
-  for (int t = mptr[I]; t < mptr[I + 1]; ++t) {
-    const int i = mem[t], r0 = rowptr[i], len = rowptr[i + 1] - r0;
-    for (int k = lane; k < len; k += G) {
-      uk[g][off + k] = agg[col[r0 + k]];
-      uv[g][off + k] = val[r0 + k];
+  const int m0 = mptr[I], nm = mptr[I + 1] - m0;
+  if (nm <= G) {
+    // lane t holds member t's row start and its offset in the list: the entries of all members load at once
+    int r0 = 0, len = 0;
+    if (lane < nm) {
+      const int i = mem[m0 + lane];
+      r0 = rowptr[i];
+      len = rowptr[i + 1] - r0;
     }
-    off += len;
+    int incl = len;
+#pragma unroll
+    for (int d = 1; d < G; d <<= 1) {
+      const int v = __shfl_up_sync(gmask, incl, d, G);
+      if (lane >= d) incl += v;
+    }
+    mr0[g][lane] = r0 - (incl - len);  // entry e of member t sits at mr0[t] + e
+    mend[g][lane] = incl;             // one past member t's last entry
+    __syncwarp(gmask);
+    for (int e = lane; e < L; e += G) {
+      int t = 0;
+      while (mend[g][t] <= e) ++t;
+      const int k = mr0[g][t] + e;
+      uk[g][e] = agg[col[k]];
+      uv[g][e] = val[k];
+    }
+  } else {
+    int off = 0;
+    for (int t = m0; t < m0 + nm; ++t) {
+      const int i = mem[t], r0 = rowptr[i], len = rowptr[i + 1] - r0;
+      for (int k = lane; k < len; k += G) {
+        uk[g][off + k] = agg[col[r0 + k]];
+        uv[g][off + k] = val[r0 + k];
+      }
+      off += len;
+    }
   }
   __syncwarp(gmask);
   for (int e = lane; e < L; e += G) {
