@@ -207,13 +207,13 @@ __global__ void k_row_max(int n, const int* __restrict__ rowptr, const int* __re
 // every unmatched vertex points to its best unmatched candidate neighbour (state = match[])
 __global__ void k_propose(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
                           const double* __restrict__ val, const double* __restrict__ m, double beta,
-                          uint64_t salt, const int* __restrict__ match, int* __restrict__ ptr,
+                          uint64_t salt, int* __restrict__ match, int* __restrict__ ptr,
                           const int* __restrict__ prev_added) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   if (prev_added && *prev_added == 0) return;  // the matching was already maximal a round ago (rounds are queued ahead)
   int best_j = -1;
-  if (match[i] < 0) {
+  if (match[i] == -1) {
     EdgeKey best{};
     double mi = m[i];
     for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
@@ -226,6 +226,9 @@ __global__ void k_propose(int n, const int* __restrict__ rowptr, const int* __re
         best_j = j;
       }
     }
+    // no unmatched candidate left: there will be none in any later round either (the matched set only grows), so the
+    // row retires (-2: still "unmatched" for every reader) and later rounds skip its edge scan
+    if (best_j < 0) match[i] = -2;
   }
   ptr[i] = best_j;
 }
@@ -765,14 +768,25 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   }
   const int nsl = (nr + 31) >> 5;
   if (tid == 0) {
-    // stable counting sort by descending length; slice widths = length of the slice's first row
+    // stable counting sort by descending length: hist[l] = first sorted position of the rows of length l
     int acc = 0;
     for (int l = s_maxlen; l >= 0; --l) {
       const int c = hist[l];
       hist[l] = acc;
       acc += c;
     }
-    for (int lr = 0; lr < nr; ++lr) srow[hist[len[lr]]++] = lr;
+  }
+  __syncthreads();
+  // sorted position of a row = first position of its length + the rows of that length before it (every thread walks
+  // len[] with the same index: broadcast reads)
+  for (int lr = tid; lr < nr; lr += PK_THREADS) {
+    const int l = len[lr];
+    int before = 0;
+    for (int q = 0; q < lr; ++q) before += (len[q] == l);
+    srow[hist[l] + before] = lr;
+  }
+  __syncthreads();
+  if (tid == 0) {  // slice widths = length of the slice's first row
     int off = 0;
     for (int j = 0; j < nsl; ++j) {
       const int w = len[srow[j * 32]];
@@ -853,36 +867,40 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);  // vb == 4: mixed-precision hierarchy
-  for (int j = 0; j < nsl; ++j) {
-    const int off = sl_off[j], w = sl_w[j];
-    for (int q = tid; q < 32 * w; q += PK_THREADS) {
-      const int k = q >> 5, lane = q & 31, s = j * 32 + lane;
+  // one thread per row (sorted position s = slice j, lane): its entries k = 0 .. w_j - 1, zero-padded past the row's
+  // length; the loads of a row are independent of one another, the stores of a warp for a fixed k are contiguous
+  for (int s = tid; s < nsl * 32; s += PK_THREADS) {
+    const int j = s >> 5, lane = s & 31;
+    const int off = sl_off[j] + lane, w = sl_w[j];
+    int ln = 0, kk0 = 0;
+    if (s < nr) {
+      const int lr = srow[s];
+      ln = len[lr];
+      kk0 = rowptr[r0 + lr];
+    }
+    for (int k = 0; k < w; ++k) {
       unsigned short c16 = 0;
       double v = 0.0;
-      if (s < nr) {
-        const int lr = srow[s];
-        if (k < len[lr]) {
-          const int kk = rowptr[r0 + lr] + k;
-          const int c = col[kk];
-          v = val[kk];
-          if (c >= r0 && c < r1) {
-            c16 = (unsigned short)(c - r0);
-          } else {
-            int lo = 0, hi = d.nhalo;  // first entry >= c
-            while (lo < hi) {
-              const int mid = (lo + hi) >> 1;
-              if (halo[mid] < c) lo = mid + 1;
-              else hi = mid;
-            }
-            c16 = (unsigned short)(nr + lo);
+      if (k < ln) {
+        const int c = col[kk0 + k];
+        v = val[kk0 + k];
+        if (c >= r0 && c < r1) {
+          c16 = (unsigned short)(c - r0);
+        } else {
+          int lo = 0, hi = d.nhalo;  // first entry >= c
+          while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (halo[mid] < c) lo = mid + 1;
+            else hi = mid;
           }
+          c16 = (unsigned short)(nr + lo);
         }
       }
-      o_col[off + q] = c16;
+      o_col[off + k * 32] = c16;
       if (vb == 4)
-        o_val32[off + q] = (float)v;
+        o_val32[off + k * 32] = (float)v;
       else
-        o_val[off + q] = v;
+        o_val[off + k * 32] = v;
     }
   }
   // tail of the u16 column section up to its 16-byte rounding
