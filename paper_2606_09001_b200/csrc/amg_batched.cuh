@@ -60,11 +60,14 @@ struct RowArgsB {
 };
 
 // ---- placement of a tile inside its ring stage (after the TP_DESC_BYTES header); blob at 0 ----
+// Every operation keeps a ROW BUFFER [nr][NB] in the stage (64 bytes per row, the layout the vectors
+// have in global memory): the tile's rows of b arrive in it by one bulk-async copy, the result of a
+// row overwrites its b in place, and the finished tile leaves by one bulk-async store.
 struct StageLayoutB {
   int ra2, nrv;  // dinv slice (even start / count)
   int Ia4, nap;  // agg_ptr slice
   int Ia2, nec;  // dinv_c slice
-  int o_d, o_agg, o_dc, o_out, end;
+  int o_d, o_agg, o_dc, o_row, end;
 };
 enum { TPB_D = 1, TPB_RESTRICT = 2 };
 __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) {
@@ -84,8 +87,8 @@ __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) 
   if (flags & TPB_RESTRICT) o += 4 * t.nap;
   t.o_dc = o;
   if (flags & TPB_RESTRICT) o += 8 * t.nec;
-  t.o_out = o;
-  if (flags & TPB_RESTRICT) o += 8 * NB * d.nr;
+  t.o_row = o;
+  o += 8 * NB * d.nr;
   t.end = o;
   return t;
 }
@@ -93,8 +96,8 @@ __host__ __device__ inline int tpb_stage_need(const TileDesc& d) {
   const int a = tpb_stage(d, TPB_D).end, b = tpb_stage(d, TPB_RESTRICT).end;
   return TP_DESC_BYTES + (a > b ? a : b);
 }
-__host__ __device__ inline int tpb_ncolp(int nr, int nhalo) { return (nr + nhalo) | 1; }  // odd plane pitch
-__host__ __device__ inline int tpb_xslot_need(const TileDesc& d) { return 16 * NB2 * tpb_ncolp(d.nr, d.nhalo); }
+// x slot: [column][NB] (own rows first, then the halo columns), 64 bytes per column
+__host__ __device__ inline int tpb_xslot_need(const TileDesc& d) { return 8 * NB * (d.nr + d.nhalo); }
 
 // ---- per-column finalisation of a reduction; a finished column is frozen ----
 __device__ inline void krylov_finalize_b(KrylovCtlB* cb, int fin, const double* s0) {
@@ -166,51 +169,98 @@ __device__ __forceinline__ void grid_reduce_finalize_b(double (&v)[NB], double* 
 
 // ------------------------------------------------------------------------------------------
 // Batched row-tile kernel.  OP: OP_SPMV (dot: x.out per column), OP_JACOBI (dot: b.out),
-// OP_RESTRICT, OP_JACOBI_PROLONG (dot: b.out).  Everything the producer stages (blob, dinv,
-// agg_ptr, dinv_c) is setup data, so its first copies are issued before the grid dependency.
+// OP_RESTRICT, OP_JACOBI_PROLONG (dot: b.out).
+//
+// Everything contiguous moves by bulk-async copies (TMA), not through the load/store pipe, which
+// is what bounds this kernel: the tile's blob, dinv / agg_ptr / dinv_c slices (setup data, issued
+// before the grid dependency), its rows of b (into the stage's row buffer), its OWN rows of x
+// (straight into the x slot; the gather warps fetch the halo columns only) and its rows of the
+// result (row buffer -> global, one bulk store per tile issued by the producer thread once every
+// consumer warp has released the stage).  Only the prolongation-fused sweep, whose own rows are
+// x + gamma ec[agg], assembles them in the gather warps.
+//
+// Shared-memory layout of the vectors is the global one, [row or column][NB] = 64 bytes each.  A
+// consumer lane reads the NB2 16-byte chunks of a column in the order h ^ rot, rot = (lane / 2) & 3:
+// its accumulator pair h belongs to right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1.  With that
+// rotation the 16 lanes of a half-warp that walk 16 consecutive rows (row buffer, own x) hit every
+// 16-byte bank group exactly twice -- the minimum for a 128-bit access -- and the random columns of
+// the entry loop spread over the bank groups as evenly as a plane layout would.
 // ------------------------------------------------------------------------------------------
 struct StageDescB {  // TP_DESC_BYTES at the start of a stage, written by the producer
   int r0, nr, I0, nA;
   int nsl, nhalo, roff, aoff;  // roff = r0 - ra2 (dinv slice), aoff = I0 - Ia4 (agg_ptr slice)
   int o_perm, o_col, o_val, o_d;
-  int o_agg, o_out, o_dc, eoff;  // eoff = Ia2 (dcs[I - eoff] = dinv_c[I])
+  int o_agg, o_row, o_dc, eoff;  // eoff = Ia2 (dcs[I - eoff] = dinv_c[I])
   int vb;                        // bytes per stored value (8, or 4 with the mixed-precision hierarchy)
   int pad[15];
 };
 static_assert(sizeof(StageDescB) == TP_DESC_BYTES, "stage header size");
 
+// shared -> global bulk-async store; completion is tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// mode 0: header + every copy, all on `bar`;  mode 1: header + the setup data (blob, dinv, agg_ptr,
+// dinv_c), on `bar` (issued before the grid dependency);  mode 2: the tile's rows of b only, on `bar`
 template <int OP, bool STREAM>
 __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
-                                             uint64_t pol) {
+                                             uint64_t pol, int mode) {
   constexpr bool SWEEP = (OP == OP_JACOBI || OP == OP_JACOBI_PROLONG);
   constexpr bool RES = (OP == OP_RESTRICT);
+  constexpr bool HASB = (OP != OP_SPMV);
   const bool dc = RES && a.dinv_c != nullptr;
   const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const StageLayoutB t = tpb_stage(d, (SWEEP ? TPB_D : 0) | (RES ? TPB_RESTRICT : 0));
-  StageDescB sd;
-  sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
-  sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
-  sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_d = t.o_d;
-  sd.o_agg = t.o_agg, sd.o_out = t.o_out, sd.o_dc = t.o_dc, sd.eoff = t.Ia2;
-  sd.vb = d.vb;
-  int4* dst = reinterpret_cast<int4*>(stage);
-  const int4* src = reinterpret_cast<const int4*>(&sd);
+  if (mode != 2) {
+    StageDescB sd;
+    sd.r0 = d.r0, sd.nr = d.nr, sd.I0 = d.I0, sd.nA = d.nA;
+    sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
+    sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_d = t.o_d;
+    sd.o_agg = t.o_agg, sd.o_row = t.o_row, sd.o_dc = t.o_dc, sd.eoff = t.Ia2;
+    sd.vb = d.vb;
+    int4* dst = reinterpret_cast<int4*>(stage);
+    const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
-  for (int q = 0; q < 5; ++q) dst[q] = src[q];
+    for (int q = 0; q < 5; ++q) dst[q] = src[q];
+  }
   if (d.nr <= 0) {
     mbar_arrive(bar);
     return;
   }
   unsigned char* base = stage + TP_DESC_BYTES;
-  uint32_t bytes = (uint32_t)p.end;
-  if (SWEEP) bytes += 8u * (uint32_t)t.nrv;
-  if (RES) bytes += 4u * (uint32_t)t.nap;
-  if (dc) bytes += 8u * (uint32_t)t.nec;
+  const uint32_t rowbytes = 8u * NB * (uint32_t)d.nr;
+  uint32_t bytes = 0;
+  if (mode != 2) {
+    bytes += (uint32_t)p.end;
+    if (SWEEP) bytes += 8u * (uint32_t)t.nrv;
+    if (RES) bytes += 4u * (uint32_t)t.nap;
+    if (dc) bytes += 8u * (uint32_t)t.nec;
+  }
+  if (mode != 1 && HASB) bytes += rowbytes;
+  if (bytes == 0) {  // mode 2 of an operation without b
+    mbar_arrive(bar);
+    return;
+  }
   mbar_arrive_expect_tx(bar, bytes);
-  bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, (uint32_t)p.end, bar, pol);
-  if (SWEEP) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, 8u * (uint32_t)t.nrv, bar, pol);
-  if (RES) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
-  if (dc) bulk_g2s<false>(base + t.o_dc, a.dinv_c + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
+  if (mode != 2) {
+    bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, (uint32_t)p.end, bar, pol);
+    if (SWEEP) bulk_g2s<false>(base + t.o_d, a.dinv + t.ra2, 8u * (uint32_t)t.nrv, bar, pol);
+    if (RES) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
+    if (dc) bulk_g2s<false>(base + t.o_dc, a.dinv_c + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
+  }
+  if (mode != 1 && HASB) bulk_g2s<false>(base + t.o_row, a.b + (size_t)d.r0 * NB, rowbytes, bar, pol);
+}
+
+// the finished rows of the tile in `stage` leave by one bulk store (producer thread)
+__device__ __forceinline__ void tile_store_b(const RowArgsB& a, unsigned char* stage) {
+  const StageDescB* sd = reinterpret_cast<const StageDescB*>(stage);
+  if (sd->nr > 0)
+    bulk_s2g(a.out + (size_t)sd->r0 * NB, stage + TP_DESC_BYTES + sd->o_row, 8u * NB * (uint32_t)sd->nr);
 }
 
 struct GTileB {
@@ -230,8 +280,12 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty = full + RTB_MAXS;
   uint64_t* resdone = empty + RTB_MAXS;
-  uint64_t* xready = resdone + RTB_MAXS;
+  uint64_t* pre = resdone + RTB_MAXS;  // setup data of the first ring stages, issued before the grid dependency
+  uint64_t* xready = pre + RTB_MAXS;
   uint64_t* xempty = xready + RTB_MAXS;
+  static_assert(6 * RTB_MAXS * 8 <= RTB_HEADER, "barrier header");
+  constexpr bool OWN_TMA = (OP != OP_JACOBI_PROLONG);  // the tile's own rows of x arrive by a bulk copy
+  constexpr bool STORE = (OP != OP_RESTRICT);          // the tile's rows of the result leave by a bulk store
   const int S = a.stages, XS = a.xslots;
   unsigned char* stage0 = smem + RTB_HEADER;
   unsigned char* xslot0 = stage0 + (size_t)S * a.stage_bytes;
@@ -246,9 +300,10 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
       mbar_init(full + s, 1);
       mbar_init(empty + s, NCW);
       mbar_init(resdone + s, NCW);
+      mbar_init(pre + s, 1);
     }
     for (int q = 0; q < XS; ++q) {
-      mbar_init(xready + q, NGW / NG);
+      mbar_init(xready + q, NGW / NG + (OWN_TMA ? 1 : 0));
       mbar_init(xempty + q, NCW);
     }
     fence_mbar_init();
@@ -258,7 +313,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
   if (tid == RTB_CONSUMERS)  // the first ring stages: operator blobs and setup vectors only
     for (int it = 0; it < npre; ++it)
-      tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, full + it, pol);
+      tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, pre + it, pol, 1);
   // gather warps: descriptor and column indices of their first tile
   constexpr int GS = RTB_GATHERERS / NG;  // threads of a group
   constexpr int CL = GS / NB2;            // column lanes of a group
@@ -268,20 +323,23 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   const int sub = g & (NB2 - 1), cl = g / NB2;
   const bool is_gather = tid >= RTB_CONSUMERS + 32;
   GTileB gc, gn;
-  int src[GU], cag[GU];  // level index of this thread's columns (own rows, then halo), their coarse indices
+  int src[GU], cag[GU];  // level index of this thread's columns, their coarse indices
   gc.load(a, t_begin, my, is_gather ? gg : my);
   gn.load(a, t_begin, my, is_gather ? gg + NG : my);
+  // the columns the gather warps fill: the halo columns; for the prolongation-fused sweep the own rows too
   auto load_indices = [&](const GTileB& t, int (&si)[GU], int (&ci)[GU]) {
 #pragma unroll
     for (int u = 0; u < GU; ++u) {
       const int c = cl + u * CL;
       si[u] = -1, ci[u] = 0;
-      if (c < t.nr) {
+      if (OWN_TMA) {
+        if (c < t.nhalo) si[u] = __ldg(a.halo_idx + t.hoff + c);
+      } else if (c < t.nr) {
         si[u] = t.r0 + c;
-        if (OP == OP_JACOBI_PROLONG) ci[u] = __ldg(a.agg + t.r0 + c);
+        ci[u] = __ldg(a.agg + t.r0 + c);
       } else if (c < t.nr + t.nhalo) {
         si[u] = __ldg(a.halo_idx + t.hoff + c - t.nr);
-        if (OP == OP_JACOBI_PROLONG) ci[u] = __ldg(a.halo_cagg + t.hoff + c - t.nr);
+        ci[u] = __ldg(a.halo_cagg + t.hoff + c - t.nr);
       }
     }
   };
@@ -289,24 +347,26 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   pdl_wait();
   if (a.ctl != nullptr && a.ctl->all_done) {
     if (tid == RTB_CONSUMERS)  // the copies in flight target this CTA's shared memory: let them land
-      for (int it = 0; it < npre; ++it) mbar_wait(full + it, 0);
+      for (int it = 0; it < npre; ++it) mbar_wait(pre + it, 0);
     return;
   }
   double dots[NB];
 #pragma unroll
   for (int j = 0; j < NB; ++j) dots[j] = 0.0;
+  const int rot = ((tid & 31) >> 1) & (NB2 - 1);  // chunk rotation of a consumer lane
   const double2* x2g = reinterpret_cast<const double2*>(a.x);
   const double2* e2g = reinterpret_cast<const double2*>(a.ec);
 
   if (is_gather) {
-    // ---------------- gather warps: x slots [plane h][column], up to XS tiles ahead ----------------
+    // ---------------- gather warps: x slots [column][NB], up to XS tiles ahead ----------------
     for (int it = gg; it < my; it += NG) {
       const int q = it % XS;
       GTileB gnn;
       gnn.load(a, t_begin, my, it + 2 * NG);
       int srcn[GU], cagn[GU];
       load_indices(gn, srcn, cagn);  // the next tile's indices travel while this tile is gathered
-      const int ncol = gc.nr + gc.nhalo, ncolp = tpb_ncolp(gc.nr, gc.nhalo);
+      const int c0 = OWN_TMA ? gc.nr : 0;                         // first column of the slot the gather warps write
+      const int ng = OWN_TMA ? gc.nhalo : gc.nr + gc.nhalo;       // how many they write
       double2 v[GU];
 #pragma unroll
       for (int u = 0; u < GU; ++u) {
@@ -320,25 +380,37 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         }
       }
       if (it >= XS) mbar_wait(xempty + q, (uint32_t)(((it / XS) - 1) & 1));
-      double2* xc = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes) + (size_t)sub * ncolp;
+      double2* xs = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes);
+      if (OWN_TMA && g == 0) {  // the tile's own rows: contiguous in global memory, one bulk copy
+        if (gc.nr > 0) {
+          const uint32_t bytes = 8u * NB * (uint32_t)gc.nr;
+          mbar_arrive_expect_tx(xready + q, bytes);
+          bulk_g2s<false>(xs, a.x + (size_t)gc.r0 * NB, bytes, xready + q, 0);
+        } else {
+          mbar_arrive(xready + q);
+        }
+      }
+      double2* xc = xs + (size_t)c0 * NB2 + sub;
 #pragma unroll
       for (int u = 0; u < GU; ++u)
-        if (src[u] >= 0) xc[cl + u * CL] = v[u];
-      for (int c = cl + GU * CL; c < ncol; c += CL) {  // more columns than the index registers hold
+        if (src[u] >= 0) xc[(size_t)(cl + u * CL) * NB2] = v[u];
+      for (int c = cl + GU * CL; c < ng; c += CL) {  // more columns than the index registers hold
         int s_, c_ = 0;
-        if (c < gc.nr) {
+        if (OWN_TMA) {
+          s_ = __ldg(a.halo_idx + gc.hoff + c);
+        } else if (c < gc.nr) {
           s_ = gc.r0 + c;
-          if (OP == OP_JACOBI_PROLONG) c_ = __ldg(a.agg + s_);
+          c_ = __ldg(a.agg + s_);
         } else {
           s_ = __ldg(a.halo_idx + gc.hoff + c - gc.nr);
-          if (OP == OP_JACOBI_PROLONG) c_ = __ldg(a.halo_cagg + gc.hoff + c - gc.nr);
+          c_ = __ldg(a.halo_cagg + gc.hoff + c - gc.nr);
         }
         double2 w = __ldg(x2g + (size_t)s_ * NB2 + sub);
         if (OP == OP_JACOBI_PROLONG) {
           const double2 e = __ldg(e2g + (size_t)c_ * NB2 + sub);
           w.x += a.gamma * e.x, w.y += a.gamma * e.y;
         }
-        xc[c] = w;
+        xc[(size_t)c * NB2] = w;
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(xready + q);
@@ -348,23 +420,43 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
     }
   } else if (tid >= RTB_CONSUMERS) {
     // ---------------- producer warp ----------------
-    if (tid == RTB_CONSUMERS)
+    if (tid == RTB_CONSUMERS && my > 0) {
+      for (int it = 0; it < npre; ++it)  // their setup data is already on the way: the rows of b
+        tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, full + it, pol, 2);
       for (int it = npre; it < my; ++it) {
         const int s = it % S;
         const TileDesc d = a.tiles[RT_TILE(t_begin, it)];
-        mbar_wait(empty + s, (uint32_t)(((it / S) - 1) & 1));
-        tile_issue_b<OP, STREAM>(a, d, stage0 + (size_t)s * a.stage_bytes, full + s, pol);
+        unsigned char* stage = stage0 + (size_t)s * a.stage_bytes;
+        mbar_wait(empty + s, (uint32_t)(((it / S) - 1) & 1));  // every consumer warp is done with tile it - S
+        if (STORE) {
+          tile_store_b(a, stage);
+          bulk_commit();
+          bulk_wait_read_all();  // the store has read the row buffer: the stage may be overwritten
+        }
+        tile_issue_b<OP, STREAM>(a, d, stage, full + s, pol, 0);
       }
+      if (STORE) {
+        for (int it = my > S ? my - S : 0; it < my; ++it) {  // the tiles still in the ring
+          const int s = it % S;
+          mbar_wait(empty + s, (uint32_t)((it / S) & 1));
+          tile_store_b(a, stage0 + (size_t)s * a.stage_bytes);
+          bulk_commit();
+        }
+        bulk_wait_all();
+      }
+    }
   } else {
     // ---------------- consumers ----------------
     const int lane = tid & 31, w = tid >> 5;
-    const double2* b2g = reinterpret_cast<const double2*>(a.b);
-    double2* o2g = reinterpret_cast<double2*>(a.out);
+    int o4[NB2];
+#pragma unroll
+    for (int h = 0; h < NB2; ++h) o4[h] = h ^ rot;
     int sbase = 0;  // slices of the tiles so far: the round-robin deal continues across tiles
     for (int it = 0; it < my; ++it) {
       const int s = it % S, q = it % XS;
       const uint32_t par = (uint32_t)((it / S) & 1);
       unsigned char* stage = stage0 + (size_t)s * a.stage_bytes;
+      if (it < S) mbar_wait(pre + s, 0);
       mbar_wait(full + s, par);                                // the bulk copies have landed ...
       mbar_wait(xready + q, (uint32_t)((it / XS) & 1));        // ... and the tile's x slot is assembled
       const StageDescB* sd = reinterpret_cast<const StageDescB*>(stage);
@@ -377,21 +469,13 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
         const bool v32 = sd->vb == 4;
-        const int ncolp = tpb_ncolp(nr, sd->nhalo);
-        const double2* xc = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes);
+        const double2* xc = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes);  // [column][NB2]
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
-        double2* outs = reinterpret_cast<double2*>(base + sd->o_out);  // [row][NB2]: residuals of the tile
+        double2* rowb = reinterpret_cast<double2*>(base + sd->o_row);  // [row][NB2]: b in, result out
         for (int j = (w - sbase) & (NCW - 1); j < nsl; j += NCW) {
           const int2 sl = slices[j];
           const int lr = perm[j * 32 + lane];
           const bool valid = lr != 0xFFFF;
-          double2 bv[NB2];
-#pragma unroll
-          for (int h = 0; h < NB2; ++h) bv[h] = make_double2(0.0, 0.0);
-          if (OP != OP_SPMV && valid) {  // 64 contiguous bytes of b, consumed after the row walk
-#pragma unroll
-            for (int h = 0; h < NB2; ++h) bv[h] = __ldg(b2g + (size_t)(r0 + lr) * NB2 + h);
-          }
           const unsigned short* cp = scol + sl.x;
           const double* vp = sval + sl.x;
           const float* vp32 = sval32 + sl.x;
@@ -401,34 +485,39 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
 #pragma unroll 2
           for (int k = 0; k < sl.y; ++k) {
             const double av = v32 ? (double)vp32[k * 32] : vp[k * 32];
-            const double2* xp = xc + cp[k * 32];
+            const double2* xp = xc + (size_t)cp[k * 32] * NB2;
 #pragma unroll
             for (int h = 0; h < NB2; ++h) {
-              const double2 xv = xp[(size_t)h * ncolp];
+              const double2 xv = xp[o4[h]];
               acc[2 * h] += av * xv.x;
               acc[2 * h + 1] += av * xv.y;
             }
           }
           if (valid) {
+            double2* rb = rowb + (size_t)lr * NB2;
+            const double2* xo = xc + (size_t)lr * NB2;  // the row's own x (its column of the slot)
             if (OP == OP_RESTRICT) {
 #pragma unroll
-              for (int h = 0; h < NB2; ++h)
-                outs[lr * NB2 + h] = make_double2(bv[h].x - acc[2 * h], bv[h].y - acc[2 * h + 1]);
+              for (int h = 0; h < NB2; ++h) {
+                const double2 bv = rb[o4[h]];
+                rb[o4[h]] = make_double2(bv.x - acc[2 * h], bv.y - acc[2 * h + 1]);
+              }
             } else {
               const double di = (OP == OP_SPMV) ? 0.0 : ds[lr];
 #pragma unroll
               for (int h = 0; h < NB2; ++h) {
                 double2 o;
-                const double2 xo = xc[(size_t)h * ncolp + lr];  // the row's own x (SpMV: for the dot)
+                const double2 xv = xo[o4[h]];
                 if (OP == OP_SPMV) {
                   o = make_double2(acc[2 * h], acc[2 * h + 1]);
-                  if (NDOT) dots[2 * h] += xo.x * o.x, dots[2 * h + 1] += xo.y * o.y;
+                  if (NDOT) dots[2 * h] += xv.x * o.x, dots[2 * h + 1] += xv.y * o.y;
                 } else {
-                  o.x = xo.x + di * (bv[h].x - acc[2 * h]);
-                  o.y = xo.y + di * (bv[h].y - acc[2 * h + 1]);
-                  if (NDOT) dots[2 * h] += bv[h].x * o.x, dots[2 * h + 1] += bv[h].y * o.y;
+                  const double2 bv = rb[o4[h]];
+                  o.x = xv.x + di * (bv.x - acc[2 * h]);
+                  o.y = xv.y + di * (bv.y - acc[2 * h + 1]);
+                  if (NDOT) dots[2 * h] += bv.x * o.x, dots[2 * h + 1] += bv.y * o.y;
                 }
-                o2g[(size_t)(r0 + lr) * NB2 + h] = o;
+                rb[o4[h]] = o;
               }
             }
           }
@@ -441,12 +530,13 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           const int nA = sd->nA, I0 = sd->I0;
           const int* aps = reinterpret_cast<const int*>(base + sd->o_agg) + sd->aoff;      // aps[al] = agg_ptr[I0 + al]
           const double* dcs = reinterpret_cast<const double*>(base + sd->o_dc) - sd->eoff;  // dcs[I] = dinv_c[I]
+          double2* o2g = reinterpret_cast<double2*>(a.out);
           double2* o22g = reinterpret_cast<double2*>(a.out2);
           for (int t = tid; t < nA * NB2; t += RTB_CONSUMERS) {
             const int al = t / NB2, h = t % NB2;
             double2 sum = make_double2(0.0, 0.0);
             for (int lr = aps[al] - r0, le = aps[al + 1] - r0; lr < le; ++lr) {
-              const double2 rv = outs[lr * NB2 + h];
+              const double2 rv = rowb[lr * NB2 + h];
               sum.x += rv.x, sum.y += rv.y;
             }
             o2g[(size_t)(I0 + al) * NB2 + h] = sum;
@@ -458,8 +548,9 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         }
       }
       sbase = (sbase + nsl) & (NCW - 1);
-      // ---- this warp is done with the stage and the x slot ----
-      if (OP == OP_RESTRICT) fence_proxy_async();  // residuals were written into a region the next bulk copy overwrites
+      // ---- this warp is done with the stage and the x slot: its writes to the row buffer become visible to
+      // the async proxy (the bulk store reads them, the next bulk copy overwrites them) ----
+      fence_proxy_async();
       __syncwarp();
       if (lane == 0) {
         mbar_arrive(empty + s);
@@ -467,7 +558,18 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
       }
     }
   }
-  if (NDOT > 0) grid_reduce_finalize_b<RTB_THREADS>(dots, a.partials, a.counter, a.ctl, a.fin);
+  if (NDOT > 0) {
+    // a consumer lane's accumulator pair h holds the right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1
+    double dt[NB];
+#pragma unroll
+    for (int hh = 0; hh < NB2; ++hh) {
+      dt[2 * hh] = dt[2 * hh + 1] = 0.0;
+#pragma unroll
+      for (int h = 0; h < NB2; ++h)
+        if ((h ^ rot) == hh) dt[2 * hh] = dots[2 * h], dt[2 * hh + 1] = dots[2 * h + 1];
+    }
+    grid_reduce_finalize_b<RTB_THREADS>(dt, a.partials, a.counter, a.ctl, a.fin);
+  }
 }
 
 // ------------------------------------------------------------------------------------------
