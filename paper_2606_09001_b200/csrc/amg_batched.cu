@@ -127,7 +127,15 @@ amg_status vcycle_b(amg_handle_s* H, int l, const double* b, double** out, Krylo
   double* ec = nullptr;
   AMG_TRY(vcycle_b(H, lc, Bt.b[lc], &ec, ctl, false, st));
   const bool want_dot = fuse_rz && l == 0;
-  {
+  const int split_rows = H->opt.split_prolong_rows < RTB_SPLIT_ROWS ? H->opt.split_prolong_rows : RTB_SPLIT_ROWS;
+  if (split_rows > 0 && L.n >= split_rows) {
+    // the coarse correction as its own unit-stride pass, then a plain sweep (own rows by bulk copy, one gather
+    // per halo column): level 0 of cfg 3, 8 right-hand sides: 337 us fused against 153 + ~45 us
+    launch_b(k_prolong_add_b, red_grid_b(H, (int64_t)L.n * NB2), RED_THREADS, 0, st, L.n, (const int*)L.agg,
+             (const double*)ec, H->opt.coarse_scale, cur, (const KrylovCtlB*)ctl);
+    op_jacobi_b(H, l, b, cur, oth, want_dot && nu2 == 1, ctl, st, nu1);
+    std::swap(cur, oth);
+  } else {
     RowArgsB a = args_b(ctl);
     a.x = cur, a.b = b, a.ec = ec, a.out = oth, a.fin = FIN_RZ, a.dinv = L.dsw[nu1];
     if (want_dot && nu2 == 1)

@@ -21,13 +21,14 @@
 
 constexpr int NB = 8;        // right-hand sides per batch
 constexpr int NB2 = NB / 2;  // double2 per row
-constexpr int RTB_CONSUMERS = 256;
-constexpr int RTB_GATHERERS = 448;  // 14 warps in RTB_GGROUPS groups
+constexpr int RTB_CONSUMERS = 512;  // 16 warps walk the slices (a row walk is a chain of dependent shared-memory reads)
+constexpr int RTB_GATHERERS = 256;  // 8 warps in RTB_GGROUPS groups: they fetch the halo columns only
 constexpr int RTB_GGROUPS = 2;
 constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
 constexpr int RTB_GU = 12;          // columns per gather thread whose indices are held in registers
 constexpr int RTB_MAXS = 4;         // most ring stages / x slots
 constexpr int RTB_HEADER = 256;
+constexpr int RTB_SPLIT_ROWS = 32768;  // levels with at least this many rows apply the coarse correction as its own pass
 constexpr int RTB_SMEM_MAX = 224 * 1024;  // dynamic part: the reductions keep ~2 KB of static shared memory
 
 struct KrylovCtlB {
@@ -145,6 +146,64 @@ __device__ __forceinline__ void grid_reduce_finalize_b(double (&v)[NB], double* 
   if (!is_last) return;
   __threadfence();
 #pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    double s = 0.0;
+    for (unsigned q = tid; q < gridDim.x; q += THREADS) s += __ldcg(partials + (size_t)j * gridDim.x + q);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) sh[j][w] = s;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double tot[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      double s = 0.0;
+#pragma unroll
+      for (int q = 0; q < THREADS / 32; ++q) s += sh[j][q];
+      tot[j] = s;
+    }
+    *counter = 0;
+    krylov_finalize_b(ctl, fin, tot);
+  }
+}
+
+// The same reduction for a kernel in which only NW warps hold values (the consumer warps of the row-tile kernel):
+// they leave their warp totals in `sh` inside their own branch (cta_partial_b), so that the NB accumulators are
+// live in that branch only; every thread of the CTA then calls grid_finalize_b.
+template <int NW>
+__device__ __forceinline__ void cta_partial_b(const double (&v)[NB], double (*sh)[NW], int w, int lane) {
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    double s = v[j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) sh[j][w] = s;
+  }
+}
+template <int THREADS, int NW>
+__device__ __forceinline__ void grid_finalize_b(double (*shw)[NW], double* partials, unsigned* counter, KrylovCtlB* ctl,
+                                                int fin) {
+  __shared__ double sh[NB][THREADS / 32];
+  __shared__ bool is_last;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  __syncthreads();
+  if (tid < NB) {
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < NW; ++q) s += shw[tid][q];
+    partials[(size_t)tid * gridDim.x + blockIdx.x] = s;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    unsigned t = atomicAdd(counter, 1u);
+    is_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+#pragma unroll 1
   for (int j = 0; j < NB; ++j) {
     double s = 0.0;
     for (unsigned q = tid; q < gridDim.x; q += THREADS) s += __ldcg(partials + (size_t)j * gridDim.x + q);
@@ -350,17 +409,14 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
       for (int it = 0; it < npre; ++it) mbar_wait(pre + it, 0);
     return;
   }
-  double dots[NB];
-#pragma unroll
-  for (int j = 0; j < NB; ++j) dots[j] = 0.0;
-  const int rot = ((tid & 31) >> 1) & (NB2 - 1);  // chunk rotation of a consumer lane
+  __shared__ double shdot[NB][RTB_CONSUMERS / 32];  // warp totals of the fused dot products (consumer warps)
   const double2* x2g = reinterpret_cast<const double2*>(a.x);
   const double2* e2g = reinterpret_cast<const double2*>(a.ec);
 
   if (is_gather) {
     // ---------------- gather warps: x slots [column][NB], up to XS tiles ahead ----------------
+    int q = gg % XS, xk = gg / XS;  // slot and use count of the slot for tile `it` (no division in the loop)
     for (int it = gg; it < my; it += NG) {
-      const int q = it % XS;
       GTileB gnn;
       gnn.load(a, t_begin, my, it + 2 * NG);
       int srcn[GU], cagn[GU];
@@ -379,7 +435,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           }
         }
       }
-      if (it >= XS) mbar_wait(xempty + q, (uint32_t)(((it / XS) - 1) & 1));
+      if (xk > 0) mbar_wait(xempty + q, (uint32_t)((xk - 1) & 1));
       double2* xs = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes);
       if (OWN_TMA && g == 0) {  // the tile's own rows: contiguous in global memory, one bulk copy
         if (gc.nr > 0) {
@@ -417,30 +473,36 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
       gc = gn, gn = gnn;
 #pragma unroll
       for (int u = 0; u < GU; ++u) src[u] = srcn[u], cag[u] = cagn[u];
+      q += NG;
+      while (q >= XS) q -= XS, ++xk;
     }
   } else if (tid >= RTB_CONSUMERS) {
     // ---------------- producer warp ----------------
     if (tid == RTB_CONSUMERS && my > 0) {
       for (int it = 0; it < npre; ++it)  // their setup data is already on the way: the rows of b
         tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, full + it, pol, 2);
+      int s = 0, sk = 1;  // stage and use count of the stage for tile `it` (it = npre = S here if the loop runs)
       for (int it = npre; it < my; ++it) {
-        const int s = it % S;
         const TileDesc d = a.tiles[RT_TILE(t_begin, it)];
         unsigned char* stage = stage0 + (size_t)s * a.stage_bytes;
-        mbar_wait(empty + s, (uint32_t)(((it / S) - 1) & 1));  // every consumer warp is done with tile it - S
+        mbar_wait(empty + s, (uint32_t)((sk - 1) & 1));  // every consumer warp is done with tile it - S
         if (STORE) {
           tile_store_b(a, stage);
           bulk_commit();
           bulk_wait_read_all();  // the store has read the row buffer: the stage may be overwritten
         }
         tile_issue_b<OP, STREAM>(a, d, stage, full + s, pol, 0);
+        if (++s == S) s = 0, ++sk;
       }
       if (STORE) {
-        for (int it = my > S ? my - S : 0; it < my; ++it) {  // the tiles still in the ring
-          const int s = it % S;
-          mbar_wait(empty + s, (uint32_t)((it / S) & 1));
-          tile_store_b(a, stage0 + (size_t)s * a.stage_bytes);
+        // the tiles still in the ring: tile `it` is use number it / S of stage it % S
+        int it = my > S ? my - S : 0;
+        int s2 = it % S, k2 = it / S;
+        for (; it < my; ++it) {
+          mbar_wait(empty + s2, (uint32_t)(k2 & 1));
+          tile_store_b(a, stage0 + (size_t)s2 * a.stage_bytes);
           bulk_commit();
+          if (++s2 == S) s2 = 0, ++k2;
         }
         bulk_wait_all();
       }
@@ -448,17 +510,22 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   } else {
     // ---------------- consumers ----------------
     const int lane = tid & 31, w = tid >> 5;
+    const int rot = (lane >> 1) & (NB2 - 1);  // chunk rotation of this lane
     int o4[NB2];
 #pragma unroll
     for (int h = 0; h < NB2; ++h) o4[h] = h ^ rot;
+    constexpr int ND = NDOT > 0 ? NB : 1;
+    double dots[ND];
+#pragma unroll
+    for (int j = 0; j < ND; ++j) dots[j] = 0.0;
     int sbase = 0;  // slices of the tiles so far: the round-robin deal continues across tiles
+    int s = 0, q = 0;
+    uint32_t par = 0, xpar = 0;  // phase parities of the stage / the x slot of tile `it`
     for (int it = 0; it < my; ++it) {
-      const int s = it % S, q = it % XS;
-      const uint32_t par = (uint32_t)((it / S) & 1);
       unsigned char* stage = stage0 + (size_t)s * a.stage_bytes;
       if (it < S) mbar_wait(pre + s, 0);
-      mbar_wait(full + s, par);                                // the bulk copies have landed ...
-      mbar_wait(xready + q, (uint32_t)((it / XS) & 1));        // ... and the tile's x slot is assembled
+      mbar_wait(full + s, par);           // the bulk copies have landed ...
+      mbar_wait(xready + q, xpar);        // ... and the tile's x slot is assembled
       const StageDescB* sd = reinterpret_cast<const StageDescB*>(stage);
       const int nr = sd->nr, nsl = sd->nsl, r0 = sd->r0;
       if (nr > 0) {
@@ -510,12 +577,12 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
                 const double2 xv = xo[o4[h]];
                 if (OP == OP_SPMV) {
                   o = make_double2(acc[2 * h], acc[2 * h + 1]);
-                  if (NDOT) dots[2 * h] += xv.x * o.x, dots[2 * h + 1] += xv.y * o.y;
+                  if (NDOT) dots[(2 * h) % ND] += xv.x * o.x, dots[(2 * h + 1) % ND] += xv.y * o.y;
                 } else {
                   const double2 bv = rb[o4[h]];
                   o.x = xv.x + di * (bv.x - acc[2 * h]);
                   o.y = xv.y + di * (bv.y - acc[2 * h + 1]);
-                  if (NDOT) dots[2 * h] += bv.x * o.x, dots[2 * h + 1] += bv.y * o.y;
+                  if (NDOT) dots[(2 * h) % ND] += bv.x * o.x, dots[(2 * h + 1) % ND] += bv.y * o.y;
                 }
                 rb[o4[h]] = o;
               }
@@ -556,20 +623,23 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         mbar_arrive(empty + s);
         mbar_arrive(xempty + q);
       }
+      if (++s == S) s = 0, par ^= 1u;
+      if (++q == XS) q = 0, xpar ^= 1u;
+    }
+    if (NDOT > 0) {
+      // this lane's accumulator pair h holds the right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1
+      double dt[NB];
+#pragma unroll
+      for (int hh = 0; hh < NB2; ++hh) {
+        dt[2 * hh] = dt[2 * hh + 1] = 0.0;
+#pragma unroll
+        for (int h = 0; h < NB2; ++h)
+          if ((h ^ rot) == hh) dt[2 * hh] = dots[(2 * h) % ND], dt[2 * hh + 1] = dots[(2 * h + 1) % ND];
+      }
+      cta_partial_b<RTB_CONSUMERS / 32>(dt, shdot, w, lane);
     }
   }
-  if (NDOT > 0) {
-    // a consumer lane's accumulator pair h holds the right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1
-    double dt[NB];
-#pragma unroll
-    for (int hh = 0; hh < NB2; ++hh) {
-      dt[2 * hh] = dt[2 * hh + 1] = 0.0;
-#pragma unroll
-      for (int h = 0; h < NB2; ++h)
-        if ((h ^ rot) == hh) dt[2 * hh] = dots[2 * h], dt[2 * hh + 1] = dots[2 * h + 1];
-    }
-    grid_reduce_finalize_b<RTB_THREADS>(dt, a.partials, a.counter, a.ctl, a.fin);
-  }
+  if (NDOT > 0) grid_finalize_b<RTB_THREADS, RTB_CONSUMERS / 32>(shdot, a.partials, a.counter, a.ctl, a.fin);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -667,6 +737,25 @@ static __global__ void __launch_bounds__(RED_THREADS) k_pcg_p_b(int n, const dou
     pv.x = b0 != 0.0 ? zv.x + b0 * pv.x : zv.x;
     pv.y = b1 != 0.0 ? zv.y + b1 * pv.y : zv.y;
     p2[t] = pv;
+  }
+}
+
+// x[i][s] += gamma ec[agg[i]][s]: the coarse correction as its own unit-stride pass (large levels: the
+// prolongation-fused sweep needs two gathers per column and assembles the own rows in the gather warps)
+static __global__ void __launch_bounds__(RED_THREADS) k_prolong_add_b(int n, const int* __restrict__ agg,
+                                                               const double* __restrict__ ec, double gamma,
+                                                               double* __restrict__ x, const KrylovCtlB* ctl) {
+  pdl_sync();
+  if (ctl != nullptr && ctl->all_done) return;
+  const int64_t m = (int64_t)n * NB2, stride = (int64_t)gridDim.x * RED_THREADS;
+  const double2* e2 = reinterpret_cast<const double2*>(ec);
+  double2* x2 = reinterpret_cast<double2*>(x);
+  for (int64_t t = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; t < m; t += stride) {
+    const int i = (int)(t / NB2), h = (int)(t % NB2);
+    const double2 e = __ldg(e2 + (size_t)__ldg(agg + i) * NB2 + h);
+    double2 v = x2[t];
+    v.x += gamma * e.x, v.y += gamma * e.y;
+    x2[t] = v;
   }
 }
 
