@@ -127,23 +127,13 @@ amg_status vcycle_b(amg_handle_s* H, int l, const double* b, double** out, Krylo
   double* ec = nullptr;
   AMG_TRY(vcycle_b(H, lc, Bt.b[lc], &ec, ctl, false, st));
   const bool want_dot = fuse_rz && l == 0;
-  const int split_rows = H->opt.split_prolong_rows < RTB_SPLIT_ROWS ? H->opt.split_prolong_rows : RTB_SPLIT_ROWS;
-  if (split_rows > 0 && L.n >= split_rows) {
-    // the coarse correction as its own unit-stride pass, then a plain sweep (own rows by bulk copy, one gather
-    // per halo column): level 0 of cfg 3, 8 right-hand sides: 337 us fused against 153 + ~45 us
-    launch_b(k_prolong_add_b, red_grid_b(H, (int64_t)L.n * NB2), RED_THREADS, 0, st, L.n, (const int*)L.agg,
-             (const double*)ec, H->opt.coarse_scale, cur, (const KrylovCtlB*)ctl);
-    op_jacobi_b(H, l, b, cur, oth, want_dot && nu2 == 1, ctl, st, nu1);
-    std::swap(cur, oth);
-  } else {
-    RowArgsB a = args_b(ctl);
-    a.x = cur, a.b = b, a.ec = ec, a.out = oth, a.fin = FIN_RZ, a.dinv = L.dsw[nu1];
-    if (want_dot && nu2 == 1)
-      launch_rowtile_b<OP_JACOBI_PROLONG, 1>(H, L, Bt.geom[l], a, st);
-    else
-      launch_rowtile_b<OP_JACOBI_PROLONG, 0>(H, L, Bt.geom[l], a, st);
-    std::swap(cur, oth);
-  }
+  // the coarse correction x += gamma P e_c is its own unit-stride pass, then a plain sweep: the fused variant
+  // needs two gathers per column and keeps the own rows off the bulk copies (level 0 of cfg 3, 8 right-hand
+  // sides: 337 us fused against 143 + 45 us)
+  launch_b(k_prolong_add_b, red_grid_b(H, (int64_t)L.n * NB2), RED_THREADS, 0, st, L.n, (const int*)L.agg,
+           (const double*)ec, H->opt.coarse_scale, cur, (const KrylovCtlB*)ctl);
+  op_jacobi_b(H, l, b, cur, oth, want_dot && nu2 == 1, ctl, st, nu1);
+  std::swap(cur, oth);
   for (int s = 1; s < nu2; ++s) {
     op_jacobi_b(H, l, b, cur, oth, want_dot && s == nu2 - 1, ctl, st, nu1 + s);
     std::swap(cur, oth);
@@ -321,7 +311,6 @@ int amg_batch_prepare(amg_handle_s* H, cudaStream_t st) {
   for (auto& e : B.ev)
     if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return 0;
   set_attr_b<OP_SPMV, 1>(), set_attr_b<OP_JACOBI, 0>(), set_attr_b<OP_JACOBI, 1>(), set_attr_b<OP_RESTRICT, 0>();
-  set_attr_b<OP_JACOBI_PROLONG, 0>(), set_attr_b<OP_JACOBI_PROLONG, 1>();
   cudaGetLastError();
   B.eligible = 1;
   return 1;

@@ -28,7 +28,6 @@ constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
 constexpr int RTB_GU = 12;          // columns per gather thread whose indices are held in registers
 constexpr int RTB_MAXS = 4;         // most ring stages / x slots
 constexpr int RTB_HEADER = 256;
-constexpr int RTB_SPLIT_ROWS = 32768;  // levels with at least this many rows apply the coarse correction as its own pass
 constexpr int RTB_SMEM_MAX = 224 * 1024;  // dynamic part: the reductions keep ~2 KB of static shared memory
 
 struct KrylovCtlB {
@@ -68,7 +67,7 @@ struct StageLayoutB {
   int ra2, nrv;  // dinv slice (even start / count)
   int Ia4, nap;  // agg_ptr slice
   int Ia2, nec;  // dinv_c slice
-  int o_d, o_agg, o_dc, o_row, end;
+  int o_d, o_agg, o_dc, o_row, o_xown, end;
 };
 enum { TPB_D = 1, TPB_RESTRICT = 2 };
 __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) {
@@ -90,6 +89,8 @@ __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) 
   if (flags & TPB_RESTRICT) o += 8 * t.nec;
   t.o_row = o;
   o += 8 * NB * d.nr;
+  t.o_xown = o;  // the tile's own rows of x, [nr][NB]
+  o += 8 * NB * d.nr;
   t.end = o;
   return t;
 }
@@ -97,8 +98,8 @@ __host__ __device__ inline int tpb_stage_need(const TileDesc& d) {
   const int a = tpb_stage(d, TPB_D).end, b = tpb_stage(d, TPB_RESTRICT).end;
   return TP_DESC_BYTES + (a > b ? a : b);
 }
-// x slot: [column][NB] (own rows first, then the halo columns), 64 bytes per column
-__host__ __device__ inline int tpb_xslot_need(const TileDesc& d) { return 8 * NB * (d.nr + d.nhalo); }
+// x slot: the tile's halo columns, [nhalo][NB], 64 bytes per column (the own rows travel with the stage)
+__host__ __device__ inline int tpb_xslot_need(const TileDesc& d) { return 8 * NB * (d.nhalo > 0 ? d.nhalo : 1); }
 
 // ---- per-column finalisation of a reduction; a finished column is frozen ----
 __device__ inline void krylov_finalize_b(KrylovCtlB* cb, int fin, const double* s0) {
@@ -251,7 +252,8 @@ struct StageDescB {  // TP_DESC_BYTES at the start of a stage, written by the pr
   int o_perm, o_col, o_val, o_d;
   int o_agg, o_row, o_dc, eoff;  // eoff = Ia2 (dcs[I - eoff] = dinv_c[I])
   int vb;                        // bytes per stored value (8, or 4 with the mixed-precision hierarchy)
-  int pad[15];
+  int o_xown;
+  int pad[14];
 };
 static_assert(sizeof(StageDescB) == TP_DESC_BYTES, "stage header size");
 
@@ -265,11 +267,11 @@ __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bu
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 // mode 0: header + every copy, all on `bar`;  mode 1: header + the setup data (blob, dinv, agg_ptr,
-// dinv_c), on `bar` (issued before the grid dependency);  mode 2: the tile's rows of b only, on `bar`
+// dinv_c), on `bar` (issued before the grid dependency);  mode 2: the tile's rows of b and x only, on `bar`
 template <int OP, bool STREAM>
 __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& d, unsigned char* stage, uint64_t* bar,
                                              uint64_t pol, int mode) {
-  constexpr bool SWEEP = (OP == OP_JACOBI || OP == OP_JACOBI_PROLONG);
+  constexpr bool SWEEP = (OP == OP_JACOBI);
   constexpr bool RES = (OP == OP_RESTRICT);
   constexpr bool HASB = (OP != OP_SPMV);
   const bool dc = RES && a.dinv_c != nullptr;
@@ -281,7 +283,7 @@ __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& 
     sd.nsl = d.nsl, sd.nhalo = d.nhalo, sd.roff = d.r0 - t.ra2, sd.aoff = d.I0 - t.Ia4;
     sd.o_perm = p.o_perm, sd.o_col = p.o_col, sd.o_val = p.o_val, sd.o_d = t.o_d;
     sd.o_agg = t.o_agg, sd.o_row = t.o_row, sd.o_dc = t.o_dc, sd.eoff = t.Ia2;
-    sd.vb = d.vb;
+    sd.vb = d.vb, sd.o_xown = t.o_xown;
     int4* dst = reinterpret_cast<int4*>(stage);
     const int4* src = reinterpret_cast<const int4*>(&sd);
 #pragma unroll
@@ -300,11 +302,7 @@ __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& 
     if (RES) bytes += 4u * (uint32_t)t.nap;
     if (dc) bytes += 8u * (uint32_t)t.nec;
   }
-  if (mode != 1 && HASB) bytes += rowbytes;
-  if (bytes == 0) {  // mode 2 of an operation without b
-    mbar_arrive(bar);
-    return;
-  }
+  if (mode != 1) bytes += (HASB ? 2u : 1u) * rowbytes;
   mbar_arrive_expect_tx(bar, bytes);
   if (mode != 2) {
     bulk_g2s<STREAM>(base, a.blob + (size_t)d.blob16 * 16u, (uint32_t)p.end, bar, pol);
@@ -312,7 +310,10 @@ __device__ __forceinline__ void tile_issue_b(const RowArgsB& a, const TileDesc& 
     if (RES) bulk_g2s<false>(base + t.o_agg, a.agg_ptr + t.Ia4, 4u * (uint32_t)t.nap, bar, pol);
     if (dc) bulk_g2s<false>(base + t.o_dc, a.dinv_c + t.Ia2, 8u * (uint32_t)t.nec, bar, pol);
   }
-  if (mode != 1 && HASB) bulk_g2s<false>(base + t.o_row, a.b + (size_t)d.r0 * NB, rowbytes, bar, pol);
+  if (mode != 1) {
+    if (HASB) bulk_g2s<false>(base + t.o_row, a.b + (size_t)d.r0 * NB, rowbytes, bar, pol);
+    bulk_g2s<false>(base + t.o_xown, a.x + (size_t)d.r0 * NB, rowbytes, bar, pol);
+  }
 }
 
 // the finished rows of the tile in `stage` leave by one bulk store (producer thread)
@@ -343,7 +344,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   uint64_t* xready = pre + RTB_MAXS;
   uint64_t* xempty = xready + RTB_MAXS;
   static_assert(6 * RTB_MAXS * 8 <= RTB_HEADER, "barrier header");
-  constexpr bool OWN_TMA = (OP != OP_JACOBI_PROLONG);  // the tile's own rows of x arrive by a bulk copy
+  static_assert(OP == OP_SPMV || OP == OP_JACOBI || OP == OP_RESTRICT, "operations of the batched kernel");
   constexpr bool STORE = (OP != OP_RESTRICT);          // the tile's rows of the result leave by a bulk store
   const int S = a.stages, XS = a.xslots;
   unsigned char* stage0 = smem + RTB_HEADER;
@@ -362,7 +363,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
       mbar_init(pre + s, 1);
     }
     for (int q = 0; q < XS; ++q) {
-      mbar_init(xready + q, NGW / NG + (OWN_TMA ? 1 : 0));
+      mbar_init(xready + q, NGW / NG);
       mbar_init(xempty + q, NCW);
     }
     fence_mbar_init();
@@ -373,7 +374,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   if (tid == RTB_CONSUMERS)  // the first ring stages: operator blobs and setup vectors only
     for (int it = 0; it < npre; ++it)
       tile_issue_b<OP, STREAM>(a, a.tiles[RT_TILE(t_begin, it)], stage0 + (size_t)it * a.stage_bytes, pre + it, pol, 1);
-  // gather warps: descriptor and column indices of their first tile
+  // gather warps: descriptor and halo column indices of their first tile
   constexpr int GS = RTB_GATHERERS / NG;  // threads of a group
   constexpr int CL = GS / NB2;            // column lanes of a group
   constexpr int GU = RTB_GU;
@@ -382,27 +383,17 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   const int sub = g & (NB2 - 1), cl = g / NB2;
   const bool is_gather = tid >= RTB_CONSUMERS + 32;
   GTileB gc, gn;
-  int src[GU], cag[GU];  // level index of this thread's columns, their coarse indices
+  int src[GU];  // level index of this thread's halo columns
   gc.load(a, t_begin, my, is_gather ? gg : my);
   gn.load(a, t_begin, my, is_gather ? gg + NG : my);
-  // the columns the gather warps fill: the halo columns; for the prolongation-fused sweep the own rows too
-  auto load_indices = [&](const GTileB& t, int (&si)[GU], int (&ci)[GU]) {
+  auto load_indices = [&](const GTileB& t, int (&si)[GU]) {
 #pragma unroll
     for (int u = 0; u < GU; ++u) {
       const int c = cl + u * CL;
-      si[u] = -1, ci[u] = 0;
-      if (OWN_TMA) {
-        if (c < t.nhalo) si[u] = __ldg(a.halo_idx + t.hoff + c);
-      } else if (c < t.nr) {
-        si[u] = t.r0 + c;
-        ci[u] = __ldg(a.agg + t.r0 + c);
-      } else if (c < t.nr + t.nhalo) {
-        si[u] = __ldg(a.halo_idx + t.hoff + c - t.nr);
-        ci[u] = __ldg(a.halo_cagg + t.hoff + c - t.nr);
-      }
+      si[u] = c < t.nhalo ? __ldg(a.halo_idx + t.hoff + c) : -1;
     }
   };
-  if (is_gather) load_indices(gc, src, cag);
+  if (is_gather) load_indices(gc, src);
   pdl_wait();
   if (a.ctl != nullptr && a.ctl->all_done) {
     if (tid == RTB_CONSUMERS)  // the copies in flight target this CTA's shared memory: let them land
@@ -411,68 +402,34 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
   }
   __shared__ double shdot[NB][RTB_CONSUMERS / 32];  // warp totals of the fused dot products (consumer warps)
   const double2* x2g = reinterpret_cast<const double2*>(a.x);
-  const double2* e2g = reinterpret_cast<const double2*>(a.ec);
 
   if (is_gather) {
-    // ---------------- gather warps: x slots [column][NB], up to XS tiles ahead ----------------
+    // ---------------- gather warps: x slots [halo column][NB], up to XS tiles ahead ----------------
+    // every load of a tile is issued before the slot is waited for: a slot is busy for a store burst only
     int q = gg % XS, xk = gg / XS;  // slot and use count of the slot for tile `it` (no division in the loop)
     for (int it = gg; it < my; it += NG) {
       GTileB gnn;
       gnn.load(a, t_begin, my, it + 2 * NG);
-      int srcn[GU], cagn[GU];
-      load_indices(gn, srcn, cagn);  // the next tile's indices travel while this tile is gathered
-      const int c0 = OWN_TMA ? gc.nr : 0;                         // first column of the slot the gather warps write
-      const int ng = OWN_TMA ? gc.nhalo : gc.nr + gc.nhalo;       // how many they write
+      int srcn[GU];
+      load_indices(gn, srcn);  // the next tile's indices travel while this tile is gathered
       double2 v[GU];
 #pragma unroll
       for (int u = 0; u < GU; ++u) {
         v[u] = make_double2(0.0, 0.0);
-        if (src[u] >= 0) {
-          v[u] = __ldg(x2g + (size_t)src[u] * NB2 + sub);
-          if (OP == OP_JACOBI_PROLONG) {
-            const double2 e = __ldg(e2g + (size_t)cag[u] * NB2 + sub);
-            v[u].x += a.gamma * e.x, v[u].y += a.gamma * e.y;
-          }
-        }
+        if (src[u] >= 0) v[u] = __ldg(x2g + (size_t)src[u] * NB2 + sub);
       }
       if (xk > 0) mbar_wait(xempty + q, (uint32_t)((xk - 1) & 1));
-      double2* xs = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes);
-      if (OWN_TMA && g == 0) {  // the tile's own rows: contiguous in global memory, one bulk copy
-        if (gc.nr > 0) {
-          const uint32_t bytes = 8u * NB * (uint32_t)gc.nr;
-          mbar_arrive_expect_tx(xready + q, bytes);
-          bulk_g2s<false>(xs, a.x + (size_t)gc.r0 * NB, bytes, xready + q, 0);
-        } else {
-          mbar_arrive(xready + q);
-        }
-      }
-      double2* xc = xs + (size_t)c0 * NB2 + sub;
+      double2* xc = reinterpret_cast<double2*>(xslot0 + (size_t)q * a.xslot_bytes) + sub;
 #pragma unroll
       for (int u = 0; u < GU; ++u)
         if (src[u] >= 0) xc[(size_t)(cl + u * CL) * NB2] = v[u];
-      for (int c = cl + GU * CL; c < ng; c += CL) {  // more columns than the index registers hold
-        int s_, c_ = 0;
-        if (OWN_TMA) {
-          s_ = __ldg(a.halo_idx + gc.hoff + c);
-        } else if (c < gc.nr) {
-          s_ = gc.r0 + c;
-          c_ = __ldg(a.agg + s_);
-        } else {
-          s_ = __ldg(a.halo_idx + gc.hoff + c - gc.nr);
-          c_ = __ldg(a.halo_cagg + gc.hoff + c - gc.nr);
-        }
-        double2 w = __ldg(x2g + (size_t)s_ * NB2 + sub);
-        if (OP == OP_JACOBI_PROLONG) {
-          const double2 e = __ldg(e2g + (size_t)c_ * NB2 + sub);
-          w.x += a.gamma * e.x, w.y += a.gamma * e.y;
-        }
-        xc[(size_t)c * NB2] = w;
-      }
+      for (int c = cl + GU * CL; c < gc.nhalo; c += CL)  // more halo columns than the index registers hold
+        xc[(size_t)c * NB2] = __ldg(x2g + (size_t)__ldg(a.halo_idx + gc.hoff + c) * NB2 + sub);
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(xready + q);
       gc = gn, gn = gnn;
 #pragma unroll
-      for (int u = 0; u < GU; ++u) src[u] = srcn[u], cag[u] = cagn[u];
+      for (int u = 0; u < GU; ++u) src[u] = srcn[u];
       q += NG;
       while (q >= XS) q -= XS, ++xk;
     }
@@ -536,7 +493,9 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
         const bool v32 = sd->vb == 4;
-        const double2* xc = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes);  // [column][NB2]
+        // tile-local column c: c < nr -> own row c (stage), else halo column c - nr (x slot); both [..][NB2]
+        const double2* xown = reinterpret_cast<const double2*>(base + sd->o_xown);
+        const double2* xhal = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes) - (size_t)nr * NB2;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
         double2* rowb = reinterpret_cast<double2*>(base + sd->o_row);  // [row][NB2]: b in, result out
         for (int j = (w - sbase) & (NCW - 1); j < nsl; j += NCW) {
@@ -552,7 +511,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
 #pragma unroll 2
           for (int k = 0; k < sl.y; ++k) {
             const double av = v32 ? (double)vp32[k * 32] : vp[k * 32];
-            const double2* xp = xc + (size_t)cp[k * 32] * NB2;
+            const int c = cp[k * 32];
+            const double2* xp = (c < nr ? xown : xhal) + (size_t)c * NB2;
 #pragma unroll
             for (int h = 0; h < NB2; ++h) {
               const double2 xv = xp[o4[h]];
@@ -562,7 +522,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           }
           if (valid) {
             double2* rb = rowb + (size_t)lr * NB2;
-            const double2* xo = xc + (size_t)lr * NB2;  // the row's own x (its column of the slot)
+            const double2* xo = xown + (size_t)lr * NB2;  // the row's own x
             if (OP == OP_RESTRICT) {
 #pragma unroll
               for (int h = 0; h < NB2; ++h) {
