@@ -21,7 +21,8 @@
 
 constexpr int NB = 8;        // right-hand sides per batch
 constexpr int NB2 = NB / 2;  // double2 per row
-constexpr int RTB_CONSUMERS = 512;  // 16 warps walk the slices (a row walk is a chain of dependent shared-memory reads)
+constexpr int RTB_CONSUMERS = 384;  // 12 warps walk the slices (672 threads per CTA leave 96 registers per thread: no spills;
+                                    // measured on cfg 3 / cfg 4, 8 right-hand sides: 8 warps 33.8 / 155.6 ms, 12: 32.7 / 150.4, 16: 35.3 / 161.1)
 constexpr int RTB_GATHERERS = 256;  // 8 warps in RTB_GGROUPS groups: they fetch the halo columns only
 constexpr int RTB_GGROUPS = 2;
 constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
@@ -498,7 +499,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const double2* xhal = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes) - (size_t)nr * NB2;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
         double2* rowb = reinterpret_cast<double2*>(base + sd->o_row);  // [row][NB2]: b in, result out
-        for (int j = (w - sbase) & (NCW - 1); j < nsl; j += NCW) {
+        for (int j = (w >= sbase ? w - sbase : w - sbase + NCW); j < nsl; j += NCW) {
           const int2 sl = slices[j];
           const int lr = perm[j * 32 + lane];
           const bool valid = lr != 0xFFFF;
@@ -574,7 +575,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           }
         }
       }
-      sbase = (sbase + nsl) & (NCW - 1);
+      sbase = (sbase + nsl) % NCW;
       // ---- this warp is done with the stage and the x slot: its writes to the row buffer become visible to
       // the async proxy (the bulk store reads them, the next bulk copy overwrites them) ----
       fence_proxy_async();
