@@ -215,6 +215,24 @@ AMG_API amg_status amg_solve_host(amg_handle h, const double* h_b, double* h_x, 
 AMG_API amg_status amg_grad_values(amg_handle h, const double* d_lambda, const double* d_x, int32_t nrhs,
                            int64_t ld, double* d_gA, int32_t accumulate, void* cuda_stream);
 
+/* G2 without any allocation and without a handle (for callers under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same result as amg_grad_values (Eq. 2),
+ *   gA[k] (+)= - sum_{s < nrhs} lambda_s[i] * x_s[col[k]]  for rowptr[i] <= k < rowptr[i+1],
+ * on the pattern the CALLER passes: d_rowptr int32[n + 1], d_col int32[nnz], d_gA f64[nnz], d_lambda / d_x
+ * f64 with column s at s * ld (ld >= n); all DEVICE pointers owned by the caller, on the current device.
+ * The interleaved copy of X that the batched kernel gathers from lives in a file-scope static device array of
+ * AMG_NOALLOC_MAX_DOUBLES values (8 MiB; every GPU that loads the library holds it until the process exits).
+ * Limits: n * nrhs <= AMG_NOALLOC_MAX_DOUBLES and nrhs <= 94, else AMG_ERR_UNSUPPORTED with a message in
+ * amg_last_error(NULL); null pointers / ld < n: AMG_ERR_INVALID_ARG.  The call enqueues two kernels on
+ * cuda_stream and returns; it calls no cudaMalloc, cudaFree or allocating library routine and does not
+ * synchronise.  Every call on a device shares the one array, which keeps the previous call's contents (each
+ * call overwrites what it reads, nothing needs clearing): calls that OVERLAP on the GPU -- different streams, or
+ * several host threads on one device -- race on it; order them on one stream or with events. */
+#define AMG_NOALLOC_MAX_DOUBLES (1 << 20)
+AMG_API amg_status amg_grad_values_noalloc(int64_t n, int64_t nnz, const int32_t* d_rowptr, const int32_t* d_col,
+                                           const double* d_lambda, const double* d_x, int32_t nrhs, int64_t ld,
+                                           double* d_gA, int32_t accumulate, void* cuda_stream);
+
 /* z = B r: one V-cycle from a zero guess (the preconditioner; also the V-cycle timing hook). */
 AMG_API amg_status amg_apply_preconditioner(amg_handle h, const double* d_r, double* d_z,
                                     void* cuda_stream);

@@ -23,7 +23,7 @@ AMG_CONVERGED, AMG_MAXIT, AMG_BREAKDOWN, AMG_NONFINITE = 0, 1, 2, 3
 
 EXPORTS = ["amg_options_default", "amg_set_allocator", "amg_setup", "amg_setup_with_aggregates", "amg_resetup_values",
            "amg_destroy", "amg_solve", "amg_solve_ex", "amg_solve_transpose", "amg_solve_batched",
-           "amg_solve_host", "amg_grad_values", "amg_apply_preconditioner", "amg_get_num_levels",
+           "amg_solve_host", "amg_grad_values", "amg_grad_values_noalloc", "amg_apply_preconditioner", "amg_get_num_levels",
            "amg_get_level_info", "amg_get_aggregates", "amg_get_level_csr", "amg_get_setup_stats",
            "amg_get_level_path", "amg_get_symmetric", "amg_get_residual_history", "amg_write_report", "amg_get_algorithmic_bytes", "amg_get_last_launches", "amg_level_op", "amg_last_error",
            "amg_cache_create", "amg_cache_get", "amg_cache_stats", "amg_cache_destroy"]
@@ -189,6 +189,14 @@ def amg_grad_values(h, d_lambda, d_x, nrhs, ld, d_gA, accumulate):
     _check(load_library().amg_grad_values(h, _ptr(d_lambda, torch.float64), _ptr(d_x, torch.float64),
                                           C.c_int32(nrhs), C.c_int64(ld), _ptr(d_gA, torch.float64),
                                           C.c_int32(accumulate), _stream()), h)
+
+
+def amg_grad_values_noalloc(n, nnz, d_rowptr, d_col, d_lambda, d_x, nrhs, ld, d_gA, accumulate):
+    """Handle-free, allocation-free G2 (static device scratch: n * nrhs <= AMG_NOALLOC_MAX_DOUBLES)."""
+    _check(load_library().amg_grad_values_noalloc(C.c_int64(n), C.c_int64(nnz), _ptr(d_rowptr, torch.int32),
+                                                  _ptr(d_col, torch.int32), _ptr(d_lambda, torch.float64),
+                                                  _ptr(d_x, torch.float64), C.c_int32(nrhs), C.c_int64(ld),
+                                                  _ptr(d_gA, torch.float64), C.c_int32(accumulate), _stream()))
 
 
 def amg_apply_preconditioner(h, d_r, d_z):
