@@ -88,8 +88,11 @@ __host__ __device__ inline StageLayoutB tpb_stage(const TileDesc& d, int flags) 
   if (flags & TPB_RESTRICT) o += 4 * t.nap;
   t.o_dc = o;
   if (flags & TPB_RESTRICT) o += 8 * t.nec;
+  // both 128-byte aligned (stages and x slots are): the class of a column the packer orders a row's entries by
+  // (amg_setup.cu, k_pack_tiles) is then the half of the 128-byte bank line its 64 bytes occupy
+  o = tp_up(o, 128);
   t.o_row = o;
-  o += 8 * NB * d.nr;
+  o += tp_up(8 * NB * d.nr, 128);
   t.o_xown = o;  // the tile's own rows of x, [nr][NB]
   o += 8 * NB * d.nr;
   t.end = o;

@@ -867,8 +867,35 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);  // vb == 4: mixed-precision hierarchy
-  // one thread per row (sorted position s = slice j, lane): its entries k = 0 .. w_j - 1, zero-padded past the row's
-  // length; the loads of a row are independent of one another, the stores of a warp for a fixed k are contiguous
+  // tile-local column of every entry of the tile, one thread per entry (ext[] is free again: reused as u16[])
+  unsigned short* c16s = reinterpret_cast<unsigned short*>(ext);
+  __syncthreads();
+  for (int e = tid; e < k1 - k0; e += PK_THREADS) {
+    const int c = col[k0 + e];
+    unsigned short c16;
+    if (c >= r0 && c < r1) {
+      c16 = (unsigned short)(c - r0);
+    } else {
+      int lo = 0, hi = d.nhalo;  // first entry >= c
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (halo[mid] < c) lo = mid + 1;
+        else hi = mid;
+      }
+      c16 = (unsigned short)(nr + lo);
+    }
+    c16s[e] = c16;
+  }
+  __syncthreads();
+  // One thread per row (sorted position s = slice j, lane): its entries in slots k = 0 .. w_j - 1, zero-padded past
+  // the row's length; the stores of a warp for a fixed k are contiguous.
+  // ORDER of a row's entries (any order is a valid row sum; this one is fixed by the pattern alone): the batched
+  // kernel reads, per entry, the 64 bytes [8 right-hand sides] of the entry's column from shared memory, 16 lanes at
+  // a time; the columns of a tile sit 64 bytes apart from a 128-byte aligned base (own rows: stage; halo columns:
+  // x slot), so a column's CLASS = parity of its position there decides which half of the 128-byte bank line it
+  // occupies.  Lane `lane` wants class (lane ^ k) & 1 at step k: then every 16-byte bank group is read by exactly 2
+  // of the 16 lanes (the minimum).  Each row serves the wanted class from its remaining entries in ascending CSR
+  // position, and falls back to the other class when that one is exhausted.
   for (int s = tid; s < nsl * 32; s += PK_THREADS) {
     const int j = s >> 5, lane = s & 31;
     const int off = sl_off[j] + lane, w = sl_w[j];
@@ -878,23 +905,26 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
       ln = len[lr];
       kk0 = rowptr[r0 + lr];
     }
+    const unsigned short* rc = c16s + (kk0 - k0);
+    auto cls = [&](int q) {
+      const int c = rc[q];
+      return (c < nr ? c : c - nr) & 1;
+    };
+    int cur[2] = {0, 0};  // next unserved entry of class 0 / 1
+    while (cur[0] < ln && cls(cur[0]) != 0) ++cur[0];
+    while (cur[1] < ln && cls(cur[1]) != 1) ++cur[1];
     for (int k = 0; k < w; ++k) {
       unsigned short c16 = 0;
       double v = 0.0;
       if (k < ln) {
-        const int c = col[kk0 + k];
-        v = val[kk0 + k];
-        if (c >= r0 && c < r1) {
-          c16 = (unsigned short)(c - r0);
-        } else {
-          int lo = 0, hi = d.nhalo;  // first entry >= c
-          while (lo < hi) {
-            const int mid = (lo + hi) >> 1;
-            if (halo[mid] < c) lo = mid + 1;
-            else hi = mid;
-          }
-          c16 = (unsigned short)(nr + lo);
-        }
+        int t = (lane ^ k) & 1;
+        if (cur[t] >= ln) t ^= 1;
+        const int q = cur[t];
+        c16 = rc[q];
+        v = val[kk0 + q];
+        int nx = q + 1;
+        while (nx < ln && cls(nx) != t) ++nx;
+        cur[t] = nx;
       }
       o_col[off + k * 32] = c16;
       if (vb == 4)
@@ -1687,8 +1717,11 @@ __global__ void k_rap_numeric(int m, const int* __restrict__ cptr, const int* __
 
 // value section of every tile blob from the level's CSR values (the slices / perm sections say where)
 __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc* __restrict__ tiles,
-                                                     const int* __restrict__ rowptr, const double* __restrict__ val,
+                                                     const int* __restrict__ rowptr, const int* __restrict__ col,
+                                                     const double* __restrict__ val, const int* __restrict__ halo_idx,
                                                      unsigned char* __restrict__ blob) {
+  // the column section of the blob says which entry every slot holds (whatever order the packer chose): slot ->
+  // tile-local column -> level column -> position in the CSR row (ascending unique columns: binary search)
   const int t = blockIdx.x;
   if (t >= ntiles) return;
   const TileDesc d = tiles[t];
@@ -1697,6 +1730,7 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
   const BlobLayout p = tp_blob(d.nsl, d.nslots, d.vb);
   const int2* slices = reinterpret_cast<const int2*>(base);
   const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + p.o_perm);
+  const unsigned short* o_col = reinterpret_cast<const unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);
   for (int j = 0; j < d.nsl; ++j) {
@@ -1707,8 +1741,18 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
       double v = 0.0;
       if (lr != 0xFFFF) {
         const int r = d.r0 + lr;
-        const int s = rowptr[r];
-        if (k < rowptr[r + 1] - s) v = val[s + k];
+        const int s = rowptr[r], e = rowptr[r + 1];
+        if (k < e - s) {
+          const int c16 = o_col[sl.x + q];
+          const int c = c16 < d.nr ? d.r0 + c16 : halo_idx[d.halo_off + c16 - d.nr];
+          int lo = s, hi = e;  // first entry >= c
+          while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (col[mid] < c) lo = mid + 1;
+            else hi = mid;
+          }
+          v = val[lo];
+        }
       }
       if (d.vb == 4)
         o_val32[sl.x + q] = (float)v;
@@ -1836,12 +1880,12 @@ amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fa
   for (int l = 0; l <= Lc; ++l) {
     Level& L = H->lv[l];
     if (l < Lc) k_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, o.smoother, o.omega, L.dinv);
-    if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.val, L.blob);
-    if (L.K.fast) k_blob_refill<<<L.K.nblk, 256, 0, st>>>(L.K.nblk, L.K.tiles, L.rowptr, L.val, L.K.blob);
+    if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.col, L.val, L.halo_idx, L.blob);
+    if (L.K.fast) k_blob_refill<<<L.K.nblk, 256, 0, st>>>(L.K.nblk, L.K.tiles, L.rowptr, L.col, L.val, L.K.halo_idx, L.K.blob);
     if (H->have_T) {
       k_gather_vals<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, L.val, L.T.src, L.T.val);
-      if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.val, L.T.blob);
-      if (L.KT.fast) k_blob_refill<<<L.KT.nblk, 256, 0, st>>>(L.KT.nblk, L.KT.tiles, L.T.rowptr, L.T.val, L.KT.blob);
+      if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.col, L.T.val, L.T.halo_idx, L.T.blob);
+      if (L.KT.fast) k_blob_refill<<<L.KT.nblk, 256, 0, st>>>(L.KT.nblk, L.KT.tiles, L.T.rowptr, L.T.col, L.T.val, L.KT.halo_idx, L.KT.blob);
     }
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
