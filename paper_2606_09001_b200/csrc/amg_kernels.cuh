@@ -1187,6 +1187,51 @@ static __global__ void __launch_bounds__(256) k_grad_values_rows(int n, const in
   }
 }
 
+// Single right-hand side, any row length: ONE lane per stored ENTRY.  A warp owns 32 consecutive rows, i.e. one
+// contiguous run of entries; lane l keeps rowptr[i0 + l] and lambda[i0 + l], the row of an entry is found by a
+// 5-step binary search over the lanes' row pointers (shuffles), its lambda by one more shuffle: col and gA are read
+// and written fully coalesced, the only gather is x[col[k]], with 4 independent entries per lane in flight.
+static __global__ void __launch_bounds__(256) k_grad_values_entries(int n, const int* __restrict__ rowptr,
+                                                                    const int* __restrict__ col,
+                                                                    const double* __restrict__ lam,
+                                                                    const double* __restrict__ x,
+                                                                    double* __restrict__ gA, int accumulate) {
+  const int lane = threadIdx.x & 31;
+  const int i0 = (blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32;
+  if (i0 >= n) return;  // whole warp
+  const int il = min(i0 + lane, n - 1);
+  const int rp = __ldg(rowptr + il);  // non-decreasing over the lanes (rows past n repeat the last row: never found)
+  const double li = __ldg(lam + il);
+  const int kb = __shfl_sync(0xffffffffu, rp, 0), ke = __ldg(rowptr + min(i0 + 32, n));
+  constexpr int U = 4;
+  for (int k = kb; k < ke; k += 32 * U) {
+    int c[U], r[U];
+    double xv[U], old[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int e = k + u * 32 + lane;
+      c[u] = e < ke ? __ldg(col + e) : -1;
+      int lo = 0;  // largest lane with rp <= e
+#pragma unroll
+      for (int st = 16; st > 0; st >>= 1) {
+        const int v = __shfl_sync(0xffffffffu, rp, (lo + st) & 31);
+        if (lo + st < 32 && v <= e) lo += st;
+      }
+      r[u] = lo;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      xv[u] = c[u] >= 0 ? __ldg(x + c[u]) : 0.0;
+      old[u] = (accumulate && c[u] >= 0) ? gA[k + u * 32 + lane] : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const double l = __shfl_sync(0xffffffffu, li, r[u]);
+      if (c[u] >= 0) gA[k + u * 32 + lane] = old[u] - l * xv[u];
+    }
+  }
+}
+
 // Batched G2 (nrhs > 1).  With the right-hand sides stored one after the other, the gather
 // x_s[col[k]] touches a different 32-byte sector for every s: 16 sectors per stored entry on the
 // permuted systems (cfg 5: 14 ms, 170 GB/s).  X is therefore first interleaved to XT[j][s] (one
@@ -1245,3 +1290,50 @@ static __global__ void __launch_bounds__(256) k_grad_values_batched(int n, const
   }
 }
 
+// Batched G2, NR = 8 or 16 right-hand sides, cooperative gather: G = NR / 2 lanes share one stored entry, lane j
+// holds lambda of the right-hand sides 2j, 2j + 1 of its row and reads the 16 bytes [2j, 2j + 1] of XT[col[k]]:
+// one entry is ONE coalesced 64- / 128-byte request (the lane-per-entry kernel above issues NR / 2 separate
+// 16-byte loads of that line per lane: 8 x the tag lookups, which is what bounds it on randomly permuted
+// systems); the products are summed over the G lanes by shuffles.  All loads of up to 8 entries of a row are
+// issued before any is used.
+template <int NR>
+static __global__ void __launch_bounds__(256, 4) k_grad_values_coop(int n, const int* __restrict__ rowptr,
+                                                                 const int* __restrict__ col,
+                                                                 const double* __restrict__ lam, int64_t ld,
+                                                                 const double* __restrict__ XT,
+                                                                 double* __restrict__ gA, int accumulate) {
+  constexpr int G = NR / 2;
+  const int64_t gt = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t iw = gt / G;
+  const int j = (int)(gt % G);
+  const bool live = iw < n;
+  const int i = live ? (int)iw : n - 1;
+  const double l0 = __ldg(lam + (size_t)(2 * j) * ld + i), l1 = __ldg(lam + (size_t)(2 * j + 1) * ld + i);
+  const int k0 = __ldg(rowptr + i), k1 = live ? __ldg(rowptr + i + 1) : k0;
+  const double2* X2 = reinterpret_cast<const double2*>(XT);
+  // the trip count is made uniform over the warp (the shuffles need every lane)
+  int len = k1 - k0;
+#pragma unroll
+  for (int o = 16; o >= G; o >>= 1) len = max(len, __shfl_xor_sync(0xffffffffu, len, o));
+  constexpr int U = 8;
+  for (int kk = 0; kk < len; kk += U) {
+    int c[U];
+    double2 v[U];
+    double old[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) c[u] = k0 + kk + u < k1 ? __ldg(col + k0 + kk + u) : -1;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      v[u] = c[u] >= 0 ? __ldg(X2 + (size_t)c[u] * G + j) : make_double2(0.0, 0.0);
+      old[u] = (accumulate && j == 0 && c[u] >= 0) ? gA[k0 + kk + u] : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      double acc = l0 * v[u].x;
+      acc += l1 * v[u].y;
+#pragma unroll
+      for (int o = G / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if (j == 0 && c[u] >= 0) gA[k0 + kk + u] = old[u] - acc;
+    }
+  }
+}

@@ -888,8 +888,12 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
     switch (nrhs) {
       case 2: AMG_GRAD_CASE(2) break;
       case 4: AMG_GRAD_CASE(4) break;
-      case 8: AMG_GRAD_CASE(8) break;
-      case 16: AMG_GRAD_CASE(16) break;
+      case 8:  // nrhs / 2 lanes per stored entry: one coalesced request per entry
+        ++g_nlaunch, launch(k_grad_values_coop<8>, div_up((int64_t)n * 4, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, ld, XT, d_gA, accumulate);
+        break;
+      case 16:
+        ++g_nlaunch, launch(k_grad_values_coop<16>, div_up((int64_t)n * 8, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, ld, XT, d_gA, accumulate);
+        break;
       default: AMG_GRAD_CASE(0) break;
     }
 #undef AMG_GRAD_CASE
@@ -897,7 +901,9 @@ amg_status amg_grad_values_impl(amg_handle_s* H, const double* d_lambda, const d
     H->last_launches = 2;
     return AMG_OK;
   }
-  if (mean <= 12.0 && nrhs == 1) {
+  if (nrhs == 1 && H->opt.force_generic == 0) {
+    ++g_nlaunch, launch(k_grad_values_entries, div_up(n, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, d_gA, accumulate);
+  } else if (mean <= 12.0 && nrhs == 1) {
     ++g_nlaunch, launch(k_grad_values_rows, div_up(n, 256), 256, 0, st)(n, H->nat_rowptr, H->nat_col, d_lambda, d_x, d_gA, accumulate);
   } else if (mean <= 12.0) {
     const int64_t threads = (int64_t)n * 8;
