@@ -313,6 +313,43 @@ def test_grad_values_batched_kernel(cases, B, name, nrhs, generic):
     assert np.max(np.abs(gA.cpu().numpy() - 2 * want)) <= 1e-14 * scale * nrhs * 2
 
 
+@pytest.mark.parametrize("n", [1, 31, 33, 1000, 4099])
+def test_grad_values_ragged_sizes_and_row_lengths(oracle_mod, B, n):
+    """The gradient kernels on patterns whose row count is not a multiple of 32 (the entry-parallel kernel deals 32
+    rows to a warp) and whose rows have very different lengths (1 .. ~200 entries: one warp's run of entries spans
+    several trips; the cooperative kernel's trip count is the longest row of the warp), against the oracle's
+    definition of Eq. 2, for 1, 8 and 16 right-hand sides, overwrite and accumulate."""
+    import scipy.sparse as sp
+
+    rng = np.random.default_rng(700 + n)
+    deg = np.minimum(n - 1, rng.choice([0, 1, 2, 5, 9, 40, 200], size=n, p=[0.1, 0.2, 0.2, 0.2, 0.2, 0.07, 0.03]))
+    rows = np.repeat(np.arange(n), deg)
+    cols = rng.integers(0, n, rows.size)
+    W = sp.coo_matrix((rng.uniform(0.1, 1.0, rows.size), (rows, cols)), shape=(n, n)).tocsr()
+    W = W + W.T
+    W.setdiag(0)
+    W.eliminate_zeros()
+    A = (sp.diags(np.asarray(W.sum(axis=1)).ravel() + 1.0) - W).tocsr()  # symmetric, strictly diagonally dominant
+    A.sort_indices()
+    rowptr, col, val = A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(np.float64)
+    o = oracle_mod.Oracle(rowptr, col, val)
+    s = B.AmgSolver(rowptr, col, val, device="cuda:0")
+    nnz = int(rowptr[-1])
+    for nrhs in (1, 8, 16):
+        lam = rng.standard_normal((nrhs, n))
+        x = rng.standard_normal((nrhs, n))
+        want = o.grad_values(lam, x)
+        scale = max(np.max(np.abs(want)), 1e-300)
+        gA = torch.full((nnz,), float("nan"), dtype=torch.float64, device="cuda")
+        d_lam, d_x = torch.as_tensor(lam).cuda().contiguous(), torch.as_tensor(x).cuda().contiguous()
+        B.amg_grad_values(s.h, d_lam, d_x, nrhs, n, gA, 0)
+        assert np.max(np.abs(gA.cpu().numpy() - want)) <= 1e-14 * scale * nrhs
+        B.amg_grad_values(s.h, d_lam, d_x, nrhs, n, gA, 1)
+        assert np.max(np.abs(gA.cpu().numpy() - 2 * want)) <= 1e-14 * scale * nrhs * 2
+    s.close()
+    o.close()
+
+
 # ------------------------------------------------------------------------------------------
 # options, imported aggregates, edge cases
 # ------------------------------------------------------------------------------------------
