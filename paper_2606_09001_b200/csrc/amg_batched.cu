@@ -62,10 +62,10 @@ void set_attr_b() {
 template <int OP, int NDOT>
 void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowArgsB& a, cudaStream_t st,
                       const LevelOpT* K = nullptr) {
-  a.n = L.n, a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob, a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
-  if (K) a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx, a.halo_cagg = K->halo_cagg;
+  a.n = L.n, a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob, a.halo_idx = L.halo_idx;
+  if (K) a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx;
   if (!a.dinv) a.dinv = L.dinv;  // (the sweeps pass the diagonal of their own sweep index: Chebyshev weights)
-  a.agg = L.agg, a.agg_ptr = L.agg_ptr, a.gamma = H->opt.coarse_scale;
+  a.agg_ptr = L.agg_ptr;
   a.partials = H->batch->partials, a.counter = H->batch->counter;
   a.stages = G.stages, a.xslots = G.xslots, a.stage_bytes = G.stage_bytes, a.xslot_bytes = G.xslot_bytes;
   int grid = H->sm_count;  // one CTA per SM

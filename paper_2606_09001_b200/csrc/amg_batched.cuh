@@ -4,18 +4,18 @@
 // riding on one stream the per-RHS traffic drops to M/8 + vectors.
 //
 // Vectors are interleaved [row][NB] (64 contiguous bytes per row), so that the gather of a halo column
-// fetches all 8 right-hand sides as two full 32-byte sectors, and a row's operands / results are one
-// 64-byte access.  The row-tile kernel is the single-RHS one (amg_kernels.cuh) with
+// fetches all 8 right-hand sides as two full 32-byte sectors, and a tile's rows of any vector are ONE
+// contiguous range.  The row-tile kernel is the single-RHS one (amg_kernels.cuh) with
 //   - the same tile blobs (one bulk-async copy per tile), nothing else of the operator;
-//   - x slots [NB/2 planes][columns] of double2: the consumer's per-entry reads are NB/2 LDS.128;
-//   - 8 accumulators per row in registers; b rows are read straight from global memory before the
-//     row walk (64 B per lane, latency hidden behind the walk), results written straight to global;
-//   - one CTA per SM (the x slots are 8 x larger), 14 gather warps in two groups;
+//   - the tile's rows of b and x brought into the stage, and its rows of the result taken out of it, by
+//     bulk-async copies / one bulk-async store; x slots [halo column][NB] for the halo only;
+//   - 8 accumulators per row in registers, NB/2 LDS.128 per stored entry;
+//   - one CTA per SM, 12 consumer warps, 8 gather warps in two groups;
 //   - per-column Krylov scalars and convergence flags (KrylovCtlB): a converged column keeps riding
 //     with alpha = beta = 0 (its x, r stay as they are) until every column is done.
-// The fused operations with two gathers per column are split in batched mode where that is simpler:
-// the first sweep from zero (x1 = dinv o r) is emitted by the kernel that produces r (level 0) or by
-// the restriction above (other levels), as in the single-RHS path.
+// The operations with two gathers per column are split: the first sweep from zero (x1 = dinv o r) is
+// emitted by the kernel that produces r (level 0) or by the restriction above (other levels), as in the
+// single-RHS path, and the coarse correction is its own pass (k_prolong_add_b).
 #pragma once
 #include "amg_kernels.cuh"
 
@@ -42,17 +42,13 @@ struct RowArgsB {
   int ntiles;
   const unsigned char* blob;
   const int* halo_idx;
-  const int* halo_cagg;
   const double* x;       // gathered vector, [n][NB]
   const double* b;
   const double* dinv;    // [n]
   double* out;
   const double* dinv_c;  // restriction, optional: smoother diagonal of the coarse level ...
   double* out2;          // ... then out2[I][s] = dinv_c[I] * out[I][s]
-  const int* agg;
   const int* agg_ptr;
-  const double* ec;      // [nc][NB]
-  double gamma;
   double* partials;      // [NB][gridDim.x]
   unsigned* counter;
   KrylovCtlB* ctl;       // may be null (hooks)
@@ -232,23 +228,25 @@ __device__ __forceinline__ void grid_finalize_b(double (*shw)[NW], double* parti
 }
 
 // ------------------------------------------------------------------------------------------
-// Batched row-tile kernel.  OP: OP_SPMV (dot: x.out per column), OP_JACOBI (dot: b.out),
-// OP_RESTRICT, OP_JACOBI_PROLONG (dot: b.out).
+// Batched row-tile kernel.  OP: OP_SPMV (dot: x.out per column), OP_JACOBI (dot: b.out), OP_RESTRICT.
+// (The coarse correction x += gamma P e_c is its own pass, k_prolong_add_b: a prolongation-fused sweep needs
+// two gathers per column and keeps the own rows off the bulk copies; measured slower on every level.)
 //
 // Everything contiguous moves by bulk-async copies (TMA), not through the load/store pipe, which
 // is what bounds this kernel: the tile's blob, dinv / agg_ptr / dinv_c slices (setup data, issued
-// before the grid dependency), its rows of b (into the stage's row buffer), its OWN rows of x
-// (straight into the x slot; the gather warps fetch the halo columns only) and its rows of the
-// result (row buffer -> global, one bulk store per tile issued by the producer thread once every
-// consumer warp has released the stage).  Only the prolongation-fused sweep, whose own rows are
-// x + gamma ec[agg], assembles them in the gather warps.
+// before the grid dependency), its rows of b (into the stage's row buffer), its OWN rows of x (into
+// the stage as well; the gather warps fetch the halo columns only, into the x slot) and its rows of
+// the result (row buffer -> global, one bulk store per tile issued by the producer thread once every
+// consumer warp has released the stage).
 //
 // Shared-memory layout of the vectors is the global one, [row or column][NB] = 64 bytes each.  A
 // consumer lane reads the NB2 16-byte chunks of a column in the order h ^ rot, rot = (lane / 2) & 3:
-// its accumulator pair h belongs to right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1.  With that
-// rotation the 16 lanes of a half-warp that walk 16 consecutive rows (row buffer, own x) hit every
-// 16-byte bank group exactly twice -- the minimum for a 128-bit access -- and the random columns of
-// the entry loop spread over the bank groups as evenly as a plane layout would.
+// its accumulator pair h belongs to right-hand sides 2 (h ^ rot), 2 (h ^ rot) + 1.  The row buffers
+// and x slots start on 128-byte lines, so a column's 64 bytes are the lower or the upper half of a
+// line; the packer (amg_setup.cu, k_pack_tiles) stores a row's entries so that lane l reads a
+// lower-half column at step k when (l ^ k) is even and an upper-half one when it is odd.  With the
+// rotation every 16-byte bank group is then read by exactly 2 of the 16 lanes of a half-warp -- the
+// minimum for a 128-bit access.
 // ------------------------------------------------------------------------------------------
 struct StageDescB {  // TP_DESC_BYTES at the start of a stage, written by the producer
   int r0, nr, I0, nA;
