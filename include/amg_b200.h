@@ -121,7 +121,10 @@ typedef struct {
                                arithmetic; dinv, the coarsest LU, the Krylov operator A (level 0 keeps an fp64 copy), all
                                vectors and all sums stay fp64.  The solve still converges to rtol in fp64.  In this mode
                                the per-level hooks (amg_level_op) see the rounded operators.  default 0            */
-  int32_t reserved1;
+  int32_t value_dict;       /* 1 (default) = value dictionary: a level whose operator holds at most 255 distinct fp64 values
+                               (constant-coefficient stencils and their Galerkin sums) is stored in the tile blobs as
+                               8-bit codes into a table of those values -- 3 bytes per entry instead of 10, the values and
+                               every result bit-identical; other levels keep fp64 values.  Ignored with hierarchy_fp32 = 1 */
   double cheby_ratio;       /* smoother = 2: smoothing interval [1/cheby_ratio, 1]; default 6                    */
 } amg_options;
 

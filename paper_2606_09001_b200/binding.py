@@ -39,7 +39,7 @@ class amg_options(C.Structure):
                 ("split_prolong_rows", C.c_int32), ("use_while", C.c_int32),
                 ("omega", C.c_double),
                 ("strong_beta", C.c_double), ("coarse_scale", C.c_double), ("hash_seed", C.c_uint64),
-                ("hierarchy_fp32", C.c_int32), ("reserved1", C.c_int32), ("cheby_ratio", C.c_double)]
+                ("hierarchy_fp32", C.c_int32), ("value_dict", C.c_int32), ("cheby_ratio", C.c_double)]
 
 
 class amg_info(C.Structure):

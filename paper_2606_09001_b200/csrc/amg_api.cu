@@ -211,6 +211,7 @@ amg_status amg_options_default(amg_options* o) {
   o->coarse_scale = 1.0;
   o->hash_seed = 0;
   o->hierarchy_fp32 = 0;
+  o->value_dict = 1;
   o->cheby_ratio = 6.0;
   return AMG_OK;
 }

@@ -64,6 +64,7 @@ void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowA
                       const LevelOpT* K = nullptr) {
   a.n = L.n, a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob, a.halo_idx = L.halo_idx;
   if (K) a.tiles = K->tiles, a.ntiles = K->nblk, a.blob = K->blob, a.halo_idx = K->halo_idx;
+  a.vdict = (L.ndict > 0 && !K) ? L.vdict : nullptr;
   if (!a.dinv) a.dinv = L.dinv;  // (the sweeps pass the diagonal of their own sweep index: Chebyshev weights)
   a.agg_ptr = L.agg_ptr;
   a.partials = H->batch->partials, a.counter = H->batch->counter;

@@ -29,7 +29,7 @@ constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
 constexpr int RTB_GU = 12;          // columns per gather thread whose indices are held in registers
 constexpr int RTB_MAXS = 4;         // most ring stages / x slots
 constexpr int RTB_HEADER = 256;
-constexpr int RTB_SMEM_MAX = 224 * 1024;  // dynamic part: the reductions keep ~2 KB of static shared memory
+constexpr int RTB_SMEM_MAX = 220 * 1024;  // dynamic part: the reductions and the value dictionary keep ~4.5 KB of static shared memory
 
 struct KrylovCtlB {
   KrylovCtl c[NB];
@@ -49,6 +49,7 @@ struct RowArgsB {
   const double* dinv_c;  // restriction, optional: smoother diagonal of the coarse level ...
   double* out2;          // ... then out2[I][s] = dinv_c[I] * out[I][s]
   const int* agg_ptr;
+  const double* vdict;   // value dictionary of the level ([256]; tiles with vb = 1 hold 8-bit codes), or null
   double* partials;      // [NB][gridDim.x]
   unsigned* counter;
   KrylovCtlB* ctl;       // may be null (hooks)
@@ -370,6 +371,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
     }
     fence_mbar_init();
   }
+  __shared__ double sdict[256];  // value dictionary of the level (setup data)
+  if (a.vdict != nullptr && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
   __syncthreads();
   pdl_launch_dependents();
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
@@ -494,7 +497,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
-        const bool v32 = sd->vb == 4;
+        const unsigned char* sval8 = base + sd->o_val + lane;
+        const bool v32 = sd->vb == 4, v8 = sd->vb == 1;
         // tile-local column c: c < nr -> own row c (stage), else halo column c - nr (x slot); both [..][NB2]
         const double2* xown = reinterpret_cast<const double2*>(base + sd->o_xown);
         const double2* xhal = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes) - (size_t)nr * NB2;
@@ -507,12 +511,13 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           const unsigned short* cp = scol + sl.x;
           const double* vp = sval + sl.x;
           const float* vp32 = sval32 + sl.x;
+          const unsigned char* vp8 = sval8 + sl.x;
           double acc[NB];
 #pragma unroll
           for (int t = 0; t < NB; ++t) acc[t] = 0.0;
 #pragma unroll 2
           for (int k = 0; k < sl.y; ++k) {
-            const double av = v32 ? (double)vp32[k * 32] : vp[k * 32];
+            const double av = v8 ? sdict[vp8[k * 32]] : (v32 ? (double)vp32[k * 32] : vp[k * 32]);
             const int c = cp[k * 32];
             const double2* xp = (c < nr ? xown : xhal) + (size_t)c * NB2;
 #pragma unroll

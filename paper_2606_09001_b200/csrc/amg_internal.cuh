@@ -107,6 +107,8 @@ struct Level {
   // A_0^T (KT) for the Krylov method's own SpMV
   LevelOpT K, KT;
   int v32 = 0;              // 1: this level's V-cycle operator is the fp64 one rounded to fp32
+  double* vdict = nullptr;  // [256] value dictionary of the level (ascending distinct values, [255] = 0 for padding
+  int ndict = 0;            //   slots); ndict > 0: the tile blobs hold 8-bit codes (TileDesc::vb = 1)
   int lpr = 8;              // lanes per row of the fallback kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary

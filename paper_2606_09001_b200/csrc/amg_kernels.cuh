@@ -58,6 +58,7 @@ struct RowArgs {
   KrylovCtl* ctl;       // may be null (hooks)
   int fin;
   int v32;              // row-vector fallback: round every CSR value to fp32 on the fly (mixed-precision hierarchy)
+  const double* vdict;  // value dictionary of the level ([256]; tiles with vb = 1 hold 8-bit codes into it), or null
 };
 
 // ------------------------------------------------------------------------------------------
@@ -481,6 +482,9 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
     }
     fence_mbar_init();
   }
+  // value dictionary of the level (setup data): tiles with vb = 1 hold 8-bit codes into it
+  __shared__ double sdict[256];
+  if (a.vdict != nullptr && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
   __syncthreads();
   pdl_launch_dependents();
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
@@ -652,7 +656,8 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;  // mixed-precision hierarchy
-        const bool v32 = sd->vb == 4;
+        const unsigned char* sval8 = base + sd->o_val + lane;                            // value dictionary
+        const bool v32 = sd->vb == 4, v8 = sd->vb == 1;
         const double* xc = reinterpret_cast<const double*>(xslot0 + q * RT_XSLOT_BYTES);
         const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
@@ -661,7 +666,11 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
           const int2 sl = slices[j];
           const unsigned short* cp = scol + sl.x;
           double sum = 0.0;
-          if (v32) {  // values stored in fp32 (exactly representable), arithmetic in fp64
+          if (v8) {  // 8-bit codes into the level's table of distinct fp64 values: the same values, bit for bit
+            const unsigned char* vp = sval8 + sl.x;
+#pragma unroll 4
+            for (int k = 0; k < sl.y; ++k) sum += sdict[vp[k * 32]] * xc[cp[k * 32]];
+          } else if (v32) {  // values stored in fp32 (exactly representable), arithmetic in fp64
             const float* vp = sval32 + sl.x;
 #pragma unroll 4
             for (int k = 0; k < sl.y; ++k) sum += (double)vp[k * 32] * xc[cp[k * 32]];

@@ -702,6 +702,68 @@ __global__ void k_blk_partition(int nblk, int target, int nnz_w, int nunits, con
 // columns; pass 2 (after a scan of the blob sizes) repeats that and writes the blob.
 // info[0] = largest stage footprint (bytes), info[1] = a tile exceeds the packer's scratch
 // ------------------------------------------------------------------------------------------
+// ------------------------------------------------------------------------------------------
+// Value dictionary of a level (amg_options::value_dict): the distinct fp64 values of its operator, if there are
+// at most VD_MAX of them -- constant-coefficient stencils and their Galerkin sums hold a handful.  The tile blobs
+// of such a level store an 8-bit code per entry instead of the value (3 bytes per entry instead of 10); the
+// kernels look the value up in a 256-entry table in shared memory: the same fp64 value, bit for bit.
+// Distinct values are collected in a small open-addressing hash table (the insertion stops at the first overflow:
+// a level with all-different values costs a few thousand probes), then sorted ascending, so that the codes are a
+// function of the value set alone.  Code 255 is 0.0: the padding slots of the tiles.
+// ------------------------------------------------------------------------------------------
+constexpr int VD_SLOTS = 1024, VD_MAX = 255;
+constexpr unsigned long long VD_EMPTY = 0xFFFFFFFFFFFFFFFFull;  // (a NaN pattern: never a validated matrix value)
+__global__ void k_vdict_insert(int nnz, const double* __restrict__ val, unsigned long long* table, int* count) {
+  volatile int* over = count + 1;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nnz; i += gridDim.x * blockDim.x) {
+    if (*over) return;
+    const unsigned long long key = (unsigned long long)__double_as_longlong(val[i]);
+    unsigned h = (unsigned)(mix64(key) & (VD_SLOTS - 1));
+    for (int probe = 0; probe < VD_SLOTS; ++probe) {
+      unsigned long long cur = *((volatile unsigned long long*)(table + h));
+      if (cur == VD_EMPTY) {
+        cur = atomicCAS(table + h, VD_EMPTY, key);
+        if (cur == VD_EMPTY) {
+          if (atomicAdd(count, 1) + 1 > VD_MAX) *over = 1;
+          break;
+        }
+      }
+      if (cur == key) break;
+      h = (h + 1) & (VD_SLOTS - 1);
+    }
+  }
+}
+// one CTA of VD_SLOTS threads: the keys sorted ascending as doubles -> dict[0 .. count), dict[255] = 0
+__global__ void __launch_bounds__(VD_SLOTS) k_vdict_finalize(const unsigned long long* __restrict__ table,
+                                                             const int* __restrict__ count, double* __restrict__ dict) {
+  __shared__ double v[VD_SLOTS];
+  const int tid = threadIdx.x;
+  const unsigned long long key = table[tid];
+  v[tid] = key == VD_EMPTY ? __longlong_as_double(0x7FF0000000000000ll) : __longlong_as_double((long long)key);
+  __syncthreads();
+  for (int k = 2; k <= VD_SLOTS; k <<= 1)
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      const int p = tid ^ j;
+      if (p > tid) {
+        const double a = v[tid], b = v[p];
+        const bool asc = (tid & k) == 0;
+        if ((a > b) == asc) v[tid] = b, v[p] = a;
+      }
+      __syncthreads();
+    }
+  if (tid < 256) dict[tid] = (tid < *count && tid < VD_MAX) ? v[tid] : 0.0;
+}
+// code of a value: its position in the ascending dictionary (exact match by construction)
+__device__ __forceinline__ unsigned char vdict_code(const double* dict, int ndict, double v) {
+  int lo = 0, hi = ndict;  // first entry >= v
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (dict[mid] < v) lo = mid + 1;
+    else hi = mid;
+  }
+  return (unsigned char)lo;
+}
+
 constexpr int PK_THREADS = 256;
 constexpr int PK_MAX_LEN = 512;
 __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int* __restrict__ blk_ptr,
@@ -711,7 +773,8 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
                                                            const int* __restrict__ halo_off, int* __restrict__ size16,
                                                            int* __restrict__ nhalo_out, int* __restrict__ info,
                                                            TileDesc* __restrict__ tiles, unsigned char* __restrict__ blob,
-                                                           int* __restrict__ halo_idx, int* __restrict__ halo_cagg) {
+                                                           int* __restrict__ halo_idx, int* __restrict__ halo_cagg,
+                                                           const double* __restrict__ vdict, int ndict) {
   __shared__ int ext[RT_MAX_NNZ];
   __shared__ int halo[RT_MAX_NNZ];
   __shared__ int len[RT_MAX_ROWS];
@@ -867,6 +930,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);  // vb == 4: mixed-precision hierarchy
+  unsigned char* o_val8 = base + p.o_val;                      // vb == 1: codes into the level's value dictionary
   // tile-local column of every entry of the tile, one thread per entry (ext[] is free again: reused as u16[])
   unsigned short* c16s = reinterpret_cast<unsigned short*>(ext);
   __syncthreads();
@@ -927,7 +991,9 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
         cur[t] = nx;
       }
       o_col[off + k * 32] = c16;
-      if (vb == 4)
+      if (vb == 1)
+        o_val8[off + k * 32] = k < ln ? vdict_code(vdict, ndict, v) : (unsigned char)255;
+      else if (vb == 4)
         o_val32[off + k * 32] = (float)v;
       else
         o_val[off + k * 32] = v;
@@ -1261,6 +1327,35 @@ amg_status dense_lu_of(amg_handle_s* H, int n, const int* rowptr, const int* col
   return AMG_OK;
 }
 
+// Value dictionary of a level: *ndict = number of distinct values (1 .. VD_MAX) and dict[256] filled, or 0 if the
+// level holds more (dict untouched).  `dict` is allocated on the first success and reused by a warm resetup.
+amg_status build_vdict(amg_handle_s* H, const double* val, int nnz, double** dict, int* ndict, cudaStream_t st) {
+  *ndict = 0;
+  if (nnz <= 0) return AMG_OK;
+  unsigned long long* table;
+  int* count;
+  AMG_ALLOC(H, table, unsigned long long, VD_SLOTS, st);
+  AMG_ALLOC(H, count, int, 2, st);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(table, 0xFF, sizeof(unsigned long long) * VD_SLOTS, st));
+  AMG_CUDA_TRY(H, cudaMemsetAsync(count, 0, 2 * sizeof(int), st));
+  int g = div_up(nnz, TPB * 8);
+  if (g > H->sm_count * 8) g = H->sm_count * 8;
+  k_vdict_insert<<<g, TPB, 0, st>>>(nnz, val, table, count);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  int h_count[2] = {0, 0};
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(h_count, count, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  if (!h_count[1] && h_count[0] >= 1 && h_count[0] <= VD_MAX) {
+    if (!*dict) AMG_ALLOC(H, *dict, double, 256, st);
+    k_vdict_finalize<<<1, VD_SLOTS, 0, st>>>(table, count, *dict);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    *ndict = h_count[0];
+  }
+  amg_dev_free(H, table);
+  amg_dev_free(H, count);
+  return AMG_OK;
+}
+
 // Row-tile partition by stage bytes, then the tile packer (amg_tilepack.cuh) for one operator of a
 // level (A_l or A_l^T) in permuted numbering.  The byte model of the partition is approximate (the
 // halo of a tile is only known once it is cut), so the target is rescaled until every tile fits a
@@ -1279,8 +1374,8 @@ struct TilePack {
 // search starts a little above it instead of at 1: one attempt per level instead of two or three)
 amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
                       const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st,
-                      double* scale_io = nullptr, int vb = 8) {
-  const int nnz_w = 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value
+                      double* scale_io = nullptr, int vb = 8, const double* vdict = nullptr, int ndict = 0) {
+  const int nnz_w = 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value (or its 8-bit code)
   const int64_t total_w = nnz_w * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
   double scale = scale_io ? (*scale_io * 1.12 < 1.0 ? *scale_io * 1.12 : 1.0) : 1.0;
   for (int attempt = 0; attempt < 6 && !P.fast; ++attempt) {
@@ -1302,7 +1397,7 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
     k_blk_partition<<<grid_for(P.nblk + 1), TPB, 0, st>>>(P.nblk, target, nnz_w, agg_ptr ? nc : n, agg_ptr, rowptr, n,
                                                          P.blk_ptr);
     k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, vb, 0, nullptr, nullptr, size16, nh,
-                                               info, P.tiles, nullptr, nullptr, nullptr);
+                                               info, P.tiles, nullptr, nullptr, nullptr, vdict, ndict);
     AMG_CUDA_TRY(H, cudaGetLastError());
     int h_info[4];
     AMG_CUDA_TRY(H, cudaMemcpyAsync(h_info, info, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -1327,7 +1422,7 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
       AMG_ALLOC(H, P.halo_idx, int, total_h + 4, st);
       AMG_ALLOC(H, P.halo_cagg, int, total_h + 4, st);
       k_pack_tiles<<<P.nblk, PK_THREADS, 0, st>>>(P.nblk, P.blk_ptr, rowptr, col, val, agg, vb, 1, off16, hoff, size16, nh, info,
-                                                 P.tiles, P.blob, P.halo_idx, P.halo_cagg);
+                                                 P.tiles, P.blob, P.halo_idx, P.halo_cagg, vdict, ndict);
       AMG_CUDA_TRY(H, cudaGetLastError());
       P.fast = 1;
       if (scale_io) *scale_io = scale;
@@ -1507,6 +1602,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     amg_dev_free(H, sizep);
   }
   double pack_scale = 1.0;
+  double pack_scale1 = 0.55;  // levels stored as 8-bit codes: the x slot, not the stage, bounds a tile
   for (int q = 0; q <= Lc; ++q) {
     Level& L = H->lv[q];
     const NatCsr& N = nat[q];
@@ -1524,9 +1620,11 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     L.fast = 0;
     L.v32 = (o.hierarchy_fp32 && q < Lc) ? 1 : 0;  // mixed-precision hierarchy: the V-cycle's operators in fp32
     if (!o.force_generic && L.n > 0) {
+      if (o.value_dict && !o.hierarchy_fp32) AMG_TRY(build_vdict(H, L.val, L.nnz, &L.vdict, &L.ndict, st));
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
-                         q < Lc ? L.nc : 0, P, st, &pack_scale, L.v32 ? 4 : 8));
+                         q < Lc ? L.nc : 0, P, st, L.ndict > 0 ? &pack_scale1 : &pack_scale, L.ndict > 0 ? 1 : (L.v32 ? 4 : 8),
+                         L.vdict, L.ndict));
       L.blk_ptr = P.blk_ptr, L.tiles = P.tiles, L.blob = P.blob, L.halo_idx = P.halo_idx, L.halo_cagg = P.halo_cagg;
       L.blob_bytes = P.blob_bytes, L.nblk = P.nblk, L.fast = P.fast;
       if (L.v32 && q == 0) {  // the Krylov method's own SpMV keeps the fp64 operator
@@ -1593,7 +1691,7 @@ amg_status amg_ensure_transposed(amg_handle_s* H, cudaStream_t st) {
     if (!H->opt.force_generic && L.n > 0) {
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, T.rowptr, T.col, T.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
-                         q < Lc ? L.nc : 0, P, st, nullptr, L.v32 ? 4 : 8));
+                         q < Lc ? L.nc : 0, P, st, nullptr, L.ndict > 0 ? 1 : (L.v32 ? 4 : 8), L.vdict, L.ndict));
       T.blk_ptr = P.blk_ptr, T.tiles = P.tiles, T.blob = P.blob, T.halo_idx = P.halo_idx, T.halo_cagg = P.halo_cagg;
       T.blob_bytes = P.blob_bytes, T.nblk = P.nblk, T.fast = P.fast;
       if (L.v32 && q == 0) {  // fp64 blobs of A_0^T for the Krylov method's SpMV
@@ -1719,7 +1817,8 @@ __global__ void k_rap_numeric(int m, const int* __restrict__ cptr, const int* __
 __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc* __restrict__ tiles,
                                                      const int* __restrict__ rowptr, const int* __restrict__ col,
                                                      const double* __restrict__ val, const int* __restrict__ halo_idx,
-                                                     unsigned char* __restrict__ blob) {
+                                                     unsigned char* __restrict__ blob, const double* __restrict__ vdict,
+                                                     int ndict) {
   // the column section of the blob says which entry every slot holds (whatever order the packer chose): slot ->
   // tile-local column -> level column -> position in the CSR row (ascending unique columns: binary search)
   const int t = blockIdx.x;
@@ -1739,10 +1838,12 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
       const int k = q >> 5, lane = q & 31;
       const int lr = perm[j * 32 + lane];
       double v = 0.0;
+      bool in_row = false;
       if (lr != 0xFFFF) {
         const int r = d.r0 + lr;
         const int s = rowptr[r], e = rowptr[r + 1];
         if (k < e - s) {
+          in_row = true;
           const int c16 = o_col[sl.x + q];
           const int c = c16 < d.nr ? d.r0 + c16 : halo_idx[d.halo_off + c16 - d.nr];
           int lo = s, hi = e;  // first entry >= c
@@ -1754,7 +1855,9 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
           v = val[lo];
         }
       }
-      if (d.vb == 4)
+      if (d.vb == 1)
+        (base + p.o_val)[sl.x + q] = in_row ? vdict_code(vdict, ndict, v) : (unsigned char)255;
+      else if (d.vb == 4)
         o_val32[sl.x + q] = (float)v;
       else
         o_val[sl.x + q] = v;
@@ -1876,16 +1979,28 @@ amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fa
     k_rap_numeric<<<grid_for(C.nnz), TPB, 0, st>>>(C.nnz, L.contrib_ptr, L.contrib_idx, L.val, C.val);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
+  // ---- value dictionaries of the levels stored as 8-bit codes: the new values must fit one again ----
+  for (int l = 0; l <= Lc; ++l) {
+    Level& L = H->lv[l];
+    if (L.ndict <= 0) continue;
+    int nd = 0;
+    AMG_TRY(build_vdict(H, L.val, L.nnz, &L.vdict, &nd, st));
+    if (nd <= 0) {  // more than 255 distinct values now: the blobs need the fp64 layout
+      *fallback = 1;
+      return AMG_OK;
+    }
+    L.ndict = nd;
+  }
   // ---- smoother diagonals, blob value sections, transposed values ----
   for (int l = 0; l <= Lc; ++l) {
     Level& L = H->lv[l];
     if (l < Lc) k_dinv<<<grid_for(L.n), TPB, 0, st>>>(L.n, L.rowptr, L.col, L.val, o.smoother, o.omega, L.dinv);
-    if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.col, L.val, L.halo_idx, L.blob);
-    if (L.K.fast) k_blob_refill<<<L.K.nblk, 256, 0, st>>>(L.K.nblk, L.K.tiles, L.rowptr, L.col, L.val, L.K.halo_idx, L.K.blob);
+    if (L.fast) k_blob_refill<<<L.nblk, 256, 0, st>>>(L.nblk, L.tiles, L.rowptr, L.col, L.val, L.halo_idx, L.blob, L.vdict, L.ndict);
+    if (L.K.fast) k_blob_refill<<<L.K.nblk, 256, 0, st>>>(L.K.nblk, L.K.tiles, L.rowptr, L.col, L.val, L.K.halo_idx, L.K.blob, nullptr, 0);
     if (H->have_T) {
       k_gather_vals<<<grid_for(L.nnz), TPB, 0, st>>>(L.nnz, L.val, L.T.src, L.T.val);
-      if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.col, L.T.val, L.T.halo_idx, L.T.blob);
-      if (L.KT.fast) k_blob_refill<<<L.KT.nblk, 256, 0, st>>>(L.KT.nblk, L.KT.tiles, L.T.rowptr, L.T.col, L.T.val, L.KT.halo_idx, L.KT.blob);
+      if (L.T.fast) k_blob_refill<<<L.T.nblk, 256, 0, st>>>(L.T.nblk, L.T.tiles, L.T.rowptr, L.T.col, L.T.val, L.T.halo_idx, L.T.blob, L.vdict, L.ndict);
+      if (L.KT.fast) k_blob_refill<<<L.KT.nblk, 256, 0, st>>>(L.KT.nblk, L.KT.tiles, L.T.rowptr, L.T.col, L.T.val, L.KT.halo_idx, L.KT.blob, nullptr, 0);
     }
   }
   AMG_CUDA_TRY(H, cudaGetLastError());

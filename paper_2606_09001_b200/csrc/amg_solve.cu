@@ -120,6 +120,7 @@ RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
     a.tiles = L.tiles, a.ntiles = L.nblk, a.blob = L.blob;
     a.halo_idx = L.halo_idx, a.halo_cagg = L.halo_cagg;
   }
+  a.vdict = L.ndict > 0 ? L.vdict : nullptr;  // (A_l^T holds the same values: the same dictionary)
   a.dinv = L.dinv;
   a.dinv_x1 = L.dinv;
   a.agg = L.agg;
