@@ -263,7 +263,8 @@ AMG_API amg_status amg_get_setup_stats(amg_handle h, amg_setup_stats* stats);
 AMG_API amg_status amg_get_level_path(amg_handle h, int32_t level, int32_t* fast_path);
 /* Algorithmic bytes of: which = 0 one level-0 SpMV, 1 one V-cycle,
  * 2 one PCG iteration (SpMV + vector ops + V-cycle), 3 one BiCGSTAB iteration,
- * 4 one level-0 smoother sweep. */
+ * 4 one level-0 smoother sweep.  Stored sizes (not algorithmic): 10 = bytes of the tile blobs of all levels the
+ * V-cycle streams, 11 = of level 0 alone, 12 = number of levels stored as 8-bit codes (value_dict). */
 AMG_API amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes);
 
 /* Kernel launches enqueued by the last amg_solve* / amg_level_op / amg_grad_values call on this

@@ -22,6 +22,23 @@ constexpr int RT_CTAS = 2;            // persistent CTAs per SM
 constexpr int RT_STAGE_BYTES = 29696; // shared memory of one ring stage (descriptor + operands of one tile)
 constexpr int RT_XSLOTS = 4;          // x slots (side ring): how many tiles the gather warps run ahead
 constexpr int RT_XSLOT_BYTES = 5632;  // one x slot: 8 bytes x (rows + halo columns of a tile)
+// Ring geometry of the row-tile kernel per kind of level: 0 = fp64 / fp32 values (the constants above), 1 = levels
+// stored as 8-bit codes into a value dictionary (3 bytes per entry: a tile of the same bytes holds ~2.4 x the rows,
+// so the x slots grow and the stages shrink; one more stage keeps as many bytes in flight)
+template <int GEO> struct RtGeo;
+template <> struct RtGeo<0> {
+  static constexpr int STAGES = RT_STAGES, STAGE_BYTES = RT_STAGE_BYTES, XSLOTS = RT_XSLOTS, XSLOT_BYTES = RT_XSLOT_BYTES;
+  static constexpr int GATHER_UNROLL = RT_GATHER_UNROLL, GATHER_ROWS = RT_GATHER_ROWS;
+};
+template <> struct RtGeo<1> {
+  static constexpr int STAGES = 4, STAGE_BYTES = 18432, XSLOTS = 4, XSLOT_BYTES = 8192;
+  static constexpr int GATHER_UNROLL = 6, GATHER_ROWS = 5;
+};
+template <int GEO> constexpr int rt_smem_bytes() {
+  return 256 + RtGeo<GEO>::STAGES * RtGeo<GEO>::STAGE_BYTES + RtGeo<GEO>::XSLOTS * RtGeo<GEO>::XSLOT_BYTES;
+}
+inline int rt_stage_bytes(int geo) { return geo ? RtGeo<1>::STAGE_BYTES : RtGeo<0>::STAGE_BYTES; }
+inline int rt_xslot_bytes(int geo) { return geo ? RtGeo<1>::XSLOT_BYTES : RtGeo<0>::XSLOT_BYTES; }
 constexpr int RT_MAX_NNZ = 4096;                   // most entries / halo columns of a tile (packer scratch)
 constexpr int RT_MAX_ROWS = 1024;                  // most rows of a tile
 constexpr int VEC_PAD = 8;        // every vector / index array is over-allocated by this many elements:
@@ -109,6 +126,8 @@ struct Level {
   int v32 = 0;              // 1: this level's V-cycle operator is the fp64 one rounded to fp32
   double* vdict = nullptr;  // [256] value dictionary of the level (ascending distinct values, [255] = 0 for padding
   int ndict = 0;            //   slots); ndict > 0: the tile blobs hold 8-bit codes (TileDesc::vb = 1)
+  unsigned long long* vd_table = nullptr;  // hash set of the distinct values (kept for warm resetups)
+  int* vd_count = nullptr;                 // {distinct values, overflow}
   int lpr = 8;              // lanes per row of the fallback kernels
   int stream_hint = 0;      // 1: matrix larger than half of L2 -> evict-first loads
   // natural numbering (the caller's / oracle's): hooks and the ABI boundary

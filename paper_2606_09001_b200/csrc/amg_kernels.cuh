@@ -452,8 +452,14 @@ struct GTile {  // what the gather warps need of a tile descriptor
   }
 };
 
-template <int OP, int NDOT, bool STREAM>
+template <int OP, int NDOT, bool STREAM, int GEO>
 static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
+  // ring geometry of this kind of level (the names shadow the fp64 geometry's constants)
+  constexpr int RT_STAGES = RtGeo<GEO>::STAGES, RT_STAGE_BYTES = RtGeo<GEO>::STAGE_BYTES;
+  constexpr int RT_XSLOTS = RtGeo<GEO>::XSLOTS, RT_XSLOT_BYTES = RtGeo<GEO>::XSLOT_BYTES;
+  constexpr int RT_GATHER_UNROLL = RtGeo<GEO>::GATHER_UNROLL, RT_GATHER_ROWS = RtGeo<GEO>::GATHER_ROWS;
+  static_assert((4 * RT_STAGES + 2 * RT_XSLOTS) * 8 <= rt::HEADER_BYTES && RT_XSLOTS >= 2 * RT_GGROUPS, "ring header");
+  static_assert(RT_STAGE_BYTES % 128 == 0 && RT_XSLOT_BYTES % 128 == 0, "stage / slot sizes must keep 128-byte alignment");
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
   uint64_t* empty = full + RT_STAGES;

@@ -719,17 +719,24 @@ __global__ void k_vdict_insert(int nnz, const double* __restrict__ val, unsigned
     if (*over) return;
     const unsigned long long key = (unsigned long long)__double_as_longlong(val[i]);
     unsigned h = (unsigned)(mix64(key) & (VD_SLOTS - 1));
-    for (int probe = 0; probe < VD_SLOTS; ++probe) {
+    bool placed = false;
+    // at most VD_MAX keys in VD_SLOTS slots: a probe sequence longer than 64 means the table is being flooded
+    for (int probe = 0; probe < 64 && !placed; ++probe) {
       unsigned long long cur = *((volatile unsigned long long*)(table + h));
       if (cur == VD_EMPTY) {
+        if (*over) return;
         cur = atomicCAS(table + h, VD_EMPTY, key);
         if (cur == VD_EMPTY) {
           if (atomicAdd(count, 1) + 1 > VD_MAX) *over = 1;
-          break;
+          placed = true;
         }
       }
-      if (cur == key) break;
+      if (cur == key) placed = true;
       h = (h + 1) & (VD_SLOTS - 1);
+    }
+    if (!placed) {
+      *over = 1;
+      return;
     }
   }
 }
@@ -1327,33 +1334,56 @@ amg_status dense_lu_of(amg_handle_s* H, int n, const int* rowptr, const int* col
   return AMG_OK;
 }
 
-// Value dictionary of a level: *ndict = number of distinct values (1 .. VD_MAX) and dict[256] filled, or 0 if the
-// level holds more (dict untouched).  `dict` is allocated on the first success and reused by a warm resetup.
-amg_status build_vdict(amg_handle_s* H, const double* val, int nnz, double** dict, int* ndict, cudaStream_t st) {
-  *ndict = 0;
-  if (nnz <= 0) return AMG_OK;
-  unsigned long long* table;
-  int* count;
-  AMG_ALLOC(H, table, unsigned long long, VD_SLOTS, st);
-  AMG_ALLOC(H, count, int, 2, st);
-  AMG_CUDA_TRY(H, cudaMemsetAsync(table, 0xFF, sizeof(unsigned long long) * VD_SLOTS, st));
-  AMG_CUDA_TRY(H, cudaMemsetAsync(count, 0, 2 * sizeof(int), st));
-  int g = div_up(nnz, TPB * 8);
-  if (g > H->sm_count * 8) g = H->sm_count * 8;
-  k_vdict_insert<<<g, TPB, 0, st>>>(nnz, val, table, count);
-  AMG_CUDA_TRY(H, cudaGetLastError());
-  int h_count[2] = {0, 0};
-  AMG_CUDA_TRY(H, cudaMemcpyAsync(h_count, count, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
-  if (!h_count[1] && h_count[0] >= 1 && h_count[0] <= VD_MAX) {
-    if (!*dict) AMG_ALLOC(H, *dict, double, 256, st);
-    k_vdict_finalize<<<1, VD_SLOTS, 0, st>>>(table, count, *dict);
-    AMG_CUDA_TRY(H, cudaGetLastError());
-    *ndict = h_count[0];
+// Value dictionary of a level, in two stream-ordered halves so that a warm resetup can queue all levels and
+// synchronise once: vdict_collect (hash-set insertion; table and counters stay on the level) and, once the host has
+// read the counters, vdict_finish (sort -> L.vdict[256]).
+amg_status vdict_collect(amg_handle_s* H, Level& L, cudaStream_t st) {
+  if (!L.vd_table) {
+    AMG_ALLOC(H, L.vd_table, unsigned long long, VD_SLOTS, st);
+    AMG_ALLOC(H, L.vd_count, int, 2, st);
   }
-  amg_dev_free(H, table);
-  amg_dev_free(H, count);
+  AMG_CUDA_TRY(H, cudaMemsetAsync(L.vd_table, 0xFF, sizeof(unsigned long long) * VD_SLOTS, st));
+  AMG_CUDA_TRY(H, cudaMemsetAsync(L.vd_count, 0, 2 * sizeof(int), st));
+  int g = div_up(L.nnz, TPB * 8);
+  if (g > H->sm_count * 8) g = H->sm_count * 8;
+  if (g < 1) g = 1;
+  k_vdict_insert<<<g, TPB, 0, st>>>(L.nnz, L.val, L.vd_table, L.vd_count);
+  AMG_CUDA_TRY(H, cudaGetLastError());
   return AMG_OK;
+}
+// h_count = the level's two counters as read by the host; returns the number of distinct values, 0 = no dictionary
+amg_status vdict_finish(amg_handle_s* H, Level& L, const int* h_count, int* ndict, cudaStream_t st) {
+  *ndict = 0;
+  if (h_count[1] || h_count[0] < 1 || h_count[0] > VD_MAX) return AMG_OK;
+  if (!L.vdict) AMG_ALLOC(H, L.vdict, double, 256, st);
+  k_vdict_finalize<<<1, VD_SLOTS, 0, st>>>(L.vd_table, L.vd_count, L.vdict);
+  AMG_CUDA_TRY(H, cudaGetLastError());
+  *ndict = h_count[0];
+  return AMG_OK;
+}
+amg_status build_vdict(amg_handle_s* H, Level& L, cudaStream_t st) {
+  L.ndict = 0;
+  if (L.nnz <= 0) return AMG_OK;
+  int h_count[2] = {0, 0};
+  if (L.nnz > 16384) {
+    // a cheap look at the first entries first: a level with all-different values (variable coefficients) is
+    // recognised by one CTA instead of a full-grid insertion that floods the table
+    if (!L.vd_table) {
+      AMG_ALLOC(H, L.vd_table, unsigned long long, VD_SLOTS, st);
+      AMG_ALLOC(H, L.vd_count, int, 2, st);
+    }
+    AMG_CUDA_TRY(H, cudaMemsetAsync(L.vd_table, 0xFF, sizeof(unsigned long long) * VD_SLOTS, st));
+    AMG_CUDA_TRY(H, cudaMemsetAsync(L.vd_count, 0, 2 * sizeof(int), st));
+    k_vdict_insert<<<1, 1024, 0, st>>>(8192, L.val, L.vd_table, L.vd_count);
+    AMG_CUDA_TRY(H, cudaGetLastError());
+    AMG_CUDA_TRY(H, cudaMemcpyAsync(h_count, L.vd_count, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    if (h_count[1]) return AMG_OK;
+  }
+  AMG_TRY(vdict_collect(H, L, st));
+  AMG_CUDA_TRY(H, cudaMemcpyAsync(h_count, L.vd_count, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+  AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+  return vdict_finish(H, L, h_count, &L.ndict, st);
 }
 
 // Row-tile partition by stage bytes, then the tile packer (amg_tilepack.cuh) for one operator of a
@@ -1376,10 +1406,11 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
                       const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st,
                       double* scale_io = nullptr, int vb = 8, const double* vdict = nullptr, int ndict = 0) {
   const int nnz_w = 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value (or its 8-bit code)
+  const int stage_cap = rt_stage_bytes(vb == 1), xslot_cap = rt_xslot_bytes(vb == 1);  // ring geometry of the level kind
   const int64_t total_w = nnz_w * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
   double scale = scale_io ? (*scale_io * 1.12 < 1.0 ? *scale_io * 1.12 : 1.0) : 1.0;
   for (int attempt = 0; attempt < 6 && !P.fast; ++attempt) {
-    const int target = (int)((RT_STAGE_BYTES - TP_DESC_BYTES - 256) * scale);
+    const int target = (int)((stage_cap - TP_DESC_BYTES - 256) * scale);
     if (target < 512) break;
     if (P.blk_ptr) amg_dev_free(H, P.blk_ptr);
     if (P.tiles) amg_dev_free(H, P.tiles);
@@ -1404,8 +1435,8 @@ amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const 
     AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
     if (h_info[1]) {
       scale *= 0.5;
-    } else if (h_info[0] > RT_STAGE_BYTES || h_info[2] > RT_XSLOT_BYTES) {
-      const double f1 = (double)RT_STAGE_BYTES / (double)h_info[0], f2 = (double)RT_XSLOT_BYTES / (double)h_info[2];
+    } else if (h_info[0] > stage_cap || h_info[2] > xslot_cap) {
+      const double f1 = (double)stage_cap / (double)h_info[0], f2 = (double)xslot_cap / (double)h_info[2];
       scale *= 0.96 * (f1 < f2 ? f1 : f2);
     } else {
       AMG_TRY(amg_exclusive_scan(H, size16, off16, P.nblk, st));
@@ -1602,7 +1633,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     amg_dev_free(H, sizep);
   }
   double pack_scale = 1.0;
-  double pack_scale1 = 0.55;  // levels stored as 8-bit codes: the x slot, not the stage, bounds a tile
+  double pack_scale1 = 1.0;   // (levels stored as 8-bit codes have their own ring geometry: their own scale)
   for (int q = 0; q <= Lc; ++q) {
     Level& L = H->lv[q];
     const NatCsr& N = nat[q];
@@ -1620,7 +1651,7 @@ amg_status amg_build_hierarchy(amg_handle_s* H, const int32_t* d_rowptr, const i
     L.fast = 0;
     L.v32 = (o.hierarchy_fp32 && q < Lc) ? 1 : 0;  // mixed-precision hierarchy: the V-cycle's operators in fp32
     if (!o.force_generic && L.n > 0) {
-      if (o.value_dict && !o.hierarchy_fp32) AMG_TRY(build_vdict(H, L.val, L.nnz, &L.vdict, &L.ndict, st));
+      if (o.value_dict && !o.hierarchy_fp32 && q < 64) AMG_TRY(build_vdict(H, L, st));  // (64: the warm path's counter array)
       TilePack P;
       AMG_TRY(pack_tiles(H, L.n, L.nnz, L.rowptr, L.col, L.val, q < Lc ? L.agg : nullptr, q < Lc ? L.agg_ptr : nullptr,
                          q < Lc ? L.nc : 0, P, st, L.ndict > 0 ? &pack_scale1 : &pack_scale, L.ndict > 0 ? 1 : (L.v32 ? 4 : 8),
@@ -1979,17 +2010,30 @@ amg_status amg_resetup_values_warm(amg_handle_s* H, const double* d_val, int* fa
     k_rap_numeric<<<grid_for(C.nnz), TPB, 0, st>>>(C.nnz, L.contrib_ptr, L.contrib_idx, L.val, C.val);
   }
   AMG_CUDA_TRY(H, cudaGetLastError());
-  // ---- value dictionaries of the levels stored as 8-bit codes: the new values must fit one again ----
-  for (int l = 0; l <= Lc; ++l) {
-    Level& L = H->lv[l];
-    if (L.ndict <= 0) continue;
-    int nd = 0;
-    AMG_TRY(build_vdict(H, L.val, L.nnz, &L.vdict, &nd, st));
-    if (nd <= 0) {  // more than 255 distinct values now: the blobs need the fp64 layout
-      *fallback = 1;
-      return AMG_OK;
+  // ---- value dictionaries of the levels stored as 8-bit codes: the new values must fit one again (all levels
+  // queued, one synchronisation) ----
+  {
+    int h_counts[64][2];
+    int nd_levels = 0;
+    for (int l = 0; l <= Lc && l < 64; ++l) {
+      Level& L = H->lv[l];
+      if (L.ndict <= 0) continue;
+      AMG_TRY(vdict_collect(H, L, st));
+      AMG_CUDA_TRY(H, cudaMemcpyAsync(h_counts[l], L.vd_count, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+      ++nd_levels;
     }
-    L.ndict = nd;
+    if (nd_levels) AMG_CUDA_TRY(H, cudaStreamSynchronize(st));
+    for (int l = 0; l <= Lc && l < 64; ++l) {
+      Level& L = H->lv[l];
+      if (L.ndict <= 0) continue;
+      int nd = 0;
+      AMG_TRY(vdict_finish(H, L, h_counts[l], &nd, st));
+      if (nd <= 0) {  // more than 255 distinct values now: the blobs need the fp64 layout
+        *fallback = 1;
+        return AMG_OK;
+      }
+      L.ndict = nd;
+    }
   }
   // ---- smoother diagonals, blob value sections, transposed values ----
   for (int l = 0; l <= Lc; ++l) {

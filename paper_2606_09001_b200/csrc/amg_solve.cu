@@ -69,11 +69,17 @@ inline int lv_nblk(const Level& L) {
   return g_tr ? L.T.nblk : L.nblk;
 }
 
+inline int lv_geo(const Level& L) {  // ring geometry of the blobs about to be streamed (RtGeo)
+  return (lv_kop(L) == nullptr && L.ndict > 0) ? 1 : 0;
+}
 template <int OP, int NDOT, bool STREAM>
 void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStream_t st) {
   int grid = H->sm_count * RT_CTAS;
   if (grid > lv_nblk(L)) grid = lv_nblk(L);
-  ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM>, grid, RT_THREADS, rt::SMEM_BYTES, st)(a);
+  if (lv_geo(L))
+    ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM, 1>, grid, RT_THREADS, rt_smem_bytes<1>(), st)(a);
+  else
+    ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM, 0>, grid, RT_THREADS, rt_smem_bytes<0>(), st)(a);
 }
 
 template <int OP, int NDOT>
@@ -99,8 +105,10 @@ void launch_row(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaStr
 
 template <int OP, int NDOT>
 void set_tile_attr() {
-  cudaFuncSetAttribute(k_rowtile<OP, NDOT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
-  cudaFuncSetAttribute(k_rowtile<OP, NDOT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt::SMEM_BYTES);
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem_bytes<0>());
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem_bytes<0>());
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem_bytes<1>());
+  cudaFuncSetAttribute(k_rowtile<OP, NDOT, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem_bytes<1>());
 }
 
 RowArgs base_args(const amg_handle_s* H, const Level& L, KrylovCtl* ctl) {
@@ -953,6 +961,17 @@ double amg_algorithmic_bytes(amg_handle_s* H, int which) {
     case 2: return (M(0) + 2 * V(0)) + 6 * V(0) + 3 * V(0) + vcycle();
     case 3: return 2 * (M(0) + 2 * V(0)) + 2 * vcycle() + (4 + 3 + 8) * V(0) + 2 * V(0);
     case 4: return M(0) + 4 * V(0);
+    case 10: {  // bytes the V-cycle's operators occupy as stored: tile blobs + halo index lists (else the CSR)
+      double tot = 0.0;
+      for (int l = 0; l < Lc; ++l) tot += H->lv[l].fast ? (double)H->lv[l].blob_bytes : M(l);
+      return tot;
+    }
+    case 11: return H->lv[0].fast ? (double)H->lv[0].blob_bytes : M(0);  // level 0 alone
+    case 12: {  // levels stored as 8-bit codes into a value dictionary
+      double cnt = 0.0;
+      for (int l = 0; l < Lc; ++l) cnt += H->lv[l].ndict > 0 ? 1.0 : 0.0;
+      return cnt;
+    }
     default: return 0.0;
   }
 }
