@@ -438,7 +438,7 @@ amg_status amg_get_level_path(amg_handle h, int32_t level, int32_t* fast_path) {
 }
 
 amg_status amg_get_algorithmic_bytes(amg_handle h, int32_t which, double* bytes) {
-  if (!h || !bytes || which < 0 || which > 4) return AMG_ERR_INVALID_ARG;
+  if (!h || !bytes || which < 0 || (which > 4 && (which < 10 || which > 12))) return AMG_ERR_INVALID_ARG;
   *bytes = amg_algorithmic_bytes(h, which);
   return AMG_OK;
 }

@@ -372,6 +372,99 @@ def test_full_size_headline_options_against_the_oracle(oracle_mod, B):
         oracle_mod.set_threads(1)
 
 
+@pytest.mark.parametrize("opts", [dict(), dict(smoother=2, agg_passes=2, coarse_scale=1.6), dict(krylov=1)])
+def test_value_dictionary_is_bit_faithful_storage(oracle_mod, B, opts):
+    """amg_options::value_dict: a level with at most 255 distinct fp64 values stores 8-bit codes into a table of
+    those values.  The operator is the same, value for value: against the oracle (V-cycle <= 1e-12, solve, iteration
+    count) exactly like the fp64 layout, and against the fp64 layout of the same handle options to rounding (tile
+    boundaries differ, so row sums associate differently).  A Poisson hierarchy takes the dictionary on every level
+    that runs the row-tile kernels, a variable-coefficient one on none."""
+    A = inputs.config_matrix(3, 40)
+    b = inputs.config_rhs(3, A.n)
+    okw = {k: v for k, v in opts.items() if k != "krylov"}
+    o = oracle_mod.Oracle(A.rowptr, A.col, A.val, **okw)
+    sd = B.AmgSolver(A.rowptr, A.col, A.val, value_dict=1, **opts)
+    s8 = B.AmgSolver(A.rowptr, A.col, A.val, value_dict=0, **opts)
+    try:
+        nd = int(B.amg_get_algorithmic_bytes(sd.h, 12))
+        assert nd >= 2 and int(B.amg_get_algorithmic_bytes(s8.h, 12)) == 0
+        # 3 bytes per entry instead of 10
+        assert B.amg_get_algorithmic_bytes(sd.h, 11) < 0.45 * B.amg_get_algorithmic_bytes(s8.h, 11)
+        r = torch.as_tensor(b, device="cuda")
+        zo = o.vcycle(b)
+        zd, z8 = sd.apply_preconditioner(r).cpu().numpy(), s8.apply_preconditioner(r).cpu().numpy()
+        assert rel(zd, zo) <= 1e-12 and rel(z8, zo) <= 1e-12 and rel(zd, z8) <= 1e-12
+        kry = opts.get("krylov", 0)
+        xo, io = o.solve(b, 1e-13, 500, kry, 1)
+        xd, idd = sd.solve(b, 1e-11, 500, kry)
+        x8, i8 = s8.solve(b, 1e-11, 500, kry)
+        assert idd.status == 0 and idd.iterations == i8.iterations
+        assert rel(xd.cpu().numpy(), xo) <= 1e-6 and rel(xd.cpu().numpy(), x8.cpu().numpy()) <= 1e-9
+        _, i1 = sd.solve(b, 1e-8, 500, kry)
+        _, io1 = o.solve(b, 1e-8, 500, kry, 1)
+        assert abs(i1.iterations - io1.iterations) <= 2
+        # 8 right-hand sides at once through the batched kernel (symmetric PCG handles)
+        if kry == 0:
+            Bm = torch.as_tensor(np.stack([inputs.config_rhs(5, A.n, k) for k in range(8)]), device="cuda").contiguous()
+            Xd, X8 = torch.empty_like(Bm), torch.empty_like(Bm)
+            B.amg_solve_batched(sd.h, 0, Bm, Xd, 8, A.n, 1e-11, 500)
+            B.amg_solve_batched(s8.h, 0, Bm, X8, 8, A.n, 1e-11, 500)
+            assert rel(Xd.cpu().numpy(), X8.cpu().numpy()) <= 1e-9
+    finally:
+        sd.close(), s8.close(), o.close()
+    A4 = inputs.config_matrix(4, 20)
+    s4 = B.AmgSolver(A4.rowptr, A4.col, A4.val)
+    assert int(B.amg_get_algorithmic_bytes(s4.h, 12)) == 0  # all values different: fp64 blobs as before
+    s4.close()
+
+
+def test_value_dictionary_warm_resetup(oracle_mod, B):
+    """Warm resetup of a hierarchy stored as codes: new values with few distinct entries rebuild the dictionaries
+    in place (the handle stays, graphs stay); new values that are all different do not fit a dictionary: the call
+    falls back to the rebuild with fp64 blobs.  Both equal a fresh oracle on the new values."""
+    A = inputs.config_matrix(3, 32)
+    b = inputs.config_rhs(3, A.n)
+    s = B.AmgSolver(A.rowptr, A.col, A.val)
+    try:
+        assert int(B.amg_get_algorithmic_bytes(s.h, 12)) >= 2
+        x0, _ = s.solve(b, 1e-11, 300)
+        # (i) another constant-coefficient operator on the same pattern: 2.5 A + 0.75 I
+        v1 = 2.5 * A.val
+        diag = A.col == np.repeat(np.arange(A.n), np.diff(A.rowptr))
+        v1[diag] += 0.75
+        s.resetup_values(v1, keep_aggregates=True)
+        assert int(B.amg_get_algorithmic_bytes(s.h, 12)) >= 2
+        o1 = oracle_mod.Oracle(A.rowptr, A.col, v1)
+        x1, i1 = s.solve(b, 1e-11, 300)
+        xo1, _ = o1.solve(b, 1e-13, 300, 0, 1)
+        assert i1.status == 0 and rel(x1.cpu().numpy(), xo1) <= 1e-6
+        z1 = s.apply_preconditioner(torch.as_tensor(b, device="cuda")).cpu().numpy()
+        assert rel(z1, o1.vcycle(b)) <= 1e-12
+        o1.close()
+        # (ii) symmetric random perturbation of every off-diagonal: ~ nnz / 2 distinct values
+        import scipy.sparse as sp
+
+        rng = np.random.default_rng(77)
+        M = sp.csr_matrix((A.val.copy(), A.col, A.rowptr), shape=(A.n, A.n)).tocoo()
+        lo, hi = np.minimum(M.row, M.col), np.maximum(M.row, M.col)
+        pert = 1.0 + 0.2 * np.sin(1.0 + 0.37 * lo + 0.11 * hi) * (lo != hi)  # same factor for (i, j) and (j, i)
+        M2 = sp.csr_matrix((M.data * pert, (M.row, M.col)), shape=(A.n, A.n))
+        M2.sort_indices()
+        assert np.array_equal(M2.indices, A.col)
+        v2 = M2.data.copy()
+        v2[diag] = 6.5
+        s.resetup_values(v2, keep_aggregates=True)
+        assert int(B.amg_get_algorithmic_bytes(s.h, 12)) == 0  # fell back to fp64 blobs
+        o2 = oracle_mod.Oracle(A.rowptr, A.col, v2, aggregates=[s.aggregates(l).cpu().numpy() for l in range(s.num_levels - 1)])
+        x2, i2 = s.solve(b, 1e-11, 300)
+        xo2, _ = o2.solve(b, 1e-13, 300, 0, 1)
+        assert i2.status == 0 and rel(x2.cpu().numpy(), xo2) <= 1e-6
+        o2.close()
+        del x0
+    finally:
+        s.close()
+
+
 def test_report_file(B, tmp_path):
     """optional file-based output with the hierarchy statistics and the residual history."""
     A = inputs.config_matrix(3, 24)
