@@ -458,6 +458,10 @@ def run_b200(args):
     d_x = torch.empty_like(d_b)
     bytes_spmv, bytes_vcycle, bytes_pcg_it, bytes_bicg_it, bytes_sweep = (B.amg_get_algorithmic_bytes(h, w) for w in range(5))
     hier_bytes = sum(12 * z + 4 * (r + 1) for r, z in levels)
+    l2_note = (f"no flush: one iteration streams the hierarchy ({hier_bytes / 1e6:.0f} MB as CSR, "
+               f"{B.amg_get_algorithmic_bytes(h, 10) / 1e6:.0f} MB as stored: {int(B.amg_get_algorithmic_bytes(h, 12))} "
+               f"levels as 8-bit codes into a value dictionary) and {(9 + 3) * 8 * n / 1e6:.0f} MB of level-0 "
+               "vectors: more than the 126 MB L2")
 
     # ---- dominant kernel: the level-0 smoother sweep (k_rowtile<OP_JACOBI>) --------------
     def timed_level_op(level, op, in0, in1, out, reps):
@@ -668,10 +672,7 @@ def run_b200(args):
             "dtype": "f64", "data": "synthetic",
             "config": config_dict(args.cfg, args.edge, n, nnz),
             "levels": nlev, "parallelism": "replicas only" if world > 1 else "1 GPU",
-            "l2": (f"no flush: one iteration streams the hierarchy ({hier_bytes / 1e6:.0f} MB as CSR, "
-                   f"{B.amg_get_algorithmic_bytes(h, 10) / 1e6:.0f} MB as stored: {int(B.amg_get_algorithmic_bytes(h, 12))} "
-                   f"levels as 8-bit codes into a value dictionary) and {(9 + 3) * 8 * n / 1e6:.0f} MB of level-0 "
-                   "vectors: more than the 126 MB L2"),
+            "l2": l2_note,
             "iterations": iters, "rel_residual": info.rel_residual, "true_rel_residual_host_fp64": true_res,
             "status": info.status, "step_ms_median": round(statistics.median(step_ms), 4),
             "step_ms_min": round(min(step_ms), 4),

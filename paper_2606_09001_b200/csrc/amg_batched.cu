@@ -55,8 +55,10 @@ inline int red_grid_b(const amg_handle_s* H, int64_t units) {
 
 template <int OP, int NDOT>
 void set_attr_b() {
-  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX);
-  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX);
+  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX);
+  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX);
+  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX_VD);
+  cudaFuncSetAttribute(k_rowtile_b<OP, NDOT, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RTB_SMEM_MAX_VD);
 }
 
 template <int OP, int NDOT>
@@ -71,10 +73,14 @@ void launch_rowtile_b(amg_handle_s* H, const Level& L, const LevelGeomB& G, RowA
   a.stages = G.stages, a.xslots = G.xslots, a.stage_bytes = G.stage_bytes, a.xslot_bytes = G.xslot_bytes;
   int grid = H->sm_count;  // one CTA per SM
   if (grid > a.ntiles) grid = a.ntiles;
-  if (L.stream_hint)
-    launch_b(k_rowtile_b<OP, NDOT, true>, grid, RTB_THREADS, G.smem, st, a);
-  else
-    launch_b(k_rowtile_b<OP, NDOT, false>, grid, RTB_THREADS, G.smem, st, a);
+  const bool vd = a.vdict != nullptr;
+  if (L.stream_hint) {
+    if (vd) launch_b(k_rowtile_b<OP, NDOT, true, true>, grid, RTB_THREADS, G.smem, st, a);
+    else launch_b(k_rowtile_b<OP, NDOT, true, false>, grid, RTB_THREADS, G.smem, st, a);
+  } else {
+    if (vd) launch_b(k_rowtile_b<OP, NDOT, false, true>, grid, RTB_THREADS, G.smem, st, a);
+    else launch_b(k_rowtile_b<OP, NDOT, false, false>, grid, RTB_THREADS, G.smem, st, a);
+  }
 }
 
 RowArgsB args_b(KrylovCtlB* ctl) {
@@ -283,8 +289,9 @@ int amg_batch_prepare(amg_handle_s* H, cudaStream_t st) {
     sb = (sb + 127) & ~127, xb = (xb + 127) & ~127;
     LevelGeomB& G = l < 0 ? B.geomK : B.geom[l];
     G.stage_bytes = sb, G.xslot_bytes = xb;
+    const int smem_cap = (l >= 0 && L.ndict > 0) ? RTB_SMEM_MAX_VD : RTB_SMEM_MAX;
     for (int S = 3; S >= 2 && !G.stages; --S) {
-      const int left = RTB_SMEM_MAX - RTB_HEADER - S * sb;
+      const int left = smem_cap - RTB_HEADER - S * sb;
       const int XS = left / xb > RTB_MAXS ? RTB_MAXS : left / xb;
       if (XS >= 2) G.stages = S, G.xslots = XS;
     }

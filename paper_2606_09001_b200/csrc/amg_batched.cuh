@@ -29,7 +29,8 @@ constexpr int RTB_THREADS = RTB_CONSUMERS + 32 + RTB_GATHERERS;
 constexpr int RTB_GU = 12;          // columns per gather thread whose indices are held in registers
 constexpr int RTB_MAXS = 4;         // most ring stages / x slots
 constexpr int RTB_HEADER = 256;
-constexpr int RTB_SMEM_MAX = 220 * 1024;  // dynamic part: the reductions and the value dictionary keep ~4.5 KB of static shared memory
+constexpr int RTB_SMEM_MAX = 224 * 1024;  // dynamic part: the reductions keep ~2.5 KB of static shared memory ...
+constexpr int RTB_SMEM_MAX_VD = 222 * 1024;  // ... and the value dictionary of a level stored as 8-bit codes 2 KB more
 
 struct KrylovCtlB {
   KrylovCtl c[NB];
@@ -337,7 +338,7 @@ struct GTileB {
   }
 };
 
-template <int OP, int NDOT, bool STREAM>
+template <int OP, int NDOT, bool STREAM, bool VD>  // VD: the level is stored as 8-bit codes (every tile has vb = 1)
 static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a) {
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);
@@ -371,8 +372,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
     }
     fence_mbar_init();
   }
-  __shared__ double sdict[256];  // value dictionary of the level (setup data)
-  if (a.vdict != nullptr && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
+  double* sdict = DictStore<VD>::get();  // value dictionary of the level (setup data)
+  if (VD && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
   __syncthreads();
   pdl_launch_dependents();
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
@@ -498,7 +499,8 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
         const unsigned char* sval8 = base + sd->o_val + lane;
-        const bool v32 = sd->vb == 4, v8 = sd->vb == 1;
+        const bool v32 = sd->vb == 4;
+        constexpr bool v8 = VD;
         // tile-local column c: c < nr -> own row c (stage), else halo column c - nr (x slot); both [..][NB2]
         const double2* xown = reinterpret_cast<const double2*>(base + sd->o_xown);
         const double2* xhal = reinterpret_cast<const double2*>(xslot0 + (size_t)q * a.xslot_bytes) - (size_t)nr * NB2;

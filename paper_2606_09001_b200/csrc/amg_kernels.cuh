@@ -452,6 +452,19 @@ struct GTile {  // what the gather warps need of a tile descriptor
   }
 };
 
+// 256-entry value dictionary in static shared memory, only in the kernels that are instantiated for dictionary levels
+template <bool ON>
+struct DictStore {
+  __device__ __forceinline__ static double* get() {
+    __shared__ double s[256];
+    return s;
+  }
+};
+template <>
+struct DictStore<false> {
+  __device__ __forceinline__ static double* get() { return nullptr; }
+};
+
 template <int OP, int NDOT, bool STREAM, int GEO>
 static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   // ring geometry of this kind of level (the names shadow the fp64 geometry's constants)
@@ -488,9 +501,9 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
     }
     fence_mbar_init();
   }
-  // value dictionary of the level (setup data): tiles with vb = 1 hold 8-bit codes into it
-  __shared__ double sdict[256];
-  if (a.vdict != nullptr && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
+  // value dictionary of the level (setup data; GEO 1 = levels stored as 8-bit codes: every tile has vb = 1)
+  double* sdict = DictStore<GEO == 1>::get();
+  if (GEO == 1 && tid < 256) sdict[tid] = __ldg(a.vdict + tid);
   __syncthreads();
   pdl_launch_dependents();
   const uint64_t pol = STREAM ? l2_policy_evict_first() : 0;
@@ -663,7 +676,8 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;  // mixed-precision hierarchy
         const unsigned char* sval8 = base + sd->o_val + lane;                            // value dictionary
-        const bool v32 = sd->vb == 4, v8 = sd->vb == 1;
+        const bool v32 = sd->vb == 4;
+        constexpr bool v8 = (GEO == 1);
         const double* xc = reinterpret_cast<const double*>(xslot0 + q * RT_XSLOT_BYTES);
         const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
