@@ -498,7 +498,7 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;
-        const unsigned char* sval8 = base + sd->o_val + lane;
+        const uint32_t* scw = reinterpret_cast<const uint32_t*>(base + sd->o_col) + lane;  // column | code << 16
         const bool v32 = sd->vb == 4;
         constexpr bool v8 = VD;
         // tile-local column c: c < nr -> own row c (stage), else halo column c - nr (x slot); both [..][NB2]
@@ -513,14 +513,20 @@ static __global__ void __launch_bounds__(RTB_THREADS, 1) k_rowtile_b(RowArgsB a)
           const unsigned short* cp = scol + sl.x;
           const double* vp = sval + sl.x;
           const float* vp32 = sval32 + sl.x;
-          const unsigned char* vp8 = sval8 + sl.x;
+          const uint32_t* wp = scw + sl.x;
           double acc[NB];
 #pragma unroll
           for (int t = 0; t < NB; ++t) acc[t] = 0.0;
 #pragma unroll 2
           for (int k = 0; k < sl.y; ++k) {
-            const double av = v8 ? sdict[vp8[k * 32]] : (v32 ? (double)vp32[k * 32] : vp[k * 32]);
-            const int c = cp[k * 32];
+            int c;
+            double av;
+            if (v8) {
+              const uint32_t w = wp[k * 32];
+              av = sdict[w >> 16], c = (int)(w & 0xFFFFu);
+            } else {
+              av = v32 ? (double)vp32[k * 32] : vp[k * 32], c = cp[k * 32];
+            }
             const double2* xp = (c < nr ? xown : xhal) + (size_t)c * NB2;
 #pragma unroll
             for (int h = 0; h < NB2; ++h) {

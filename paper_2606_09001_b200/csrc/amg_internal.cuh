@@ -23,7 +23,7 @@ constexpr int RT_STAGE_BYTES = 29696; // shared memory of one ring stage (descri
 constexpr int RT_XSLOTS = 4;          // x slots (side ring): how many tiles the gather warps run ahead
 constexpr int RT_XSLOT_BYTES = 5632;  // one x slot: 8 bytes x (rows + halo columns of a tile)
 // Ring geometry of the row-tile kernel per kind of level: 0 = fp64 / fp32 values (the constants above), 1 = levels
-// stored as 8-bit codes into a value dictionary (3 bytes per entry: a tile of the same bytes holds ~2.4 x the rows,
+// stored as 8-bit codes into a value dictionary (4 bytes per entry: a tile of the same bytes holds ~2 x the rows,
 // so the x slots grow and the stages shrink; one more stage keeps as many bytes in flight)
 template <int GEO> struct RtGeo;
 template <> struct RtGeo<0> {
@@ -31,7 +31,7 @@ template <> struct RtGeo<0> {
   static constexpr int GATHER_UNROLL = RT_GATHER_UNROLL, GATHER_ROWS = RT_GATHER_ROWS;
 };
 template <> struct RtGeo<1> {
-  static constexpr int STAGES = 4, STAGE_BYTES = 18432, XSLOTS = 4, XSLOT_BYTES = 8192;
+  static constexpr int STAGES = 4, STAGE_BYTES = 19456, XSLOTS = 4, XSLOT_BYTES = 8192;
   static constexpr int GATHER_UNROLL = 6, GATHER_ROWS = 5;
 };
 template <int GEO> constexpr int rt_smem_bytes() {

@@ -675,7 +675,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         const unsigned short* scol = reinterpret_cast<const unsigned short*>(base + sd->o_col) + lane;
         const double* sval = reinterpret_cast<const double*>(base + sd->o_val) + lane;
         const float* sval32 = reinterpret_cast<const float*>(base + sd->o_val) + lane;  // mixed-precision hierarchy
-        const unsigned char* sval8 = base + sd->o_val + lane;                            // value dictionary
+        const uint32_t* scw = reinterpret_cast<const uint32_t*>(base + sd->o_col) + lane;  // value dictionary: column | code << 16
         const bool v32 = sd->vb == 4;
         constexpr bool v8 = (GEO == 1);
         const double* xc = reinterpret_cast<const double*>(xslot0 + q * RT_XSLOT_BYTES);
@@ -687,9 +687,12 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
           const unsigned short* cp = scol + sl.x;
           double sum = 0.0;
           if (v8) {  // 8-bit codes into the level's table of distinct fp64 values: the same values, bit for bit
-            const unsigned char* vp = sval8 + sl.x;
+            const uint32_t* wp = scw + sl.x;
 #pragma unroll 4
-            for (int k = 0; k < sl.y; ++k) sum += sdict[vp[k * 32]] * xc[cp[k * 32]];
+            for (int k = 0; k < sl.y; ++k) {
+              const uint32_t w = wp[k * 32];
+              sum += sdict[w >> 16] * xc[w & 0xFFFFu];
+            }
           } else if (v32) {  // values stored in fp32 (exactly representable), arithmetic in fp64
             const float* vp = sval32 + sl.x;
 #pragma unroll 4

@@ -937,7 +937,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
   unsigned short* o_col = reinterpret_cast<unsigned short*>(base + p.o_col);
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);  // vb == 4: mixed-precision hierarchy
-  unsigned char* o_val8 = base + p.o_val;                      // vb == 1: codes into the level's value dictionary
+  uint32_t* o_cw = reinterpret_cast<uint32_t*>(base + p.o_col);  // vb == 1: column | dictionary code << 16
   // tile-local column of every entry of the tile, one thread per entry (ext[] is free again: reused as u16[])
   unsigned short* c16s = reinterpret_cast<unsigned short*>(ext);
   __syncthreads();
@@ -997,17 +997,20 @@ __global__ void __launch_bounds__(PK_THREADS) k_pack_tiles(int ntiles, const int
         while (nx < ln && cls(nx) != t) ++nx;
         cur[t] = nx;
       }
+      if (vb == 1) {
+        o_cw[off + k * 32] = (uint32_t)c16 | ((uint32_t)(k < ln ? vdict_code(vdict, ndict, v) : (unsigned char)255) << 16);
+        continue;
+      }
       o_col[off + k * 32] = c16;
-      if (vb == 1)
-        o_val8[off + k * 32] = k < ln ? vdict_code(vdict, ndict, v) : (unsigned char)255;
-      else if (vb == 4)
+      if (vb == 4)
         o_val32[off + k * 32] = (float)v;
       else
         o_val[off + k * 32] = v;
     }
   }
   // tail of the u16 column section up to its 16-byte rounding
-  for (int q = d.nslots + tid; q < tp_up(2 * d.nslots, 16) / 2; q += PK_THREADS) o_col[q] = 0;
+  if (vb != 1)
+    for (int q = d.nslots + tid; q < tp_up(2 * d.nslots, 16) / 2; q += PK_THREADS) o_col[q] = 0;
 }
 
 __global__ void k_pad_tail(int nnz, int nnz_alloc, int* __restrict__ col, double* __restrict__ val) {
@@ -1405,7 +1408,7 @@ struct TilePack {
 amg_status pack_tiles(amg_handle_s* H, int n, int nnz, const int* rowptr, const int* col, const double* val,
                       const int* agg, const int* agg_ptr, int nc, TilePack& P, cudaStream_t st,
                       double* scale_io = nullptr, int vb = 8, const double* vdict = nullptr, int ndict = 0) {
-  const int nnz_w = 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value (or its 8-bit code)
+  const int nnz_w = vb == 1 ? 4 : 2 + vb;  // bytes a stored entry costs in a ring stage: 16-bit column + value, or column | code
   const int stage_cap = rt_stage_bytes(vb == 1), xslot_cap = rt_xslot_bytes(vb == 1);  // ring geometry of the level kind
   const int64_t total_w = nnz_w * (int64_t)nnz + (int64_t)RT_ROW_WEIGHT * n;
   double scale = scale_io ? (*scale_io * 1.12 < 1.0 ? *scale_io * 1.12 : 1.0) : 1.0;
@@ -1861,6 +1864,7 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
   const int2* slices = reinterpret_cast<const int2*>(base);
   const unsigned short* perm = reinterpret_cast<const unsigned short*>(base + p.o_perm);
   const unsigned short* o_col = reinterpret_cast<const unsigned short*>(base + p.o_col);
+  uint32_t* o_cw = reinterpret_cast<uint32_t*>(base + p.o_col);  // vb == 1: column | dictionary code << 16
   double* o_val = reinterpret_cast<double*>(base + p.o_val);
   float* o_val32 = reinterpret_cast<float*>(base + p.o_val);
   for (int j = 0; j < d.nsl; ++j) {
@@ -1875,7 +1879,7 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
         const int s = rowptr[r], e = rowptr[r + 1];
         if (k < e - s) {
           in_row = true;
-          const int c16 = o_col[sl.x + q];
+          const int c16 = d.vb == 1 ? (int)(o_cw[sl.x + q] & 0xFFFFu) : (int)o_col[sl.x + q];
           const int c = c16 < d.nr ? d.r0 + c16 : halo_idx[d.halo_off + c16 - d.nr];
           int lo = s, hi = e;  // first entry >= c
           while (lo < hi) {
@@ -1887,7 +1891,7 @@ __global__ void __launch_bounds__(256) k_blob_refill(int ntiles, const TileDesc*
         }
       }
       if (d.vb == 1)
-        (base + p.o_val)[sl.x + q] = in_row ? vdict_code(vdict, ndict, v) : (unsigned char)255;
+        o_cw[sl.x + q] = (o_cw[sl.x + q] & 0xFFFFu) | ((uint32_t)(in_row ? vdict_code(vdict, ndict, v) : (unsigned char)255) << 16);
       else if (d.vb == 4)
         o_val32[sl.x + q] = (float)v;
       else

@@ -15,6 +15,8 @@
 //                          slice k-major: slot = first + 32 k + lane  (conflict-free shared-memory reads)
 //   val     f64[nslots]    matrix values, same order; padding slots are {col 0, val 0}
 //           (f32[nslots] with the mixed-precision hierarchy, TileDesc::vb = 4: 6 bytes per entry)
+//   -- or, for a level stored as 8-bit codes into a value dictionary (TileDesc::vb = 1), col and val merged:
+//   cw      u32[nslots]    tile-local column | code << 16 (code 255 = 0.0: padding); 4 bytes per entry
 //
 // and a range [halo_off, halo_off + nhalo) of the level's halo arrays
 //
@@ -51,6 +53,11 @@ __host__ __device__ inline BlobLayout tp_blob(int nsl, int nslots, int vb) {
   BlobLayout p;
   p.o_perm = tp_up(8 * nsl, 16);
   p.o_col = p.o_perm + 64 * nsl;
+  if (vb == 1) {  // value dictionary: ONE u32 per slot, tile-local column | code << 16 (one shared-memory read per entry)
+    p.o_val = p.o_col;
+    p.end = p.o_col + tp_up(4 * nslots, 16);
+    return p;
+  }
   p.o_val = p.o_col + tp_up(2 * nslots, 16);
   p.end = p.o_val + tp_up(vb * nslots, 16);
   return p;
