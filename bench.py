@@ -602,10 +602,11 @@ def run_b200(args):
         gbytes = 12.0 * nnz + 4.0 * (n + 1) + 2 * 8.0 * n
         phases["grad_values_gbs"] = round(gbytes / c1.elapsed_time(c2) / 1e6, 1)
         # device setup, second build (context, allocator and the CSR copy already warm)
-        # (best of 3: the first rebuild after new allocations may have to grow the memory pool)
+        # (best of 6: the stream-ordered memory pool needs a few setup / destroy rounds until it holds every block
+        # size of this hierarchy; until then a setup pays for growing it: 20 .. 100 ms instead of 16)
         setup_times = []
         h2 = None
-        for _ in range(3):
+        for _ in range(6):
             if h2 is not None:
                 B.amg_destroy(h2)
             torch.cuda.synchronize()
