@@ -556,11 +556,15 @@ def run_b200(args):
                 "traffic": traffic, "traffic_source": "profiles/r02_level0_sweep_dram.csv (profiles/r02_roofline.md)",
                 "traffic_gbs": round(traffic / (sweep_ms * 1e-3) / 1e9, 1) if traffic else None,
                 "traffic_frac": round(traffic / (sweep_ms * 1e-3) / 1e9 / peak, 4) if traffic else None,
-                "note": "achieved / frac count ALGORITHMIC (CSR-based) bytes: M_0 + 4 V_0; the tile blobs store 10 bytes per "
-                        "entry instead of 12 + row pointers, so the DRAM traffic is smaller (traffic_frac = traffic / time / peak)",
+                "note": "achieved / frac count ALGORITHMIC (CSR-based) bytes: M_0 + 4 V_0 at 12 bytes per entry + row pointers; "
+                        "the tile blobs store 10 bytes per entry, or 4 where the level's values fit a 255-entry dictionary "
+                        "(value_dict; level 0 of cfg 3: 2 distinct values), so the DRAM traffic is smaller: traffic_frac = "
+                        "traffic / time / peak.  With the dictionary frac exceeds 1 and the kernel is bound by the L1 / "
+                        "shared-memory pipe, not by HBM (profiles/r02_roofline.md)",
+                "stored_operator_bytes_level0": B.amg_get_algorithmic_bytes(h, 11),
                 "bytes_per_launch": bytes_sweep, "us_per_launch": round(sweep_ms * 1e3, 2), "peak_source": peak_src,
                 "how": "CUDA events around 10 and 60 back-to-back launches (amg_level_op op 1), difference / 50; the launches "
-                       "rotate over 3 sets of x, b, dinv, out (12 vectors, 201 MB) + the 146 MB operator (evict-first): no "
+                       "rotate over 3 sets of x, b, dinv, out (12 vectors, 201 MB) + the operator blobs (evict-first): no "
                        "operand of a launch is still in the 126 MB L2 from the launch before"}
         vc = {"ms": round(vcycle_ms, 4), "bytes": bytes_vcycle, "gbs": round(bytes_vcycle / vcycle_ms / 1e6, 1),
               "frac_of_peak": round(bytes_vcycle / vcycle_ms / 1e6 / peak, 4),
