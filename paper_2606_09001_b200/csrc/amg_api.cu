@@ -480,17 +480,17 @@ amg_status amg_write_report(amg_handle h, const char* path, void* cuda_stream) {
   fprintf(f, "rows %lld  nonzeros %lld  symmetric %d  levels %d\n", (long long)h->n, (long long)h->nnz, h->symmetric,
           (int)h->lv.size());
   fprintf(f, "options: krylov %d  agg_passes %d  sweeps %d+%d  smoother %d (omega %.6g, cheby_ratio %.6g)  strong_beta %.6g  "
-             "coarse_scale %.6g  coarse_max_rows %d  hierarchy_fp32 %d  tail_dense_rows %d  use_graph %d  use_pdl %d  use_while %d\n",
+             "coarse_scale %.6g  coarse_max_rows %d  hierarchy_fp32 %d  value_dict %d  tail_dense_rows %d  use_graph %d  use_pdl %d  use_while %d\n",
           o.krylov, o.agg_passes, o.pre_sweeps, o.post_sweeps, o.smoother, o.omega, o.cheby_ratio, o.strong_beta,
-          o.coarse_scale, o.coarse_max_rows, o.hierarchy_fp32, o.tail_dense_rows, o.use_graph, o.use_pdl, o.use_while);
+          o.coarse_scale, o.coarse_max_rows, o.hierarchy_fp32, o.value_dict, o.tail_dense_rows, o.use_graph, o.use_pdl, o.use_while);
   double sn = 0.0, sz = 0.0;
-  fprintf(f, "%5s %12s %14s %9s %7s %6s %8s %12s\n", "level", "rows", "nonzeros", "nnz/row", "rounds", "tiles", "kernels",
-          "blob MB");
+  fprintf(f, "%5s %12s %14s %9s %7s %6s %8s %12s %11s\n", "level", "rows", "nonzeros", "nnz/row", "rounds", "tiles", "kernels",
+          "blob MB", "dict values");
   for (size_t l = 0; l < h->lv.size(); ++l) {
     const Level& L = h->lv[l];
     sn += L.n, sz += L.nnz;
-    fprintf(f, "%5d %12d %14d %9.2f %7d %6d %8s %12.2f\n", (int)l, L.n, L.nnz, L.n ? (double)L.nnz / L.n : 0.0,
-            L.match_rounds, L.nblk, L.fast ? "row-tile" : "row-vec", L.blob_bytes / 1e6);
+    fprintf(f, "%5d %12d %14d %9.2f %7d %6d %8s %12.2f %11d\n", (int)l, L.n, L.nnz, L.n ? (double)L.nnz / L.n : 0.0,
+            L.match_rounds, L.nblk, L.fast ? "row-tile" : "row-vec", L.blob_bytes / 1e6, L.ndict);
   }
   fprintf(f, "grid complexity %.4f  operator complexity %.4f  coarsest dense LU %d x %d  dense tail from level %d\n",
           h->n ? sn / (double)h->n : 0.0, h->nnz ? sz / (double)h->nnz : 0.0, h->nL, h->nL, h->tail_dense_level);
