@@ -475,7 +475,9 @@ def test_report_file(B, tmp_path):
         B.amg_write_report(s.h, p)
         txt = p.read_text().splitlines()
         assert txt[0].startswith("amg_b200 hierarchy report") and f"levels {s.num_levels}" in txt[1]
-        rows = [l.split() for l in txt if l.split() and l.split()[0].isdigit() and len(l.split()) == 8]
+        rows = [l.split() for l in txt if l.split() and l.split()[0].isdigit() and len(l.split()) == 9]
+        # last column: size of the level's value dictionary (a 24^3 Poisson level 0 holds 2 distinct values: -1, 6)
+        assert int(rows[0][8]) == 2 and all(0 <= int(r[8]) <= 255 for r in rows)
         assert [(int(r[1]), int(r[2])) for r in rows] == [s.level_info(l) for l in range(s.num_levels)]
         hist = [float(l.split()[1]) for l in txt[txt.index(next(t for t in txt if t.startswith("residual history"))) + 1:]]
         assert len(hist) == info.iterations and np.array_equal(np.array(hist), s.residual_history())
