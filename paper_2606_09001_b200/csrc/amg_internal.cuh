@@ -29,10 +29,12 @@ template <int GEO> struct RtGeo;
 template <> struct RtGeo<0> {
   static constexpr int STAGES = RT_STAGES, STAGE_BYTES = RT_STAGE_BYTES, XSLOTS = RT_XSLOTS, XSLOT_BYTES = RT_XSLOT_BYTES;
   static constexpr int GATHER_UNROLL = RT_GATHER_UNROLL, GATHER_ROWS = RT_GATHER_ROWS;
+  static constexpr int CONSUMERS = RT_CONSUMERS, GATHERERS = RT_GATHERERS, THREADS = RT_THREADS;
 };
 template <> struct RtGeo<1> {
   static constexpr int STAGES = 4, STAGE_BYTES = 19456, XSLOTS = 4, XSLOT_BYTES = 8192;
-  static constexpr int GATHER_UNROLL = 6, GATHER_ROWS = 5;
+  static constexpr int GATHER_UNROLL = 4, GATHER_ROWS = 4;
+  static constexpr int CONSUMERS = 256, GATHERERS = 256, THREADS = CONSUMERS + 32 + GATHERERS;  // 8 + 8 warps: the gather bounds these levels
 };
 template <int GEO> constexpr int rt_smem_bytes() {
   return 256 + RtGeo<GEO>::STAGES * RtGeo<GEO>::STAGE_BYTES + RtGeo<GEO>::XSLOTS * RtGeo<GEO>::XSLOT_BYTES;

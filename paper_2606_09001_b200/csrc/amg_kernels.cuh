@@ -466,11 +466,14 @@ struct DictStore<false> {
 };
 
 template <int OP, int NDOT, bool STREAM, int GEO>
-static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs a) {
+static __global__ void __launch_bounds__(RtGeo<GEO>::THREADS, RT_CTAS) k_rowtile(RowArgs a) {
   // ring geometry of this kind of level (the names shadow the fp64 geometry's constants)
   constexpr int RT_STAGES = RtGeo<GEO>::STAGES, RT_STAGE_BYTES = RtGeo<GEO>::STAGE_BYTES;
   constexpr int RT_XSLOTS = RtGeo<GEO>::XSLOTS, RT_XSLOT_BYTES = RtGeo<GEO>::XSLOT_BYTES;
   constexpr int RT_GATHER_UNROLL = RtGeo<GEO>::GATHER_UNROLL, RT_GATHER_ROWS = RtGeo<GEO>::GATHER_ROWS;
+  constexpr int RT_CONSUMERS = RtGeo<GEO>::CONSUMERS, RT_GATHERERS = RtGeo<GEO>::GATHERERS, RT_THREADS = RtGeo<GEO>::THREADS;
+  constexpr int NCW = RT_CONSUMERS / 32, NGW = RT_GATHERERS / 32;  // consumer / gather warps of this kind of level
+  static_assert((NCW & (NCW - 1)) == 0 && NGW % RT_GGROUPS == 0, "consumer warps: a power of two; gather warps: whole groups");
   static_assert((4 * RT_STAGES + 2 * RT_XSLOTS) * 8 <= rt::HEADER_BYTES && RT_XSLOTS >= 2 * RT_GGROUPS, "ring header");
   static_assert(RT_STAGE_BYTES % 128 == 0 && RT_XSLOT_BYTES % 128 == 0, "stage / slot sizes must keep 128-byte alignment");
   extern __shared__ __align__(128) unsigned char smem[];
@@ -491,13 +494,13 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
   if (tid == 0) {
     for (int s = 0; s < RT_STAGES; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, rt::NCW);
-      mbar_init(resdone + s, rt::NCW);
+      mbar_init(empty + s, NCW);
+      mbar_init(resdone + s, NCW);
       mbar_init(pre + s, 1);
     }
     for (int q = 0; q < RT_XSLOTS; ++q) {
-      mbar_init(xready + q, rt::NGW / RT_GGROUPS);
-      mbar_init(xempty + q, rt::NCW);
+      mbar_init(xready + q, NGW / RT_GGROUPS);
+      mbar_init(xempty + q, NCW);
     }
     fence_mbar_init();
   }
@@ -682,7 +685,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
         const double* bs = reinterpret_cast<const double*>(base + sd->o_b) + sd->roff;
         const double* ds = reinterpret_cast<const double*>(base + sd->o_d) + sd->roff;
         double* outs = reinterpret_cast<double*>(base + sd->o_out);
-        for (int j = (w - sbase) & (rt::NCW - 1); j < nsl; j += rt::NCW) {
+        for (int j = (w - sbase) & (NCW - 1); j < nsl; j += NCW) {
           const int2 sl = slices[j];
           const unsigned short* cp = scol + sl.x;
           double sum = 0.0;
@@ -734,7 +737,7 @@ static __global__ void __launch_bounds__(RT_THREADS, RT_CTAS) k_rowtile(RowArgs 
           }
         }
       }
-      sbase = (sbase + nsl) & (rt::NCW - 1);
+      sbase = (sbase + nsl) & (NCW - 1);
       // ---- this warp is done with the stage and the x slot ----
       if (OP == OP_RESTRICT) fence_proxy_async();  // residuals were written into a region the next bulk copy overwrites
       __syncwarp();

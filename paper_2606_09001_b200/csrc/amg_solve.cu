@@ -77,7 +77,7 @@ void launch_tile(const amg_handle_s* H, const Level& L, const RowArgs& a, cudaSt
   int grid = H->sm_count * RT_CTAS;
   if (grid > lv_nblk(L)) grid = lv_nblk(L);
   if (lv_geo(L))
-    ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM, 1>, grid, RT_THREADS, rt_smem_bytes<1>(), st)(a);
+    ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM, 1>, grid, RtGeo<1>::THREADS, rt_smem_bytes<1>(), st)(a);
   else
     ++g_nlaunch, launch(k_rowtile<OP, NDOT, STREAM, 0>, grid, RT_THREADS, rt_smem_bytes<0>(), st)(a);
 }
